@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the transient F-statistic hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (bounds, exp-window
+weighted sums, cell closure, fused marginalisation, batched over templates) over one batch of
+synthetic input: BASELINE.json configs[3], the batched template search (4096 templates x 2880
+atoms, 96 x 1417 grid, 1.078e12 window-atom terms), through tfstat_search of the C ABI.
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "exp-window window-atom terms/s"
+UNIT = "terms/s"
+WORKLOAD = "cfg4_search_4096x2880atoms_96x1417"
+# algorithmic work per window-atom term: 1 FFMA (exp argument) + 1 FMUL (w^2)
+# + 7 FFMA (A,B,C,Re/Im Fa,Re/Im Fb) on the FP32 pipe, + 1 MUFU.EX2 on the XU pipe
+FP32_OPS_PER_TERM = 9
+FP32_LANES_PER_CLK_SM = 128  # cc 10.0: 4 SMSPs x 32 FP32 lanes
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)),
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows = []
+        self.proc = None
+        self.gpu_index = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-i", str(self.gpu_index), "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, power, reasons = [], [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                smax.append(float(r[2]))
+                power.append(float(r[3]))
+            except (ValueError, IndexError):
+                continue
+            for name, col in (("hw_slowdown", 5), ("hw_thermal_slowdown", 6),
+                              ("sw_thermal_slowdown", 7), ("sw_power_cap", 8)):
+                if len(r) > col and r[col].lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # "under load": samples in the upper half of the power range seen
+        thr = 0.5 * (max(power) + min(power))
+        load = [s for s, p in zip(sm, power) if p >= thr] or sm
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(smax),
+                "power_w_max": max(power), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    return rank, local, world
+
+
+# ------------------------------------------------------------------------------------------
+# reference arm: the fp64 oracle as it stands, on the host cores
+# ------------------------------------------------------------------------------------------
+def oracle_leg(n_templates: int, seed_offset: int = 0):
+    """Times oracle.search on `n_templates` templates of config 4.  Returns
+    (terms_per_s, seconds, terms, cores)."""
+    import oracle
+    from synth import make_workload
+
+    wl = make_workload(4, templates=range(seed_offset, seed_offset + n_templates))
+    cores = oracle.num_threads()
+    t0 = time.perf_counter()
+    _, terms = oracle.search(wl.data.atoms, wl.data.t, 1, wl.grid, n_threads=cores)
+    dt = time.perf_counter() - t0
+    return terms / dt, dt, terms, min(cores, n_templates)
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+
+    cores = oracle.num_threads()
+    n_tpl = max(1, min(cores, 16))  # one template (2.6e8 terms, a few seconds) per core
+    for _ in range(args.warmup if args.warmup < 1 else 1):
+        oracle_leg(1)
+    times, terms = [], 0
+    for s in range(args.steps):
+        _, dt, terms, used = oracle_leg(n_tpl, seed_offset=s * n_tpl)
+        times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    value = terms / (ms * 1e-3)
+    sample = (f"{n_tpl} of 4096 templates of config 4 per step (full 96x1417 grid each, "
+              f"{terms:.3e} terms), OpenMP over templates")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": min(cores, n_tpl),
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------
+def time_calls(torch, fn, n, stream=None):
+    """CUDA-event time of n back-to-back calls on the current stream, ms per call."""
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n
+
+
+def side_workloads(torch, pkg, peaks):
+    """Kernel-level numbers for the other BASELINE.json configs (context, not the bench line)."""
+    from synth import make_workload
+
+    out = {}
+    l2_flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn, reps=5):
+        ms = []
+        for _ in range(reps):
+            l2_flush.zero_()
+            ms.append(time_calls(torch, fn, 1))
+        return min(ms), statistics.median(ms)
+
+    for cfg, window, wname in ((2, 1, "exp"), (3, 1, "exp"), (3, 0, "rect"), (5, 0, "rect"),
+                               (5, 1, "exp")):
+        wl = make_workload(cfg)
+        atoms = torch.from_numpy(wl.data.atoms).cuda()
+        t = torch.from_numpy(wl.data.t).cuda()
+        terms = pkg.count_terms(t, window, wl.grid)
+        cells = wl.grid.n_cells
+        ws = torch.empty(pkg.workspace_bytes(window, t.shape[0], 1, wl.grid), dtype=torch.uint8,
+                         device="cuda")
+        maps = torch.empty((wl.grid.N_t0, wl.grid.N_tau), dtype=torch.float32, device="cuda")
+        fn_map = lambda: pkg.tfstat_map(atoms[0], t, window, wl.grid, out_map=maps, workspace=ws)
+        fn_fused = lambda: pkg.tfstat_search(atoms, t, window, wl.grid, workspace=ws)
+        for _ in range(3):
+            fn_map()
+            fn_fused()
+        best_map, med_map = timed(fn_map)
+        best_fused, med_fused = timed(fn_fused)
+        rec = {"cells": cells, "terms": terms, "map_ms": med_map, "fused_marginals_ms": med_fused}
+        if window == 1:
+            rec["terms_per_s_map"] = terms / (med_map * 1e-3)
+            rec["terms_per_s_fused"] = terms / (med_fused * 1e-3)
+        else:
+            by = 32 * int(t.shape[0]) + 4 * cells  # atoms once + 4 B per cell
+            rec["cells_per_s_map"] = cells / (med_map * 1e-3)
+            rec["algorithmic_GBps_map"] = by / (med_map * 1e-3) / 1e9
+            rec["hbm_frac_map"] = rec["algorithmic_GBps_map"] / peaks["hbm_gbs"]
+        out[f"cfg{cfg}_{wname}"] = rec
+        # marginalise-from-HBM (row a5 standalone), HBM-bound: 4 B per cell read
+        if cfg == 5 and window == 0:
+            fn_m = lambda: pkg.tfstat_marginalise(maps)
+            for _ in range(3):
+                fn_m()
+            b, med = timed(fn_m)
+            out["cfg5_marginalise"] = {"cells": cells, "ms": med,
+                                       "algorithmic_GBps": 4 * cells / (med * 1e-3) / 1e9,
+                                       "hbm_frac": 4 * cells / (med * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    return out
+
+
+def run_ours(args):
+    import torch
+
+    import paper_1805_05652_b200 as pkg
+    from synth import make_workload
+
+    rank, local, world = dist_env()
+    if world != args.gpus:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("--gpus N > 1 must be launched with torch.distributed.run")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pkg.load_library()  # no fallback: raises if libtfstat.so is missing
+    peaks = read_peaks()
+
+    n_tpl = args.templates
+    # weak scaling: every rank searches its own n_tpl templates (distinct seeds), no data-path
+    # collective
+    wl = make_workload(4, templates=range(rank * n_tpl, rank * n_tpl + n_tpl))
+    grid = wl.grid
+    atoms_h = torch.from_numpy(wl.data.atoms).pin_memory()
+    t_h = torch.from_numpy(wl.data.t).pin_memory()
+    atoms = atoms_h.cuda()
+    t = t_h.cuda()
+    terms_per_template = pkg.count_terms(t, pkg.EXP, grid)
+    terms = terms_per_template * n_tpl
+    cells = grid.n_cells * n_tpl
+    ws = torch.empty(pkg.workspace_bytes(pkg.EXP, int(t.shape[0]), n_tpl, grid),
+                     dtype=torch.uint8, device="cuda")
+    out = torch.empty((n_tpl, 5), dtype=torch.int32, device="cuda")
+
+    def step(events=None):
+        return pkg.tfstat_search(atoms, t, pkg.EXP, grid, workspace=ws, out=out,
+                                 main_kernel_events=events)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: exactly K steps, barrier + sync on both sides ----------
+    kernel_events = []
+    for _ in range(args.steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        b.record()
+        kernel_events.append((a, b))
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(args.steps):
+        step(kernel_events[k])
+    e1.record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = e0.elapsed_time(e1)
+    kernel_ms = [a.elapsed_time(b) for a, b in kernel_events]
+    if dist:
+        tt = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_per_step = ms_total / args.steps
+    value = terms * world / (ms_per_step * 1e-3)
+    res_dev = out.cpu().numpy().copy()
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + compute + D2H inside) -----
+    for _ in range(1):
+        pkg.tfstat_search_host(atoms_h, t_h, pkg.EXP, grid)
+    if dist:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        res_host, _ = pkg.tfstat_search_host(atoms_h, t_h, pkg.EXP, grid)
+    e2e_s = (time.perf_counter() - t0) / args.steps
+    if dist:
+        tt = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    assert np.array_equal(res_host.view(np.int32).reshape(-1, 5), res_dev), \
+        "host-buffer path and device-resident path disagree"
+    h2d = atoms_h.numel() * 4 + t_h.numel() * 4
+    d2h = n_tpl * 20
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (exp_direct_kernel) -----------------------------
+    k_ms = statistics.mean(kernel_ms)
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_ops = FP32_LANES_PER_CLK_SM * n_sm * peaks["sm_max_mhz"] * 1e6  # lane-ops/s at max clock
+    ach_ops = terms * FP32_OPS_PER_TERM / (k_ms * 1e-3)
+    probes = {k: pkg.probe_alu(k) for k in ("ffma", "fadd", "mufu_ex2", "ffma2", "ffma_mufu",
+                                             "lds128", "dfma")}
+    roofline = {
+        "bound": "alu", "kernel": "exp_direct_kernel",
+        "achieved": ach_ops / 1e12, "peak": peak_ops / 1e12, "unit": "T FP32 lane-op/s",
+        "frac": ach_ops / peak_ops,
+        "peak_source": (f"{FP32_LANES_PER_CLK_SM} FP32 lanes/clk/SM x {n_sm} SMs x "
+                        f"{peaks['sm_max_mhz']:.0f} MHz (max SM clock, {peaks['source']})"),
+        "algorithmic_ops_per_term": FP32_OPS_PER_TERM,
+        "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
+        "terms_per_s_kernel": terms / (k_ms * 1e-3),
+        "terms_per_clk_sm": terms / (k_ms * 1e-3) / n_sm /
+        ((clocks or {}).get("sm_mhz") or peaks["sm_max_mhz"]) / 1e6,
+        "measured_ffma_lane_ops_per_s": probes["ffma"]["lane_ops_per_s"],
+        "frac_of_measured_ffma": ach_ops / probes["ffma"]["lane_ops_per_s"],
+        "traffic": None,
+        "probes_ops_per_clk_sm": {k: round(v["ops_per_clk_sm"], 2) for k, v in probes.items()},
+        "probe_sm_mhz": round(probes["ffma"]["sm_mhz"], 1),
+    }
+
+    # ---- CPU baseline: the oracle as it stands on this box's host cores -------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+
+        cores = oracle.num_threads()
+        n_s = max(1, min(cores, 16))
+        v, dt, tms, used = oracle_leg(n_s)
+        cpu = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle", "seconds": dt,
+               "sample": f"{n_s} of 4096 templates of config 4 (full 96x1417 grid each, "
+                         f"{tms:.3e} terms), OpenMP over templates"}
+
+    side = None if args.no_side else side_workloads(torch, pkg, peaks)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "templates_per_gpu": n_tpl, "n_atoms": int(t.shape[0]),
+                   "N_t0": grid.N_t0, "N_tau": grid.N_tau, "window": "exp",
+                   "exp_method": "direct", "terms_per_step_per_gpu": terms,
+                   "cells_per_step_per_gpu": cells,
+                   "l2": f"inputs {atoms.numel() * 4 / 2**20:.0f} MiB per step > 126 MB L2, no flush",
+                   "parallelism": f"templates sharded over {world} GPU(s), no collective"},
+        "cells_per_s": cells * world / (ms_per_step * 1e-3),
+        "e2e": {"value": terms * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
+        "gpu_launches": 3 * args.steps,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "clocks": clocks,
+        "other_workloads": side,
+    }
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--templates", type=int, default=4096,
+                    help="templates per GPU (4096 = BASELINE.json configs[3]; smaller values are "
+                         "for debugging only and are not a valid bench line)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-side", action="store_true", help="skip the other-config numbers")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

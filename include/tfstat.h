@@ -1,0 +1,160 @@
+/*
+ * tfstat.h -- C ABI of libtfstat: the transient F-statistic map on NVIDIA B200 (sm_100a).
+ *
+ * The operation is the one stated in Keitel & Ashton 2018 (arXiv:1805.05652), section 3
+ * (PAPER.md:88): "atoms + window type + {t0, tau} grid -> F_mn", eq. (8), with
+ * the per-cell statistic of eq. (7) evaluated on window-weighted partial sums
+ * of the atoms, windows (3)/(4), followed by the marginalisation of the map
+ * (eq. (5); c_marg footnote PAPER.md:227) and batched over templates lambda
+ * (PAPER.md:114, 142).  Conventions the paper leaves open are the readings R1-R16 of
+ * DESIGN.md (half-open windows on atom start times, >= min_atoms atoms per cell, map stores
+ * 2F, logB = log sum exp F over valid cells).
+ *
+ * General rules
+ *  - Pointers are DEVICE pointers unless the parameter name ends in `_host` (or the function
+ *    name does).  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *  - The caller owns every buffer, including `workspace`; the library allocates no device
+ *    memory in the device-pointer calls, keeps no global state and is re-entrant.  Work is
+ *    enqueued asynchronously on `stream`; outputs are valid once the caller synchronises.
+ *  - Return value: 0 (TFSTAT_OK) or a negative tfstat_status.  Nothing throws or aborts.
+ *  - Times (atom start times, t0_min, dt0, tau_min, dtau) are integer seconds relative to a
+ *    caller-chosen epoch.  Window membership is decided in integers.
+ *  - Atoms: 7 rows of `ld` (>= n_atoms) fp32 each, row order a2, b2, ab, Re Fa, Im Fa,
+ *    Re Fb, Im Fb (the 7 x N_SFT real32 matrix of PAPER.md:88); multi-detector data merged
+ *    per timestamp by the caller.  `t_atoms` strictly increasing (precondition).
+ *  - Map: fp32, row-major, tau fastest: map[m*N_tau + n] = 2F(t0_min + m dt0, tau_min + n dtau)
+ *    (eq. 8: m <-> t0, n <-> tau).
+ *  - Degenerate cells (fewer than opts->min_atoms atoms in the window: flag bit 0; D <= 0 or
+ *    NaN: flag bit 1) store 2F = 0 and are excluded from the marginals.  Empty windows and
+ *    all-degenerate maps are NOT errors (the full matrix is always returned).
+ */
+#ifndef TFSTAT_H_
+#define TFSTAT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TFSTAT_VERSION 100 /* 0.1.0 */
+
+/* window functions, eqs. (3), (4) */
+#define TFSTAT_WINDOW_RECT 0 /* w = 1 on [t0, t0 + tau)                          */
+#define TFSTAT_WINDOW_EXP 1  /* w = exp(-(t - t0)/tau) on [t0, t0 + 3 tau)       */
+
+/* how the exponential-window sums are evaluated (tfstat_opts.exp_method) */
+#define TFSTAT_EXP_AUTO 0   /* = DIRECT */
+#define TFSTAT_EXP_DIRECT 1 /* truncated weighted sum per cell, the paper's
+                               brute-force definition, register-tiled                     */
+#define TFSTAT_EXP_SCAN 2   /* exact factorised form: per-tau backward recurrence
+                               G_k = x_k + exp(-(t_{k+1}-t_k)/tau) G_{k+1}, window sum
+                               = G_lo - exp(-(t_hi-t_lo)/tau) G_hi */
+
+typedef enum tfstat_status {
+    TFSTAT_OK = 0,
+    TFSTAT_EINVAL = -1,     /* null required pointer, n_atoms < 1, N_t0 < 1, N_tau < 1,
+                               tau_min < 1, dt0 < 1 with N_t0 > 1, dtau < 1 with N_tau > 1,
+                               ld < n_atoms, unknown window/method, N_t0*N_tau >= 2^31      */
+    TFSTAT_EWORKSPACE = -2, /* workspace NULL or smaller than tfstat_workspace_bytes()     */
+    TFSTAT_ECUDA = -3,      /* a CUDA call failed; see tfstat_last_cuda_error()            */
+    TFSTAT_EOVERFLOW = -4   /* t0_max + 3 tau_max (or any grid time) exceeds int32         */
+} tfstat_status;
+
+/* Marginals of one map (20 bytes, written on the device). */
+typedef struct tfstat_result {
+    float max2F;     /* max over valid cells of 2F; 0 if n_valid == 0                     */
+    int32_t m;       /* t0 index of the maximum (lowest flat index m*N_tau+n on exact     */
+    int32_t n;       /* ties), tau index; (-1,-1) if n_valid == 0                          */
+    float logB;      /* log sum_valid exp(F), F = 2F/2; -inf if n_valid == 0               */
+    int32_t n_valid; /* number of non-degenerate cells                                     */
+} tfstat_result;
+
+/* Options; a HOST pointer in every call, NULL = defaults. */
+typedef struct tfstat_opts {
+    int32_t min_atoms;  /* cells with fewer atoms are degenerate; 0 or unset -> 2
+                           ("at least 2 SFTs per F_mn")                      */
+    int32_t exp_method; /* TFSTAT_EXP_*                                                    */
+    int32_t reserved[2];
+    /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
+     * immediately before and after the dominant kernel of the call (the window-sum +
+     * closure kernel; for the rectangular window: prefix + cells kernels).  NULL = off. */
+    void *ev_main_begin;
+    void *ev_main_end;
+} tfstat_opts;
+
+/* ---- host-only helpers (no CUDA calls) ------------------------------------------------ */
+int tfstat_version(void);
+const char *tfstat_strerror(int status);
+/* Bytes of device workspace tfstat_map/tfstat_search need for this problem shape.
+ * Returns 0 on invalid arguments. */
+size_t tfstat_workspace_bytes(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
+                              int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                              int32_t N_tau, const tfstat_opts *opts_host);
+/* cudaError_t of the last failing CUDA call made by this thread inside the library. */
+int tfstat_last_cuda_error(void);
+
+/* ---- the hot path --------------------------------------------------------------------- */
+
+/* One template: atoms + window + grid -> full map (eq. 8).
+ *   atoms      [7][ld] fp32              t_atoms   [n_atoms] int32
+ *   out_map    [N_t0][N_tau] fp32 2F     out_flags [N_t0][N_tau] uint8, nullable
+ *   workspace  >= tfstat_workspace_bytes(window, n_atoms, 1, grid...) bytes, 256-B aligned */
+int tfstat_map(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
+               int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
+               int32_t dtau, int32_t N_tau, float *out_map, uint8_t *out_flags,
+               void *workspace, size_t workspace_bytes, void *stream,
+               const tfstat_opts *opts_host);
+
+/* Marginalise a map already in device memory: max 2F + argmax, logB, n_valid.
+ *   flags nullable (NULL: every cell valid).  out: one tfstat_result on the device.
+ *   workspace: >= tfstat_marginalise_workspace_bytes(N_t0, N_tau) bytes.                   */
+size_t tfstat_marginalise_workspace_bytes(int32_t N_t0, int32_t N_tau);
+int tfstat_marginalise(const float *map, const uint8_t *flags, int32_t N_t0, int32_t N_tau,
+                       tfstat_result *out, void *workspace, size_t workspace_bytes,
+                       void *stream);
+
+/* Batched search over n_templates independent atom sets that share timestamps and grid;
+ * map evaluation, cell closure and marginalisation fused, so only n_templates results reach
+ * memory unless out_maps is given (eq. 5).
+ *   atoms      template k, row r, atom i at atoms[k*template_stride + r*ld + i]
+ *   out        [n_templates] tfstat_result
+ *   out_maps   nullable; [n_templates][N_t0][N_tau] fp32, streamed as computed
+ *   out_flags  nullable; same shape, uint8                                                */
+int tfstat_search(const float *atoms, int64_t template_stride, int64_t ld,
+                  const int32_t *t_atoms, int32_t n_atoms, int32_t n_templates, int window,
+                  int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                  int32_t N_tau, tfstat_result *out, float *out_maps, uint8_t *out_flags,
+                  void *workspace, size_t workspace_bytes, void *stream,
+                  const tfstat_opts *opts_host);
+
+/* Number of (cell, atom-in-window) terms of the grid, the N_sums of eqs. (A.5)/(A.6)
+ * generalised to gaps: sum over cells of the atoms in
+ * [t0, t0 + k tau), k = 1 (rect) or 3 (exp).  *out_terms is a DEVICE int64.
+ *   workspace: >= tfstat_workspace_bytes(window, n_atoms, 1, grid...) bytes.               */
+int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int32_t t0_min,
+                       int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                       int32_t N_tau, int64_t *out_terms, void *workspace,
+                       size_t workspace_bytes, void *stream);
+
+/* ---- end-to-end entry point with HOST buffers ----------------------------------------- */
+
+/* tfstat_search on host memory: copies atoms host->device in template chunks on internal
+ * streams (overlapped with compute), runs the fused search, copies results (and maps, if
+ * asked) device->host, and returns after everything has completed.  Host buffers should be
+ * page-locked for the copies to overlap.  Allocates its own device memory (cudaMalloc) and
+ * frees it before returning; `max_device_bytes` bounds that (0 = 2 GiB).
+ *   atoms_host, t_atoms_host, out_host, out_maps_host (nullable): HOST pointers, layouts as
+ *   in tfstat_search.                                                                      */
+int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t ld,
+                       const int32_t *t_atoms_host, int32_t n_atoms, int32_t n_templates,
+                       int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
+                       int32_t dtau, int32_t N_tau, tfstat_result *out_host,
+                       float *out_maps_host, size_t max_device_bytes,
+                       const tfstat_opts *opts_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TFSTAT_H_ */

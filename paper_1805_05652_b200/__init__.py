@@ -1,0 +1,26 @@
+"""paper_1805_05652_b200 -- the transient F-statistic map (Keitel & Ashton 2018,
+arXiv:1805.05652) as hand-written CUDA for NVIDIA B200 (sm_100a).
+
+The product is `libtfstat.so` (C ABI in `include/tfstat.h`, sources in `csrc/`).  This Python
+package is a thin ctypes binding with the same call names: argument marshalling only, every
+step of the path runs in the CUDA kernels.  There is no CPU fallback: importing the binding
+without the built library raises.
+"""
+from .binding import (  # noqa: F401
+    EXP,
+    EXP_AUTO,
+    EXP_DIRECT,
+    EXP_SCAN,
+    RECT,
+    RESULT_DTYPE,
+    TfstatError,
+    count_terms,
+    lib_path,
+    load_library,
+    probe_alu,
+    tfstat_map,
+    tfstat_marginalise,
+    tfstat_search,
+    tfstat_search_host,
+    workspace_bytes,
+)

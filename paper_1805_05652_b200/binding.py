@@ -1,0 +1,287 @@
+"""ctypes binding of libtfstat.so (include/tfstat.h).  Argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the hot path runs inside the
+CUDA kernels of csrc/.  There is no CPU fallback: a missing library raises TfstatError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+import torch
+
+RECT, EXP = 0, 1
+EXP_AUTO, EXP_DIRECT, EXP_SCAN = 0, 1, 2
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libtfstat.so")
+_lib = None
+
+# tfstat_result, 20 bytes (include/tfstat.h)
+RESULT_DTYPE = np.dtype([("max2F", "<f4"), ("m", "<i4"), ("n", "<i4"), ("logB", "<f4"),
+                         ("n_valid", "<i4")])
+
+
+class TfstatError(RuntimeError):
+    pass
+
+
+class _Opts(C.Structure):
+    _fields_ = [("min_atoms", C.c_int32), ("exp_method", C.c_int32),
+                ("reserved", C.c_int32 * 2), ("ev_main_begin", C.c_void_p),
+                ("ev_main_end", C.c_void_p)]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libtfstat.so; raises if it has not been built (python -m paper_1805_05652_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise TfstatError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_1805_05652_b200.build` "
+            "(nvcc, sm_100a).  libtfstat has no CPU fallback.")
+    lib = C.CDLL(_LIB_PATH)
+    i32, i64, vp, sz = C.c_int32, C.c_int64, C.c_void_p, C.c_size_t
+    grid = [i32] * 6
+    op = C.POINTER(_Opts)
+    lib.tfstat_version.restype = C.c_int
+    lib.tfstat_strerror.restype = C.c_char_p
+    lib.tfstat_strerror.argtypes = [C.c_int]
+    lib.tfstat_last_cuda_error.restype = C.c_int
+    lib.tfstat_workspace_bytes.restype = sz
+    lib.tfstat_workspace_bytes.argtypes = [C.c_int, i32, i32] + grid + [op]
+    lib.tfstat_map.argtypes = [vp, i64, vp, i32, C.c_int] + grid + [vp, vp, vp, sz, vp, op]
+    lib.tfstat_marginalise_workspace_bytes.restype = sz
+    lib.tfstat_marginalise_workspace_bytes.argtypes = [i32, i32]
+    lib.tfstat_marginalise.argtypes = [vp, vp, i32, i32, vp, vp, sz, vp]
+    lib.tfstat_search.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
+        vp, vp, vp, vp, sz, vp, op]
+    lib.tfstat_count_terms.argtypes = [vp, i32, C.c_int] + grid + [vp, vp, sz, vp]
+    lib.tfstat_search_host.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
+        vp, vp, sz, op]
+    lib.tfstat_probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double),
+                                     C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        lib = load_library()
+        msg = lib.tfstat_strerror(rc).decode()
+        extra = f" (cudaError {lib.tfstat_last_cuda_error()})" if rc == -3 else ""
+        raise TfstatError(f"{what}: {msg}{extra} [status {rc}]")
+
+
+def _grid_args(g):
+    return [int(g.t0_min), int(g.dt0), int(g.N_t0), int(g.tau_min), int(g.dtau), int(g.N_tau)]
+
+
+def _opts(min_atoms: int, exp_method: int, events=None) -> _Opts:
+    o = _Opts()
+    o.min_atoms = int(min_atoms)
+    o.exp_method = int(exp_method)
+    if events is not None:  # (begin, end): recorded torch.cuda.Event(enable_timing=True)
+        o.ev_main_begin = int(events[0].cuda_event)
+        o.ev_main_end = int(events[1].cuda_event)
+    return o
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev_f32(x: torch.Tensor, name: str) -> torch.Tensor:
+    if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float32):
+        raise TfstatError(f"{name} must be a CUDA float32 tensor")
+    return x
+
+
+def _dev_i32(x: torch.Tensor, name: str) -> torch.Tensor:
+    if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.int32
+            and x.is_contiguous()):
+        raise TfstatError(f"{name} must be a contiguous CUDA int32 tensor")
+    return x
+
+
+def workspace_bytes(window: int, n_atoms: int, n_templates: int, grid, *, min_atoms: int = 2,
+                    exp_method: int = EXP_AUTO) -> int:
+    lib = load_library()
+    o = _opts(min_atoms, exp_method)
+    n = lib.tfstat_workspace_bytes(window, n_atoms, n_templates, *_grid_args(grid), C.byref(o))
+    if n == 0:
+        raise TfstatError("tfstat_workspace_bytes: invalid problem shape")
+    return int(n)
+
+
+def _workspace(nbytes: int, device, workspace: Optional[torch.Tensor]) -> torch.Tensor:
+    if workspace is not None:
+        if workspace.numel() * workspace.element_size() < nbytes:
+            raise TfstatError("workspace tensor too small")
+        return workspace
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+@dataclass
+class Results:
+    """Marginals of T maps; `raw` is the [T,5] int32 device image of tfstat_result[T]."""
+
+    raw: torch.Tensor
+    maps: Optional[torch.Tensor] = None
+    flags: Optional[torch.Tensor] = None
+
+    def numpy(self) -> np.ndarray:
+        return self.raw.cpu().numpy().view(RESULT_DTYPE).reshape(-1)
+
+    @property
+    def max2F(self) -> torch.Tensor:
+        return self.raw[:, 0].view(torch.float32)
+
+    @property
+    def logB(self) -> torch.Tensor:
+        return self.raw[:, 3].view(torch.float32)
+
+
+def tfstat_map(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
+               min_atoms: int = 2, exp_method: int = EXP_AUTO, want_flags: bool = False,
+               out_map: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+               stream=None):
+    """atoms [7, N] (row stride = ld) -> (map [N_t0, N_tau] fp32 of 2F, flags uint8 or None)."""
+    lib = load_library()
+    _dev_f32(atoms, "atoms")
+    _dev_i32(t_atoms, "t_atoms")
+    if atoms.dim() != 2 or atoms.shape[0] != 7 or atoms.stride(1) != 1:
+        raise TfstatError("atoms must be [7, N] with unit stride along N")
+    n_atoms, ld = int(t_atoms.shape[0]), int(atoms.stride(0))
+    if atoms.shape[1] != n_atoms:
+        raise TfstatError("atoms / t_atoms length mismatch")
+    dev = atoms.device
+    if out_map is None:
+        out_map = torch.empty((grid.N_t0, grid.N_tau), dtype=torch.float32, device=dev)
+    flags = (torch.empty((grid.N_t0, grid.N_tau), dtype=torch.uint8, device=dev)
+             if want_flags else None)
+    nbytes = workspace_bytes(window, n_atoms, 1, grid, min_atoms=min_atoms, exp_method=exp_method)
+    ws = _workspace(nbytes, dev, workspace)
+    o = _opts(min_atoms, exp_method)
+    rc = lib.tfstat_map(atoms.data_ptr(), ld, t_atoms.data_ptr(), n_atoms, window,
+                        *_grid_args(grid), out_map.data_ptr(),
+                        flags.data_ptr() if flags is not None else None, ws.data_ptr(), nbytes,
+                        _stream_ptr(stream), C.byref(o))
+    _check(rc, "tfstat_map")
+    return out_map, flags
+
+
+def tfstat_marginalise(map2F: torch.Tensor, flags: Optional[torch.Tensor] = None, *,
+                       stream=None) -> Results:
+    lib = load_library()
+    _dev_f32(map2F, "map")
+    if map2F.dim() != 2 or not map2F.is_contiguous():
+        raise TfstatError("map must be a contiguous [N_t0, N_tau] tensor")
+    if flags is not None and not (flags.is_cuda and flags.dtype == torch.uint8
+                                  and flags.is_contiguous() and flags.shape == map2F.shape):
+        raise TfstatError("flags must be a contiguous CUDA uint8 tensor shaped like map")
+    N_t0, N_tau = map2F.shape
+    nbytes = int(lib.tfstat_marginalise_workspace_bytes(N_t0, N_tau))
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=map2F.device)
+    out = torch.empty((1, 5), dtype=torch.int32, device=map2F.device)
+    rc = lib.tfstat_marginalise(map2F.data_ptr(), flags.data_ptr() if flags is not None else None,
+                                N_t0, N_tau, out.data_ptr(), ws.data_ptr(), nbytes,
+                                _stream_ptr(stream))
+    _check(rc, "tfstat_marginalise")
+    return Results(out)
+
+
+def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
+                  min_atoms: int = 2, exp_method: int = EXP_AUTO, want_maps: bool = False,
+                  want_flags: bool = False, workspace: Optional[torch.Tensor] = None,
+                  out: Optional[torch.Tensor] = None, stream=None,
+                  main_kernel_events=None) -> Results:
+    """atoms [T, 7, N] -> marginals of the T maps (and the maps / flags if asked)."""
+    lib = load_library()
+    _dev_f32(atoms, "atoms")
+    _dev_i32(t_atoms, "t_atoms")
+    if atoms.dim() != 3 or atoms.shape[1] != 7 or atoms.stride(2) != 1:
+        raise TfstatError("atoms must be [T, 7, N] with unit stride along N")
+    T, n_atoms = int(atoms.shape[0]), int(t_atoms.shape[0])
+    if atoms.shape[2] != n_atoms:
+        raise TfstatError("atoms / t_atoms length mismatch")
+    tstride, ld = int(atoms.stride(0)), int(atoms.stride(1))
+    dev = atoms.device
+    if out is None:
+        out = torch.empty((T, 5), dtype=torch.int32, device=dev)
+    maps = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.float32, device=dev)
+            if want_maps else None)
+    flags = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.uint8, device=dev)
+             if want_flags else None)
+    nbytes = workspace_bytes(window, n_atoms, T, grid, min_atoms=min_atoms, exp_method=exp_method)
+    ws = _workspace(nbytes, dev, workspace)
+    o = _opts(min_atoms, exp_method, main_kernel_events)
+    rc = lib.tfstat_search(atoms.data_ptr(), tstride, ld, t_atoms.data_ptr(), n_atoms, T, window,
+                           *_grid_args(grid), out.data_ptr(),
+                           maps.data_ptr() if maps is not None else None,
+                           flags.data_ptr() if flags is not None else None, ws.data_ptr(), nbytes,
+                           _stream_ptr(stream), C.byref(o))
+    _check(rc, "tfstat_search")
+    return Results(out, maps, flags)
+
+
+def count_terms(t_atoms: torch.Tensor, window: int, grid, *, stream=None) -> int:
+    """N_sums of eqs. (A.5)/(A.6) with gaps: total (cell, atom-in-window) pairs of the grid."""
+    lib = load_library()
+    _dev_i32(t_atoms, "t_atoms")
+    n_atoms = int(t_atoms.shape[0])
+    nbytes = workspace_bytes(window, n_atoms, 1, grid)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=t_atoms.device)
+    out = torch.zeros(1, dtype=torch.int64, device=t_atoms.device)
+    rc = lib.tfstat_count_terms(t_atoms.data_ptr(), n_atoms, window, *_grid_args(grid),
+                                out.data_ptr(), ws.data_ptr(), nbytes, _stream_ptr(stream))
+    _check(rc, "tfstat_count_terms")
+    return int(out.item())
+
+
+def tfstat_search_host(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
+                       min_atoms: int = 2, exp_method: int = EXP_AUTO, want_maps: bool = False,
+                       max_device_bytes: int = 0):
+    """End-to-end call on HOST tensors (pinned for overlap): H2D copies, fused search and D2H
+    of the results all happen inside the library.  Returns (results ndarray, maps or None)."""
+    lib = load_library()
+    if atoms.is_cuda or t_atoms.is_cuda:
+        raise TfstatError("tfstat_search_host takes host (CPU) tensors")
+    if atoms.dtype != torch.float32 or t_atoms.dtype != torch.int32:
+        raise TfstatError("atoms must be float32 and t_atoms int32")
+    if atoms.dim() != 3 or atoms.shape[1] != 7 or atoms.stride(2) != 1:
+        raise TfstatError("atoms must be [T, 7, N] with unit stride along N")
+    T, n_atoms = int(atoms.shape[0]), int(t_atoms.shape[0])
+    out = torch.empty((T, 5), dtype=torch.int32).pin_memory()
+    maps = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.float32).pin_memory()
+            if want_maps else None)
+    o = _opts(min_atoms, exp_method)
+    rc = lib.tfstat_search_host(atoms.data_ptr(), int(atoms.stride(0)), int(atoms.stride(1)),
+                                t_atoms.data_ptr(), n_atoms, T, window, *_grid_args(grid),
+                                out.data_ptr(), maps.data_ptr() if maps is not None else None,
+                                int(max_device_bytes), C.byref(o))
+    _check(rc, "tfstat_search_host")
+    return out.numpy().view(RESULT_DTYPE).reshape(-1), maps
+
+
+PROBE_KINDS = {"ffma": 0, "fadd": 1, "mufu_ex2": 2, "ffma2": 3, "fadd2": 4, "ffma_mufu": 5,
+               "lds128": 6, "dfma": 7}
+
+
+def probe_alu(kind: str, reps: int = 3) -> dict:
+    """Measured issue rate of one instruction class on the current GPU (tfstat_probe.h)."""
+    lib = load_library()
+    a, b, c = C.c_double(0), C.c_double(0), C.c_double(0)
+    rc = lib.tfstat_probe_alu(PROBE_KINDS[kind], reps, C.byref(a), C.byref(b), C.byref(c))
+    _check(rc, f"tfstat_probe_alu({kind})")
+    return dict(kind=kind, lane_ops_per_s=a.value, ops_per_clk_sm=b.value, sm_mhz=c.value)

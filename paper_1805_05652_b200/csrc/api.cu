@@ -1,0 +1,350 @@
+// api.cu -- the C ABI of include/tfstat.h: argument validation, the problem plan (workspace
+// layout, tile shapes) and the launch sequences.  No arithmetic of the method lives here.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "plan.h"
+
+namespace tfstat {
+
+static thread_local int g_last_cuda_error = 0;
+
+static int cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    return TFSTAT_ECUDA;
+}
+#define TF_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e__ = (call);                       \
+        if (e__ != cudaSuccess) return cuda_fail(e__);  \
+    } while (0)
+
+Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min, int32_t dt0,
+               int32_t N_t0, int32_t tau_min, int32_t dtau, int32_t N_tau,
+               const tfstat_opts *opts)
+{
+    Plan pl;
+    std::memset(&pl, 0, sizeof(pl));
+    pl.status = TFSTAT_EINVAL;
+    if (window != TFSTAT_WINDOW_RECT && window != TFSTAT_WINDOW_EXP) return pl;
+    if (n_atoms < 1 || n_templates < 1 || N_t0 < 1 || N_tau < 1 || tau_min < 1) return pl;
+    if ((N_t0 > 1 && dt0 < 1) || (N_tau > 1 && dtau < 1)) return pl;
+    if ((int64_t)N_t0 * N_tau >= (int64_t(1) << 31)) return pl;
+    int method = opts ? opts->exp_method : TFSTAT_EXP_AUTO;
+    if (method == TFSTAT_EXP_AUTO) method = TFSTAT_EXP_DIRECT;
+    if (method != TFSTAT_EXP_DIRECT && method != TFSTAT_EXP_SCAN) return pl;
+    const int64_t k = window == TFSTAT_WINDOW_EXP ? 3 : 1;
+    const int64_t t0_max = (int64_t)t0_min + (int64_t)(N_t0 - 1) * (N_t0 > 1 ? dt0 : 0);
+    const int64_t tau_max = (int64_t)tau_min + (int64_t)(N_tau - 1) * (N_tau > 1 ? dtau : 0);
+    if (t0_max + k * tau_max > INT32_MAX || t0_max > INT32_MAX || tau_max > INT32_MAX) {
+        pl.status = TFSTAT_EOVERFLOW;
+        return pl;
+    }
+    pl.window = window;
+    pl.exp_method = method;
+    pl.n_atoms = n_atoms;
+    pl.n_templates = n_templates;
+    pl.min_atoms = (opts && opts->min_atoms > 0) ? opts->min_atoms : 2;
+    pl.ev_main_begin = opts ? static_cast<cudaEvent_t>(opts->ev_main_begin) : nullptr;
+    pl.ev_main_end = opts ? static_cast<cudaEvent_t>(opts->ev_main_end) : nullptr;
+    pl.grid.t0_min = t0_min;
+    pl.grid.dt0 = N_t0 > 1 ? dt0 : 0;
+    pl.grid.N_t0 = N_t0;
+    pl.grid.tau_min = tau_min;
+    pl.grid.dtau = N_tau > 1 ? dtau : 0;
+    pl.grid.N_tau = N_tau;
+    pl.grid.k = (int32_t)k;
+
+    // a1 edge lattice: every window end t0_m + k tau_n sits on base + j g
+    const int64_t sa = pl.grid.dt0, sb = k * pl.grid.dtau;
+    int64_t g = gcd64(sa, sb);
+    if (g == 0) g = 1;
+    pl.g = g;
+    pl.e_m = (int32_t)(sa / g);
+    pl.e_n = (int32_t)(sb / g);
+    pl.J = (int64_t)(N_t0 - 1) * pl.e_m + (int64_t)(N_tau - 1) * pl.e_n + 1;
+    if (pl.J > kMaxEdgeEntries) {
+        pl.J = 0;  // per-cell binary search instead
+        pl.e_m = pl.e_n = 0;
+    }
+
+    // exp direct tile shape: largest tile that still yields a few waves of CTAs on 148 SMs
+    const int64_t cells = (int64_t)N_t0 * N_tau;
+    const int64_t total = cells * n_templates;
+    if (total >= (int64_t)8 * 256 * 148 * 4) pl.tile = ExpTile{8, 256};
+    else if (total >= (int64_t)4 * 128 * 148 * 4) pl.tile = ExpTile{4, 128};
+    else pl.tile = ExpTile{2, 64};
+    pl.n_mtiles = (N_t0 + pl.tile.C - 1) / pl.tile.C;
+    pl.n_nblocks = (N_tau + pl.tile.NT - 1) / pl.tile.NT;
+    pl.tiles_per_template = (int64_t)pl.n_mtiles * pl.n_nblocks;
+    pl.cell_blocks_per_template = (int32_t)((cells + 255) / 256);
+
+    const bool direct = window == TFSTAT_WINDOW_EXP && method == TFSTAT_EXP_DIRECT;
+    pl.partials_per_template = direct ? pl.tiles_per_template : pl.cell_blocks_per_template;
+    if (pl.partials_per_template * n_templates >= (int64_t(1) << 31)) return pl;
+
+    size_t off = 0;
+    pl.off_lo = off;
+    off += align_up(sizeof(int32_t) * (size_t)N_t0);
+    pl.off_edge = off;
+    off += align_up(sizeof(int32_t) * (size_t)pl.J);
+    pl.off_partials = off;
+    off += align_up(sizeof(Partial) * (size_t)pl.partials_per_template * n_templates);
+    pl.off_prefix = off;
+    if (window == TFSTAT_WINDOW_RECT)
+        off += align_up(sizeof(double) * 8 * ((size_t)n_atoms + 1) * n_templates);
+    pl.off_scan = off;
+    pl.bytes = off;
+    pl.status = TFSTAT_OK;
+    return pl;
+}
+
+static int run_device(const Plan &pl, const float *atoms, int64_t template_stride, int64_t ld,
+                      const int32_t *t_atoms, tfstat_result *out, float *out_maps,
+                      uint8_t *out_flags, void *ws, cudaStream_t st, bool do_bounds)
+{
+    if (do_bounds) TF_CUDA(launch_bounds(pl, t_atoms, ws, st));
+    Problem pr;
+    pr.atoms = atoms;
+    pr.template_stride = template_stride;
+    pr.ld = ld;
+    pr.n_templates = pl.n_templates;
+    pr.min_atoms = pl.min_atoms;
+    pr.grid = pl.grid;
+    pr.bounds = make_bounds(pl, t_atoms, ws);
+    pr.out = out;
+    pr.out_maps = out_maps;
+    pr.out_flags = out_flags;
+    Partial *partials =
+        out ? reinterpret_cast<Partial *>(static_cast<char *>(ws) + pl.off_partials) : nullptr;
+    if (pl.ev_main_begin) TF_CUDA(cudaEventRecord(pl.ev_main_begin, st));
+    if (pl.window == TFSTAT_WINDOW_RECT) {
+        double *prefix = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_prefix);
+        TF_CUDA(launch_rect(pl, pr, prefix, partials, st));
+    } else if (pl.exp_method == TFSTAT_EXP_DIRECT) {
+        TF_CUDA(launch_exp_direct(pl, pr, partials, st));
+    } else {
+        float *scan_ws = reinterpret_cast<float *>(static_cast<char *>(ws) + pl.off_scan);
+        TF_CUDA(launch_exp_scan(pl, pr, scan_ws, partials, st));
+    }
+    if (pl.ev_main_end) TF_CUDA(cudaEventRecord(pl.ev_main_end, st));
+    if (out)
+        TF_CUDA(launch_finalize(partials, pl.partials_per_template, pl.n_templates,
+                                pl.grid.N_tau, out, st));
+    return TFSTAT_OK;
+}
+
+}  // namespace tfstat
+
+using namespace tfstat;
+
+extern "C" {
+
+int tfstat_version(void) { return TFSTAT_VERSION; }
+
+const char *tfstat_strerror(int status)
+{
+    switch (status) {
+    case TFSTAT_OK: return "ok";
+    case TFSTAT_EINVAL: return "invalid argument";
+    case TFSTAT_EWORKSPACE: return "workspace missing or too small";
+    case TFSTAT_ECUDA: return "CUDA error (see tfstat_last_cuda_error)";
+    case TFSTAT_EOVERFLOW: return "grid times exceed int32";
+    default: return "unknown status";
+    }
+}
+
+int tfstat_last_cuda_error(void) { return g_last_cuda_error; }
+
+size_t tfstat_workspace_bytes(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
+                              int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                              int32_t N_tau, const tfstat_opts *opts_host)
+{
+    const Plan pl = make_plan(window, n_atoms, n_templates, t0_min, dt0, N_t0, tau_min, dtau,
+                              N_tau, opts_host);
+    return pl.status == TFSTAT_OK ? std::max(pl.bytes, kAlign) : 0;
+}
+
+int tfstat_search(const float *atoms, int64_t template_stride, int64_t ld,
+                  const int32_t *t_atoms, int32_t n_atoms, int32_t n_templates, int window,
+                  int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                  int32_t N_tau, tfstat_result *out, float *out_maps, uint8_t *out_flags,
+                  void *workspace, size_t workspace_bytes, void *stream,
+                  const tfstat_opts *opts_host)
+{
+    if (!atoms || !t_atoms || (!out && !out_maps)) return TFSTAT_EINVAL;
+    if (ld < n_atoms || (n_templates > 1 && template_stride < 7 * ld)) return TFSTAT_EINVAL;
+    const Plan pl = make_plan(window, n_atoms, n_templates, t0_min, dt0, N_t0, tau_min, dtau,
+                              N_tau, opts_host);
+    if (pl.status != TFSTAT_OK) return pl.status;
+    if (!workspace || workspace_bytes < pl.bytes ||
+        (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)))
+        return TFSTAT_EWORKSPACE;
+    return run_device(pl, atoms, template_stride, ld, t_atoms, out, out_maps, out_flags,
+                      workspace, static_cast<cudaStream_t>(stream), true);
+}
+
+int tfstat_map(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
+               int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
+               int32_t dtau, int32_t N_tau, float *out_map, uint8_t *out_flags,
+               void *workspace, size_t workspace_bytes, void *stream,
+               const tfstat_opts *opts_host)
+{
+    if (!out_map) return TFSTAT_EINVAL;
+    return tfstat_search(atoms, 7 * ld, ld, t_atoms, n_atoms, 1, window, t0_min, dt0, N_t0,
+                         tau_min, dtau, N_tau, nullptr, out_map, out_flags, workspace,
+                         workspace_bytes, stream, opts_host);
+}
+
+size_t tfstat_marginalise_workspace_bytes(int32_t N_t0, int32_t N_tau)
+{
+    if (N_t0 < 1 || N_tau < 1) return 0;
+    return align_up(sizeof(Partial) * (size_t)marginalise_blocks((int64_t)N_t0 * N_tau));
+}
+
+int tfstat_marginalise(const float *map, const uint8_t *flags, int32_t N_t0, int32_t N_tau,
+                       tfstat_result *out, void *workspace, size_t workspace_bytes,
+                       void *stream)
+{
+    if (!map || !out || N_t0 < 1 || N_tau < 1) return TFSTAT_EINVAL;
+    const int64_t n_cells = (int64_t)N_t0 * N_tau;
+    if (n_cells >= (int64_t(1) << 31)) return TFSTAT_EINVAL;
+    const int32_t nb = marginalise_blocks(n_cells);
+    if (!workspace || workspace_bytes < sizeof(Partial) * (size_t)nb) return TFSTAT_EWORKSPACE;
+    TF_CUDA(launch_marginalise(map, flags, n_cells, N_tau, static_cast<Partial *>(workspace),
+                               nb, out, static_cast<cudaStream_t>(stream)));
+    return TFSTAT_OK;
+}
+
+int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int32_t t0_min,
+                       int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                       int32_t N_tau, int64_t *out_terms, void *workspace,
+                       size_t workspace_bytes, void *stream)
+{
+    if (!t_atoms || !out_terms) return TFSTAT_EINVAL;
+    const Plan pl = make_plan(window, n_atoms, 1, t0_min, dt0, N_t0, tau_min, dtau, N_tau,
+                              nullptr);
+    if (pl.status != TFSTAT_OK) return pl.status;
+    if (!workspace || workspace_bytes < pl.bytes) return TFSTAT_EWORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    TF_CUDA(launch_bounds(pl, t_atoms, workspace, st));
+    TF_CUDA(launch_count_terms(pl, make_bounds(pl, t_atoms, workspace), out_terms, st));
+    return TFSTAT_OK;
+}
+
+int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t ld,
+                       const int32_t *t_atoms_host, int32_t n_atoms, int32_t n_templates,
+                       int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
+                       int32_t dtau, int32_t N_tau, tfstat_result *out_host,
+                       float *out_maps_host, size_t max_device_bytes,
+                       const tfstat_opts *opts_host)
+{
+    if (!atoms_host || !t_atoms_host || !out_host) return TFSTAT_EINVAL;
+    if (ld < n_atoms || (n_templates > 1 && template_stride < 7 * ld)) return TFSTAT_EINVAL;
+    if (n_templates < 1) return TFSTAT_EINVAL;
+    if (max_device_bytes == 0) max_device_bytes = size_t(2) << 30;
+    const int64_t cells = (int64_t)N_t0 * N_tau;
+    // templates per chunk: two atom buffers (+ two map buffers) + workspace within the budget
+    const size_t tpl_bytes = sizeof(float) * (size_t)template_stride;
+    const size_t map_bytes = out_maps_host ? sizeof(float) * (size_t)cells : 0;
+    int32_t Tc = std::min<int32_t>(n_templates, 256);
+    Plan pl;
+    for (;; Tc = (Tc + 1) / 2) {
+        pl = make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts_host);
+        if (pl.status != TFSTAT_OK) return pl.status;
+        const size_t need = 2 * Tc * (tpl_bytes + map_bytes) + pl.bytes;
+        if (need <= max_device_bytes || Tc == 1) break;
+    }
+    const int n_chunks = (n_templates + Tc - 1) / Tc;
+
+    char *d_atoms[2] = {nullptr, nullptr};
+    float *d_maps[2] = {nullptr, nullptr};
+    void *d_ws = nullptr;
+    int32_t *d_t = nullptr;
+    tfstat_result *d_out = nullptr;
+    cudaStream_t s_copy = nullptr, s_comp = nullptr, s_back = nullptr;
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr},
+                ev_back[2] = {nullptr, nullptr};
+    int rc = TFSTAT_OK;
+    auto chk = [&](cudaError_t e) {
+        if (e != cudaSuccess && rc == TFSTAT_OK) rc = cuda_fail(e);
+        return e == cudaSuccess;
+    };
+    do {
+        if (!chk(cudaStreamCreateWithFlags(&s_copy, cudaStreamNonBlocking))) break;
+        if (!chk(cudaStreamCreateWithFlags(&s_comp, cudaStreamNonBlocking))) break;
+        if (!chk(cudaStreamCreateWithFlags(&s_back, cudaStreamNonBlocking))) break;
+        bool ok = true;
+        for (int b = 0; b < 2 && ok; ++b) {
+            ok = chk(cudaMalloc(&d_atoms[b], Tc * tpl_bytes)) &&
+                 chk(cudaEventCreateWithFlags(&ev_in[b], cudaEventDisableTiming)) &&
+                 chk(cudaEventCreateWithFlags(&ev_done[b], cudaEventDisableTiming)) &&
+                 chk(cudaEventCreateWithFlags(&ev_back[b], cudaEventDisableTiming));
+            if (ok && map_bytes) ok = chk(cudaMalloc(&d_maps[b], Tc * map_bytes));
+        }
+        if (!ok) break;
+        if (!chk(cudaMalloc(&d_ws, std::max(pl.bytes, kAlign)))) break;
+        if (!chk(cudaMalloc(&d_t, sizeof(int32_t) * (size_t)n_atoms))) break;
+        if (!chk(cudaMalloc(&d_out, sizeof(tfstat_result) * (size_t)n_templates))) break;
+        if (!chk(cudaMemcpyAsync(d_t, t_atoms_host, sizeof(int32_t) * (size_t)n_atoms,
+                                 cudaMemcpyHostToDevice, s_comp)))
+            break;
+        for (int c = 0; c < n_chunks && rc == TFSTAT_OK; ++c) {
+            const int b = c & 1;
+            const int32_t k0 = c * Tc;
+            const int32_t cnt = std::min<int32_t>(Tc, n_templates - k0);
+            Plan plc = pl;
+            if (cnt != Tc)
+                plc = make_plan(window, n_atoms, cnt, t0_min, dt0, N_t0, tau_min, dtau, N_tau,
+                                opts_host);
+            // buffer b is free once chunk c-2 has been computed (and its maps copied back)
+            if (c >= 2) {
+                chk(cudaStreamWaitEvent(s_copy, ev_done[b], 0));
+                if (map_bytes) chk(cudaStreamWaitEvent(s_comp, ev_back[b], 0));
+            }
+            const size_t n_float = (size_t)(cnt - 1) * template_stride + 6 * ld + n_atoms;
+            chk(cudaMemcpyAsync(d_atoms[b], atoms_host + (size_t)k0 * template_stride,
+                                sizeof(float) * n_float, cudaMemcpyHostToDevice, s_copy));
+            chk(cudaEventRecord(ev_in[b], s_copy));
+            chk(cudaStreamWaitEvent(s_comp, ev_in[b], 0));
+            const int r = run_device(plc, reinterpret_cast<const float *>(d_atoms[b]),
+                                     template_stride, ld, d_t, d_out + k0, d_maps[b], nullptr,
+                                     d_ws, s_comp, c == 0);
+            if (r != TFSTAT_OK) rc = r;
+            chk(cudaEventRecord(ev_done[b], s_comp));
+            if (map_bytes) {
+                chk(cudaStreamWaitEvent(s_back, ev_done[b], 0));
+                chk(cudaMemcpyAsync(out_maps_host + (size_t)k0 * cells, d_maps[b],
+                                    (size_t)cnt * map_bytes, cudaMemcpyDeviceToHost, s_back));
+                chk(cudaEventRecord(ev_back[b], s_back));
+            }
+        }
+        if (rc != TFSTAT_OK) break;
+        chk(cudaMemcpyAsync(out_host, d_out, sizeof(tfstat_result) * (size_t)n_templates,
+                            cudaMemcpyDeviceToHost, s_comp));
+        chk(cudaStreamSynchronize(s_comp));
+        chk(cudaStreamSynchronize(s_back));
+    } while (0);
+    if (s_copy) cudaStreamSynchronize(s_copy);
+    if (s_comp) cudaStreamSynchronize(s_comp);
+    if (s_back) cudaStreamSynchronize(s_back);
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(d_atoms[b]);
+        cudaFree(d_maps[b]);
+        if (ev_in[b]) cudaEventDestroy(ev_in[b]);
+        if (ev_done[b]) cudaEventDestroy(ev_done[b]);
+        if (ev_back[b]) cudaEventDestroy(ev_back[b]);
+    }
+    cudaFree(d_ws);
+    cudaFree(d_t);
+    cudaFree(d_out);
+    if (s_copy) cudaStreamDestroy(s_copy);
+    if (s_comp) cudaStreamDestroy(s_comp);
+    if (s_back) cudaStreamDestroy(s_back);
+    return rc;
+}
+
+}  // extern "C"

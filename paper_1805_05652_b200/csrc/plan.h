@@ -1,0 +1,92 @@
+// plan.h -- host-side problem plan: validation, edge-lattice, tile shapes, workspace layout.
+// One function of the problem shape, used by tfstat_workspace_bytes() and by every launcher,
+// so the caller-provided workspace and the kernels always agree.
+#pragma once
+#include <stddef.h>
+#include <stdint.h>
+
+#include "tfstat_dev.cuh"
+
+namespace tfstat {
+
+constexpr int64_t kMaxEdgeEntries = int64_t(1) << 22;  // 16 MiB of int32; beyond: binary search
+constexpr size_t kAlign = 256;
+
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+inline int64_t gcd64(int64_t a, int64_t b)
+{
+    while (b) {
+        const int64_t r = a % b;
+        a = b;
+        b = r;
+    }
+    return a;
+}
+
+// exp direct kernel tile shapes: C cells along t0 per thread, NT tau values per CTA
+struct ExpTile {
+    int C;
+    int NT;
+};
+
+struct Plan {
+    int status;  // TFSTAT_OK or error
+    int window;
+    int exp_method;
+    int32_t n_atoms, n_templates, min_atoms;
+    Grid grid;
+    // a1 edge lattice
+    int64_t g;  // lattice step (s)
+    int32_t e_m, e_n;
+    int64_t J;  // entries; 0 if the per-cell binary-search fallback is used
+    // exp direct tiling
+    ExpTile tile;
+    int32_t n_mtiles, n_nblocks;
+    int64_t tiles_per_template;
+    // rect / marginalise tiling
+    int32_t cell_blocks_per_template;
+    // workspace layout (byte offsets)
+    size_t off_lo, off_edge, off_partials, off_prefix, off_scan, bytes;
+    int64_t partials_per_template;
+    int32_t scan_chunk_templates;
+    cudaEvent_t ev_main_begin, ev_main_end;  // optional profiling hooks (tfstat_opts)
+};
+
+Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min, int32_t dt0,
+               int32_t N_t0, int32_t tau_min, int32_t dtau, int32_t N_tau,
+               const tfstat_opts *opts);
+
+// launchers -------------------------------------------------------------------------------
+cudaError_t launch_bounds(const Plan &pl, const int32_t *t_atoms, void *ws, cudaStream_t st);
+cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_terms,
+                               cudaStream_t st);
+cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,
+                              cudaStream_t st);
+cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, Partial *partials,
+                        cudaStream_t st);
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, float *scan_ws,
+                            Partial *partials, cudaStream_t st);
+cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_template,
+                            int32_t n_templates, int32_t N_tau, tfstat_result *out,
+                            cudaStream_t st);
+cudaError_t launch_marginalise(const float *map, const uint8_t *flags, int64_t n_cells,
+                               int32_t N_tau, Partial *partials, int32_t n_blocks,
+                               tfstat_result *out, cudaStream_t st);
+int32_t marginalise_blocks(int64_t n_cells);
+
+inline Bounds make_bounds(const Plan &pl, const int32_t *t_atoms, void *ws)
+{
+    Bounds b;
+    b.t = t_atoms;
+    b.n_atoms = pl.n_atoms;
+    b.lo = reinterpret_cast<const int32_t *>(static_cast<char *>(ws) + pl.off_lo);
+    b.edge = pl.J > 0 ? reinterpret_cast<const int32_t *>(static_cast<char *>(ws) + pl.off_edge)
+                      : nullptr;
+    b.e_m = pl.e_m;
+    b.e_n = pl.e_n;
+    b.J = (int32_t)pl.J;
+    return b;
+}
+
+}  // namespace tfstat

@@ -1,0 +1,172 @@
+// probe.cu -- register-only micro-kernels that measure the FP32 / XU / LDS issue rates of the
+// GPU the bench runs on (include/tfstat_probe.h).  They give the ALU roofline its denominator.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tfstat.h"
+#include "../../include/tfstat_probe.h"
+
+namespace {
+
+constexpr int kNT = 256;
+constexpr int kIters = 4096;
+constexpr int kChains = 16;
+
+template <int KIND>
+__global__ void __launch_bounds__(kNT) probe_kernel(const float *__restrict__ in,
+                                                    float *__restrict__ out,
+                                                    long long *__restrict__ cycles)
+{
+    __shared__ float4 s_v[64];
+    const float a = in[0], b = in[1];
+    if (threadIdx.x < 64) s_v[threadIdx.x] = make_float4(a, b, a, b);
+    __syncthreads();
+    float acc[kChains];
+#pragma unroll
+    for (int j = 0; j < kChains; ++j) acc[j] = a * (float)(threadIdx.x + j);
+    unsigned long long acc2[kChains / 2];
+#pragma unroll
+    for (int j = 0; j < kChains / 2; ++j)
+        acc2[j] = ((unsigned long long)__float_as_uint(acc[2 * j + 1]) << 32) |
+                  __float_as_uint(acc[2 * j]);
+    const unsigned long long ab2 =
+        ((unsigned long long)__float_as_uint(b) << 32) | __float_as_uint(a);
+    double dacc[kChains / 2];
+#pragma unroll
+    for (int j = 0; j < kChains / 2; ++j) dacc[j] = (double)acc[j];
+    const double da = (double)a, db = (double)b;
+    int sidx = threadIdx.x >> 5;
+    float xu0 = -a, xu1 = -b;
+
+    const long long c0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < kIters; ++it) {
+        if (KIND == TFSTAT_PROBE_FFMA) {
+#pragma unroll
+            for (int j = 0; j < kChains; ++j) acc[j] = fmaf(a, b, acc[j]);
+        } else if (KIND == TFSTAT_PROBE_FADD) {
+#pragma unroll
+            for (int j = 0; j < kChains; ++j) acc[j] = acc[j] + a;
+        } else if (KIND == TFSTAT_PROBE_MUFU_EX2) {
+#pragma unroll
+            for (int j = 0; j < kChains; ++j)
+                asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(acc[j]));
+        } else if (KIND == TFSTAT_PROBE_FFMA2) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j)
+                asm volatile("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(acc2[j]) : "l"(ab2));
+        } else if (KIND == TFSTAT_PROBE_FADD2) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j)
+                asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(acc2[j]) : "l"(ab2));
+        } else if (KIND == TFSTAT_PROBE_FFMA_MUFU) {
+#pragma unroll
+            for (int j = 0; j < kChains; ++j) acc[j] = fmaf(a, b, acc[j]);
+            asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(xu0));
+            asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(xu1));
+        } else if (KIND == TFSTAT_PROBE_LDS128) {
+#pragma unroll
+            for (int j = 0; j < kChains / 4; ++j) {
+                const float4 v = s_v[(sidx + j) & 63];
+                acc[4 * j] += v.x;
+                sidx += (int)v.y;  // b == 0 at run time; keeps the address data-dependent
+            }
+        } else if (KIND == TFSTAT_PROBE_DFMA) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j) dacc[j] = fma(da, db, dacc[j]);
+        }
+    }
+    const long long c1 = clock64();
+    float r = 0.f;
+#pragma unroll
+    for (int j = 0; j < kChains; ++j) r += acc[j];
+#pragma unroll
+    for (int j = 0; j < kChains / 2; ++j)
+        r += __uint_as_float((unsigned)acc2[j]) + __uint_as_float((unsigned)(acc2[j] >> 32)) +
+             (float)dacc[j];
+    out[(size_t)blockIdx.x * kNT + threadIdx.x] = r + (float)sidx + xu0 + xu1;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *cycles = c1 - c0;
+}
+
+int ops_per_iter(int kind)
+{
+    switch (kind) {
+    case TFSTAT_PROBE_FFMA:
+    case TFSTAT_PROBE_FADD:
+    case TFSTAT_PROBE_MUFU_EX2:
+    case TFSTAT_PROBE_FFMA2:
+    case TFSTAT_PROBE_FADD2: return kChains;
+    case TFSTAT_PROBE_FFMA_MUFU: return kChains + 2;
+    case TFSTAT_PROBE_LDS128: return kChains / 4;
+    case TFSTAT_PROBE_DFMA: return kChains / 2;
+    }
+    return 0;
+}
+
+template <int KIND>
+void launch(int grid, const float *in, float *out, long long *cyc)
+{
+    probe_kernel<KIND><<<grid, kNT>>>(in, out, cyc);
+}
+
+}  // namespace
+
+extern "C" int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s,
+                                double *ops_per_clk_sm, double *sm_mhz)
+{
+    if (kind < 0 || kind >= TFSTAT_PROBE_KINDS || !lane_ops_per_s) return TFSTAT_EINVAL;
+    if (reps < 1) reps = 3;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return TFSTAT_ECUDA;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return TFSTAT_ECUDA;
+    const int ctas_per_sm = 4;  // 1024 threads / SM, 8 warps per scheduler
+    const int grid = n_sm * ctas_per_sm;
+    float *in = nullptr, *out = nullptr;
+    long long *cyc = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = TFSTAT_ECUDA;
+    do {
+        if (cudaMalloc(&in, 2 * sizeof(float)) != cudaSuccess) break;
+        if (cudaMalloc(&out, sizeof(float) * (size_t)grid * kNT) != cudaSuccess) break;
+        if (cudaMalloc(&cyc, sizeof(long long)) != cudaSuccess) break;
+        const float h_in[2] = {kind == TFSTAT_PROBE_MUFU_EX2 ? -0.5f : 1.0000001f,
+                               kind == TFSTAT_PROBE_LDS128 ? 0.0f : 1e-9f};
+        if (cudaMemcpy(in, h_in, sizeof(h_in), cudaMemcpyHostToDevice) != cudaSuccess) break;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+        float best_ms = 1e30f;
+        for (int r = 0; r <= reps; ++r) {
+            cudaEventRecord(e0);
+            switch (kind) {
+            case 0: launch<0>(grid, in, out, cyc); break;
+            case 1: launch<1>(grid, in, out, cyc); break;
+            case 2: launch<2>(grid, in, out, cyc); break;
+            case 3: launch<3>(grid, in, out, cyc); break;
+            case 4: launch<4>(grid, in, out, cyc); break;
+            case 5: launch<5>(grid, in, out, cyc); break;
+            case 6: launch<6>(grid, in, out, cyc); break;
+            case 7: launch<7>(grid, in, out, cyc); break;
+            }
+            cudaEventRecord(e1);
+            if (cudaEventSynchronize(e1) != cudaSuccess) break;
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (r > 0 && ms < best_ms) best_ms = ms;
+        }
+        if (cudaGetLastError() != cudaSuccess || best_ms > 1e29f) break;
+        long long h_cyc = 0;
+        if (cudaMemcpy(&h_cyc, cyc, sizeof(h_cyc), cudaMemcpyDeviceToHost) != cudaSuccess) break;
+        const double ops = (double)grid * kNT * (double)kIters * ops_per_iter(kind);
+        *lane_ops_per_s = ops / (best_ms * 1e-3);
+        if (ops_per_clk_sm)
+            *ops_per_clk_sm = (double)ctas_per_sm * kNT * kIters * ops_per_iter(kind) / (double)h_cyc;
+        if (sm_mhz) *sm_mhz = (double)h_cyc / (best_ms * 1e-3) * 1e-6;
+        rc = TFSTAT_OK;
+    } while (0);
+    cudaFree(in);
+    cudaFree(out);
+    cudaFree(cyc);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    return rc;
+}

@@ -1,0 +1,216 @@
+// tfstat_dev.cuh -- shared device-side definitions for libtfstat (sm_100a).
+//
+// Notation follows the paper: atoms alpha with start times t_alpha; grid t0_m, tau_n; window
+// support W(m,n) = {alpha : t0_m <= t_alpha < t0_m + k tau_n}, k = 1 (rect, eq. 3) or 3 (exp,
+// eq. 4); sums A,B,C,Fa,Fb; D = AB - C^2 and eq. (7).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tfstat.h"
+
+namespace tfstat {
+
+// ---------------------------------------------------------------------------------------
+// problem description passed by value to every kernel
+// ---------------------------------------------------------------------------------------
+struct Grid {
+    int32_t t0_min, dt0, N_t0;
+    int32_t tau_min, dtau, N_tau;
+    int32_t k;  // window length in units of tau: 1 rect, 3 exp
+};
+
+// Step a1: window -> atom-index bounds.
+//   lo[m]   = first alpha with t_alpha >= t0_m
+//   hi(m,n) = first alpha with t_alpha >= t0_m + k tau_n
+// All window end times lie on the lattice base + j*g, g = gcd(dt0, k dtau), so one table
+// edge[j] = lower_bound(t, base + j g), j = m*e_m + n*e_n, serves every cell (and every
+// template: timestamps are shared).  If the lattice is too fine (edge == nullptr) kernels
+// fall back to a binary search per cell.
+struct Bounds {
+    const int32_t *t;     // [n_atoms] timestamps
+    const int32_t *lo;    // [N_t0]
+    const int32_t *edge;  // [J] or nullptr
+    int32_t n_atoms;
+    int32_t e_m, e_n;
+    int32_t J;
+};
+
+__device__ __forceinline__ int lower_bound_t(const int32_t *__restrict__ t, int n, long long x)
+{
+    int a = 0, b = n;  // first index with t[i] >= x
+    while (a < b) {
+        const int mid = (a + b) >> 1;
+        if ((long long)__ldg(t + mid) < x) a = mid + 1;
+        else b = mid;
+    }
+    return a;
+}
+
+__device__ __forceinline__ long long t0_of(const Grid &g, int m)
+{
+    return (long long)g.t0_min + (long long)m * g.dt0;
+}
+__device__ __forceinline__ long long tau_of(const Grid &g, int n)
+{
+    return (long long)g.tau_min + (long long)n * g.dtau;
+}
+
+__device__ __forceinline__ int hi_index(const Bounds &b, const Grid &g, int m, int n)
+{
+    if (b.edge) return __ldg(b.edge + (long long)m * b.e_m + (long long)n * b.e_n);
+    return lower_bound_t(b.t, b.n_atoms, t0_of(g, m) + (long long)g.k * tau_of(g, n));
+}
+
+// ---------------------------------------------------------------------------------------
+// step a4: cell closure, eq. (7).  Sums come in as fp32 (exp path) or fp64 (rect path); the
+// closure itself runs in fp64 because D = AB - C^2 and the numerator both cancel by the
+// conditioning number D/(AB).
+// ---------------------------------------------------------------------------------------
+struct Sums64 {
+    double A, B, C, far, fai, fbr, fbi;
+};
+
+__device__ __forceinline__ float closure_2F(const Sums64 &s, int cnt, int min_atoms,
+                                            uint32_t &flags)
+{
+    const double D = s.A * s.B - s.C * s.C;
+    flags = (cnt < min_atoms ? 1u : 0u) | (!(D > 0.0) ? 2u : 0u);
+    if (flags) return 0.0f;
+    const double na = s.far * s.far + s.fai * s.fai;
+    const double nb = s.fbr * s.fbr + s.fbi * s.fbi;
+    const double re = s.far * s.fbr + s.fai * s.fbi;
+    const double num = s.B * na + s.A * nb - 2.0 * s.C * re;
+    return (float)(2.0 * num / D);
+}
+
+// ---------------------------------------------------------------------------------------
+// step a5: marginalisation state (max 2F with lowest-index argmax; online log-sum-exp)
+// ---------------------------------------------------------------------------------------
+struct Marg {
+    float best;    // max 2F so far (-inf if none)
+    int32_t idx;   // flat index of best (INT_MAX if none)
+    float M;       // running max of F = 2F/2 (-inf if none)
+    float S;       // sum exp(F - M)
+    int32_t nvalid;
+};
+
+struct __align__(16) Partial {  // one per CTA in the workspace, 32 bytes
+    float best;
+    int32_t idx;
+    float M;
+    float S;
+    int32_t nvalid;
+    int32_t pad[3];
+};
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+#define TFSTAT_LOG2E_F 1.4426950408889634f
+
+__device__ __forceinline__ void marg_init(Marg &a)
+{
+    a.best = -INFINITY;
+    a.idx = 0x7fffffff;
+    a.M = -INFINITY;
+    a.S = 0.0f;
+    a.nvalid = 0;
+}
+
+__device__ __forceinline__ void marg_add(Marg &a, float twoF, int32_t flat)
+{
+    if (twoF > a.best || (twoF == a.best && flat < a.idx)) {
+        a.best = twoF;
+        a.idx = flat;
+    }
+    const float F = 0.5f * twoF;
+    if (F > a.M) {
+        a.S = a.S * ex2_approx((a.M - F) * TFSTAT_LOG2E_F) + 1.0f;  // M = -inf: S*0 + 1
+        a.M = F;
+    } else {
+        a.S += ex2_approx((F - a.M) * TFSTAT_LOG2E_F);
+    }
+    a.nvalid += 1;
+}
+
+__device__ __forceinline__ void marg_merge(Marg &a, const Marg &b)
+{
+    if (b.best > a.best || (b.best == a.best && b.idx < a.idx)) {
+        a.best = b.best;
+        a.idx = b.idx;
+    }
+    const float M = fmaxf(a.M, b.M);
+    if (M > -INFINITY) {
+        a.S = a.S * ex2_approx((a.M - M) * TFSTAT_LOG2E_F) +
+              b.S * ex2_approx((b.M - M) * TFSTAT_LOG2E_F);
+        a.M = M;
+    }
+    a.nvalid += b.nvalid;
+}
+
+__device__ __forceinline__ Marg marg_shfl_xor(const Marg &a, int lane_mask)
+{
+    Marg b;
+    b.best = __shfl_xor_sync(0xffffffffu, a.best, lane_mask);
+    b.idx = __shfl_xor_sync(0xffffffffu, a.idx, lane_mask);
+    b.M = __shfl_xor_sync(0xffffffffu, a.M, lane_mask);
+    b.S = __shfl_xor_sync(0xffffffffu, a.S, lane_mask);
+    b.nvalid = __shfl_xor_sync(0xffffffffu, a.nvalid, lane_mask);
+    return b;
+}
+
+__device__ __forceinline__ void marg_warp_reduce(Marg &a)
+{
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        const Marg b = marg_shfl_xor(a, s);
+        marg_merge(a, b);
+    }
+}
+
+// Block reduce; result valid in thread 0.  `scratch` holds >= 32 Marg.
+template <int NT>
+__device__ __forceinline__ void marg_block_reduce(Marg &a, Marg *scratch)
+{
+    marg_warp_reduce(a);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) scratch[warp] = a;
+    __syncthreads();
+    if (warp == 0) {
+        if (lane < NT / 32) a = scratch[lane];
+        else marg_init(a);
+        marg_warp_reduce(a);
+    }
+}
+
+__device__ __forceinline__ void partial_store(Partial *p, const Marg &a)
+{
+    p->best = a.best;
+    p->idx = a.idx;
+    p->M = a.M;
+    p->S = a.S;
+    p->nvalid = a.nvalid;
+}
+
+// ---------------------------------------------------------------------------------------
+// host-side launchers (one per .cu file)
+// ---------------------------------------------------------------------------------------
+struct Problem {
+    const float *atoms;        // [T][7][ld]
+    int64_t template_stride;   // floats
+    int64_t ld;
+    int32_t n_templates;
+    int32_t min_atoms;
+    Grid grid;
+    Bounds bounds;
+    tfstat_result *out;        // [T] or nullptr
+    float *out_maps;           // [T][N_t0][N_tau] or nullptr
+    uint8_t *out_flags;        // same shape or nullptr
+};
+
+}  // namespace tfstat

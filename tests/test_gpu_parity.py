@@ -1,0 +1,244 @@
+"""GPU parity: the CUDA path through the C ABI against the fp64 oracle, element by element on
+the same seeded inputs (-m gpu).  Sizes span several tiles and a ragged tail; the five
+BASELINE.json configs are covered in full or on sampled cells the oracle computes one by one."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from synth import Grid, make_workload, tiny_workload  # noqa: E402
+from tests.golden.load_golden import load  # noqa: E402
+from tests.parity import TOL_2F, check_cells, check_result  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+RECT, EXP = 0, 1
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import paper_1805_05652_b200 as p
+
+    p.load_library()  # fails loudly if libtfstat.so is missing: there is no fallback
+    assert torch.cuda.is_available()
+    return p
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def run_map(pkg, atoms, t, window, grid, **kw):
+    m, f = pkg.tfstat_map(dev(atoms), dev(t), window, grid, want_flags=True, **kw)
+    torch.cuda.synchronize()
+    return m.cpu().numpy(), f.cpu().numpy()
+
+
+# ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("wname,window", [("rect", RECT), ("exp", EXP)])
+def test_T0_toy(pkg, wname, window):
+    g = load("T0_toy.txt")
+    atoms = np.stack([g[k] for k in ("a2", "b2", "ab", "FaRe", "FaIm", "FbRe", "FbIm")]).astype(
+        np.float32)
+    t = g["t_atoms"].astype(np.int32)
+    grid = Grid(*(int(x) for x in g["grid_t0"]), *(int(x) for x in g["grid_tau"]))
+    m, f = run_map(pkg, atoms, t, window, grid)
+    np.testing.assert_allclose(m.ravel(), g[f"{wname}_2F"], rtol=2e-6, atol=2e-6)
+    assert np.array_equal((f.ravel() != 0).astype(int), g[f"{wname}_flagged"].astype(int))
+    r = pkg.tfstat_marginalise(dev(m), dev(f)).numpy()[0]
+    assert r["m"] * grid.N_tau + r["n"] == int(g[f"{wname}_argmax_flat"][0])
+    assert r["n_valid"] == int(g[f"{wname}_n_valid"][0])
+    assert abs(r["logB"] - g[f"{wname}_logB"][0]) < 1e-5
+    assert abs(r["max2F"] - g[f"{wname}_max2F"][0]) < 1e-5
+
+
+TINY = [
+    # seed, slots, gaps, grid                                    what it exercises
+    (101, 64, 0.0, Grid(0, 1800, 12, 3600, 1800, 10)),          # smallest tile shape
+    (102, 400, 0.2, Grid(0, 1800, 37, 3600, 1800, 300)),        # several n-blocks, ragged tails
+    (103, 300, 0.3, Grid(-5400, 2700, 45, 1800, 3100, 150)),    # off-lattice steps, before data
+    (104, 500, 0.1, Grid(400 * 1800, 900, 130, 7200, 7200, 70)),  # windows overrun the data end
+    (105, 2500, 0.15, Grid(0, 1800, 50, 43200, 1800, 700)),     # > 1 staging chunk of atoms
+    (106, 200, 0.1, Grid(0, 1801, 40, 3600, 1800, 1000)),       # gcd 1: per-cell binary search
+    (107, 120, 0.0, Grid(0, 1800, 1, 3600, 1800, 90)),          # N_t0 = 1
+    (108, 120, 0.0, Grid(0, 1800, 75, 7200, 1800, 1)),          # N_tau = 1
+]
+
+
+@pytest.mark.parametrize("window", [RECT, EXP])
+@pytest.mark.parametrize("seed,slots,gaps,grid", TINY)
+def test_tiny_maps(pkg, window, seed, slots, gaps, grid):
+    wl = tiny_workload(seed, slots, gaps, grid)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    ref = oracle.map2F(atoms, t, window, grid)
+    m, f = run_map(pkg, atoms, t, window, grid)
+    check_cells(m, f, ref, f"tiny{seed}")
+    assert pkg.count_terms(dev(t), window, grid) == int(ref["cnt"].sum())
+    r = pkg.tfstat_marginalise(dev(m), dev(f)).numpy()[0]
+    check_result(r, ref["twoF"], ref["flags"], grid.N_tau, f"tiny{seed} marginalise")
+
+
+@pytest.mark.parametrize("window", [RECT, EXP])
+def test_search_batched_small(pkg, window):
+    """Batched fused search == per-template map + marginalise == oracle; padded layout."""
+    grid = Grid(0, 1800, 23, 3600, 3600, 140)
+    wl = tiny_workload(201, 350, 0.1, grid, n_templates=7, phi_random=True)
+    T, _, N = wl.data.atoms.shape
+    ld, tstride = N + 5, 7 * (N + 5) + 11  # padded rows and templates
+    buf = torch.full((T * tstride,), float("nan"), dtype=torch.float32, device="cuda")
+    a = torch.as_strided(buf, (T, 7, N), (tstride, ld, 1))
+    a.copy_(dev(wl.data.atoms))
+    res = pkg.tfstat_search(a, dev(wl.data.t), window, grid, want_maps=True, want_flags=True)
+    torch.cuda.synchronize()
+    got = res.numpy()
+    for k in range(T):
+        ref = oracle.map2F(wl.data.atoms[k], wl.data.t, window, grid)
+        check_cells(res.maps[k].cpu().numpy(), res.flags[k].cpu().numpy(), ref, f"tpl{k}")
+        check_result(got[k], ref["twoF"], ref["flags"], grid.N_tau, f"tpl{k}")
+    # results-only call gives the same records
+    res2 = pkg.tfstat_search(a, dev(wl.data.t), window, grid)
+    assert np.array_equal(res2.numpy(), got)
+
+
+def test_search_host_equals_device(pkg):
+    grid = Grid(0, 1800, 16, 3600, 1800, 100)
+    wl = tiny_workload(202, 260, 0.05, grid, n_templates=9, phi_random=True)
+    a_h = torch.from_numpy(wl.data.atoms).pin_memory()
+    t_h = torch.from_numpy(wl.data.t).pin_memory()
+    for window in (EXP, RECT):
+        r_dev = pkg.tfstat_search(dev(wl.data.atoms), dev(wl.data.t), window, grid,
+                                  want_maps=True)
+        # small device budget: forces several chunks through the double-buffered copies
+        r_host, maps = pkg.tfstat_search_host(a_h, t_h, window, grid, want_maps=True,
+                                              max_device_bytes=3 * a_h[0].numel() * 4 * 2)
+        assert np.array_equal(r_host, r_dev.numpy())
+        assert np.array_equal(maps.numpy(), r_dev.maps.cpu().numpy())
+
+
+def test_degenerate_maps(pkg):
+    t = (np.arange(40) * 1800).astype(np.int32)
+    wl = tiny_workload(203, 40, 0.0, Grid(0, 1800, 2, 3600, 1800, 2))
+    atoms = wl.data.atoms[0]
+    for window in (RECT, EXP):
+        # every window lies after the data: all cells empty, not an error
+        g = Grid(10 ** 6, 1800, 5, 3600, 1800, 40)
+        res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, g, want_maps=True,
+                                want_flags=True)
+        r = res.numpy()[0]
+        assert (r["n_valid"], r["m"], r["n"], r["max2F"]) == (0, -1, -1, 0.0)
+        assert r["logB"] == -np.inf
+        assert torch.all(res.maps == 0) and torch.all(res.flags == 3)
+        # min_atoms is honoured
+        g2 = Grid(0, 1800, 6, 1800, 1800, 5)
+        for min_atoms in (1, 2, 4):
+            ref = oracle.map2F(atoms, t, window, g2, min_atoms=min_atoms)
+            m, f = run_map(pkg, atoms, t, window, g2, min_atoms=min_atoms)
+            check_cells(m, f, ref, f"min_atoms={min_atoms}")
+    # a single atom, single cell
+    m, f = run_map(pkg, atoms[:, :1].copy(), t[:1], RECT, Grid(0, 1, 1, 1800, 1, 1))
+    assert m[0, 0] == 0 and f[0, 0] & 1
+
+
+# ---------------------------------------------------------------------------------------
+# BASELINE.json configs
+# ---------------------------------------------------------------------------------------
+def test_config1_rect_full(pkg):
+    wl = make_workload(1)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    ref = oracle.map2F(atoms, t, RECT, wl.grid)
+    m, f = run_map(pkg, atoms, t, RECT, wl.grid)
+    check_cells(m, f, ref, "cfg1")
+    assert np.count_nonzero(f) == 24
+    r = pkg.tfstat_marginalise(dev(m), dev(f)).numpy()[0]
+    check_result(r, ref["twoF"], ref["flags"], wl.grid.N_tau, "cfg1")
+
+
+def test_config2_exp_full_map_and_injection(pkg):
+    wl = make_workload(2)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    ref = oracle.map2F(atoms, t, EXP, wl.grid)
+    m, f = run_map(pkg, atoms, t, EXP, wl.grid)
+    worst = check_cells(m, f, ref, "cfg2")
+    assert worst < 0.5  # comfortably inside the tolerance, not just scraping it
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), EXP, wl.grid)
+    check_result(res.numpy()[0], ref["twoF"], ref["flags"], wl.grid.N_tau, "cfg2")
+    (m_inj, n_inj, rho), = wl.injections.values()
+    assert abs(int(res.numpy()[0]["m"]) - m_inj) <= 6
+    assert pkg.count_terms(dev(t), EXP, wl.grid) == 436248960  # eq. (A.6)
+
+
+def _sample_cells(grid, n, seed):
+    rng = np.random.default_rng(seed)
+    ms = rng.integers(0, grid.N_t0, size=n)
+    ns = rng.integers(0, grid.N_tau, size=n)
+    # always include the corners and the first/last rows and columns' ends
+    ms[:4] = [0, 0, grid.N_t0 - 1, grid.N_t0 - 1]
+    ns[:4] = [0, grid.N_tau - 1, 0, grid.N_tau - 1]
+    return ms.astype(np.int32), ns.astype(np.int32)
+
+
+@pytest.mark.parametrize("window", [EXP, RECT])
+def test_config3_glitch_scale(pkg, window):
+    wl = make_workload(3)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    assert t.shape[0] == 4608
+    m, f = run_map(pkg, atoms, t, window, wl.grid)
+    if window == RECT:
+        ref = oracle.map2F(atoms, t, window, wl.grid)
+        check_cells(m, f, ref, "cfg3 rect")
+        res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, wl.grid)
+        check_result(res.numpy()[0], ref["twoF"], ref["flags"], wl.grid.N_tau, "cfg3 rect")
+    else:
+        ms, ns = _sample_cells(wl.grid, 30000, 3)
+        ref = oracle.cells(atoms, t, window, wl.grid, ms, ns)
+        check_cells(m[ms, ns], f[ms, ns], ref, "cfg3 exp sampled")
+        # fused marginals agree with marginalising the GPU's own full map in fp64
+        res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, wl.grid).numpy()[0]
+        _check_self_consistent(res, m, f, wl.grid)
+
+
+def _check_self_consistent(res, m, f, grid):
+    """Properties that hold at any size: fused marginals == fp64 marginals of the same map."""
+    mg = oracle.marginalise(m.astype(np.float64), f)
+    assert int(res["n_valid"]) == mg.n_valid
+    assert abs(res["max2F"] - mg.max2F) <= 1e-6 * max(1.0, mg.max2F)
+    assert (int(res["m"]), int(res["n"])) == (mg.m, mg.n)
+    assert abs(res["logB"] - mg.logB) <= 1e-4 * max(1.0, abs(mg.logB))
+
+
+def test_config4_batched_search_subset(pkg):
+    """8 templates of config 4 (2 with injections), full oracle maps."""
+    from synth.configs import cfg4_injection_plan
+
+    plan = cfg4_injection_plan()
+    inj = sorted(plan)[:2]
+    idx = sorted(set([0, 1, 2, 3, 4, 5] + inj))
+    wl = make_workload(4, templates=idx)
+    res = pkg.tfstat_search(dev(wl.data.atoms), dev(wl.data.t), EXP, wl.grid).numpy()
+    for j, k in enumerate(idx):
+        ref = oracle.map2F(wl.data.atoms[j], wl.data.t, EXP, wl.grid)
+        check_result(res[j], ref["twoF"], ref["flags"], wl.grid.N_tau, f"cfg4 tpl{k}")
+        if k in plan:
+            m_inj, n_inj, rho = plan[k]
+            assert res[j]["max2F"] >= ref["twoF"][m_inj, n_inj] * (1 - 2 * TOL_2F)
+            assert res[j]["max2F"] > 30.0  # rho = 8 stands out of chi^2_4 noise
+
+
+@pytest.mark.parametrize("window", [RECT, EXP])
+def test_config5_year_sampled(pkg, window):
+    wl = make_workload(5)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    assert t.shape[0] == 13140
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, wl.grid, want_maps=True,
+                            want_flags=True)
+    torch.cuda.synchronize()
+    m, f = res.maps[0].cpu().numpy(), res.flags[0].cpu().numpy()
+    ms, ns = _sample_cells(wl.grid, 20000 if window == EXP else 100000, 5)
+    ref = oracle.cells(atoms, t, window, wl.grid, ms, ns)
+    check_cells(m[ms, ns], f[ms, ns], ref, f"cfg5 w{window} sampled")
+    _check_self_consistent(res.numpy()[0], m, f, wl.grid)
+    # all cells the oracle says are count-degenerate on the last rows (end of data) are flagged
+    last = oracle.cells(atoms, t, window, wl.grid, np.full(720, wl.grid.N_t0 - 1, np.int32),
+                        np.arange(720, dtype=np.int32))
+    assert np.array_equal(f[-1] & 1, last["flags"] & 1)
