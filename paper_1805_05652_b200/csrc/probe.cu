@@ -9,7 +9,7 @@
 namespace {
 
 constexpr int kNT = 256;
-constexpr int kIters = 4096;
+constexpr int kIters = 4096;  // multiple of the unroll factor below
 constexpr int kChains = 16;
 
 template <int KIND>
@@ -38,8 +38,10 @@ __global__ void __launch_bounds__(kNT) probe_kernel(const float *__restrict__ in
     int sidx = threadIdx.x >> 5;
     float xu0 = -a, xu1 = -b;
 
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
     const long long c0 = clock64();
-#pragma unroll 1
+#pragma unroll 8
     for (int it = 0; it < kIters; ++it) {
         if (KIND == TFSTAT_PROBE_FFMA) {
 #pragma unroll
@@ -85,7 +87,12 @@ __global__ void __launch_bounds__(kNT) probe_kernel(const float *__restrict__ in
         r += __uint_as_float((unsigned)acc2[j]) + __uint_as_float((unsigned)(acc2[j] >> 32)) +
              (float)dacc[j];
     out[(size_t)blockIdx.x * kNT + threadIdx.x] = r + (float)sidx + xu0 + xu1;
-    if (blockIdx.x == 0 && threadIdx.x == 0) *cycles = c1 - c0;
+    // warps are not scheduled fairly, so one warp's elapsed clocks say nothing: take the span
+    // from the first start to the last end over every warp that ran on SM 0
+    if (smid == 0 && (threadIdx.x & 31) == 0) {
+        atomicMin(reinterpret_cast<unsigned long long *>(cycles), (unsigned long long)c0);
+        atomicMax(reinterpret_cast<unsigned long long *>(cycles) + 1, (unsigned long long)c1);
+    }
 }
 
 int ops_per_iter(int kind)
@@ -129,13 +136,15 @@ extern "C" int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s,
     do {
         if (cudaMalloc(&in, 2 * sizeof(float)) != cudaSuccess) break;
         if (cudaMalloc(&out, sizeof(float) * (size_t)grid * kNT) != cudaSuccess) break;
-        if (cudaMalloc(&cyc, sizeof(long long)) != cudaSuccess) break;
+        if (cudaMalloc(&cyc, 2 * sizeof(long long)) != cudaSuccess) break;
         const float h_in[2] = {kind == TFSTAT_PROBE_MUFU_EX2 ? -0.5f : 1.0000001f,
                                kind == TFSTAT_PROBE_LDS128 ? 0.0f : 1e-9f};
         if (cudaMemcpy(in, h_in, sizeof(h_in), cudaMemcpyHostToDevice) != cudaSuccess) break;
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
         float best_ms = 1e30f;
         for (int r = 0; r <= reps; ++r) {
+            const unsigned long long init[2] = {~0ull, 0ull};
+            cudaMemcpy(cyc, init, sizeof(init), cudaMemcpyHostToDevice);
             cudaEventRecord(e0);
             switch (kind) {
             case 0: launch<0>(grid, in, out, cyc); break;
@@ -154,8 +163,9 @@ extern "C" int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s,
             if (r > 0 && ms < best_ms) best_ms = ms;
         }
         if (cudaGetLastError() != cudaSuccess || best_ms > 1e29f) break;
-        long long h_cyc = 0;
-        if (cudaMemcpy(&h_cyc, cyc, sizeof(h_cyc), cudaMemcpyDeviceToHost) != cudaSuccess) break;
+        unsigned long long h_span[2] = {0, 0};
+        if (cudaMemcpy(h_span, cyc, sizeof(h_span), cudaMemcpyDeviceToHost) != cudaSuccess) break;
+        const long long h_cyc = (long long)(h_span[1] - h_span[0]);
         const double ops = (double)grid * kNT * (double)kIters * ops_per_iter(kind);
         *lane_ops_per_s = ops / (best_ms * 1e-3);
         if (ops_per_clk_sm)
