@@ -76,7 +76,9 @@ typedef struct tfstat_opts {
     int32_t min_atoms;  /* cells with fewer atoms are degenerate; 0 or unset -> 2
                            ("at least 2 SFTs per F_mn")                      */
     int32_t exp_method; /* TFSTAT_EXP_*                                                    */
-    int32_t reserved[2];
+    int32_t tile_c;     /* tuning: t0 cells per thread of the direct exp kernel (1,2,4,8);
+                           0 = chosen from the problem shape                               */
+    int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
     /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
      * immediately before and after the dominant kernel of the call (the window-sum +
      * closure kernel; for the rectangular window: prefix + cells kernels).  NULL = off. */

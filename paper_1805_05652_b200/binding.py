@@ -31,7 +31,7 @@ class TfstatError(RuntimeError):
 
 class _Opts(C.Structure):
     _fields_ = [("min_atoms", C.c_int32), ("exp_method", C.c_int32),
-                ("reserved", C.c_int32 * 2), ("ev_main_begin", C.c_void_p),
+                ("tile_c", C.c_int32), ("tile_nt", C.c_int32), ("ev_main_begin", C.c_void_p),
                 ("ev_main_end", C.c_void_p)]
 
 
@@ -85,10 +85,12 @@ def _grid_args(g):
     return [int(g.t0_min), int(g.dt0), int(g.N_t0), int(g.tau_min), int(g.dtau), int(g.N_tau)]
 
 
-def _opts(min_atoms: int, exp_method: int, events=None) -> _Opts:
+def _opts(min_atoms: int, exp_method: int, events=None, tile=None) -> _Opts:
     o = _Opts()
     o.min_atoms = int(min_atoms)
     o.exp_method = int(exp_method)
+    if tile is not None:  # (cells per thread, threads per CTA): tuning override
+        o.tile_c, o.tile_nt = int(tile[0]), int(tile[1])
     if events is not None:  # (begin, end): recorded torch.cuda.Event(enable_timing=True)
         o.ev_main_begin = int(events[0].cuda_event)
         o.ev_main_end = int(events[1].cuda_event)
@@ -115,9 +117,9 @@ def _dev_i32(x: torch.Tensor, name: str) -> torch.Tensor:
 
 
 def workspace_bytes(window: int, n_atoms: int, n_templates: int, grid, *, min_atoms: int = 2,
-                    exp_method: int = EXP_AUTO) -> int:
+                    exp_method: int = EXP_AUTO, tile=None) -> int:
     lib = load_library()
-    o = _opts(min_atoms, exp_method)
+    o = _opts(min_atoms, exp_method, tile=tile)
     n = lib.tfstat_workspace_bytes(window, n_atoms, n_templates, *_grid_args(grid), C.byref(o))
     if n == 0:
         raise TfstatError("tfstat_workspace_bytes: invalid problem shape")
@@ -155,7 +157,7 @@ class Results:
 def tfstat_map(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
                min_atoms: int = 2, exp_method: int = EXP_AUTO, want_flags: bool = False,
                out_map: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
-               stream=None):
+               stream=None, tile=None):
     """atoms [7, N] (row stride = ld) -> (map [N_t0, N_tau] fp32 of 2F, flags uint8 or None)."""
     lib = load_library()
     _dev_f32(atoms, "atoms")
@@ -170,9 +172,10 @@ def tfstat_map(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
         out_map = torch.empty((grid.N_t0, grid.N_tau), dtype=torch.float32, device=dev)
     flags = (torch.empty((grid.N_t0, grid.N_tau), dtype=torch.uint8, device=dev)
              if want_flags else None)
-    nbytes = workspace_bytes(window, n_atoms, 1, grid, min_atoms=min_atoms, exp_method=exp_method)
+    nbytes = workspace_bytes(window, n_atoms, 1, grid, min_atoms=min_atoms, exp_method=exp_method,
+                             tile=tile)
     ws = _workspace(nbytes, dev, workspace)
-    o = _opts(min_atoms, exp_method)
+    o = _opts(min_atoms, exp_method, tile=tile)
     rc = lib.tfstat_map(atoms.data_ptr(), ld, t_atoms.data_ptr(), n_atoms, window,
                         *_grid_args(grid), out_map.data_ptr(),
                         flags.data_ptr() if flags is not None else None, ws.data_ptr(), nbytes,
@@ -205,7 +208,7 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
                   min_atoms: int = 2, exp_method: int = EXP_AUTO, want_maps: bool = False,
                   want_flags: bool = False, workspace: Optional[torch.Tensor] = None,
                   out: Optional[torch.Tensor] = None, stream=None,
-                  main_kernel_events=None) -> Results:
+                  main_kernel_events=None, tile=None) -> Results:
     """atoms [T, 7, N] -> marginals of the T maps (and the maps / flags if asked)."""
     lib = load_library()
     _dev_f32(atoms, "atoms")
@@ -223,9 +226,10 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
             if want_maps else None)
     flags = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.uint8, device=dev)
              if want_flags else None)
-    nbytes = workspace_bytes(window, n_atoms, T, grid, min_atoms=min_atoms, exp_method=exp_method)
+    nbytes = workspace_bytes(window, n_atoms, T, grid, min_atoms=min_atoms, exp_method=exp_method,
+                             tile=tile)
     ws = _workspace(nbytes, dev, workspace)
-    o = _opts(min_atoms, exp_method, main_kernel_events)
+    o = _opts(min_atoms, exp_method, main_kernel_events, tile=tile)
     rc = lib.tfstat_search(atoms.data_ptr(), tstride, ld, t_atoms.data_ptr(), n_atoms, T, window,
                            *_grid_args(grid), out.data_ptr(),
                            maps.data_ptr() if maps is not None else None,

@@ -74,9 +74,21 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     // exp direct tile shape: largest tile that still yields a few waves of CTAs on 148 SMs
     const int64_t cells = (int64_t)N_t0 * N_tau;
     const int64_t total = cells * n_templates;
-    if (total >= (int64_t)8 * 256 * 148 * 4) pl.tile = ExpTile{8, 256};
-    else if (total >= (int64_t)4 * 128 * 148 * 4) pl.tile = ExpTile{4, 128};
-    else pl.tile = ExpTile{2, 64};
+    int C = total >= 300000 ? 8 : total >= 100000 ? 4 : 2;
+    // one weight per t0 tile (exp_direct.cu): the per-cell factor exp(-(c dt0)/tau) that the
+    // closure is invariant to must stay well inside fp32 range
+    while (C > 1 && (int64_t)(C - 1) * pl.grid.dt0 > (int64_t)8 * tau_min) C >>= 1;
+    pl.tile = ExpTile{C, (total / C) / 128 >= 148 * 8 ? 128 : 64};
+    if (opts && opts->tile_c) {
+        const int c = opts->tile_c;
+        if (c != 1 && c != 2 && c != 4 && c != 8 && c != 16) return pl;
+        pl.tile.C = c;
+    }
+    if (opts && opts->tile_nt) {
+        const int nt = opts->tile_nt;
+        if (nt != 32 && nt != 64 && nt != 128 && nt != 256) return pl;
+        pl.tile.NT = nt;
+    }
     pl.n_mtiles = (N_t0 + pl.tile.C - 1) / pl.tile.C;
     pl.n_nblocks = (N_tau + pl.tile.NT - 1) / pl.tile.NT;
     pl.tiles_per_template = (int64_t)pl.n_mtiles * pl.n_nblocks;
