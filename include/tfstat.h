@@ -48,9 +48,11 @@ extern "C" {
 #define TFSTAT_EXP_AUTO 0   /* = DIRECT */
 #define TFSTAT_EXP_DIRECT 1 /* truncated weighted sum per cell, the paper's
                                brute-force definition, register-tiled                     */
-#define TFSTAT_EXP_SCAN 2   /* exact factorised form: per-tau backward recurrence
-                               G_k = x_k + exp(-(t_{k+1}-t_k)/tau) G_{k+1}, window sum
-                               = G_lo - exp(-(t_hi-t_lo)/tau) G_hi */
+#define TFSTAT_EXP_SCAN 2   /* exact factorised, sliding form: per tau, weights
+                               E_a = exp(-(t_a - t_ref)/tau) shared by all t0 (the per-cell
+                               factor cancels in eq. 7); one initial window sum, then each
+                               t0 step adds the entering and subtracts the leaving atoms,
+                               backwards in t0 (csrc/exp_scan.cu)            */
 
 typedef enum tfstat_status {
     TFSTAT_OK = 0,
@@ -79,6 +81,8 @@ typedef struct tfstat_opts {
     int32_t tile_c;     /* tuning: t0 cells per thread of the direct exp kernel (1,2,4,8);
                            0 = chosen from the problem shape                               */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
+    int32_t seg_len;    /* tuning (TFSTAT_EXP_SCAN): t0 steps per sliding segment; 0 = auto   */
+    int32_t reserved;   /* must be 0                                                       */
     /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
      * immediately before and after the dominant kernel of the call (the window-sum +
      * closure kernel; for the rectangular window: prefix + cells kernels).  NULL = off. */

@@ -31,7 +31,8 @@ class TfstatError(RuntimeError):
 
 class _Opts(C.Structure):
     _fields_ = [("min_atoms", C.c_int32), ("exp_method", C.c_int32),
-                ("tile_c", C.c_int32), ("tile_nt", C.c_int32), ("ev_main_begin", C.c_void_p),
+                ("tile_c", C.c_int32), ("tile_nt", C.c_int32), ("seg_len", C.c_int32),
+                ("reserved", C.c_int32), ("ev_main_begin", C.c_void_p),
                 ("ev_main_end", C.c_void_p)]
 
 
@@ -89,8 +90,10 @@ def _opts(min_atoms: int, exp_method: int, events=None, tile=None) -> _Opts:
     o = _Opts()
     o.min_atoms = int(min_atoms)
     o.exp_method = int(exp_method)
-    if tile is not None:  # (cells per thread, threads per CTA): tuning override
+    if tile is not None:  # (cells per thread, threads per CTA[, t0 steps per segment]): tuning
         o.tile_c, o.tile_nt = int(tile[0]), int(tile[1])
+        if len(tile) > 2:
+            o.seg_len = int(tile[2])
     if events is not None:  # (begin, end): recorded torch.cuda.Event(enable_timing=True)
         o.ev_main_begin = int(events[0].cuda_event)
         o.ev_main_end = int(events[1].cuda_event)

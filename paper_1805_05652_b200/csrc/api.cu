@@ -95,7 +95,33 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     pl.cell_blocks_per_template = (int32_t)((cells + 255) / 256);
 
     const bool direct = window == TFSTAT_WINDOW_EXP && method == TFSTAT_EXP_DIRECT;
-    pl.partials_per_template = direct ? pl.tiles_per_template : pl.cell_blocks_per_template;
+    const bool slide = window == TFSTAT_WINDOW_EXP && method == TFSTAT_EXP_SCAN;
+    if (slide) {
+        // sliding form: one thread per tau, NT tau per CTA, t0 cut into segments only when
+        // (templates x tau blocks) alone cannot fill 148 SMs with ~16 warps each
+        int NT = 128;
+        const int64_t want_warps = 148 * 16;
+        while (NT > 32 && (int64_t)n_templates * ((N_tau + NT - 1) / NT) * (NT / 32) < want_warps)
+            NT >>= 1;
+        if (opts && opts->tile_nt) {
+            if (opts->tile_nt != 32 && opts->tile_nt != 64 && opts->tile_nt != 128) return pl;
+            NT = opts->tile_nt;
+        }
+        pl.tile.NT = NT;
+        pl.n_nblocks = (N_tau + NT - 1) / NT;
+        const int64_t warps = (int64_t)n_templates * pl.n_nblocks * (NT / 32);
+        int64_t segs = (want_warps + warps - 1) / warps;
+        const int64_t max_segs = (N_t0 + 31) / 32;  // a segment holds at least 32 t0 steps
+        if (segs > max_segs) segs = max_segs;
+        if (segs < 1) segs = 1;
+        int32_t len = (int32_t)((N_t0 + segs - 1) / segs);
+        if (opts && opts->seg_len > 0) len = opts->seg_len < N_t0 ? opts->seg_len : N_t0;
+        pl.seg_len = len;
+        pl.n_segs = (N_t0 + len - 1) / len;
+    }
+    pl.partials_per_template = direct  ? pl.tiles_per_template
+                               : slide ? (int64_t)pl.n_nblocks * pl.n_segs
+                                       : pl.cell_blocks_per_template;
     if (pl.partials_per_template * n_templates >= (int64_t(1) << 31)) return pl;
 
     size_t off = 0;
@@ -108,7 +134,6 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     pl.off_prefix = off;
     if (window == TFSTAT_WINDOW_RECT)
         off += align_up(sizeof(double) * 8 * ((size_t)n_atoms + 1) * n_templates);
-    pl.off_scan = off;
     pl.bytes = off;
     pl.status = TFSTAT_OK;
     return pl;
@@ -139,8 +164,7 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     } else if (pl.exp_method == TFSTAT_EXP_DIRECT) {
         TF_CUDA(launch_exp_direct(pl, pr, partials, st));
     } else {
-        float *scan_ws = reinterpret_cast<float *>(static_cast<char *>(ws) + pl.off_scan);
-        TF_CUDA(launch_exp_scan(pl, pr, scan_ws, partials, st));
+        TF_CUDA(launch_exp_scan(pl, pr, partials, st));
     }
     if (pl.ev_main_end) TF_CUDA(cudaEventRecord(pl.ev_main_end, st));
     if (out)

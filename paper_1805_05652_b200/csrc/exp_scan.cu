@@ -1,12 +1,248 @@
-// exp_scan.cu -- exact factorised exponential-window path (SURVEY.md 8(a) row a3').
-// Not implemented yet: the plan rejects nothing, the launcher reports it.
+// exp_scan.cu -- steps a0 + a3' + a4 + a5: the exponential window in its exact FACTORISED,
+// SLIDING form (SURVEY.md 8(a) row a3', BASELINE.json north_star "exact factorised form
+// exp(-(t-t0)/tau) = exp(t0/tau) exp(-t/tau) ... kept only if it matches the oracle").
+//
+// The paper sums every cell's window on its own ("brute-force grid").  But for a
+// fixed tau_n the weights of all t0 share one series:
+//     exp(-(t_a - t0_m)/tau) = exp(-(t_a - t_ref)/tau) * exp(-(t_ref - t0_m)/tau),
+// and eq. (7) is invariant under a per-cell rescaling of the window (A,B,C ~ k^2, Fa,Fb ~ k;
+// DESIGN.md invariant I3), so the per-cell factor never has to be applied.  With
+//     E_a = exp(-(t_a - t_ref)/tau)
+// the window sums of cell m are  W_m = sum_{a in [lo_m, hi_mn)} E_a x_a  (E_a^2 for a2,b2,ab),
+// and neighbouring cells differ by the few atoms that enter at the low end and leave at the
+// high end:
+//     W_{m-1} = W_m + sum_{[lo_{m-1}, lo_m)} E_a x_a - sum_{[hi_{m-1,n}, hi_{m,n})} E_a x_a.
+// One thread owns one tau_n and slides BACKWARDS in t0 (the stable direction: entering atoms
+// carry the largest weights of the window, leaving atoms the smallest, ~e^-3 of them, so the
+// subtraction never cancels the bulk of the sum).  Every weight is computed directly from its
+// time stamp (no multiplicative recurrence, hence no drift), an atom leaves with the same weight
+// it entered with, and t_ref is moved (accumulators rescaled by one exp) whenever
+// (t_ref - t0_m)/tau exceeds kReanchor so nothing overflows.  If a window loses most of its
+// weight (gaps, end of data) or does not overlap its neighbour, it is summed afresh.
+//
+// Work per (template, tau): |window of the last t0| + 2 atoms per t0 step, instead of
+// |window| atoms per cell: 60x fewer weighted terms on BASELINE.json config 4, 300x on
+// config 5.  Terms/s reported for this path are EFFECTIVE terms (eq. A.6 count / time).
+//
+// Layout: lanes of a warp hold consecutive tau_n (same template), so the initial window is
+// streamed through shared memory and broadcast exactly like exp_direct.cu; a CTA is
+// (template, block of NT tau, segment of t0).  Long t0 grids with few tau (config 5) are cut
+// into segments, each with its own initial sum, to fill the GPU.
 #include "plan.h"
 
 namespace tfstat {
 
-cudaError_t launch_exp_scan(const Plan &, const Problem &, float *, Partial *, cudaStream_t)
+namespace {
+
+constexpr float kReanchor = 4.0f;  // move t_ref when (t_ref - t0_m)/tau exceeds this
+constexpr float kGuard = 64.0f;    // re-sum a window whose A fell below 1/kGuard of its maximum
+
+struct SlideAcc {
+    u64 ab;  // (A, B)
+    u64 fa;  // (Re Fa, Im Fa)
+    u64 fb;  // (Re Fb, Im Fb)
+    float c;
+};
+
+__device__ __forceinline__ void acc_zero(SlideAcc &a)
 {
-    return cudaErrorNotSupported;
+    a.ab = a.fa = a.fb = 0ull;
+    a.c = 0.0f;
+}
+
+// acc += s * E x  (s = +1 entering, -1 leaving): w carries the sign, w2 = w * |w|
+__device__ __forceinline__ void acc_add(SlideAcc &a, const float w, const float w2, const u64 a2b2,
+                                        const float ab, const u64 fa, const u64 fb)
+{
+    const u64 ww = pack2(w, w);
+    ffma2(a.ab, pack2(w2, w2), a2b2);
+    ffma2(a.fa, ww, fa);
+    ffma2(a.fb, ww, fb);
+    a.c = fmaf(w2, ab, a.c);
+}
+
+// atom `al` straight from global memory (entering / leaving / re-summed atoms)
+__device__ __forceinline__ void acc_add_global(SlideAcc &a, const float *__restrict__ base,
+                                               const int64_t ld, const int32_t *__restrict__ t,
+                                               const int al, const long long t_ref,
+                                               const float kexp, const float sign)
+{
+    const float dt = (float)((long long)__ldg(t + al) - t_ref);
+    const float e = ex2_approx(dt * kexp);
+    const float w = sign * e;
+    acc_add(a, w, w * e, pack2(__ldg(base + al), __ldg(base + ld + al)), __ldg(base + 2 * ld + al),
+            pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al)),
+            pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al)));
+}
+
+__device__ __forceinline__ void acc_scale(SlideAcc &a, const float c)
+{
+    const float c2 = c * c;
+    a.ab = fmul2(a.ab, pack2(c2, c2));
+    a.fa = fmul2(a.fa, pack2(c, c));
+    a.fb = fmul2(a.fb, pack2(c, c));
+    a.c *= c2;
+}
+
+template <int NT, int KC>
+__global__ void __launch_bounds__(NT)
+    exp_slide_kernel(const Problem pr, Partial *__restrict__ partials, const int n_nblocks,
+                     const int n_segs, const int seg_len)
+{
+    __shared__ ulonglong2 s_a[KC];  // {(dt, ab), (a2, b2)}
+    __shared__ ulonglong2 s_b[KC];  // {(Re Fa, Im Fa), (Re Fb, Im Fb)}
+    __shared__ Marg s_red[32];
+
+    const Grid g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    // blockIdx.x = (tpl * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
+    const int j = (int)(blockIdx.x % n_nblocks);
+    const int seg = (int)((blockIdx.x / n_nblocks) % n_segs);
+    const int tpl = (int)(blockIdx.x / ((int64_t)n_nblocks * n_segs));
+    const int nb = n_nblocks - 1 - j;
+    const int n_first = nb * NT;
+    const int n_count = min(NT, g.N_tau - n_first);
+    const bool n_ok = (int)threadIdx.x < n_count;
+    const int n = n_first + (n_ok ? (int)threadIdx.x : 0);
+    const int m_beg = seg * seg_len;
+    const int m_end = min(m_beg + seg_len, g.N_t0);
+
+    const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+    const int64_t ld = pr.ld;
+    const double tau = (double)tau_of(g, n);
+    const float kexp = (float)(-1.4426950408889634 / tau);
+    const float inv_tau = (float)(1.0 / tau);
+
+    // ---- initial window: cell (m_end - 1, n), streamed through shared memory -----------------
+    int m = m_end - 1;
+    int lo_m = __ldg(bd.lo + m);
+    int hi = n_ok ? max(hi_index(bd, g, m, n), lo_m) : lo_m;
+    long long t_ref = t0_of(g, m);
+    const int cta_e = max(hi_index(bd, g, m, n_first + n_count - 1), lo_m);  // hi is monotone in n
+
+    SlideAcc acc;
+    acc_zero(acc);
+#pragma unroll 1
+    for (int cs = lo_m; cs < cta_e; cs += KC) {
+        const int n_stage = min(KC, cta_e - cs);
+        for (int i = threadIdx.x; i < n_stage; i += NT) {
+            const int al = cs + i;
+            const float dt = (float)((long long)__ldg(bd.t + al) - t_ref);
+            ulonglong2 ra, rb;
+            ra.x = pack2(dt, __ldg(base + 2 * ld + al));
+            ra.y = pack2(__ldg(base + al), __ldg(base + ld + al));
+            rb.x = pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al));
+            rb.y = pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al));
+            s_a[i] = ra;
+            s_b[i] = rb;
+        }
+        __syncthreads();
+        const int x1 = min(cs + n_stage, hi) - cs;
+#pragma unroll 4
+        for (int i = 0; i < x1; ++i) {
+            const ulonglong2 ra = s_a[i], rb = s_b[i];
+            float dt, ab;
+            unpack2(ra.x, dt, ab);
+            const float e = ex2_approx(dt * kexp);
+            acc_add(acc, e, e * e, ra.y, ab, rb.x, rb.y);
+        }
+        __syncthreads();
+    }
+    float A_max;
+    {
+        float A, B;
+        unpack2(acc.ab, A, B);
+        A_max = A;
+    }
+
+    // ---- slide backwards in t0: closure of cell m, then step to m - 1 ------------------------
+    Marg mg;
+    marg_init(mg);
+    const int64_t map_base = (int64_t)tpl * g.N_t0 * g.N_tau;
+#pragma unroll 1
+    for (;;) {
+        if (n_ok) {
+            Sums64 s;
+            float A, B, far, fai, fbr, fbi;
+            unpack2(acc.ab, A, B);
+            unpack2(acc.fa, far, fai);
+            unpack2(acc.fb, fbr, fbi);
+            s.A = A;
+            s.B = B;
+            s.C = acc.c;
+            s.far = far;
+            s.fai = fai;
+            s.fbr = fbr;
+            s.fbi = fbi;
+            uint32_t fl;
+            const float twoF = closure_2F(s, hi - lo_m, pr.min_atoms, fl);
+            const int32_t flat = m * g.N_tau + n;
+            if (pr.out_maps) pr.out_maps[map_base + flat] = twoF;
+            if (pr.out_flags) pr.out_flags[map_base + flat] = (uint8_t)fl;
+            if (!fl) marg_add(mg, twoF, flat);
+        }
+        if (m == m_beg) break;
+        const int m2 = m - 1;
+        const int lo2 = __ldg(bd.lo + m2);
+        const int hi2 = n_ok ? max(hi_index(bd, g, m2, n), lo2) : lo2;
+        const long long t0_2 = t0_of(g, m2);
+        bool fresh = (hi2 <= lo_m) || (hi2 == lo2);  // no overlap with window m, or empty
+        if (!fresh) {
+            const float sh = (float)(t_ref - t0_2);
+            if (sh * inv_tau > kReanchor) {  // keep the weights of entering atoms <= e^kReanchor
+                const float c = ex2_approx(sh * kexp);
+                acc_scale(acc, c);
+                A_max *= c * c;
+                t_ref = t0_2;
+            }
+            for (int al = lo2; al < lo_m; ++al)  // entering at the low end
+                acc_add_global(acc, base, ld, bd.t, al, t_ref, kexp, 1.0f);
+            for (int al = max(hi2, lo_m); al < hi; ++al)  // leaving at the high end
+                acc_add_global(acc, base, ld, bd.t, al, t_ref, kexp, -1.0f);
+            float A, B;
+            unpack2(acc.ab, A, B);
+            A_max = fmaxf(A_max, A);
+            fresh = A * kGuard < A_max;  // the window lost most of its weight: re-sum it
+        }
+        if (fresh) {
+            acc_zero(acc);
+            t_ref = t0_2;
+            for (int al = lo2; al < hi2; ++al)
+                acc_add_global(acc, base, ld, bd.t, al, t_ref, kexp, 1.0f);
+            float A, B;
+            unpack2(acc.ab, A, B);
+            A_max = A;
+        }
+        m = m2;
+        lo_m = lo2;
+        hi = hi2;
+    }
+    if (partials) {
+        marg_block_reduce<NT>(mg, s_red);
+        if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
+    }
+}
+
+template <int NT>
+cudaError_t launch_nt(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
+{
+    const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * pl.n_templates;
+    exp_slide_kernel<NT, 512><<<(unsigned)n_ctas, NT, 0, st>>>(pr, partials, pl.n_nblocks,
+                                                               pl.n_segs, pl.seg_len);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,
+                            cudaStream_t st)
+{
+    switch (pl.tile.NT) {
+    case 128: return launch_nt<128>(pl, pr, partials, st);
+    case 64: return launch_nt<64>(pl, pr, partials, st);
+    case 32: return launch_nt<32>(pl, pr, partials, st);
+    }
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace tfstat

@@ -44,12 +44,13 @@ struct Plan {
     ExpTile tile;
     int32_t n_mtiles, n_nblocks;
     int64_t tiles_per_template;
+    // exp sliding form (exp_scan.cu): t0 segments per (template, tau block)
+    int32_t n_segs, seg_len;
     // rect / marginalise tiling
     int32_t cell_blocks_per_template;
     // workspace layout (byte offsets)
-    size_t off_lo, off_edge, off_partials, off_prefix, off_scan, bytes;
+    size_t off_lo, off_edge, off_partials, off_prefix, bytes;
     int64_t partials_per_template;
-    int32_t scan_chunk_templates;
     cudaEvent_t ev_main_begin, ev_main_end;  // optional profiling hooks (tfstat_opts)
 };
 
@@ -65,8 +66,8 @@ cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partia
                               cudaStream_t st);
 cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, Partial *partials,
                         cudaStream_t st);
-cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, float *scan_ws,
-                            Partial *partials, cudaStream_t st);
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,
+                            cudaStream_t st);
 cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_template,
                             int32_t n_templates, int32_t N_tau, tfstat_result *out,
                             cudaStream_t st);

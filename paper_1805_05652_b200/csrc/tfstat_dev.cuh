@@ -113,6 +113,31 @@ __device__ __forceinline__ float ex2_approx(float x)
 
 #define TFSTAT_LOG2E_F 1.4426950408889634f
 
+// packed fp32x2 arithmetic (sm_100: SASS FFMA2 / FMUL2), two lanes of one 64-bit register
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 pack2(const float lo, const float hi)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(const u64 v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ void ffma2(u64 &d, const u64 a, const u64 b)
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ u64 fmul2(const u64 a, const u64 b)
+{
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+
 __device__ __forceinline__ void marg_init(Marg &a)
 {
     a.best = -INFINITY;

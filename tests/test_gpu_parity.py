@@ -242,3 +242,112 @@ def test_config5_year_sampled(pkg, window):
     last = oracle.cells(atoms, t, window, wl.grid, np.full(720, wl.grid.N_t0 - 1, np.int32),
                         np.arange(720, dtype=np.int32))
     assert np.array_equal(f[-1] & 1, last["flags"] & 1)
+
+
+# ---------------------------------------------------------------------------------------
+# exact factorised / sliding exponential path (SURVEY.md 8(a) row a3', TFSTAT_EXP_SCAN):
+# the same oracle, the same tolerances
+# ---------------------------------------------------------------------------------------
+SCAN = 2
+
+
+@pytest.mark.parametrize("seg_len", [0, 1, 7, 32])
+@pytest.mark.parametrize("seed,slots,gaps,grid", TINY)
+def test_tiny_maps_exp_scan(pkg, seed, slots, gaps, grid, seg_len):
+    wl = tiny_workload(seed, slots, gaps, grid)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    ref = oracle.map2F(atoms, t, EXP, grid)
+    m, f = run_map(pkg, atoms, t, EXP, grid, exp_method=SCAN, tile=(0, 0, seg_len))
+    check_cells(m, f, ref, f"scan tiny{seed} seg{seg_len}")
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), EXP, grid, exp_method=SCAN,
+                            tile=(0, 0, seg_len)).numpy()[0]
+    check_result(res, ref["twoF"], ref["flags"], grid.N_tau, f"scan tiny{seed} seg{seg_len}")
+
+
+def test_exp_scan_long_gaps_and_disjoint_windows(pkg):
+    """Windows that lose most of their atoms while sliding (long gaps), windows shorter than
+    the t0 step (no overlap between neighbours), tau >> data span, min_atoms variants."""
+    rng = np.random.default_rng(77)
+    slots = np.concatenate([np.arange(0, 40), np.arange(400, 420), np.arange(1000, 1300),
+                            np.arange(1302, 1304), np.arange(2500, 2600)])
+    t = (slots * 1800).astype(np.int32)
+    from synth import make_atoms
+    atoms = make_atoms(t, rng).astype(np.float32)
+    for grid in (Grid(0, 1800, 700, 3600, 5400, 60),          # slides through the long gaps
+                 Grid(0, 36000, 120, 1800, 1800, 12),          # 3 tau < dt0 for small tau: disjoint
+                 Grid(-90000, 1800, 300, 86400 * 50, 86400 * 25, 40),  # tau >> span, starts before data
+                 Grid(1000 * 1800, 900, 640, 1800, 900, 33)):  # half-slot steps
+        ref = oracle.map2F(atoms, t, EXP, grid)
+        for seg_len in (0, 50):
+            m, f = run_map(pkg, atoms, t, EXP, grid, exp_method=SCAN, tile=(0, 0, seg_len))
+            check_cells(m, f, ref, f"scan gaps {grid} seg{seg_len}")
+    g = Grid(0, 1800, 50, 1800, 1800, 20)
+    for min_atoms in (1, 3):
+        ref = oracle.map2F(atoms, t, EXP, g, min_atoms=min_atoms)
+        m, f = run_map(pkg, atoms, t, EXP, g, exp_method=SCAN, min_atoms=min_atoms)
+        check_cells(m, f, ref, f"scan min_atoms={min_atoms}")
+
+
+def test_exp_scan_batched_equals_oracle_and_direct(pkg):
+    grid = Grid(0, 1800, 23, 3600, 3600, 140)
+    wl = tiny_workload(201, 350, 0.1, grid, n_templates=7, phi_random=True)
+    a, t = dev(wl.data.atoms), dev(wl.data.t)
+    res = pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, want_maps=True, want_flags=True)
+    direct = pkg.tfstat_search(a, t, EXP, grid, exp_method=1, want_flags=True)
+    torch.cuda.synchronize()
+    assert torch.equal(res.flags, direct.flags)
+    got = res.numpy()
+    for k in range(wl.n_templates):
+        ref = oracle.map2F(wl.data.atoms[k], wl.data.t, EXP, grid)
+        check_cells(res.maps[k].cpu().numpy(), res.flags[k].cpu().numpy(), ref, f"scan tpl{k}")
+        check_result(got[k], ref["twoF"], ref["flags"], grid.N_tau, f"scan tpl{k}")
+
+
+def test_exp_scan_config2_full(pkg):
+    wl = make_workload(2)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    ref = oracle.map2F(atoms, t, EXP, wl.grid)
+    m, f = run_map(pkg, atoms, t, EXP, wl.grid, exp_method=SCAN)
+    worst = check_cells(m, f, ref, "scan cfg2")
+    assert worst < 0.5
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), EXP, wl.grid, exp_method=SCAN)
+    check_result(res.numpy()[0], ref["twoF"], ref["flags"], wl.grid.N_tau, "scan cfg2")
+
+
+def test_exp_scan_config3_sampled(pkg):
+    wl = make_workload(3)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    m, f = run_map(pkg, atoms, t, EXP, wl.grid, exp_method=SCAN)
+    ms, ns = _sample_cells(wl.grid, 30000, 3)
+    ref = oracle.cells(atoms, t, EXP, wl.grid, ms, ns)
+    worst = check_cells(m[ms, ns], f[ms, ns], ref, "scan cfg3 sampled")
+    assert worst < 0.5
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), EXP, wl.grid, exp_method=SCAN).numpy()[0]
+    _check_self_consistent(res, m, f, wl.grid)
+
+
+def test_exp_scan_config4_subset(pkg):
+    from synth.configs import cfg4_injection_plan
+
+    plan = cfg4_injection_plan()
+    idx = sorted(set([0, 1, 2, 3] + sorted(plan)[:2]))
+    wl = make_workload(4, templates=idx)
+    res = pkg.tfstat_search(dev(wl.data.atoms), dev(wl.data.t), EXP, wl.grid,
+                            exp_method=SCAN).numpy()
+    for j, k in enumerate(idx):
+        ref = oracle.map2F(wl.data.atoms[j], wl.data.t, EXP, wl.grid)
+        check_result(res[j], ref["twoF"], ref["flags"], wl.grid.N_tau, f"scan cfg4 tpl{k}")
+
+
+def test_exp_scan_config5_sampled(pkg):
+    wl = make_workload(5)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), EXP, wl.grid, exp_method=SCAN,
+                            want_maps=True, want_flags=True)
+    torch.cuda.synchronize()
+    m, f = res.maps[0].cpu().numpy(), res.flags[0].cpu().numpy()
+    ms, ns = _sample_cells(wl.grid, 20000, 55)
+    ref = oracle.cells(atoms, t, EXP, wl.grid, ms, ns)
+    worst = check_cells(m[ms, ns], f[ms, ns], ref, "scan cfg5 sampled")
+    assert worst < 0.5
+    _check_self_consistent(res.numpy()[0], m, f, wl.grid)
