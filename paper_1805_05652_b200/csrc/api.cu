@@ -119,9 +119,13 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         pl.seg_len = len;
         pl.n_segs = (N_t0 + len - 1) / len;
     }
+    if (window == TFSTAT_WINDOW_RECT)
+        pl.rect = plan_rect_run(pl.grid, pl.e_m, pl.e_n, pl.J, n_templates);
     pl.partials_per_template = direct  ? pl.tiles_per_template
                                : slide ? (int64_t)pl.n_nblocks * pl.n_segs
-                                       : pl.cell_blocks_per_template;
+                               : pl.rect.enabled
+                                   ? (int64_t)pl.rect.n_rowtiles * pl.rect.n_coltiles
+                                   : pl.cell_blocks_per_template;
     if (pl.partials_per_template * n_templates >= (int64_t(1) << 31)) return pl;
 
     size_t off = 0;
@@ -134,6 +138,12 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     pl.off_prefix = off;
     if (window == TFSTAT_WINDOW_RECT)
         off += align_up(sizeof(double) * 8 * ((size_t)n_atoms + 1) * n_templates);
+    pl.off_tot = off;
+    if (window == TFSTAT_WINDOW_RECT)
+        off += align_up(sizeof(double) * 8 * (size_t)rect_scan_blocks(n_atoms) * n_templates);
+    pl.off_steps = off;
+    if (window == TFSTAT_WINDOW_RECT && pl.rect.enabled)
+        off += align_up((size_t)32 * (size_t)(pl.J + 1) * n_templates);
     pl.bytes = off;
     pl.status = TFSTAT_OK;
     return pl;
@@ -160,7 +170,9 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     if (pl.ev_main_begin) TF_CUDA(cudaEventRecord(pl.ev_main_begin, st));
     if (pl.window == TFSTAT_WINDOW_RECT) {
         double *prefix = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_prefix);
-        TF_CUDA(launch_rect(pl, pr, prefix, partials, st));
+        double *tot = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_tot);
+        TF_CUDA(launch_rect(pl, pr, prefix, tot, static_cast<char *>(ws) + pl.off_steps, partials,
+                            st));
     } else if (pl.exp_method == TFSTAT_EXP_DIRECT) {
         TF_CUDA(launch_exp_direct(pl, pr, partials, st));
     } else {

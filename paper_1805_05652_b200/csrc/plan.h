@@ -30,6 +30,13 @@ struct ExpTile {
     int NT;
 };
 
+// rect running-sum kernel (rect.cu): a thread owns Q rows m, m+r, ..; a CTA owns NTu threads
+// (Q NTu rows) x seg_cols columns
+struct RectRun {
+    int32_t enabled;  // 0: per-cell kernel (no edge lattice / very few rows)
+    int32_t Q, r, NTu, seg_cols, n_rowtiles, n_coltiles;
+};
+
 struct Plan {
     int status;  // TFSTAT_OK or error
     int window;
@@ -48,8 +55,9 @@ struct Plan {
     int32_t n_segs, seg_len;
     // rect / marginalise tiling
     int32_t cell_blocks_per_template;
+    RectRun rect;
     // workspace layout (byte offsets)
-    size_t off_lo, off_edge, off_partials, off_prefix, bytes;
+    size_t off_lo, off_edge, off_partials, off_prefix, off_tot, off_steps, bytes;
     int64_t partials_per_template;
     cudaEvent_t ev_main_begin, ev_main_end;  // optional profiling hooks (tfstat_opts)
 };
@@ -64,8 +72,10 @@ cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_ter
                                cudaStream_t st);
 cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,
                               cudaStream_t st);
-cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, Partial *partials,
-                        cudaStream_t st);
+RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates);
+int rect_scan_blocks(int32_t n_atoms);
+cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *tot,
+                        void *steps, Partial *partials, cudaStream_t st);
 cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,
                             cudaStream_t st);
 cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_template,

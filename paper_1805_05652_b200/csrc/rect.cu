@@ -1,77 +1,160 @@
 // rect.cu -- steps a2 + a4 + a5 for the rectangular window (eq. 3).
 //
-// The paper keeps running partial sums over tau per t0 (N_t0 workers).  Here every
-// cell is independent: S(m,n) = P[hi(m,n)] - P[lo(m)] with P the exclusive prefix sums of the
-// 7 atom channels.  P is kept in fp64: an fp32 prefix over a year of atoms cancels
-// catastrophically for short windows far from the origin, fp64 differences of
-// fp32 data are exact to ~1e-13.  The closure (eq. 7) runs in fp64 on those differences.
+// The paper keeps running partial sums over tau per t0 with N_t0 workers.  Here:
+//
+//  1. rect_totals_kernel + rect_prefix_kernel: exclusive prefix sums P of the 7 atom channels in
+//     fp64, 1024 atoms per CTA (block totals first, then block scans) (an fp32 prefix
+//     over a year of atoms cancels catastrophically for short windows far from the origin,
+//     SURVEY.md H1; fp64 differences of fp32 data are exact to ~1e-13).
+//  2. rect_steps_kernel: every window end t0_m + tau_n lies on the edge lattice (bounds.cu), so
+//     the atoms that ENTER a window when tau grows by one grid step are the same for every cell
+//     with the same lattice point j:  G[j] = P[edge[j + e_n]] - P[edge[j]], rounded once to
+//     fp32 (a sum of a few atoms: exact to 2^-24 of its own size), 32 bytes per lattice point.
+//  3. rect_run_kernel: one thread walks one t0 row along tau.  It starts each column tile from
+//     the exact window sum P[hi] - P[lo] and then only ADDS G steps -- the paper's running sum,
+//     but with pre-aggregated steps, so a cell costs 4 packed fp32 adds + the closure.  Rows
+//     m, m+r, m+2r, m+3r (r = k dtau / dt0) use the same G entries one column later, so a thread
+//     owns those Q = 4 rows and keeps a sliding register window of G: 8 bytes of L1 traffic per
+//     cell.  The closure (eq. 7) runs in fp32 when the cell is well conditioned
+//     (D > AB/64, error <= ~1e-4 relative); other cells are recomputed in fp64 from P.
+//     2F values are transposed through shared memory (thread = row, but the map is tau-fastest)
+//     and leave as 64-byte row segments.
+//
+// Grids without an edge lattice (J = 0) or with very few t0 rows use the per-cell kernel
+// rect_cells_kernel: S(m,n) = P[hi(m,n)] - P[lo(m)], closure in fp64.
 #include "plan.h"
 
 namespace tfstat {
 
 namespace {
 
-constexpr int kPrefixNT = 1024;
+constexpr int kScanNT = 256;
+constexpr int kScanPer = 4;                       // atoms per thread
+constexpr int kScanBlock = kScanNT * kScanPer;    // atoms per CTA
 
-// P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.
-__global__ void __launch_bounds__(kPrefixNT)
-    rect_prefix_kernel(const Problem pr, double *__restrict__ prefix)
+// Pass 1: per-block totals of the 7 channels, tot[tpl][blk][8] (fp64).
+__global__ void __launch_bounds__(kScanNT)
+    rect_totals_kernel(const Problem pr, double *__restrict__ tot, const int nblk)
 {
-    __shared__ double s_warp[7][32];
-    const int tpl = blockIdx.x;
+    __shared__ double s_w[kScanNT / 32][8];
+    const int tpl = blockIdx.x / nblk, blk = blockIdx.x % nblk;
+    const int N = pr.bounds.n_atoms;
+    const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+    const int a0 = blk * kScanBlock + (int)threadIdx.x * kScanPer;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double v[7];
+#pragma unroll
+    for (int ch = 0; ch < 7; ++ch) {
+        float x[kScanPer];
+#pragma unroll
+        for (int i = 0; i < kScanPer; ++i)
+            x[i] = (a0 + i < N) ? __ldg(base + ch * pr.ld + a0 + i) : 0.0f;
+        double sacc = 0.0;
+#pragma unroll
+        for (int i = 0; i < kScanPer; ++i) sacc += (double)x[i];
+        v[ch] = sacc;
+    }
+#pragma unroll
+    for (int ch = 0; ch < 7; ++ch) {
+#pragma unroll
+        for (int sh = 16; sh >= 1; sh >>= 1) v[ch] += __shfl_xor_sync(0xffffffffu, v[ch], sh);
+        if (lane == 0) s_w[warp][ch] = v[ch];
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        double t = 0.0;
+        if (threadIdx.x < 7)
+            for (int w = 0; w < kScanNT / 32; ++w) t += s_w[w][threadIdx.x];
+        tot[(int64_t)blockIdx.x * 8 + threadIdx.x] = t;
+    }
+}
+
+// Pass 2: P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.  Each block adds
+// the totals of the blocks before it to the scan of its own kScanBlock atoms.
+__global__ void __launch_bounds__(kScanNT)
+    rect_prefix_kernel(const Problem pr, const double *__restrict__ tot,
+                       double *__restrict__ prefix, const int nblk)
+{
+    __shared__ double s_off[8];
+    __shared__ double s_w[7][kScanNT / 32];
+    const int tpl = blockIdx.x / nblk, blk = blockIdx.x % nblk;
     const int N = pr.bounds.n_atoms;
     const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
     double *__restrict__ P = prefix + (int64_t)tpl * (N + 1) * 8;
-    const int seg = (N + kPrefixNT - 1) / kPrefixNT;
-    const int a0 = min((int)threadIdx.x * seg, N), a1 = min(a0 + seg, N);
+    const int a0 = blk * kScanBlock + (int)threadIdx.x * kScanPer;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    double tot[7];
+    float x[7][kScanPer];
 #pragma unroll
-    for (int ch = 0; ch < 7; ++ch) {
-        double s = 0.0;
-        for (int al = a0; al < a1; ++al) s += (double)__ldg(base + ch * pr.ld + al);
-        tot[ch] = s;
+    for (int ch = 0; ch < 7; ++ch)
+#pragma unroll
+        for (int i = 0; i < kScanPer; ++i)
+            x[ch][i] = (a0 + i < N) ? __ldg(base + ch * pr.ld + a0 + i) : 0.0f;
+
+    // offset of this block: warp ch sums tot[tpl][0..blk)[ch]
+    if (warp < 7) {
+        double t = 0.0;
+        for (int b = lane; b < blk; b += 32) t += __ldg(tot + ((int64_t)tpl * nblk + b) * 8 + warp);
+#pragma unroll
+        for (int sh = 16; sh >= 1; sh >>= 1) t += __shfl_xor_sync(0xffffffffu, t, sh);
+        if (lane == 0) s_off[warp] = t;
     }
-    // inclusive scan of the per-thread totals across the block
-    double incl[7];
+
+    double incl[7], tsum[7];
 #pragma unroll
     for (int ch = 0; ch < 7; ++ch) {
-        double v = tot[ch];
+        double t = 0.0;
 #pragma unroll
-        for (int s = 1; s < 32; s <<= 1) {
-            const double u = __shfl_up_sync(0xffffffffu, v, s);
-            if (lane >= s) v += u;
+        for (int i = 0; i < kScanPer; ++i) t += (double)x[ch][i];
+        tsum[ch] = t;
+#pragma unroll
+        for (int sh = 1; sh < 32; sh <<= 1) {
+            const double up = __shfl_up_sync(0xffffffffu, t, sh);
+            if (lane >= sh) t += up;
         }
-        incl[ch] = v;
-        if (lane == 31) s_warp[ch][warp] = v;
+        incl[ch] = t;
+        if (lane == 31) s_w[ch][warp] = t;
     }
     __syncthreads();
-    if (warp == 0) {
+    if (threadIdx.x == 0 && blk == 0) {
 #pragma unroll
-        for (int ch = 0; ch < 7; ++ch) {
-            double v = s_warp[ch][lane];
-#pragma unroll
-            for (int s = 1; s < 32; s <<= 1) {
-                const double u = __shfl_up_sync(0xffffffffu, v, s);
-                if (lane >= s) v += u;
-            }
-            s_warp[ch][lane] = v;
-        }
+        for (int ch = 0; ch < 8; ++ch) P[ch] = 0.0;
     }
-    __syncthreads();
 #pragma unroll
     for (int ch = 0; ch < 7; ++ch) {
-        double run = incl[ch] - tot[ch] + (warp > 0 ? s_warp[ch][warp - 1] : 0.0);
-        for (int al = a0; al < a1; ++al) {
-            run += (double)__ldg(base + ch * pr.ld + al);
-            P[(int64_t)(al + 1) * 8 + ch] = run;
-            if (ch == 6) P[(int64_t)(al + 1) * 8 + 7] = 0.0;  // pad lane of the 64-B entry
+        double run = s_off[ch] + incl[ch] - tsum[ch];
+        for (int w = 0; w < warp; ++w) run += s_w[ch][w];
+#pragma unroll
+        for (int i = 0; i < kScanPer; ++i) {
+            run += (double)x[ch][i];
+            if (a0 + i < N) P[(int64_t)(a0 + i + 1) * 8 + ch] = run;
         }
     }
-    if (threadIdx.x < 8) P[threadIdx.x] = 0.0;
+    // pad lane of the 64-B entries stays unwritten: nothing reads it
 }
 
+// window sums of atoms [lo, hi) from the prefix, in fp64
+__device__ __forceinline__ Sums64 prefix_diff(const double2 *__restrict__ P, const int lo,
+                                              const int hi)
+{
+    const double2 l0 = __ldg(P + (int64_t)lo * 4), l1 = __ldg(P + (int64_t)lo * 4 + 1),
+                  l2 = __ldg(P + (int64_t)lo * 4 + 2), l3 = __ldg(P + (int64_t)lo * 4 + 3);
+    const double2 h0 = __ldg(P + (int64_t)hi * 4), h1 = __ldg(P + (int64_t)hi * 4 + 1),
+                  h2 = __ldg(P + (int64_t)hi * 4 + 2), h3 = __ldg(P + (int64_t)hi * 4 + 3);
+    Sums64 s;
+    s.A = h0.x - l0.x;
+    s.B = h0.y - l0.y;
+    s.C = h1.x - l1.x;
+    s.far = h1.y - l1.y;
+    s.fai = h2.x - l2.x;
+    s.fbr = h2.y - l2.y;
+    s.fbi = h3.x - l3.x;
+    return s;
+}
+
+// ---------------------------------------------------------------------------------------
+// generic per-cell kernel (no edge lattice / very few t0 rows)
+// ---------------------------------------------------------------------------------------
 constexpr int kCellNT = 256;
 
 __global__ void __launch_bounds__(kCellNT)
@@ -93,18 +176,7 @@ __global__ void __launch_bounds__(kCellNT)
         const int hi = max(hi_index(bd, g, m, n), lo);
         const double2 *__restrict__ P = reinterpret_cast<const double2 *>(
             prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
-        const double2 l0 = __ldg(P + (int64_t)lo * 4), l1 = __ldg(P + (int64_t)lo * 4 + 1),
-                      l2 = __ldg(P + (int64_t)lo * 4 + 2), l3 = __ldg(P + (int64_t)lo * 4 + 3);
-        const double2 h0 = __ldg(P + (int64_t)hi * 4), h1 = __ldg(P + (int64_t)hi * 4 + 1),
-                      h2 = __ldg(P + (int64_t)hi * 4 + 2), h3 = __ldg(P + (int64_t)hi * 4 + 3);
-        Sums64 s;
-        s.A = h0.x - l0.x;
-        s.B = h0.y - l0.y;
-        s.C = h1.x - l1.x;
-        s.far = h1.y - l1.y;
-        s.fai = h2.x - l2.x;
-        s.fbr = h2.y - l2.y;
-        s.fbi = h3.x - l3.x;
+        const Sums64 s = prefix_diff(P, lo, hi);
         uint32_t fl;
         const float twoF = closure_2F(s, hi - lo, pr.min_atoms, fl);
         const int64_t o = (int64_t)tpl * n_cells + i;
@@ -118,18 +190,500 @@ __global__ void __launch_bounds__(kCellNT)
     }
 }
 
+// The running Fa, Fb sums are carried scaled by sqrt(2), so eq. (7) on them yields 2F directly.
+constexpr double kSqrt2 = 1.41421356237309504880;
+
+// ---------------------------------------------------------------------------------------
+// lattice steps G[tpl][j], j = 0..J, 32 bytes each:
+//   {(A, B), (Re Fa, Re Fb)}, {(Im Fa, Im Fb), (C, count)}
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+    rect_steps_kernel(const Problem pr, const double *__restrict__ prefix,
+                      ulonglong2 *__restrict__ G, const int blocks_per_template)
+{
+    const Bounds &bd = pr.bounds;
+    const int tpl = blockIdx.x / blocks_per_template;
+    const int j = (blockIdx.x % blocks_per_template) * 256 + threadIdx.x;
+    if (j > bd.J) return;  // entry J is the all-zero entry out-of-range reads are clamped to
+    const int j2 = j + bd.e_n;
+    ulonglong2 ga = make_ulonglong2(0ull, 0ull), gb = make_ulonglong2(0ull, 0ull);
+    if (j2 < bd.J) {
+        const int a = __ldg(bd.edge + j), b = __ldg(bd.edge + j2);
+        const double2 *__restrict__ P = reinterpret_cast<const double2 *>(
+            prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
+        const Sums64 s = prefix_diff(P, a, b);
+        ga.x = pack2((float)s.A, (float)s.B);
+        ga.y = pack2((float)(kSqrt2 * s.far), (float)(kSqrt2 * s.fbr));  // see rect_run_kernel
+        gb.x = pack2((float)(kSqrt2 * s.fai), (float)(kSqrt2 * s.fbi));
+        gb.y = pack2((float)s.C, (float)(b - a));
+    }
+    ulonglong2 *__restrict__ o = G + ((int64_t)tpl * (bd.J + 1) + j) * 2;
+    o[0] = ga;
+    o[1] = gb;
+}
+
+// ---------------------------------------------------------------------------------------
+// running-sum kernel
+// ---------------------------------------------------------------------------------------
+constexpr int kRunNT = 128;
+constexpr int kChunk = 16;   // columns between two write-outs of the transposed tile
+constexpr int kPitch = 20;   // floats per tile row: conflict-free STS.128 and aligned LDS.128
+constexpr int kFPitch = 5;   // 32-bit words per flag-tile row (16 flag bytes + pad)
+constexpr float kCondFast = 1.0f / 64.0f;  // fp32 closure only if D > kCondFast * A * B
+constexpr float kHalfLog2e = 0.72134752044448170368f;
+
+__device__ __forceinline__ u64 fadd2(const u64 a, const u64 b)
+{
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+__device__ __forceinline__ float rcp_approx(const float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ill-conditioned, short or empty cell (m, n): the plain way, in fp64 straight from the prefix.
+// Returns (2F, flags) packed in one 64-bit register.
+__device__ __noinline__ u64 rect_cell_slow(const double2 *__restrict__ P,
+                                           const int32_t *__restrict__ lo_tab,
+                                           const int32_t *__restrict__ edge, const int m,
+                                           const int64_t j, const int min_atoms)
+{
+    const int lo = __ldg(lo_tab + m);
+    const int hi = max(__ldg(edge + j), lo);
+    const Sums64 s = prefix_diff(P, lo, hi);
+    uint32_t f;
+    const float twoF = closure_2F(s, hi - lo, min_atoms, f);
+    return pack2(twoF, __uint_as_float(f));
+}
+
+struct RunMarg {
+    float best;   // max 2F
+    int32_t idx;  // its flat index
+    float ref2;   // reference exponent (log2 units) of the running sum
+    float sum;    // sum 2^(F log2e - ref2)
+    int32_t nv;
+};
+
+// generic per-cell update (groups with flagged cells, ragged tails, rows outside the grid)
+__device__ __noinline__ void run_marg_add(RunMarg &a, const float twoF, const int32_t flat)
+{
+    if (twoF > a.best || (twoF == a.best && flat < a.idx)) {
+        a.best = twoF;
+        a.idx = flat;
+    }
+    float d = fmaf(twoF, kHalfLog2e, -a.ref2);
+    if (d > 60.0f) {  // move the reference up (first cell: ref2 = -inf, sum = 0)
+        a.sum *= ex2_approx(-d);
+        a.ref2 = twoF * kHalfLog2e;
+        d = 0.0f;
+    }
+    a.sum += ex2_approx(d);
+    a.nv += 1;
+}
+
+template <int Q, bool MARG>
+__global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : 5)
+    rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
+                    const ulonglong2 *__restrict__ G, Partial *__restrict__ partials, const int r, const int NTu,
+                    const int seg_cols, const int n_rowtiles, const int n_coltiles,
+                    const int vec_ok)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ Marg s_red[32];
+    const int nrows = Q * NTu;
+    float *tile = reinterpret_cast<float *>(smem_raw);                 // [nrows][kPitch]
+    int *s_rowm = reinterpret_cast<int *>(tile + (size_t)nrows * kPitch);  // [nrows]
+    uint32_t *ftile = reinterpret_cast<uint32_t *>(s_rowm + nrows);   // [nrows][kFPitch]
+
+    const Grid g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    const int rowtile = blockIdx.x % n_rowtiles;
+    const int coltile = (blockIdx.x / n_rowtiles) % n_coltiles;
+    const int tpl = blockIdx.x / (n_rowtiles * n_coltiles);
+    const int lt = threadIdx.x;
+    const bool active = lt < NTu;
+    const int u = rowtile * NTu + min(lt, NTu - 1);
+    int mbase = u;
+    if (Q > 1) {
+        const int grp = u / r;
+        mbase = grp * r * Q + (u - grp * r);
+    }
+    const int n0 = coltile * seg_cols;
+    const int n_end = min(n0 + seg_cols, g.N_tau);
+    const double2 *__restrict__ P =
+        reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
+    const ulonglong2 *__restrict__ g_t = G + (int64_t)tpl * (bd.J + 1) * 2;
+    const float min_atoms_f = (float)pr.min_atoms;
+
+    // ---- exact start of every row at column n0 ----------------------------------------------
+    // Rows outside the grid (and the idle lanes of the last warp) carry a dummy, perfectly
+    // conditioned state so that they stay on the fast path; nothing of theirs is stored.
+    u64 S[Q][4];
+    bool rvalid[Q];
+    bool all_valid = true;
+    int n_valid_rows = 0;
+    const bool want_map = pr.out_maps != nullptr, want_flags = pr.out_flags != nullptr;
+    const int64_t map_base = (int64_t)tpl * g.N_t0 * g.N_tau;
+#pragma unroll
+    for (int b = 0; b < Q; ++b) {
+        const int m = mbase + b * r;
+        bool valid = active && m < g.N_t0;
+        const int mc = min(m, g.N_t0 - 1);
+        const int lo = __ldg(bd.lo + mc);
+        const int64_t j0 = (int64_t)mc * bd.e_m + (int64_t)n0 * bd.e_n;
+        const int hi = max(__ldg(bd.edge + j0), lo);
+        // A row whose window still holds at most one atom (fewer than min_atoms) at the LAST
+        // column of this tile is degenerate throughout: its cells are written here, directly,
+        // and the row then runs as a dummy (rows at the end of the data or inside long gaps
+        // would otherwise send every one of their cells through the fp64 path).
+        const int cnt_end =
+            max(__ldg(bd.edge + j0 + (int64_t)(n_end - 1 - n0) * bd.e_n), lo) - lo;
+        if (valid && cnt_end <= 1 && cnt_end < pr.min_atoms) {
+            uint32_t f1 = 3u;  // flags of a single-atom cell: bit 1 from the atom's own D in fp64
+            if (cnt_end == 1) {
+                const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+                const double a2 = (double)__ldg(base + lo), b2 = (double)__ldg(base + pr.ld + lo),
+                             ab = (double)__ldg(base + 2 * pr.ld + lo);
+                f1 = 1u | ((a2 * b2 - ab * ab > 0.0) ? 0u : 2u);
+            }
+            for (int n = n0; n < n_end; ++n) {
+                const int64_t o = map_base + (int64_t)m * g.N_tau + n;
+                if (want_map) pr.out_maps[o] = 0.0f;
+                if (want_flags) {
+                    const int c =
+                        max(__ldg(bd.edge + j0 + (int64_t)(n - n0) * bd.e_n), lo) - lo;
+                    pr.out_flags[o] = (uint8_t)(c == 0 ? 3u : f1);
+                }
+            }
+            valid = false;
+        }
+        const Sums64 s = prefix_diff(P, lo, hi);
+        S[b][0] = valid ? pack2((float)s.A, (float)s.B) : pack2(1.0e15f, 1.0e15f);
+        S[b][1] = valid ? pack2((float)(kSqrt2 * s.far), (float)(kSqrt2 * s.fbr)) : 0ull;
+        S[b][2] = valid ? pack2((float)(kSqrt2 * s.fai), (float)(kSqrt2 * s.fbi)) : 0ull;
+        S[b][3] = valid ? pack2((float)s.C, (float)(hi - lo)) : pack2(0.0f, 1.0e9f);
+        rvalid[b] = valid;
+        all_valid = all_valid && valid;
+        n_valid_rows += valid ? 1 : 0;
+        if (active) s_rowm[b * NTu + lt] = valid ? m : -1;
+    }
+
+    // ---- sliding window of G: slot k % NS holds step k of row 0 (row b uses step k + b).  A
+    // slot is refilled right after row 0 has used it, i.e. NS - Q + 1 steps (at least Q - 1
+    // cells of work) before its next use, which hides the L1/L2 latency of the load.
+    constexpr int NS = Q == 1 ? 2 : Q;
+    u64 W[NS][4];
+    // 32-bit lattice index (J <= 2^22); reads beyond the lattice are clamped to the zero entry J
+    int jw = (int)min((int64_t)mbase * bd.e_m + (int64_t)n0 * bd.e_n, (int64_t)bd.J);
+    auto load_g = [&](u64(&w)[4]) {
+        const ulonglong2 *__restrict__ e = g_t + 2 * (int64_t)min(jw, bd.J);
+        const ulonglong2 a = __ldg(e), b2 = __ldg(e + 1);
+        w[0] = a.x;
+        w[1] = a.y;
+        w[2] = b2.x;
+        w[3] = b2.y;
+        jw = min(jw + bd.e_n, bd.J);
+    };
+#pragma unroll
+    for (int k = 0; k < NS; ++k) load_g(W[k]);
+
+    RunMarg rm;
+    rm.best = -INFINITY;
+    rm.idx = 0x7fffffff;
+    rm.ref2 = -INFINITY;
+    rm.sum = 0.0f;
+    rm.nv = 0;
+
+#pragma unroll 1
+    for (int n = n0; n < n_end; n += kChunk) {
+        const int ncols = min(kChunk, n_end - n);
+#pragma unroll 1
+        for (int c4 = 0; c4 < kChunk; c4 += 4) {
+            const int left = ncols - c4;  // columns of this group inside the map (may be <= 0)
+            if (left <= 0) break;
+            // ---- 4 columns x Q rows, straight-line fp32; cells that fail the conditioning
+            // test are only marked here and redone afterwards --------------------------------
+            float res[Q][4];
+            uint32_t slow = 0u;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+#pragma unroll
+                for (int b = 0; b < Q; ++b) {
+                    float A, B, far, fbr, fai, fbi, C, cnt;
+                    unpack2(S[b][0], A, B);
+                    unpack2(S[b][3], C, cnt);
+                    const float p = A * B;
+                    const float D = fmaf(-C, C, p);
+                    if (!(D > kCondFast * p && cnt >= min_atoms_f)) slow |= 1u << (b * 4 + s);
+                    u64 n2 = fmul2(S[b][1], S[b][1]);
+                    ffma2(n2, S[b][2], S[b][2]);
+                    float na, nb;
+                    unpack2(n2, na, nb);  // 2|Fa|^2, 2|Fb|^2
+                    unpack2(S[b][1], far, fbr);
+                    unpack2(S[b][2], fai, fbi);
+                    const float re = fmaf(fai, fbi, far * fbr);
+                    float num = B * na;
+                    num = fmaf(A, nb, num);
+                    num = fmaf(-2.0f * C, re, num);
+                    res[b][s] = num * rcp_approx(D);
+                    S[b][0] = fadd2(S[b][0], W[(s + b) % NS][0]);
+                    S[b][1] = fadd2(S[b][1], W[(s + b) % NS][1]);
+                    S[b][2] = fadd2(S[b][2], W[(s + b) % NS][2]);
+                    S[b][3] = fadd2(S[b][3], W[(s + b) % NS][3]);
+                    if (b == 0) load_g(W[s % NS]);
+                }
+            }
+            uint32_t fw[Q];
+#pragma unroll
+            for (int b = 0; b < Q; ++b) fw[b] = 0u;
+            if (slow) {  // rare
+#pragma unroll
+                for (int b = 0; b < Q; ++b) {
+#pragma unroll
+                    for (int s = 0; s < 4; ++s) {
+                        if (((slow >> (b * 4 + s)) & 1u) && s < left && rvalid[b]) {
+                            const int m = mbase + b * r;
+                            const int64_t j =
+                                (int64_t)m * bd.e_m + (int64_t)(n + c4 + s) * bd.e_n;
+                            float twoF, flf;
+                            unpack2(rect_cell_slow(P, bd.lo, bd.edge, m, j, pr.min_atoms), twoF,
+                                    flf);
+                            res[b][s] = twoF;
+                            fw[b] |= __float_as_uint(flf) << (8 * s);
+                        }
+                    }
+                }
+            }
+            if (active) {
+#pragma unroll
+                for (int b = 0; b < Q; ++b) {
+                    if (want_map)
+                        *reinterpret_cast<float4 *>(tile + (size_t)(b * NTu + lt) * kPitch + c4) =
+                            make_float4(res[b][0], res[b][1], res[b][2], res[b][3]);
+                    if (want_flags) ftile[(b * NTu + lt) * kFPitch + (c4 >> 2)] = fw[b];
+                }
+            }
+            if (MARG && n_valid_rows > 0) {
+                const uint32_t any_fl = Q == 4 ? (fw[0] | fw[1 % Q] | fw[2 % Q] | fw[3 % Q]) : fw[0];
+                if (any_fl == 0u) {
+                    // cells outside the map (rows beyond N_t0, degenerate rows, columns beyond
+                    // N_tau) become -inf: they lose every max and add exp(-inf) = 0
+                    if (!all_valid || left < 4) {
+#pragma unroll
+                        for (int b = 0; b < Q; ++b)
+#pragma unroll
+                            for (int s = 0; s < 4; ++s)
+                                if (!rvalid[b] || s >= left) res[b][s] = -INFINITY;
+                    }
+                    float gmax = res[0][0];
+#pragma unroll
+                    for (int b = 0; b < Q; ++b)
+#pragma unroll
+                        for (int s = 0; s < 4; ++s) gmax = fmaxf(gmax, res[b][s]);
+                    if (gmax > rm.best) {  // rare: first cell of the group, in flat order
+                        bool found = false;
+#pragma unroll
+                        for (int b = 0; b < Q; ++b)
+#pragma unroll
+                            for (int s = 0; s < 4; ++s)
+                                if (!found && res[b][s] == gmax) {
+                                    found = true;
+                                    rm.idx = (mbase + b * r) * g.N_tau + n + c4 + s;
+                                }
+                        rm.best = gmax;
+                    }
+                    if (fmaf(gmax, kHalfLog2e, -rm.ref2) > 60.0f) {  // rare: move the reference
+                        rm.sum *= ex2_approx(rm.ref2 - gmax * kHalfLog2e);
+                        rm.ref2 = gmax * kHalfLog2e;
+                    }
+                    float acc = 0.0f;
+#pragma unroll
+                    for (int b = 0; b < Q; ++b)
+#pragma unroll
+                        for (int s = 0; s < 4; ++s)
+                            acc += ex2_approx(fmaf(res[b][s], kHalfLog2e, -rm.ref2));
+                    rm.sum += acc;
+                    rm.nv += n_valid_rows * min(left, 4);
+                } else {
+#pragma unroll
+                    for (int b = 0; b < Q; ++b)
+#pragma unroll
+                        for (int s = 0; s < 4; ++s)
+                            if (((fw[b] >> (8 * s)) & 0xffu) == 0u && s < left && rvalid[b])
+                                run_marg_add(rm, res[b][s],
+                                             (mbase + b * r) * g.N_tau + n + c4 + s);
+                }
+            }
+        }
+        if (want_map && !want_flags && vec_ok && ncols == kChunk) {  // the common, lean case
+            __syncthreads();
+            float *__restrict__ dst = pr.out_maps + map_base + n + 4 * (threadIdx.x & 3);
+            const float4 *__restrict__ src =
+                reinterpret_cast<const float4 *>(tile) + (threadIdx.x & 3);
+#pragma unroll 4
+            for (int row = threadIdx.x >> 2; row < nrows; row += kRunNT / 4) {
+                const int m = s_rowm[row];
+                if (m >= 0)
+                    __stcs(reinterpret_cast<float4 *>(dst + (int64_t)m * g.N_tau),
+                           src[row * (kPitch / 4)]);
+            }
+            __syncthreads();
+        } else if (want_map || want_flags) {
+            __syncthreads();
+            const int q4 = threadIdx.x & 3;
+            for (int row = threadIdx.x >> 2; row < nrows; row += kRunNT / 4) {
+                const int m = s_rowm[row];
+                if (m < 0) continue;
+                const int64_t o = map_base + (int64_t)m * g.N_tau + n + 4 * q4;
+                const int left = ncols - 4 * q4;
+                if (left <= 0) continue;
+                if (want_map) {
+                    const float4 v =
+                        *reinterpret_cast<const float4 *>(tile + (size_t)row * kPitch + 4 * q4);
+                    if (vec_ok && left >= 4) {
+                        __stcs(reinterpret_cast<float4 *>(pr.out_maps + o), v);
+                    } else {
+                        pr.out_maps[o] = v.x;
+                        if (left > 1) pr.out_maps[o + 1] = v.y;
+                        if (left > 2) pr.out_maps[o + 2] = v.z;
+                        if (left > 3) pr.out_maps[o + 3] = v.w;
+                    }
+                }
+                if (want_flags) {
+                    const uint32_t f = ftile[row * kFPitch + q4];
+                    if (vec_ok && left >= 4) {
+                        *reinterpret_cast<uint32_t *>(pr.out_flags + o) = f;
+                    } else {
+                        pr.out_flags[o] = (uint8_t)(f & 0xffu);
+                        if (left > 1) pr.out_flags[o + 1] = (uint8_t)((f >> 8) & 0xffu);
+                        if (left > 2) pr.out_flags[o + 2] = (uint8_t)((f >> 16) & 0xffu);
+                        if (left > 3) pr.out_flags[o + 3] = (uint8_t)(f >> 24);
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    if (MARG) {
+        Marg mg;
+        marg_init(mg);
+        if (rm.nv > 0) {
+            mg.best = rm.best;
+            mg.idx = rm.idx;
+            mg.M = 0.5f * rm.best;
+            mg.S = rm.sum * ex2_approx(rm.ref2 - rm.best * kHalfLog2e);
+            mg.nvalid = rm.nv;
+        }
+        marg_block_reduce<kRunNT>(mg, s_red);
+        if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
+    }
+}
+
+template <int Q>
+cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
+                       const ulonglong2 *G, Partial *partials, cudaStream_t st)
+{
+    const RectRun &rr = pl.rect;
+    const int nrows = Q * rr.NTu;
+    const size_t smem = (size_t)nrows * (kPitch * 4 + 4 + kFPitch * 4);
+    const int64_t cells = (int64_t)pl.grid.N_t0 * pl.grid.N_tau;
+    const bool vec = (pl.grid.N_tau % 4 == 0) && (cells % 4 == 0) &&
+                     ((reinterpret_cast<uintptr_t>(pr.out_maps) & 15u) == 0) &&
+                     ((reinterpret_cast<uintptr_t>(pr.out_flags) & 3u) == 0);
+    const int64_t n_ctas = (int64_t)rr.n_rowtiles * rr.n_coltiles * pl.n_templates;
+    cudaError_t e;
+    if (partials) {
+        e = cudaFuncSetAttribute(rect_run_kernel<Q, true>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        rect_run_kernel<Q, true><<<(unsigned)n_ctas, kRunNT, smem, st>>>(
+            pr, prefix, G, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
+            vec ? 1 : 0);
+    } else {
+        e = cudaFuncSetAttribute(rect_run_kernel<Q, false>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        rect_run_kernel<Q, false><<<(unsigned)n_ctas, kRunNT, smem, st>>>(
+            pr, prefix, G, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
+            vec ? 1 : 0);
+    }
+    return cudaGetLastError();
+}
+
 }  // namespace
 
-cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, Partial *partials,
-                        cudaStream_t st)
+// Tile shapes of the running-sum kernel; called by make_plan (api.cu).
+RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates)
 {
-    rect_prefix_kernel<<<pl.n_templates, kPrefixNT, 0, st>>>(pr, prefix);
+    RectRun rr;
+    rr.enabled = (J > 0 && g.N_t0 >= 8) ? 1 : 0;
+    rr.Q = 1;
+    rr.r = 1;
+    if (e_m > 0 && e_n > 0 && e_n % e_m == 0) {
+        const int r = e_n / e_m;
+        if (r >= 8 && g.N_t0 >= 4 * r) {
+            rr.Q = 4;
+            rr.r = r;
+        }
+    }
+    rr.NTu = (rr.Q > 1 && rr.r < kRunNT) ? (kRunNT / rr.r) * rr.r : kRunNT;
+    const int64_t units =
+        rr.Q > 1 ? ((int64_t)g.N_t0 + (int64_t)rr.r * rr.Q - 1) / ((int64_t)rr.r * rr.Q) * rr.r
+                 : g.N_t0;
+    rr.n_rowtiles = (int32_t)((units + rr.NTu - 1) / rr.NTu);
+    // columns per CTA: whole waves of 148 SMs x 4 resident CTAs; a row start costs about as
+    // much as 12 cells
+    const int seg_max = (g.N_tau + kChunk - 1) / kChunk * kChunk;
+    int seg = seg_max;
+    int64_t best_cost = INT64_MAX;
+    for (int cand = seg_max; cand >= kChunk; cand -= kChunk) {
+        const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
+        const int64_t waves = (ctas + 148 * 4 - 1) / (148 * 4);
+        const int64_t cost = waves * (cand + 12);
+        if (cost < best_cost) {
+            best_cost = cost;
+            seg = cand;
+        }
+        if (ctas >= (int64_t)148 * 4 * 64) break;  // many waves: quantisation no longer matters
+    }
+    rr.seg_cols = seg;
+    rr.n_coltiles = (g.N_tau + seg - 1) / seg;
+    return rr;
+}
+
+int rect_scan_blocks(int32_t n_atoms) { return (n_atoms + kScanBlock - 1) / kScanBlock; }
+
+cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *tot,
+                        void *steps, Partial *partials, cudaStream_t st)
+{
+    const int nblk = (pl.n_atoms + kScanBlock - 1) / kScanBlock;
+    const unsigned n_scan = (unsigned)((int64_t)nblk * pl.n_templates);
+    rect_totals_kernel<<<n_scan, kScanNT, 0, st>>>(pr, tot, nblk);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const int64_t n_ctas = (int64_t)pl.cell_blocks_per_template * pl.n_templates;
-    rect_cells_kernel<<<(unsigned)n_ctas, kCellNT, 0, st>>>(pr, prefix, partials,
-                                                            pl.cell_blocks_per_template);
-    return cudaGetLastError();
+    rect_prefix_kernel<<<n_scan, kScanNT, 0, st>>>(pr, tot, prefix, nblk);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (!pl.rect.enabled) {
+        const int64_t n_ctas = (int64_t)pl.cell_blocks_per_template * pl.n_templates;
+        rect_cells_kernel<<<(unsigned)n_ctas, kCellNT, 0, st>>>(pr, prefix, partials,
+                                                                pl.cell_blocks_per_template);
+        return cudaGetLastError();
+    }
+    ulonglong2 *G = static_cast<ulonglong2 *>(steps);
+    const int bpt = (int)((pl.J + 1 + 255) / 256);
+    rect_steps_kernel<<<(unsigned)((int64_t)bpt * pl.n_templates), 256, 0, st>>>(pr, prefix, G,
+                                                                                 bpt);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (pl.rect.Q == 4) return launch_run<4>(pl, pr, prefix, G, partials, st);
+    return launch_run<1>(pl, pr, prefix, G, partials, st);
 }
 
 }  // namespace tfstat
