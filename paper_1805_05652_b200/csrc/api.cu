@@ -120,7 +120,7 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         pl.n_segs = (N_t0 + len - 1) / len;
     }
     if (window == TFSTAT_WINDOW_RECT)
-        pl.rect = plan_rect_run(pl.grid, pl.e_m, pl.e_n, pl.J, n_templates);
+        pl.rect = plan_rect_run(pl.grid, pl.e_m, pl.e_n, pl.J, n_templates, opts ? opts->tile_c : 0);
     pl.partials_per_template = direct  ? pl.tiles_per_template
                                : slide ? (int64_t)pl.n_nblocks * pl.n_segs
                                : pl.rect.enabled
@@ -141,6 +141,12 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     pl.off_tot = off;
     if (window == TFSTAT_WINDOW_RECT)
         off += align_up(sizeof(double) * 8 * (size_t)rect_scan_blocks(n_atoms) * n_templates);
+    pl.off_flags = off;
+    pl.flags_bytes = 0;
+    if (window == TFSTAT_WINDOW_RECT) {
+        pl.flags_bytes = sizeof(int32_t) * 2 * (size_t)rect_scan_blocks(n_atoms) * n_templates;
+        off += align_up(pl.flags_bytes);
+    }
     pl.off_steps = off;
     if (window == TFSTAT_WINDOW_RECT && pl.rect.enabled)
         off += align_up((size_t)32 * (size_t)(pl.J + 1) * n_templates);
@@ -154,6 +160,8 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
                       uint8_t *out_flags, void *ws, cudaStream_t st, bool do_bounds)
 {
     if (do_bounds) TF_CUDA(launch_bounds(pl, t_atoms, ws, st));
+    else if (pl.flags_bytes)
+        TF_CUDA(cudaMemsetAsync(static_cast<char *>(ws) + pl.off_flags, 0, pl.flags_bytes, st));
     Problem pr;
     pr.atoms = atoms;
     pr.template_stride = template_stride;
@@ -170,9 +178,10 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     if (pl.ev_main_begin) TF_CUDA(cudaEventRecord(pl.ev_main_begin, st));
     if (pl.window == TFSTAT_WINDOW_RECT) {
         double *prefix = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_prefix);
-        double *tot = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_tot);
-        TF_CUDA(launch_rect(pl, pr, prefix, tot, static_cast<char *>(ws) + pl.off_steps, partials,
-                            st));
+        double *agg = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_tot);
+        int32_t *flags = reinterpret_cast<int32_t *>(static_cast<char *>(ws) + pl.off_flags);
+        TF_CUDA(launch_rect(pl, pr, prefix, agg, flags, static_cast<char *>(ws) + pl.off_steps,
+                            partials, st));
     } else if (pl.exp_method == TFSTAT_EXP_DIRECT) {
         TF_CUDA(launch_exp_direct(pl, pr, partials, st));
     } else {

@@ -7,14 +7,61 @@
 
 namespace tfstat {
 
-__global__ void bounds_kernel(const int32_t *__restrict__ t, int n_atoms, Grid g, int64_t lat_g,
-                              int64_t J, int32_t *__restrict__ lo, int32_t *__restrict__ edge)
+// One lower_bound per t0 and per lattice point.  A plain binary search is a chain of ~log2(N)
+// dependent global loads; here every CTA first stages a coarse sample of the timestamps (the
+// last one of every `stride` atoms, at most kMaxSamples of them) in shared memory, searches
+// that, and finishes with independent loads inside one block of atoms: two global round
+// trips instead of log2(N).
+constexpr int kBoundsNT = 256;
+constexpr int kMaxSamples = 4096;
+
+__device__ __forceinline__ int sampled_lower_bound(const int32_t *__restrict__ t, const int n,
+                                                   const int32_t *__restrict__ s_t,
+                                                   const int n_samples, const int stride,
+                                                   const long long x)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < g.N_t0) lo[i] = lower_bound_t(t, n_atoms, t0_of(g, (int)i));
+    int a = 0, b = n_samples;  // first sample >= x
+    while (a < b) {
+        const int mid = (a + b) >> 1;
+        if ((long long)s_t[mid] < x) a = mid + 1;
+        else b = mid;
+    }
+    if (a == n_samples) return n;
+    int lo = a * stride, hi = min(lo + stride, n);  // the answer is in [lo, hi)
+    while (hi - lo > 16) {
+        const int mid = (lo + hi) >> 1;
+        if ((long long)__ldg(t + mid) < x) lo = mid + 1;
+        else hi = mid;
+    }
+    int v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = (lo + i < hi) ? __ldg(t + lo + i) : INT32_MAX;
+    int cnt = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) cnt += (lo + i < hi && (long long)v[i] < x) ? 1 : 0;
+    return lo + cnt;
+}
+
+__global__ void __launch_bounds__(kBoundsNT)
+    bounds_kernel(const int32_t *__restrict__ t, int n_atoms, Grid g, int64_t lat_g, int64_t J,
+                  int stride, int n_samples, int32_t *__restrict__ lo,
+                  int32_t *__restrict__ edge, int32_t *__restrict__ zero, int64_t n_zero)
+{
+    // scan flags of the rectangular path (rect.cu), zeroed here to save a memset node
+    for (int64_t z = (int64_t)blockIdx.x * kBoundsNT + threadIdx.x; z < n_zero;
+         z += (int64_t)gridDim.x * kBoundsNT)
+        zero[z] = 0;
+    __shared__ int32_t s_t[kMaxSamples];
+    for (int i = threadIdx.x; i < n_samples; i += kBoundsNT)
+        s_t[i] = __ldg(t + min((i + 1) * stride - 1, n_atoms - 1));
+    __syncthreads();
+    const int64_t i = (int64_t)blockIdx.x * kBoundsNT + threadIdx.x;
+    if (i < g.N_t0)
+        lo[i] = sampled_lower_bound(t, n_atoms, s_t, n_samples, stride, t0_of(g, (int)i));
     if (i < J) {
         const long long base = (long long)g.t0_min + (long long)g.k * g.tau_min;
-        edge[i] = lower_bound_t(t, n_atoms, base + (long long)i * lat_g);
+        edge[i] =
+            sampled_lower_bound(t, n_atoms, s_t, n_samples, stride, base + (long long)i * lat_g);
     }
 }
 
@@ -23,9 +70,13 @@ cudaError_t launch_bounds(const Plan &pl, const int32_t *t_atoms, void *ws, cuda
     int32_t *lo = reinterpret_cast<int32_t *>(static_cast<char *>(ws) + pl.off_lo);
     int32_t *edge = reinterpret_cast<int32_t *>(static_cast<char *>(ws) + pl.off_edge);
     const int64_t n = pl.J > pl.grid.N_t0 ? pl.J : pl.grid.N_t0;
-    const int nt = 256;
-    bounds_kernel<<<(unsigned)((n + nt - 1) / nt), nt, 0, st>>>(t_atoms, pl.n_atoms, pl.grid,
-                                                                pl.g, pl.J, lo, edge);
+    int stride = 16;
+    while ((pl.n_atoms + stride - 1) / stride > kMaxSamples) stride <<= 1;
+    const int n_samples = (pl.n_atoms + stride - 1) / stride;
+    bounds_kernel<<<(unsigned)((n + kBoundsNT - 1) / kBoundsNT), kBoundsNT, 0, st>>>(
+        t_atoms, pl.n_atoms, pl.grid, pl.g, pl.J, stride, n_samples, lo, edge,
+        reinterpret_cast<int32_t *>(static_cast<char *>(ws) + pl.off_flags),
+        (int64_t)(pl.flags_bytes / sizeof(int32_t)));
     return cudaGetLastError();
 }
 

@@ -57,7 +57,8 @@ struct Plan {
     int32_t cell_blocks_per_template;
     RectRun rect;
     // workspace layout (byte offsets)
-    size_t off_lo, off_edge, off_partials, off_prefix, off_tot, off_steps, bytes;
+    size_t off_lo, off_edge, off_partials, off_prefix, off_tot, off_flags, off_steps, bytes;
+    size_t flags_bytes;  // rect: scan flags the bounds kernel (or a memset) zeroes
     int64_t partials_per_template;
     cudaEvent_t ev_main_begin, ev_main_end;  // optional profiling hooks (tfstat_opts)
 };
@@ -72,10 +73,11 @@ cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_ter
                                cudaStream_t st);
 cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,
                               cudaStream_t st);
-RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates);
+RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates,
+                      int32_t q_override);
 int rect_scan_blocks(int32_t n_atoms);
-cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *tot,
-                        void *steps, Partial *partials, cudaStream_t st);
+cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,
+                        int32_t *flags, void *steps, Partial *partials, cudaStream_t st);
 cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,
                             cudaStream_t st);
 cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_template,

@@ -2,11 +2,11 @@
 //
 // The paper keeps running partial sums over tau per t0 with N_t0 workers.  Here:
 //
-//  1. rect_totals_kernel + rect_prefix_kernel: exclusive prefix sums P of the 7 atom channels in
-//     fp64, 1024 atoms per CTA (block totals first, then block scans) (an fp32 prefix
+//  1. rect_scan_kernel, scan blocks: exclusive prefix sums P of the 7 atom channels in fp64,
+//     1024 atoms per CTA, block totals exchanged through flags inside the launch (an fp32 prefix
 //     over a year of atoms cancels catastrophically for short windows far from the origin,
 //     SURVEY.md H1; fp64 differences of fp32 data are exact to ~1e-13).
-//  2. rect_steps_kernel: every window end t0_m + tau_n lies on the edge lattice (bounds.cu), so
+//  2. rect_scan_kernel, step blocks (same launch): every window end t0_m + tau_n lies on the edge lattice (bounds.cu), so
 //     the atoms that ENTER a window when tau grows by one grid step are the same for every cell
 //     with the same lattice point j:  G[j] = P[edge[j + e_n]] - P[edge[j]], rounded once to
 //     fp32 (a sum of a few atoms: exact to 2^-24 of its own size), 32 bytes per lattice point.
@@ -32,53 +32,119 @@ constexpr int kScanNT = 256;
 constexpr int kScanPer = 4;                       // atoms per thread
 constexpr int kScanBlock = kScanNT * kScanPer;    // atoms per CTA
 
-// Pass 1: per-block totals of the 7 channels, tot[tpl][blk][8] (fp64).
-__global__ void __launch_bounds__(kScanNT)
-    rect_totals_kernel(const Problem pr, double *__restrict__ tot, const int nblk)
+// ---------------------------------------------------------------------------------------
+// rect_scan_kernel: ONE launch builds the fp64 prefix P and the fp32 lattice steps G.
+//
+//  * scan blocks (blockIdx < n_scan): kScanBlock atoms each.  A block publishes the totals of
+//    its 7 channels (agg + ready flag) BEFORE it waits for anybody, then sums the totals of
+//    the blocks in front of it, scans its own atoms and writes P (done flag).  Blocks only wait
+//    for lower blockIdx, which the hardware dispatches first, so the wait cannot deadlock.
+//  * step blocks (blockIdx >= n_scan): 256 lattice points each; a thread waits for the scan
+//    blocks that own its two P entries, then G[j] = P[edge[j + e_n]] - P[edge[j]].
+//  Flags are zeroed by bounds_kernel (or a memset) before the launch.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void st_release(int32_t *p, const int32_t v)
 {
-    __shared__ double s_w[kScanNT / 32][8];
-    const int tpl = blockIdx.x / nblk, blk = blockIdx.x % nblk;
-    const int N = pr.bounds.n_atoms;
-    const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
-    const int a0 = blk * kScanBlock + (int)threadIdx.x * kScanPer;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double v[7];
-#pragma unroll
-    for (int ch = 0; ch < 7; ++ch) {
-        float x[kScanPer];
-#pragma unroll
-        for (int i = 0; i < kScanPer; ++i)
-            x[i] = (a0 + i < N) ? __ldg(base + ch * pr.ld + a0 + i) : 0.0f;
-        double sacc = 0.0;
-#pragma unroll
-        for (int i = 0; i < kScanPer; ++i) sacc += (double)x[i];
-        v[ch] = sacc;
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// Poll with relaxed loads and a back-off (an acquire load per poll invalidates the whole L1 and
+// starves the producers of issue slots), then one acquire fence.
+__device__ __forceinline__ void wait_flag(const int32_t *p)
+{
+    int32_t v;
+    for (;;) {
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+        if (v != 0) break;
+        __nanosleep(64);
     }
-#pragma unroll
-    for (int ch = 0; ch < 7; ++ch) {
-#pragma unroll
-        for (int sh = 16; sh >= 1; sh >>= 1) v[ch] += __shfl_xor_sync(0xffffffffu, v[ch], sh);
-        if (lane == 0) s_w[warp][ch] = v[ch];
-    }
-    __syncthreads();
-    if (threadIdx.x < 8) {
-        double t = 0.0;
-        if (threadIdx.x < 7)
-            for (int w = 0; w < kScanNT / 32; ++w) t += s_w[w][threadIdx.x];
-        tot[(int64_t)blockIdx.x * 8 + threadIdx.x] = t;
-    }
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
 }
 
-// Pass 2: P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.  Each block adds
-// the totals of the blocks before it to the scan of its own kScanBlock atoms.
+// window sums of atoms [lo, hi) from the prefix, in fp64; L2 loads (P may have been written by
+// another SM during this very launch)
+__device__ __forceinline__ Sums64 prefix_diff_cg(const double2 *P, const int lo, const int hi)
+{
+    const double2 l0 = __ldcg(P + (int64_t)lo * 4), l1 = __ldcg(P + (int64_t)lo * 4 + 1),
+                  l2 = __ldcg(P + (int64_t)lo * 4 + 2), l3 = __ldcg(P + (int64_t)lo * 4 + 3);
+    const double2 h0 = __ldcg(P + (int64_t)hi * 4), h1 = __ldcg(P + (int64_t)hi * 4 + 1),
+                  h2 = __ldcg(P + (int64_t)hi * 4 + 2), h3 = __ldcg(P + (int64_t)hi * 4 + 3);
+    Sums64 s;
+    s.A = h0.x - l0.x;
+    s.B = h0.y - l0.y;
+    s.C = h1.x - l1.x;
+    s.far = h1.y - l1.y;
+    s.fai = h2.x - l2.x;
+    s.fbr = h2.y - l2.y;
+    s.fbi = h3.x - l3.x;
+    return s;
+}
+
+// The running Fa, Fb sums are carried scaled by sqrt(2), so eq. (7) on them yields 2F directly.
+constexpr double kSqrt2 = 1.41421356237309504880;
+constexpr int kDirectStep = 32;    // lattice steps of at most this many atoms are summed directly
+
+// P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.
+// G[tpl][j], j = 0..J, 32 B per entry: {(A, B), (Re Fa, Re Fb)}, {(Im Fa, Im Fb), (C, count)};
+// entry J is all zero (out-of-range reads of the running kernel are clamped to it).
 __global__ void __launch_bounds__(kScanNT)
-    rect_prefix_kernel(const Problem pr, const double *__restrict__ tot,
-                       double *__restrict__ prefix, const int nblk)
+    rect_scan_kernel(const Problem pr, double *__restrict__ agg, int32_t *__restrict__ flags,
+                     double *__restrict__ prefix, ulonglong2 *__restrict__ G, const int nblk,
+                     const int n_scan, const int steps_per_template)
 {
     __shared__ double s_off[8];
     __shared__ double s_w[7][kScanNT / 32];
+    const Bounds &bd = pr.bounds;
+    const int N = bd.n_atoms;
+    int32_t *ready = flags, *done = flags + n_scan;
+
+    if ((int)blockIdx.x >= n_scan) {  // ---- step role ------------------------------------
+        const int sb = blockIdx.x - n_scan;
+        const int tpl = sb / steps_per_template;
+        const int j = (sb % steps_per_template) * kScanNT + threadIdx.x;
+        if (j > bd.J) return;
+        const int j2 = j + bd.e_n;
+        ulonglong2 ga = make_ulonglong2(0ull, 0ull), gb = make_ulonglong2(0ull, 0ull);
+        if (j2 < bd.J) {
+            const int a = __ldg(bd.edge + j), b = __ldg(bd.edge + j2);
+            Sums64 s;
+            if (b - a <= kDirectStep) {
+                // short step: sum its atoms directly (fp64), independent of the scan blocks
+                const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+                double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll 8
+                for (int al = a; al < b; ++al) {
+#pragma unroll
+                    for (int ch = 0; ch < 7; ++ch) acc[ch] += (double)__ldg(base + ch * pr.ld + al);
+                }
+                s.A = acc[0];
+                s.B = acc[1];
+                s.C = acc[2];
+                s.far = acc[3];
+                s.fai = acc[4];
+                s.fbr = acc[5];
+                s.fbi = acc[6];
+            } else {
+                const int32_t *da = done + tpl * nblk + max(a - 1, 0) / kScanBlock;
+                const int32_t *db = done + tpl * nblk + max(b - 1, 0) / kScanBlock;
+                wait_flag(db);  // scan blocks finish roughly in order: the later one first
+                wait_flag(da);
+                const double2 *P =
+                    reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (N + 1) * 8);
+                s = prefix_diff_cg(P, a, b);
+            }
+            ga.x = pack2((float)s.A, (float)s.B);
+            ga.y = pack2((float)(kSqrt2 * s.far), (float)(kSqrt2 * s.fbr));
+            gb.x = pack2((float)(kSqrt2 * s.fai), (float)(kSqrt2 * s.fbi));
+            gb.y = pack2((float)s.C, (float)(b - a));
+        }
+        ulonglong2 *__restrict__ o = G + ((int64_t)tpl * (bd.J + 1) + j) * 2;
+        o[0] = ga;
+        o[1] = gb;
+        return;
+    }
+
+    // ---- scan role --------------------------------------------------------------------------
     const int tpl = blockIdx.x / nblk, blk = blockIdx.x % nblk;
-    const int N = pr.bounds.n_atoms;
     const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
     double *__restrict__ P = prefix + (int64_t)tpl * (N + 1) * 8;
     const int a0 = blk * kScanBlock + (int)threadIdx.x * kScanPer;
@@ -90,15 +156,6 @@ __global__ void __launch_bounds__(kScanNT)
 #pragma unroll
         for (int i = 0; i < kScanPer; ++i)
             x[ch][i] = (a0 + i < N) ? __ldg(base + ch * pr.ld + a0 + i) : 0.0f;
-
-    // offset of this block: warp ch sums tot[tpl][0..blk)[ch]
-    if (warp < 7) {
-        double t = 0.0;
-        for (int b = lane; b < blk; b += 32) t += __ldg(tot + ((int64_t)tpl * nblk + b) * 8 + warp);
-#pragma unroll
-        for (int sh = 16; sh >= 1; sh >>= 1) t += __shfl_xor_sync(0xffffffffu, t, sh);
-        if (lane == 0) s_off[warp] = t;
-    }
 
     double incl[7], tsum[7];
 #pragma unroll
@@ -116,6 +173,32 @@ __global__ void __launch_bounds__(kScanNT)
         if (lane == 31) s_w[ch][warp] = t;
     }
     __syncthreads();
+    {
+        // publish this block's totals before waiting for anyone
+        if (threadIdx.x < 32) {
+            if (threadIdx.x < 7) {
+                double t = 0.0;
+#pragma unroll
+                for (int w = 0; w < kScanNT / 32; ++w) t += s_w[threadIdx.x][w];
+                __stcg(agg + (int64_t)blockIdx.x * 8 + threadIdx.x, t);
+                __threadfence();
+            }
+            __syncwarp();
+            if (threadIdx.x == 0) st_release(ready + blockIdx.x, 1);
+        }
+        // offset of this block: warp ch sums the totals of blocks [0, blk) of this template
+        if (warp < 7) {
+            double t = 0.0;
+            for (int b = lane; b < blk; b += 32) {
+                wait_flag(ready + tpl * nblk + b);
+                t += __ldcg(agg + ((int64_t)tpl * nblk + b) * 8 + warp);
+            }
+#pragma unroll
+            for (int sh = 16; sh >= 1; sh >>= 1) t += __shfl_xor_sync(0xffffffffu, t, sh);
+            if (lane == 0) s_off[warp] = t;
+        }
+    }
+    __syncthreads();
     if (threadIdx.x == 0 && blk == 0) {
 #pragma unroll
         for (int ch = 0; ch < 8; ++ch) P[ch] = 0.0;
@@ -130,7 +213,10 @@ __global__ void __launch_bounds__(kScanNT)
             if (a0 + i < N) P[(int64_t)(a0 + i + 1) * 8 + ch] = run;
         }
     }
-    // pad lane of the 64-B entries stays unwritten: nothing reads it
+    // pad lane of the 64-B entries stays unwritten: nothing uses it
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) st_release(done + blockIdx.x, 1);
 }
 
 // window sums of atoms [lo, hi) from the prefix, in fp64
@@ -190,38 +276,6 @@ __global__ void __launch_bounds__(kCellNT)
     }
 }
 
-// The running Fa, Fb sums are carried scaled by sqrt(2), so eq. (7) on them yields 2F directly.
-constexpr double kSqrt2 = 1.41421356237309504880;
-
-// ---------------------------------------------------------------------------------------
-// lattice steps G[tpl][j], j = 0..J, 32 bytes each:
-//   {(A, B), (Re Fa, Re Fb)}, {(Im Fa, Im Fb), (C, count)}
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-    rect_steps_kernel(const Problem pr, const double *__restrict__ prefix,
-                      ulonglong2 *__restrict__ G, const int blocks_per_template)
-{
-    const Bounds &bd = pr.bounds;
-    const int tpl = blockIdx.x / blocks_per_template;
-    const int j = (blockIdx.x % blocks_per_template) * 256 + threadIdx.x;
-    if (j > bd.J) return;  // entry J is the all-zero entry out-of-range reads are clamped to
-    const int j2 = j + bd.e_n;
-    ulonglong2 ga = make_ulonglong2(0ull, 0ull), gb = make_ulonglong2(0ull, 0ull);
-    if (j2 < bd.J) {
-        const int a = __ldg(bd.edge + j), b = __ldg(bd.edge + j2);
-        const double2 *__restrict__ P = reinterpret_cast<const double2 *>(
-            prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
-        const Sums64 s = prefix_diff(P, a, b);
-        ga.x = pack2((float)s.A, (float)s.B);
-        ga.y = pack2((float)(kSqrt2 * s.far), (float)(kSqrt2 * s.fbr));  // see rect_run_kernel
-        gb.x = pack2((float)(kSqrt2 * s.fai), (float)(kSqrt2 * s.fbi));
-        gb.y = pack2((float)s.C, (float)(b - a));
-    }
-    ulonglong2 *__restrict__ o = G + ((int64_t)tpl * (bd.J + 1) + j) * 2;
-    o[0] = ga;
-    o[1] = gb;
-}
-
 // ---------------------------------------------------------------------------------------
 // running-sum kernel
 // ---------------------------------------------------------------------------------------
@@ -269,25 +323,8 @@ struct RunMarg {
     int32_t nv;
 };
 
-// generic per-cell update (groups with flagged cells, ragged tails, rows outside the grid)
-__device__ __noinline__ void run_marg_add(RunMarg &a, const float twoF, const int32_t flat)
-{
-    if (twoF > a.best || (twoF == a.best && flat < a.idx)) {
-        a.best = twoF;
-        a.idx = flat;
-    }
-    float d = fmaf(twoF, kHalfLog2e, -a.ref2);
-    if (d > 60.0f) {  // move the reference up (first cell: ref2 = -inf, sum = 0)
-        a.sum *= ex2_approx(-d);
-        a.ref2 = twoF * kHalfLog2e;
-        d = 0.0f;
-    }
-    a.sum += ex2_approx(d);
-    a.nv += 1;
-}
-
 template <int Q, bool MARG>
-__global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : 5)
+__global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
     rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
                     const ulonglong2 *__restrict__ G, Partial *__restrict__ partials, const int r, const int NTu,
                     const int seg_cols, const int n_rowtiles, const int n_coltiles,
@@ -469,17 +506,26 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : 5)
                 }
             }
             if (MARG && n_valid_rows > 0) {
-                const uint32_t any_fl = Q == 4 ? (fw[0] | fw[1 % Q] | fw[2 % Q] | fw[3 % Q]) : fw[0];
-                if (any_fl == 0u) {
-                    // cells outside the map (rows beyond N_t0, degenerate rows, columns beyond
-                    // N_tau) become -inf: they lose every max and add exp(-inf) = 0
-                    if (!all_valid || left < 4) {
+                uint32_t any_fl = 0u;
 #pragma unroll
-                        for (int b = 0; b < Q; ++b)
+                for (int b = 0; b < Q; ++b) any_fl |= fw[b];
+                int n_ok = 4 * n_valid_rows;
+                // cells outside the map (rows beyond N_t0, degenerate rows, columns beyond
+                // N_tau) and flagged cells become -inf: they lose every max and add
+                // exp(-inf) = 0
+                if (any_fl != 0u || !all_valid || left < 4) {
+                    n_ok = 0;
 #pragma unroll
-                            for (int s = 0; s < 4; ++s)
-                                if (!rvalid[b] || s >= left) res[b][s] = -INFINITY;
-                    }
+                    for (int b = 0; b < Q; ++b)
+#pragma unroll
+                        for (int s = 0; s < 4; ++s) {
+                            if (!rvalid[b] || s >= left || ((fw[b] >> (8 * s)) & 0xffu) != 0u)
+                                res[b][s] = -INFINITY;
+                            else
+                                n_ok += 1;
+                        }
+                }
+                if (n_ok > 0) {
                     float gmax = res[0][0];
 #pragma unroll
                     for (int b = 0; b < Q; ++b)
@@ -508,15 +554,7 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : 5)
                         for (int s = 0; s < 4; ++s)
                             acc += ex2_approx(fmaf(res[b][s], kHalfLog2e, -rm.ref2));
                     rm.sum += acc;
-                    rm.nv += n_valid_rows * min(left, 4);
-                } else {
-#pragma unroll
-                    for (int b = 0; b < Q; ++b)
-#pragma unroll
-                        for (int s = 0; s < 4; ++s)
-                            if (((fw[b] >> (8 * s)) & 0xffu) == 0u && s < left && rvalid[b])
-                                run_marg_add(rm, res[b][s],
-                                             (mbase + b * r) * g.N_tau + n + c4 + s);
+                    rm.nv += n_ok;
                 }
             }
         }
@@ -619,7 +657,8 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
 }  // namespace
 
 // Tile shapes of the running-sum kernel; called by make_plan (api.cu).
-RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates)
+RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates,
+                      int32_t q_override)
 {
     RectRun rr;
     rr.enabled = (J > 0 && g.N_t0 >= 8) ? 1 : 0;
@@ -627,9 +666,19 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     rr.r = 1;
     if (e_m > 0 && e_n > 0 && e_n % e_m == 0) {
         const int r = e_n / e_m;
-        if (r >= 8 && g.N_t0 >= 4 * r) {
+        // Q = 2 measured best on B200 (config 5): 80 registers, 6 CTAs per SM; Q = 4 halves
+        // the G traffic again but runs at 4 CTAs per SM
+        if (r >= 8 && g.N_t0 >= 2 * r) {
+            rr.Q = 2;
+            rr.r = r;
+        }
+        if (q_override == 4 && r >= 8 && g.N_t0 >= 4 * r) {
             rr.Q = 4;
             rr.r = r;
+        }
+        if (q_override == 1) {
+            rr.Q = 1;
+            rr.r = 1;
         }
     }
     rr.NTu = (rr.Q > 1 && rr.r < kRunNT) ? (kRunNT / rr.r) * rr.r : kRunNT;
@@ -644,7 +693,8 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     int64_t best_cost = INT64_MAX;
     for (int cand = seg_max; cand >= kChunk; cand -= kChunk) {
         const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
-        const int64_t waves = (ctas + 148 * 4 - 1) / (148 * 4);
+        const int64_t per_wave = 148 * (rr.Q == 4 ? 4 : rr.Q == 2 ? 6 : 5);
+        const int64_t waves = (ctas + per_wave - 1) / per_wave;
         const int64_t cost = waves * (cand + 12);
         if (cost < best_cost) {
             best_cost = cost;
@@ -659,16 +709,19 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
 
 int rect_scan_blocks(int32_t n_atoms) { return (n_atoms + kScanBlock - 1) / kScanBlock; }
 
-cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *tot,
-                        void *steps, Partial *partials, cudaStream_t st)
+cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,
+                        int32_t *flags, void *steps, Partial *partials, cudaStream_t st)
 {
-    const int nblk = (pl.n_atoms + kScanBlock - 1) / kScanBlock;
-    const unsigned n_scan = (unsigned)((int64_t)nblk * pl.n_templates);
-    rect_totals_kernel<<<n_scan, kScanNT, 0, st>>>(pr, tot, nblk);
+    // flags (ready + done per scan block) must be zero here: launch_bounds zeroes them, and
+    // run_device memsets them when the bounds of an earlier call are reused
+    const int nblk = rect_scan_blocks(pl.n_atoms);
+    const int n_scan = nblk * pl.n_templates;
+    ulonglong2 *G = static_cast<ulonglong2 *>(steps);
+    const int spt = pl.rect.enabled ? (int)((pl.J + 1 + kScanNT - 1) / kScanNT) : 0;
+    const int64_t n_blocks = (int64_t)n_scan + (int64_t)spt * pl.n_templates;
+    rect_scan_kernel<<<(unsigned)n_blocks, kScanNT, 0, st>>>(pr, agg, flags, prefix, G, nblk,
+                                                             n_scan, spt);
     cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    rect_prefix_kernel<<<n_scan, kScanNT, 0, st>>>(pr, tot, prefix, nblk);
-    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (!pl.rect.enabled) {
         const int64_t n_ctas = (int64_t)pl.cell_blocks_per_template * pl.n_templates;
@@ -676,13 +729,8 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
                                                                 pl.cell_blocks_per_template);
         return cudaGetLastError();
     }
-    ulonglong2 *G = static_cast<ulonglong2 *>(steps);
-    const int bpt = (int)((pl.J + 1 + 255) / 256);
-    rect_steps_kernel<<<(unsigned)((int64_t)bpt * pl.n_templates), 256, 0, st>>>(pr, prefix, G,
-                                                                                 bpt);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
     if (pl.rect.Q == 4) return launch_run<4>(pl, pr, prefix, G, partials, st);
+    if (pl.rect.Q == 2) return launch_run<2>(pl, pr, prefix, G, partials, st);
     return launch_run<1>(pl, pr, prefix, G, partials, st);
 }
 
