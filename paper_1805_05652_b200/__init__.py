@@ -24,3 +24,4 @@ from .binding import (  # noqa: F401
     tfstat_search_host,
     workspace_bytes,
 )
+from .shard import gather_results, template_shard  # noqa: F401,E402

@@ -101,6 +101,23 @@ def test_search_batched_small(pkg, window):
     assert np.array_equal(res2.numpy(), got)
 
 
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_search_equals_unsharded(pkg, world):
+    """Template sharding (paper_1805_05652_b200/shard.py): every rank's contiguous shard run on
+    its own gives bit-identical records to the one unsharded call (no data-path collective)."""
+    grid = Grid(0, 1800, 23, 3600, 3600, 140)
+    wl = tiny_workload(204, 300, 0.1, grid, n_templates=7, phi_random=True)
+    a, t = dev(wl.data.atoms), dev(wl.data.t)
+    for window in (EXP, RECT):
+        full = pkg.tfstat_search(a, t, window, grid).numpy()
+        parts = []
+        for rank in range(world):
+            lo, cnt = pkg.template_shard(a.shape[0], rank, world)
+            if cnt:
+                parts.append(pkg.tfstat_search(a[lo:lo + cnt], t, window, grid).numpy())
+        assert np.array_equal(np.concatenate(parts), full)
+
+
 def test_search_host_equals_device(pkg):
     grid = Grid(0, 1800, 16, 3600, 1800, 100)
     wl = tiny_workload(202, 260, 0.05, grid, n_templates=9, phi_random=True)
