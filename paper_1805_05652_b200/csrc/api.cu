@@ -120,7 +120,8 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         pl.n_segs = (N_t0 + len - 1) / len;
     }
     if (window == TFSTAT_WINDOW_RECT)
-        pl.rect = plan_rect_run(pl.grid, pl.e_m, pl.e_n, pl.J, n_templates, opts ? opts->tile_c : 0);
+        pl.rect = plan_rect_run(pl.grid, pl.e_m, pl.e_n, pl.J, n_templates, opts ? opts->tile_c : 0,
+                                opts ? opts->seg_len : 0);
     pl.partials_per_template = direct  ? pl.tiles_per_template
                                : slide ? (int64_t)pl.n_nblocks * pl.n_segs
                                : pl.rect.enabled
@@ -149,7 +150,7 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     }
     pl.off_steps = off;
     if (window == TFSTAT_WINDOW_RECT && pl.rect.enabled)
-        off += align_up((size_t)32 * (size_t)(pl.J + 1) * n_templates);
+        off += align_up((size_t)64 * (size_t)(pl.J + 1) * n_templates);
     pl.bytes = off;
     pl.status = TFSTAT_OK;
     return pl;

@@ -30,8 +30,8 @@ struct ExpTile {
     int NT;
 };
 
-// rect running-sum kernel (rect.cu): a thread owns Q rows m, m+r, ..; a CTA owns NTu threads
-// (Q NTu rows) x seg_cols columns
+// rect running-sum kernel (rect.cu): a thread owns Q rows m, m+r, ..; a CTA owns NTu residues
+// x 128 / NTu row groups x seg_cols columns
 struct RectRun {
     int32_t enabled;  // 0: per-cell kernel (no edge lattice / very few rows)
     int32_t Q, r, NTu, seg_cols, n_rowtiles, n_coltiles;
@@ -74,7 +74,7 @@ cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_ter
 cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,
                               cudaStream_t st);
 RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates,
-                      int32_t q_override);
+                      int32_t q_override, int32_t seg_override);
 int rect_scan_blocks(int32_t n_atoms);
 cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,
                         int32_t *flags, void *steps, Partial *partials, cudaStream_t st);

@@ -6,22 +6,29 @@
 //     1024 atoms per CTA, block totals exchanged through flags inside the launch (an fp32 prefix
 //     over a year of atoms cancels catastrophically for short windows far from the origin,
 //     SURVEY.md H1; fp64 differences of fp32 data are exact to ~1e-13).
-//  2. rect_scan_kernel, step blocks (same launch): every window end t0_m + tau_n lies on the edge lattice (bounds.cu), so
-//     the atoms that ENTER a window when tau grows by one grid step are the same for every cell
-//     with the same lattice point j:  G[j] = P[edge[j + e_n]] - P[edge[j]], rounded once to
-//     fp32 (a sum of a few atoms: exact to 2^-24 of its own size), 32 bytes per lattice point.
-//  3. rect_run_kernel: one thread walks one t0 row along tau.  It starts each column tile from
-//     the exact window sum P[hi] - P[lo] and then only ADDS G steps -- the paper's running sum,
-//     but with pre-aggregated steps, so a cell costs 4 packed fp32 adds + the closure.  Rows
-//     m, m+r, m+2r, m+3r (r = k dtau / dt0) use the same G entries one column later, so a thread
-//     owns those Q = 4 rows and keeps a sliding register window of G: 8 bytes of L1 traffic per
-//     cell.  The closure (eq. 7) runs in fp32 when the cell is well conditioned
-//     (D > AB/64, error <= ~1e-4 relative); other cells are recomputed in fp64 from P.
-//     2F values are transposed through shared memory (thread = row, but the map is tau-fastest)
-//     and leave as 64-byte row segments.
+//  2. rect_scan_kernel, step blocks (same launch): every window end t0_m + tau_n lies on the
+//     edge lattice (bounds.cu), so the atoms that ENTER a window when tau grows by TWO grid
+//     steps are the same for every cell with the same lattice point j:
+//     H[j] = P[edge[j + 2 e_n]] - P[edge[j]], rounded once to fp32 (a sum of a few atoms: exact
+//     to 2^-24 of its own size).  The table K[j] = (H[j], H[j + e_n]) holds them as channel
+//     pairs, 64 bytes per lattice point, planar so that a warp reads whole 128-byte lines.
+//  3. rect_run_kernel: one thread walks one t0 row along tau, two columns at a time: its state
+//     is the seven sums of columns (n, n+1) as packed fp32x2 pairs.  It starts each column tile
+//     from the exact window sums P[hi] - P[lo] and then only ADDS K -- the paper's running sum,
+//     with pre-aggregated steps -- so two cells cost 8 packed adds + 13 packed multiply-adds +
+//     2 MUFU.RCP (eq. 7, pair_closure).  Row m + 2 e_n / e_m uses the same K entries one
+//     pair-step later, so a thread owns Q = 2 such rows and keeps a sliding register window of
+//     K: 16 bytes of L1 traffic per cell; the other row groups of its CTA find them in L1.  The
+//     closure runs in fp32 where the cell is well conditioned (D > AB/64, error <= ~1e-4
+//     relative); groups with any other cell, and the leading columns that hold fewer than
+//     min_atoms atoms, are recomputed in fp64 from P.  2F values are transposed through
+//     (swizzled) shared memory (thread = row, but the map is tau-fastest) and leave as 64-byte
+//     row segments.
 //
 // Grids without an edge lattice (J = 0) or with very few t0 rows use the per-cell kernel
 // rect_cells_kernel: S(m,n) = P[hi(m,n)] - P[lo(m)], closure in fp64.
+#include <algorithm>
+
 #include "plan.h"
 
 namespace tfstat {
@@ -81,14 +88,15 @@ __device__ __forceinline__ Sums64 prefix_diff_cg(const double2 *P, const int lo,
 
 // The running Fa, Fb sums are carried scaled by sqrt(2), so eq. (7) on them yields 2F directly.
 constexpr double kSqrt2 = 1.41421356237309504880;
-constexpr int kDirectStep = 32;    // lattice steps of at most this many atoms are summed directly
+constexpr int kDirectStep = 64;    // lattice steps of at most this many atoms are summed directly
 
 // P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.
-// G[tpl][j], j = 0..J, 32 B per entry: {(A, B), (Re Fa, Re Fb)}, {(Im Fa, Im Fb), (C, count)};
-// entry J is all zero (out-of-range reads of the running kernel are clamped to it).
+// K[tpl][q][j], q = 0..3, j = 0..J, 16 B per element (64 B per lattice point): the channel pairs (x of H[j], x of H[j + e_n]) for
+// x = A, B | C, -C | Re Fa, Im Fa | Re Fb, Im Fb (Fa, Fb scaled by sqrt 2); entry J is all zero
+// (out-of-range reads of the running kernel are clamped to it).
 __global__ void __launch_bounds__(kScanNT)
     rect_scan_kernel(const Problem pr, double *__restrict__ agg, int32_t *__restrict__ flags,
-                     double *__restrict__ prefix, ulonglong2 *__restrict__ G, const int nblk,
+                     double *__restrict__ prefix, ulonglong2 *__restrict__ K, const int nblk,
                      const int n_scan, const int steps_per_template)
 {
     __shared__ double s_off[8];
@@ -102,27 +110,31 @@ __global__ void __launch_bounds__(kScanNT)
         const int tpl = sb / steps_per_template;
         const int j = (sb % steps_per_template) * kScanNT + threadIdx.x;
         if (j > bd.J) return;
-        const int j2 = j + bd.e_n;
-        ulonglong2 ga = make_ulonglong2(0ull, 0ull), gb = make_ulonglong2(0ull, 0ull);
-        if (j2 < bd.J) {
-            const int a = __ldg(bd.edge + j), b = __ldg(bd.edge + j2);
-            Sums64 s;
+        // K[j] = (H[j], H[j + e_n]), H[i] = sums of the atoms in [edge[i], edge[i + 2 e_n]):
+        // what the column PAIR (n, n+1) of a row gains when it moves on to (n+2, n+3)
+        Sums64 h[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            h[q].A = h[q].B = h[q].C = h[q].far = h[q].fai = h[q].fbr = h[q].fbi = 0.0;
+            const int64_t ja = (int64_t)j + (int64_t)q * bd.e_n, jb = ja + 2 * (int64_t)bd.e_n;
+            if (jb >= bd.J) continue;  // beyond the lattice: only cells outside the map use it
+            const int a = __ldg(bd.edge + ja), b = __ldg(bd.edge + jb);
             if (b - a <= kDirectStep) {
                 // short step: sum its atoms directly (fp64), independent of the scan blocks
                 const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
                 double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-#pragma unroll 8
+#pragma unroll 4
                 for (int al = a; al < b; ++al) {
 #pragma unroll
                     for (int ch = 0; ch < 7; ++ch) acc[ch] += (double)__ldg(base + ch * pr.ld + al);
                 }
-                s.A = acc[0];
-                s.B = acc[1];
-                s.C = acc[2];
-                s.far = acc[3];
-                s.fai = acc[4];
-                s.fbr = acc[5];
-                s.fbi = acc[6];
+                h[q].A = acc[0];
+                h[q].B = acc[1];
+                h[q].C = acc[2];
+                h[q].far = acc[3];
+                h[q].fai = acc[4];
+                h[q].fbr = acc[5];
+                h[q].fbi = acc[6];
             } else {
                 const int32_t *da = done + tpl * nblk + max(a - 1, 0) / kScanBlock;
                 const int32_t *db = done + tpl * nblk + max(b - 1, 0) / kScanBlock;
@@ -130,16 +142,21 @@ __global__ void __launch_bounds__(kScanNT)
                 wait_flag(da);
                 const double2 *P =
                     reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (N + 1) * 8);
-                s = prefix_diff_cg(P, a, b);
+                h[q] = prefix_diff_cg(P, a, b);
             }
-            ga.x = pack2((float)s.A, (float)s.B);
-            ga.y = pack2((float)(kSqrt2 * s.far), (float)(kSqrt2 * s.fbr));
-            gb.x = pack2((float)(kSqrt2 * s.fai), (float)(kSqrt2 * s.fbi));
-            gb.y = pack2((float)s.C, (float)(b - a));
         }
-        ulonglong2 *__restrict__ o = G + ((int64_t)tpl * (bd.J + 1) + j) * 2;
-        o[0] = ga;
-        o[1] = gb;
+        // planar: plane q of template tpl holds J + 1 16-byte elements, so that the lanes of a
+        // warp (consecutive rows = consecutive j) read consecutive 16-byte words
+        ulonglong2 *__restrict__ o = K + (int64_t)tpl * 4 * (bd.J + 1) + j;
+        const int64_t pl = (int64_t)bd.J + 1;
+        o[0] = make_ulonglong2(pack2((float)h[0].A, (float)h[1].A),
+                               pack2((float)h[0].B, (float)h[1].B));
+        o[pl] = make_ulonglong2(pack2((float)h[0].C, (float)h[1].C),
+                               pack2((float)-h[0].C, (float)-h[1].C));
+        o[2 * pl] = make_ulonglong2(pack2((float)(kSqrt2 * h[0].far), (float)(kSqrt2 * h[1].far)),
+                               pack2((float)(kSqrt2 * h[0].fai), (float)(kSqrt2 * h[1].fai)));
+        o[3 * pl] = make_ulonglong2(pack2((float)(kSqrt2 * h[0].fbr), (float)(kSqrt2 * h[1].fbr)),
+                               pack2((float)(kSqrt2 * h[0].fbi), (float)(kSqrt2 * h[1].fbi)));
         return;
     }
 
@@ -281,7 +298,8 @@ __global__ void __launch_bounds__(kCellNT)
 // ---------------------------------------------------------------------------------------
 constexpr int kRunNT = 128;
 constexpr int kChunk = 16;   // columns between two write-outs of the transposed tile
-constexpr int kPitch = 20;   // floats per tile row: conflict-free STS.128 and aligned LDS.128
+constexpr int kPitch = 16;   // floats per tile row; the four 16-byte column groups of row i are
+                             // XOR-swizzled with (i >> 1) & 3: conflict-free STS.128 and LDS.128
 constexpr int kFPitch = 5;   // 32-bit words per flag-tile row (16 flag bytes + pad)
 constexpr float kCondFast = 1.0f / 64.0f;  // fp32 closure only if D > kCondFast * A * B
 constexpr float kHalfLog2e = 0.72134752044448170368f;
@@ -323,19 +341,56 @@ struct RunMarg {
     int32_t nv;
 };
 
+// Row state of the running kernel: 8 channel pairs, each (column n, column n + 1):
+//   0 A   1 B   2 C   3 -C   4 Re Fa   5 Im Fa   6 Re Fb   7 Im Fb      (Fa, Fb times sqrt 2)
+// so eq. (7) for TWO cells is 13 packed fp32x2 operations and 2 MUFU.RCP:
+//   D = A B + (-C) C;  2|Fa|^2, 2|Fb|^2, 2 Re(Fa conj Fb);  num = B 2|Fa|^2 + A 2|Fb|^2
+//   + 2 (-C) 2Re;  2F = num / D.
+// -C is carried as a channel of its own because fma.rn.f32x2 has no operand negation.
+struct PairOut {
+    u64 res;  // 2F of (column n, column n + 1), fp32 fast path
+    u64 t;    // D - kCondFast A B of the two cells: the fast path holds where t > 0
+};
+
+__device__ __forceinline__ PairOut pair_closure(const u64 (&S)[8])
+{
+    const u64 p = fmul2(S[0], S[1]);
+    u64 D = p;
+    ffma2(D, S[3], S[2]);
+    PairOut o;
+    o.t = D;
+    ffma2(o.t, p, pack2(-kCondFast, -kCondFast));
+    u64 na = fmul2(S[4], S[4]);
+    ffma2(na, S[5], S[5]);
+    u64 nb = fmul2(S[6], S[6]);
+    ffma2(nb, S[7], S[7]);
+    u64 re = fmul2(S[4], S[6]);
+    ffma2(re, S[5], S[7]);
+    u64 num = fmul2(S[1], na);
+    ffma2(num, S[0], nb);
+    ffma2(num, S[3], re);
+    ffma2(num, S[3], re);
+    float d0, d1;
+    unpack2(D, d0, d1);
+    o.res = fmul2(num, pack2(rcp_approx(d0), rcp_approx(d1)));
+    return o;
+}
+
+// 4 CTAs per SM for Q = 2 (128 registers): measured on B200 against 3 (162 registers, no spill),
+// 5 (96) and 6 (80, spilling) CTAs per SM, which are 13 % to 58 % slower on config 5
 template <int Q, bool MARG>
-__global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
+__global__ void __launch_bounds__(kRunNT, Q == 2 ? 4 : 5)
     rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
-                    const ulonglong2 *__restrict__ G, Partial *__restrict__ partials, const int r, const int NTu,
-                    const int seg_cols, const int n_rowtiles, const int n_coltiles,
-                    const int vec_ok)
+                    const ulonglong2 *__restrict__ K, Partial *__restrict__ partials,
+                    const int roff, const int R, const int seg_cols, const int n_rowtiles,
+                    const int n_coltiles, const int vec_ok)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Marg s_red[32];
-    const int nrows = Q * NTu;
-    float *tile = reinterpret_cast<float *>(smem_raw);                 // [nrows][kPitch]
+    constexpr int nrows = Q * kRunNT;
+    float *tile = reinterpret_cast<float *>(smem_raw);                     // [nrows][kPitch]
     int *s_rowm = reinterpret_cast<int *>(tile + (size_t)nrows * kPitch);  // [nrows]
-    uint32_t *ftile = reinterpret_cast<uint32_t *>(s_rowm + nrows);   // [nrows][kFPitch]
+    uint32_t *ftile = reinterpret_cast<uint32_t *>(s_rowm + nrows);        // [nrows][kFPitch]
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -343,43 +398,50 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
     const int coltile = (blockIdx.x / n_rowtiles) % n_coltiles;
     const int tpl = blockIdx.x / (n_rowtiles * n_coltiles);
     const int lt = threadIdx.x;
-    const bool active = lt < NTu;
-    const int u = rowtile * NTu + min(lt, NTu - 1);
-    int mbase = u;
+    // Rows come in groups of Q roff consecutive rows; a thread owns rows res, res + roff, ..
+    // of one group.  A CTA is R consecutive residues x (kRunNT / R) consecutive groups: the
+    // same residue of the NEXT group walks the same K entries 2 Q columns later, so the groups
+    // of a CTA find them in L1.
+    int mbase = rowtile * kRunNT + lt;
     if (Q > 1) {
-        const int grp = u / r;
-        mbase = grp * r * Q + (u - grp * r);
+        const int gpc = kRunNT / R;           // groups per CTA
+        const int n_restiles = (roff + R - 1) / R;
+        const int res = (rowtile % n_restiles) * R + lt % R;
+        const int grp = (rowtile / n_restiles) * gpc + lt / R;
+        mbase = res < roff ? grp * roff * Q + res : g.N_t0;  // ragged residue tile: no rows
     }
     const int n0 = coltile * seg_cols;
     const int n_end = min(n0 + seg_cols, g.N_tau);
     const double2 *__restrict__ P =
         reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
-    const ulonglong2 *__restrict__ g_t = G + (int64_t)tpl * (bd.J + 1) * 2;
-    const float min_atoms_f = (float)pr.min_atoms;
+    const ulonglong2 *__restrict__ k_t = K + (int64_t)tpl * (bd.J + 1) * 4;
+    const int k_plane = bd.J + 1;
 
-    // ---- exact start of every row at column n0 ----------------------------------------------
-    // Rows outside the grid (and the idle lanes of the last warp) carry a dummy, perfectly
-    // conditioned state so that they stay on the fast path; nothing of theirs is stored.
-    u64 S[Q][4];
+    // ---- exact start of every row at columns n0, n0 + 1 -------------------------------------
+    // Rows outside the grid carry a dummy, perfectly conditioned state so that they stay on
+    // the fast path; nothing of theirs is stored.
+    u64 S[Q][8];
     bool rvalid[Q];
+    int n_first[Q];  // first column of the row with at least min_atoms atoms (n0 if none earlier)
     bool all_valid = true;
-    int n_valid_rows = 0;
+    int n_valid_rows = 0, n_slow_end = n0;
     const bool want_map = pr.out_maps != nullptr, want_flags = pr.out_flags != nullptr;
     const int64_t map_base = (int64_t)tpl * g.N_t0 * g.N_tau;
 #pragma unroll
     for (int b = 0; b < Q; ++b) {
-        const int m = mbase + b * r;
-        bool valid = active && m < g.N_t0;
+        const int m = min(mbase + b * roff, g.N_t0);
+        bool valid = m < g.N_t0;
         const int mc = min(m, g.N_t0 - 1);
         const int lo = __ldg(bd.lo + mc);
         const int64_t j0 = (int64_t)mc * bd.e_m + (int64_t)n0 * bd.e_n;
-        const int hi = max(__ldg(bd.edge + j0), lo);
+        const int hi0 = max(__ldg(bd.edge + j0), lo);
+        const int hi1 = max(__ldg(bd.edge + min(j0 + bd.e_n, (int64_t)bd.J - 1)), lo);
+        const int cnt_end =
+            max(__ldg(bd.edge + j0 + (int64_t)(n_end - 1 - n0) * bd.e_n), lo) - lo;
         // A row whose window still holds at most one atom (fewer than min_atoms) at the LAST
         // column of this tile is degenerate throughout: its cells are written here, directly,
         // and the row then runs as a dummy (rows at the end of the data or inside long gaps
         // would otherwise send every one of their cells through the fp64 path).
-        const int cnt_end =
-            max(__ldg(bd.edge + j0 + (int64_t)(n_end - 1 - n0) * bd.e_n), lo) - lo;
         if (valid && cnt_end <= 1 && cnt_end < pr.min_atoms) {
             uint32_t f1 = 3u;  // flags of a single-atom cell: bit 1 from the atom's own D in fp64
             if (cnt_end == 1) {
@@ -399,35 +461,66 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
             }
             valid = false;
         }
-        const Sums64 s = prefix_diff(P, lo, hi);
-        S[b][0] = valid ? pack2((float)s.A, (float)s.B) : pack2(1.0e15f, 1.0e15f);
-        S[b][1] = valid ? pack2((float)(kSqrt2 * s.far), (float)(kSqrt2 * s.fbr)) : 0ull;
-        S[b][2] = valid ? pack2((float)(kSqrt2 * s.fai), (float)(kSqrt2 * s.fbi)) : 0ull;
-        S[b][3] = valid ? pack2((float)s.C, (float)(hi - lo)) : pack2(0.0f, 1.0e9f);
+        // columns [n0, n_ok) hold fewer than min_atoms atoms (counts grow with n): fp64 path
+        int nk = n0;
+        if (valid && hi0 - lo < pr.min_atoms) {
+            int a = n0 + 1, e = n_end;  // first n in [a, e) with enough atoms, else n_end
+            while (a < e) {
+                const int mid = (a + e) >> 1;
+                const int c = max(__ldg(bd.edge + j0 + (int64_t)(mid - n0) * bd.e_n), lo) - lo;
+                if (c < pr.min_atoms) a = mid + 1;
+                else e = mid;
+            }
+            nk = a;
+        }
+        n_first[b] = nk;
+        n_slow_end = max(n_slow_end, nk);
+        const Sums64 s0 = prefix_diff(P, lo, hi0), s1 = prefix_diff(P, lo, hi1);
+        if (valid) {
+            S[b][0] = pack2((float)s0.A, (float)s1.A);
+            S[b][1] = pack2((float)s0.B, (float)s1.B);
+            S[b][2] = pack2((float)s0.C, (float)s1.C);
+            S[b][3] = pack2((float)-s0.C, (float)-s1.C);
+            S[b][4] = pack2((float)(kSqrt2 * s0.far), (float)(kSqrt2 * s1.far));
+            S[b][5] = pack2((float)(kSqrt2 * s0.fai), (float)(kSqrt2 * s1.fai));
+            S[b][6] = pack2((float)(kSqrt2 * s0.fbr), (float)(kSqrt2 * s1.fbr));
+            S[b][7] = pack2((float)(kSqrt2 * s0.fbi), (float)(kSqrt2 * s1.fbi));
+        } else {
+            S[b][0] = S[b][1] = pack2(1.0e15f, 1.0e15f);
+#pragma unroll
+            for (int ch = 2; ch < 8; ++ch) S[b][ch] = 0ull;
+        }
         rvalid[b] = valid;
         all_valid = all_valid && valid;
         n_valid_rows += valid ? 1 : 0;
-        if (active) s_rowm[b * NTu + lt] = valid ? m : -1;
+        s_rowm[b * kRunNT + lt] = valid ? m * g.N_tau : -1;  // element offset of the row
     }
 
-    // ---- sliding window of G: slot k % NS holds step k of row 0 (row b uses step k + b).  A
-    // slot is refilled right after row 0 has used it, i.e. NS - Q + 1 steps (at least Q - 1
-    // cells of work) before its next use, which hides the L1/L2 latency of the load.
+    // ---- sliding window of K: slot i % Q holds pair-step i of row 0; row b is b steps ahead
+    // (row m + b roff at column n sits on the lattice point of row m at column n + 2 b).  A
+    // slot is refilled right after row 0 has used it, one whole pair-step of the other rows
+    // before its next use, which hides the L1/L2 latency of the load.
     constexpr int NS = Q == 1 ? 2 : Q;
-    u64 W[NS][4];
+    u64 W[NS][8];
     // 32-bit lattice index (J <= 2^22); reads beyond the lattice are clamped to the zero entry J
+    const int jstep = 2 * bd.e_n;
     int jw = (int)min((int64_t)mbase * bd.e_m + (int64_t)n0 * bd.e_n, (int64_t)bd.J);
-    auto load_g = [&](u64(&w)[4]) {
-        const ulonglong2 *__restrict__ e = g_t + 2 * (int64_t)min(jw, bd.J);
-        const ulonglong2 a = __ldg(e), b2 = __ldg(e + 1);
-        w[0] = a.x;
-        w[1] = a.y;
-        w[2] = b2.x;
-        w[3] = b2.y;
-        jw = min(jw + bd.e_n, bd.J);
+    auto load_k = [&](u64(&w)[8]) {
+        const ulonglong2 *__restrict__ e = k_t + jw;
+        const ulonglong2 q0 = __ldg(e), q1 = __ldg(e + k_plane), q2 = __ldg(e + 2 * k_plane),
+                         q3 = __ldg(e + 3 * k_plane);
+        w[0] = q0.x;
+        w[1] = q0.y;
+        w[2] = q1.x;
+        w[3] = q1.y;
+        w[4] = q2.x;
+        w[5] = q2.y;
+        w[6] = q3.x;
+        w[7] = q3.y;
+        jw = min(jw + jstep, bd.J);
     };
 #pragma unroll
-    for (int k = 0; k < NS; ++k) load_g(W[k]);
+    for (int k = 0; k < NS; ++k) load_k(W[k]);
 
     RunMarg rm;
     rm.best = -INFINITY;
@@ -443,48 +536,37 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
         for (int c4 = 0; c4 < kChunk; c4 += 4) {
             const int left = ncols - c4;  // columns of this group inside the map (may be <= 0)
             if (left <= 0) break;
-            // ---- 4 columns x Q rows, straight-line fp32; cells that fail the conditioning
-            // test are only marked here and redone afterwards --------------------------------
+            // ---- 2 pair-steps (4 columns) x Q rows, straight-line packed fp32; cells that
+            // fail the conditioning test are only marked here and redone afterwards ----------
             float res[Q][4];
-            uint32_t slow = 0u;
+            bool fast = true;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
+            for (int s = 0; s < 2; ++s) {
 #pragma unroll
                 for (int b = 0; b < Q; ++b) {
-                    float A, B, far, fbr, fai, fbi, C, cnt;
-                    unpack2(S[b][0], A, B);
-                    unpack2(S[b][3], C, cnt);
-                    const float p = A * B;
-                    const float D = fmaf(-C, C, p);
-                    if (!(D > kCondFast * p && cnt >= min_atoms_f)) slow |= 1u << (b * 4 + s);
-                    u64 n2 = fmul2(S[b][1], S[b][1]);
-                    ffma2(n2, S[b][2], S[b][2]);
-                    float na, nb;
-                    unpack2(n2, na, nb);  // 2|Fa|^2, 2|Fb|^2
-                    unpack2(S[b][1], far, fbr);
-                    unpack2(S[b][2], fai, fbi);
-                    const float re = fmaf(fai, fbi, far * fbr);
-                    float num = B * na;
-                    num = fmaf(A, nb, num);
-                    num = fmaf(-2.0f * C, re, num);
-                    res[b][s] = num * rcp_approx(D);
-                    S[b][0] = fadd2(S[b][0], W[(s + b) % NS][0]);
-                    S[b][1] = fadd2(S[b][1], W[(s + b) % NS][1]);
-                    S[b][2] = fadd2(S[b][2], W[(s + b) % NS][2]);
-                    S[b][3] = fadd2(S[b][3], W[(s + b) % NS][3]);
-                    if (b == 0) load_g(W[s % NS]);
+                    const PairOut o = pair_closure(S[b]);
+                    unpack2(o.res, res[b][2 * s], res[b][2 * s + 1]);
+                    float t0, t1;
+                    unpack2(o.t, t0, t1);
+                    fast = fast && (t0 > 0.0f) && (t1 > 0.0f);
+#pragma unroll
+                    for (int ch = 0; ch < 8; ++ch)
+                        S[b][ch] = fadd2(S[b][ch], W[(s + b) % NS][ch]);
+                    if (b == 0) load_k(W[s % NS]);
                 }
             }
             uint32_t fw[Q];
 #pragma unroll
             for (int b = 0; b < Q; ++b) fw[b] = 0u;
-            if (slow) {  // rare
+            if (!fast || n + c4 < n_slow_end) {
+                // rare (a few hundred warps per million cells): every cell of the group is
+                // redone the plain way, in fp64 from the prefix sums
 #pragma unroll
                 for (int b = 0; b < Q; ++b) {
 #pragma unroll
                     for (int s = 0; s < 4; ++s) {
-                        if (((slow >> (b * 4 + s)) & 1u) && s < left && rvalid[b]) {
-                            const int m = mbase + b * r;
+                        if (s < left && rvalid[b]) {
+                            const int m = mbase + b * roff;
                             const int64_t j =
                                 (int64_t)m * bd.e_m + (int64_t)(n + c4 + s) * bd.e_n;
                             float twoF, flf;
@@ -496,14 +578,13 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
                     }
                 }
             }
-            if (active) {
 #pragma unroll
-                for (int b = 0; b < Q; ++b) {
-                    if (want_map)
-                        *reinterpret_cast<float4 *>(tile + (size_t)(b * NTu + lt) * kPitch + c4) =
-                            make_float4(res[b][0], res[b][1], res[b][2], res[b][3]);
-                    if (want_flags) ftile[(b * NTu + lt) * kFPitch + (c4 >> 2)] = fw[b];
-                }
+            for (int b = 0; b < Q; ++b) {
+                if (want_map)
+                    *reinterpret_cast<float4 *>(tile + (size_t)(b * kRunNT + lt) * kPitch +
+                                                4 * ((c4 >> 2) ^ ((lt >> 1) & 3))) =
+                        make_float4(res[b][0], res[b][1], res[b][2], res[b][3]);
+                if (want_flags) ftile[(b * kRunNT + lt) * kFPitch + (c4 >> 2)] = fw[b];
             }
             if (MARG && n_valid_rows > 0) {
                 uint32_t any_fl = 0u;
@@ -539,7 +620,7 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
                             for (int s = 0; s < 4; ++s)
                                 if (!found && res[b][s] == gmax) {
                                     found = true;
-                                    rm.idx = (mbase + b * r) * g.N_tau + n + c4 + s;
+                                    rm.idx = (mbase + b * roff) * g.N_tau + n + c4 + s;
                                 }
                         rm.best = gmax;
                     }
@@ -560,29 +641,31 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
         }
         if (want_map && !want_flags && vec_ok && ncols == kChunk) {  // the common, lean case
             __syncthreads();
+            // 4 threads write the 64 bytes of one row; kRunNT / 4 rows per pass, all with the
+            // same (row >> 1) & 3, so the swizzled word of a thread is the same in every pass
             float *__restrict__ dst = pr.out_maps + map_base + n + 4 * (threadIdx.x & 3);
-            const float4 *__restrict__ src =
-                reinterpret_cast<const float4 *>(tile) + (threadIdx.x & 3);
+            const float4 *__restrict__ src = reinterpret_cast<const float4 *>(tile) +
+                                             ((threadIdx.x & 3) ^ ((threadIdx.x >> 3) & 3));
 #pragma unroll 4
             for (int row = threadIdx.x >> 2; row < nrows; row += kRunNT / 4) {
-                const int m = s_rowm[row];
-                if (m >= 0)
-                    __stcs(reinterpret_cast<float4 *>(dst + (int64_t)m * g.N_tau),
-                           src[row * (kPitch / 4)]);
+                const int off = s_rowm[row];
+                const float4 v = src[row * (kPitch / 4)];
+                if (off >= 0) __stcs(reinterpret_cast<float4 *>(dst + off), v);
             }
             __syncthreads();
         } else if (want_map || want_flags) {
             __syncthreads();
             const int q4 = threadIdx.x & 3;
             for (int row = threadIdx.x >> 2; row < nrows; row += kRunNT / 4) {
-                const int m = s_rowm[row];
-                if (m < 0) continue;
-                const int64_t o = map_base + (int64_t)m * g.N_tau + n + 4 * q4;
+                const int off = s_rowm[row];
+                if (off < 0) continue;
+                const int64_t o = map_base + off + n + 4 * q4;
                 const int left = ncols - 4 * q4;
                 if (left <= 0) continue;
                 if (want_map) {
                     const float4 v =
-                        *reinterpret_cast<const float4 *>(tile + (size_t)row * kPitch + 4 * q4);
+                        *reinterpret_cast<const float4 *>(tile + (size_t)row * kPitch +
+                                                          4 * (q4 ^ ((row >> 1) & 3)));
                     if (vec_ok && left >= 4) {
                         __stcs(reinterpret_cast<float4 *>(pr.out_maps + o), v);
                     } else {
@@ -625,11 +708,12 @@ __global__ void __launch_bounds__(kRunNT, Q == 4 ? 4 : Q == 2 ? 6 : 5)
 
 template <int Q>
 cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
-                       const ulonglong2 *G, Partial *partials, cudaStream_t st)
+                       const ulonglong2 *K, Partial *partials, cudaStream_t st)
 {
     const RectRun &rr = pl.rect;
-    const int nrows = Q * rr.NTu;
-    const size_t smem = (size_t)nrows * (kPitch * 4 + 4 + kFPitch * 4);
+    const int nrows = Q * kRunNT;
+    // the flag tile is only there when flags are asked for: shared memory not taken is L1
+    const size_t smem = (size_t)nrows * (kPitch * 4 + 4 + (pr.out_flags ? kFPitch * 4 : 0));
     const int64_t cells = (int64_t)pl.grid.N_t0 * pl.grid.N_tau;
     const bool vec = (pl.grid.N_tau % 4 == 0) && (cells % 4 == 0) &&
                      ((reinterpret_cast<uintptr_t>(pr.out_maps) & 15u) == 0) &&
@@ -641,14 +725,14 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         rect_run_kernel<Q, true><<<(unsigned)n_ctas, kRunNT, smem, st>>>(
-            pr, prefix, G, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
+            pr, prefix, K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
             vec ? 1 : 0);
     } else {
         e = cudaFuncSetAttribute(rect_run_kernel<Q, false>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         rect_run_kernel<Q, false><<<(unsigned)n_ctas, kRunNT, smem, st>>>(
-            pr, prefix, G, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
+            pr, prefix, K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
             vec ? 1 : 0);
     }
     return cudaGetLastError();
@@ -658,50 +742,51 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
 
 // Tile shapes of the running-sum kernel; called by make_plan (api.cu).
 RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates,
-                      int32_t q_override)
+                      int32_t q_override, int32_t seg_override)
 {
     RectRun rr;
     rr.enabled = (J > 0 && g.N_t0 >= 8) ? 1 : 0;
     rr.Q = 1;
     rr.r = 1;
-    if (e_m > 0 && e_n > 0 && e_n % e_m == 0) {
-        const int r = e_n / e_m;
-        // Q = 2 measured best on B200 (config 5): 80 registers, 6 CTAs per SM; Q = 4 halves
-        // the G traffic again but runs at 4 CTAs per SM
-        if (r >= 8 && g.N_t0 >= 2 * r) {
+    // Row m + roff, roff = 2 e_n / e_m, sits at column n on the lattice point that row m
+    // reaches two columns (one pair-step) later: a thread that owns both loads every K entry
+    // once for two rows.
+    if (e_m > 0 && e_n > 0 && (2 * (int64_t)e_n) % e_m == 0 && q_override != 1) {
+        const int64_t roff = 2 * (int64_t)e_n / e_m;
+        if (g.N_t0 >= 2 * roff) {
             rr.Q = 2;
-            rr.r = r;
-        }
-        if (q_override == 4 && r >= 8 && g.N_t0 >= 4 * r) {
-            rr.Q = 4;
-            rr.r = r;
-        }
-        if (q_override == 1) {
-            rr.Q = 1;
-            rr.r = 1;
+            rr.r = (int32_t)roff;
         }
     }
-    rr.NTu = (rr.Q > 1 && rr.r < kRunNT) ? (kRunNT / rr.r) * rr.r : kRunNT;
-    const int64_t units =
-        rr.Q > 1 ? ((int64_t)g.N_t0 + (int64_t)rr.r * rr.Q - 1) / ((int64_t)rr.r * rr.Q) * rr.r
-                 : g.N_t0;
-    rr.n_rowtiles = (int32_t)((units + rr.NTu - 1) / rr.NTu);
-    // columns per CTA: whole waves of 148 SMs x 4 resident CTAs; a row start costs about as
-    // much as 12 cells
+    // NTu = R: residues per CTA (a power of two <= 16, so that a warp still reads K in runs of
+    // at least min(roff, 16) x 16 bytes); the CTA's other lanes hold the following groups
+    int R = 16;
+    while (R > rr.r) R >>= 1;
+    rr.NTu = rr.Q > 1 ? R : kRunNT;
+    if (rr.Q > 1) {
+        const int64_t groups = ((int64_t)g.N_t0 + (int64_t)rr.r * rr.Q - 1) / ((int64_t)rr.r * rr.Q);
+        const int64_t gpc = kRunNT / R;
+        rr.n_rowtiles = (int32_t)(((rr.r + R - 1) / R) * ((groups + gpc - 1) / gpc));
+    } else {
+        rr.n_rowtiles = (int32_t)(((int64_t)g.N_t0 + kRunNT - 1) / kRunNT);
+    }
+    // columns per CTA: whole waves of 148 SMs x resident CTAs; a row start costs about as
+    // much as 24 cells
     const int seg_max = (g.N_tau + kChunk - 1) / kChunk * kChunk;
     int seg = seg_max;
     int64_t best_cost = INT64_MAX;
     for (int cand = seg_max; cand >= kChunk; cand -= kChunk) {
         const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
-        const int64_t per_wave = 148 * (rr.Q == 4 ? 4 : rr.Q == 2 ? 6 : 5);
+        const int64_t per_wave = 148 * (rr.Q == 2 ? 4 : 5);
         const int64_t waves = (ctas + per_wave - 1) / per_wave;
-        const int64_t cost = waves * (cand + 12);
+        const int64_t cost = waves * (cand + 24);
         if (cost < best_cost) {
             best_cost = cost;
             seg = cand;
         }
         if (ctas >= (int64_t)148 * 4 * 64) break;  // many waves: quantisation no longer matters
     }
+    if (seg_override > 0) seg = std::min(seg_max, (seg_override + kChunk - 1) / kChunk * kChunk);
     rr.seg_cols = seg;
     rr.n_coltiles = (g.N_tau + seg - 1) / seg;
     return rr;
@@ -716,10 +801,10 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
     // run_device memsets them when the bounds of an earlier call are reused
     const int nblk = rect_scan_blocks(pl.n_atoms);
     const int n_scan = nblk * pl.n_templates;
-    ulonglong2 *G = static_cast<ulonglong2 *>(steps);
+    ulonglong2 *K = static_cast<ulonglong2 *>(steps);
     const int spt = pl.rect.enabled ? (int)((pl.J + 1 + kScanNT - 1) / kScanNT) : 0;
     const int64_t n_blocks = (int64_t)n_scan + (int64_t)spt * pl.n_templates;
-    rect_scan_kernel<<<(unsigned)n_blocks, kScanNT, 0, st>>>(pr, agg, flags, prefix, G, nblk,
+    rect_scan_kernel<<<(unsigned)n_blocks, kScanNT, 0, st>>>(pr, agg, flags, prefix, K, nblk,
                                                              n_scan, spt);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -729,9 +814,8 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
                                                                 pl.cell_blocks_per_template);
         return cudaGetLastError();
     }
-    if (pl.rect.Q == 4) return launch_run<4>(pl, pr, prefix, G, partials, st);
-    if (pl.rect.Q == 2) return launch_run<2>(pl, pr, prefix, G, partials, st);
-    return launch_run<1>(pl, pr, prefix, G, partials, st);
+    if (pl.rect.Q == 2) return launch_run<2>(pl, pr, prefix, K, partials, st);
+    return launch_run<1>(pl, pr, prefix, K, partials, st);
 }
 
 }  // namespace tfstat
