@@ -67,6 +67,18 @@ __device__ __forceinline__ void wait_flag(const int32_t *p)
     asm volatile("fence.acq_rel.gpu;" ::: "memory");
 }
 
+__device__ __forceinline__ void wait_flags2(const int32_t *p, const int32_t *q)
+{
+    int32_t v, w;
+    for (;;) {
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(w) : "l"(q) : "memory");
+        if (v != 0 && w != 0) break;
+        __nanosleep(64);
+    }
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+}
+
 // window sums of atoms [lo, hi) from the prefix, in fp64; L2 loads (P may have been written by
 // another SM during this very launch)
 __device__ __forceinline__ Sums64 prefix_diff_cg(const double2 *P, const int lo, const int hi)
@@ -88,6 +100,8 @@ __device__ __forceinline__ Sums64 prefix_diff_cg(const double2 *P, const int lo,
 
 // The running Fa, Fb sums are carried scaled by sqrt(2), so eq. (7) on them yields 2F directly.
 constexpr double kSqrt2 = 1.41421356237309504880;
+constexpr int kStepSplit = 4;                    // threads per lattice point (step role)
+constexpr int kStepPts = kScanNT / kStepSplit;   // lattice points per step CTA
 constexpr int kDirectStep = 64;    // lattice steps of at most this many atoms are summed directly
 
 // P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.
@@ -106,57 +120,68 @@ __global__ void __launch_bounds__(kScanNT)
     int32_t *ready = flags, *done = flags + n_scan;
 
     if ((int)blockIdx.x >= n_scan) {  // ---- step role ------------------------------------
+        // kStepSplit threads per lattice point j share the sum H[j] of the atoms in
+        // [edge[j], edge[j + 2 e_n]): what a row gains when it moves on by two columns.  H[j] is
+        // the first half of the pairs of K[j] and the second half of the pairs of K[j - e_n].
         const int sb = blockIdx.x - n_scan;
         const int tpl = sb / steps_per_template;
-        const int j = (sb % steps_per_template) * kScanNT + threadIdx.x;
-        if (j > bd.J) return;
-        // K[j] = (H[j], H[j + e_n]), H[i] = sums of the atoms in [edge[i], edge[i + 2 e_n]):
-        // what the column PAIR (n, n+1) of a row gains when it moves on to (n+2, n+3)
-        Sums64 h[2];
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            h[q].A = h[q].B = h[q].C = h[q].far = h[q].fai = h[q].fbr = h[q].fbi = 0.0;
-            const int64_t ja = (int64_t)j + (int64_t)q * bd.e_n, jb = ja + 2 * (int64_t)bd.e_n;
-            if (jb >= bd.J) continue;  // beyond the lattice: only cells outside the map use it
-            const int a = __ldg(bd.edge + ja), b = __ldg(bd.edge + jb);
-            if (b - a <= kDirectStep) {
-                // short step: sum its atoms directly (fp64), independent of the scan blocks
-                const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
-                double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-#pragma unroll 4
-                for (int al = a; al < b; ++al) {
-#pragma unroll
-                    for (int ch = 0; ch < 7; ++ch) acc[ch] += (double)__ldg(base + ch * pr.ld + al);
-                }
-                h[q].A = acc[0];
-                h[q].B = acc[1];
-                h[q].C = acc[2];
-                h[q].far = acc[3];
-                h[q].fai = acc[4];
-                h[q].fbr = acc[5];
-                h[q].fbi = acc[6];
-            } else {
-                const int32_t *da = done + tpl * nblk + max(a - 1, 0) / kScanBlock;
-                const int32_t *db = done + tpl * nblk + max(b - 1, 0) / kScanBlock;
-                wait_flag(db);  // scan blocks finish roughly in order: the later one first
-                wait_flag(da);
-                const double2 *P =
-                    reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (N + 1) * 8);
-                h[q] = prefix_diff_cg(P, a, b);
-            }
+        const int j = (sb % steps_per_template) * kStepPts + (int)threadIdx.x / kStepSplit;
+        const int sub = threadIdx.x % kStepSplit;
+        // the kStepSplit lanes of a lattice point branch together, the warp need not
+        const unsigned grp_mask = ((1u << kStepSplit) - 1u) << ((threadIdx.x & 31) - sub);
+        const int64_t jb = (int64_t)j + 2 * (int64_t)bd.e_n;
+        const bool in_lattice = jb < bd.J;  // beyond: only cells outside the map would use it
+        double acc[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        int a = 0, b = 0;
+        if (in_lattice) {
+            a = __ldg(bd.edge + j);
+            b = __ldg(bd.edge + jb);
         }
+        if (b - a <= kDirectStep) {
+            // short step: sum its atoms directly (fp64), independent of the scan blocks
+            const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+#pragma unroll 2
+            for (int al = a + sub; al < b; al += kStepSplit) {
+#pragma unroll
+                for (int ch = 0; ch < 7; ++ch) acc[ch] += (double)__ldg(base + ch * pr.ld + al);
+            }
+#pragma unroll
+            for (int ch = 0; ch < 7; ++ch)
+#pragma unroll
+                for (int sh = 1; sh < kStepSplit; sh <<= 1)
+                    acc[ch] += __shfl_xor_sync(grp_mask, acc[ch], sh);
+        } else {  // whole groups of kStepSplit lanes take this branch together
+            const int32_t *da = done + tpl * nblk + max(a - 1, 0) / kScanBlock;
+            const int32_t *db = done + tpl * nblk + max(b - 1, 0) / kScanBlock;
+            wait_flags2(db, da);  // scan blocks finish roughly in order: the later one first
+            const double2 *P =
+                reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (N + 1) * 8);
+            const Sums64 h = prefix_diff_cg(P, a, b);
+            acc[0] = h.A;
+            acc[1] = h.B;
+            acc[2] = h.C;
+            acc[3] = h.far;
+            acc[4] = h.fai;
+            acc[5] = h.fbr;
+            acc[6] = h.fbi;
+        }
+        if (sub != 0 || j > bd.J) return;
         // planar: plane q of template tpl holds J + 1 16-byte elements, so that the lanes of a
         // warp (consecutive rows = consecutive j) read consecutive 16-byte words
-        ulonglong2 *__restrict__ o = K + (int64_t)tpl * 4 * (bd.J + 1) + j;
         const int64_t pl = (int64_t)bd.J + 1;
-        o[0] = make_ulonglong2(pack2((float)h[0].A, (float)h[1].A),
-                               pack2((float)h[0].B, (float)h[1].B));
-        o[pl] = make_ulonglong2(pack2((float)h[0].C, (float)h[1].C),
-                               pack2((float)-h[0].C, (float)-h[1].C));
-        o[2 * pl] = make_ulonglong2(pack2((float)(kSqrt2 * h[0].far), (float)(kSqrt2 * h[1].far)),
-                               pack2((float)(kSqrt2 * h[0].fai), (float)(kSqrt2 * h[1].fai)));
-        o[3 * pl] = make_ulonglong2(pack2((float)(kSqrt2 * h[0].fbr), (float)(kSqrt2 * h[1].fbr)),
-                               pack2((float)(kSqrt2 * h[0].fbi), (float)(kSqrt2 * h[1].fbi)));
+        float *__restrict__ kf = reinterpret_cast<float *>(K + (int64_t)tpl * 4 * pl);
+        const float v[8] = {(float)acc[0], (float)acc[1], (float)acc[2], (float)-acc[2],
+                            (float)(kSqrt2 * acc[3]), (float)(kSqrt2 * acc[4]),
+                            (float)(kSqrt2 * acc[5]), (float)(kSqrt2 * acc[6])};
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            // channel c lives in plane c / 2, 8-byte pair c % 2 of the 16-byte element
+            float *__restrict__ e = kf + ((int64_t)(c >> 1) * pl) * 4 + (c & 1) * 2;
+            e[(int64_t)j * 4] = v[c];                                // first of the pair of K[j]
+            if (j >= bd.e_n) e[((int64_t)j - bd.e_n) * 4 + 1] = v[c];  // second of K[j - e_n]
+            // K[j]'s second halves for j > J - e_n belong to H beyond the lattice: zero
+            if (j + bd.e_n > bd.J) e[(int64_t)j * 4 + 1] = 0.0f;
+        }
         return;
     }
 
@@ -205,11 +230,25 @@ __global__ void __launch_bounds__(kScanNT)
         }
         // offset of this block: warp ch sums the totals of blocks [0, blk) of this template
         if (warp < 7) {
-            double t = 0.0;
-            for (int b = lane; b < blk; b += 32) {
-                wait_flag(ready + tpl * nblk + b);
-                t += __ldcg(agg + ((int64_t)tpl * nblk + b) * 8 + warp);
+            // all lanes poll their flags together and the warp takes ONE acquire fence: a
+            // wait_flag per lane would diverge and serialise up to 32 fences
+            for (int b0 = 0; b0 < blk; b0 += 32) {
+                const int b = b0 + lane;
+                for (;;) {
+                    int32_t v = 1;
+                    if (b < blk)
+                        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];"
+                                     : "=r"(v)
+                                     : "l"(ready + tpl * nblk + b)
+                                     : "memory");
+                    if (__all_sync(0xffffffffu, v != 0)) break;
+                    __nanosleep(32);
+                }
             }
+            asm volatile("fence.acq_rel.gpu;" ::: "memory");
+            double t = 0.0;
+            for (int b = lane; b < blk; b += 32)
+                t += __ldcg(agg + ((int64_t)tpl * nblk + b) * 8 + warp);
 #pragma unroll
             for (int sh = 16; sh >= 1; sh >>= 1) t += __shfl_xor_sync(0xffffffffu, t, sh);
             if (lane == 0) s_off[warp] = t;
@@ -802,7 +841,7 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
     const int nblk = rect_scan_blocks(pl.n_atoms);
     const int n_scan = nblk * pl.n_templates;
     ulonglong2 *K = static_cast<ulonglong2 *>(steps);
-    const int spt = pl.rect.enabled ? (int)((pl.J + 1 + kScanNT - 1) / kScanNT) : 0;
+    const int spt = pl.rect.enabled ? (int)((pl.J + 1 + kStepPts - 1) / kStepPts) : 0;
     const int64_t n_blocks = (int64_t)n_scan + (int64_t)spt * pl.n_templates;
     rect_scan_kernel<<<(unsigned)n_blocks, kScanNT, 0, st>>>(pr, agg, flags, prefix, K, nblk,
                                                              n_scan, spt);
