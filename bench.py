@@ -337,9 +337,14 @@ def run_ours(args):
     if dist:
         dist.barrier()
     t0 = time.perf_counter()
+    e2e_each = []
     for _ in range(args.steps):
+        t1 = time.perf_counter()
         res_host, _ = pkg.tfstat_search_host(atoms_h, t_h, pkg.EXP, grid)
+        e2e_each.append((time.perf_counter() - t1) * 1e3)
     e2e_s = (time.perf_counter() - t0) / args.steps
+    if os.environ.get("TFSTAT_BENCH_VERBOSE"):
+        print("e2e ms per call:", [round(x, 1) for x in e2e_each], file=sys.stderr)
     if dist:
         tt = torch.tensor([e2e_s], device="cuda")
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)

@@ -149,16 +149,29 @@ int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int3
 /* tfstat_search on host memory: copies atoms host->device in template chunks on internal
  * streams (overlapped with compute), runs the fused search, copies results (and maps, if
  * asked) device->host, and returns after everything has completed.  Host buffers should be
- * page-locked for the copies to overlap.  Allocates its own device memory (cudaMalloc) and
- * frees it before returning; `max_device_bytes` bounds that (0 = 2 GiB).
+ * page-locked for the copies to overlap.  This is the paper's per-template copy-in / kernel /
+ * copy-out without the per-template round trip.
  *   atoms_host, t_atoms_host, out_host, out_maps_host (nullable): HOST pointers, layouts as
- *   in tfstat_search.                                                                      */
+ *   in tfstat_search.
+ *   device_scratch: DEVICE buffer of device_scratch_bytes bytes (256-B aligned) that holds the
+ *   double-buffered chunks, the workspace and the results.  Any size from one template's worth
+ *   up works (smaller => more, smaller chunks); tfstat_search_host_scratch_bytes() gives the
+ *   size at which chunks are the preferred 256 templates.  NULL: the library cudaMallocs up to
+ *   device_scratch_bytes (0 = 2 GiB) itself and frees it before returning -- convenient, but
+ *   cudaFree can stall for ~100 ms, so callers in a loop should pass their own buffer.
+ *   Errors: TFSTAT_EWORKSPACE if a given scratch is misaligned or too small for one template. */
 int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t ld,
                        const int32_t *t_atoms_host, int32_t n_atoms, int32_t n_templates,
                        int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
                        int32_t dtau, int32_t N_tau, tfstat_result *out_host,
-                       float *out_maps_host, size_t max_device_bytes,
+                       float *out_maps_host, void *device_scratch, size_t device_scratch_bytes,
                        const tfstat_opts *opts_host);
+/* Host-only: scratch size for chunks of min(n_templates, 256) templates; 0 on invalid input. */
+size_t tfstat_search_host_scratch_bytes(int64_t template_stride, int32_t n_atoms,
+                                        int32_t n_templates, int window, int32_t t0_min,
+                                        int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                                        int32_t N_tau, int want_maps,
+                                        const tfstat_opts *opts_host);
 
 #ifdef __cplusplus
 }

@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     lib_path,
     load_library,
     probe_alu,
+    search_host_scratch_bytes,
     tfstat_map,
     tfstat_marginalise,
     tfstat_search,

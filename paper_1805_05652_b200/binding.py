@@ -67,7 +67,9 @@ def load_library():
         vp, vp, vp, vp, sz, vp, op]
     lib.tfstat_count_terms.argtypes = [vp, i32, C.c_int] + grid + [vp, vp, sz, vp]
     lib.tfstat_search_host.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
-        vp, vp, sz, op]
+        vp, vp, vp, sz, op]
+    lib.tfstat_search_host_scratch_bytes.restype = sz
+    lib.tfstat_search_host_scratch_bytes.argtypes = [i64, i32, i32, C.c_int] + grid + [C.c_int, op]
     lib.tfstat_probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
     _lib = lib
@@ -256,11 +258,34 @@ def count_terms(t_atoms: torch.Tensor, window: int, grid, *, stream=None) -> int
     return int(out.item())
 
 
+_host_scratch: Optional[torch.Tensor] = None  # device scratch reused by tfstat_search_host
+
+
+def search_host_scratch_bytes(template_stride: int, n_atoms: int, n_templates: int, window: int,
+                              grid, *, want_maps: bool = False, min_atoms: int = 2,
+                              exp_method: int = EXP_AUTO) -> int:
+    """Device scratch tfstat_search_host wants for chunks of min(n_templates, 256) templates."""
+    lib = load_library()
+    o = _opts(min_atoms, exp_method)
+    n = int(lib.tfstat_search_host_scratch_bytes(int(template_stride), n_atoms, n_templates,
+                                                 window, *_grid_args(grid), int(want_maps),
+                                                 C.byref(o)))
+    if n == 0:
+        raise TfstatError("tfstat_search_host_scratch_bytes: invalid problem shape")
+    return n
+
+
 def tfstat_search_host(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
                        min_atoms: int = 2, exp_method: int = EXP_AUTO, want_maps: bool = False,
-                       max_device_bytes: int = 0):
+                       max_device_bytes: int = 0, scratch: Optional[torch.Tensor] = None,
+                       library_malloc: bool = False):
     """End-to-end call on HOST tensors (pinned for overlap): H2D copies, fused search and D2H
-    of the results all happen inside the library.  Returns (results ndarray, maps or None)."""
+    of the results all happen inside the library.  Returns (results ndarray, maps or None).
+
+    The device scratch buffer is a torch tensor kept between calls (or `scratch`, a CUDA uint8
+    tensor of the caller); `max_device_bytes` > 0 caps its size (smaller chunks);
+    `library_malloc` passes no scratch at all: the library cudaMallocs and frees its own."""
+    global _host_scratch
     lib = load_library()
     if atoms.is_cuda or t_atoms.is_cuda:
         raise TfstatError("tfstat_search_host takes host (CPU) tensors")
@@ -273,10 +298,34 @@ def tfstat_search_host(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, 
     maps = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.float32).pin_memory()
             if want_maps else None)
     o = _opts(min_atoms, exp_method)
+    if library_malloc:
+        rc = lib.tfstat_search_host(atoms.data_ptr(), int(atoms.stride(0)), int(atoms.stride(1)),
+                                    t_atoms.data_ptr(), n_atoms, T, window, *_grid_args(grid),
+                                    out.data_ptr(),
+                                    maps.data_ptr() if maps is not None else None, None,
+                                    int(max_device_bytes), C.byref(o))
+        _check(rc, "tfstat_search_host")
+        return out.numpy().view(RESULT_DTYPE).reshape(-1), maps
+    if scratch is None:
+        need = int(lib.tfstat_search_host_scratch_bytes(int(atoms.stride(0)), n_atoms, T, window,
+                                                        *_grid_args(grid), int(want_maps),
+                                                        C.byref(o)))
+        if need == 0:
+            raise TfstatError("tfstat_search_host_scratch_bytes: invalid problem shape")
+        if max_device_bytes:
+            need = min(need, int(max_device_bytes))
+        if _host_scratch is None or _host_scratch.numel() < need:
+            _host_scratch = None
+            _host_scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
+        scratch, nbytes = _host_scratch, need
+    else:
+        if not (scratch.is_cuda and scratch.dtype == torch.uint8 and scratch.is_contiguous()):
+            raise TfstatError("scratch must be a contiguous CUDA uint8 tensor")
+        nbytes = scratch.numel()
     rc = lib.tfstat_search_host(atoms.data_ptr(), int(atoms.stride(0)), int(atoms.stride(1)),
                                 t_atoms.data_ptr(), n_atoms, T, window, *_grid_args(grid),
                                 out.data_ptr(), maps.data_ptr() if maps is not None else None,
-                                int(max_device_bytes), C.byref(o))
+                                scratch.data_ptr(), nbytes, C.byref(o))
     _check(rc, "tfstat_search_host")
     return out.numpy().view(RESULT_DTYPE).reshape(-1), maps
 

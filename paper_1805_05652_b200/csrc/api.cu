@@ -297,32 +297,37 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
                        const int32_t *t_atoms_host, int32_t n_atoms, int32_t n_templates,
                        int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
                        int32_t dtau, int32_t N_tau, tfstat_result *out_host,
-                       float *out_maps_host, size_t max_device_bytes,
+                       float *out_maps_host, void *device_scratch, size_t device_scratch_bytes,
                        const tfstat_opts *opts_host)
 {
     if (!atoms_host || !t_atoms_host || !out_host) return TFSTAT_EINVAL;
     if (ld < n_atoms || (n_templates > 1 && template_stride < 7 * ld)) return TFSTAT_EINVAL;
     if (n_templates < 1) return TFSTAT_EINVAL;
-    if (max_device_bytes == 0) max_device_bytes = size_t(2) << 30;
+    if (device_scratch && (reinterpret_cast<uintptr_t>(device_scratch) & (kAlign - 1)))
+        return TFSTAT_EWORKSPACE;
+    const size_t budget = device_scratch_bytes ? device_scratch_bytes : size_t(2) << 30;
     const int64_t cells = (int64_t)N_t0 * N_tau;
-    // templates per chunk: two atom buffers (+ two map buffers) + workspace within the budget
+    // device layout: two atom buffers (+ two map buffers) of Tc templates, workspace, time
+    // stamps, results; Tc = templates per chunk, the largest that fits the budget
     const size_t tpl_bytes = sizeof(float) * (size_t)template_stride;
     const size_t map_bytes = out_maps_host ? sizeof(float) * (size_t)cells : 0;
+    const size_t t_bytes = align_up(sizeof(int32_t) * (size_t)n_atoms);
+    const size_t out_bytes = align_up(sizeof(tfstat_result) * (size_t)n_templates);
     int32_t Tc = std::min<int32_t>(n_templates, 256);
     Plan pl;
+    size_t need = 0;
     for (;; Tc = (Tc + 1) / 2) {
         pl = make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts_host);
         if (pl.status != TFSTAT_OK) return pl.status;
-        const size_t need = 2 * Tc * (tpl_bytes + map_bytes) + pl.bytes;
-        if (need <= max_device_bytes || Tc == 1) break;
+        need = 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) +
+               align_up(std::max(pl.bytes, kAlign)) + t_bytes + out_bytes;
+        if (need <= budget || Tc == 1) break;
     }
+    if (device_scratch && need > budget) return TFSTAT_EWORKSPACE;
     const int n_chunks = (n_templates + Tc - 1) / Tc;
 
-    char *d_atoms[2] = {nullptr, nullptr};
-    float *d_maps[2] = {nullptr, nullptr};
-    void *d_ws = nullptr;
-    int32_t *d_t = nullptr;
-    tfstat_result *d_out = nullptr;
+    char *base = static_cast<char *>(device_scratch);
+    bool own = false;
     cudaStream_t s_copy = nullptr, s_comp = nullptr, s_back = nullptr;
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr},
                 ev_back[2] = {nullptr, nullptr};
@@ -332,21 +337,36 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
         return e == cudaSuccess;
     };
     do {
+        if (!base) {
+            if (!chk(cudaMalloc(&base, need))) break;
+            own = true;
+        }
+        size_t off = 0;
+        auto carve = [&](size_t n) {
+            char *q = base + off;
+            off += align_up(n);
+            return q;
+        };
+        char *d_atoms[2] = {carve(Tc * tpl_bytes), carve(Tc * tpl_bytes)};
+        float *d_maps[2] = {nullptr, nullptr};
+        if (map_bytes)
+            for (int b = 0; b < 2; ++b) d_maps[b] = reinterpret_cast<float *>(carve(Tc * map_bytes));
+        void *d_ws = carve(std::max(pl.bytes, kAlign));
+        int32_t *d_t = reinterpret_cast<int32_t *>(carve(sizeof(int32_t) * (size_t)n_atoms));
+        tfstat_result *d_out =
+            reinterpret_cast<tfstat_result *>(carve(sizeof(tfstat_result) * (size_t)n_templates));
+
         if (!chk(cudaStreamCreateWithFlags(&s_copy, cudaStreamNonBlocking))) break;
         if (!chk(cudaStreamCreateWithFlags(&s_comp, cudaStreamNonBlocking))) break;
-        if (!chk(cudaStreamCreateWithFlags(&s_back, cudaStreamNonBlocking))) break;
+        if (map_bytes && !chk(cudaStreamCreateWithFlags(&s_back, cudaStreamNonBlocking))) break;
         bool ok = true;
         for (int b = 0; b < 2 && ok; ++b) {
-            ok = chk(cudaMalloc(&d_atoms[b], Tc * tpl_bytes)) &&
-                 chk(cudaEventCreateWithFlags(&ev_in[b], cudaEventDisableTiming)) &&
-                 chk(cudaEventCreateWithFlags(&ev_done[b], cudaEventDisableTiming)) &&
-                 chk(cudaEventCreateWithFlags(&ev_back[b], cudaEventDisableTiming));
-            if (ok && map_bytes) ok = chk(cudaMalloc(&d_maps[b], Tc * map_bytes));
+            ok = chk(cudaEventCreateWithFlags(&ev_in[b], cudaEventDisableTiming)) &&
+                 chk(cudaEventCreateWithFlags(&ev_done[b], cudaEventDisableTiming));
+            if (ok && map_bytes)
+                ok = chk(cudaEventCreateWithFlags(&ev_back[b], cudaEventDisableTiming));
         }
         if (!ok) break;
-        if (!chk(cudaMalloc(&d_ws, std::max(pl.bytes, kAlign)))) break;
-        if (!chk(cudaMalloc(&d_t, sizeof(int32_t) * (size_t)n_atoms))) break;
-        if (!chk(cudaMalloc(&d_out, sizeof(tfstat_result) * (size_t)n_templates))) break;
         if (!chk(cudaMemcpyAsync(d_t, t_atoms_host, sizeof(int32_t) * (size_t)n_atoms,
                                  cudaMemcpyHostToDevice, s_comp)))
             break;
@@ -383,26 +403,38 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
         if (rc != TFSTAT_OK) break;
         chk(cudaMemcpyAsync(out_host, d_out, sizeof(tfstat_result) * (size_t)n_templates,
                             cudaMemcpyDeviceToHost, s_comp));
-        chk(cudaStreamSynchronize(s_comp));
-        chk(cudaStreamSynchronize(s_back));
     } while (0);
     if (s_copy) cudaStreamSynchronize(s_copy);
     if (s_comp) cudaStreamSynchronize(s_comp);
     if (s_back) cudaStreamSynchronize(s_back);
     for (int b = 0; b < 2; ++b) {
-        cudaFree(d_atoms[b]);
-        cudaFree(d_maps[b]);
         if (ev_in[b]) cudaEventDestroy(ev_in[b]);
         if (ev_done[b]) cudaEventDestroy(ev_done[b]);
         if (ev_back[b]) cudaEventDestroy(ev_back[b]);
     }
-    cudaFree(d_ws);
-    cudaFree(d_t);
-    cudaFree(d_out);
     if (s_copy) cudaStreamDestroy(s_copy);
     if (s_comp) cudaStreamDestroy(s_comp);
     if (s_back) cudaStreamDestroy(s_back);
+    if (own) cudaFree(base);
     return rc;
+}
+
+size_t tfstat_search_host_scratch_bytes(int64_t template_stride, int32_t n_atoms,
+                                        int32_t n_templates, int window, int32_t t0_min,
+                                        int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
+                                        int32_t N_tau, int want_maps,
+                                        const tfstat_opts *opts_host)
+{
+    if (n_templates < 1 || template_stride < 1) return 0;
+    const int32_t Tc = std::min<int32_t>(n_templates, 256);
+    const Plan pl =
+        make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts_host);
+    if (pl.status != TFSTAT_OK) return 0;
+    const size_t tpl_bytes = sizeof(float) * (size_t)template_stride;
+    const size_t map_bytes = want_maps ? sizeof(float) * (size_t)N_t0 * N_tau : 0;
+    return 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) +
+           align_up(std::max(pl.bytes, kAlign)) + align_up(sizeof(int32_t) * (size_t)n_atoms) +
+           align_up(sizeof(tfstat_result) * (size_t)n_templates);
 }
 
 }  // extern "C"

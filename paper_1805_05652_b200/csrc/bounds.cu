@@ -47,6 +47,7 @@ __global__ void __launch_bounds__(kBoundsNT)
                   int stride, int n_samples, int32_t *__restrict__ lo,
                   int32_t *__restrict__ edge, int32_t *__restrict__ zero, int64_t n_zero)
 {
+    pdl_trigger();
     // scan flags of the rectangular path (rect.cu), zeroed here to save a memset node
     for (int64_t z = (int64_t)blockIdx.x * kBoundsNT + threadIdx.x; z < n_zero;
          z += (int64_t)gridDim.x * kBoundsNT)
@@ -82,6 +83,7 @@ cudaError_t launch_bounds(const Plan &pl, const int32_t *t_atoms, void *ws, cuda
 
 __global__ void count_terms_kernel(Grid g, Bounds b, unsigned long long *out)
 {
+    pdl_wait();
     const int64_t n_cells = (int64_t)g.N_t0 * g.N_tau;
     unsigned long long acc = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_cells;
@@ -105,7 +107,7 @@ cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_ter
     const int nt = 256;
     int64_t nb = (n_cells + nt - 1) / nt;
     if (nb > 148 * 16) nb = 148 * 16;
-    count_terms_kernel<<<(unsigned)nb, nt, 0, st>>>(
+    count_terms_kernel<<<(unsigned)nb, nt, 0, st>>>(  // follows a memset node: plain launch
         pl.grid, b, reinterpret_cast<unsigned long long *>(out_terms));
     return cudaGetLastError();
 }

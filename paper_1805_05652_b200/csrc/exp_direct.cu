@@ -75,6 +75,8 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
     __shared__ ulonglong2 s_a[KC];
     __shared__ ulonglong2 s_b[KC];
     __shared__ Marg s_red[32];
+    pdl_trigger();
+    pdl_wait();  // bounds_kernel's lo / edge tables
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -227,9 +229,8 @@ template <int C, int NT>
 cudaError_t launch_one(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
 {
     const int64_t n_ctas = pl.tiles_per_template * pl.n_templates;
-    exp_direct_kernel<C, NT, 512><<<(unsigned)n_ctas, NT, 0, st>>>(pr, partials, pl.n_mtiles,
-                                                                   pl.n_nblocks);
-    return cudaGetLastError();
+    return launch_pdl(exp_direct_kernel<C, NT, 512>, (unsigned)n_ctas, NT, 0, st, pr, partials,
+                      pl.n_mtiles, pl.n_nblocks);
 }
 
 template <int C>

@@ -92,6 +92,8 @@ __global__ void __launch_bounds__(NT)
     __shared__ ulonglong2 s_a[KC];  // {(dt, ab), (a2, b2)}
     __shared__ ulonglong2 s_b[KC];  // {(Re Fa, Im Fa), (Re Fb, Im Fb)}
     __shared__ Marg s_red[32];
+    pdl_trigger();
+    pdl_wait();  // bounds_kernel's lo / edge tables
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -227,9 +229,8 @@ template <int NT>
 cudaError_t launch_nt(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
 {
     const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * pl.n_templates;
-    exp_slide_kernel<NT, 512><<<(unsigned)n_ctas, NT, 0, st>>>(pr, partials, pl.n_nblocks,
-                                                               pl.n_segs, pl.seg_len);
-    return cudaGetLastError();
+    return launch_pdl(exp_slide_kernel<NT, 512>, (unsigned)n_ctas, NT, 0, st, pr, partials,
+                      pl.n_nblocks, pl.n_segs, pl.seg_len);
 }
 
 }  // namespace

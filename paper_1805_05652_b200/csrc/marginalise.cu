@@ -10,36 +10,102 @@ namespace tfstat {
 namespace {
 
 constexpr int kMargNT = 256;
+constexpr int kMargUnroll = 4;
 
-__device__ __forceinline__ void marg_add4(Marg &a, const float4 v, const uint32_t fl4,
-                                          const int32_t flat0)
+// Per-thread running marginals in the cheap form: max with a RARE branch for the argmax, and the
+// log-sum-exp as sum 2^(F log2e - ref2) against a reference exponent that only moves when a value
+// exceeds it by more than 2^60 (so nothing overflows and the common path is FFMA + MUFU.EX2 + FADD
+// per cell).  Converted to a Marg at the end.
+struct StreamMarg {
+    float best;
+    int32_t idx;
+    float ref2;
+    float sum;
+    int32_t nv;
+};
+constexpr float kHalfLog2eM = 0.72134752044448170368f;  // log2(e) / 2: F log2e = 2F * this
+
+template <bool FLAGS>
+__device__ __forceinline__ void stream_add4(StreamMarg &a, const float4 v, const uint32_t fl4,
+                                            const int32_t flat0)
 {
-    const float x[4] = {v.x, v.y, v.z, v.w};
-    float m4 = -INFINITY;
-    int nv = 0;
+    float x[4] = {v.x, v.y, v.z, v.w};
+    if (FLAGS) {
+        if (fl4 != 0u) {  // flagged cells lose every max and add 2^-inf = 0
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const bool ok = ((fl4 >> (8 * j)) & 0xffu) == 0u;
-        if (ok) {
-            if (x[j] > a.best) {  // ascending flat index within a thread: '>' keeps the lowest
-                a.best = x[j];
-                a.idx = flat0 + j;
-            }
-            m4 = fmaxf(m4, 0.5f * x[j]);
-            nv += 1;
+            for (int j = 0; j < 4; ++j)
+                if (((fl4 >> (8 * j)) & 0xffu) != 0u) x[j] = -INFINITY;
+        }
+        a.nv += 4 - (((fl4 & 0xffu) != 0u) + ((fl4 & 0xff00u) != 0u) + ((fl4 & 0xff0000u) != 0u) +
+                     ((fl4 & 0xff000000u) != 0u));
+    } else {
+        a.nv += 4;
+    }
+    const float m4 = fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3]));
+    if (m4 > a.best) {  // rare; ascending flat index within a thread: '>' keeps the lowest
+#pragma unroll
+        for (int j = 3; j >= 0; --j)
+            if (x[j] == m4) a.idx = flat0 + j;
+        a.best = m4;
+        if (fmaf(m4, kHalfLog2eM, -a.ref2) > 60.0f) {  // rarer: move the reference
+            a.sum *= ex2_approx(a.ref2 - m4 * kHalfLog2eM);
+            a.ref2 = m4 * kHalfLog2eM;
         }
     }
-    if (nv == 0) return;
-    if (m4 > a.M) {
-        a.S *= ex2_approx((a.M - m4) * TFSTAT_LOG2E_F);
-        a.M = m4;
-    }
+    float acc = 0.0f;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const bool ok = ((fl4 >> (8 * j)) & 0xffu) == 0u;
-        if (ok) a.S += ex2_approx((0.5f * x[j] - a.M) * TFSTAT_LOG2E_F);
+    for (int j = 0; j < 4; ++j) acc += ex2_approx(fmaf(x[j], kHalfLog2eM, -a.ref2));
+    a.sum += acc;
+}
+
+template <bool FLAGS>
+__device__ __forceinline__ void marginalise_body(const float *__restrict__ map,
+                                                 const uint8_t *__restrict__ flags,
+                                                 const int64_t n_cells, Marg &mg)
+{
+    StreamMarg sm;
+    sm.best = -INFINITY;
+    sm.idx = 0x7fffffff;
+    sm.ref2 = -1.0e30f;  // finite: a flagged cell (-inf) must give 2^-inf = 0, not inf - inf
+    sm.sum = 0.0f;
+    sm.nv = 0;
+    const bool vec = ((reinterpret_cast<uintptr_t>(map) & 15u) == 0) &&
+                     (!FLAGS || (reinterpret_cast<uintptr_t>(flags) & 3u) == 0);
+    const int64_t n4 = vec ? n_cells / 4 : 0;
+    const int64_t stride = (int64_t)gridDim.x * kMargNT;
+    // kMargUnroll independent 16-byte loads in flight per thread (6.5 TB/s x ~1 us of latency
+    // is ~45 KB per SM), consumed in ascending index order
+    int64_t q = (int64_t)blockIdx.x * kMargNT + threadIdx.x;
+    for (; q + (kMargUnroll - 1) * stride < n4; q += kMargUnroll * stride) {
+        float4 v[kMargUnroll];
+        uint32_t f[kMargUnroll];
+#pragma unroll
+        for (int k = 0; k < kMargUnroll; ++k) {
+            v[k] = __ldcs(reinterpret_cast<const float4 *>(map) + q + k * stride);
+            f[k] = FLAGS ? __ldcs(reinterpret_cast<const uint32_t *>(flags) + q + k * stride) : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < kMargUnroll; ++k)
+            stream_add4<FLAGS>(sm, v[k], f[k], (int32_t)(4 * (q + k * stride)));
     }
-    a.nvalid += nv;
+    for (; q < n4; q += stride) {
+        const float4 v = __ldcs(reinterpret_cast<const float4 *>(map) + q);
+        const uint32_t f = FLAGS ? __ldcs(reinterpret_cast<const uint32_t *>(flags) + q) : 0u;
+        stream_add4<FLAGS>(sm, v, f, (int32_t)(4 * q));
+    }
+    marg_init(mg);
+    mg.nvalid = sm.nv;
+    if (sm.best > -INFINITY) {
+        mg.best = sm.best;
+        mg.idx = sm.idx;
+        mg.M = 0.5f * sm.best;
+        mg.S = sm.sum * ex2_approx(sm.ref2 - sm.best * kHalfLog2eM);
+    }
+    // ragged tail (and unaligned maps): the plain per-cell way; indices above all of the above
+    for (int64_t i = 4 * n4 + (int64_t)blockIdx.x * kMargNT + threadIdx.x; i < n_cells;
+         i += stride) {
+        if (!FLAGS || flags[i] == 0) marg_add(mg, map[i], (int32_t)i);
+    }
 }
 
 __global__ void __launch_bounds__(kMargNT)
@@ -47,22 +113,10 @@ __global__ void __launch_bounds__(kMargNT)
                        const int64_t n_cells, Partial *__restrict__ partials)
 {
     __shared__ Marg s_red[32];
+    pdl_trigger();
     Marg mg;
-    marg_init(mg);
-    const bool vec = ((reinterpret_cast<uintptr_t>(map) & 15u) == 0) &&
-                     (!flags || (reinterpret_cast<uintptr_t>(flags) & 3u) == 0);
-    const int64_t n4 = vec ? n_cells / 4 : 0;
-    const int64_t stride = (int64_t)gridDim.x * kMargNT;
-    // each thread walks ascending indices, so ties inside a thread keep the lowest index
-    for (int64_t q = (int64_t)blockIdx.x * kMargNT + threadIdx.x; q < n4; q += stride) {
-        const float4 v = __ldcs(reinterpret_cast<const float4 *>(map) + q);
-        const uint32_t f = flags ? __ldcs(reinterpret_cast<const uint32_t *>(flags) + q) : 0u;
-        marg_add4(mg, v, f, (int32_t)(4 * q));
-    }
-    for (int64_t i = 4 * n4 + (int64_t)blockIdx.x * kMargNT + threadIdx.x; i < n_cells;
-         i += stride) {
-        if (!flags || flags[i] == 0) marg_add(mg, map[i], (int32_t)i);
-    }
+    if (flags) marginalise_body<true>(map, flags, n_cells, mg);
+    else marginalise_body<false>(map, flags, n_cells, mg);
     marg_block_reduce<kMargNT>(mg, s_red);
     if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
 }
@@ -77,6 +131,8 @@ __global__ void __launch_bounds__(256)
     __shared__ float s_M[256];
     __shared__ double s_S[256];
     __shared__ int32_t s_nv[256];
+    pdl_trigger();
+    pdl_wait();  // the partial marginals of the map kernel
     const Partial *__restrict__ p = partials + (int64_t)blockIdx.x * per_template;
     const int tid = threadIdx.x;
     float best = -INFINITY, M = -INFINITY;
@@ -152,8 +208,8 @@ cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_templa
                             int32_t n_templates, int32_t N_tau, tfstat_result *out,
                             cudaStream_t st)
 {
-    finalize_kernel<<<n_templates, 256, 0, st>>>(partials, partials_per_template, N_tau, out);
-    return cudaGetLastError();
+    return launch_pdl(finalize_kernel, (unsigned)n_templates, 256, 0, st, partials,
+                      partials_per_template, N_tau, out);
 }
 
 cudaError_t launch_marginalise(const float *map, const uint8_t *flags, int64_t n_cells,

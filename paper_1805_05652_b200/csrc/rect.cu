@@ -115,6 +115,8 @@ __global__ void __launch_bounds__(kScanNT)
 {
     __shared__ double s_off[8];
     __shared__ double s_w[7][kScanNT / 32];
+    pdl_trigger();
+    pdl_wait();  // bounds_kernel: edge table and the zeroed scan flags
     const Bounds &bd = pr.bounds;
     const int N = bd.n_atoms;
     int32_t *ready = flags, *done = flags + n_scan;
@@ -304,6 +306,8 @@ __global__ void __launch_bounds__(kCellNT)
                       Partial *__restrict__ partials, const int blocks_per_template)
 {
     __shared__ Marg s_red[32];
+    pdl_trigger();
+    pdl_wait();  // rect_scan_kernel's prefix sums
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
     const int tpl = blockIdx.x / blocks_per_template;
@@ -426,6 +430,8 @@ __global__ void __launch_bounds__(kRunNT, Q == 2 ? 4 : 5)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Marg s_red[32];
+    pdl_trigger();
+    pdl_wait();  // rect_scan_kernel's prefix sums and K table
     constexpr int nrows = Q * kRunNT;
     float *tile = reinterpret_cast<float *>(smem_raw);                     // [nrows][kPitch]
     int *s_rowm = reinterpret_cast<int *>(tile + (size_t)nrows * kPitch);  // [nrows]
@@ -763,18 +769,17 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
         e = cudaFuncSetAttribute(rect_run_kernel<Q, true>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        rect_run_kernel<Q, true><<<(unsigned)n_ctas, kRunNT, smem, st>>>(
-            pr, prefix, K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
-            vec ? 1 : 0);
+        return launch_pdl(rect_run_kernel<Q, true>, (unsigned)n_ctas, kRunNT, smem, st, pr, prefix,
+                          K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
+                          vec ? 1 : 0);
     } else {
         e = cudaFuncSetAttribute(rect_run_kernel<Q, false>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        rect_run_kernel<Q, false><<<(unsigned)n_ctas, kRunNT, smem, st>>>(
-            pr, prefix, K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
-            vec ? 1 : 0);
+        return launch_pdl(rect_run_kernel<Q, false>, (unsigned)n_ctas, kRunNT, smem, st, pr,
+                          prefix, K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles,
+                          rr.n_coltiles, vec ? 1 : 0);
     }
-    return cudaGetLastError();
 }
 
 }  // namespace
@@ -843,15 +848,13 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
     ulonglong2 *K = static_cast<ulonglong2 *>(steps);
     const int spt = pl.rect.enabled ? (int)((pl.J + 1 + kStepPts - 1) / kStepPts) : 0;
     const int64_t n_blocks = (int64_t)n_scan + (int64_t)spt * pl.n_templates;
-    rect_scan_kernel<<<(unsigned)n_blocks, kScanNT, 0, st>>>(pr, agg, flags, prefix, K, nblk,
-                                                             n_scan, spt);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = launch_pdl(rect_scan_kernel, (unsigned)n_blocks, kScanNT, 0, st, pr, agg, flags,
+                               prefix, K, nblk, n_scan, spt);
     if (e != cudaSuccess) return e;
     if (!pl.rect.enabled) {
         const int64_t n_ctas = (int64_t)pl.cell_blocks_per_template * pl.n_templates;
-        rect_cells_kernel<<<(unsigned)n_ctas, kCellNT, 0, st>>>(pr, prefix, partials,
-                                                                pl.cell_blocks_per_template);
-        return cudaGetLastError();
+        return launch_pdl(rect_cells_kernel, (unsigned)n_ctas, kCellNT, 0, st, pr, prefix, partials,
+                          pl.cell_blocks_per_template);
     }
     if (pl.rect.Q == 2) return launch_run<2>(pl, pr, prefix, K, partials, st);
     return launch_run<1>(pl, pr, prefix, K, partials, st);

@@ -223,6 +223,34 @@ __device__ __forceinline__ void partial_store(Partial *p, const Marg &a)
 }
 
 // ---------------------------------------------------------------------------------------
+// Programmatic dependent launch (sm_90+): the kernels of one call form a chain on the stream
+// (bounds -> sums -> finalize).  A kernel launched with launch_pdl() may be scheduled while its
+// predecessor is still running; it must call pdl_wait() before touching anything the
+// predecessor writes (the wait returns once the predecessor grid has completed and its writes
+// are visible), and every kernel calls pdl_trigger() at its start so that its own successor
+// can be set up early.  Only the launch latency is overlapped: ~2-3 us per kernel boundary.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem,
+                              cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+// ---------------------------------------------------------------------------------------
 // host-side launchers (one per .cu file)
 // ---------------------------------------------------------------------------------------
 struct Problem {

@@ -126,11 +126,28 @@ def test_search_host_equals_device(pkg):
     for window in (EXP, RECT):
         r_dev = pkg.tfstat_search(dev(wl.data.atoms), dev(wl.data.t), window, grid,
                                   want_maps=True)
-        # small device budget: forces several chunks through the double-buffered copies
+        # small device budget (chunks of 2 of the 9 templates): several chunks go through the
+        # double-buffered copies
+        small = pkg.search_host_scratch_bytes(a_h.stride(0), a_h.shape[2], 2, window, grid,
+                                              want_maps=True) + 256
         r_host, maps = pkg.tfstat_search_host(a_h, t_h, window, grid, want_maps=True,
-                                              max_device_bytes=3 * a_h[0].numel() * 4 * 2)
+                                              max_device_bytes=small)
         assert np.array_equal(r_host, r_dev.numpy())
         assert np.array_equal(maps.numpy(), r_dev.maps.cpu().numpy())
+        # a scratch tensor of the caller, and the library's own cudaMalloc, give the same
+        mine = torch.empty(small, dtype=torch.uint8, device="cuda")
+        r2, maps2 = pkg.tfstat_search_host(a_h, t_h, window, grid, want_maps=True, scratch=mine)
+        r3, maps3 = pkg.tfstat_search_host(a_h, t_h, window, grid, want_maps=True,
+                                           library_malloc=True, max_device_bytes=small)
+        r4, _ = pkg.tfstat_search_host(a_h, t_h, window, grid)  # cached scratch, results only
+        for r, m in ((r2, maps2), (r3, maps3), (r4, None)):
+            assert np.array_equal(r, r_dev.numpy())
+            if m is not None:
+                assert np.array_equal(m.numpy(), r_dev.maps.cpu().numpy())
+        # a scratch too small for one template is an error, not a crash
+        with pytest.raises(pkg.TfstatError):
+            pkg.tfstat_search_host(a_h, t_h, window, grid, want_maps=True,
+                                   scratch=torch.empty(4096, dtype=torch.uint8, device="cuda"))
 
 
 def test_degenerate_maps(pkg):
