@@ -9,7 +9,7 @@ from typing import Optional, Tuple
 
 import numpy as np
 
-RECT, EXP = 0, 1
+RECT, EXP, TABLE = 0, 1, 2
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "tfstat_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle_tfstat.so")
@@ -56,6 +56,8 @@ def _load():
         lib.oracle_tfstat_marginalise.argtypes = [vp, vp, i32, i32, C.POINTER(_Result)]
         lib.oracle_tfstat_search.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
             i32, vp, vp, C.c_int]
+        lib.oracle_tfstat_map_general.argtypes = [vp, i64, vp, i32, C.c_int, i32, i32, vp, i32,
+                                                  vp, i32, vp, i32, i32, vp, vp, vp, vp, C.c_int]
         lib.oracle_num_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -90,6 +92,28 @@ def map2F(atoms, t, window, grid, min_atoms: int = 2, n_threads: int = 0):
                                    _ptr(cnt), n_threads)
     if rc != 0:
         raise ValueError(f"oracle_tfstat_map rc={rc}")
+    return dict(twoF=twoF, flags=flags, cond=cond, cnt=cnt)
+
+
+def map2F_general(atoms, t, kind, support, t0_grid, tau_grid, table=None, min_atoms: int = 2,
+                  n_threads: int = 0):
+    """General window on explicit grids.  support = (num, den) in units of tau; table = fp32
+    samples of w(u) for kind TABLE.  Returns the same dict as map2F."""
+    atoms, t = _check_atoms(atoms, t)
+    t0_grid = np.ascontiguousarray(t0_grid, dtype=np.int32)
+    tau_grid = np.ascontiguousarray(tau_grid, dtype=np.int32)
+    tab = None if table is None else np.ascontiguousarray(table, dtype=np.float32)
+    shape = (t0_grid.shape[0], tau_grid.shape[0])
+    twoF = np.empty(shape, np.float64)
+    flags = np.empty(shape, np.uint8)
+    cond = np.empty(shape, np.float64)
+    cnt = np.empty(shape, np.int32)
+    rc = _load().oracle_tfstat_map_general(
+        _ptr(atoms), atoms.shape[1], _ptr(t), t.shape[0], kind, int(support[0]), int(support[1]),
+        _ptr(tab), 0 if tab is None else tab.shape[0], _ptr(t0_grid), shape[0], _ptr(tau_grid),
+        shape[1], min_atoms, _ptr(twoF), _ptr(flags), _ptr(cond), _ptr(cnt), n_threads)
+    if rc != 0:
+        raise ValueError(f"oracle_tfstat_map_general rc={rc}")
     return dict(twoF=twoF, flags=flags, cond=cond, cnt=cnt)
 
 

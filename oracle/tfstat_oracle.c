@@ -257,6 +257,99 @@ int oracle_tfstat_search(const float *atoms, int64_t template_stride, int64_t ld
     return rc;
 }
 
+/* ---------------------------------------------------------------------------------------
+ * General windows on explicit grids.
+ *
+ * "Different window functions for the amplitude evolution could also be considered, and would
+ * generically follow the GPU kernel grid setup and timing model for the exponential window"
+ * (PAPER.md:192), and the {t0, tau} grid may have "a coarser or even variable sampling"
+ * (PAPER.md:74).  The definition is the same cell by cell, with
+ *   - t0_grid[m], tau_grid[n]: explicit integer-second arrays, any order, tau >= 1;
+ *   - support = sup_num / sup_den (in units of tau): atom alpha is in the window iff
+ *       t0 <= t_alpha  and  (t_alpha - t0) * sup_den < sup_num * tau     (integers, half-open);
+ *   - weight w(u), u = (t_alpha - t0) / tau in [0, support):
+ *       kind 0 (rect) w = 1;  kind 1 (exp) w = exp(-u);
+ *       kind 2 (table) w = linear interpolation of n_table >= 2 samples table[i] = w(u_i),
+ *                      u_i = i * support / (n_table - 1).
+ *   With (rect, 1/1) and (exp, 3/1) this is exactly eqs. (3), (4).
+ * PARITY UNPINNED BY THE PAPER for the table convention (the paper names no other window): it
+ * is DESIGN.md reading R17, pinned against numpy.interp and against the rect / exp special
+ * cases in tests/test_oracle_pins.py.
+ * --------------------------------------------------------------------------------------- */
+#define ORACLE_TABLE 2
+
+static double general_weight(int kind, double u, double support, const float *table,
+                             int32_t n_table)
+{
+    if (kind == ORACLE_RECT) return 1.0;
+    if (kind == ORACLE_EXP) return exp(-u);
+    const double x = u / support * (double)(n_table - 1);
+    int64_t i = (int64_t)floor(x);
+    if (i < 0) i = 0;
+    if (i > n_table - 2) i = n_table - 2;
+    const double f = x - (double)i;
+    return (double)table[i] + f * ((double)table[i + 1] - (double)table[i]);
+}
+
+int oracle_tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t, int32_t n_atoms,
+                              int kind, int32_t sup_num, int32_t sup_den, const float *table,
+                              int32_t n_table, const int32_t *t0_grid, int32_t N_t0,
+                              const int32_t *tau_grid, int32_t N_tau, int32_t min_atoms,
+                              double *out_2F, uint8_t *out_flags, double *out_cond,
+                              int32_t *out_cnt, int n_threads)
+{
+    if (!atoms || !t || n_atoms < 1 || ld < n_atoms || !t0_grid || !tau_grid || N_t0 < 1 ||
+        N_tau < 1 || !out_2F || sup_num < 1 || sup_den < 1)
+        return -1;
+    if (kind != ORACLE_RECT && kind != ORACLE_EXP && kind != ORACLE_TABLE) return -1;
+    if (kind == ORACLE_TABLE && (!table || n_table < 2)) return -1;
+    for (int32_t n = 0; n < N_tau; ++n)
+        if (tau_grid[n] < 1) return -1;
+    const float *a2 = atoms, *b2 = atoms + ld, *ab = atoms + 2 * ld;
+    const float *fare = atoms + 3 * ld, *faim = atoms + 4 * ld;
+    const float *fbre = atoms + 5 * ld, *fbim = atoms + 6 * ld;
+    const double support = (double)sup_num / (double)sup_den;
+#ifdef _OPENMP
+    if (n_threads < 1) n_threads = omp_get_max_threads();
+#pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads)
+#endif
+    for (int32_t m = 0; m < N_t0; ++m) {
+        for (int32_t n = 0; n < N_tau; ++n) {
+            const int64_t t0 = t0_grid[m], tau = tau_grid[n];
+            double A = 0, B = 0, C = 0, FaRe = 0, FaIm = 0, FbRe = 0, FbIm = 0;
+            int32_t cnt = 0;
+            for (int32_t al = 0; al < n_atoms; ++al) {
+                const int64_t dt = (int64_t)t[al] - t0;
+                if (dt < 0) continue;
+                if (!(dt * sup_den < (int64_t)sup_num * tau)) continue;
+                const double w =
+                    general_weight(kind, (double)dt / (double)tau, support, table, n_table);
+                const double w2 = w * w;
+                A += w2 * (double)a2[al];
+                B += w2 * (double)b2[al];
+                C += w2 * (double)ab[al];
+                FaRe += w * (double)fare[al];
+                FaIm += w * (double)faim[al];
+                FbRe += w * (double)fbre[al];
+                FbIm += w * (double)fbim[al];
+                cnt += 1;
+            }
+            const double D = A * B - C * C;
+            uint8_t fl = 0;
+            if (cnt < min_atoms) fl |= 1;
+            if (!(D > 0.0)) fl |= 2;
+            const int64_t i = (int64_t)m * N_tau + n;
+            out_2F[i] = fl ? 0.0
+                           : 2.0 * (B * (FaRe * FaRe + FaIm * FaIm) + A * (FbRe * FbRe + FbIm * FbIm) -
+                                    2.0 * C * (FaRe * FbRe + FaIm * FbIm)) / D;
+            if (out_flags) out_flags[i] = fl;
+            if (out_cond) out_cond[i] = (A * B != 0.0) ? D / (A * B) : 0.0;
+            if (out_cnt) out_cnt[i] = cnt;
+        }
+    }
+    return 0;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP
