@@ -44,6 +44,8 @@ extern "C" {
 #define TFSTAT_WINDOW_RECT 0 /* w = 1 on [t0, t0 + tau)                          */
 #define TFSTAT_WINDOW_EXP 1  /* w = exp(-(t - t0)/tau) on [t0, t0 + 3 tau)       */
 
+#define TFSTAT_WINDOW_TABLE 2 /* tfstat_map_general only: w(u) tabulated, u = (t - t0)/tau    */
+
 /* how the exponential-window sums are evaluated (tfstat_opts.exp_method) */
 #define TFSTAT_EXP_AUTO 0   /* = DIRECT */
 #define TFSTAT_EXP_DIRECT 1 /* truncated weighted sum per cell, the paper's
@@ -143,6 +145,40 @@ int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int3
                        int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
                        int32_t N_tau, int64_t *out_terms, void *workspace,
                        size_t workspace_bytes, void *stream);
+
+/* ---- general windows on explicit grids ------------------------------------------------ */
+
+/* A window function for tfstat_map_general (a HOST struct; `table` is a DEVICE pointer).
+ * "Different window functions for the amplitude evolution could also be considered, and would
+ * generically follow the GPU kernel grid setup ... for the exponential window".
+ *   support = support_num / support_den, in units of tau: atom a is in the window iff
+ *     t0 <= t_a  and  (t_a - t0) * support_den < support_num * tau   (integers, half-open);
+ *   weight w(u), u = (t_a - t0)/tau in [0, support), applied as w on Fa, Fb and w^2 on
+ *   a2, b2, ab:   TFSTAT_WINDOW_RECT  w = 1          (support 1/1: eq. 3)
+ *                 TFSTAT_WINDOW_EXP   w = exp(-u)    (support 3/1: eq. 4)
+ *                 TFSTAT_WINDOW_TABLE w = linear interpolation of n_table >= 2 fp32 samples
+ *                                     table[i] = w(i * support / (n_table - 1)).            */
+typedef struct tfstat_window {
+    int32_t kind;
+    int32_t support_num, support_den; /* both >= 1 */
+    int32_t n_table;                  /* TABLE only */
+    const float *table;               /* TABLE only; device memory, n_table floats */
+} tfstat_window;
+
+/* Map (and / or marginals) for a general window on EXPLICIT grids: t0_grid[N_t0] and
+ * tau_grid[N_tau] are DEVICE int32 arrays of seconds in any order ("a coarser or even variable
+ * sampling is also possible"); map[m*N_tau + n] = 2F(t0_grid[m], tau_grid[n]).
+ * Every cell is the direct truncated sum.  Entries tau_grid[n] < 1 give
+ * degenerate cells (flags 3), not an error (the arrays live on the device).
+ *   out_map, out_flags, out: each nullable, at least one of out_map / out required.
+ *   workspace: >= tfstat_general_workspace_bytes(N_t0, N_tau) bytes, 256-B aligned.
+ *   opts_host: only min_atoms is used.                                                      */
+size_t tfstat_general_workspace_bytes(int32_t N_t0, int32_t N_tau);
+int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
+                       const tfstat_window *window_host, const int32_t *t0_grid, int32_t N_t0,
+                       const int32_t *tau_grid, int32_t N_tau, float *out_map,
+                       uint8_t *out_flags, tfstat_result *out, void *workspace,
+                       size_t workspace_bytes, void *stream, const tfstat_opts *opts_host);
 
 /* ---- end-to-end entry point with HOST buffers ----------------------------------------- */
 

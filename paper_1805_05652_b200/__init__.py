@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     EXP_SCAN,
     RECT,
     RESULT_DTYPE,
+    TABLE,
     TfstatError,
     count_terms,
     lib_path,
@@ -20,6 +21,7 @@ from .binding import (  # noqa: F401
     probe_alu,
     search_host_scratch_bytes,
     tfstat_map,
+    tfstat_map_general,
     tfstat_marginalise,
     tfstat_search,
     tfstat_search_host,

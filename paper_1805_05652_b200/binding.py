@@ -13,7 +13,7 @@ from typing import Optional
 import numpy as np
 import torch
 
-RECT, EXP = 0, 1
+RECT, EXP, TABLE = 0, 1, 2
 EXP_AUTO, EXP_DIRECT, EXP_SCAN = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -34,6 +34,11 @@ class _Opts(C.Structure):
                 ("tile_c", C.c_int32), ("tile_nt", C.c_int32), ("seg_len", C.c_int32),
                 ("reserved", C.c_int32), ("ev_main_begin", C.c_void_p),
                 ("ev_main_end", C.c_void_p)]
+
+
+class _Window(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("support_num", C.c_int32), ("support_den", C.c_int32),
+                ("n_table", C.c_int32), ("table", C.c_void_p)]
 
 
 def lib_path() -> str:
@@ -70,6 +75,10 @@ def load_library():
         vp, vp, vp, sz, op]
     lib.tfstat_search_host_scratch_bytes.restype = sz
     lib.tfstat_search_host_scratch_bytes.argtypes = [i64, i32, i32, C.c_int] + grid + [C.c_int, op]
+    lib.tfstat_general_workspace_bytes.restype = sz
+    lib.tfstat_general_workspace_bytes.argtypes = [i32, i32]
+    lib.tfstat_map_general.argtypes = [vp, i64, vp, i32, C.POINTER(_Window), vp, i32, vp, i32,
+                                       vp, vp, vp, vp, sz, vp, op]
     lib.tfstat_probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
     _lib = lib
@@ -242,6 +251,53 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
                            _stream_ptr(stream), C.byref(o))
     _check(rc, "tfstat_search")
     return Results(out, maps, flags)
+
+
+def tfstat_map_general(atoms: torch.Tensor, t_atoms: torch.Tensor, kind: int, support,
+                       t0_grid: torch.Tensor, tau_grid: torch.Tensor, *,
+                       table: Optional[torch.Tensor] = None, min_atoms: int = 2,
+                       want_map: bool = True, want_flags: bool = False,
+                       want_marginals: bool = True, stream=None):
+    """General window on explicit grids (include/tfstat.h, tfstat_map_general).
+
+    atoms [7, N]; t0_grid [N_t0], tau_grid [N_tau]: CUDA int32 tensors of seconds (any order);
+    support = (num, den) in units of tau; table: CUDA float32 samples of w(u) for kind TABLE.
+    Returns (map or None, flags or None, Results or None)."""
+    lib = load_library()
+    _dev_f32(atoms, "atoms")
+    _dev_i32(t_atoms, "t_atoms")
+    _dev_i32(t0_grid, "t0_grid")
+    _dev_i32(tau_grid, "tau_grid")
+    if atoms.dim() != 2 or atoms.shape[0] != 7 or atoms.stride(1) != 1:
+        raise TfstatError("atoms must be [7, N] with unit stride along N")
+    n_atoms, ld = int(t_atoms.shape[0]), int(atoms.stride(0))
+    if atoms.shape[1] != n_atoms:
+        raise TfstatError("atoms / t_atoms length mismatch")
+    if not (want_map or want_marginals):
+        raise TfstatError("nothing to compute: want_map or want_marginals")
+    w = _Window()
+    w.kind, w.support_num, w.support_den = int(kind), int(support[0]), int(support[1])
+    if table is not None:
+        _dev_f32(table, "table")
+        if not table.is_contiguous():
+            raise TfstatError("table must be contiguous")
+        w.n_table, w.table = int(table.numel()), table.data_ptr()
+    N_t0, N_tau = int(t0_grid.shape[0]), int(tau_grid.shape[0])
+    dev = atoms.device
+    out_map = torch.empty((N_t0, N_tau), dtype=torch.float32, device=dev) if want_map else None
+    flags = torch.empty((N_t0, N_tau), dtype=torch.uint8, device=dev) if want_flags else None
+    out = torch.empty((1, 5), dtype=torch.int32, device=dev) if want_marginals else None
+    nbytes = int(lib.tfstat_general_workspace_bytes(N_t0, N_tau))
+    ws = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=dev)
+    o = _opts(min_atoms, EXP_AUTO)
+    rc = lib.tfstat_map_general(atoms.data_ptr(), ld, t_atoms.data_ptr(), n_atoms, C.byref(w),
+                                t0_grid.data_ptr(), N_t0, tau_grid.data_ptr(), N_tau,
+                                out_map.data_ptr() if want_map else None,
+                                flags.data_ptr() if want_flags else None,
+                                out.data_ptr() if want_marginals else None, ws.data_ptr(),
+                                ws.numel(), _stream_ptr(stream), C.byref(o))
+    _check(rc, "tfstat_map_general")
+    return out_map, flags, (Results(out) if want_marginals else None)
 
 
 def count_terms(t_atoms: torch.Tensor, window: int, grid, *, stream=None) -> int:

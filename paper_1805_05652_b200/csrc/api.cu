@@ -293,6 +293,42 @@ int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int3
     return TFSTAT_OK;
 }
 
+size_t tfstat_general_workspace_bytes(int32_t N_t0, int32_t N_tau)
+{
+    if (N_t0 < 1 || N_tau < 1 || (int64_t)N_t0 * N_tau >= (int64_t(1) << 31)) return 0;
+    return align_up(sizeof(Partial) * (size_t)general_partials(N_t0, N_tau));
+}
+
+int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
+                       const tfstat_window *window_host, const int32_t *t0_grid, int32_t N_t0,
+                       const int32_t *tau_grid, int32_t N_tau, float *out_map,
+                       uint8_t *out_flags, tfstat_result *out, void *workspace,
+                       size_t workspace_bytes, void *stream, const tfstat_opts *opts_host)
+{
+    if (!atoms || !t_atoms || !window_host || !t0_grid || !tau_grid || (!out_map && !out))
+        return TFSTAT_EINVAL;
+    if (n_atoms < 1 || ld < n_atoms || N_t0 < 1 || N_tau < 1) return TFSTAT_EINVAL;
+    if ((int64_t)N_t0 * N_tau >= (int64_t(1) << 31)) return TFSTAT_EINVAL;
+    const tfstat_window &w = *window_host;
+    if (w.kind != TFSTAT_WINDOW_RECT && w.kind != TFSTAT_WINDOW_EXP &&
+        w.kind != TFSTAT_WINDOW_TABLE)
+        return TFSTAT_EINVAL;
+    if (w.support_num < 1 || w.support_den < 1) return TFSTAT_EINVAL;
+    if (w.kind == TFSTAT_WINDOW_TABLE && (!w.table || w.n_table < 2)) return TFSTAT_EINVAL;
+    const size_t need = tfstat_general_workspace_bytes(N_t0, N_tau);
+    if (!workspace || workspace_bytes < need ||
+        (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)))
+        return TFSTAT_EWORKSPACE;
+    const int32_t min_atoms = (opts_host && opts_host->min_atoms > 0) ? opts_host->min_atoms : 2;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Partial *partials = out ? static_cast<Partial *>(workspace) : nullptr;
+    TF_CUDA(launch_general(atoms, ld, t_atoms, n_atoms, w, t0_grid, N_t0, tau_grid, N_tau,
+                           min_atoms, out_map, out_flags, partials, st));
+    if (out)
+        TF_CUDA(launch_finalize(partials, general_partials(N_t0, N_tau), 1, N_tau, out, st));
+    return TFSTAT_OK;
+}
+
 int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t ld,
                        const int32_t *t_atoms_host, int32_t n_atoms, int32_t n_templates,
                        int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,

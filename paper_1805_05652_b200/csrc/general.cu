@@ -1,0 +1,209 @@
+// general.cu -- tfstat_map_general: the map for a general window function on explicit
+// (possibly irregular) t0 / tau arrays (R17).
+//
+// "Different window functions for the amplitude evolution could also be considered, and would
+// generically follow the GPU kernel grid setup and timing model for the exponential window,
+// since it does not assume any function-specific optimisations"; the grid may
+// have "a coarser or even variable sampling".  So this is the direct truncated
+// sum per cell, with
+//   membership  t0 <= t_a  and  (t_a - t0) * den < num * tau        (integers, half-open)
+//   weight      w(u), u = (t_a - t0) / tau:  1 | exp(-u) | linear interpolation of a table
+//   w on Fa, Fb and w^2 on a2, b2, ab; closure eq. (7); marginals eq. (5).
+//
+// One thread owns one cell at a time: a CTA is (one t0) x (NT consecutive entries of the tau
+// array).  Window bounds come from two binary searches per cell (no lattice: the arrays are
+// arbitrary).  The CTA streams the atoms [lo, max hi) through shared memory in chunks, staged
+// once as (dt, ab | a2, b2) and (Re Fa, Im Fa | Re Fb, Im Fb) records that every lane reads by
+// broadcast; each thread stops at its own hi.  No weight sharing between cells is assumed (a
+// general w(u) does not factorise), so the executed mix is the algorithmic one: per term the
+// weight, w^2, and 7 fp32 multiply-adds (4 packed fma.rn.f32x2).  The closure runs in fp64.
+#include "plan.h"
+
+namespace tfstat {
+
+namespace {
+
+constexpr int kGenNT = 128;
+constexpr int kGenKC = 512;        // atoms per staged chunk (16 KB)
+constexpr int kGenTableSmem = 4096;  // tables up to this many samples are staged in smem
+
+struct GeneralArgs {
+    const float *atoms;
+    int64_t ld;
+    const int32_t *t;
+    int32_t n_atoms;
+    const int32_t *t0_grid;
+    int32_t N_t0;
+    const int32_t *tau_grid;
+    int32_t N_tau;
+    int32_t sup_num, sup_den;
+    const float *table;
+    int32_t n_table;
+    int32_t min_atoms;
+    float *out_map;
+    uint8_t *out_flags;
+};
+
+template <int KIND>
+__global__ void __launch_bounds__(kGenNT)
+    general_kernel(const GeneralArgs a, Partial *__restrict__ partials, const int n_nblocks)
+{
+    __shared__ ulonglong2 s_a[kGenKC];
+    __shared__ ulonglong2 s_b[kGenKC];
+    __shared__ Marg s_red[32];
+    __shared__ int s_hi[kGenNT / 32];
+    __shared__ float s_tab[KIND == TFSTAT_WINDOW_TABLE ? kGenTableSmem : 1];
+    pdl_trigger();
+
+    const int m = blockIdx.x / n_nblocks;
+    const int n = (blockIdx.x % n_nblocks) * kGenNT + threadIdx.x;
+    const bool n_ok = n < a.N_tau;
+    const long long t0 = __ldg(a.t0_grid + m);
+    const long long tau = n_ok ? (long long)__ldg(a.tau_grid + n) : 0;
+    // a1: bounds.  dt * den < num * tau  <=>  t < t0 + ceil(num tau / den)
+    const int lo = lower_bound_t(a.t, a.n_atoms, t0);
+    int hi = lo;
+    if (tau >= 1) {
+        const long long len = ((long long)a.sup_num * tau + a.sup_den - 1) / a.sup_den;
+        hi = lower_bound_t(a.t, a.n_atoms, t0 + len);
+    }
+    // atom range of the CTA: [lo, max over its threads of hi)
+    int hmax = hi;
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) hmax = max(hmax, __shfl_xor_sync(0xffffffffu, hmax, s));
+    if ((threadIdx.x & 31) == 0) s_hi[threadIdx.x >> 5] = hmax;
+    const bool tab_smem = KIND == TFSTAT_WINDOW_TABLE && a.n_table <= kGenTableSmem;
+    if (tab_smem)
+        for (int i = threadIdx.x; i < a.n_table; i += kGenNT) s_tab[i] = __ldg(a.table + i);
+    __syncthreads();
+    int cta_e = s_hi[0];
+#pragma unroll
+    for (int w = 1; w < kGenNT / 32; ++w) cta_e = max(cta_e, s_hi[w]);
+
+    // weight constants: exp: w = 2^(dt * kexp); table: x = dt * kx, knots at integer x
+    const float inv_tau = tau >= 1 ? (float)(1.0 / (double)tau) : 0.0f;
+    const float kexp = -1.4426950408889634f * inv_tau;
+    const float kx = tau >= 1 ? (float)((double)(a.n_table - 1) * (double)a.sup_den /
+                                        ((double)a.sup_num * (double)tau))
+                              : 0.0f;
+    const float *__restrict__ tab = tab_smem ? s_tab : a.table;
+
+    u64 acc_ab = 0ull, acc_fa = 0ull, acc_fb = 0ull;  // (A, B), (Re Fa, Im Fa), (Re Fb, Im Fb)
+    float acc_c = 0.0f;
+#pragma unroll 1
+    for (int cs = lo; cs < cta_e; cs += kGenKC) {
+        const int n_stage = min(kGenKC, cta_e - cs);
+        for (int i = threadIdx.x; i < n_stage; i += kGenNT) {  // a0: stage atoms [cs, cs+n_stage)
+            const int al = cs + i;
+            const float dt = (float)((long long)__ldg(a.t + al) - t0);
+            ulonglong2 ra, rb;
+            ra.x = pack2(dt, __ldg(a.atoms + 2 * a.ld + al));
+            ra.y = pack2(__ldg(a.atoms + al), __ldg(a.atoms + a.ld + al));
+            rb.x = pack2(__ldg(a.atoms + 3 * a.ld + al), __ldg(a.atoms + 4 * a.ld + al));
+            rb.y = pack2(__ldg(a.atoms + 5 * a.ld + al), __ldg(a.atoms + 6 * a.ld + al));
+            s_a[i] = ra;
+            s_b[i] = rb;
+        }
+        __syncthreads();
+        const int x1 = min(cs + n_stage, hi) - cs;  // this thread's atoms of the chunk: [0, x1)
+#pragma unroll 4
+        for (int i = 0; i < x1; ++i) {
+            const ulonglong2 ra = s_a[i], rb = s_b[i];
+            float dt, ab;
+            unpack2(ra.x, dt, ab);
+            float w;
+            if (KIND == TFSTAT_WINDOW_RECT) {
+                w = 1.0f;
+            } else if (KIND == TFSTAT_WINDOW_EXP) {
+                w = ex2_approx(dt * kexp);
+            } else {
+                const float x = dt * kx;
+                const int k = min((int)x, a.n_table - 2);
+                const float t0v = tab[k], t1v = tab[k + 1];
+                w = fmaf(x - (float)k, t1v - t0v, t0v);
+            }
+            const float w2 = w * w;
+            ffma2(acc_ab, pack2(w2, w2), ra.y);
+            const u64 ww = pack2(w, w);
+            ffma2(acc_fa, ww, rb.x);
+            ffma2(acc_fb, ww, rb.y);
+            acc_c = fmaf(w2, ab, acc_c);
+        }
+        __syncthreads();
+    }
+
+    // a4 closure + a5 marginals
+    Marg mg;
+    marg_init(mg);
+    if (n_ok) {
+        Sums64 s;
+        float A, B, far, fai, fbr, fbi;
+        unpack2(acc_ab, A, B);
+        unpack2(acc_fa, far, fai);
+        unpack2(acc_fb, fbr, fbi);
+        s.A = A;
+        s.B = B;
+        s.C = acc_c;
+        s.far = far;
+        s.fai = fai;
+        s.fbr = fbr;
+        s.fbi = fbi;
+        uint32_t fl;
+        const float twoF = closure_2F(s, hi - lo, a.min_atoms, fl);
+        const int32_t flat = m * a.N_tau + n;
+        if (a.out_map) a.out_map[flat] = twoF;
+        if (a.out_flags) a.out_flags[flat] = (uint8_t)fl;
+        if (!fl) marg_add(mg, twoF, flat);
+    }
+    if (partials) {
+        marg_block_reduce<kGenNT>(mg, s_red);
+        if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
+    }
+}
+
+}  // namespace
+
+int32_t general_partials(int32_t N_t0, int32_t N_tau)
+{
+    return N_t0 * ((N_tau + kGenNT - 1) / kGenNT);
+}
+
+cudaError_t launch_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
+                           const tfstat_window &w, const int32_t *t0_grid, int32_t N_t0,
+                           const int32_t *tau_grid, int32_t N_tau, int32_t min_atoms,
+                           float *out_map, uint8_t *out_flags, Partial *partials, cudaStream_t st)
+{
+    GeneralArgs a;
+    a.atoms = atoms;
+    a.ld = ld;
+    a.t = t_atoms;
+    a.n_atoms = n_atoms;
+    a.t0_grid = t0_grid;
+    a.N_t0 = N_t0;
+    a.tau_grid = tau_grid;
+    a.N_tau = N_tau;
+    a.sup_num = w.support_num;
+    a.sup_den = w.support_den;
+    a.table = w.table;
+    a.n_table = w.n_table;
+    a.min_atoms = min_atoms;
+    a.out_map = out_map;
+    a.out_flags = out_flags;
+    const int n_nblocks = (N_tau + kGenNT - 1) / kGenNT;
+    const unsigned grid = (unsigned)N_t0 * (unsigned)n_nblocks;
+    switch (w.kind) {
+    case TFSTAT_WINDOW_RECT:
+        general_kernel<TFSTAT_WINDOW_RECT><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks);
+        break;
+    case TFSTAT_WINDOW_EXP:
+        general_kernel<TFSTAT_WINDOW_EXP><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks);
+        break;
+    case TFSTAT_WINDOW_TABLE:
+        general_kernel<TFSTAT_WINDOW_TABLE><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks);
+        break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace tfstat

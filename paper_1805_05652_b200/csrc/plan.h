@@ -87,6 +87,11 @@ cudaError_t launch_marginalise(const float *map, const uint8_t *flags, int64_t n
                                int32_t N_tau, Partial *partials, int32_t n_blocks,
                                tfstat_result *out, cudaStream_t st);
 int32_t marginalise_blocks(int64_t n_cells);
+int32_t general_partials(int32_t N_t0, int32_t N_tau);
+cudaError_t launch_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
+                           const tfstat_window &w, const int32_t *t0_grid, int32_t N_t0,
+                           const int32_t *tau_grid, int32_t N_tau, int32_t min_atoms,
+                           float *out_map, uint8_t *out_flags, Partial *partials, cudaStream_t st);
 
 inline Bounds make_bounds(const Plan &pl, const int32_t *t_atoms, void *ws)
 {
