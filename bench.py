@@ -210,6 +210,20 @@ def side_workloads(torch, pkg, peaks):
             rec["cells_per_s_map"] = cells / (med_map * 1e-3)
             rec["algorithmic_GBps_map"] = by / (med_map * 1e-3) / 1e9
             rec["hbm_frac_map"] = rec["algorithmic_GBps_map"] / peaks["hbm_gbs"]
+        if cfg == 2:
+            # the same map through tfstat_map_general (explicit grid arrays, one weight per term:
+            # the paper's own brute-force design), exp and a 1025-point table
+            t0g = torch.from_numpy(wl.grid.t0().astype(np.int32)).cuda()
+            taug = torch.from_numpy(wl.grid.tau().astype(np.int32)).cuda()
+            tab = torch.exp(-torch.linspace(0.0, 3.0, 1025, device="cuda"))
+            for gname, kind, tb in (("exp", 1, None), ("table", 2, tab)):
+                fn_g = lambda: pkg.tfstat_map_general(atoms[0], t, kind, (3, 1), t0g, taug,
+                                                      table=tb, want_marginals=False)
+                for _ in range(3):
+                    fn_g()
+                _, med_g = timed(fn_g)
+                rec[f"general_{gname}_map_ms"] = med_g
+                rec[f"general_{gname}_terms_per_s"] = terms / (med_g * 1e-3)
         out[f"cfg{cfg}_{wname}"] = rec
         if cfg == 5 and window == 0:
             # steady state of the rect map path: 8 copies of config 5 in one tfstat_search that
