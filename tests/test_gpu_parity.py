@@ -259,6 +259,46 @@ def test_config4_batched_search_subset(pkg):
             assert res[j]["max2F"] > 30.0  # rho = 8 stands out of chi^2_4 noise
 
 
+def test_config4_full_launch_all_injected_templates(pkg):
+    """BASELINE.json config 4 at full size, in the launch configuration bench.py times (one
+    tfstat_search over all 4096 templates): the 41 injected templates and 7 noise-only ones are
+    checked against the oracle's marginals (its full map where the argmax differs), every
+    template's record is sane, and a sub-launch gives bit-identical records."""
+    from synth.configs import cfg4_injection_plan
+
+    plan = cfg4_injection_plan()
+    wl = make_workload(4)
+    assert wl.data.atoms.shape == (4096, 7, 2880) and len(plan) == 41
+    a, t = dev(wl.data.atoms), dev(wl.data.t)
+    res = pkg.tfstat_search(a, t, EXP, wl.grid).numpy()
+    idx = sorted(plan) + [0, 1, 2, 1000, 2047, 3000, 4095]
+    ref, _ = oracle.search(wl.data.atoms[idx], wl.data.t, EXP, wl.grid)
+    for k, mg in zip(idx, ref):
+        got = res[k]
+        assert got["n_valid"] == mg.n_valid
+        assert abs(got["max2F"] - mg.max2F) <= TOL_2F * max(1.0, mg.max2F), f"tpl {k}: max2F"
+        assert abs(got["logB"] - mg.logB) <= 1e-4 * max(1.0, abs(mg.logB)), f"tpl {k}: logB"
+        if (int(got["m"]), int(got["n"])) != (mg.m, mg.n):  # allowed only on a tie in the oracle
+            full = oracle.map2F(wl.data.atoms[k], wl.data.t, EXP, wl.grid)
+            check_result(got, full["twoF"], full["flags"], wl.grid.N_tau, f"cfg4 tpl{k}")
+        if k in plan:
+            assert got["max2F"] > 30.0  # rho = 8 stands out of chi^2_4 noise
+    # every record: all cells valid (gapless data, tau >= 0.5 d), indices inside the grid,
+    # maxF <= logB <= maxF + log(n_valid)
+    assert np.all(res["n_valid"] == wl.grid.n_cells)
+    assert np.all((res["m"] >= 0) & (res["m"] < wl.grid.N_t0) & (res["n"] >= 0) &
+                  (res["n"] < wl.grid.N_tau))
+    assert np.all(res["logB"] >= 0.5 * res["max2F"] - 1e-3)
+    assert np.all(res["logB"] <= 0.5 * res["max2F"] + np.log(wl.grid.n_cells) + 1e-3)
+    # templates are independent: a launch over a slice gives the same bits
+    sub = pkg.tfstat_search(a[1000:1100], t, EXP, wl.grid).numpy()
+    assert np.array_equal(sub, res[1000:1100])
+    # and so does the exact sliding form, within tolerance, on all 4096
+    scan = pkg.tfstat_search(a, t, EXP, wl.grid, exp_method=pkg.EXP_SCAN).numpy()
+    assert np.all(np.abs(scan["max2F"] - res["max2F"]) <= TOL_2F * np.maximum(1.0, res["max2F"]))
+    assert np.all(np.abs(scan["logB"] - res["logB"]) <= 1e-4 * np.maximum(1.0, np.abs(res["logB"])))
+
+
 @pytest.mark.parametrize("window", [RECT, EXP])
 def test_config5_year_sampled(pkg, window):
     wl = make_workload(5)
