@@ -17,17 +17,26 @@ constexpr int kMargUnroll = 4;
 // exceeds it by more than 2^60 (so nothing overflows and the common path is FFMA + MUFU.EX2 + FADD
 // per cell).  Converted to a Marg at the end.
 struct StreamMarg {
-    float best;
-    int32_t idx;
+    float best;    // running max of 2F
+    int64_t qbest; // index of the 16-byte group that holds it (first one on ties)
     float ref2;
     float sum;
     int32_t nv;
 };
 constexpr float kHalfLog2eM = 0.72134752044448170368f;  // log2(e) / 2: F log2e = 2F * this
 
+__device__ __forceinline__ uint32_t flag_bytes_to_count(const uint32_t fl4)
+{
+    return ((fl4 & 0xffu) != 0u) + ((fl4 & 0xff00u) != 0u) + ((fl4 & 0xff0000u) != 0u) +
+           ((fl4 & 0xff000000u) != 0u);
+}
+
+// Four cells.  The max only remembers WHICH 16-byte group held it (two selects, no branch: with
+// ~10 groups per thread a branch on "new maximum" is taken by some lane of almost every warp);
+// the cell inside the group is found once, at the end, by re-reading that group.
 template <bool FLAGS>
 __device__ __forceinline__ void stream_add4(StreamMarg &a, const float4 v, const uint32_t fl4,
-                                            const int32_t flat0)
+                                            const int64_t q)
 {
     float x[4] = {v.x, v.y, v.z, v.w};
     if (FLAGS) {
@@ -36,21 +45,17 @@ __device__ __forceinline__ void stream_add4(StreamMarg &a, const float4 v, const
             for (int j = 0; j < 4; ++j)
                 if (((fl4 >> (8 * j)) & 0xffu) != 0u) x[j] = -INFINITY;
         }
-        a.nv += 4 - (((fl4 & 0xffu) != 0u) + ((fl4 & 0xff00u) != 0u) + ((fl4 & 0xff0000u) != 0u) +
-                     ((fl4 & 0xff000000u) != 0u));
+        a.nv += 4 - (int32_t)flag_bytes_to_count(fl4);
     } else {
         a.nv += 4;
     }
     const float m4 = fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3]));
-    if (m4 > a.best) {  // rare; ascending flat index within a thread: '>' keeps the lowest
-#pragma unroll
-        for (int j = 3; j >= 0; --j)
-            if (x[j] == m4) a.idx = flat0 + j;
-        a.best = m4;
-        if (fmaf(m4, kHalfLog2eM, -a.ref2) > 60.0f) {  // rarer: move the reference
-            a.sum *= ex2_approx(a.ref2 - m4 * kHalfLog2eM);
-            a.ref2 = m4 * kHalfLog2eM;
-        }
+    const bool up = m4 > a.best;  // ascending q within a thread: '>' keeps the first group
+    a.qbest = up ? q : a.qbest;
+    a.best = up ? m4 : a.best;
+    if (fmaf(m4, kHalfLog2eM, -a.ref2) > 60.0f) {  // rare: move the reference
+        a.sum *= ex2_approx(a.ref2 - m4 * kHalfLog2eM);
+        a.ref2 = m4 * kHalfLog2eM;
     }
     float acc = 0.0f;
 #pragma unroll
@@ -65,7 +70,7 @@ __device__ __forceinline__ void marginalise_body(const float *__restrict__ map,
 {
     StreamMarg sm;
     sm.best = -INFINITY;
-    sm.idx = 0x7fffffff;
+    sm.qbest = -1;
     sm.ref2 = -1.0e30f;  // finite: a flagged cell (-inf) must give 2^-inf = 0, not inf - inf
     sm.sum = 0.0f;
     sm.nv = 0;
@@ -86,18 +91,26 @@ __device__ __forceinline__ void marginalise_body(const float *__restrict__ map,
         }
 #pragma unroll
         for (int k = 0; k < kMargUnroll; ++k)
-            stream_add4<FLAGS>(sm, v[k], f[k], (int32_t)(4 * (q + k * stride)));
+            stream_add4<FLAGS>(sm, v[k], f[k], q + k * stride);
     }
     for (; q < n4; q += stride) {
         const float4 v = __ldcs(reinterpret_cast<const float4 *>(map) + q);
         const uint32_t f = FLAGS ? __ldcs(reinterpret_cast<const uint32_t *>(flags) + q) : 0u;
-        stream_add4<FLAGS>(sm, v, f, (int32_t)(4 * q));
+        stream_add4<FLAGS>(sm, v, f, q);
     }
     marg_init(mg);
     mg.nvalid = sm.nv;
     if (sm.best > -INFINITY) {
+        // the first unflagged cell of group qbest that equals the maximum
+        const float4 v = *(reinterpret_cast<const float4 *>(map) + sm.qbest);
+        const uint32_t f = FLAGS ? *(reinterpret_cast<const uint32_t *>(flags) + sm.qbest) : 0u;
+        const float x[4] = {v.x, v.y, v.z, v.w};
+        int jb = 3;
+#pragma unroll
+        for (int j = 3; j >= 0; --j)
+            if (x[j] == sm.best && ((f >> (8 * j)) & 0xffu) == 0u) jb = j;
         mg.best = sm.best;
-        mg.idx = sm.idx;
+        mg.idx = (int32_t)(4 * sm.qbest) + jb;
         mg.M = 0.5f * sm.best;
         mg.S = sm.sum * ex2_approx(sm.ref2 - sm.best * kHalfLog2eM);
     }
@@ -108,32 +121,17 @@ __device__ __forceinline__ void marginalise_body(const float *__restrict__ map,
     }
 }
 
-__global__ void __launch_bounds__(kMargNT)
-    marginalise_kernel(const float *__restrict__ map, const uint8_t *__restrict__ flags,
-                       const int64_t n_cells, Partial *__restrict__ partials)
-{
-    __shared__ Marg s_red[32];
-    pdl_trigger();
-    Marg mg;
-    if (flags) marginalise_body<true>(map, flags, n_cells, mg);
-    else marginalise_body<false>(map, flags, n_cells, mg);
-    marg_block_reduce<kMargNT>(mg, s_red);
-    if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
-}
-
-// One CTA per template: combine its partials (fixed order -> deterministic), write the result.
-__global__ void __launch_bounds__(256)
-    finalize_kernel(const Partial *__restrict__ partials, const int64_t per_template,
-                    const int32_t N_tau, tfstat_result *__restrict__ out)
+// Combine `per_template` partials (fixed order -> deterministic) and write one result.  Called by
+// all 256 threads of a CTA.  Plain (coherent) loads: the partials may have been written by other
+// CTAs of the same launch (marginalise_fused_kernel).
+__device__ __forceinline__ void finalize_body(const Partial *p, const int64_t per_template,
+                                              const int32_t N_tau, tfstat_result *__restrict__ out)
 {
     __shared__ float s_best[256];
     __shared__ int32_t s_idx[256];
     __shared__ float s_M[256];
     __shared__ double s_S[256];
     __shared__ int32_t s_nv[256];
-    pdl_trigger();
-    pdl_wait();  // the partial marginals of the map kernel
-    const Partial *__restrict__ p = partials + (int64_t)blockIdx.x * per_template;
     const int tid = threadIdx.x;
     float best = -INFINITY, M = -INFINITY;
     int32_t idx = 0x7fffffff, nv = 0;
@@ -189,8 +187,36 @@ __global__ void __launch_bounds__(256)
             r.n = -1;
             r.logB = -INFINITY;
         }
-        out[blockIdx.x] = r;
+        *out = r;
     }
+}
+
+// One CTA per template: combine its partials, write the result.
+__global__ void __launch_bounds__(256)
+    finalize_kernel(const Partial *__restrict__ partials, const int64_t per_template,
+                    const int32_t N_tau, tfstat_result *__restrict__ out)
+{
+    pdl_trigger();
+    pdl_wait();  // the partial marginals of the map kernel
+    finalize_body(partials + (int64_t)blockIdx.x * per_template, per_template, N_tau,
+                  out + blockIdx.x);
+}
+
+// tfstat_marginalise: stream the map into one partial per CTA; finalize_kernel follows.  (One
+// launch instead of two was measured and is no faster on B200: a cooperative launch with a grid
+// barrier costs 8.6 us per call on a 2 MB map, a memset node for a last-CTA ticket 10.4 us, the
+// two kernels chained by programmatic dependent launch 8.8 us.)
+__global__ void __launch_bounds__(kMargNT)
+    marginalise_kernel(const float *__restrict__ map, const uint8_t *__restrict__ flags,
+                       const int64_t n_cells, Partial *__restrict__ partials)
+{
+    __shared__ Marg s_red[32];
+    pdl_trigger();
+    Marg mg;
+    if (flags) marginalise_body<true>(map, flags, n_cells, mg);
+    else marginalise_body<false>(map, flags, n_cells, mg);
+    marg_block_reduce<kMargNT>(mg, s_red);
+    if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
 }
 
 }  // namespace
