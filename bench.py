@@ -267,6 +267,19 @@ def side_workloads(torch, pkg, peaks):
             out["cfg5_marginalise"] = {"cells": cells, "ms": med,
                                        "algorithmic_GBps": 4 * cells / (med * 1e-3) / 1e9,
                                        "hbm_frac": 4 * cells / (med * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    # row a5 standalone at a size where the two-launch chain is amortised: the map of one year at
+    # dt0 = dtau = T_SFT (17518 x 17519 cells, 1.23 GB), the largest of the paper's setups
+    # (PAPER.md:106, 146-148); values are arbitrary positive floats, the kernel is data-independent
+    big = torch.rand((17518, 17519), device="cuda") * 8.0
+    fn_b = lambda: pkg.tfstat_marginalise(big)
+    for _ in range(3):
+        fn_b()
+    ms_b = time_calls(torch, fn_b, 10)
+    out["marginalise_1yr_full_resolution"] = {
+        "cells": big.numel(), "ms": ms_b, "algorithmic_GBps": 4 * big.numel() / (ms_b * 1e-3) / 1e9,
+        "hbm_frac": 4 * big.numel() / (ms_b * 1e-3) / 1e9 / peaks["hbm_gbs"],
+        "l2": "1.23 GB per call > 126 MB L2, no flush"}
+    del big
     return out
 
 
