@@ -108,14 +108,14 @@ def dist_env():
 # ------------------------------------------------------------------------------------------
 # reference arm: the fp64 oracle as it stands, on the host cores
 # ------------------------------------------------------------------------------------------
-def oracle_leg(n_templates: int, seed_offset: int = 0):
+def oracle_leg(n_templates: int, seed_offset: int = 0, n_threads: int = 0):
     """Times oracle.search on `n_templates` templates of config 4.  Returns
     (terms_per_s, seconds, terms, cores)."""
     import oracle
     from synth import make_workload
 
     wl = make_workload(4, templates=range(seed_offset, seed_offset + n_templates))
-    cores = oracle.num_threads()
+    cores = n_threads if n_threads > 0 else oracle.num_threads()
     t0 = time.perf_counter()
     _, terms = oracle.search(wl.data.atoms, wl.data.t, 1, wl.grid, n_threads=cores)
     dt = time.perf_counter() - t0
@@ -422,11 +422,15 @@ def run_ours(args):
         import oracle
 
         cores = oracle.num_threads()
-        n_s = max(1, min(cores, 16))
+        n_s = 5 * max(1, min(cores, 16))  # ~10 s of CPU work: 5 templates of 2.6e8 terms per core
         v, dt, tms, used = oracle_leg(n_s)
+        v1, dt1, tms1, _ = oracle_leg(1, n_threads=1)  # comparable to Table 1's per-core constants
         cpu = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle", "seconds": dt,
                "sample": f"{n_s} of 4096 templates of config 4 (full 96x1417 grid each, "
-                         f"{tms:.3e} terms), OpenMP over templates"}
+                         f"{tms:.3e} terms), OpenMP over templates",
+               "single_core": {"value": v1, "unit": UNIT, "seconds": dt1,
+                               "seconds_per_term": dt1 / tms1,
+                               "sample": f"1 template, {tms1:.3e} terms, 1 thread"}}
 
     side = None if args.no_side else side_workloads(torch, pkg, peaks)
     if side is not None:
