@@ -267,6 +267,24 @@ def side_workloads(torch, pkg, peaks):
             out["cfg5_marginalise"] = {"cells": cells, "ms": med,
                                        "algorithmic_GBps": 4 * cells / (med * 1e-3) / 1e9,
                                        "hbm_frac": 4 * cells / (med * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    # config 1 (24 x 24 cells, 48 atoms; Fig. 3's one-day data set): one launch of
+    # the small-map kernel; and the same shape x 1000 seeded templates (Fig. 3's 1000 bins)
+    from synth import Grid as _G, tiny_workload as _tw
+    wl1 = make_workload(1)
+    a1 = torch.from_numpy(wl1.data.atoms).cuda()
+    t1 = torch.from_numpy(wl1.data.t).cuda()
+    ws1 = torch.empty(pkg.workspace_bytes(0, 48, 1000, wl1.grid), dtype=torch.uint8, device="cuda")
+    fn1 = lambda: pkg.tfstat_search(a1, t1, 0, wl1.grid, workspace=ws1, want_maps=True)
+    wlk = _tw(11, 48, 0.0, _G(0, 1800, 24, 1800, 1800, 24), n_templates=1000, phi_random=True)
+    ak = torch.from_numpy(wlk.data.atoms).cuda()
+    fnk = lambda: pkg.tfstat_search(ak, t1, 0, wl1.grid, workspace=ws1)
+    for _ in range(3):
+        fn1()
+        fnk()
+    out["cfg1_rect"] = {"cells": wl1.grid.n_cells, "map_and_marginals_ms": timed(fn1)[1],
+                        "x1000_templates_fused_ms": time_calls(torch, fnk, 10),
+                        "note": "one launch (rect_small_kernel); single-call time is host-launch bound"}
+    out["cfg1_rect"]["x1000_cells_per_s"] = 576e3 / (out["cfg1_rect"]["x1000_templates_fused_ms"] * 1e-3)
     # row a5 standalone at a size where the two-launch chain is amortised: the map of one year at
     # dt0 = dtau = T_SFT (17518 x 17519 cells, 1.23 GB), the largest of the paper's setups
     # (PAPER.md:106, 146-148); values are arbitrary positive floats, the kernel is data-independent

@@ -84,7 +84,9 @@ typedef struct tfstat_opts {
                            0 = chosen from the problem shape                               */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
     int32_t seg_len;    /* tuning (TFSTAT_EXP_SCAN): t0 steps per sliding segment; 0 = auto   */
-    int32_t reserved;   /* must be 0                                                       */
+    int32_t rect_method; /* rectangular window: 0 = auto; 1 = never the one-launch small-map
+                           kernel (lattice / per-cell kernels only); 2 = the small-map kernel
+                           whenever the atoms fit its shared memory (n_atoms <= 2048)          */
     /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
      * immediately before and after the dominant kernel of the call (the window-sum +
      * closure kernel; for the rectangular window: prefix + cells kernels).  NULL = off. */

@@ -32,7 +32,7 @@ class TfstatError(RuntimeError):
 class _Opts(C.Structure):
     _fields_ = [("min_atoms", C.c_int32), ("exp_method", C.c_int32),
                 ("tile_c", C.c_int32), ("tile_nt", C.c_int32), ("seg_len", C.c_int32),
-                ("reserved", C.c_int32), ("ev_main_begin", C.c_void_p),
+                ("rect_method", C.c_int32), ("ev_main_begin", C.c_void_p),
                 ("ev_main_end", C.c_void_p)]
 
 
@@ -97,10 +97,11 @@ def _grid_args(g):
     return [int(g.t0_min), int(g.dt0), int(g.N_t0), int(g.tau_min), int(g.dtau), int(g.N_tau)]
 
 
-def _opts(min_atoms: int, exp_method: int, events=None, tile=None) -> _Opts:
+def _opts(min_atoms: int, exp_method: int, events=None, tile=None, rect_method: int = 0) -> _Opts:
     o = _Opts()
     o.min_atoms = int(min_atoms)
     o.exp_method = int(exp_method)
+    o.rect_method = int(rect_method)
     if tile is not None:  # (cells per thread, threads per CTA[, t0 steps per segment]): tuning
         o.tile_c, o.tile_nt = int(tile[0]), int(tile[1])
         if len(tile) > 2:
@@ -131,9 +132,9 @@ def _dev_i32(x: torch.Tensor, name: str) -> torch.Tensor:
 
 
 def workspace_bytes(window: int, n_atoms: int, n_templates: int, grid, *, min_atoms: int = 2,
-                    exp_method: int = EXP_AUTO, tile=None) -> int:
+                    exp_method: int = EXP_AUTO, tile=None, rect_method: int = 0) -> int:
     lib = load_library()
-    o = _opts(min_atoms, exp_method, tile=tile)
+    o = _opts(min_atoms, exp_method, tile=tile, rect_method=rect_method)
     n = lib.tfstat_workspace_bytes(window, n_atoms, n_templates, *_grid_args(grid), C.byref(o))
     if n == 0:
         raise TfstatError("tfstat_workspace_bytes: invalid problem shape")
@@ -171,7 +172,7 @@ class Results:
 def tfstat_map(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
                min_atoms: int = 2, exp_method: int = EXP_AUTO, want_flags: bool = False,
                out_map: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
-               stream=None, tile=None):
+               stream=None, tile=None, rect_method: int = 0):
     """atoms [7, N] (row stride = ld) -> (map [N_t0, N_tau] fp32 of 2F, flags uint8 or None)."""
     lib = load_library()
     _dev_f32(atoms, "atoms")
@@ -187,9 +188,9 @@ def tfstat_map(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,
     flags = (torch.empty((grid.N_t0, grid.N_tau), dtype=torch.uint8, device=dev)
              if want_flags else None)
     nbytes = workspace_bytes(window, n_atoms, 1, grid, min_atoms=min_atoms, exp_method=exp_method,
-                             tile=tile)
+                             tile=tile, rect_method=rect_method)
     ws = _workspace(nbytes, dev, workspace)
-    o = _opts(min_atoms, exp_method, tile=tile)
+    o = _opts(min_atoms, exp_method, tile=tile, rect_method=rect_method)
     rc = lib.tfstat_map(atoms.data_ptr(), ld, t_atoms.data_ptr(), n_atoms, window,
                         *_grid_args(grid), out_map.data_ptr(),
                         flags.data_ptr() if flags is not None else None, ws.data_ptr(), nbytes,
@@ -222,7 +223,7 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
                   min_atoms: int = 2, exp_method: int = EXP_AUTO, want_maps: bool = False,
                   want_flags: bool = False, workspace: Optional[torch.Tensor] = None,
                   out: Optional[torch.Tensor] = None, stream=None,
-                  main_kernel_events=None, tile=None) -> Results:
+                  main_kernel_events=None, tile=None, rect_method: int = 0) -> Results:
     """atoms [T, 7, N] -> marginals of the T maps (and the maps / flags if asked)."""
     lib = load_library()
     _dev_f32(atoms, "atoms")
@@ -241,9 +242,9 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
     flags = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.uint8, device=dev)
              if want_flags else None)
     nbytes = workspace_bytes(window, n_atoms, T, grid, min_atoms=min_atoms, exp_method=exp_method,
-                             tile=tile)
+                             tile=tile, rect_method=rect_method)
     ws = _workspace(nbytes, dev, workspace)
-    o = _opts(min_atoms, exp_method, main_kernel_events, tile=tile)
+    o = _opts(min_atoms, exp_method, main_kernel_events, tile=tile, rect_method=rect_method)
     rc = lib.tfstat_search(atoms.data_ptr(), tstride, ld, t_atoms.data_ptr(), n_atoms, T, window,
                            *_grid_args(grid), out.data_ptr(),
                            maps.data_ptr() if maps is not None else None,

@@ -126,6 +126,13 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         pl.seg_len = len;
         pl.n_segs = (N_t0 + len - 1) / len;
     }
+    if (window == TFSTAT_WINDOW_RECT) {
+        const int rm = opts ? opts->rect_method : 0;
+        if (rm < 0 || rm > 2) return pl;
+        pl.rect_small = rm == 1   ? 0
+                        : rm == 2 ? (n_atoms <= 2048)
+                                  : rect_small_applies(n_atoms, n_templates, cells);
+    }
     if (window == TFSTAT_WINDOW_RECT)
         pl.rect = plan_rect_run(pl.grid, pl.e_m, pl.e_n, pl.J, n_templates, opts ? opts->tile_c : 0,
                                 opts ? opts->seg_len : 0);
@@ -167,9 +174,14 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
                       const int32_t *t_atoms, tfstat_result *out, float *out_maps,
                       uint8_t *out_flags, void *ws, cudaStream_t st, bool do_bounds)
 {
-    if (do_bounds) TF_CUDA(launch_bounds(pl, t_atoms, ws, st));
-    else if (pl.flags_bytes)
+    const bool small = pl.window == TFSTAT_WINDOW_RECT && pl.rect_small;
+    if (small) {
+        // one launch does bounds, sums, closure, marginals and the result record
+    } else if (do_bounds) {
+        TF_CUDA(launch_bounds(pl, t_atoms, ws, st));
+    } else if (pl.flags_bytes) {
         TF_CUDA(cudaMemsetAsync(static_cast<char *>(ws) + pl.off_flags, 0, pl.flags_bytes, st));
+    }
     Problem pr;
     pr.atoms = atoms;
     pr.template_stride = template_stride;
@@ -184,6 +196,11 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     Partial *partials =
         out ? reinterpret_cast<Partial *>(static_cast<char *>(ws) + pl.off_partials) : nullptr;
     if (pl.ev_main_begin) TF_CUDA(cudaEventRecord(pl.ev_main_begin, st));
+    if (small) {
+        TF_CUDA(launch_rect_small(pl, pr, st));
+        if (pl.ev_main_end) TF_CUDA(cudaEventRecord(pl.ev_main_end, st));
+        return TFSTAT_OK;
+    }
     if (pl.window == TFSTAT_WINDOW_RECT) {
         double *prefix = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_prefix);
         double *agg = reinterpret_cast<double *>(static_cast<char *>(ws) + pl.off_tot);

@@ -42,6 +42,7 @@ struct Plan {
     int window;
     int exp_method;
     int32_t n_atoms, n_templates, min_atoms;
+    int32_t rect_small;  // rectangular window: the one-launch kernel of rect.cu runs this call
     Grid grid;
     // a1 edge lattice
     int64_t g;  // lattice step (s)
@@ -76,6 +77,8 @@ cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partia
 RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates,
                       int32_t q_override, int32_t seg_override);
 int rect_scan_blocks(int32_t n_atoms);
+bool rect_small_applies(int32_t n_atoms, int32_t n_templates, int64_t cells);
+cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st);
 cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,
                         int32_t *flags, void *steps, Partial *partials, cudaStream_t st);
 cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,

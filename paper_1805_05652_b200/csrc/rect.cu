@@ -337,6 +337,109 @@ __global__ void __launch_bounds__(kCellNT)
 }
 
 // ---------------------------------------------------------------------------------------
+// small problems: everything in ONE launch, one CTA per template
+//
+// A call on a small map is otherwise a chain of four dependent launches (bounds, scan, cells,
+// finalize) of ~5 us each whatever the size -- the "overhead-dominated" regime the paper
+// reports for rectangular windows on GPUs.  Here a CTA stages the timestamps and
+// the fp64 prefix sums of its template in shared memory (one warp per channel), finds lo / hi of
+// every cell by binary search in shared memory, closes in fp64, reduces its marginals and
+// writes the tfstat_result itself: BASELINE.json config 1 (24 x 24 cells, 48 atoms) in one
+// launch, 1000 such templates in one wave.
+// ---------------------------------------------------------------------------------------
+constexpr int kSmallNT = 256;
+
+__device__ __forceinline__ int lower_bound_s(const int32_t *s_t, const int n, const long long x)
+{
+    int a = 0, b = n;
+    while (a < b) {
+        const int mid = (a + b) >> 1;
+        if ((long long)s_t[mid] < x) a = mid + 1;
+        else b = mid;
+    }
+    return a;
+}
+
+__global__ void __launch_bounds__(kSmallNT)
+    rect_small_kernel(const Problem pr)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ Marg s_red[32];
+    const Grid g = pr.grid;
+    const int N = pr.bounds.n_atoms;
+    double *s_P = reinterpret_cast<double *>(smem_raw);              // [(N + 1)][8], 7 used
+    int32_t *s_t = reinterpret_cast<int32_t *>(s_P + (size_t)(N + 1) * 8);  // [N]
+    const int tpl = blockIdx.x;
+    const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    for (int i = threadIdx.x; i < N; i += kSmallNT) s_t[i] = __ldg(pr.bounds.t + i);
+    // a2: exclusive fp64 prefix of channel `warp`, 32 atoms per step of a warp-wide scan
+    if (warp < 7) {
+        const float *__restrict__ row = base + warp * pr.ld;
+        double carry = 0.0;
+        if (lane == 0) s_P[warp] = 0.0;
+        for (int i0 = 0; i0 < N; i0 += 32) {
+            const int i = i0 + lane;
+            double v = i < N ? (double)__ldg(row + i) : 0.0;
+#pragma unroll
+            for (int sh = 1; sh < 32; sh <<= 1) {
+                const double up = __shfl_up_sync(0xffffffffu, v, sh);
+                if (lane >= sh) v += up;
+            }
+            v += carry;
+            if (i < N) s_P[(size_t)(i + 1) * 8 + warp] = v;
+            carry = __shfl_sync(0xffffffffu, v, 31);
+        }
+    }
+    __syncthreads();
+
+    Marg mg;
+    marg_init(mg);
+    const int n_cells = g.N_t0 * g.N_tau;
+    const int64_t map_base = (int64_t)tpl * n_cells;
+    for (int i = threadIdx.x; i < n_cells; i += kSmallNT) {
+        const int m = i / g.N_tau, n = i - m * g.N_tau;
+        const long long t0 = t0_of(g, m);
+        const int lo = lower_bound_s(s_t, N, t0);
+        const int hi = lower_bound_s(s_t, N, t0 + tau_of(g, n));  // k = 1: rectangular
+        const double *pl = s_P + (size_t)lo * 8, *ph = s_P + (size_t)hi * 8;
+        Sums64 s;
+        s.A = ph[0] - pl[0];
+        s.B = ph[1] - pl[1];
+        s.C = ph[2] - pl[2];
+        s.far = ph[3] - pl[3];
+        s.fai = ph[4] - pl[4];
+        s.fbr = ph[5] - pl[5];
+        s.fbi = ph[6] - pl[6];
+        uint32_t fl;
+        const float twoF = closure_2F(s, hi - lo, pr.min_atoms, fl);
+        if (pr.out_maps) pr.out_maps[map_base + i] = twoF;
+        if (pr.out_flags) pr.out_flags[map_base + i] = (uint8_t)fl;
+        if (!fl) marg_add(mg, twoF, i);
+    }
+    if (pr.out) {
+        marg_block_reduce<kSmallNT>(mg, s_red);
+        if (threadIdx.x == 0) {
+            tfstat_result r;
+            r.n_valid = mg.nvalid;
+            if (mg.nvalid > 0) {
+                r.max2F = mg.best;
+                r.m = mg.idx / g.N_tau;
+                r.n = mg.idx % g.N_tau;
+                r.logB = (float)((double)mg.M + log((double)mg.S));
+            } else {
+                r.max2F = 0.0f;
+                r.m = -1;
+                r.n = -1;
+                r.logB = -INFINITY;
+            }
+            pr.out[tpl] = r;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // running-sum kernel
 // ---------------------------------------------------------------------------------------
 constexpr int kRunNT = 128;
@@ -834,6 +937,23 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     rr.seg_cols = seg;
     rr.n_coltiles = (g.N_tau + seg - 1) / seg;
     return rr;
+}
+
+// One CTA per template pays off while the map is small, or while the templates alone fill the GPU
+bool rect_small_applies(int32_t n_atoms, int32_t n_templates, int64_t cells)
+{
+    if (n_atoms > 2048) return false;  // 64 B of fp64 prefix + 4 B per atom in shared memory
+    return cells <= 4096 || (n_templates >= 148 * 4 && cells <= 32768);
+}
+
+cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st)
+{
+    const size_t smem = (size_t)(pl.n_atoms + 1) * 64 + (size_t)pl.n_atoms * 4;
+    cudaError_t e = cudaFuncSetAttribute(rect_small_kernel,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    rect_small_kernel<<<(unsigned)pl.n_templates, kSmallNT, smem, st>>>(pr);
+    return cudaGetLastError();
 }
 
 int rect_scan_blocks(int32_t n_atoms) { return (n_atoms + kScanBlock - 1) / kScanBlock; }

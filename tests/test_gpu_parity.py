@@ -77,6 +77,15 @@ def test_tiny_maps(pkg, window, seed, slots, gaps, grid):
     assert pkg.count_terms(dev(t), window, grid) == int(ref["cnt"].sum())
     r = pkg.tfstat_marginalise(dev(m), dev(f)).numpy()[0]
     check_result(r, ref["twoF"], ref["flags"], grid.N_tau, f"tiny{seed} marginalise")
+    if window == RECT:
+        # both families of rectangular kernels on every case: 1 = lattice / per-cell kernels,
+        # 2 = the one-launch small-map kernel (needs n_atoms <= 2048)
+        for method in (1, 2) if t.shape[0] <= 2048 else (1,):
+            m2, f2 = run_map(pkg, atoms, t, window, grid, rect_method=method)
+            check_cells(m2, f2, ref, f"tiny{seed} rect_method {method}")
+            res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, grid, rect_method=method)
+            check_result(res.numpy()[0], ref["twoF"], ref["flags"], grid.N_tau,
+                         f"tiny{seed} rect_method {method} fused")
 
 
 @pytest.mark.parametrize("window", [RECT, EXP])
@@ -99,6 +108,16 @@ def test_search_batched_small(pkg, window):
     # results-only call gives the same records
     res2 = pkg.tfstat_search(a, dev(wl.data.t), window, grid)
     assert np.array_equal(res2.numpy(), got)
+    if window == RECT:  # the batched call through both families of rectangular kernels
+        for method in (1, 2):
+            r3 = pkg.tfstat_search(a, dev(wl.data.t), window, grid, want_maps=True,
+                                   want_flags=True, rect_method=method)
+            for k in range(T):
+                ref = oracle.map2F(wl.data.atoms[k], wl.data.t, window, grid)
+                check_cells(r3.maps[k].cpu().numpy(), r3.flags[k].cpu().numpy(), ref,
+                            f"tpl{k} rect_method {method}")
+                check_result(r3.numpy()[k], ref["twoF"], ref["flags"], grid.N_tau,
+                             f"tpl{k} rect_method {method}")
 
 
 @pytest.mark.parametrize("world", [2, 3])
