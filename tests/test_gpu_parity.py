@@ -137,6 +137,46 @@ def test_sharded_search_equals_unsharded(pkg, world):
         assert np.array_equal(np.concatenate(parts), full)
 
 
+@pytest.mark.parametrize("window,method", [(EXP, 0), (RECT, 1), (RECT, 2)])
+def test_calls_are_capturable_in_a_cuda_graph(pkg, window, method):
+    """The device-pointer calls only enqueue kernels on the caller's stream (no allocation, no
+    synchronisation), so a search can be captured once and replayed on new atoms."""
+    grid = Grid(0, 1800, 23, 3600, 3600, 140)
+    wl = tiny_workload(205, 300, 0.0, grid, n_templates=3, phi_random=True)
+    a, t = dev(wl.data.atoms), dev(wl.data.t)
+    ws = torch.empty(pkg.workspace_bytes(window, int(t.shape[0]), 3, grid, rect_method=method),
+                     dtype=torch.uint8, device="cuda")
+    out = torch.empty((3, 5), dtype=torch.int32, device="cuda")
+    call = lambda: pkg.tfstat_search(a, t, window, grid, workspace=ws, out=out,  # noqa: E731
+                                     rect_method=method)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        call()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        call()
+    for seed in (206, 207):  # replay on new atoms written into the captured buffers
+        wl2 = tiny_workload(seed, 300, 0.0, grid, n_templates=3, phi_random=True)
+        assert np.array_equal(wl2.data.t, wl.data.t)  # gapless: same time stamps
+        a.copy_(dev(wl2.data.atoms))
+        out.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().view(pkg.RESULT_DTYPE).reshape(-1)
+        for k in range(3):
+            ref = oracle.map2F(wl2.data.atoms[k], wl2.data.t, window, grid)
+            check_result(got[k], ref["twoF"], ref["flags"], grid.N_tau, f"graph replay tpl{k}")
+    # and the captured call itself reproduces the eager result
+    a.copy_(dev(wl.data.atoms))
+    eager = pkg.tfstat_search(a, t, window, grid, rect_method=method).numpy()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().view(pkg.RESULT_DTYPE).reshape(-1), eager)
+
+
 def test_search_host_equals_device(pkg):
     grid = Grid(0, 1800, 16, 3600, 1800, 100)
     wl = tiny_workload(202, 260, 0.05, grid, n_templates=9, phi_random=True)
