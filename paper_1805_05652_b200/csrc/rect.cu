@@ -442,7 +442,7 @@ __global__ void __launch_bounds__(kSmallNT)
 // ---------------------------------------------------------------------------------------
 // running-sum kernel
 // ---------------------------------------------------------------------------------------
-constexpr int kRunNT = 128;
+constexpr int kRunNT = 64;   // 2 warps per CTA: measured 5 % faster than 128 (cheaper transpose barrier)
 constexpr int kChunk = 16;   // columns between two write-outs of the transposed tile
 constexpr int kPitch = 16;   // floats per tile row; the four 16-byte column groups of row i are
                              // XOR-swizzled with (i >> 1) & 3: conflict-free STS.128 and LDS.128
@@ -522,10 +522,10 @@ __device__ __forceinline__ PairOut pair_closure(const u64 (&S)[8])
     return o;
 }
 
-// 4 CTAs per SM for Q = 2 (128 registers): measured on B200 against 3 (162 registers, no spill),
-// 5 (96) and 6 (80, spilling) CTAs per SM, which are 13 % to 58 % slower on config 5
+// 16 warps per SM for Q = 2 (128 registers): measured on B200 against 12 (162 registers, no
+// spill), 20 (96) and 24 (80, spilling) warps per SM, which are 13 % to 58 % slower on config 5
 template <int Q, bool MARG>
-__global__ void __launch_bounds__(kRunNT, Q == 2 ? 4 : 5)
+__global__ void __launch_bounds__(kRunNT, Q == 2 ? 8 : 10)
     rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
                     const ulonglong2 *__restrict__ K, Partial *__restrict__ partials,
                     const int roff, const int R, const int seg_cols, const int n_rowtiles,
@@ -924,7 +924,7 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     int64_t best_cost = INT64_MAX;
     for (int cand = seg_max; cand >= kChunk; cand -= kChunk) {
         const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
-        const int64_t per_wave = 148 * (rr.Q == 2 ? 4 : 5);
+        const int64_t per_wave = 148 * (rr.Q == 2 ? 8 : 10);
         const int64_t waves = (ctas + per_wave - 1) / per_wave;
         const int64_t cost = waves * (cand + 24);
         if (cost < best_cost) {
