@@ -47,7 +47,7 @@ extern "C" {
 #define TFSTAT_WINDOW_TABLE 2 /* tfstat_map_general only: w(u) tabulated, u = (t - t0)/tau    */
 
 /* how the exponential-window sums are evaluated (tfstat_opts.exp_method) */
-#define TFSTAT_EXP_AUTO 0   /* = DIRECT */
+#define TFSTAT_EXP_AUTO 0   /* = SCAN (exact, and never slower than DIRECT: DESIGN.md 6.2) */
 #define TFSTAT_EXP_DIRECT 1 /* truncated weighted sum per cell, the paper's
                                brute-force definition, register-tiled                     */
 #define TFSTAT_EXP_SCAN 2   /* exact factorised, sliding form: per tau, weights

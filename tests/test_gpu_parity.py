@@ -22,7 +22,26 @@ def pkg():
 
     p.load_library()  # fails loudly if libtfstat.so is missing: there is no fallback
     assert torch.cuda.is_available()
-    return p
+    return _DirectByDefault(p)
+
+
+class _DirectByDefault:
+    """The package with exp_method defaulting to EXP_DIRECT, so that every test written against
+    the default exercises the direct-sum kernel; the sliding form (what EXP_AUTO resolves to) is
+    tested by the tests that ask for EXP_SCAN / EXP_AUTO explicitly."""
+
+    def __init__(self, p):
+        self._p = p
+
+    def __getattr__(self, name):
+        f = getattr(self._p, name)
+        if name in ("tfstat_map", "tfstat_search", "tfstat_search_host", "workspace_bytes",
+                    "search_host_scratch_bytes"):
+            def g(*a, **k):
+                k.setdefault("exp_method", self._p.EXP_DIRECT)
+                return f(*a, **k)
+            return g
+        return f
 
 
 def dev(x):
@@ -395,6 +414,38 @@ def test_tiny_maps_exp_scan(pkg, seed, slots, gaps, grid, seg_len):
     res = pkg.tfstat_search(dev(atoms[None]), dev(t), EXP, grid, exp_method=SCAN,
                             tile=(0, 0, seg_len)).numpy()[0]
     check_result(res, ref["twoF"], ref["flags"], grid.N_tau, f"scan tiny{seed} seg{seg_len}")
+
+
+def test_exp_auto_is_the_sliding_form(pkg):
+    """EXP_AUTO (what a caller gets without options) resolves to the exact sliding form: same bits
+    as EXP_SCAN, within tolerance of the oracle, and of the direct sum."""
+    grid = Grid(0, 1800, 37, 3600, 1800, 300)
+    wl = tiny_workload(102, 400, 0.2, grid, n_templates=3, phi_random=True)
+    a, t = dev(wl.data.atoms), dev(wl.data.t)
+    auto = pkg.tfstat_search(a, t, EXP, grid, exp_method=pkg.EXP_AUTO, want_maps=True,
+                             want_flags=True)
+    scan = pkg.tfstat_search(a, t, EXP, grid, exp_method=pkg.EXP_SCAN, want_maps=True,
+                             want_flags=True)
+    direct = pkg.tfstat_search(a, t, EXP, grid, exp_method=pkg.EXP_DIRECT, want_maps=True)
+    assert np.array_equal(auto.numpy(), scan.numpy())
+    assert torch.equal(auto.maps, scan.maps) and torch.equal(auto.flags, scan.flags)
+    assert not torch.equal(auto.maps, direct.maps)  # a different kernel did run
+    for k in range(3):
+        ref = oracle.map2F(wl.data.atoms[k], wl.data.t, EXP, grid)
+        check_cells(auto.maps[k].cpu().numpy(), auto.flags[k].cpu().numpy(), ref, f"auto tpl{k}")
+        check_result(auto.numpy()[k], ref["twoF"], ref["flags"], grid.N_tau, f"auto tpl{k}")
+    # NULL options at the C level are AUTO too
+    lib = pkg.load_library()
+    out = torch.empty((3, 5), dtype=torch.int32, device="cuda")
+    ws = torch.empty(pkg.workspace_bytes(EXP, int(t.shape[0]), 3, grid, exp_method=pkg.EXP_AUTO),
+                     dtype=torch.uint8, device="cuda")
+    rc = lib.tfstat_search(a.data_ptr(), a.stride(0), a.stride(1), t.data_ptr(), int(t.shape[0]), 3,
+                           EXP, grid.t0_min, grid.dt0, grid.N_t0, grid.tau_min, grid.dtau,
+                           grid.N_tau, out.data_ptr(), None, None, ws.data_ptr(), ws.numel(),
+                           torch.cuda.current_stream().cuda_stream, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().view(pkg.RESULT_DTYPE).reshape(-1), auto.numpy())
 
 
 def test_exp_scan_long_gaps_and_disjoint_windows(pkg):
