@@ -84,6 +84,38 @@ __device__ __forceinline__ float closure_2F(const Sums64 &s, int cnt, int min_at
     return (float)(2.0 * num / D);
 }
 
+// fp32 closure for well-conditioned cells, fp64 for the rest.  With D > AB/64 the cancellation
+// in D = AB - C^2 and in the numerator amplifies the fp32 rounding of the inputs by at most ~64,
+// i.e. <= ~1e-5 relative on 2F, two orders below the 1e-3 contract; everything else (small D,
+// count-degenerate cells, NaN) takes the fp64 path, which also decides the flags.
+__device__ __forceinline__ float closure_2F_mixed(const float A, const float B, const float C,
+                                                  const float far, const float fai,
+                                                  const float fbr, const float fbi, const int cnt,
+                                                  const int min_atoms, uint32_t &flags)
+{
+    const float p = A * B;
+    const float D = fmaf(-C, C, p);
+    if (D > 0.015625f * p && cnt >= min_atoms) {
+        const float na = fmaf(far, far, fai * fai);
+        const float nb = fmaf(fbr, fbr, fbi * fbi);
+        const float re = fmaf(far, fbr, fai * fbi);
+        float num = B * na;
+        num = fmaf(A, nb, num);
+        num = fmaf(-2.0f * C, re, num);
+        flags = 0u;
+        return 2.0f * __fdividef(num, D);
+    }
+    Sums64 s;
+    s.A = A;
+    s.B = B;
+    s.C = C;
+    s.far = far;
+    s.fai = fai;
+    s.fbr = fbr;
+    s.fbi = fbi;
+    return closure_2F(s, cnt, min_atoms, flags);
+}
+
 // ---------------------------------------------------------------------------------------
 // step a5: marginalisation state (max 2F with lowest-index argmax; online log-sum-exp)
 // ---------------------------------------------------------------------------------------
