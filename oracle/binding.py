@@ -117,6 +117,28 @@ def map2F_general(atoms, t, kind, support, t0_grid, tau_grid, table=None, min_at
     return dict(twoF=twoF, flags=flags, cond=cond, cnt=cnt)
 
 
+def merge_detectors(atoms_dets, t_dets, t_out):
+    """atoms_dets: list of [7, N_x] fp32 arrays, t_dets: list of [N_x] int32 -> [7, len(t_out)] fp32."""
+    n_det = len(atoms_dets)
+    A = [np.ascontiguousarray(a, dtype=np.float32) for a in atoms_dets]
+    T = [np.ascontiguousarray(t, dtype=np.int32) for t in t_dets]
+    t_out = np.ascontiguousarray(t_out, dtype=np.int32)
+    out = np.empty((7, t_out.shape[0]), np.float32)
+    pa = (C.c_void_p * n_det)(*[a.ctypes.data for a in A])
+    pt = (C.c_void_p * n_det)(*[t.ctypes.data for t in T])
+    lds = (C.c_int64 * n_det)(*[a.shape[1] for a in A])
+    ns = (C.c_int32 * n_det)(*[t.shape[0] for t in T])
+    lib = _load()
+    lib.oracle_merge_detectors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
+                                           C.c_int64]
+    rc = lib.oracle_merge_detectors(pa, lds, pt, ns, n_det, _ptr(t_out), t_out.shape[0],
+                                    _ptr(out), out.shape[1])
+    if rc != 0:
+        raise ValueError(f"oracle_merge_detectors rc={rc}")
+    return out
+
+
 def cells(atoms, t, window, grid, ms, ns, min_atoms: int = 2, n_threads: int = 0):
     """The same per-cell definition on a list of (m, n) cells."""
     atoms, t = _check_atoms(atoms, t)

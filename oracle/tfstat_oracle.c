@@ -350,6 +350,43 @@ int oracle_tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t, 
     return 0;
 }
 
+/* ---------------------------------------------------------------------------------------
+ * Per-detector input.  The paper's atoms carry an index "over SFTs"
+ * and the map function sums whatever atoms fall into a window; with several
+ * detectors the SFTs of one time stamp contribute together.  The map entry points take atoms
+ * already merged per time stamp (BASELINE.json configs: "2 detectors merged per timestamp");
+ * this is that merge, written out: for every output time stamp t_out[i] and every channel,
+ *     out[ch][i] = sum over detectors X, in the order given, of atoms_X[ch][j]  with t_X[j] == t_out[i]
+ * in fp32 (the atoms are real32; a fixed order makes the sum reproducible to the
+ * bit).  Atoms of a detector whose time stamp is not in t_out are dropped; a t_out[i] that no
+ * detector has gives zeros.  PARITY UNPINNED BY THE PAPER (it does not describe the merge);
+ * pinned against numpy and against the merged atom model of synth/.
+ * --------------------------------------------------------------------------------------- */
+int oracle_merge_detectors(const float *const *atoms_dets, const int64_t *lds,
+                           const int32_t *const *t_dets, const int32_t *n_dets, int32_t n_det,
+                           const int32_t *t_out, int32_t n_out, float *out_atoms, int64_t ld_out)
+{
+    if (!atoms_dets || !lds || !t_dets || !n_dets || n_det < 1 || !t_out || n_out < 1 ||
+        !out_atoms || ld_out < n_out)
+        return -1;
+    for (int32_t i = 0; i < n_out; ++i) {
+        for (int ch = 0; ch < 7; ++ch) {
+            float acc = 0.0f;
+            for (int32_t x = 0; x < n_det; ++x) {
+                /* linear search: plain and obviously right; the sets are small in the tests */
+                for (int32_t j = 0; j < n_dets[x]; ++j) {
+                    if (t_dets[x][j] == t_out[i]) {
+                        acc += atoms_dets[x][ch * lds[x] + j];
+                        break;
+                    }
+                }
+            }
+            out_atoms[ch * ld_out + i] = acc;
+        }
+    }
+    return 0;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP

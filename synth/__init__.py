@@ -14,6 +14,7 @@ from .atoms import (  # noqa: F401
     antenna_terms,
     gap_mask,
     make_atoms,
+    make_detector_atoms,
     inject_exponential,
     inject_rectangular,
     template_seed,

@@ -121,6 +121,24 @@ def make_atoms(t: np.ndarray, rng: np.random.Generator, phi: float = 0.0,
     return out
 
 
+def make_detector_atoms(t: np.ndarray, rng: np.random.Generator, phi: float = 0.0) -> np.ndarray:
+    """The same atom model per detector, NOT merged: [2, 7, N] fp64 with rows a_d^2, b_d^2,
+    a_d b_d, Re/Im(a_d n_d), Re/Im(b_d n_d).  Draws the noise exactly like `make_atoms`, so for
+    the same generator state the sum over d is `make_atoms` up to fp64 rounding order.  Input
+    for the per-detector entry point (tfstat_merge_detectors): each detector may then keep its
+    own subset of the time stamps."""
+    a, b = antenna_terms(t, phi)
+    n = t.shape[0]
+    z = rng.normal(0.0, np.sqrt(0.5), size=(2, 2, n))  # [d, re/im, N]
+    nd = z[:, 0, :] + 1j * z[:, 1, :]
+    out = np.empty((2, 7, n), dtype=np.float64)
+    out[:, 0], out[:, 1], out[:, 2] = a * a, b * b, a * b
+    fa, fb = a * nd, b * nd
+    out[:, 3], out[:, 4] = fa.real, fa.imag
+    out[:, 5], out[:, 6] = fb.real, fb.imag
+    return out
+
+
 def _inject(atoms32: np.ndarray, W: np.ndarray, rho: float,
             rng: np.random.Generator) -> Tuple[complex, complex]:
     """Add W*(c1 a2 + c2 ab) to Fa and W*(c1 ab + c2 b2) to Fb in place.

@@ -118,3 +118,53 @@ def test_general_oracle_rejects_bad_arguments():
         map2F_general(atoms, t, EXP, (0, 1), g.t0(), g.tau())              # empty support
     with pytest.raises(ValueError):
         map2F_general(atoms, t, EXP, (3, 1), g.t0(), np.array([0, 1800]))  # tau < 1
+
+
+# ----------------------------------------------------------------------------------------
+# per-detector merge (oracle_merge_detectors)
+# ----------------------------------------------------------------------------------------
+def _detector_sets(seed=41, n_slots=300):
+    from synth import make_detector_atoms
+
+    rng = np.random.default_rng(seed)
+    t = (np.arange(n_slots) * TSFT).astype(np.int32)
+    per_det = make_detector_atoms(t, np.random.default_rng(seed + 1)).astype(np.float32)
+    keep = [rng.random(n_slots) > 0.25, rng.random(n_slots) > 0.4]  # each detector's own gaps
+    keep[0][:3] = False                                              # a slot neither detector has
+    keep[1][:3] = False
+    atoms = [np.ascontiguousarray(per_det[d][:, keep[d]]) for d in (0, 1)]
+    ts = [t[keep[d]] for d in (0, 1)]
+    return t, per_det, keep, atoms, ts
+
+
+def test_merge_detectors_against_numpy_bit_exact():
+    from oracle.binding import merge_detectors
+
+    t, per_det, keep, atoms, ts = _detector_sets()
+    t_out = np.union1d(ts[0], ts[1]).astype(np.int32)
+    got = merge_detectors(atoms, ts, t_out)
+    ref = np.zeros((7, len(t_out)), np.float32)
+    for d in (0, 1):  # independent formulation: scatter by searchsorted, fp32 adds, same order
+        ref[:, np.searchsorted(t_out, ts[d])] += atoms[d]
+    assert got.dtype == np.float32 and np.array_equal(got, ref)
+    # a time stamp nobody has gives zeros; atoms outside t_out are dropped
+    t_odd = np.concatenate([[0], t_out[::2]]).astype(np.int32)
+    got2 = merge_detectors(atoms, ts, t_odd)
+    assert np.all(got2[:, 0] == 0.0) and np.array_equal(got2[:, 1:], ref[:, ::2])
+
+
+def test_merged_detectors_reproduce_the_merged_atom_model():
+    """Without gaps the merge of the per-detector atoms is synth.make_atoms (the model the five
+    configs use), and the map of the merged set is the map of make_atoms within fp32 rounding."""
+    from oracle.binding import merge_detectors
+    from synth import make_atoms, make_detector_atoms
+
+    t = (np.arange(200) * TSFT).astype(np.int32)
+    per_det = make_detector_atoms(t, np.random.default_rng(7)).astype(np.float32)
+    merged = merge_detectors([per_det[0], per_det[1]], [t, t], t)
+    ref = make_atoms(t, np.random.default_rng(7)).astype(np.float32)
+    assert np.allclose(merged, ref, rtol=3e-7, atol=3e-7)
+    g = Grid(0, TSFT, 6, 4 * TSFT, 2 * TSFT, 7)
+    a = oracle.map2F(merged, t, EXP, g)["twoF"]
+    b = oracle.map2F(ref, t, EXP, g)["twoF"]
+    assert np.allclose(a, b, rtol=1e-4, atol=1e-4)
