@@ -288,6 +288,24 @@ def side_workloads(torch, pkg, peaks):
                         "x1000_templates_fused_ms": time_calls(torch, fnk, 10),
                         "note": "one launch (rect_small_kernel); single-call time is host-launch bound"}
     out["cfg1_rect"]["x1000_cells_per_s"] = 576e3 / (out["cfg1_rect"]["x1000_templates_fused_ms"] * 1e-3)
+    # per-detector merge at config-4 scale: 2 detectors x 1024 templates x 2880 atoms, each with
+    # ~20 % of its own slots missing, merged onto the union (HBM-bound: reads both sets once,
+    # writes the merged set once)
+    n_at, T_m = 2880, 1024
+    tt = torch.arange(n_at, device="cuda", dtype=torch.int32) * 1800
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    keep = [torch.rand(n_at, generator=gen, device="cuda") > 0.2 for _ in range(2)]
+    t_d = [tt[k].contiguous() for k in keep]
+    a_d = [torch.randn((T_m, 7, int(x.shape[0])), generator=gen, device="cuda") for x in t_d]
+    t_u = torch.unique(torch.cat(t_d)).to(torch.int32).contiguous()
+    fn_mg = lambda: pkg.tfstat_merge_detectors(a_d, t_d, t_u)
+    for _ in range(3):
+        fn_mg()
+    ms_mg = time_calls(torch, fn_mg, 10)
+    by_mg = 4 * (sum(a.numel() for a in a_d) + T_m * 7 * int(t_u.shape[0]))
+    out["merge_detectors_2x1024x2880"] = {"ms": ms_mg, "algorithmic_GBps": by_mg / (ms_mg * 1e-3) / 1e9,
+                                          "hbm_frac": by_mg / (ms_mg * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    del a_d
     # row a5 standalone at a size where the two-launch chain is amortised: the map of one year at
     # dt0 = dtau = T_SFT (17518 x 17519 cells, 1.23 GB), the largest of the paper's setups
     # (PAPER.md:106, 146-148); values are arbitrary positive floats, the kernel is data-independent

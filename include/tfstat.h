@@ -182,6 +182,28 @@ int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, i
                        uint8_t *out_flags, tfstat_result *out, void *workspace,
                        size_t workspace_bytes, void *stream, const tfstat_opts *opts_host);
 
+/* ---- per-detector input ----------------------------------------------------------------- */
+
+#define TFSTAT_MAX_DETECTORS 8
+
+/* Merge per-detector atoms onto one set of time stamps (atoms are indexed "over SFTs",
+ * PAPER.md:65; the map entry points above take them merged per time stamp):
+ *   out[k][ch][i] = sum over detectors X = 0..n_det-1, in this order, of atoms_X[k][ch][j]
+ *                   with t_X[j] == t_out[i]                (fp32; reproducible to the bit)
+ * Atoms of a detector whose time stamp is not in t_out are dropped; a t_out[i] that no detector
+ * has gives zeros.  The caller chooses t_out (normally the sorted union of the t_X).
+ *   atoms_dets, t_dets: HOST arrays of n_det DEVICE pointers; atoms_dets[X] is laid out like the
+ *   atoms of tfstat_search with template_strides[X], lds[X] (HOST arrays); t_dets[X] has
+ *   n_atoms_dets[X] strictly increasing int32 time stamps, shared by all templates.
+ *   t_out: DEVICE [n_out] strictly increasing; out_atoms: DEVICE [n_templates][7][ld_out].
+ * Errors: TFSTAT_EINVAL (null pointers, n_det outside 1..TFSTAT_MAX_DETECTORS, sizes < 1,
+ * ld < n).                                                                                  */
+int tfstat_merge_detectors(const float *const *atoms_dets, const int64_t *template_strides,
+                           const int64_t *lds, const int32_t *const *t_dets,
+                           const int32_t *n_atoms_dets, int32_t n_det, int32_t n_templates,
+                           const int32_t *t_out, int32_t n_out, float *out_atoms,
+                           int64_t template_stride_out, int64_t ld_out, void *stream);
+
 /* ---- end-to-end entry point with HOST buffers ----------------------------------------- */
 
 /* tfstat_search on host memory: copies atoms host->device in template chunks on internal

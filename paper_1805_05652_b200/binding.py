@@ -79,6 +79,7 @@ def load_library():
     lib.tfstat_general_workspace_bytes.argtypes = [i32, i32]
     lib.tfstat_map_general.argtypes = [vp, i64, vp, i32, C.POINTER(_Window), vp, i32, vp, i32,
                                        vp, vp, vp, vp, sz, vp, op]
+    lib.tfstat_merge_detectors.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, i32, vp, i64, i64, vp]
     lib.tfstat_probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
     _lib = lib
@@ -299,6 +300,38 @@ def tfstat_map_general(atoms: torch.Tensor, t_atoms: torch.Tensor, kind: int, su
                                 ws.numel(), _stream_ptr(stream), C.byref(o))
     _check(rc, "tfstat_map_general")
     return out_map, flags, (Results(out) if want_marginals else None)
+
+
+def tfstat_merge_detectors(atoms_dets, t_dets, t_out: torch.Tensor, *, stream=None) -> torch.Tensor:
+    """Per-detector atoms -> atoms merged per time stamp (include/tfstat.h).
+
+    atoms_dets: list of CUDA float32 tensors [T, 7, N_x] (or [7, N_x]); t_dets: list of CUDA int32
+    [N_x]; t_out: CUDA int32 [N] (normally the sorted union).  Returns [T, 7, N] (or [7, N])."""
+    lib = load_library()
+    n_det = len(atoms_dets)
+    if n_det != len(t_dets) or n_det < 1:
+        raise TfstatError("need one time-stamp tensor per detector")
+    squeeze = atoms_dets[0].dim() == 2
+    A = [a[None] if squeeze else a for a in atoms_dets]
+    T = int(A[0].shape[0])
+    for a, t in zip(A, t_dets):
+        _dev_f32(a, "atoms_dets[x]")
+        _dev_i32(t, "t_dets[x]")
+        if a.dim() != 3 or a.shape[0] != T or a.shape[1] != 7 or a.stride(2) != 1 \
+                or a.shape[2] != t.shape[0]:
+            raise TfstatError("atoms_dets[x] must be [T, 7, N_x] matching t_dets[x]")
+    _dev_i32(t_out, "t_out")
+    n_out = int(t_out.shape[0])
+    out = torch.empty((T, 7, n_out), dtype=torch.float32, device=t_out.device)
+    pa = (C.c_void_p * n_det)(*[a.data_ptr() for a in A])
+    pt = (C.c_void_p * n_det)(*[t.data_ptr() for t in t_dets])
+    ts = (C.c_int64 * n_det)(*[int(a.stride(0)) for a in A])
+    lds = (C.c_int64 * n_det)(*[int(a.stride(1)) for a in A])
+    ns = (C.c_int32 * n_det)(*[int(t.shape[0]) for t in t_dets])
+    rc = lib.tfstat_merge_detectors(pa, ts, lds, pt, ns, n_det, T, t_out.data_ptr(), n_out,
+                                    out.data_ptr(), 7 * n_out, n_out, _stream_ptr(stream))
+    _check(rc, "tfstat_merge_detectors")
+    return out[0] if squeeze else out
 
 
 def count_terms(t_atoms: torch.Tensor, window: int, grid, *, stream=None) -> int:

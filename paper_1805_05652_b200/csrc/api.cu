@@ -356,6 +356,29 @@ int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, i
     return TFSTAT_OK;
 }
 
+int tfstat_merge_detectors(const float *const *atoms_dets, const int64_t *template_strides,
+                           const int64_t *lds, const int32_t *const *t_dets,
+                           const int32_t *n_atoms_dets, int32_t n_det, int32_t n_templates,
+                           const int32_t *t_out, int32_t n_out, float *out_atoms,
+                           int64_t template_stride_out, int64_t ld_out, void *stream)
+{
+    if (!atoms_dets || !template_strides || !lds || !t_dets || !n_atoms_dets || !t_out ||
+        !out_atoms)
+        return TFSTAT_EINVAL;
+    if (n_det < 1 || n_det > TFSTAT_MAX_DETECTORS || n_templates < 1 || n_out < 1 ||
+        ld_out < n_out || (n_templates > 1 && template_stride_out < 7 * ld_out))
+        return TFSTAT_EINVAL;
+    for (int x = 0; x < n_det; ++x) {
+        if (!atoms_dets[x] || !t_dets[x] || n_atoms_dets[x] < 1 || lds[x] < n_atoms_dets[x] ||
+            (n_templates > 1 && template_strides[x] < 7 * lds[x]))
+            return TFSTAT_EINVAL;
+    }
+    TF_CUDA(launch_merge(atoms_dets, template_strides, lds, t_dets, n_atoms_dets, n_det,
+                         n_templates, t_out, n_out, out_atoms, template_stride_out, ld_out,
+                         static_cast<cudaStream_t>(stream)));
+    return TFSTAT_OK;
+}
+
 int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t ld,
                        const int32_t *t_atoms_host, int32_t n_atoms, int32_t n_templates,
                        int window, int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,

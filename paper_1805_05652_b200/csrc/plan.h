@@ -90,6 +90,10 @@ cudaError_t launch_marginalise(const float *map, const uint8_t *flags, int64_t n
                                int32_t N_tau, Partial *partials, int32_t n_blocks,
                                tfstat_result *out, cudaStream_t st);
 int32_t marginalise_blocks(int64_t n_cells);
+cudaError_t launch_merge(const float *const *atoms, const int64_t *tstrides, const int64_t *lds,
+                         const int32_t *const *ts, const int32_t *ns, int32_t n_det,
+                         int32_t n_templates, const int32_t *t_out, int32_t n_out, float *out,
+                         int64_t tstride_out, int64_t ld_out, cudaStream_t st);
 int32_t general_partials(int32_t N_t0, int32_t N_tau);
 cudaError_t launch_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
                            const tfstat_window &w, const int32_t *t0_grid, int32_t N_t0,

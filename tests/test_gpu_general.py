@@ -138,3 +138,43 @@ def test_general_degenerate_and_errors(pkg):
         pkg.tfstat_map_general(dev(atoms), dev(t), EXP, (0, 1), dev(t0g), dev(taug))
     with pytest.raises(pkg.TfstatError):
         pkg.tfstat_map_general(dev(atoms), dev(t), 7, (1, 1), dev(t0g), dev(taug))
+
+
+def test_merge_detectors_bit_exact_and_end_to_end(pkg):
+    """tfstat_merge_detectors against oracle_merge_detectors, bit for bit (fp32 adds in a fixed
+    order), batched over templates with detectors that have their own gaps; then the merged atoms
+    through tfstat_search against the oracle's map of the oracle's merge."""
+    from oracle.binding import merge_detectors
+    from synth import make_detector_atoms
+
+    n_slots, T = 700, 3
+    t = (np.arange(n_slots) * TSFT).astype(np.int32)
+    rng = np.random.default_rng(11)
+    keep = [rng.random(n_slots) > 0.2, rng.random(n_slots) > 0.35, rng.random(n_slots) > 0.5]
+    for k in keep:
+        k[100:130] = False  # a common gap: time stamps nobody has do not appear in the union
+    per = [np.stack([make_detector_atoms(t, np.random.default_rng(100 + 10 * tpl), phi=0.3 * tpl)
+                     .astype(np.float32) for tpl in range(T)]) for _ in range(1)][0]  # [T, 2, 7, N]
+    # three "detectors": the model's two, and a second copy of detector 0 scaled (a third site)
+    dets = [per[:, 0][:, :, keep[0]], per[:, 1][:, :, keep[1]], 0.5 * per[:, 0][:, :, keep[2]]]
+    ts = [t[k] for k in keep]
+    t_out = np.union1d(np.union1d(ts[0], ts[1]), ts[2]).astype(np.int32)
+    assert len(t_out) < n_slots
+    got = pkg.tfstat_merge_detectors([dev(d) for d in dets], [dev(x) for x in ts], dev(t_out))
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    for tpl in range(T):
+        ref = merge_detectors([d[tpl] for d in dets], ts, t_out)
+        assert np.array_equal(got[tpl], ref), f"template {tpl}: merge differs from the oracle"
+    # single-template form, and a t_out with a stamp nobody has / without some stamps
+    t_odd = np.concatenate([[-TSFT], t_out[::3]]).astype(np.int32)
+    g1 = pkg.tfstat_merge_detectors([dev(d[0]) for d in dets], [dev(x) for x in ts], dev(t_odd))
+    assert np.array_equal(g1.cpu().numpy(), merge_detectors([d[0] for d in dets], ts, t_odd))
+    # end to end: merged atoms -> search
+    grid = Grid(0, TSFT, 30, 4 * TSFT, 2 * TSFT, 150)
+    res = pkg.tfstat_search(dev(got), dev(t_out), EXP, grid, want_maps=True, want_flags=True)
+    for tpl in range(T):
+        ref = oracle.map2F(got[tpl], t_out, EXP, grid)
+        check_cells(res.maps[tpl].cpu().numpy(), res.flags[tpl].cpu().numpy(), ref, f"merged {tpl}")
+    with pytest.raises(pkg.TfstatError):
+        pkg.tfstat_merge_detectors([dev(dets[0])] * 9, [dev(ts[0])] * 9, dev(t_out))  # > 8 detectors
