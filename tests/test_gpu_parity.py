@@ -82,6 +82,7 @@ TINY = [
     (106, 200, 0.1, Grid(0, 1801, 40, 3600, 1800, 1000)),       # gcd 1: per-cell binary search
     (107, 120, 0.0, Grid(0, 1800, 1, 3600, 1800, 90)),          # N_t0 = 1
     (108, 120, 0.0, Grid(0, 1800, 75, 7200, 1800, 1)),          # N_tau = 1
+    (109, 1200, 0.1, Grid(0, 1801, 40, 3600, 4801, 900)),       # lattice > 2^22 points for rect too
 ]
 
 
