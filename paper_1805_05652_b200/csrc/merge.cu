@@ -14,6 +14,7 @@ namespace tfstat {
 namespace {
 
 constexpr int kMergeNT = 128;
+constexpr int kMergeRows = 48;  // grid.y: a thread amortises its binary searches over T / 48 templates
 
 struct MergeArgs {
     const float *atoms[TFSTAT_MAX_DETECTORS];
@@ -81,7 +82,7 @@ cudaError_t launch_merge(const float *const *atoms, const int64_t *tstrides, con
     a.tstride_out = tstride_out;
     a.ld_out = ld_out;
     const dim3 grid((unsigned)((n_out + kMergeNT - 1) / kMergeNT),
-                    (unsigned)std::min<int32_t>(n_templates, 4096), 1);
+                    (unsigned)std::min<int32_t>(n_templates, kMergeRows), 1);
     merge_kernel<<<grid, kMergeNT, 0, st>>>(a);
     return cudaGetLastError();
 }
