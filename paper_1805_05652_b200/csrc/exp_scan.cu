@@ -61,8 +61,11 @@ __device__ __forceinline__ void acc_add(SlideAcc &a, const float w, const float 
     a.c = fmaf(w2, ab, a.c);
 }
 
-// atom `al` straight from global memory (entering / leaving / re-summed atoms)
-__device__ __forceinline__ void acc_add_global(SlideAcc &a, const float *__restrict__ base,
+// atom `al` straight from global memory (entering / leaving / re-summed atoms), one weight for
+// the TPC templates of the CTA
+template <int TPC>
+__device__ __forceinline__ void acc_add_global(SlideAcc (&a)[TPC],
+                                               const float *__restrict__ const (&base)[TPC],
                                                const int64_t ld, const int32_t *__restrict__ t,
                                                const int al, const long long t_ref,
                                                const float kexp, const float sign)
@@ -70,9 +73,14 @@ __device__ __forceinline__ void acc_add_global(SlideAcc &a, const float *__restr
     const float dt = (float)((long long)__ldg(t + al) - t_ref);
     const float e = ex2_approx(dt * kexp);
     const float w = sign * e;
-    acc_add(a, w, w * e, pack2(__ldg(base + al), __ldg(base + ld + al)), __ldg(base + 2 * ld + al),
-            pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al)),
-            pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al)));
+    const float w2 = w * e;
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
+        const float *__restrict__ bq = base[q];
+        acc_add(a[q], w, w2, pack2(__ldg(bq + al), __ldg(bq + ld + al)), __ldg(bq + 2 * ld + al),
+                pack2(__ldg(bq + 3 * ld + al), __ldg(bq + 4 * ld + al)),
+                pack2(__ldg(bq + 5 * ld + al), __ldg(bq + 6 * ld + al)));
+    }
 }
 
 __device__ __forceinline__ void acc_scale(SlideAcc &a, const float c)
@@ -84,23 +92,26 @@ __device__ __forceinline__ void acc_scale(SlideAcc &a, const float c)
     a.c *= c2;
 }
 
-template <int NT, int KC>
+// TPC templates per CTA: the weights E_a depend on (atom, tau) only, not on the template, so one
+// MUFU.EX2 (+ the argument and E^2 multiplies) serves TPC templates; per (atom, template) the
+// initial window sum costs 2 LDS.128 + 4 multiply-adds + 3 / TPC instead of + 3.
+template <int NT, int KC, int TPC>
 __global__ void __launch_bounds__(NT)
     exp_slide_kernel(const Problem pr, Partial *__restrict__ partials, const int n_nblocks,
                      const int n_segs, const int seg_len)
 {
-    __shared__ ulonglong2 s_a[KC];  // {(dt, ab), (a2, b2)}
-    __shared__ ulonglong2 s_b[KC];  // {(Re Fa, Im Fa), (Re Fb, Im Fb)}
+    __shared__ ulonglong2 s_a[TPC][KC];  // {(dt, ab), (a2, b2)}
+    __shared__ ulonglong2 s_b[TPC][KC];  // {(Re Fa, Im Fa), (Re Fb, Im Fb)}
     __shared__ Marg s_red[32];
     pdl_trigger();
     pdl_wait();  // bounds_kernel's lo / edge tables
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
-    // blockIdx.x = (tpl * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
+    // blockIdx.x = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
     const int j = (int)(blockIdx.x % n_nblocks);
     const int seg = (int)((blockIdx.x / n_nblocks) % n_segs);
-    const int tpl = (int)(blockIdx.x / ((int64_t)n_nblocks * n_segs));
+    const int tpl0 = (int)(blockIdx.x / ((int64_t)n_nblocks * n_segs)) * TPC;
     const int nb = n_nblocks - 1 - j;
     const int n_first = nb * NT;
     const int n_count = min(NT, g.N_tau - n_first);
@@ -109,7 +120,12 @@ __global__ void __launch_bounds__(NT)
     const int m_beg = seg * seg_len;
     const int m_end = min(m_beg + seg_len, g.N_t0);
 
-    const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
+    // templates beyond the batch (ragged last group) alias the last real one; nothing of theirs
+    // is stored
+    const float *__restrict__ base[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q)
+        base[q] = pr.atoms + (int64_t)min(tpl0 + q, pr.n_templates - 1) * pr.template_stride;
     const int64_t ld = pr.ld;
     const double tau = (double)tau_of(g, n);
     const float kexp = (float)(-1.4426950408889634 / tau);
@@ -122,60 +138,79 @@ __global__ void __launch_bounds__(NT)
     long long t_ref = t0_of(g, m);
     const int cta_e = max(hi_index(bd, g, m, n_first + n_count - 1), lo_m);  // hi is monotone in n
 
-    SlideAcc acc;
-    acc_zero(acc);
+    SlideAcc acc[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) acc_zero(acc[q]);
 #pragma unroll 1
     for (int cs = lo_m; cs < cta_e; cs += KC) {
         const int n_stage = min(KC, cta_e - cs);
         for (int i = threadIdx.x; i < n_stage; i += NT) {
             const int al = cs + i;
             const float dt = (float)((long long)__ldg(bd.t + al) - t_ref);
-            ulonglong2 ra, rb;
-            ra.x = pack2(dt, __ldg(base + 2 * ld + al));
-            ra.y = pack2(__ldg(base + al), __ldg(base + ld + al));
-            rb.x = pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al));
-            rb.y = pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al));
-            s_a[i] = ra;
-            s_b[i] = rb;
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                const float *__restrict__ bq = base[q];
+                ulonglong2 ra, rb;
+                ra.x = pack2(dt, __ldg(bq + 2 * ld + al));
+                ra.y = pack2(__ldg(bq + al), __ldg(bq + ld + al));
+                rb.x = pack2(__ldg(bq + 3 * ld + al), __ldg(bq + 4 * ld + al));
+                rb.y = pack2(__ldg(bq + 5 * ld + al), __ldg(bq + 6 * ld + al));
+                s_a[q][i] = ra;
+                s_b[q][i] = rb;
+            }
         }
         __syncthreads();
         const int x1 = min(cs + n_stage, hi) - cs;
 #pragma unroll 4
         for (int i = 0; i < x1; ++i) {
-            const ulonglong2 ra = s_a[i], rb = s_b[i];
-            float dt, ab;
-            unpack2(ra.x, dt, ab);
-            const float e = ex2_approx(dt * kexp);
-            acc_add(acc, e, e * e, ra.y, ab, rb.x, rb.y);
+            float e = 0.0f, e2 = 0.0f;
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                const ulonglong2 ra = s_a[q][i], rb = s_b[q][i];
+                float dt, ab;
+                unpack2(ra.x, dt, ab);
+                if (q == 0) {
+                    e = ex2_approx(dt * kexp);
+                    e2 = e * e;
+                }
+                acc_add(acc[q], e, e2, ra.y, ab, rb.x, rb.y);
+            }
         }
         __syncthreads();
     }
-    float A_max;
-    {
+    float A_max[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
         float A, B;
-        unpack2(acc.ab, A, B);
-        A_max = A;
+        unpack2(acc[q].ab, A, B);
+        A_max[q] = A;
     }
 
     // ---- slide backwards in t0: closure of cell m, then step to m - 1 ------------------------
-    Marg mg;
-    marg_init(mg);
-    const int64_t map_base = (int64_t)tpl * g.N_t0 * g.N_tau;
+    Marg mg[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) marg_init(mg[q]);
+    const int64_t cells = (int64_t)g.N_t0 * g.N_tau;
 #pragma unroll 1
     for (;;) {
         if (n_ok) {
-            float A, B, far, fai, fbr, fbi;
-            unpack2(acc.ab, A, B);
-            unpack2(acc.fa, far, fai);
-            unpack2(acc.fb, fbr, fbi);
-            uint32_t fl;
-            // one closure per t0 step is a quarter of this kernel's instructions in fp64
-            const float twoF =
-                closure_2F_mixed(A, B, acc.c, far, fai, fbr, fbi, hi - lo_m, pr.min_atoms, fl);
             const int32_t flat = m * g.N_tau + n;
-            if (pr.out_maps) pr.out_maps[map_base + flat] = twoF;
-            if (pr.out_flags) pr.out_flags[map_base + flat] = (uint8_t)fl;
-            if (!fl) marg_add(mg, twoF, flat);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                if (tpl0 + q >= pr.n_templates) continue;
+                float A, B, far, fai, fbr, fbi;
+                unpack2(acc[q].ab, A, B);
+                unpack2(acc[q].fa, far, fai);
+                unpack2(acc[q].fb, fbr, fbi);
+                uint32_t fl;
+                // one closure per t0 step is a quarter of this kernel's instructions in fp64
+                const float twoF = closure_2F_mixed(A, B, acc[q].c, far, fai, fbr, fbi, hi - lo_m,
+                                                    pr.min_atoms, fl);
+                const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
+                if (pr.out_maps) pr.out_maps[o] = twoF;
+                if (pr.out_flags) pr.out_flags[o] = (uint8_t)fl;
+                if (!fl) marg_add(mg[q], twoF, flat);
+            }
         }
         if (m == m_beg) break;
         const int m2 = m - 1;
@@ -187,44 +222,73 @@ __global__ void __launch_bounds__(NT)
             const float sh = (float)(t_ref - t0_2);
             if (sh * inv_tau > kReanchor) {  // keep the weights of entering atoms <= e^kReanchor
                 const float c = ex2_approx(sh * kexp);
-                acc_scale(acc, c);
-                A_max *= c * c;
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    acc_scale(acc[q], c);
+                    A_max[q] *= c * c;
+                }
                 t_ref = t0_2;
             }
             for (int al = lo2; al < lo_m; ++al)  // entering at the low end
-                acc_add_global(acc, base, ld, bd.t, al, t_ref, kexp, 1.0f);
+                acc_add_global<TPC>(acc, base, ld, bd.t, al, t_ref, kexp, 1.0f);
             for (int al = max(hi2, lo_m); al < hi; ++al)  // leaving at the high end
-                acc_add_global(acc, base, ld, bd.t, al, t_ref, kexp, -1.0f);
-            float A, B;
-            unpack2(acc.ab, A, B);
-            A_max = fmaxf(A_max, A);
-            fresh = A * kGuard < A_max;  // the window lost most of its weight: re-sum it
+                acc_add_global<TPC>(acc, base, ld, bd.t, al, t_ref, kexp, -1.0f);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                float A, B;
+                unpack2(acc[q].ab, A, B);
+                A_max[q] = fmaxf(A_max[q], A);
+                // a window that lost most of its weight is re-summed (for all TPC templates:
+                // a fresh sum is always right)
+                fresh = fresh || (A * kGuard < A_max[q]);
+            }
         }
         if (fresh) {
-            acc_zero(acc);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) acc_zero(acc[q]);
             t_ref = t0_2;
             for (int al = lo2; al < hi2; ++al)
-                acc_add_global(acc, base, ld, bd.t, al, t_ref, kexp, 1.0f);
-            float A, B;
-            unpack2(acc.ab, A, B);
-            A_max = A;
+                acc_add_global<TPC>(acc, base, ld, bd.t, al, t_ref, kexp, 1.0f);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                float A, B;
+                unpack2(acc[q].ab, A, B);
+                A_max[q] = A;
+            }
         }
         m = m2;
         lo_m = lo2;
         hi = hi2;
     }
     if (partials) {
-        marg_block_reduce<NT>(mg, s_red);
-        if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            if (q > 0) __syncthreads();  // s_red is reused
+            marg_block_reduce<NT>(mg[q], s_red);
+            if (threadIdx.x == 0 && tpl0 + q < pr.n_templates)
+                partial_store(partials + ((int64_t)(tpl0 + q) * n_segs + seg) * n_nblocks + j,
+                              mg[q]);
+        }
     }
+}
+
+template <int NT, int TPC>
+cudaError_t launch_tpc(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
+{
+    const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
+    const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * groups;
+    return launch_pdl(exp_slide_kernel<NT, (TPC == 4 ? 256 : 512), TPC>, (unsigned)n_ctas, NT, 0,
+                      st, pr, partials, pl.n_nblocks, pl.n_segs, pl.seg_len);
 }
 
 template <int NT>
 cudaError_t launch_nt(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
 {
-    const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * pl.n_templates;
-    return launch_pdl(exp_slide_kernel<NT, 512>, (unsigned)n_ctas, NT, 0, st, pr, partials,
-                      pl.n_nblocks, pl.n_segs, pl.seg_len);
+    switch (pl.slide_tpc) {
+    case 4: return launch_tpc<NT, 4>(pl, pr, partials, st);
+    case 2: return launch_tpc<NT, 2>(pl, pr, partials, st);
+    default: return launch_tpc<NT, 1>(pl, pr, partials, st);
+    }
 }
 
 }  // namespace

@@ -54,6 +54,7 @@ struct Plan {
     int64_t tiles_per_template;
     // exp sliding form (exp_scan.cu): t0 segments per (template, tau block)
     int32_t n_segs, seg_len;
+    int32_t slide_tpc;  // templates per CTA (1, 2, 4): they share the weights
     // rect / marginalise tiling
     int32_t cell_blocks_per_template;
     RectRun rect;

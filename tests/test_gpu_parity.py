@@ -473,11 +473,14 @@ def test_exp_scan_long_gaps_and_disjoint_windows(pkg):
         check_cells(m, f, ref, f"scan min_atoms={min_atoms}")
 
 
-def test_exp_scan_batched_equals_oracle_and_direct(pkg):
+@pytest.mark.parametrize("tpc,seg_len", [(0, 0), (1, 0), (2, 5), (4, 0), (4, 7)])
+def test_exp_scan_batched_equals_oracle_and_direct(pkg, tpc, seg_len):
+    """7 templates: with 2 or 4 templates per CTA (shared weights) the last group is ragged."""
     grid = Grid(0, 1800, 23, 3600, 3600, 140)
     wl = tiny_workload(201, 350, 0.1, grid, n_templates=7, phi_random=True)
     a, t = dev(wl.data.atoms), dev(wl.data.t)
-    res = pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, want_maps=True, want_flags=True)
+    res = pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, want_maps=True, want_flags=True,
+                            tile=(tpc, 0, seg_len))
     direct = pkg.tfstat_search(a, t, EXP, grid, exp_method=1, want_flags=True)
     torch.cuda.synchronize()
     assert torch.equal(res.flags, direct.flags)
