@@ -216,7 +216,7 @@ int tfstat_merge_detectors(const float *const *atoms_dets, const int64_t *templa
  *   device_scratch: DEVICE buffer of device_scratch_bytes bytes (256-B aligned) that holds the
  *   double-buffered chunks, the workspace and the results.  Any size from one template's worth
  *   up works (smaller => more, smaller chunks); tfstat_search_host_scratch_bytes() gives the
- *   size at which chunks are the preferred 256 templates.  NULL: the library cudaMallocs up to
+ *   size for the preferred chunks.  NULL: the library cudaMallocs up to
  *   device_scratch_bytes (0 = 2 GiB) itself and frees it before returning -- convenient, but
  *   cudaFree can stall for ~100 ms, so callers in a loop should pass their own buffer.
  *   Errors: TFSTAT_EWORKSPACE if a given scratch is misaligned or too small for one template. */
@@ -226,7 +226,8 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
                        int32_t dtau, int32_t N_tau, tfstat_result *out_host,
                        float *out_maps_host, void *device_scratch, size_t device_scratch_bytes,
                        const tfstat_opts *opts_host);
-/* Host-only: scratch size for chunks of min(n_templates, 256) templates; 0 on invalid input. */
+/* Host-only: scratch size for the preferred chunks (n_templates / 4, clamped to 256..1024
+ * templates); 0 on invalid input. */
 size_t tfstat_search_host_scratch_bytes(int64_t template_stride, int32_t n_atoms,
                                         int32_t n_templates, int window, int32_t t0_min,
                                         int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,

@@ -231,6 +231,14 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     return TFSTAT_OK;
 }
 
+// Templates per chunk of tfstat_search_host: about four chunks per call (so that the copies
+// overlap the compute), at least 256 and at most 1024 templates (a chunk must still fill the GPU
+// with the sliding form, which runs up to 4 templates per CTA).
+static int32_t host_chunk_templates(int32_t n_templates)
+{
+    return std::min<int32_t>(n_templates, std::max<int32_t>(256, std::min<int32_t>(1024, n_templates / 4)));
+}
+
 }  // namespace tfstat
 
 using namespace tfstat;
@@ -408,7 +416,7 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
     const size_t map_bytes = out_maps_host ? sizeof(float) * (size_t)cells : 0;
     const size_t t_bytes = align_up(sizeof(int32_t) * (size_t)n_atoms);
     const size_t out_bytes = align_up(sizeof(tfstat_result) * (size_t)n_templates);
-    int32_t Tc = std::min<int32_t>(n_templates, 256);
+    int32_t Tc = host_chunk_templates(n_templates);
     Plan pl;
     size_t need = 0;
     for (;; Tc = (Tc + 1) / 2) {
@@ -521,7 +529,7 @@ size_t tfstat_search_host_scratch_bytes(int64_t template_stride, int32_t n_atoms
                                         const tfstat_opts *opts_host)
 {
     if (n_templates < 1 || template_stride < 1) return 0;
-    const int32_t Tc = std::min<int32_t>(n_templates, 256);
+    const int32_t Tc = host_chunk_templates(n_templates);
     const Plan pl =
         make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts_host);
     if (pl.status != TFSTAT_OK) return 0;
