@@ -76,7 +76,6 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
 
     // exp direct tile shape: largest tile that still yields a few waves of CTAs on 148 SMs
     const int64_t cells = (int64_t)N_t0 * N_tau;
-    const int64_t total = cells * n_templates;
     // C = 8 executes 7.25 FP32 ops per term, C = 4 7.5 (3 % more) but gives twice the CTAs: take
     // C = 8 only when it still fills 148 SMs x 4 resident CTAs about 8 times over (measured on
     // B200: configs 2 and 3, under one wave at C = 8, are 25-30 % faster at C = 4)

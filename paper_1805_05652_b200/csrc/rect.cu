@@ -54,19 +54,8 @@ __device__ __forceinline__ void st_release(int32_t *p, const int32_t v)
 {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-// Poll with relaxed loads and a back-off (an acquire load per poll invalidates the whole L1 and
-// starves the producers of issue slots), then one acquire fence.
-__device__ __forceinline__ void wait_flag(const int32_t *p)
-{
-    int32_t v;
-    for (;;) {
-        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-        if (v != 0) break;
-        __nanosleep(64);
-    }
-    asm volatile("fence.acq_rel.gpu;" ::: "memory");
-}
-
+// Wait for two flags: poll with relaxed loads and a back-off (an acquire load per poll
+// invalidates the whole L1 and starves the producers of issue slots), then ONE acquire fence.
 __device__ __forceinline__ void wait_flags2(const int32_t *p, const int32_t *q)
 {
     int32_t v, w;
