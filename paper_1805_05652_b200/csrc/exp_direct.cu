@@ -201,18 +201,14 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
             unpack2(acc.fb[c], fbr, fbi);
             unpack2(acc.cc[c / 2], cc0, cc1);
             Cc = (c & 1) ? cc1 : cc0;
-            Sums64 s;
-            s.A = A;
-            s.B = B;
-            s.C = Cc;
-            s.far = far;
-            s.fai = fai;
-            s.fbr = fbr;
-            s.fbi = fbi;
             const int lo_c = __ldg(bd.lo + m);
             const int cnt = max(hi_index(bd, g, m, n) - lo_c, 0);
             uint32_t fl;
-            const float twoF = closure_2F(s, cnt, pr.min_atoms, fl);
+            // the sums carry the weight of the tile's first cell; eq. (7) does not care, and the
+            // fp64 redo of short ill-conditioned windows uses the cell's own t0
+            const float twoF = closure_2F_exp(A, B, Cc, far, fai, fbr, fbi, lo_c, cnt,
+                                              pr.min_atoms, fl, base, ld, bd.t, t0_of(g, m),
+                                              (double)tau_of(g, n));
             const int32_t flat = m * g.N_tau + n;
             if (pr.out_maps) pr.out_maps[map_base + flat] = twoF;
             if (pr.out_flags) pr.out_flags[map_base + flat] = (uint8_t)fl;

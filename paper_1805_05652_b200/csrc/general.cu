@@ -44,6 +44,39 @@ struct GeneralArgs {
     uint8_t *out_flags;
 };
 
+// fp64 redo of a short, ill-conditioned window (tfstat_dev.cuh, closure_2F_exp): the window's
+// sums straight from the atoms with the weight of the kind evaluated in fp64
+template <int KIND>
+__device__ __noinline__ Sums64 general_resum64(const GeneralArgs &a, const int lo, const int hi,
+                                               const long long t0, const double tau)
+{
+    Sums64 s;
+    s.A = s.B = s.C = s.far = s.fai = s.fbr = s.fbi = 0.0;
+    const double support = (double)a.sup_num / (double)a.sup_den;
+    for (int al = lo; al < hi; ++al) {
+        const double u = (double)((long long)__ldg(a.t + al) - t0) / tau;
+        double w = 1.0;
+        if (KIND == TFSTAT_WINDOW_EXP) {
+            w = exp(-u);
+        } else if (KIND == TFSTAT_WINDOW_TABLE) {
+            const double x = u / support * (double)(a.n_table - 1);
+            int k = (int)floor(x);
+            k = max(0, min(k, a.n_table - 2));
+            const double t0v = (double)__ldg(a.table + k), t1v = (double)__ldg(a.table + k + 1);
+            w = t0v + (x - (double)k) * (t1v - t0v);
+        }
+        const double w2 = w * w;
+        s.A += w2 * (double)__ldg(a.atoms + al);
+        s.B += w2 * (double)__ldg(a.atoms + a.ld + al);
+        s.C += w2 * (double)__ldg(a.atoms + 2 * a.ld + al);
+        s.far += w * (double)__ldg(a.atoms + 3 * a.ld + al);
+        s.fai += w * (double)__ldg(a.atoms + 4 * a.ld + al);
+        s.fbr += w * (double)__ldg(a.atoms + 5 * a.ld + al);
+        s.fbi += w * (double)__ldg(a.atoms + 6 * a.ld + al);
+    }
+    return s;
+}
+
 template <int KIND>
 __global__ void __launch_bounds__(kGenNT)
     general_kernel(const GeneralArgs a, Partial *__restrict__ partials, const int n_nblocks)
@@ -148,8 +181,12 @@ __global__ void __launch_bounds__(kGenNT)
         s.fai = fai;
         s.fbr = fbr;
         s.fbi = fbi;
+        const int cnt = hi - lo;
+        if (cnt >= a.min_atoms && cnt >= 1 && cnt <= kRedoMaxAtoms &&
+            !(s.A * s.B - s.C * s.C > 0.015625 * s.A * s.B))
+            s = general_resum64<KIND>(a, lo, hi, t0, (double)tau);
         uint32_t fl;
-        const float twoF = closure_2F(s, hi - lo, a.min_atoms, fl);
+        const float twoF = closure_2F(s, cnt, a.min_atoms, fl);
         const int32_t flat = m * a.N_tau + n;
         if (a.out_map) a.out_map[flat] = twoF;
         if (a.out_flags) a.out_flags[flat] = (uint8_t)fl;

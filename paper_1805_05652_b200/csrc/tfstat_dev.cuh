@@ -84,14 +84,46 @@ __device__ __forceinline__ float closure_2F(const Sums64 &s, int cnt, int min_at
     return (float)(2.0 * num / D);
 }
 
-// fp32 closure for well-conditioned cells, fp64 for the rest.  With D > AB/64 the cancellation
-// in D = AB - C^2 and in the numerator amplifies the fp32 rounding of the inputs by at most ~64,
-// i.e. <= ~1e-5 relative on 2F, two orders below the 1e-3 contract; everything else (small D,
-// count-degenerate cells, NaN) takes the fp64 path, which also decides the flags.
-__device__ __forceinline__ float closure_2F_mixed(const float A, const float B, const float C,
-                                                  const float far, const float fai,
-                                                  const float fbr, const float fbi, const int cnt,
-                                                  const int min_atoms, uint32_t &flags)
+// Exponential-window cell from fp32 sums: fp32 closure where the cell is well conditioned
+// (D > AB/64: the cancellation in D = AB - C^2 and in the numerator amplifies the fp32 rounding of
+// the sums by at most ~64, i.e. <= ~1e-5 relative on 2F), fp64 closure otherwise, with a safety
+// net for ill-conditioned SHORT windows.
+// fp32 sums carry ~6e-8 relative rounding per channel, which D = AB - C^2 amplifies by AB/D: a
+// window of one or two atoms can have AB/D ~ 1e4..1e6 (a single two-detector atom reaches 3e6),
+// and then no fp32 accumulation meets the 1e-3 contract.  Such cells are cheap to do properly:
+// if D <= AB/64 and the window holds at most kRedoMaxAtoms atoms, its sums are recomputed in
+// fp64 straight from the atoms (libm-grade exp), exactly as the oracle defines them.  Long
+// windows (more atoms than that) mix many antenna phases and are well conditioned in practice;
+// they keep the fp32 sums and the fp64 closure.
+constexpr int kRedoMaxAtoms = 64;
+
+static __device__ __noinline__ Sums64 exp_resum64(const float *__restrict__ base, const int64_t ld,
+                                           const int32_t *__restrict__ t, const int lo,
+                                           const int hi, const long long t0, const double tau)
+{
+    Sums64 s;
+    s.A = s.B = s.C = s.far = s.fai = s.fbr = s.fbi = 0.0;
+    for (int al = lo; al < hi; ++al) {
+        const double w = exp(-(double)((long long)__ldg(t + al) - t0) / tau);
+        const double w2 = w * w;
+        s.A += w2 * (double)__ldg(base + al);
+        s.B += w2 * (double)__ldg(base + ld + al);
+        s.C += w2 * (double)__ldg(base + 2 * ld + al);
+        s.far += w * (double)__ldg(base + 3 * ld + al);
+        s.fai += w * (double)__ldg(base + 4 * ld + al);
+        s.fbr += w * (double)__ldg(base + 5 * ld + al);
+        s.fbi += w * (double)__ldg(base + 6 * ld + al);
+    }
+    return s;
+}
+
+__device__ __forceinline__ float closure_2F_exp(const float A, const float B, const float C,
+                                                const float far, const float fai,
+                                                const float fbr, const float fbi, const int lo,
+                                                const int cnt, const int min_atoms,
+                                                uint32_t &flags, const float *__restrict__ base,
+                                                const int64_t ld, const int32_t *__restrict__ t,
+                                                const long long t0, const double tau)
 {
     const float p = A * B;
     const float D = fmaf(-C, C, p);
@@ -106,13 +138,17 @@ __device__ __forceinline__ float closure_2F_mixed(const float A, const float B, 
         return 2.0f * __fdividef(num, D);
     }
     Sums64 s;
-    s.A = A;
-    s.B = B;
-    s.C = C;
-    s.far = far;
-    s.fai = fai;
-    s.fbr = fbr;
-    s.fbi = fbi;
+    if (cnt >= min_atoms && cnt >= 1 && cnt <= kRedoMaxAtoms) {
+        s = exp_resum64(base, ld, t, lo, lo + cnt, t0, tau);
+    } else {
+        s.A = A;
+        s.B = B;
+        s.C = C;
+        s.far = far;
+        s.fai = fai;
+        s.fbr = fbr;
+        s.fbi = fbi;
+    }
     return closure_2F(s, cnt, min_atoms, flags);
 }
 

@@ -197,6 +197,64 @@ def test_calls_are_capturable_in_a_cuda_graph(pkg, window, method):
     assert np.array_equal(out.cpu().numpy().view(pkg.RESULT_DTYPE).reshape(-1), eager)
 
 
+@pytest.mark.parametrize("case", range(16))
+def test_random_grids_all_kernel_families(pkg, case):
+    """Seeded random data sets and grids (odd steps, negative and late t0, tau from one second to
+    longer than the data, heavy gaps, min_atoms 1..4) through every kernel family."""
+    rng = np.random.default_rng(5000 + case)
+    slots = int(rng.integers(20, 900))
+    gaps = float(rng.choice([0.0, 0.1, 0.4, 0.7]))
+    dt0 = int(rng.choice([1800, 900, 2700, 1801, 3600, 7200, 777]))
+    dtau = int(rng.choice([1800, 900, 3600, 5400, 1799, 43200, 1234]))
+    N_t0, N_tau = int(rng.integers(1, 60)), int(rng.integers(1, 200))
+    t0_min = int(rng.integers(-5, slots)) * 1800 + int(rng.choice([0, 0, 17]))
+    tau_min = int(rng.choice([1, 1800, 3600, 1800 * 7 + 3]))
+    grid = Grid(t0_min, dt0, N_t0, tau_min, dtau, N_tau)
+    min_atoms = int(rng.integers(1, 5))
+    wl = tiny_workload(6000 + case, slots, gaps, grid)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN},
+                                 {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 3)}]),
+                        (RECT, [{"rect_method": 1}, {"rect_method": 2}])):
+        ref = oracle.map2F(atoms, t, window, grid, min_atoms=min_atoms)
+        for kw in kws:
+            what = f"case {case} window {window} {kw}"
+            m, f = run_map(pkg, atoms, t, window, grid, min_atoms=min_atoms, **kw)
+            check_cells(m, f, ref, what)
+            res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, grid, min_atoms=min_atoms,
+                                    **kw)
+            check_result(res.numpy()[0], ref["twoF"], ref["flags"], grid.N_tau, what)
+        # the same window through the general entry point on arrays spelling out the grid
+        mg, fg, rg = pkg.tfstat_map_general(dev(atoms), dev(t), window, (3, 1) if window == EXP else (1, 1),
+                                            dev(grid.t0().astype(np.int32)),
+                                            dev(grid.tau().astype(np.int32)), want_flags=True,
+                                            min_atoms=min_atoms)
+        check_cells(mg.cpu().numpy(), fg.cpu().numpy(), ref, f"case {case} window {window} general")
+        check_result(rg.numpy()[0], ref["twoF"], ref["flags"], grid.N_tau,
+                     f"case {case} window {window} general")
+
+
+def test_concurrent_streams_do_not_interfere(pkg):
+    """The library keeps no state between calls: searches enqueued on two streams at once, each
+    with its own workspace, give the bits of the same searches run one after the other."""
+    grid = Grid(0, 1800, 40, 3600, 1800, 260)
+    wls = [tiny_workload(210 + i, 500, 0.1, grid, n_templates=5, phi_random=True) for i in (0, 1)]
+    dat = [(dev(w.data.atoms), dev(w.data.t)) for w in wls]
+    for window, kw in ((EXP, {}), (EXP, {"exp_method": pkg.EXP_SCAN}), (RECT, {"rect_method": 1})):
+        ref = [pkg.tfstat_search(a, t, window, grid, **kw).numpy() for a, t in dat]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        torch.cuda.synchronize()
+        out = [None, None]
+        for rep in range(4):  # interleave the enqueues
+            for i in (0, 1):
+                with torch.cuda.stream(streams[i]):
+                    out[i] = pkg.tfstat_search(dat[i][0], dat[i][1], window, grid,
+                                               stream=streams[i], **kw)
+        torch.cuda.synchronize()
+        for i in (0, 1):
+            assert np.array_equal(out[i].numpy(), ref[i]), f"window {window} {kw}: stream {i}"
+
+
 def test_search_host_equals_device(pkg):
     grid = Grid(0, 1800, 16, 3600, 1800, 100)
     wl = tiny_workload(202, 260, 0.05, grid, n_templates=9, phi_random=True)
