@@ -197,22 +197,26 @@ def test_calls_are_capturable_in_a_cuda_graph(pkg, window, method):
     assert np.array_equal(out.cpu().numpy().view(pkg.RESULT_DTYPE).reshape(-1), eager)
 
 
-@pytest.mark.parametrize("case", range(16))
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("TFSTAT_FUZZ_CASES", "64"))))
 def test_random_grids_all_kernel_families(pkg, case):
     """Seeded random data sets and grids (odd steps, negative and late t0, tau from one second to
     longer than the data, heavy gaps, min_atoms 1..4) through every kernel family."""
     rng = np.random.default_rng(5000 + case)
-    slots = int(rng.integers(20, 900))
+    big = case % 8 == 7  # every eighth case: several staging chunks, CTAs and column tiles
+    slots = int(rng.integers(20, 900)) * (6 if big else 1)
     gaps = float(rng.choice([0.0, 0.1, 0.4, 0.7]))
     dt0 = int(rng.choice([1800, 900, 2700, 1801, 3600, 7200, 777]))
     dtau = int(rng.choice([1800, 900, 3600, 5400, 1799, 43200, 1234]))
     N_t0, N_tau = int(rng.integers(1, 60)), int(rng.integers(1, 200))
+    if big:
+        N_t0, N_tau = 4 * N_t0, 3 * N_tau
     t0_min = int(rng.integers(-5, slots)) * 1800 + int(rng.choice([0, 0, 17]))
     tau_min = int(rng.choice([1, 1800, 3600, 1800 * 7 + 3]))
     grid = Grid(t0_min, dt0, N_t0, tau_min, dtau, N_tau)
     min_atoms = int(rng.integers(1, 5))
-    wl = tiny_workload(6000 + case, slots, gaps, grid)
-    atoms, t = wl.data.atoms[0], wl.data.t
+    T = 1 + case % 3  # the batched search sees 1..3 templates; maps are checked on the last one
+    wl = tiny_workload(6000 + case, slots, gaps, grid, n_templates=T, phi_random=True)
+    atoms, t = wl.data.atoms[T - 1], wl.data.t
     for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN},
                                  {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 3)}]),
                         (RECT, [{"rect_method": 1}, {"rect_method": 2}])):
@@ -221,9 +225,9 @@ def test_random_grids_all_kernel_families(pkg, case):
             what = f"case {case} window {window} {kw}"
             m, f = run_map(pkg, atoms, t, window, grid, min_atoms=min_atoms, **kw)
             check_cells(m, f, ref, what)
-            res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, grid, min_atoms=min_atoms,
-                                    **kw)
-            check_result(res.numpy()[0], ref["twoF"], ref["flags"], grid.N_tau, what)
+            res = pkg.tfstat_search(dev(wl.data.atoms), dev(t), window, grid,
+                                    min_atoms=min_atoms, **kw)
+            check_result(res.numpy()[T - 1], ref["twoF"], ref["flags"], grid.N_tau, what)
         # the same window through the general entry point on arrays spelling out the grid
         mg, fg, rg = pkg.tfstat_map_general(dev(atoms), dev(t), window, (3, 1) if window == EXP else (1, 1),
                                             dev(grid.t0().astype(np.int32)),
