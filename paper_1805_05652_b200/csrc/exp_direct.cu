@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
             uint32_t fl;
             // the sums carry the weight of the tile's first cell; eq. (7) does not care, and the
             // fp64 redo of short ill-conditioned windows uses the cell's own t0
-            const float twoF = closure_2F_exp(A, B, Cc, far, fai, fbr, fbi, lo_c, cnt,
+            const float twoF = closure_2F_exp<false>(A, B, Cc, far, fai, fbr, fbi, lo_c, cnt,
                                               pr.min_atoms, fl, base, ld, bd.t, t0_of(g, m),
                                               (double)tau_of(g, n));
             const int32_t flat = m * g.N_tau + n;

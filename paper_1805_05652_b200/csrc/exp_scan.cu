@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(NT)
                 uint32_t fl;
                 // one closure per t0 step is a quarter of this kernel's instructions in fp64
                 const float twoF =
-                    closure_2F_exp(A, B, acc[q].c, far, fai, fbr, fbi, lo_m, hi - lo_m,
+                    closure_2F_exp<true>(A, B, acc[q].c, far, fai, fbr, fbi, lo_m, hi - lo_m,
                                    pr.min_atoms, fl, base[q], ld, bd.t, t0_of(g, m), tau);
                 const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
                 if (pr.out_maps) pr.out_maps[o] = twoF;

@@ -97,12 +97,13 @@ __device__ __forceinline__ float closure_2F(const Sums64 &s, int cnt, int min_at
 // they keep the fp32 sums and the fp64 closure.
 constexpr int kRedoMaxAtoms = 64;
 
-static __device__ __noinline__ Sums64 exp_resum64(const float *__restrict__ base, const int64_t ld,
+static __device__ __forceinline__ Sums64 exp_resum64_inline(const float *__restrict__ base, const int64_t ld,
                                            const int32_t *__restrict__ t, const int lo,
                                            const int hi, const long long t0, const double tau)
 {
     Sums64 s;
     s.A = s.B = s.C = s.far = s.fai = s.fbr = s.fbi = 0.0;
+#pragma unroll 1
     for (int al = lo; al < hi; ++al) {
         const double w = exp(-(double)((long long)__ldg(t + al) - t0) / tau);
         const double w2 = w * w;
@@ -117,6 +118,20 @@ static __device__ __noinline__ Sums64 exp_resum64(const float *__restrict__ base
     return s;
 }
 
+static __device__ __noinline__ Sums64 exp_resum64_call(const float *__restrict__ base,
+                                                       const int64_t ld,
+                                                       const int32_t *__restrict__ t, const int lo,
+                                                       const int hi, const long long t0,
+                                                       const double tau)
+{
+    return exp_resum64_inline(base, ld, t, lo, hi, t0, tau);
+}
+
+// REDO_INLINE: how the rare fp64 re-sum is attached.  Measured on B200: as a call it costs the
+// direct kernel nothing (3.76e12 terms/s; inlined 3.59e12, the allocator gives the fp64 loop
+// registers the packed accumulators need), while the sliding kernel, whose closure sits inside
+// the t0 loop, is better off with it inlined (96 registers instead of 121).
+template <bool REDO_INLINE>
 __device__ __forceinline__ float closure_2F_exp(const float A, const float B, const float C,
                                                 const float far, const float fai,
                                                 const float fbr, const float fbi, const int lo,
@@ -139,7 +154,8 @@ __device__ __forceinline__ float closure_2F_exp(const float A, const float B, co
     }
     Sums64 s;
     if (cnt >= min_atoms && cnt >= 1 && cnt <= kRedoMaxAtoms) {
-        s = exp_resum64(base, ld, t, lo, lo + cnt, t0, tau);
+        s = REDO_INLINE ? exp_resum64_inline(base, ld, t, lo, lo + cnt, t0, tau)
+                        : exp_resum64_call(base, ld, t, lo, lo + cnt, t0, tau);
     } else {
         s.A = A;
         s.B = B;
