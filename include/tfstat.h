@@ -174,7 +174,7 @@ typedef struct tfstat_window {
  * degenerate cells (flags 3), not an error (the arrays live on the device).
  *   out_map, out_flags, out: each nullable, at least one of out_map / out required.
  *   workspace: >= tfstat_general_workspace_bytes(N_t0, N_tau) bytes, 256-B aligned.
- *   opts_host: only min_atoms is used.                                                      */
+ *   opts_host: min_atoms, and tile_c (tuning: tau cells per thread, 1 / 2 / 4; 0 = auto).     */
 size_t tfstat_general_workspace_bytes(int32_t N_t0, int32_t N_tau);
 int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
                        const tfstat_window *window_host, const int32_t *t0_grid, int32_t N_t0,

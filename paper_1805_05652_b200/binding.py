@@ -259,7 +259,7 @@ def tfstat_map_general(atoms: torch.Tensor, t_atoms: torch.Tensor, kind: int, su
                        t0_grid: torch.Tensor, tau_grid: torch.Tensor, *,
                        table: Optional[torch.Tensor] = None, min_atoms: int = 2,
                        want_map: bool = True, want_flags: bool = False,
-                       want_marginals: bool = True, stream=None):
+                       want_marginals: bool = True, stream=None, cells_per_thread: int = 0):
     """General window on explicit grids (include/tfstat.h, tfstat_map_general).
 
     atoms [7, N]; t0_grid [N_t0], tau_grid [N_tau]: CUDA int32 tensors of seconds (any order);
@@ -292,6 +292,7 @@ def tfstat_map_general(atoms: torch.Tensor, t_atoms: torch.Tensor, kind: int, su
     nbytes = int(lib.tfstat_general_workspace_bytes(N_t0, N_tau))
     ws = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=dev)
     o = _opts(min_atoms, EXP_AUTO)
+    o.tile_c = int(cells_per_thread)
     rc = lib.tfstat_map_general(atoms.data_ptr(), ld, t_atoms.data_ptr(), n_atoms, C.byref(w),
                                 t0_grid.data_ptr(), N_t0, tau_grid.data_ptr(), N_tau,
                                 out_map.data_ptr() if want_map else None,

@@ -365,10 +365,11 @@ int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, i
     const int32_t min_atoms = (opts_host && opts_host->min_atoms > 0) ? opts_host->min_atoms : 2;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     Partial *partials = out ? static_cast<Partial *>(workspace) : nullptr;
+    int32_t n_partials = 0;
     TF_CUDA(launch_general(atoms, ld, t_atoms, n_atoms, w, t0_grid, N_t0, tau_grid, N_tau,
-                           min_atoms, out_map, out_flags, partials, st));
-    if (out)
-        TF_CUDA(launch_finalize(partials, general_partials(N_t0, N_tau), 1, N_tau, out, st));
+                           min_atoms, out_map, out_flags, partials, &n_partials,
+                           opts_host ? opts_host->tile_c : 0, st));
+    if (out) TF_CUDA(launch_finalize(partials, n_partials, 1, N_tau, out, st));
     return TFSTAT_OK;
 }
 

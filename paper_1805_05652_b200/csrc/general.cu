@@ -77,7 +77,12 @@ __device__ __noinline__ Sums64 general_resum64(const GeneralArgs &a, const int l
     return s;
 }
 
-template <int KIND>
+// CT cells per thread (consecutive tau indices of the CTA's NT x CT block): one broadcast read
+// of an atom record serves CT cells; the weights stay per cell.  With CT = 1 the two LDS.128 per
+// term put the L1 wavefront counter at 78 % of its peak (ncu), but measured on B200 CT = 2 is
+// only 3 % faster (configs 2, 3, 5) and CT = 4 is 7-20 % slower (fewer, longer CTAs; one select
+// per term for the ragged window ends): the kernel is bound by its ~11 instructions per term.
+template <int KIND, int CT>
 __global__ void __launch_bounds__(kGenNT)
     general_kernel(const GeneralArgs a, Partial *__restrict__ partials, const int n_nblocks)
 {
@@ -89,19 +94,34 @@ __global__ void __launch_bounds__(kGenNT)
     pdl_trigger();
 
     const int m = blockIdx.x / n_nblocks;
-    const int n = (blockIdx.x % n_nblocks) * kGenNT + threadIdx.x;
-    const bool n_ok = n < a.N_tau;
+    // a thread's CT cells are CONSECUTIVE entries of the tau array: on a sorted array their
+    // windows have nearly the same length, so little of the shared atom loop is wasted
+    const int n0 = (blockIdx.x % n_nblocks) * (kGenNT * CT) + threadIdx.x * CT;
     const long long t0 = __ldg(a.t0_grid + m);
-    const long long tau = n_ok ? (long long)__ldg(a.tau_grid + n) : 0;
     // a1: bounds.  dt * den < num * tau  <=>  t < t0 + ceil(num tau / den)
     const int lo = lower_bound_t(a.t, a.n_atoms, t0);
-    int hi = lo;
-    if (tau >= 1) {
-        const long long len = ((long long)a.sup_num * tau + a.sup_den - 1) / a.sup_den;
-        hi = lower_bound_t(a.t, a.n_atoms, t0 + len);
+    long long tau[CT];
+    int hi[CT];
+    float kw[CT];  // exp: w = 2^(dt * kw); table: x = dt * kw, knots at integer x
+    int hmax = lo;
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+        const int n = n0 + c;
+        tau[c] = n < a.N_tau ? (long long)__ldg(a.tau_grid + n) : 0;
+        hi[c] = lo;
+        kw[c] = 0.0f;
+        if (tau[c] >= 1) {
+            const long long len = ((long long)a.sup_num * tau[c] + a.sup_den - 1) / a.sup_den;
+            hi[c] = lower_bound_t(a.t, a.n_atoms, t0 + len);
+            kw[c] = KIND == TFSTAT_WINDOW_EXP
+                        ? (float)(-1.4426950408889634 / (double)tau[c])
+                        : (float)((double)(a.n_table - 1) * (double)a.sup_den /
+                                  ((double)a.sup_num * (double)tau[c]));
+        }
+        hmax = max(hmax, hi[c]);
     }
-    // atom range of the CTA: [lo, max over its threads of hi)
-    int hmax = hi;
+    // atom range of the CTA: [lo, max over its cells of hi)
+    const int my_e = hmax;
 #pragma unroll
     for (int s = 16; s >= 1; s >>= 1) hmax = max(hmax, __shfl_xor_sync(0xffffffffu, hmax, s));
     if ((threadIdx.x & 31) == 0) s_hi[threadIdx.x >> 5] = hmax;
@@ -112,17 +132,15 @@ __global__ void __launch_bounds__(kGenNT)
     int cta_e = s_hi[0];
 #pragma unroll
     for (int w = 1; w < kGenNT / 32; ++w) cta_e = max(cta_e, s_hi[w]);
-
-    // weight constants: exp: w = 2^(dt * kexp); table: x = dt * kx, knots at integer x
-    const float inv_tau = tau >= 1 ? (float)(1.0 / (double)tau) : 0.0f;
-    const float kexp = -1.4426950408889634f * inv_tau;
-    const float kx = tau >= 1 ? (float)((double)(a.n_table - 1) * (double)a.sup_den /
-                                        ((double)a.sup_num * (double)tau))
-                              : 0.0f;
     const float *__restrict__ tab = tab_smem ? s_tab : a.table;
 
-    u64 acc_ab = 0ull, acc_fa = 0ull, acc_fb = 0ull;  // (A, B), (Re Fa, Im Fa), (Re Fb, Im Fb)
-    float acc_c = 0.0f;
+    u64 acc_ab[CT], acc_fa[CT], acc_fb[CT];  // (A, B), (Re Fa, Im Fa), (Re Fb, Im Fb)
+    float acc_c[CT];
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+        acc_ab[c] = acc_fa[c] = acc_fb[c] = 0ull;
+        acc_c[c] = 0.0f;
+    }
 #pragma unroll 1
     for (int cs = lo; cs < cta_e; cs += kGenKC) {
         const int n_stage = min(kGenKC, cta_e - cs);
@@ -138,29 +156,33 @@ __global__ void __launch_bounds__(kGenNT)
             s_b[i] = rb;
         }
         __syncthreads();
-        const int x1 = min(cs + n_stage, hi) - cs;  // this thread's atoms of the chunk: [0, x1)
-#pragma unroll 4
+        const int x1 = min(cs + n_stage, my_e) - cs;  // this thread's atoms of the chunk: [0, x1)
+#pragma unroll 2
         for (int i = 0; i < x1; ++i) {
             const ulonglong2 ra = s_a[i], rb = s_b[i];
             float dt, ab;
             unpack2(ra.x, dt, ab);
-            float w;
-            if (KIND == TFSTAT_WINDOW_RECT) {
-                w = 1.0f;
-            } else if (KIND == TFSTAT_WINDOW_EXP) {
-                w = ex2_approx(dt * kexp);
-            } else {
-                const float x = dt * kx;
-                const int k = min((int)x, a.n_table - 2);
-                const float t0v = tab[k], t1v = tab[k + 1];
-                w = fmaf(x - (float)k, t1v - t0v, t0v);
+#pragma unroll
+            for (int c = 0; c < CT; ++c) {
+                float w;
+                if (KIND == TFSTAT_WINDOW_RECT) {
+                    w = 1.0f;
+                } else if (KIND == TFSTAT_WINDOW_EXP) {
+                    w = ex2_approx(dt * kw[c]);
+                } else {
+                    const float x = dt * kw[c];
+                    const int k = min((int)x, a.n_table - 2);
+                    const float t0v = tab[k], t1v = tab[k + 1];
+                    w = fmaf(x - (float)k, t1v - t0v, t0v);
+                }
+                if (CT > 1) w = cs + i < hi[c] ? w : 0.0f;  // beyond this cell's own window
+                const float w2 = w * w;
+                ffma2(acc_ab[c], pack2(w2, w2), ra.y);
+                const u64 ww = pack2(w, w);
+                ffma2(acc_fa[c], ww, rb.x);
+                ffma2(acc_fb[c], ww, rb.y);
+                acc_c[c] = fmaf(w2, ab, acc_c[c]);
             }
-            const float w2 = w * w;
-            ffma2(acc_ab, pack2(w2, w2), ra.y);
-            const u64 ww = pack2(w, w);
-            ffma2(acc_fa, ww, rb.x);
-            ffma2(acc_fb, ww, rb.y);
-            acc_c = fmaf(w2, ab, acc_c);
         }
         __syncthreads();
     }
@@ -168,23 +190,26 @@ __global__ void __launch_bounds__(kGenNT)
     // a4 closure + a5 marginals
     Marg mg;
     marg_init(mg);
-    if (n_ok) {
+#pragma unroll
+    for (int c = 0; c < CT; ++c) {
+        const int n = n0 + c;
+        if (n >= a.N_tau) continue;
         Sums64 s;
         float A, B, far, fai, fbr, fbi;
-        unpack2(acc_ab, A, B);
-        unpack2(acc_fa, far, fai);
-        unpack2(acc_fb, fbr, fbi);
+        unpack2(acc_ab[c], A, B);
+        unpack2(acc_fa[c], far, fai);
+        unpack2(acc_fb[c], fbr, fbi);
         s.A = A;
         s.B = B;
-        s.C = acc_c;
+        s.C = acc_c[c];
         s.far = far;
         s.fai = fai;
         s.fbr = fbr;
         s.fbi = fbi;
-        const int cnt = hi - lo;
+        const int cnt = hi[c] - lo;
         if (cnt >= a.min_atoms && cnt >= 1 && cnt <= kRedoMaxAtoms &&
             !(s.A * s.B - s.C * s.C > 0.015625 * s.A * s.B))
-            s = general_resum64<KIND>(a, lo, hi, t0, (double)tau);
+            s = general_resum64<KIND>(a, lo, hi[c], t0, (double)tau[c]);
         uint32_t fl;
         const float twoF = closure_2F(s, cnt, a.min_atoms, fl);
         const int32_t flat = m * a.N_tau + n;
@@ -198,6 +223,19 @@ __global__ void __launch_bounds__(kGenNT)
     }
 }
 
+template <int KIND>
+cudaError_t launch_kind(const GeneralArgs &a, Partial *partials, int ct, cudaStream_t st)
+{
+    const int n_nblocks = (a.N_tau + kGenNT * ct - 1) / (kGenNT * ct);
+    const unsigned grid = (unsigned)a.N_t0 * (unsigned)n_nblocks;
+    switch (ct) {
+    case 4: general_kernel<KIND, 4><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks); break;
+    case 2: general_kernel<KIND, 2><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks); break;
+    default: general_kernel<KIND, 1><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks); break;
+    }
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 int32_t general_partials(int32_t N_t0, int32_t N_tau)
@@ -208,7 +246,8 @@ int32_t general_partials(int32_t N_t0, int32_t N_tau)
 cudaError_t launch_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
                            const tfstat_window &w, const int32_t *t0_grid, int32_t N_t0,
                            const int32_t *tau_grid, int32_t N_tau, int32_t min_atoms,
-                           float *out_map, uint8_t *out_flags, Partial *partials, cudaStream_t st)
+                           float *out_map, uint8_t *out_flags, Partial *partials,
+                           int32_t *n_partials, int32_t ct_override, cudaStream_t st)
 {
     GeneralArgs a;
     a.atoms = atoms;
@@ -226,21 +265,17 @@ cudaError_t launch_general(const float *atoms, int64_t ld, const int32_t *t_atom
     a.min_atoms = min_atoms;
     a.out_map = out_map;
     a.out_flags = out_flags;
-    const int n_nblocks = (N_tau + kGenNT - 1) / kGenNT;
-    const unsigned grid = (unsigned)N_t0 * (unsigned)n_nblocks;
+    // cells per thread: 2 while that still leaves ~8 CTAs per SM, else 1 (4 only on request)
+    auto ctas = [&](int ct) { return (int64_t)N_t0 * ((N_tau + kGenNT * ct - 1) / (kGenNT * ct)); };
+    int ct = (N_tau >= 2 * kGenNT && ctas(2) >= 148 * 8) ? 2 : 1;
+    if (ct_override == 1 || ct_override == 2 || ct_override == 4) ct = ct_override;
+    *n_partials = (int32_t)ctas(ct);
     switch (w.kind) {
-    case TFSTAT_WINDOW_RECT:
-        general_kernel<TFSTAT_WINDOW_RECT><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks);
-        break;
-    case TFSTAT_WINDOW_EXP:
-        general_kernel<TFSTAT_WINDOW_EXP><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks);
-        break;
-    case TFSTAT_WINDOW_TABLE:
-        general_kernel<TFSTAT_WINDOW_TABLE><<<grid, kGenNT, 0, st>>>(a, partials, n_nblocks);
-        break;
-    default: return cudaErrorInvalidValue;
+    case TFSTAT_WINDOW_RECT: return launch_kind<TFSTAT_WINDOW_RECT>(a, partials, ct, st);
+    case TFSTAT_WINDOW_EXP: return launch_kind<TFSTAT_WINDOW_EXP>(a, partials, ct, st);
+    case TFSTAT_WINDOW_TABLE: return launch_kind<TFSTAT_WINDOW_TABLE>(a, partials, ct, st);
     }
-    return cudaGetLastError();
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace tfstat

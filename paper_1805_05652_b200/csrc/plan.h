@@ -99,7 +99,8 @@ int32_t general_partials(int32_t N_t0, int32_t N_tau);
 cudaError_t launch_general(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n_atoms,
                            const tfstat_window &w, const int32_t *t0_grid, int32_t N_t0,
                            const int32_t *tau_grid, int32_t N_tau, int32_t min_atoms,
-                           float *out_map, uint8_t *out_flags, Partial *partials, cudaStream_t st);
+                           float *out_map, uint8_t *out_flags, Partial *partials,
+                           int32_t *n_partials, int32_t ct_override, cudaStream_t st);
 
 inline Bounds make_bounds(const Plan &pl, const int32_t *t_atoms, void *ws)
 {

@@ -69,8 +69,9 @@ CASES = [
 ]
 
 
+@pytest.mark.parametrize("ct", [0, 1, 2, 4])
 @pytest.mark.parametrize("kind,sup,ntab", CASES)
-def test_general_irregular_grids(pkg, kind, sup, ntab):
+def test_general_irregular_grids(pkg, kind, sup, ntab, ct):
     """Unsorted, repeated, off-lattice t0 values (some before the data), 300 irregular tau values
     (three CTAs along tau with a ragged tail, long windows spanning several staged chunks)."""
     wl = tiny_workload(301, 1500, 0.2, Grid(0, TSFT, 1, TSFT, TSFT, 1))
@@ -81,7 +82,7 @@ def test_general_irregular_grids(pkg, kind, sup, ntab):
     taug = rng.permutation(np.concatenate([[1, 1799, 1800, 1801],
                                            rng.integers(TSFT, 900 * TSFT, size=296)])).astype(np.int32)
     table = None if ntab is None else power_law(sup, ntab)
-    m, f, r = run(pkg, atoms, t, kind, sup, t0g, taug, table)
+    m, f, r = run(pkg, atoms, t, kind, sup, t0g, taug, table, cells_per_thread=ct)
     ref = map2F_general(atoms, t, kind, sup, t0g, taug, table=table)
     check_cells(m, f, ref, f"general kind {kind}")
     check_result(r, ref["twoF"], ref["flags"], len(taug), f"general kind {kind}")
