@@ -33,7 +33,7 @@ WORKLOAD = "cfg4_search_4096x2880atoms_96x1417"
 # + 7 FFMA (A,B,C,Re/Im Fa,Re/Im Fb) on the FP32 pipe, + 1 MUFU.EX2 on the XU pipe
 FP32_OPS_PER_TERM = 9
 FP32_LANES_PER_CLK_SM = 128  # cc 10.0: 4 SMSPs x 32 FP32 lanes
-NCU_DRAM_BYTES_PER_TEMPLATE = 23.985408e6 / 296  # profiles/r01_pass4_kernels_full.md
+NCU_DRAM_BYTES_PER_TEMPLATE = 23.984128e6 / 296  # profiles/r01_pass4_kernels_full.md
 
 
 def read_peaks():
@@ -449,7 +449,7 @@ def run_ours(args):
         "measured_ffma_lane_ops_per_s": probes["ffma"]["lane_ops_per_s"],
         "frac_of_measured_ffma": ach_ops / probes["ffma"]["lane_ops_per_s"],
         # dram__bytes_read.sum + dram__bytes_write.sum of exp_direct_kernel from the ncu --set full
-        # capture in profiles/r01_pass4_kernels_full.md (23.99 MB for 296 templates, written
+        # capture in profiles/r01_pass4_kernels_full.md (23.98 MB for 296 templates, written
         # bytes 0), scaled per template to this launch
         "traffic": NCU_DRAM_BYTES_PER_TEMPLATE * n_tpl,
         "traffic_unit": "bytes per launch (ncu capture of 296 templates, scaled per template)",
