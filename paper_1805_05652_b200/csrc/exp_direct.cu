@@ -29,6 +29,13 @@
 //    SHORTEST windows, and CTAs are launched heaviest (largest tau) first.
 #include "plan.h"
 
+// Tuning constants of the core loop, swept on B200 (config 4, 592 templates): staging chunk KC in
+// {256, 512, 1024} atoms x unroll in {2 .. 64}.  Unrolling is what matters (unroll 4: 3.79e12
+// terms/s, 8: 3.94, 16: 4.10, 32: 4.17, 64: 4.11; the loop counter, the shared-memory address
+// arithmetic and the branch are per iteration, and the scheduler gets more independent LDS /
+// MUFU to hoist above the FFMA2 stream); KC = 1024 adds ~1 % over 512 (half the barriers).
+constexpr int kStageAtoms = 1024;
+constexpr int kCoreUnroll = 32;
 namespace tfstat {
 
 namespace {
@@ -182,7 +189,7 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
         // a3: weighted sums over this chunk, per-thread bounds
         const int x0 = max(cs, cb) - cs;
         const int x1 = min(cs + n_stage, ce) - cs;
-#pragma unroll 4
+#pragma unroll kCoreUnroll
         for (int i = x0; i < x1; ++i) accumulate_core<C>(acc, s_a[i], s_b[i], kexp);
         __syncthreads();
     }
@@ -225,7 +232,7 @@ template <int C, int NT>
 cudaError_t launch_one(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
 {
     const int64_t n_ctas = pl.tiles_per_template * pl.n_templates;
-    return launch_pdl(exp_direct_kernel<C, NT, 512>, (unsigned)n_ctas, NT, 0, st, pr, partials,
+    return launch_pdl(exp_direct_kernel<C, NT, kStageAtoms>, (unsigned)n_ctas, NT, 0, st, pr, partials,
                       pl.n_mtiles, pl.n_nblocks);
 }
 
