@@ -30,6 +30,8 @@
 // into segments, each with its own initial sum, to fill the GPU.
 #include "plan.h"
 
+// unroll of the initial-window loop: swept 2..32 on B200, 16 is 4-5 % faster than 4
+constexpr int kWindowUnroll = 16;
 namespace tfstat {
 
 namespace {
@@ -161,7 +163,7 @@ __global__ void __launch_bounds__(NT)
         }
         __syncthreads();
         const int x1 = min(cs + n_stage, hi) - cs;
-#pragma unroll 4
+#pragma unroll kWindowUnroll
         for (int i = 0; i < x1; ++i) {
             float e = 0.0f, e2 = 0.0f;
 #pragma unroll
