@@ -109,6 +109,50 @@ def test_error_codes_before_any_cuda_call(lib):
     assert lib.tfstat_marginalise(None, None, 4, 4, fake, fake, 1 << 20, None) == -1
     assert lib.tfstat_marginalise(fake, None, 4, 4, fake, fake, 0, None) == -2
     assert lib.tfstat_strerror(-2).decode().startswith("workspace")
+    # rect_method / exp_method out of range
+    import paper_1805_05652_b200.binding as b
+    o = b._Opts()
+    o.rect_method = 3
+    assert lib.tfstat_search(fake, 70, 10, fake, 10, 1, 0, *grid, fake, None, None, fake, 1 << 20,
+                             None, C.byref(o)) == -1
+    o = b._Opts()
+    o.exp_method = 9
+    assert lib.tfstat_search(fake, 70, 10, fake, 10, 1, 1, *grid, fake, None, None, fake, 1 << 20,
+                             None, C.byref(o)) == -1
+    # tfstat_map_general: null window, bad kind, empty support, table missing, workspace
+    w = b._Window()
+    w.kind, w.support_num, w.support_den = 1, 3, 1
+    args = lambda win, ws=fake, nws=1 << 20: (fake, 10, fake, 10, win, fake, 4, fake, 4, fake, None,  # noqa: E731
+                                              None, ws, nws, None, None)
+    assert lib.tfstat_map_general(*args(None)) == -1
+    assert lib.tfstat_map_general(*args(C.byref(w), None)) == -2
+    assert lib.tfstat_map_general(*args(C.byref(w), fake, 8)) == -2
+    w.kind = 7
+    assert lib.tfstat_map_general(*args(C.byref(w))) == -1
+    w.kind, w.support_num = 1, 0
+    assert lib.tfstat_map_general(*args(C.byref(w))) == -1
+    w.kind, w.support_num, w.n_table = 2, 1, 0
+    assert lib.tfstat_map_general(*args(C.byref(w))) == -1
+    assert lib.tfstat_general_workspace_bytes(0, 4) == 0
+    assert lib.tfstat_general_workspace_bytes(4, 300) == 256 * ((32 * 4 * 3 + 255) // 256)
+    # tfstat_merge_detectors: n_det out of range, null arrays, ld < n
+    pa = (C.c_void_p * 1)(0x1000)
+    i64 = (C.c_int64 * 1)(70)
+    ld = (C.c_int64 * 1)(10)
+    n = (C.c_int32 * 1)(10)
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 0, 1, fake, 10, fake, 70, 10, None) == -1
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 9, 1, fake, 10, fake, 70, 10, None) == -1
+    assert lib.tfstat_merge_detectors(None, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 10, None) == -1
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 9, None) == -1
+    ld[0] = 9
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 10, None) == -1
+    # tfstat_search_host: null host pointers, misaligned scratch
+    assert lib.tfstat_search_host(None, 70, 10, fake, 10, 1, 1, *grid, fake, None, None, 0,
+                                  None) == -1
+    assert lib.tfstat_search_host(fake, 70, 10, fake, 10, 1, 1, *grid, fake, None,
+                                  C.c_void_p(0x1001), 1 << 20, None) == -2
+    assert lib.tfstat_search_host_scratch_bytes(70, 10, 0, 1, *grid, 0, None) == 0
+    assert lib.tfstat_search_host_scratch_bytes(70, 10, 5, 1, *grid, 1, None) > 5 * 70 * 4 * 2
 
 
 def test_missing_library_fails_loudly(monkeypatch):
