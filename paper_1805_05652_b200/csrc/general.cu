@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(kGenNT)
         s.fbr = fbr;
         s.fbi = fbi;
         const int cnt = hi[c] - lo;
-        if (cnt >= a.min_atoms && cnt >= 1 && cnt <= kRedoMaxAtoms &&
+        if (cnt >= 1 && cnt <= kRedoMaxAtoms &&
             !(s.A * s.B - s.C * s.C > 0.015625 * s.A * s.B))
             s = general_resum64<KIND>(a, lo, hi[c], t0, (double)tau[c]);
         uint32_t fl;

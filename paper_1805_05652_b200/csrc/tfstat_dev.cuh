@@ -153,7 +153,7 @@ __device__ __forceinline__ float closure_2F_exp(const float A, const float B, co
         return 2.0f * __fdividef(num, D);
     }
     Sums64 s;
-    if (cnt >= min_atoms && cnt >= 1 && cnt <= kRedoMaxAtoms) {
+    if (cnt >= 1 && cnt <= kRedoMaxAtoms) {  // also cells with too few atoms: their D flag counts
         s = REDO_INLINE ? exp_resum64_inline(base, ld, t, lo, lo + cnt, t0, tau)
                         : exp_resum64_call(base, ld, t, lo, lo + cnt, t0, tau);
     } else {
