@@ -236,6 +236,17 @@ def test_random_grids_all_kernel_families(pkg, case):
         check_cells(mg.cpu().numpy(), fg.cpu().numpy(), ref, f"case {case} window {window} general")
         check_result(rg.numpy()[0], ref["twoF"], ref["flags"], grid.N_tau,
                      f"case {case} window {window} general")
+    # a random tabulated window with a rational support on the same (explicit) grid
+    from oracle.binding import map2F_general
+
+    sup = (int(rng.integers(1, 8)), int(rng.integers(1, 4)))
+    table = rng.uniform(0.05, 1.0, size=int(rng.integers(2, 40))).astype(np.float32)
+    t0g, taug = grid.t0().astype(np.int32), grid.tau().astype(np.int32)
+    mg, fg, rg = pkg.tfstat_map_general(dev(atoms), dev(t), 2, sup, dev(t0g), dev(taug),
+                                        table=dev(table), want_flags=True, min_atoms=min_atoms)
+    reft = map2F_general(atoms, t, 2, sup, t0g, taug, table=table, min_atoms=min_atoms)
+    check_cells(mg.cpu().numpy(), fg.cpu().numpy(), reft, f"case {case} table window")
+    check_result(rg.numpy()[0], reft["twoF"], reft["flags"], grid.N_tau, f"case {case} table window")
 
 
 def test_concurrent_streams_do_not_interfere(pkg):
