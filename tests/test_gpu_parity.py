@@ -249,6 +249,45 @@ def test_random_grids_all_kernel_families(pkg, case):
     check_result(rg.numpy()[0], reft["twoF"], reft["flags"], grid.N_tau, f"case {case} table window")
 
 
+def test_rect_maximum_grid_size_marginals(pkg):
+    """The largest grid the ABI accepts (N_t0 N_tau just under 2^31 cells: flat indices up to the
+    int32 limit), fused marginals only (the 8.6 GB map is never written).  n_valid is checked
+    against integer window counts, the maximum against the oracle at the argmax and on a random
+    sample, logB against its bounds."""
+    N = 46340  # 46340^2 = 2 147 395 600 < 2^31
+    grid = Grid(0, 1800, N, 1800, 1800, N)
+    assert grid.n_cells < 2 ** 31 and (N + 1) ** 2 >= 2 ** 31
+    lib = pkg.load_library()
+    assert lib.tfstat_workspace_bytes(RECT, 100, 1, 0, 1800, N + 1, 1800, 1800, N + 1, None) == 0
+    wl = tiny_workload(220, 60000, 0.1, grid)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    res = pkg.tfstat_search(dev(atoms[None]), dev(t), RECT, grid).numpy()[0]
+    # integer count of valid cells: cnt(m, n) >= 2, counts grow with n (all such cells have D > 0
+    # here: two-detector atoms, checked on the sample below)
+    t64 = t.astype(np.int64)
+    lo = np.searchsorted(t64, grid.t0())
+    n_valid = 0
+    for m0 in range(0, N, 4096):  # rows in slabs: first n with >= 2 atoms in the window
+        rows = slice(m0, min(m0 + 4096, N))
+        need = np.minimum(lo[rows] + 1, len(t64) - 1)          # index of the window's 2nd atom
+        has2 = lo[rows] + 1 < len(t64)
+        tau_need = t64[need] - grid.t0()[rows] + 1              # smallest tau that includes it
+        n_first = np.maximum(0, -(-(tau_need - grid.tau_min) // grid.dtau))
+        n_valid += int(np.sum(np.where(has2, np.clip(N - n_first, 0, N), 0)))
+    assert int(res["n_valid"]) == n_valid
+    assert 0 <= res["m"] < N and 0 <= res["n"] < N
+    at = oracle.cells(atoms, t, RECT, grid, np.array([res["m"]], np.int32),
+                      np.array([res["n"]], np.int32))
+    assert abs(at["twoF"][0] - res["max2F"]) <= TOL_2F * max(1.0, at["twoF"][0])
+    rng = np.random.default_rng(3)
+    ms = rng.integers(0, N, 3000).astype(np.int32)
+    ns = rng.integers(0, N, 3000).astype(np.int32)
+    smp = oracle.cells(atoms, t, RECT, grid, ms, ns)
+    assert np.all(smp["twoF"] <= res["max2F"] * (1 + TOL_2F) + TOL_2F)
+    assert np.all((smp["flags"] & 2) == ((smp["cnt"] == 0) * 2))  # D > 0 wherever there are atoms
+    assert 0.5 * res["max2F"] - 1e-3 <= res["logB"] <= 0.5 * res["max2F"] + np.log(n_valid) + 1e-3
+
+
 def test_concurrent_streams_do_not_interfere(pkg):
     """The library keeps no state between calls: searches enqueued on two streams at once, each
     with its own workspace, give the bits of the same searches run one after the other."""
