@@ -437,6 +437,7 @@ constexpr int kPitch = 16;   // floats per tile row; the four 16-byte column gro
                              // XOR-swizzled with (i >> 1) & 3: conflict-free STS.128 and LDS.128
 constexpr int kFPitch = 5;   // 32-bit words per flag-tile row (16 flag bytes + pad)
 constexpr float kCondFast = 1.0f / 64.0f;  // fp32 closure only if D > kCondFast * A * B
+constexpr float kTiny = 1.0e-30f;          // ... and D > kTiny
 constexpr float kHalfLog2e = 0.72134752044448170368f;
 
 __device__ __forceinline__ u64 fadd2(const u64 a, const u64 b)
@@ -493,7 +494,9 @@ __device__ __forceinline__ PairOut pair_closure(const u64 (&S)[8])
     u64 D = p;
     ffma2(D, S[3], S[2]);
     PairOut o;
-    o.t = D;
+    // t = D - kCondFast A B - kTiny: the fast path also needs D well inside the normal fp32
+    // range (atoms scaled far down: rcp.approx.ftz of a subnormal D is inf)
+    o.t = fadd2(D, pack2(-kTiny, -kTiny));
     ffma2(o.t, p, pack2(-kCondFast, -kCondFast));
     u64 na = fmul2(S[4], S[4]);
     ffma2(na, S[5], S[5]);
@@ -505,6 +508,9 @@ __device__ __forceinline__ PairOut pair_closure(const u64 (&S)[8])
     ffma2(num, S[0], nb);
     ffma2(num, S[3], re);
     ffma2(num, S[3], re);
+    // atoms scaled far up: rcp.approx.ftz of D > 2^126 is 0 and the numerator overflows; 0 x inf
+    // = NaN poisons t whenever num * A B leaves the fp32 range (false alarms only cost the fp64 path)
+    ffma2(o.t, fmul2(num, p), 0ull);
     float d0, d1;
     unpack2(D, d0, d1);
     o.res = fmul2(num, pack2(rcp_approx(d0), rcp_approx(d1)));

@@ -142,15 +142,20 @@ __device__ __forceinline__ float closure_2F_exp(const float A, const float B, co
 {
     const float p = A * B;
     const float D = fmaf(-C, C, p);
-    if (D > 0.015625f * p && cnt >= min_atoms) {
+    // (1e-30 < p < 1e30: with atoms scaled far down D would be subnormal and the fast divide inf,
+    // scaled far up __fdividef returns 0 for D > 2^126 and the numerator overflows)
+    if (D > 0.015625f * p && p > 1.0e-30f && p < 1.0e30f && cnt >= min_atoms) {
         const float na = fmaf(far, far, fai * fai);
         const float nb = fmaf(fbr, fbr, fbi * fbi);
         const float re = fmaf(far, fbr, fai * fbi);
         float num = B * na;
         num = fmaf(A, nb, num);
         num = fmaf(-2.0f * C, re, num);
-        flags = 0u;
-        return 2.0f * __fdividef(num, D);
+        const float r = 2.0f * __fdividef(num, D);
+        if (fabsf(r) < 3.0e38f) {  // atoms scaled far up overflow the numerator: fp64 below
+            flags = 0u;
+            return r;
+        }
     }
     Sums64 s;
     if (cnt >= 1 && cnt <= kRedoMaxAtoms) {  // also cells with too few atoms: their D flag counts

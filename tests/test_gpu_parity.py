@@ -288,6 +288,39 @@ def test_rect_maximum_grid_size_marginals(pkg):
     assert 0.5 * res["max2F"] - 1e-3 <= res["logB"] <= 0.5 * res["max2F"] + np.log(n_valid) + 1e-3
 
 
+@pytest.mark.parametrize("scale", [1e-9, 1e-5, 1e6, 1e9])
+def test_amplitude_scaling_far_from_unity(pkg, scale):
+    """I5: (a2, b2, ab) x s^2 and (Fa, Fb) x s leave 2F unchanged.  With s = 1e9 the products
+    A B overflow fp32, with s = 1e-9 they underflow: the fp32 fast paths must hand such cells to
+    the fp64 closure instead of producing inf / NaN / 0."""
+    grid = Grid(0, 1800, 40, 3600, 1800, 160)
+    wl = tiny_workload(230, 500, 0.1, grid)
+    atoms, t = wl.data.atoms[0], wl.data.t
+    scaled = atoms.astype(np.float64).copy()
+    scaled[0:3] *= scale * scale
+    scaled[3:7] *= scale
+    scaled = scaled.astype(np.float32)
+    assert np.all(np.isfinite(scaled)) and np.all(scaled[0] > 0)
+    for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN}]),
+                        (RECT, [{"rect_method": 1}, {"rect_method": 2}])):
+        ref = oracle.map2F(scaled, t, window, grid)        # fp64: fine at any of these scales
+        ref1 = oracle.map2F(atoms, t, window, grid)
+        ok = ref1["flags"] == 0
+        # I5 itself, up to the fresh fp32 rounding of the scaled atoms times the conditioning
+        assert np.allclose(ref["twoF"][ok], ref1["twoF"][ok], rtol=2e-3, atol=2e-3)
+        for kw in kws:
+            m, f = run_map(pkg, scaled, t, window, grid, **kw)
+            check_cells(m, f, ref, f"scale {scale} window {window} {kw}")
+            res = pkg.tfstat_search(dev(scaled[None]), dev(t), window, grid, **kw)
+            check_result(res.numpy()[0], ref["twoF"], ref["flags"], grid.N_tau,
+                         f"scale {scale} window {window} {kw}")
+    mg, fg, _ = pkg.tfstat_map_general(dev(scaled), dev(t), EXP, (3, 1),
+                                       dev(grid.t0().astype(np.int32)),
+                                       dev(grid.tau().astype(np.int32)), want_flags=True)
+    check_cells(mg.cpu().numpy(), fg.cpu().numpy(), oracle.map2F(scaled, t, EXP, grid),
+                f"scale {scale} general")
+
+
 def test_concurrent_streams_do_not_interfere(pkg):
     """The library keeps no state between calls: searches enqueued on two streams at once, each
     with its own workspace, give the bits of the same searches run one after the other."""
