@@ -31,11 +31,11 @@
 
 // Tuning constants of the core loop, swept on B200 (config 4, 592 templates): staging chunk KC in
 // {256, 512, 1024} atoms x unroll in {2 .. 64}.  Unrolling is what matters (unroll 4: 3.79e12
-// terms/s, 8: 3.94, 16: 4.10, 32: 4.17, 64: 4.11; the loop counter, the shared-memory address
+// terms/s, 8: 3.94, 16: 4.10, 24..32: 4.12-4.17, 64: 4.11; the loop counter, the shared-memory address
 // arithmetic and the branch are per iteration, and the scheduler gets more independent LDS /
 // MUFU to hoist above the FFMA2 stream); KC = 1024 adds ~1 % over 512 (half the barriers).
 constexpr int kStageAtoms = 1024;
-constexpr int kCoreUnroll = 32;
+constexpr int kCoreUnroll = 24;
 namespace tfstat {
 
 namespace {
@@ -148,23 +148,23 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
             const float ab = __ldg(base + 2 * ld + al);
             const u64 fa = pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al));
             const u64 fb = pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al));
-            float wc[C + 1];
-#pragma unroll
-            for (int c = 0; c < C; ++c) wc[c] = (al >= lo[c] && al < hi[c]) ? w : 0.0f;
-            wc[C] = 0.0f;
+            // cells that do not hold this atom are SKIPPED, not weighted by zero: 0 x NaN of a
+            // non-finite atom (a bad SFT) would spoil windows it is not part of
+            const u64 ww = pack2(w, w);
+            const u64 w2 = fmul2(ww, ww);
+            const float w2ab = w * w * ab;
 #pragma unroll
             for (int c = 0; c < C; ++c) {
-                const u64 ww = pack2(wc[c], wc[c]);
-                const u64 w2 = fmul2(ww, ww);
-                ffma2(acc.ab[c], w2, a2b2);
-                ffma2(acc.fa[c], ww, fa);
-                ffma2(acc.fb[c], ww, fb);
-            }
-            const u64 abab = pack2(ab, ab);
-#pragma unroll
-            for (int p = 0; p < (C + 1) / 2; ++p) {
-                const u64 ww = pack2(wc[2 * p], wc[2 * p + 1]);
-                ffma2(acc.cc[p], fmul2(ww, ww), abab);
+                if (al >= lo[c] && al < hi[c]) {
+                    ffma2(acc.ab[c], w2, a2b2);
+                    ffma2(acc.fa[c], ww, fa);
+                    ffma2(acc.fb[c], ww, fb);
+                    float c0, c1;
+                    unpack2(acc.cc[c / 2], c0, c1);
+                    if (c & 1) c1 += w2ab;
+                    else c0 += w2ab;
+                    acc.cc[c / 2] = pack2(c0, c1);
+                }
             }
         }
     }

@@ -243,7 +243,9 @@ __global__ void __launch_bounds__(NT)
                 A_max[q] = fmaxf(A_max[q], A);
                 // a window that lost most of its weight is re-summed (for all TPC templates:
                 // a fresh sum is always right)
-                fresh = fresh || (A * kGuard < A_max[q]);
+                // (written so that a NaN / inf atom in the running sums also forces a fresh
+                // sum: once it has left the window it must not linger)
+                fresh = fresh || !(A * kGuard >= A_max[q]);
             }
         }
         if (fresh) {

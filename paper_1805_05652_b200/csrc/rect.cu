@@ -84,6 +84,7 @@ __device__ __forceinline__ Sums64 prefix_diff_cg(const double2 *P, const int lo,
     s.fai = h2.x - l2.x;
     s.fbr = h2.y - l2.y;
     s.fbi = h3.x - l3.x;
+    if (h3.y - l3.y > 0.5) s.A = nan("");  // the window holds a non-finite atom: D <= 0 flag
     return s;
 }
 
@@ -103,7 +104,7 @@ __global__ void __launch_bounds__(kScanNT)
                      const int n_scan, const int steps_per_template)
 {
     __shared__ double s_off[8];
-    __shared__ double s_w[7][kScanNT / 32];
+    __shared__ double s_w[8][kScanNT / 32];
     pdl_trigger();
     pdl_wait();  // bounds_kernel: edge table and the zeroed scan flags
     const Bounds &bd = pr.bounds;
@@ -183,16 +184,30 @@ __global__ void __launch_bounds__(kScanNT)
     const int a0 = blk * kScanBlock + (int)threadIdx.x * kScanPer;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    float x[7][kScanPer];
+    // channel 7 counts the atoms that are not finite (a bad SFT): they enter the prefix as zeros
+    // plus a count, so that only the windows that hold one are spoiled (prefix_diff), not every
+    // window behind it
+    float x[8][kScanPer];
 #pragma unroll
     for (int ch = 0; ch < 7; ++ch)
 #pragma unroll
         for (int i = 0; i < kScanPer; ++i)
             x[ch][i] = (a0 + i < N) ? __ldg(base + ch * pr.ld + a0 + i) : 0.0f;
-
-    double incl[7], tsum[7];
 #pragma unroll
-    for (int ch = 0; ch < 7; ++ch) {
+    for (int i = 0; i < kScanPer; ++i) {
+        bool bad = false;
+#pragma unroll
+        for (int ch = 0; ch < 7; ++ch) bad = bad || !(fabsf(x[ch][i]) < INFINITY);
+        x[7][i] = bad ? 1.0f : 0.0f;
+        if (bad) {
+#pragma unroll
+            for (int ch = 0; ch < 7; ++ch) x[ch][i] = 0.0f;
+        }
+    }
+
+    double incl[8], tsum[8];
+#pragma unroll
+    for (int ch = 0; ch < 8; ++ch) {
         double t = 0.0;
 #pragma unroll
         for (int i = 0; i < kScanPer; ++i) t += (double)x[ch][i];
@@ -209,7 +224,7 @@ __global__ void __launch_bounds__(kScanNT)
     {
         // publish this block's totals before waiting for anyone
         if (threadIdx.x < 32) {
-            if (threadIdx.x < 7) {
+            if (threadIdx.x < 8) {
                 double t = 0.0;
 #pragma unroll
                 for (int w = 0; w < kScanNT / 32; ++w) t += s_w[threadIdx.x][w];
@@ -220,7 +235,7 @@ __global__ void __launch_bounds__(kScanNT)
             if (threadIdx.x == 0) st_release(ready + blockIdx.x, 1);
         }
         // offset of this block: warp ch sums the totals of blocks [0, blk) of this template
-        if (warp < 7) {
+        if (warp < 8) {
             // all lanes poll their flags together and the warp takes ONE acquire fence: a
             // wait_flag per lane would diverge and serialise up to 32 fences
             for (int b0 = 0; b0 < blk; b0 += 32) {
@@ -251,7 +266,7 @@ __global__ void __launch_bounds__(kScanNT)
         for (int ch = 0; ch < 8; ++ch) P[ch] = 0.0;
     }
 #pragma unroll
-    for (int ch = 0; ch < 7; ++ch) {
+    for (int ch = 0; ch < 8; ++ch) {
         double run = s_off[ch] + incl[ch] - tsum[ch];
         for (int w = 0; w < warp; ++w) run += s_w[ch][w];
 #pragma unroll
@@ -260,7 +275,6 @@ __global__ void __launch_bounds__(kScanNT)
             if (a0 + i < N) P[(int64_t)(a0 + i + 1) * 8 + ch] = run;
         }
     }
-    // pad lane of the 64-B entries stays unwritten: nothing uses it
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) st_release(done + blockIdx.x, 1);
@@ -282,6 +296,7 @@ __device__ __forceinline__ Sums64 prefix_diff(const double2 *__restrict__ P, con
     s.fai = h2.x - l2.x;
     s.fbr = h2.y - l2.y;
     s.fbi = h3.x - l3.x;
+    if (h3.y - l3.y > 0.5) s.A = nan("");  // the window holds a non-finite atom: D <= 0 flag
     return s;
 }
 
@@ -362,15 +377,25 @@ __global__ void __launch_bounds__(kSmallNT)
     const float *__restrict__ base = pr.atoms + (int64_t)tpl * pr.template_stride;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    for (int i = threadIdx.x; i < N; i += kSmallNT) s_t[i] = __ldg(pr.bounds.t + i);
-    // a2: exclusive fp64 prefix of channel `warp`, 32 atoms per step of a warp-wide scan
-    if (warp < 7) {
-        const float *__restrict__ row = base + warp * pr.ld;
+    uint8_t *s_bad = reinterpret_cast<uint8_t *>(s_t + N);  // [N]: atom is not finite (bad SFT)
+    for (int i = threadIdx.x; i < N; i += kSmallNT) {
+        s_t[i] = __ldg(pr.bounds.t + i);
+        bool bad = false;
+#pragma unroll
+        for (int ch = 0; ch < 7; ++ch) bad = bad || !(fabsf(__ldg(base + ch * pr.ld + i)) < INFINITY);
+        s_bad[i] = bad ? 1 : 0;
+    }
+    __syncthreads();
+    // a2: exclusive fp64 prefix of channel `warp`, 32 atoms per step of a warp-wide scan; bad
+    // atoms enter as zeros and are counted in channel 7, so that they only spoil their own windows
+    {
+        const float *__restrict__ row = base + min(warp, 6) * pr.ld;
         double carry = 0.0;
         if (lane == 0) s_P[warp] = 0.0;
         for (int i0 = 0; i0 < N; i0 += 32) {
             const int i = i0 + lane;
-            double v = i < N ? (double)__ldg(row + i) : 0.0;
+            double v = 0.0;
+            if (i < N) v = warp == 7 ? (double)s_bad[i] : s_bad[i] ? 0.0 : (double)__ldg(row + i);
 #pragma unroll
             for (int sh = 1; sh < 32; sh <<= 1) {
                 const double up = __shfl_up_sync(0xffffffffu, v, sh);
@@ -401,6 +426,7 @@ __global__ void __launch_bounds__(kSmallNT)
         s.fai = ph[4] - pl[4];
         s.fbr = ph[5] - pl[5];
         s.fbi = ph[6] - pl[6];
+        if (ph[7] - pl[7] > 0.5) s.A = nan("");  // the window holds a non-finite atom
         uint32_t fl;
         const float twoF = closure_2F(s, hi - lo, pr.min_atoms, fl);
         if (pr.out_maps) pr.out_maps[map_base + i] = twoF;
@@ -943,7 +969,7 @@ bool rect_small_applies(int32_t n_atoms, int32_t n_templates, int64_t cells)
 
 cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st)
 {
-    const size_t smem = (size_t)(pl.n_atoms + 1) * 64 + (size_t)pl.n_atoms * 4;
+    const size_t smem = (size_t)(pl.n_atoms + 1) * 64 + (size_t)pl.n_atoms * 5;
     cudaError_t e = cudaFuncSetAttribute(rect_small_kernel,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

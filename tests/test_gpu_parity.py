@@ -321,6 +321,49 @@ def test_amplitude_scaling_far_from_unity(pkg, scale):
                 f"scale {scale} general")
 
 
+def test_nan_and_inf_atoms_only_spoil_their_own_windows(pkg):
+    """A NaN atom and an inf atom (a bad SFT): every window that contains one is degenerate
+    (flag bit 1, 2F = 0, out of the marginals), every other window is untouched -- also in the
+    sliding form, where a bad atom that has LEFT the window must not linger in the running sums."""
+    grid = Grid(0, 1800, 60, 3600, 1800, 40)
+    wl = tiny_workload(240, 300, 0.0, grid)
+    atoms, t = wl.data.atoms[0].copy(), wl.data.t
+    atoms[:, 70] = np.nan
+    atoms[3, 150] = np.inf
+    for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN},
+                                 {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 7)}]),
+                        (RECT, [{"rect_method": 1}, {"rect_method": 2}])):
+        with np.errstate(invalid="ignore"):
+            ref = oracle.map2F(atoms, t, window, grid)
+        k = 3 if window == EXP else 1
+        t0 = grid.t0()[:, None]
+        tau = grid.tau()[None, :]
+        hit = np.zeros((grid.N_t0, grid.N_tau), bool)
+        for bad_t in (t[70], t[150]):
+            hit |= (bad_t >= t0) & (bad_t < t0 + k * tau)
+        assert hit.any() and (~hit).any()
+        assert np.all(ref["flags"][hit] & 2) and np.all(ref["flags"][~hit] == 0)
+        for kw in kws:
+            what = f"window {window} {kw}"
+            m, f = run_map(pkg, atoms, t, window, grid, **kw)
+            assert np.all(f[hit] & 2) and np.all(m[hit] == 0.0), what
+            assert np.all(f[~hit] == 0), what
+            err = np.abs(m[~hit] - ref["twoF"][~hit])
+            assert np.all(err <= TOL_2F * np.maximum(1.0, ref["twoF"][~hit])), what
+            res = pkg.tfstat_search(dev(atoms[None]), dev(t), window, grid, **kw).numpy()[0]
+            assert res["n_valid"] == int((~hit).sum()), what
+            assert np.isfinite(res["max2F"]) and np.isfinite(res["logB"]), what
+            assert abs(res["max2F"] - ref["twoF"][~hit].max()) <= TOL_2F * ref["twoF"][~hit].max()
+        mg, fg, rg = pkg.tfstat_map_general(dev(atoms), dev(t), window, (k, 1),
+                                            dev(grid.t0().astype(np.int32)),
+                                            dev(grid.tau().astype(np.int32)), want_flags=True)
+        mg, fg = mg.cpu().numpy(), fg.cpu().numpy()
+        assert np.all(fg[hit] & 2) and np.all(mg[hit] == 0.0) and np.all(fg[~hit] == 0)
+        assert np.all(np.abs(mg[~hit] - ref["twoF"][~hit]) <=
+                      TOL_2F * np.maximum(1.0, ref["twoF"][~hit]))
+        assert rg.numpy()[0]["n_valid"] == int((~hit).sum())
+
+
 def test_concurrent_streams_do_not_interfere(pkg):
     """The library keeps no state between calls: searches enqueued on two streams at once, each
     with its own workspace, give the bits of the same searches run one after the other."""
