@@ -33,7 +33,7 @@ WORKLOAD = "cfg4_search_4096x2880atoms_96x1417"
 # + 7 FFMA (A,B,C,Re/Im Fa,Re/Im Fb) on the FP32 pipe, + 1 MUFU.EX2 on the XU pipe
 FP32_OPS_PER_TERM = 9
 FP32_LANES_PER_CLK_SM = 128  # cc 10.0: 4 SMSPs x 32 FP32 lanes
-NCU_DRAM_BYTES_PER_TEMPLATE = 23.982848e6 / 296  # profiles/r01_pass4_kernels_full.md
+NCU_DRAM_BYTES_PER_TEMPLATE = 23.976704e6 / 296  # profiles/r01_pass4_kernels_full.md
 
 
 def read_peaks():
