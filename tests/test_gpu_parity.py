@@ -364,6 +364,30 @@ def test_nan_and_inf_atoms_only_spoil_their_own_windows(pkg):
         assert rg.numpy()[0]["n_valid"] == int((~hit).sum())
 
 
+@pytest.mark.parametrize("case", range(24))
+def test_marginalise_random_maps_with_ties(pkg, case):
+    """tfstat_marginalise on random maps quantised so that the maximum is attained many times
+    (the lowest flat index must win, exactly), with random flags, odd shapes (ragged tails,
+    unaligned sizes), huge dynamic range in F, and all-flagged maps."""
+    rng = np.random.default_rng(7000 + case)
+    N_t0, N_tau = int(rng.integers(1, 400)), int(rng.integers(1, 700))
+    levels = int(rng.choice([2, 5, 50, 100000]))
+    scale = float(rng.choice([1.0, 30.0, 2000.0]))
+    m = (rng.integers(0, levels, size=(N_t0, N_tau)) * (scale / levels)).astype(np.float32)
+    p_flag = float(rng.choice([0.0, 0.1, 0.9, 1.0]))
+    fl = (rng.random((N_t0, N_tau)) < p_flag).astype(np.uint8) * rng.integers(1, 4, (N_t0, N_tau)).astype(np.uint8)
+    for flags in (None, fl):
+        got = pkg.tfstat_marginalise(dev(m), None if flags is None else dev(flags)).numpy()[0]
+        ref = oracle.marginalise(m.astype(np.float64), flags)
+        assert got["n_valid"] == ref.n_valid
+        if ref.n_valid == 0:
+            assert (got["m"], got["n"], got["max2F"]) == (-1, -1, 0.0) and got["logB"] == -np.inf
+            continue
+        assert got["max2F"] == np.float32(ref.max2F)
+        assert (got["m"], got["n"]) == (ref.m, ref.n)  # exact ties: lowest flat index
+        assert abs(got["logB"] - ref.logB) <= 1e-4 * max(1.0, abs(ref.logB))
+
+
 def test_concurrent_streams_do_not_interfere(pkg):
     """The library keeps no state between calls: searches enqueued on two streams at once, each
     with its own workspace, give the bits of the same searches run one after the other."""
