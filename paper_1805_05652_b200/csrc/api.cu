@@ -127,11 +127,11 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         if (opts && opts->seg_len > 0) len = opts->seg_len < N_t0 ? opts->seg_len : N_t0;
         pl.seg_len = len;
         pl.n_segs = (N_t0 + len - 1) / len;
-        // templates per CTA (they share the weights): as many as still leave ~16 CTAs per SM
+        // templates per CTA (they share the weights): 2 while that still leaves ~16 CTAs per SM
+        // (measured on B200, config 4 x 2048: 1 -> 5.26 ms, 2 -> 4.57 ms, 4 -> 4.78 ms: at 4 the
+        // 162 registers cost more occupancy than the shared weights save; 4 only on request)
         const int64_t ctas1 = (int64_t)n_templates * pl.n_nblocks * pl.n_segs;
-        pl.slide_tpc = (n_templates >= 4 && ctas1 / 4 >= 148 * 16)   ? 4
-                       : (n_templates >= 2 && ctas1 / 2 >= 148 * 16) ? 2
-                                                                     : 1;
+        pl.slide_tpc = (n_templates >= 2 && ctas1 / 2 >= 148 * 16) ? 2 : 1;
         if (opts && opts->tile_c) {
             if (opts->tile_c != 1 && opts->tile_c != 2 && opts->tile_c != 4) return pl;
             pl.slide_tpc = opts->tile_c;
