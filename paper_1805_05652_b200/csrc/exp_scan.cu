@@ -97,8 +97,11 @@ __device__ __forceinline__ void acc_scale(SlideAcc &a, const float c)
 // TPC templates per CTA: the weights E_a depend on (atom, tau) only, not on the template, so one
 // MUFU.EX2 (+ the argument and E^2 multiplies) serves TPC templates; per (atom, template) the
 // initial window sum costs 2 LDS.128 + 4 multiply-adds + 3 / TPC instead of + 3.
+// Resident CTAs per SM asked of ptxas (measured on B200, config 4 x 2048 templates): one
+// template per CTA 5.26 ms unconstrained (96 registers), 5.09 at 5 CTAs, 4.85 at 6 (80 registers);
+// two templates 4.56 unconstrained (128 registers), 4.47 at 5 (96), 5.10 at 6 (spills).
 template <int NT, int KC, int TPC>
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, TPC == 1 ? (NT == 128 ? 6 : 1) : TPC == 2 ? (NT == 128 ? 5 : 1) : 1)
     exp_slide_kernel(const Problem pr, Partial *__restrict__ partials, const int n_nblocks,
                      const int n_segs, const int seg_len)
 {
