@@ -94,11 +94,13 @@ def time_map(atoms, t, window, grid, min_ms: float = 20.0, reps: int = 5) -> flo
     """Median over `reps` CUDA-event intervals, each spanning enough back-to-back calls to exceed
     `min_ms` (SURVEY.md 8(d) timing protocol); seconds per call."""
     out_map = torch.empty((grid.N_t0, grid.N_tau), dtype=torch.float32, device="cuda")
-    # the model is the paper's: the exponential window as the direct ("brute-force") sum
-    ws = torch.empty(B.workspace_bytes(window, int(t.shape[0]), 1, grid,
-                                       exp_method=B.EXP_DIRECT), dtype=torch.uint8, device="cuda")
+    # the model is the paper's: the exponential window as the direct ("brute-force") sum, and ONE
+    # code path per window (rect_method = 1: no one-launch small-map kernel, whose fixed cost is
+    # half that of the three-launch chain and would be booked on c_SFTs)
+    ws = torch.empty(B.workspace_bytes(window, int(t.shape[0]), 1, grid, exp_method=B.EXP_DIRECT,
+                                       rect_method=1), dtype=torch.uint8, device="cuda")
     fn = lambda: B.tfstat_map(atoms, t, window, grid, out_map=out_map, workspace=ws,  # noqa: E731
-                              exp_method=B.EXP_DIRECT)
+                              exp_method=B.EXP_DIRECT, rect_method=1)
     for _ in range(3):
         fn()
     torch.cuda.synchronize()
