@@ -80,10 +80,13 @@ typedef struct tfstat_opts {
     int32_t min_atoms;  /* cells with fewer atoms are degenerate; 0 or unset -> 2
                            ("at least 2 SFTs per F_mn")                      */
     int32_t exp_method; /* TFSTAT_EXP_*                                                    */
-    int32_t tile_c;     /* tuning: t0 cells per thread of the direct exp kernel (1,2,4,8);
-                           0 = chosen from the problem shape                               */
+    int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
+                           per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
+                           (1,2,4); tfstat_map_general: tau cells per thread (1,2,4); lattice
+                           rect kernel: 1 = one row per thread instead of two                */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
-    int32_t seg_len;    /* tuning (TFSTAT_EXP_SCAN): t0 steps per sliding segment; 0 = auto   */
+    int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice
+                           rect kernel: columns per CTA (rounded up to 16)                   */
     int32_t rect_method; /* rectangular window: 0 = auto; 1 = never the one-launch small-map
                            kernel (lattice / per-cell kernels only); 2 = the small-map kernel
                            whenever the atoms fit its shared memory (n_atoms <= 2048)          */
