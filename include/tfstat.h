@@ -83,7 +83,7 @@ typedef struct tfstat_opts {
     int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
                            per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
                            (1,2,4); tfstat_map_general: tau cells per thread (1,2,4); lattice
-                           rect kernel: 1 = one row per thread instead of two                */
+                           rect kernel: 1 / 2 = one / two rows per thread                    */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
     int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice
                            rect kernel: columns per CTA (rounded up to 16)                   */

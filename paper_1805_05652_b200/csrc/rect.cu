@@ -921,7 +921,10 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     // once for two rows.
     if (e_m > 0 && e_n > 0 && (2 * (int64_t)e_n) % e_m == 0 && q_override != 1) {
         const int64_t roff = 2 * (int64_t)e_n / e_m;
-        if (g.N_t0 >= 2 * roff) {
+        // ... if a warp still reads K in runs of 16 lattice points (roff >= 16): for dt0 = dtau
+        // (roff = 2) the lanes of a row pair touch every other pair of entries, and one row per
+        // thread is 8 % faster (one-year map at full resolution) although it loads K twice
+        if (g.N_t0 >= 2 * roff && (roff >= 16 || q_override == 2)) {
             rr.Q = 2;
             rr.r = (int32_t)roff;
         }
@@ -943,7 +946,13 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     const int seg_max = (g.N_tau + kChunk - 1) / kChunk * kChunk;
     int seg = seg_max;
     int64_t best_cost = INT64_MAX;
-    for (int cand = seg_max; cand >= kChunk; cand -= kChunk) {
+    // plenty of CTAs even with short column tiles: 64 columns (measured best of 32 .. whole rows
+    // on the one-year map at full resolution; short fp32 running sums besides)
+    const int seg_pref = std::min(seg_max, 64);
+    const bool plenty = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + seg_pref - 1) / seg_pref) >=
+                        (int64_t)148 * 8 * 16;
+    if (plenty) seg = seg_pref;
+    for (int cand = seg_max; !plenty && cand >= kChunk; cand -= kChunk) {
         const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
         const int64_t per_wave = 148 * (rr.Q == 2 ? 8 : 10);
         const int64_t waves = (ctas + per_wave - 1) / per_wave;
