@@ -545,8 +545,9 @@ __device__ __forceinline__ PairOut pair_closure(const u64 (&S)[8])
 
 // 16 warps per SM for Q = 2 (128 registers): measured on B200 against 12 (162 registers, no
 // spill), 20 (96) and 24 (80, spilling) warps per SM, which are 13 % to 58 % slower on config 5
+// (one row per thread: 8 CTAs per SM too -- 5 % faster than 10, 12 % faster than 12)
 template <int Q, bool MARG>
-__global__ void __launch_bounds__(kRunNT, Q == 2 ? 8 : 10)
+__global__ void __launch_bounds__(kRunNT, 8)
     rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
                     const ulonglong2 *__restrict__ K, Partial *__restrict__ partials,
                     const int roff, const int R, const int seg_cols, const int n_rowtiles,
@@ -954,7 +955,7 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     if (plenty) seg = seg_pref;
     for (int cand = seg_max; !plenty && cand >= kChunk; cand -= kChunk) {
         const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
-        const int64_t per_wave = 148 * (rr.Q == 2 ? 8 : 10);
+        const int64_t per_wave = 148 * 8;
         const int64_t waves = (ctas + per_wave - 1) / per_wave;
         const int64_t cost = waves * (cand + 24);
         if (cost < best_cost) {
