@@ -462,6 +462,7 @@ constexpr int kChunk = 16;   // columns between two write-outs of the transposed
 constexpr int kPitch = 16;   // floats per tile row; the four 16-byte column groups of row i are
                              // XOR-swizzled with (i >> 1) & 3: conflict-free STS.128 and LDS.128
 constexpr int kFPitch = 5;   // 32-bit words per flag-tile row (16 flag bytes + pad)
+constexpr int kKsMaxEntries = 320;  // 64 B each: at most 20 KB of K per CTA in shared memory
 constexpr float kCondFast = 1.0f / 64.0f;  // fp32 closure only if D > kCondFast * A * B
 constexpr float kTiny = 1.0e-30f;          // ... and D > kTiny
 constexpr float kHalfLog2e = 0.72134752044448170368f;
@@ -546,12 +547,18 @@ __device__ __forceinline__ PairOut pair_closure(const u64 (&S)[8])
 // 16 warps per SM for Q = 2 (128 registers): measured on B200 against 12 (162 registers, no
 // spill), 20 (96) and 24 (80, spilling) warps per SM, which are 13 % to 58 % slower on config 5
 // (one row per thread: 8 CTAs per SM too -- 5 % faster than 10, 12 % faster than 12)
-template <int Q, bool MARG>
+//
+// KS: the K entries a CTA walks (a run of ks_cap lattice points at most, see launch_run) are
+// copied to shared memory first.  A warp's LDG.128 of 32 consecutive 16-byte entries starts at
+// any multiple of 16 bytes, so each quarter-warp straddles two 128-byte lines and the load costs
+// 7 to 8 L1 wavefronts; the same LDS.128 costs 4.  ncu on the one-year map: L1 data-pipe
+// wavefronts 75 % of peak before, the limiter of this kernel.
+template <int Q, bool MARG, bool KS>
 __global__ void __launch_bounds__(kRunNT, 8)
     rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
                     const ulonglong2 *__restrict__ K, Partial *__restrict__ partials,
                     const int roff, const int R, const int seg_cols, const int n_rowtiles,
-                    const int n_coltiles, const int vec_ok)
+                    const int n_coltiles, const int vec_ok, const int ks_cap)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Marg s_red[32];
@@ -586,6 +593,24 @@ __global__ void __launch_bounds__(kRunNT, 8)
         reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
     const ulonglong2 *__restrict__ k_t = K + (int64_t)tpl * (bd.J + 1) * 4;
     const int k_plane = bd.J + 1;
+    // lattice points of this CTA: [jlo, jcap]; jcap = J (the zero entry) unless staged
+    int jlo = 0, jcap = bd.J;
+    ulonglong2 *ks = reinterpret_cast<ulonglong2 *>(
+        smem_raw + (size_t)nrows * (kPitch * 4 + 4 + (pr.out_flags ? kFPitch * 4 : 0)));
+    if (KS) {
+        int mb_lo = rowtile * kRunNT;
+        if (Q > 1) {
+            const int gpc = kRunNT / R, n_restiles = (roff + R - 1) / R;
+            mb_lo = (rowtile / n_restiles) * gpc * roff * Q + (rowtile % n_restiles) * R;
+        }
+        jlo = (int)min((int64_t)mb_lo * bd.e_m + (int64_t)n0 * bd.e_n, (int64_t)bd.J);
+        jcap = (int)min((int64_t)jlo + ks_cap - 1, (int64_t)bd.J);
+        const int ne = jcap - jlo + 1;
+        for (int i = lt; i < 4 * ne; i += kRunNT) {
+            const int pln = i / ne, j = i - pln * ne;
+            ks[pln * ks_cap + j] = __ldg(k_t + (int64_t)pln * k_plane + jlo + j);
+        }
+    }
 
     // ---- exact start of every row at columns n0, n0 + 1 -------------------------------------
     // Rows outside the grid carry a dummy, perfectly conditioned state so that they stay on
@@ -674,11 +699,18 @@ __global__ void __launch_bounds__(kRunNT, 8)
     u64 W[NS][8];
     // 32-bit lattice index (J <= 2^22); reads beyond the lattice are clamped to the zero entry J
     const int jstep = 2 * bd.e_n;
-    int jw = (int)min((int64_t)mbase * bd.e_m + (int64_t)n0 * bd.e_n, (int64_t)bd.J);
+    int jw = (int)min((int64_t)mbase * bd.e_m + (int64_t)n0 * bd.e_n, (int64_t)jcap);
+    if (KS) __syncthreads();
     auto load_k = [&](u64(&w)[8]) {
-        const ulonglong2 *__restrict__ e = k_t + jw;
-        const ulonglong2 q0 = __ldg(e), q1 = __ldg(e + k_plane), q2 = __ldg(e + 2 * k_plane),
-                         q3 = __ldg(e + 3 * k_plane);
+        ulonglong2 q0, q1, q2, q3;
+        if (KS) {
+            const ulonglong2 *e = ks + (jw - jlo);
+            q0 = e[0], q1 = e[ks_cap], q2 = e[2 * ks_cap], q3 = e[3 * ks_cap];
+        } else {
+            const ulonglong2 *__restrict__ e = k_t + jw;
+            q0 = __ldg(e), q1 = __ldg(e + k_plane), q2 = __ldg(e + 2 * k_plane),
+            q3 = __ldg(e + 3 * k_plane);
+        }
         w[0] = q0.x;
         w[1] = q0.y;
         w[2] = q1.x;
@@ -687,7 +719,7 @@ __global__ void __launch_bounds__(kRunNT, 8)
         w[5] = q2.y;
         w[6] = q3.x;
         w[7] = q3.y;
-        jw = min(jw + jstep, bd.J);
+        jw = min(jw + jstep, jcap);
     };
 #pragma unroll
     for (int k = 0; k < NS; ++k) load_k(W[k]);
@@ -823,7 +855,7 @@ __global__ void __launch_bounds__(kRunNT, 8)
                 if (off >= 0) __stcs(reinterpret_cast<float4 *>(dst + off), v);
             }
             __syncthreads();
-        } else if (want_map || want_flags) {
+        } else if ((want_map || want_flags) && vec_ok) {
             __syncthreads();
             const int q4 = threadIdx.x & 3;
             for (int row = threadIdx.x >> 2; row < nrows; row += kRunNT / 4) {
@@ -858,6 +890,29 @@ __global__ void __launch_bounds__(kRunNT, 8)
                 }
             }
             __syncthreads();
+        } else if (want_map || want_flags) {
+            // rows that are not 16-byte aligned (N_tau not a multiple of 4), ragged last chunk,
+            // flags: 16 lanes write the 16 columns of one row, so a warp stores two runs of
+            // 64 contiguous bytes (4 scalar stores per thread at a 16-byte stride cost four
+            // times the L1 wavefronts and L2 sectors: one-year map 985 us, now see DESIGN 6.3)
+            __syncthreads();
+            const int c = threadIdx.x & 15;
+            if (c < ncols) {
+                const int gsel = c >> 2, w = c & 3;
+#pragma unroll 4
+                for (int row = threadIdx.x >> 4; row < nrows; row += kRunNT / 16) {
+                    const int off = s_rowm[row];
+                    if (off < 0) continue;
+                    const int64_t o = map_base + off + n + c;
+                    if (want_map)
+                        __stcs(pr.out_maps + o,
+                               tile[(size_t)row * kPitch + 4 * (gsel ^ ((row >> 1) & 3)) + w]);
+                    if (want_flags)
+                        pr.out_flags[o] =
+                            (uint8_t)((ftile[row * kFPitch + gsel] >> (8 * w)) & 0xffu);
+                }
+            }
+            __syncthreads();
         }
     }
 
@@ -889,22 +944,19 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
                      ((reinterpret_cast<uintptr_t>(pr.out_maps) & 15u) == 0) &&
                      ((reinterpret_cast<uintptr_t>(pr.out_flags) & 3u) == 0);
     const int64_t n_ctas = (int64_t)rr.n_rowtiles * rr.n_coltiles * pl.n_templates;
-    cudaError_t e;
-    if (partials) {
-        e = cudaFuncSetAttribute(rect_run_kernel<Q, true>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const int ks_cap = rr.ks_cap;
+    const bool ks = ks_cap > 0;
+    const size_t smem_all = smem + (size_t)ks_cap * 64;
+    auto go = [&](auto kern) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)smem_all);
         if (e != cudaSuccess) return e;
-        return launch_pdl(rect_run_kernel<Q, true>, (unsigned)n_ctas, kRunNT, smem, st, pr, prefix,
-                          K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles,
-                          vec ? 1 : 0);
-    } else {
-        e = cudaFuncSetAttribute(rect_run_kernel<Q, false>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        return launch_pdl(rect_run_kernel<Q, false>, (unsigned)n_ctas, kRunNT, smem, st, pr,
-                          prefix, K, partials, rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles,
-                          rr.n_coltiles, vec ? 1 : 0);
-    }
+        return launch_pdl(kern, (unsigned)n_ctas, kRunNT, smem_all, st, pr, prefix, K, partials,
+                          rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles, vec ? 1 : 0,
+                          ks_cap);
+    };
+    if (partials) return ks ? go(rect_run_kernel<Q, true, true>) : go(rect_run_kernel<Q, true, false>);
+    return ks ? go(rect_run_kernel<Q, false, true>) : go(rect_run_kernel<Q, false, false>);
 }
 
 }  // namespace
@@ -947,12 +999,27 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     const int seg_max = (g.N_tau + kChunk - 1) / kChunk * kChunk;
     int seg = seg_max;
     int64_t best_cost = INT64_MAX;
-    // plenty of CTAs even with short column tiles: 64 columns (measured best of 32 .. whole rows
-    // on the one-year map at full resolution; short fp32 running sums besides)
-    const int seg_pref = std::min(seg_max, 64);
-    const bool plenty = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + seg_pref - 1) / seg_pref) >=
-                        (int64_t)148 * 8 * 16;
-    if (plenty) seg = seg_pref;
+    // lattice points one CTA walks: its rows' starting points plus the pair-steps of one row
+    // (the loads run NS ahead of their use; what lies beyond the run is never used)
+    auto ks_span = [&](const int sc) -> int64_t {
+        const int64_t row_span =
+            rr.Q == 1 ? kRunNT - 1 : (int64_t)(kRunNT / R - 1) * rr.r * rr.Q + R - 1;
+        return row_span * e_m + (int64_t)(2 * ((sc + 3) / 4) + rr.Q) * 2 * e_n + 1;
+    };
+    // plenty of CTAs even with short column tiles: the widest of 192, 128, 64 columns whose K
+    // run still fits in shared memory (one-year map at full resolution, K staged: 64 columns
+    // 646 us, 128 586 us, 192 570 us, 256 -- K from L1 again -- 657 us; short fp32 running sums
+    // besides)
+    bool plenty = false;
+    for (const int pref : {192, 128, 64}) {
+        const int sp = std::min(seg_max, pref);
+        if ((int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + sp - 1) / sp) < (int64_t)148 * 8 * 16)
+            continue;
+        if (pref > 64 && ks_span(sp) > kKsMaxEntries) continue;
+        plenty = true;
+        seg = sp;
+        break;
+    }
     for (int cand = seg_max; !plenty && cand >= kChunk; cand -= kChunk) {
         const int64_t ctas = (int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + cand - 1) / cand);
         const int64_t per_wave = 148 * 8;
@@ -967,6 +1034,7 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     if (seg_override > 0) seg = std::min(seg_max, (seg_override + kChunk - 1) / kChunk * kChunk);
     rr.seg_cols = seg;
     rr.n_coltiles = (g.N_tau + seg - 1) / seg;
+    rr.ks_cap = ks_span(seg) <= kKsMaxEntries ? (int32_t)ks_span(seg) : 0;
     return rr;
 }
 
