@@ -318,6 +318,29 @@ def side_workloads(torch, pkg, peaks):
         "cells": big.numel(), "ms": ms_b, "algorithmic_GBps": 4 * big.numel() / (ms_b * 1e-3) / 1e9,
         "hbm_frac": 4 * big.numel() / (ms_b * 1e-3) / 1e9 / peaks["hbm_gbs"],
         "l2": "1.23 GB per call > 126 MB L2, no flush"}
+    # rows a2-a4 at the same size: the rectangular map of one year of gapless SFTs at dt0 = dtau =
+    # T_SFT, written into the same 1.23 GB buffer; once with N_tau = 17519 (rows not 16-byte
+    # aligned: scalar coalesced write-out) and once with N_tau = 17516 (vector write-out)
+    from synth.atoms import Grid as SGrid, make_atoms
+    n_y = 17520
+    t_y = np.arange(n_y, dtype=np.int64) * 1800
+    at_y = torch.from_numpy(make_atoms(t_y, np.random.default_rng(11)).astype(np.float32)).cuda()
+    tt_y = torch.from_numpy(t_y.astype(np.int32)).cuda()
+    leg = {}
+    for n_tau in (n_y - 1, n_y - 4):
+        g_y = SGrid(0, 1800, n_y - 2, 3600, 1800, n_tau)
+        m_y = big.view(-1)[: g_y.n_cells].view(g_y.N_t0, g_y.N_tau)
+        ws_y = torch.empty(pkg.workspace_bytes(pkg.RECT, n_y, 1, g_y, rect_method=1),
+                           dtype=torch.uint8, device="cuda")
+        fn_y = lambda: pkg.tfstat_map(at_y, tt_y, pkg.RECT, g_y, out_map=m_y, workspace=ws_y,
+                                      rect_method=1)
+        for _ in range(3):
+            fn_y()
+        ms_y = time_calls(torch, fn_y, 10)
+        leg[f"N_tau_{n_tau}"] = {"cells": g_y.n_cells, "ms": ms_y,
+                                 "algorithmic_GBps": 4 * g_y.n_cells / (ms_y * 1e-3) / 1e9,
+                                 "hbm_frac": 4 * g_y.n_cells / (ms_y * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    out["rect_map_1yr_full_resolution"] = leg
     del big
     return out
 

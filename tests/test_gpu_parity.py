@@ -609,6 +609,43 @@ def test_config5_year_sampled(pkg, window):
     assert np.array_equal(f[-1] & 1, last["flags"] & 1)
 
 
+@pytest.mark.parametrize("n_tau", [17519, 17516])
+def test_one_year_full_resolution_rect_map_sampled(pkg, n_tau):
+    """The largest of the paper's setups (one year at dt0 = dtau = T_SFT,
+    3.07e8 cells, 1.23 GB), in the launch configuration bench.py's rect_map_1yr_full_resolution
+    leg times: one row per thread, K run in shared memory, 192-column tiles.  N_tau = 17519 leaves
+    the rows unaligned (coalesced scalar write-out), 17516 takes the vector write-out."""
+    from synth.atoms import Grid, make_atoms
+    rng = np.random.default_rng(2026)
+    t = np.arange(17520, dtype=np.int64) * 1800
+    t = t[rng.random(t.shape[0]) > 0.01]  # 1 % of the SFTs missing
+    atoms = make_atoms(t, rng).astype(np.float32)
+    t = t.astype(np.int32)
+    grid = Grid(0, 1800, 17518, 3600, 1800, n_tau)
+    a_d, t_d = dev(atoms[None]), dev(t)
+    m_d = torch.empty((grid.N_t0, grid.N_tau), dtype=torch.float32, device="cuda")
+    pkg.tfstat_map(a_d[0], t_d, RECT, grid, out_map=m_d, rect_method=1)
+    ms, ns = _sample_cells(grid, 60000, 17)
+    # the end of the data: the last rows, whose windows run out of atoms
+    ms[4:2004] = grid.N_t0 - 1 - (np.arange(2000) % 50)
+    mi, ni = torch.from_numpy(ms.astype(np.int64)).cuda(), torch.from_numpy(ns.astype(np.int64)).cuda()
+    got = m_d[mi, ni].cpu().numpy()
+    res = pkg.tfstat_search(a_d, t_d, RECT, grid, want_maps=True, want_flags=True, rect_method=1)
+    torch.cuda.synchronize()
+    # the flag-writing launch computes the same cells bit for bit
+    assert torch.equal(res.maps[0], m_d)
+    f = res.flags[0][mi, ni].cpu().numpy()
+    ref = oracle.cells(atoms, t, RECT, grid, ms, ns)
+    check_cells(got, f, ref, f"one-year rect N_tau={n_tau} sampled")
+    # fused marginals of the same launch against a GPU reduction of its own map
+    r0 = res.numpy()[0]
+    valid = res.flags[0] == 0
+    assert int(r0["n_valid"]) == int(valid.sum().item())
+    best = torch.where(valid, res.maps[0], torch.full_like(res.maps[0], -1.0)).max().item()
+    assert float(r0["max2F"]) == best
+    assert float(res.maps[0][int(r0["m"]), int(r0["n"])].item()) == best
+
+
 # ---------------------------------------------------------------------------------------
 # exact factorised / sliding exponential path (SURVEY.md 8(a) row a3', TFSTAT_EXP_SCAN):
 # the same oracle, the same tolerances
