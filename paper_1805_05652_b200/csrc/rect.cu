@@ -558,7 +558,7 @@ __global__ void __launch_bounds__(kRunNT, 8)
     rect_run_kernel(const Problem pr, const double *__restrict__ prefix,
                     const ulonglong2 *__restrict__ K, Partial *__restrict__ partials,
                     const int roff, const int R, const int seg_cols, const int n_rowtiles,
-                    const int n_coltiles, const int vec_ok, const int ks_cap)
+                    const int n_coltiles, const int vec_ok, const int ks_cap, const int ks_lg)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Marg s_red[32];
@@ -594,6 +594,15 @@ __global__ void __launch_bounds__(kRunNT, 8)
     const ulonglong2 *__restrict__ k_t = K + (int64_t)tpl * (bd.J + 1) * 4;
     const int k_plane = bd.J + 1;
     // lattice points of this CTA: [jlo, jcap]; jcap = J (the zero entry) unless staged
+    // Two rows per thread with roff = R = 2 or 4 (e_m = 1): the lanes of a warp read runs of R
+    // entries 2 R apart, a 2-way bank conflict.  ks_lg = log2 R >= 0 stores the run in two halves,
+    // the entries with an even (j / R) first: a warp is then on one half at every pair-step, on
+    // 32 consecutive entries.
+    const int ks_half = ks_cap >> 1;
+    auto ks_pos = [&](const int j) -> int {
+        if (ks_lg < 0) return j;
+        return ((j >> ks_lg) & 1) * ks_half + ((j >> (ks_lg + 1)) << ks_lg) + (j & ((1 << ks_lg) - 1));
+    };
     int jlo = 0, jcap = bd.J;
     ulonglong2 *ks = reinterpret_cast<ulonglong2 *>(
         smem_raw + (size_t)nrows * (kPitch * 4 + 4 + (pr.out_flags ? kFPitch * 4 : 0)));
@@ -608,7 +617,7 @@ __global__ void __launch_bounds__(kRunNT, 8)
         const int ne = jcap - jlo + 1;
         for (int i = lt; i < 4 * ne; i += kRunNT) {
             const int pln = i / ne, j = i - pln * ne;
-            ks[pln * ks_cap + j] = __ldg(k_t + (int64_t)pln * k_plane + jlo + j);
+            ks[pln * ks_cap + ks_pos(j)] = __ldg(k_t + (int64_t)pln * k_plane + jlo + j);
         }
     }
 
@@ -704,7 +713,7 @@ __global__ void __launch_bounds__(kRunNT, 8)
     auto load_k = [&](u64(&w)[8]) {
         ulonglong2 q0, q1, q2, q3;
         if (KS) {
-            const ulonglong2 *e = ks + (jw - jlo);
+            const ulonglong2 *e = ks + ks_pos(jw - jlo);
             q0 = e[0], q1 = e[ks_cap], q2 = e[2 * ks_cap], q3 = e[3 * ks_cap];
         } else {
             const ulonglong2 *__restrict__ e = k_t + jw;
@@ -953,7 +962,7 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
         if (e != cudaSuccess) return e;
         return launch_pdl(kern, (unsigned)n_ctas, kRunNT, smem_all, st, pr, prefix, K, partials,
                           rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles, vec ? 1 : 0,
-                          ks_cap);
+                          ks_cap, rr.ks_lg);
     };
     if (partials) return ks ? go(rect_run_kernel<Q, true, true>) : go(rect_run_kernel<Q, true, false>);
     return ks ? go(rect_run_kernel<Q, false, true>) : go(rect_run_kernel<Q, false, false>);
@@ -969,15 +978,20 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     rr.enabled = (J > 0 && g.N_t0 >= 8) ? 1 : 0;
     rr.Q = 1;
     rr.r = 1;
+    bool perm_ok = false;
     // Row m + roff, roff = 2 e_n / e_m, sits at column n on the lattice point that row m
     // reaches two columns (one pair-step) later: a thread that owns both loads every K entry
     // once for two rows.
     if (e_m > 0 && e_n > 0 && (2 * (int64_t)e_n) % e_m == 0 && q_override != 1) {
         const int64_t roff = 2 * (int64_t)e_n / e_m;
-        // ... if a warp still reads K in runs of 16 lattice points (roff >= 16): for dt0 = dtau
+        // ... if a warp still reads K in runs of 16 lattice points (roff >= 16).  For dt0 = dtau
         // (roff = 2) the lanes of a row pair touch every other pair of entries, and one row per
-        // thread is 8 % faster (one-year map at full resolution) although it loads K twice
-        if (g.N_t0 >= 2 * roff && (roff >= 16 || q_override == 2)) {
+        // thread is faster although it loads K twice -- also when the run is staged in shared
+        // memory in two conflict-free halves (ks_lg, used when two rows are forced for dtau =
+        // dt0 or 2 dt0): one-year map at full resolution 646 us against 561 us.
+        perm_ok = e_m == 1 && (roff == 2 || roff == 4);
+        const bool two = roff >= 16 || q_override == 2;
+        if (g.N_t0 >= 2 * roff && two) {
             rr.Q = 2;
             rr.r = (int32_t)roff;
         }
@@ -1010,12 +1024,14 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     // run still fits in shared memory (one-year map at full resolution, K staged: 64 columns
     // 646 us, 128 586 us, 192 570 us, 256 -- K from L1 again -- 657 us; short fp32 running sums
     // besides)
+    // 8 CTAs per SM: 64-byte entries beside the transposed tile (4 KB, two rows per thread 8 KB)
+    const int ks_max = rr.Q == 1 ? kKsMaxEntries : kKsMaxEntries - 32;
     bool plenty = false;
     for (const int pref : {192, 128, 64}) {
         const int sp = std::min(seg_max, pref);
         if ((int64_t)n_templates * rr.n_rowtiles * ((g.N_tau + sp - 1) / sp) < (int64_t)148 * 8 * 16)
             continue;
-        if (pref > 64 && ks_span(sp) > kKsMaxEntries) continue;
+        if (pref > 64 && ks_span(sp) > ks_max) continue;
         plenty = true;
         seg = sp;
         break;
@@ -1034,7 +1050,12 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     if (seg_override > 0) seg = std::min(seg_max, (seg_override + kChunk - 1) / kChunk * kChunk);
     rr.seg_cols = seg;
     rr.n_coltiles = (g.N_tau + seg - 1) / seg;
-    rr.ks_cap = ks_span(seg) <= kKsMaxEntries ? (int32_t)ks_span(seg) : 0;
+    rr.ks_cap = ks_span(seg) <= ks_max ? (int32_t)ks_span(seg) : 0;
+    rr.ks_lg = -1;
+    if (rr.ks_cap > 0 && rr.Q == 2 && perm_ok && R == rr.r) {
+        rr.ks_lg = R == 2 ? 1 : 2;
+        rr.ks_cap = 2 * R * ((rr.ks_cap - 1) / (2 * R) + 1);  // two halves, whole runs of R
+    }
     return rr;
 }
 

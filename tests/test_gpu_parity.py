@@ -219,7 +219,8 @@ def test_random_grids_all_kernel_families(pkg, case):
     atoms, t = wl.data.atoms[T - 1], wl.data.t
     for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN},
                                  {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 3)}]),
-                        (RECT, [{"rect_method": 1}, {"rect_method": 2}])):
+                        (RECT, [{"rect_method": 1}, {"rect_method": 2},
+                                  {"rect_method": 1, "tile": (2, 0, 0)}])):  # two rows per thread
         ref = oracle.map2F(atoms, t, window, grid, min_atoms=min_atoms)
         for kw in kws:
             what = f"case {case} window {window} {kw}"
