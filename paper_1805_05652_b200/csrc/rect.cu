@@ -96,8 +96,9 @@ constexpr int kDirectStep = 64;    // lattice steps of at most this many atoms a
 
 // P[tpl][i][ch], i = 0..n_atoms, ch = 0..7 (7 used): 64 B per entry.
 // K[tpl][q][j], q = 0..3, j = 0..J, 16 B per element (64 B per lattice point): the channel pairs (x of H[j], x of H[j + e_n]) for
-// x = A, B | C, -C | Re Fa, Im Fa | Re Fb, Im Fb (Fa, Fb scaled by sqrt 2); entry J is all zero
-// (out-of-range reads of the running kernel are clamped to it).
+// x = A, B | C, Re Fa | Im Fa, Re Fb | Im Fb, -C (Fa, Fb scaled by sqrt 2); entry J is all zero
+// (out-of-range reads of the running kernel are clamped to it).  -C comes last so that a running
+// kernel that reads K from global memory can leave it out (see load_k).
 __global__ void __launch_bounds__(kScanNT)
     rect_scan_kernel(const Problem pr, double *__restrict__ agg, int32_t *__restrict__ flags,
                      double *__restrict__ prefix, ulonglong2 *__restrict__ K, const int nblk,
@@ -162,9 +163,9 @@ __global__ void __launch_bounds__(kScanNT)
         // warp (consecutive rows = consecutive j) read consecutive 16-byte words
         const int64_t pl = (int64_t)bd.J + 1;
         float *__restrict__ kf = reinterpret_cast<float *>(K + (int64_t)tpl * 4 * pl);
-        const float v[8] = {(float)acc[0], (float)acc[1], (float)acc[2], (float)-acc[2],
+        const float v[8] = {(float)acc[0], (float)acc[1], (float)acc[2],
                             (float)(kSqrt2 * acc[3]), (float)(kSqrt2 * acc[4]),
-                            (float)(kSqrt2 * acc[5]), (float)(kSqrt2 * acc[6])};
+                            (float)(kSqrt2 * acc[5]), (float)(kSqrt2 * acc[6]), (float)-acc[2]};
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
             // channel c lives in plane c / 2, 8-byte pair c % 2 of the 16-byte element
@@ -509,7 +510,9 @@ struct RunMarg {
 // so eq. (7) for TWO cells is 13 packed fp32x2 operations and 2 MUFU.RCP:
 //   D = A B + (-C) C;  2|Fa|^2, 2|Fb|^2, 2 Re(Fa conj Fb);  num = B 2|Fa|^2 + A 2|Fb|^2
 //   + 2 (-C) 2Re;  2F = num / D.
-// -C is carried as a channel of its own because fma.rn.f32x2 has no operand negation.
+// -C is carried as a channel of its own because fma.rn.f32x2 has no operand negation
+// (recomputing -C = -1 x C after every step instead puts a multiply on the dependent chain and
+// measured 2-4 % slower on the one-year map).
 struct PairOut {
     u64 res;  // 2F of (column n, column n + 1), fp32 fast path
     u64 t;    // D - kCondFast A B of the two cells: the fast path holds where t > 0
@@ -718,16 +721,20 @@ __global__ void __launch_bounds__(kRunNT, 8)
         } else {
             const ulonglong2 *__restrict__ e = k_t + jw;
             q0 = __ldg(e), q1 = __ldg(e + k_plane), q2 = __ldg(e + 2 * k_plane),
-            q3 = __ldg(e + 3 * k_plane);
+            // 8 of the 16 bytes: the increment of -C is that of C with both sign bits flipped
+            // (two integer-pipe operations instead of 8 bytes through L1; config 5: 4-7 % faster.
+            // From shared memory the same trade measured 2 % slower, so KS loads all 64 bytes.)
+            q3.x = __ldg(reinterpret_cast<const u64 *>(e + 3 * k_plane));
+            q3.y = q1.x ^ 0x8000000080000000ull;
         }
         w[0] = q0.x;
         w[1] = q0.y;
         w[2] = q1.x;
-        w[3] = q1.y;
-        w[4] = q2.x;
-        w[5] = q2.y;
-        w[6] = q3.x;
-        w[7] = q3.y;
+        w[3] = q3.y;
+        w[4] = q1.y;
+        w[5] = q2.x;
+        w[6] = q2.y;
+        w[7] = q3.x;
         jw = min(jw + jstep, jcap);
     };
 #pragma unroll
