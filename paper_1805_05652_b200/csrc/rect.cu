@@ -915,6 +915,30 @@ __global__ void __launch_bounds__(kRunNT, 8)
             const int c = threadIdx.x & 15;
             if (c < ncols) {
                 const int gsel = c >> 2, w = c & 3;
+                if (want_map && !want_flags) {
+                    // the common case, kept short (ncu, one-year map with N_tau = 17519: the
+                    // generic loop below made this write-out 39 % of the kernel's instructions).
+                    // row = r0 + (kRunNT / 16) k: (row >> 1) & 3 takes two values in turn, so the
+                    // two swizzled words of a thread are fixed and the offsets stay 32-bit
+                    static_assert(kRunNT / 16 == 4, "swizzle period of the scalar write-out");
+                    const int r0 = threadIdx.x >> 4;
+                    const float *__restrict__ t0p =
+                        tile + (size_t)r0 * kPitch + 4 * (gsel ^ ((r0 >> 1) & 3)) + w;
+                    const float *__restrict__ t1p =
+                        tile + (size_t)(r0 + 4) * kPitch + 4 * (gsel ^ (((r0 >> 1) + 2) & 3)) + w;
+                    float *__restrict__ dstb = pr.out_maps + map_base + n + c;
+#pragma unroll 4
+                    for (int row = r0; row < nrows; row += 8) {
+                        const int off0 = s_rowm[row];
+                        const float v0 = t0p[(row - r0) * kPitch];
+                        if (off0 >= 0) __stcs(dstb + off0, v0);
+                        if (row + 4 < nrows) {
+                            const int off1 = s_rowm[row + 4];
+                            const float v1 = t1p[(row - r0) * kPitch];
+                            if (off1 >= 0) __stcs(dstb + off1, v1);
+                        }
+                    }
+                } else
 #pragma unroll 4
                 for (int row = threadIdx.x >> 4; row < nrows; row += kRunNT / 16) {
                     const int off = s_rowm[row];
