@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define TFSTAT_VERSION 100 /* 0.1.0 */
+#define TFSTAT_VERSION 200 /* 0.2.0: tfstat_opts starts with its own size; every call takes opts */
 
 /* window functions, eqs. (3), (4) */
 #define TFSTAT_WINDOW_RECT 0 /* w = 1 on [t0, t0 + tau)                          */
@@ -58,7 +58,8 @@ extern "C" {
 
 typedef enum tfstat_status {
     TFSTAT_OK = 0,
-    TFSTAT_EINVAL = -1,     /* null required pointer, n_atoms < 1, N_t0 < 1, N_tau < 1,
+    TFSTAT_EINVAL = -1,     /* null required pointer, n_atoms < 1, N_t0 < 1, N_tau < 1, opts with
+                               struct_size < 8 or reserved fields set,
                                tau_min < 1, dt0 < 1 with N_t0 > 1, dtau < 1 with N_tau > 1,
                                ld < n_atoms, unknown window/method, N_t0*N_tau >= 2^31      */
     TFSTAT_EWORKSPACE = -2, /* workspace NULL or smaller than tfstat_workspace_bytes()     */
@@ -75,27 +76,72 @@ typedef struct tfstat_result {
     int32_t n_valid; /* number of non-degenerate cells                                     */
 } tfstat_result;
 
-/* Options; a HOST pointer in every call, NULL = defaults. */
+/* Options; a HOST pointer, the last argument of every call, NULL = defaults.
+ *
+ * The first field is the size of the struct THE CALLER was compiled against, so the struct can
+ * grow at its end without breaking old callers: the library reads min(struct_size,
+ * sizeof(tfstat_opts)) bytes and takes defaults (zeros) for the rest.  Initialise with
+ * TFSTAT_OPTS_INIT (or memset to 0 and set struct_size = sizeof(tfstat_opts)); a non-NULL opts
+ * with struct_size < 8 is TFSTAT_EINVAL.  The only CONVENTION of the method in here is min_atoms
+ * (SURVEY.md 8(b)); everything after it selects or tunes kernels and never changes what is
+ * computed beyond the rounding order. */
 typedef struct tfstat_opts {
+    uint32_t struct_size; /* = sizeof(tfstat_opts)                                          */
     int32_t min_atoms;  /* cells with fewer atoms are degenerate; 0 or unset -> 2
                            ("at least 2 SFTs per F_mn")                      */
     int32_t exp_method; /* TFSTAT_EXP_*                                                    */
-    int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
-                           per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
-                           (1,2,4); tfstat_map_general: tau cells per thread (1,2,4); lattice
-                           rect kernel: 1 / 2 = one / two rows per thread                    */
-    int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
-    int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice
-                           rect kernel: columns per CTA (rounded up to 16)                   */
     int32_t rect_method; /* rectangular window: 0 = auto; 1 = never the one-launch small-map
                            kernel (lattice / per-cell kernels only); 2 = the small-map kernel
                            whenever the atoms fit its shared memory (n_atoms <= 2048)          */
+    int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
+                           per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
+                           (1,2,4); tfstat_map_general: tau cells per thread (1,2,4); lattice
+                           rect kernel: rows per thread (1, 2, 4)                             */
+    int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
+    int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice
+                           rect kernel: columns per CTA (rounded up to 16)                   */
+    int32_t reserved0;  /* must be 0 */
     /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
      * immediately before and after the dominant kernel of the call (the window-sum +
      * closure kernel; for the rectangular window: prefix + cells kernels).  NULL = off. */
     void *ev_main_begin;
     void *ev_main_end;
+    /* Optional work counters: DEVICE pointer to TFSTAT_N_STATS uint64, or NULL.  The kernels ADD
+     * what they executed (the caller zeroes them): see TFSTAT_STAT_*.  Counting costs a few
+     * per cent; it is meant for bench.py's roofline, not for production calls. */
+    uint64_t *stats;
 } tfstat_opts;
+#define TFSTAT_OPTS_INIT {(uint32_t)sizeof(tfstat_opts), 0, 0, 0, 0, 0, 0, 0, NULL, NULL, NULL}
+
+/* tfstat_opts.stats[i]: weighted (atom, cell-or-window, template) terms executed by the
+ * exponential-window kernels, i.e. one weight applied to the 7 channels of one atom */
+#define TFSTAT_STAT_TERMS_WINDOW 0 /* initial / direct window sums                           */
+#define TFSTAT_STAT_TERMS_ENTER 1  /* sliding form: atoms entering at the low end            */
+#define TFSTAT_STAT_TERMS_LEAVE 2  /* sliding form: atoms leaving at the high end            */
+#define TFSTAT_STAT_TERMS_RESUM 3  /* sliding form: windows summed afresh (guard, no overlap) */
+#define TFSTAT_STAT_CELLS 4        /* cells closed (eq. 7 evaluated)                          */
+#define TFSTAT_STAT_REDO64 5       /* cells re-summed in fp64 (short ill-conditioned windows) */
+#define TFSTAT_N_STATS 8
+
+/* What the library will run for a problem shape (host-only; tfstat_plan_info()).  bench.py reads
+ * its roofline's executed instruction mix from here instead of re-deriving the plan. */
+#define TFSTAT_KERNEL_EXP_DIRECT 1
+#define TFSTAT_KERNEL_EXP_SLIDE 2
+#define TFSTAT_KERNEL_RECT_SMALL 3
+#define TFSTAT_KERNEL_RECT_RUN 4   /* lattice running-sum kernel                              */
+#define TFSTAT_KERNEL_RECT_CELLS 5 /* per-cell prefix differences (no lattice / few rows)     */
+typedef struct tfstat_plan {
+    uint32_t struct_size; /* in: sizeof(tfstat_plan) of the caller                           */
+    int32_t kernel;       /* TFSTAT_KERNEL_* of the dominant kernel                          */
+    int32_t tile_c;       /* cells (exp direct) / templates (slide) / rows (rect) per thread */
+    int32_t tile_nt;      /* threads per CTA of the dominant kernel                          */
+    int32_t seg_len;      /* slide: t0 steps per segment; rect run: columns per CTA          */
+    int32_t n_segs;       /* slide: segments per (template, tau block); rect: column tiles   */
+    int32_t n_launches;   /* kernels one tfstat_search call enqueues (results requested)     */
+    int32_t lattice_J;    /* entries of the window-end lattice (0: per-cell binary search)   */
+    int64_t n_ctas;       /* CTAs of the dominant kernel                                     */
+    uint64_t workspace_bytes;
+} tfstat_plan;
 
 /* ---- host-only helpers (no CUDA calls) ------------------------------------------------ */
 int tfstat_version(void);
@@ -105,6 +151,11 @@ const char *tfstat_strerror(int status);
 size_t tfstat_workspace_bytes(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
                               int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
                               int32_t N_tau, const tfstat_opts *opts_host);
+/* Fills *info (struct_size set by the caller) for this problem shape.  0 or TFSTAT_EINVAL /
+ * TFSTAT_EOVERFLOW exactly as tfstat_search would return them. */
+int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
+                     int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau, int32_t N_tau,
+                     const tfstat_opts *opts_host, tfstat_plan *info);
 /* cudaError_t of the last failing CUDA call made by this thread inside the library. */
 int tfstat_last_cuda_error(void);
 
@@ -122,11 +173,12 @@ int tfstat_map(const float *atoms, int64_t ld, const int32_t *t_atoms, int32_t n
 
 /* Marginalise a map already in device memory: max 2F + argmax, logB, n_valid.
  *   flags nullable (NULL: every cell valid).  out: one tfstat_result on the device.
- *   workspace: >= tfstat_marginalise_workspace_bytes(N_t0, N_tau) bytes.                   */
+ *   workspace: >= tfstat_marginalise_workspace_bytes(N_t0, N_tau) bytes, 16-byte aligned
+ *   (TFSTAT_EWORKSPACE otherwise).  opts_host: nothing in it applies yet (reserved).       */
 size_t tfstat_marginalise_workspace_bytes(int32_t N_t0, int32_t N_tau);
 int tfstat_marginalise(const float *map, const uint8_t *flags, int32_t N_t0, int32_t N_tau,
                        tfstat_result *out, void *workspace, size_t workspace_bytes,
-                       void *stream);
+                       void *stream, const tfstat_opts *opts_host);
 
 /* Batched search over n_templates independent atom sets that share timestamps and grid;
  * map evaluation, cell closure and marginalisation fused, so only n_templates results reach
@@ -149,7 +201,15 @@ int tfstat_search(const float *atoms, int64_t template_stride, int64_t ld,
 int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int32_t t0_min,
                        int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
                        int32_t N_tau, int64_t *out_terms, void *workspace,
-                       size_t workspace_bytes, void *stream);
+                       size_t workspace_bytes, void *stream, const tfstat_opts *opts_host);
+
+/* Opt-in check of the precondition "t_atoms strictly increasing" (gaps are fine, PAPER.md:90;
+ * unsorted or duplicate time stamps are not: every kernel finds its windows by binary search).
+ * The data lives on the device, so the answer does too:
+ *   *out_first_bad (DEVICE int32) = smallest i >= 1 with t_atoms[i] <= t_atoms[i-1], or -1.
+ * Errors: TFSTAT_EINVAL (null pointer, n_atoms < 1). */
+int tfstat_validate_timestamps(const int32_t *t_atoms, int32_t n_atoms, int32_t *out_first_bad,
+                               void *stream, const tfstat_opts *opts_host);
 
 /* ---- general windows on explicit grids ------------------------------------------------ */
 
@@ -205,7 +265,8 @@ int tfstat_merge_detectors(const float *const *atoms_dets, const int64_t *templa
                            const int64_t *lds, const int32_t *const *t_dets,
                            const int32_t *n_atoms_dets, int32_t n_det, int32_t n_templates,
                            const int32_t *t_out, int32_t n_out, float *out_atoms,
-                           int64_t template_stride_out, int64_t ld_out, void *stream);
+                           int64_t template_stride_out, int64_t ld_out, void *stream,
+                           const tfstat_opts *opts_host);
 
 /* ---- end-to-end entry point with HOST buffers ----------------------------------------- */
 

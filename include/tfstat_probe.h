@@ -1,5 +1,6 @@
 /*
- * tfstat_probe.h -- ALU-roofline probe shipped with libtfstat (not part of the paper's calls).
+ * tfstat_probe.h -- ALU-roofline probe: libtfstat_probe.so, a bench-only library built beside
+ * libtfstat.so (not part of the product library, not part of the paper's calls).
  *
  * The exponential-window direct sum is bound by the FP32 and XU (MUFU) pipes, not by HBM or
  * tensor cores.  MEASURED_PEAKS.json holds only HBM and bf16 numbers, so

@@ -18,6 +18,8 @@ from .binding import (  # noqa: F401
     count_terms,
     lib_path,
     load_library,
+    load_probe_library,
+    plan_info,
     probe_alu,
     search_host_scratch_bytes,
     tfstat_map,
@@ -26,6 +28,7 @@ from .binding import (  # noqa: F401
     tfstat_merge_detectors,
     tfstat_search,
     tfstat_search_host,
+    validate_timestamps,
     workspace_bytes,
 )
 from .shard import gather_results, template_shard  # noqa: F401,E402

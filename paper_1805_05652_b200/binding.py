@@ -18,7 +18,12 @@ EXP_AUTO, EXP_DIRECT, EXP_SCAN = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libtfstat.so")
+_PROBE_LIB_PATH = os.path.join(_HERE, "libtfstat_probe.so")
 _lib = None
+_probe_lib = None
+N_STATS = 8  # TFSTAT_N_STATS
+STAT_NAMES = ("terms_window", "terms_enter", "terms_leave", "terms_resum", "cells", "redo64")
+KERNEL_NAMES = {1: "exp_direct", 2: "exp_slide", 3: "rect_small", 4: "rect_run", 5: "rect_cells"}
 
 # tfstat_result, 20 bytes (include/tfstat.h)
 RESULT_DTYPE = np.dtype([("max2F", "<f4"), ("m", "<i4"), ("n", "<i4"), ("logB", "<f4"),
@@ -30,10 +35,23 @@ class TfstatError(RuntimeError):
 
 
 class _Opts(C.Structure):
-    _fields_ = [("min_atoms", C.c_int32), ("exp_method", C.c_int32),
-                ("tile_c", C.c_int32), ("tile_nt", C.c_int32), ("seg_len", C.c_int32),
-                ("rect_method", C.c_int32), ("ev_main_begin", C.c_void_p),
-                ("ev_main_end", C.c_void_p)]
+    """tfstat_opts (include/tfstat.h); struct_size is filled in by __init__."""
+    _fields_ = [("struct_size", C.c_uint32), ("min_atoms", C.c_int32), ("exp_method", C.c_int32),
+                ("rect_method", C.c_int32), ("tile_c", C.c_int32), ("tile_nt", C.c_int32),
+                ("seg_len", C.c_int32), ("reserved0", C.c_int32), ("ev_main_begin", C.c_void_p),
+                ("ev_main_end", C.c_void_p), ("stats", C.c_void_p)]
+
+    def __init__(self, *a, **k):
+        super().__init__(*a, **k)
+        self.struct_size = C.sizeof(_Opts)
+
+
+class _Plan(C.Structure):
+    """tfstat_plan (include/tfstat.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("kernel", C.c_int32), ("tile_c", C.c_int32),
+                ("tile_nt", C.c_int32), ("seg_len", C.c_int32), ("n_segs", C.c_int32),
+                ("n_launches", C.c_int32), ("lattice_J", C.c_int32), ("n_ctas", C.c_int64),
+                ("workspace_bytes", C.c_uint64)]
 
 
 class _Window(C.Structure):
@@ -67,10 +85,12 @@ def load_library():
     lib.tfstat_map.argtypes = [vp, i64, vp, i32, C.c_int] + grid + [vp, vp, vp, sz, vp, op]
     lib.tfstat_marginalise_workspace_bytes.restype = sz
     lib.tfstat_marginalise_workspace_bytes.argtypes = [i32, i32]
-    lib.tfstat_marginalise.argtypes = [vp, vp, i32, i32, vp, vp, sz, vp]
+    lib.tfstat_marginalise.argtypes = [vp, vp, i32, i32, vp, vp, sz, vp, op]
+    lib.tfstat_plan_info.argtypes = [C.c_int, i32, i32] + grid + [op, C.POINTER(_Plan)]
+    lib.tfstat_validate_timestamps.argtypes = [vp, i32, vp, vp, op]
     lib.tfstat_search.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
         vp, vp, vp, vp, sz, vp, op]
-    lib.tfstat_count_terms.argtypes = [vp, i32, C.c_int] + grid + [vp, vp, sz, vp]
+    lib.tfstat_count_terms.argtypes = [vp, i32, C.c_int] + grid + [vp, vp, sz, vp, op]
     lib.tfstat_search_host.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
         vp, vp, vp, sz, op]
     lib.tfstat_search_host_scratch_bytes.restype = sz
@@ -79,10 +99,23 @@ def load_library():
     lib.tfstat_general_workspace_bytes.argtypes = [i32, i32]
     lib.tfstat_map_general.argtypes = [vp, i64, vp, i32, C.POINTER(_Window), vp, i32, vp, i32,
                                        vp, vp, vp, vp, sz, vp, op]
-    lib.tfstat_merge_detectors.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, i32, vp, i64, i64, vp]
+    lib.tfstat_merge_detectors.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, i32, vp, i64, i64, vp,
+                                           op]
+    _lib = lib
+    return lib
+
+
+def load_probe_library():
+    """dlopen libtfstat_probe.so, the bench-only ALU micro-benchmarks (include/tfstat_probe.h)."""
+    global _probe_lib
+    if _probe_lib is not None:
+        return _probe_lib
+    if not os.path.exists(_PROBE_LIB_PATH):
+        raise TfstatError(f"{_PROBE_LIB_PATH} is missing: `python -m paper_1805_05652_b200.build`")
+    lib = C.CDLL(_PROBE_LIB_PATH)
     lib.tfstat_probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
-    _lib = lib
+    _probe_lib = lib
     return lib
 
 
@@ -98,8 +131,14 @@ def _grid_args(g):
     return [int(g.t0_min), int(g.dt0), int(g.N_t0), int(g.tau_min), int(g.dtau), int(g.N_tau)]
 
 
-def _opts(min_atoms: int, exp_method: int, events=None, tile=None, rect_method: int = 0) -> _Opts:
+def _opts(min_atoms: int, exp_method: int, events=None, tile=None, rect_method: int = 0,
+          stats: Optional[torch.Tensor] = None) -> _Opts:
     o = _Opts()
+    if stats is not None:  # CUDA int64 tensor of N_STATS counters the kernels add to
+        if not (stats.is_cuda and stats.dtype == torch.int64 and stats.numel() >= N_STATS
+                and stats.is_contiguous()):
+            raise TfstatError("stats must be a contiguous CUDA int64 tensor of N_STATS entries")
+        o.stats = stats.data_ptr()
     o.min_atoms = int(min_atoms)
     o.exp_method = int(exp_method)
     o.rect_method = int(rect_method)
@@ -140,6 +179,34 @@ def workspace_bytes(window: int, n_atoms: int, n_templates: int, grid, *, min_at
     if n == 0:
         raise TfstatError("tfstat_workspace_bytes: invalid problem shape")
     return int(n)
+
+
+def plan_info(window: int, n_atoms: int, n_templates: int, grid, *, min_atoms: int = 2,
+              exp_method: int = EXP_AUTO, tile=None, rect_method: int = 0) -> dict:
+    """What the library will run for this problem shape (tfstat_plan_info): the dominant kernel,
+    its tile, its CTAs, the launches of one search and the workspace."""
+    lib = load_library()
+    o = _opts(min_atoms, exp_method, tile=tile, rect_method=rect_method)
+    p = _Plan()
+    p.struct_size = C.sizeof(_Plan)
+    rc = lib.tfstat_plan_info(window, n_atoms, n_templates, *_grid_args(grid), C.byref(o),
+                              C.byref(p))
+    _check(rc, "tfstat_plan_info")
+    d = {k: int(getattr(p, k)) for k, _ in _Plan._fields_ if k != "struct_size"}
+    d["kernel_name"] = KERNEL_NAMES.get(d["kernel"], "?")
+    return d
+
+
+def validate_timestamps(t_atoms: torch.Tensor, *, stream=None) -> int:
+    """Opt-in check of the precondition: index of the first time stamp that is not greater than
+    its predecessor, or -1 if t_atoms is strictly increasing (tfstat_validate_timestamps)."""
+    lib = load_library()
+    _dev_i32(t_atoms, "t_atoms")
+    out = torch.empty(1, dtype=torch.int32, device=t_atoms.device)
+    rc = lib.tfstat_validate_timestamps(t_atoms.data_ptr(), int(t_atoms.shape[0]), out.data_ptr(),
+                                        _stream_ptr(stream), None)
+    _check(rc, "tfstat_validate_timestamps")
+    return int(out.item())
 
 
 def _workspace(nbytes: int, device, workspace: Optional[torch.Tensor]) -> torch.Tensor:
@@ -215,7 +282,7 @@ def tfstat_marginalise(map2F: torch.Tensor, flags: Optional[torch.Tensor] = None
     out = torch.empty((1, 5), dtype=torch.int32, device=map2F.device)
     rc = lib.tfstat_marginalise(map2F.data_ptr(), flags.data_ptr() if flags is not None else None,
                                 N_t0, N_tau, out.data_ptr(), ws.data_ptr(), nbytes,
-                                _stream_ptr(stream))
+                                _stream_ptr(stream), None)
     _check(rc, "tfstat_marginalise")
     return Results(out)
 
@@ -224,7 +291,8 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
                   min_atoms: int = 2, exp_method: int = EXP_AUTO, want_maps: bool = False,
                   want_flags: bool = False, workspace: Optional[torch.Tensor] = None,
                   out: Optional[torch.Tensor] = None, stream=None,
-                  main_kernel_events=None, tile=None, rect_method: int = 0) -> Results:
+                  main_kernel_events=None, tile=None, rect_method: int = 0,
+                  stats: Optional[torch.Tensor] = None) -> Results:
     """atoms [T, 7, N] -> marginals of the T maps (and the maps / flags if asked)."""
     lib = load_library()
     _dev_f32(atoms, "atoms")
@@ -245,7 +313,8 @@ def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid,
     nbytes = workspace_bytes(window, n_atoms, T, grid, min_atoms=min_atoms, exp_method=exp_method,
                              tile=tile, rect_method=rect_method)
     ws = _workspace(nbytes, dev, workspace)
-    o = _opts(min_atoms, exp_method, main_kernel_events, tile=tile, rect_method=rect_method)
+    o = _opts(min_atoms, exp_method, main_kernel_events, tile=tile, rect_method=rect_method,
+              stats=stats)
     rc = lib.tfstat_search(atoms.data_ptr(), tstride, ld, t_atoms.data_ptr(), n_atoms, T, window,
                            *_grid_args(grid), out.data_ptr(),
                            maps.data_ptr() if maps is not None else None,
@@ -330,7 +399,7 @@ def tfstat_merge_detectors(atoms_dets, t_dets, t_out: torch.Tensor, *, stream=No
     lds = (C.c_int64 * n_det)(*[int(a.stride(1)) for a in A])
     ns = (C.c_int32 * n_det)(*[int(t.shape[0]) for t in t_dets])
     rc = lib.tfstat_merge_detectors(pa, ts, lds, pt, ns, n_det, T, t_out.data_ptr(), n_out,
-                                    out.data_ptr(), 7 * n_out, n_out, _stream_ptr(stream))
+                                    out.data_ptr(), 7 * n_out, n_out, _stream_ptr(stream), None)
     _check(rc, "tfstat_merge_detectors")
     return out[0] if squeeze else out
 
@@ -344,7 +413,7 @@ def count_terms(t_atoms: torch.Tensor, window: int, grid, *, stream=None) -> int
     ws = torch.empty(nbytes, dtype=torch.uint8, device=t_atoms.device)
     out = torch.zeros(1, dtype=torch.int64, device=t_atoms.device)
     rc = lib.tfstat_count_terms(t_atoms.data_ptr(), n_atoms, window, *_grid_args(grid),
-                                out.data_ptr(), ws.data_ptr(), nbytes, _stream_ptr(stream))
+                                out.data_ptr(), ws.data_ptr(), nbytes, _stream_ptr(stream), None)
     _check(rc, "tfstat_count_terms")
     return int(out.item())
 
@@ -426,9 +495,11 @@ PROBE_KINDS = {"ffma": 0, "fadd": 1, "mufu_ex2": 2, "ffma2": 3, "fadd2": 4, "ffm
 
 
 def probe_alu(kind: str, reps: int = 3) -> dict:
-    """Measured issue rate of one instruction class on the current GPU (tfstat_probe.h)."""
-    lib = load_library()
+    """Measured issue rate of one instruction class on the current GPU (tfstat_probe.h; the
+    bench-only libtfstat_probe.so)."""
+    lib = load_probe_library()
     a, b, c = C.c_double(0), C.c_double(0), C.c_double(0)
     rc = lib.tfstat_probe_alu(PROBE_KINDS[kind], reps, C.byref(a), C.byref(b), C.byref(c))
-    _check(rc, f"tfstat_probe_alu({kind})")
+    if rc != 0:
+        raise TfstatError(f"tfstat_probe_alu({kind}): status {rc}")
     return dict(kind=kind, lane_ops_per_s=a.value, ops_per_clk_sm=b.value, sm_mhz=c.value)

@@ -1,4 +1,5 @@
-"""Build libtfstat.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+"""Build libtfstat.so (the product) and libtfstat_probe.so (bench-only ALU micro-benchmarks,
+include/tfstat_probe.h) in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_1805_05652_b200.build [--force] [--verbose]
 
@@ -17,8 +18,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtfstat.so")
-SOURCES = ["api.cu", "bounds.cu", "exp_direct.cu", "exp_scan.cu", "rect.cu", "general.cu", "merge.cu", "marginalise.cu",
-           "probe.cu"]
+PROBE_LIB = os.path.join(HERE, "libtfstat_probe.so")
+SOURCES = ["api.cu", "bounds.cu", "exp_direct.cu", "exp_scan.cu", "rect.cu", "general.cu", "merge.cu", "marginalise.cu"]
+PROBE_SOURCES = ["probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC,-Wall", "-Xptxas", "-v"]
 
@@ -44,7 +46,7 @@ def _digest() -> str:
 def build(force: bool = False, verbose: bool = False) -> str:
     stamp = os.path.join(OBJ, "stamp")
     dig = _digest()
-    if not force and os.path.exists(LIB) and os.path.exists(stamp):
+    if not force and os.path.exists(LIB) and os.path.exists(PROBE_LIB) and os.path.exists(stamp):
         with open(stamp) as f:
             if f.read().strip() == dig:
                 return LIB
@@ -63,14 +65,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
             print(r.stderr, file=sys.stderr)
         return obj
 
-    with cf.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(compile_one, SOURCES))
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc, "-shared", "-o", tmp, *objs, "-gencode", "arch=compute_100a,code=sm_100a"]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
-    os.replace(tmp, LIB)
+    with cf.ThreadPoolExecutor(max_workers=len(SOURCES) + len(PROBE_SOURCES)) as ex:
+        objs = list(ex.map(compile_one, SOURCES + PROBE_SOURCES))
+    for lib, lib_objs in ((LIB, objs[:len(SOURCES)]), (PROBE_LIB, objs[len(SOURCES):])):
+        tmp = lib + f".tmp{os.getpid()}"
+        cmd = [nvcc, "-shared", "-o", tmp, *lib_objs, "-gencode", "arch=compute_100a,code=sm_100a"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+        os.replace(tmp, lib)
     with open(stamp, "w") as f:
         f.write(dig)
     return LIB

@@ -22,6 +22,27 @@ static int cuda_fail(cudaError_t e)
         if (e__ != cudaSuccess) return cuda_fail(e__);  \
     } while (0)
 
+// tfstat_opts as the caller sees it -> the library's own, complete copy: min(struct_size,
+// sizeof) bytes are the caller's, the rest defaults (include/tfstat.h)
+struct OptsIn {
+    tfstat_opts o;
+    bool ok;
+    explicit OptsIn(const tfstat_opts *in)
+    {
+        std::memset(&o, 0, sizeof(o));
+        o.struct_size = (uint32_t)sizeof(o);
+        ok = true;
+        if (!in) return;
+        if (in->struct_size < 8) {
+            ok = false;
+            return;
+        }
+        std::memcpy(&o, in, std::min<size_t>(in->struct_size, sizeof(o)));
+        o.struct_size = (uint32_t)sizeof(o);
+        if (o.reserved0 != 0) ok = false;
+    }
+};
+
 Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min, int32_t dt0,
                int32_t N_t0, int32_t tau_min, int32_t dtau, int32_t N_tau,
                const tfstat_opts *opts)
@@ -53,6 +74,7 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     pl.min_atoms = (opts && opts->min_atoms > 0) ? opts->min_atoms : 2;
     pl.ev_main_begin = opts ? static_cast<cudaEvent_t>(opts->ev_main_begin) : nullptr;
     pl.ev_main_end = opts ? static_cast<cudaEvent_t>(opts->ev_main_end) : nullptr;
+    pl.stats = opts ? reinterpret_cast<unsigned long long *>(opts->stats) : nullptr;
     pl.grid.t0_min = t0_min;
     pl.grid.dt0 = N_t0 > 1 ? dt0 : 0;
     pl.grid.N_t0 = N_t0;
@@ -92,6 +114,10 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         const int c = opts->tile_c;
         if (c != 1 && c != 2 && c != 4 && c != 8 && c != 16) return pl;
         pl.tile.C = c;
+        // the underflow guard above also binds a requested tile: the weight shared by a t0 tile
+        // drops by exp(-(C-1) dt0 / tau_min) across it
+        while (pl.tile.C > 1 && (int64_t)(pl.tile.C - 1) * pl.grid.dt0 > (int64_t)8 * tau_min)
+            pl.tile.C >>= 1;
     }
     if (opts && opts->tile_nt) {
         const int nt = opts->tile_nt;
@@ -238,6 +264,26 @@ static int32_t host_chunk_templates(int32_t n_templates)
     return std::min<int32_t>(n_templates, std::max<int32_t>(256, std::min<int32_t>(1024, n_templates / 4)));
 }
 
+// Plans of tfstat_search_host for chunks of Tc templates: the full chunks' plan, the plan of the
+// ragged last chunk (tile shapes depend on the number of templates, so it may need MORE
+// workspace than a full chunk), and the workspace that serves both.
+static int plan_host_chunks(int window, int32_t n_atoms, int32_t n_templates, int32_t Tc,
+                            int32_t t0_min, int32_t dt0, int32_t N_t0, int32_t tau_min,
+                            int32_t dtau, int32_t N_tau, const tfstat_opts *opts, Plan &pl,
+                            Plan &pl_last, size_t &ws_bytes)
+{
+    pl = make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts);
+    if (pl.status != TFSTAT_OK) return pl.status;
+    pl_last = pl;
+    const int32_t rem = n_templates % Tc;
+    if (rem != 0) {
+        pl_last = make_plan(window, n_atoms, rem, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts);
+        if (pl_last.status != TFSTAT_OK) return pl_last.status;
+    }
+    ws_bytes = align_up(std::max(std::max(pl.bytes, pl_last.bytes), kAlign));
+    return TFSTAT_OK;
+}
+
 }  // namespace tfstat
 
 using namespace tfstat;
@@ -264,9 +310,66 @@ size_t tfstat_workspace_bytes(int window, int32_t n_atoms, int32_t n_templates, 
                               int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
                               int32_t N_tau, const tfstat_opts *opts_host)
 {
+    const OptsIn oi(opts_host);
+    if (!oi.ok) return 0;
     const Plan pl = make_plan(window, n_atoms, n_templates, t0_min, dt0, N_t0, tau_min, dtau,
-                              N_tau, opts_host);
+                              N_tau, &oi.o);
     return pl.status == TFSTAT_OK ? std::max(pl.bytes, kAlign) : 0;
+}
+
+int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
+                     int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau, int32_t N_tau,
+                     const tfstat_opts *opts_host, tfstat_plan *info)
+{
+    if (!info || info->struct_size < 8) return TFSTAT_EINVAL;
+    const OptsIn oi(opts_host);
+    if (!oi.ok) return TFSTAT_EINVAL;
+    const Plan pl = make_plan(window, n_atoms, n_templates, t0_min, dt0, N_t0, tau_min, dtau,
+                              N_tau, &oi.o);
+    if (pl.status != TFSTAT_OK) return pl.status;
+    tfstat_plan p;
+    std::memset(&p, 0, sizeof(p));
+    p.lattice_J = (int32_t)pl.J;
+    p.workspace_bytes = std::max(pl.bytes, kAlign);
+    if (window == TFSTAT_WINDOW_EXP && pl.exp_method == TFSTAT_EXP_DIRECT) {
+        p.kernel = TFSTAT_KERNEL_EXP_DIRECT;
+        p.tile_c = pl.tile.C;
+        p.tile_nt = pl.tile.NT;
+        p.n_ctas = pl.tiles_per_template * n_templates;
+        p.n_launches = 3;  // bounds, sums + closure + marginals, finalize
+    } else if (window == TFSTAT_WINDOW_EXP) {
+        p.kernel = TFSTAT_KERNEL_EXP_SLIDE;
+        p.tile_c = pl.slide_tpc;
+        p.tile_nt = pl.tile.NT;
+        p.seg_len = pl.seg_len;
+        p.n_segs = pl.n_segs;
+        p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
+        p.n_launches = 3;
+    } else if (pl.rect_small) {
+        p.kernel = TFSTAT_KERNEL_RECT_SMALL;
+        p.tile_c = 1;
+        p.tile_nt = 256;
+        p.n_ctas = n_templates;
+        p.n_launches = 1;
+    } else if (pl.rect.enabled) {
+        p.kernel = TFSTAT_KERNEL_RECT_RUN;
+        p.tile_c = pl.rect.Q;
+        p.tile_nt = rect_run_threads(pl);
+        p.seg_len = pl.rect.seg_cols;
+        p.n_segs = pl.rect.n_coltiles;
+        p.n_ctas = (int64_t)pl.rect.n_rowtiles * pl.rect.n_coltiles * n_templates;
+        p.n_launches = 4;  // bounds, prefix + steps, running sums, finalize
+    } else {
+        p.kernel = TFSTAT_KERNEL_RECT_CELLS;
+        p.tile_c = 1;
+        p.tile_nt = 256;
+        p.n_ctas = (int64_t)pl.cell_blocks_per_template * n_templates;
+        p.n_launches = 4;
+    }
+    const uint32_t n = std::min<uint32_t>(info->struct_size, (uint32_t)sizeof(p));
+    p.struct_size = n;
+    std::memcpy(info, &p, n);
+    return TFSTAT_OK;
 }
 
 int tfstat_search(const float *atoms, int64_t template_stride, int64_t ld,
@@ -278,8 +381,10 @@ int tfstat_search(const float *atoms, int64_t template_stride, int64_t ld,
 {
     if (!atoms || !t_atoms || (!out && !out_maps)) return TFSTAT_EINVAL;
     if (ld < n_atoms || (n_templates > 1 && template_stride < 7 * ld)) return TFSTAT_EINVAL;
+    const OptsIn oi(opts_host);
+    if (!oi.ok) return TFSTAT_EINVAL;
     const Plan pl = make_plan(window, n_atoms, n_templates, t0_min, dt0, N_t0, tau_min, dtau,
-                              N_tau, opts_host);
+                              N_tau, &oi.o);
     if (pl.status != TFSTAT_OK) return pl.status;
     if (!workspace || workspace_bytes < pl.bytes ||
         (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)))
@@ -308,13 +413,15 @@ size_t tfstat_marginalise_workspace_bytes(int32_t N_t0, int32_t N_tau)
 
 int tfstat_marginalise(const float *map, const uint8_t *flags, int32_t N_t0, int32_t N_tau,
                        tfstat_result *out, void *workspace, size_t workspace_bytes,
-                       void *stream)
+                       void *stream, const tfstat_opts *opts_host)
 {
-    if (!map || !out || N_t0 < 1 || N_tau < 1) return TFSTAT_EINVAL;
+    if (!map || !out || N_t0 < 1 || N_tau < 1 || !OptsIn(opts_host).ok) return TFSTAT_EINVAL;
     const int64_t n_cells = (int64_t)N_t0 * N_tau;
     if (n_cells >= (int64_t(1) << 31)) return TFSTAT_EINVAL;
     const int32_t nb = marginalise_blocks(n_cells);
-    if (!workspace || workspace_bytes < sizeof(Partial) * (size_t)nb) return TFSTAT_EWORKSPACE;
+    if (!workspace || workspace_bytes < sizeof(Partial) * (size_t)nb ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15u))  // Partial is stored with 16-byte stores
+        return TFSTAT_EWORKSPACE;
     TF_CUDA(launch_marginalise(map, flags, n_cells, N_tau, static_cast<Partial *>(workspace),
                                nb, out, static_cast<cudaStream_t>(stream)));
     return TFSTAT_OK;
@@ -323,9 +430,9 @@ int tfstat_marginalise(const float *map, const uint8_t *flags, int32_t N_t0, int
 int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int32_t t0_min,
                        int32_t dt0, int32_t N_t0, int32_t tau_min, int32_t dtau,
                        int32_t N_tau, int64_t *out_terms, void *workspace,
-                       size_t workspace_bytes, void *stream)
+                       size_t workspace_bytes, void *stream, const tfstat_opts *opts_host)
 {
-    if (!t_atoms || !out_terms) return TFSTAT_EINVAL;
+    if (!t_atoms || !out_terms || !OptsIn(opts_host).ok) return TFSTAT_EINVAL;
     const Plan pl = make_plan(window, n_atoms, 1, t0_min, dt0, N_t0, tau_min, dtau, N_tau,
                               nullptr);
     if (pl.status != TFSTAT_OK) return pl.status;
@@ -333,6 +440,15 @@ int tfstat_count_terms(const int32_t *t_atoms, int32_t n_atoms, int window, int3
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     TF_CUDA(launch_bounds(pl, t_atoms, workspace, st));
     TF_CUDA(launch_count_terms(pl, make_bounds(pl, t_atoms, workspace), out_terms, st));
+    return TFSTAT_OK;
+}
+
+int tfstat_validate_timestamps(const int32_t *t_atoms, int32_t n_atoms, int32_t *out_first_bad,
+                               void *stream, const tfstat_opts *opts_host)
+{
+    if (!t_atoms || !out_first_bad || n_atoms < 1 || !OptsIn(opts_host).ok) return TFSTAT_EINVAL;
+    TF_CUDA(launch_validate_timestamps(t_atoms, n_atoms, out_first_bad,
+                                       static_cast<cudaStream_t>(stream)));
     return TFSTAT_OK;
 }
 
@@ -350,6 +466,8 @@ int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, i
 {
     if (!atoms || !t_atoms || !window_host || !t0_grid || !tau_grid || (!out_map && !out))
         return TFSTAT_EINVAL;
+    const OptsIn oi(opts_host);
+    if (!oi.ok) return TFSTAT_EINVAL;
     if (n_atoms < 1 || ld < n_atoms || N_t0 < 1 || N_tau < 1) return TFSTAT_EINVAL;
     if ((int64_t)N_t0 * N_tau >= (int64_t(1) << 31)) return TFSTAT_EINVAL;
     const tfstat_window &w = *window_host;
@@ -362,13 +480,13 @@ int tfstat_map_general(const float *atoms, int64_t ld, const int32_t *t_atoms, i
     if (!workspace || workspace_bytes < need ||
         (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)))
         return TFSTAT_EWORKSPACE;
-    const int32_t min_atoms = (opts_host && opts_host->min_atoms > 0) ? opts_host->min_atoms : 2;
+    const int32_t min_atoms = oi.o.min_atoms > 0 ? oi.o.min_atoms : 2;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     Partial *partials = out ? static_cast<Partial *>(workspace) : nullptr;
     int32_t n_partials = 0;
     TF_CUDA(launch_general(atoms, ld, t_atoms, n_atoms, w, t0_grid, N_t0, tau_grid, N_tau,
                            min_atoms, out_map, out_flags, partials, &n_partials,
-                           opts_host ? opts_host->tile_c : 0, st));
+                           oi.o.tile_c, st));
     if (out) TF_CUDA(launch_finalize(partials, n_partials, 1, N_tau, out, st));
     return TFSTAT_OK;
 }
@@ -377,10 +495,11 @@ int tfstat_merge_detectors(const float *const *atoms_dets, const int64_t *templa
                            const int64_t *lds, const int32_t *const *t_dets,
                            const int32_t *n_atoms_dets, int32_t n_det, int32_t n_templates,
                            const int32_t *t_out, int32_t n_out, float *out_atoms,
-                           int64_t template_stride_out, int64_t ld_out, void *stream)
+                           int64_t template_stride_out, int64_t ld_out, void *stream,
+                           const tfstat_opts *opts_host)
 {
     if (!atoms_dets || !template_strides || !lds || !t_dets || !n_atoms_dets || !t_out ||
-        !out_atoms)
+        !out_atoms || !OptsIn(opts_host).ok)
         return TFSTAT_EINVAL;
     if (n_det < 1 || n_det > TFSTAT_MAX_DETECTORS || n_templates < 1 || n_out < 1 ||
         ld_out < n_out || (n_templates > 1 && template_stride_out < 7 * ld_out))
@@ -406,6 +525,8 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
     if (!atoms_host || !t_atoms_host || !out_host) return TFSTAT_EINVAL;
     if (ld < n_atoms || (n_templates > 1 && template_stride < 7 * ld)) return TFSTAT_EINVAL;
     if (n_templates < 1) return TFSTAT_EINVAL;
+    const OptsIn oi(opts_host);
+    if (!oi.ok) return TFSTAT_EINVAL;
     if (device_scratch && (reinterpret_cast<uintptr_t>(device_scratch) & (kAlign - 1)))
         return TFSTAT_EWORKSPACE;
     const size_t budget = device_scratch_bytes ? device_scratch_bytes : size_t(2) << 30;
@@ -417,13 +538,14 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
     const size_t t_bytes = align_up(sizeof(int32_t) * (size_t)n_atoms);
     const size_t out_bytes = align_up(sizeof(tfstat_result) * (size_t)n_templates);
     int32_t Tc = host_chunk_templates(n_templates);
-    Plan pl;
-    size_t need = 0;
+    Plan pl, pl_last;
+    size_t need = 0, ws_bytes = 0;
     for (;; Tc = (Tc + 1) / 2) {
-        pl = make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts_host);
-        if (pl.status != TFSTAT_OK) return pl.status;
-        need = 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) +
-               align_up(std::max(pl.bytes, kAlign)) + t_bytes + out_bytes;
+        const int st = plan_host_chunks(window, n_atoms, n_templates, Tc, t0_min, dt0, N_t0,
+                                        tau_min, dtau, N_tau, &oi.o, pl, pl_last, ws_bytes);
+        if (st != TFSTAT_OK) return st;
+        need = 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) + ws_bytes + t_bytes +
+               out_bytes;
         if (need <= budget || Tc == 1) break;
     }
     if (device_scratch && need > budget) return TFSTAT_EWORKSPACE;
@@ -454,7 +576,7 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
         float *d_maps[2] = {nullptr, nullptr};
         if (map_bytes)
             for (int b = 0; b < 2; ++b) d_maps[b] = reinterpret_cast<float *>(carve(Tc * map_bytes));
-        void *d_ws = carve(std::max(pl.bytes, kAlign));
+        void *d_ws = carve(ws_bytes);
         int32_t *d_t = reinterpret_cast<int32_t *>(carve(sizeof(int32_t) * (size_t)n_atoms));
         tfstat_result *d_out =
             reinterpret_cast<tfstat_result *>(carve(sizeof(tfstat_result) * (size_t)n_templates));
@@ -473,14 +595,15 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
         if (!chk(cudaMemcpyAsync(d_t, t_atoms_host, sizeof(int32_t) * (size_t)n_atoms,
                                  cudaMemcpyHostToDevice, s_comp)))
             break;
+        // the lo / edge tables depend on the time stamps and the grid only (same offsets in every
+        // chunk's plan): built by the first chunk that needs them -- a chunk that takes the
+        // one-launch small-map kernel does not, a ragged last chunk after it may
+        bool bounds_done = false;
         for (int c = 0; c < n_chunks && rc == TFSTAT_OK; ++c) {
             const int b = c & 1;
             const int32_t k0 = c * Tc;
             const int32_t cnt = std::min<int32_t>(Tc, n_templates - k0);
-            Plan plc = pl;
-            if (cnt != Tc)
-                plc = make_plan(window, n_atoms, cnt, t0_min, dt0, N_t0, tau_min, dtau, N_tau,
-                                opts_host);
+            const Plan &plc = cnt == Tc ? pl : pl_last;
             // buffer b is free once chunk c-2 has been computed (and its maps copied back)
             if (c >= 2) {
                 chk(cudaStreamWaitEvent(s_copy, ev_done[b], 0));
@@ -491,10 +614,12 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
                                 sizeof(float) * n_float, cudaMemcpyHostToDevice, s_copy));
             chk(cudaEventRecord(ev_in[b], s_copy));
             chk(cudaStreamWaitEvent(s_comp, ev_in[b], 0));
+            const bool do_bounds = !bounds_done && !(plc.window == TFSTAT_WINDOW_RECT && plc.rect_small);
             const int r = run_device(plc, reinterpret_cast<const float *>(d_atoms[b]),
                                      template_stride, ld, d_t, d_out + k0, d_maps[b], nullptr,
-                                     d_ws, s_comp, c == 0);
+                                     d_ws, s_comp, do_bounds);
             if (r != TFSTAT_OK) rc = r;
+            bounds_done = bounds_done || do_bounds;
             chk(cudaEventRecord(ev_done[b], s_comp));
             if (map_bytes) {
                 chk(cudaStreamWaitEvent(s_back, ev_done[b], 0));
@@ -529,14 +654,18 @@ size_t tfstat_search_host_scratch_bytes(int64_t template_stride, int32_t n_atoms
                                         const tfstat_opts *opts_host)
 {
     if (n_templates < 1 || template_stride < 1) return 0;
+    const OptsIn oi(opts_host);
+    if (!oi.ok) return 0;
     const int32_t Tc = host_chunk_templates(n_templates);
-    const Plan pl =
-        make_plan(window, n_atoms, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau, opts_host);
-    if (pl.status != TFSTAT_OK) return 0;
+    Plan pl, pl_last;
+    size_t ws_bytes = 0;
+    if (plan_host_chunks(window, n_atoms, n_templates, Tc, t0_min, dt0, N_t0, tau_min, dtau, N_tau,
+                         &oi.o, pl, pl_last, ws_bytes) != TFSTAT_OK)
+        return 0;
     const size_t tpl_bytes = sizeof(float) * (size_t)template_stride;
     const size_t map_bytes = want_maps ? sizeof(float) * (size_t)N_t0 * N_tau : 0;
-    return 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) +
-           align_up(std::max(pl.bytes, kAlign)) + align_up(sizeof(int32_t) * (size_t)n_atoms) +
+    return 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) + ws_bytes +
+           align_up(sizeof(int32_t) * (size_t)n_atoms) +
            align_up(sizeof(tfstat_result) * (size_t)n_templates);
 }
 

@@ -81,6 +81,33 @@ cudaError_t launch_bounds(const Plan &pl, const int32_t *t_atoms, void *ws, cuda
     return cudaGetLastError();
 }
 
+// Opt-in validator of the precondition "time stamps strictly increasing" (include/tfstat.h).
+__global__ void validate_timestamps_kernel(const int32_t *__restrict__ t, const int n,
+                                           unsigned *__restrict__ first_bad)
+{
+    unsigned bad = 0xffffffffu;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x + 1; i < n;
+         i += (int64_t)gridDim.x * blockDim.x)
+        if (__ldg(t + i) <= __ldg(t + i - 1)) bad = min(bad, (unsigned)i);
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) bad = min(bad, __shfl_xor_sync(0xffffffffu, bad, s));
+    if ((threadIdx.x & 31) == 0 && bad != 0xffffffffu) atomicMin(first_bad, bad);
+}
+
+cudaError_t launch_validate_timestamps(const int32_t *t_atoms, int32_t n_atoms,
+                                       int32_t *out_first_bad, cudaStream_t st)
+{
+    // -1 = 0xffffffff is also the identity of the unsigned minimum
+    cudaError_t e = cudaMemsetAsync(out_first_bad, 0xff, sizeof(int32_t), st);
+    if (e != cudaSuccess) return e;
+    const int nt = 256;
+    int nb = (n_atoms + nt - 1) / nt;
+    if (nb > 148 * 8) nb = 148 * 8;
+    validate_timestamps_kernel<<<nb, nt, 0, st>>>(t_atoms, n_atoms,
+                                                  reinterpret_cast<unsigned *>(out_first_bad));
+    return cudaGetLastError();
+}
+
 __global__ void count_terms_kernel(Grid g, Bounds b, unsigned long long *out)
 {
     pdl_wait();

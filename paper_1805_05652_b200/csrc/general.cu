@@ -177,13 +177,16 @@ __global__ void __launch_bounds__(kGenNT)
                     const float t0v = tab[k], t1v = tab[k + 1];
                     w = fmaf(x - (float)k, t1v - t0v, t0v);
                 }
-                if (CT > 1) w = cs + i < hi[c] ? w : 0.0f;  // beyond this cell's own window
-                const float w2 = w * w;
-                ffma2(acc_ab[c], pack2(w2, w2), ra.y);
-                const u64 ww = pack2(w, w);
-                ffma2(acc_fa[c], ww, rb.x);
-                ffma2(acc_fb[c], ww, rb.y);
-                acc_c[c] = fmaf(w2, ab, acc_c[c]);
+                // an atom beyond this cell's own window is SKIPPED, not weighted by zero: 0 x NaN of
+                // a non-finite atom (a bad SFT) would spoil windows it is not part of
+                if (CT == 1 || cs + i < hi[c]) {
+                    const float w2 = w * w;
+                    ffma2(acc_ab[c], pack2(w2, w2), ra.y);
+                    const u64 ww = pack2(w, w);
+                    ffma2(acc_fa[c], ww, rb.x);
+                    ffma2(acc_fb[c], ww, rb.y);
+                    acc_c[c] = fmaf(w2, ab, acc_c[c]);
+                }
             }
         }
         __syncthreads();

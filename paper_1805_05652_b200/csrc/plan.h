@@ -65,6 +65,7 @@ struct Plan {
     size_t flags_bytes;  // rect: scan flags the bounds kernel (or a memset) zeroes
     int64_t partials_per_template;
     cudaEvent_t ev_main_begin, ev_main_end;  // optional profiling hooks (tfstat_opts)
+    unsigned long long *stats;               // optional device work counters (tfstat_opts)
 };
 
 Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min, int32_t dt0,
@@ -73,6 +74,9 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
 
 // launchers -------------------------------------------------------------------------------
 cudaError_t launch_bounds(const Plan &pl, const int32_t *t_atoms, void *ws, cudaStream_t st);
+cudaError_t launch_validate_timestamps(const int32_t *t_atoms, int32_t n_atoms,
+                                       int32_t *out_first_bad, cudaStream_t st);
+int rect_run_threads(const Plan &pl);
 cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_terms,
                                cudaStream_t st);
 cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,

@@ -1112,6 +1112,8 @@ cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st
     return cudaGetLastError();
 }
 
+int rect_run_threads(const Plan &) { return kRunNT; }
+
 int rect_scan_blocks(int32_t n_atoms) { return (n_atoms + kScanBlock - 1) / kScanBlock; }
 
 cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,

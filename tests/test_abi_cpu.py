@@ -18,23 +18,73 @@ def lib():
     return load_library()
 
 
-def declared_symbols():
-    names = set()
-    for h in ("tfstat.h", "tfstat_probe.h"):
-        src = open(os.path.join(ROOT, "include", h)).read()
-        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-        names |= set(re.findall(r"\b(tfstat_[a-z_0-9]+)\s*\(", src))
-    return names
+def declared_symbols(header):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return set(re.findall(r"\b(tfstat_[a-z_0-9]+)\s*\(", src))
 
 
 def test_exports_every_declared_symbol(lib):
-    names = declared_symbols()
+    names = declared_symbols("tfstat.h")
     assert {"tfstat_map", "tfstat_marginalise", "tfstat_search", "tfstat_search_host",
             "tfstat_workspace_bytes", "tfstat_count_terms", "tfstat_strerror",
-            "tfstat_version", "tfstat_probe_alu"} <= names
+            "tfstat_version", "tfstat_plan_info", "tfstat_validate_timestamps",
+            "tfstat_map_general", "tfstat_merge_detectors"} <= names
     for n in names:
-        assert hasattr(lib, n), f"{n} declared in include/ but not exported"
-    assert lib.tfstat_version() == 100
+        assert hasattr(lib, n), f"{n} declared in include/tfstat.h but not exported"
+    assert lib.tfstat_version() == 200
+    # the ALU micro-benchmarks live in a bench-only library of their own, not in the product
+    from paper_1805_05652_b200 import load_probe_library
+
+    probe = load_probe_library()
+    pnames = declared_symbols("tfstat_probe.h")
+    assert pnames == {"tfstat_probe_alu"}
+    for n in pnames:
+        assert hasattr(probe, n)
+        assert not hasattr(lib, n), f"{n} must not ship inside libtfstat.so"
+
+
+def test_opts_struct_size_and_plan_info(lib):
+    """tfstat_opts starts with its own size, so the struct can grow: a shorter (older) struct is
+    accepted and the missing fields take defaults; size 0 / reserved fields set are EINVAL.
+    tfstat_plan_info reports the kernel, tile and workspace tfstat_search would use."""
+    import paper_1805_05652_b200 as pkg
+    import paper_1805_05652_b200.binding as b
+
+    fake = C.c_void_p(0x1000)
+    grid = [0, 1800, 4, 3600, 1800, 4]
+    o = b._Opts()
+    assert o.struct_size == C.sizeof(b._Opts) == 56
+    o.struct_size = 0
+    assert lib.tfstat_search(fake, 70, 10, fake, 10, 1, 1, *grid, fake, None, None, fake, 1 << 20,
+                             None, C.byref(o)) == -1
+    assert lib.tfstat_workspace_bytes(1, 10, 1, *grid, C.byref(o)) == 0
+    o = b._Opts()
+    o.reserved0 = 1
+    assert lib.tfstat_workspace_bytes(1, 10, 1, *grid, C.byref(o)) == 0
+    # an "old" caller that only knows the fields up to exp_method: exp_method is honoured, a
+    # tile_c lying beyond its struct_size is ignored
+    g = G(0, 1800, 96, 43200, 1800, 1417)
+    o = b._Opts()
+    o.exp_method, o.tile_c = pkg.EXP_DIRECT, 2
+    p = b._Plan()
+    p.struct_size = C.sizeof(b._Plan)
+    assert lib.tfstat_plan_info(1, 2880, 4096, *b._grid_args(g), C.byref(o), C.byref(p)) == 0
+    assert (p.kernel, p.tile_c) == (1, 2)
+    o.struct_size = 12
+    assert lib.tfstat_plan_info(1, 2880, 4096, *b._grid_args(g), C.byref(o), C.byref(p)) == 0
+    assert (p.kernel, p.tile_c, p.tile_nt) == (1, 8, 128)  # config 4: the headline tile
+    assert p.n_ctas == 4096 * 12 * 12 and p.n_launches == 3
+    assert p.workspace_bytes == lib.tfstat_workspace_bytes(1, 2880, 4096, *b._grid_args(g), C.byref(o))
+    # defaults: the sliding form; config 1: the one-launch rect kernel; invalid shapes: errors
+    info = pkg.plan_info(pkg.EXP, 2880, 4096, g)
+    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 2
+    assert pkg.plan_info(pkg.RECT, 48, 1, G(0, 1800, 24, 1800, 1800, 24))["kernel_name"] == "rect_small"
+    big = pkg.plan_info(pkg.RECT, 13140, 1, G(0, 1800, 17520, 43200, 43200, 720))
+    assert big["kernel_name"] == "rect_run" and big["lattice_J"] == 17519 + 719 * 24 + 1
+    with pytest.raises(pkg.TfstatError):
+        pkg.plan_info(pkg.EXP, 10, 1, G(0, 1800, 0, 3600, 1800, 4))
+    assert lib.tfstat_plan_info(1, 10, 1, *grid, None, None) == -1
 
 
 def test_sass_is_sm100a():
@@ -106,8 +156,16 @@ def test_error_codes_before_any_cuda_call(lib):
     assert lib.tfstat_search(fake, 70, 10, fake, 10, 1, 1, *ov, fake, None, None, fake, 1 << 20,
                              None, opts) == -4
     assert lib.tfstat_map(fake, 10, fake, 10, 0, *grid, None, None, fake, 1 << 20, None, opts) == -1
-    assert lib.tfstat_marginalise(None, None, 4, 4, fake, fake, 1 << 20, None) == -1
-    assert lib.tfstat_marginalise(fake, None, 4, 4, fake, fake, 0, None) == -2
+    assert lib.tfstat_marginalise(None, None, 4, 4, fake, fake, 1 << 20, None, None) == -1
+    assert lib.tfstat_marginalise(fake, None, 4, 4, fake, fake, 0, None, None) == -2
+    # a workspace that is not 16-byte aligned is an error, not a device fault
+    assert lib.tfstat_marginalise(fake, None, 4, 4, fake, C.c_void_p(0x1004), 1 << 20, None,
+                                  None) == -2
+    # tfstat_validate_timestamps / tfstat_count_terms: null pointers, empty input
+    assert lib.tfstat_validate_timestamps(None, 10, fake, None, None) == -1
+    assert lib.tfstat_validate_timestamps(fake, 10, None, None, None) == -1
+    assert lib.tfstat_validate_timestamps(fake, 0, fake, None, None) == -1
+    assert lib.tfstat_count_terms(None, 10, 1, *grid, fake, fake, 1 << 20, None, None) == -1
     assert lib.tfstat_strerror(-2).decode().startswith("workspace")
     # rect_method / exp_method out of range
     import paper_1805_05652_b200.binding as b
@@ -140,12 +198,12 @@ def test_error_codes_before_any_cuda_call(lib):
     i64 = (C.c_int64 * 1)(70)
     ld = (C.c_int64 * 1)(10)
     n = (C.c_int32 * 1)(10)
-    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 0, 1, fake, 10, fake, 70, 10, None) == -1
-    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 9, 1, fake, 10, fake, 70, 10, None) == -1
-    assert lib.tfstat_merge_detectors(None, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 10, None) == -1
-    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 9, None) == -1
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 0, 1, fake, 10, fake, 70, 10, None, None) == -1
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 9, 1, fake, 10, fake, 70, 10, None, None) == -1
+    assert lib.tfstat_merge_detectors(None, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 10, None, None) == -1
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 9, None, None) == -1
     ld[0] = 9
-    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 10, None) == -1
+    assert lib.tfstat_merge_detectors(pa, i64, ld, pa, n, 1, 1, fake, 10, fake, 70, 10, None, None) == -1
     # tfstat_search_host: null host pointers, misaligned scratch
     assert lib.tfstat_search_host(None, 70, 10, fake, 10, 1, 1, *grid, fake, None, None, 0,
                                   None) == -1
