@@ -19,7 +19,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtfstat.so")
 PROBE_LIB = os.path.join(HERE, "libtfstat_probe.so")
-SOURCES = ["api.cu", "bounds.cu", "exp_direct.cu", "exp_scan.cu", "rect.cu", "general.cu", "merge.cu", "marginalise.cu"]
+SOURCES = ["api.cu", "bounds.cu", "exp_direct.cu", "exp_scan.cu", "rect.cu", "general.cu", "merge.cu", "marginalise.cu", "pack.cu"]
 PROBE_SOURCES = ["probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC,-Wall", "-Xptxas", "-v"]

@@ -202,6 +202,12 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     pl.off_steps = off;
     if (window == TFSTAT_WINDOW_RECT && pl.rect.enabled)
         off += align_up((size_t)64 * (size_t)(pl.J + 1) * n_templates);
+    pl.off_pack = off;
+    pl.n_pad = 0;
+    if (window == TFSTAT_WINDOW_EXP) {
+        pl.n_pad = (int32_t)(((int64_t)n_atoms + kPackBlock - 1) / kPackBlock * kPackBlock);
+        off += align_up((size_t)32 * (size_t)pl.n_pad * n_templates);
+    }
     pl.bytes = off;
     pl.status = TFSTAT_OK;
     return pl;
@@ -232,6 +238,8 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     pr.out_flags = out_flags;
     Partial *partials =
         out ? reinterpret_cast<Partial *>(static_cast<char *>(ws) + pl.off_partials) : nullptr;
+    void *packed = static_cast<char *>(ws) + pl.off_pack;
+    if (pl.window == TFSTAT_WINDOW_EXP) TF_CUDA(launch_pack(pl, pr, packed, st));
     if (pl.ev_main_begin) TF_CUDA(cudaEventRecord(pl.ev_main_begin, st));
     if (small) {
         TF_CUDA(launch_rect_small(pl, pr, st));
@@ -245,9 +253,9 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
         TF_CUDA(launch_rect(pl, pr, prefix, agg, flags, static_cast<char *>(ws) + pl.off_steps,
                             partials, st));
     } else if (pl.exp_method == TFSTAT_EXP_DIRECT) {
-        TF_CUDA(launch_exp_direct(pl, pr, partials, st));
+        TF_CUDA(launch_exp_direct(pl, pr, packed, partials, st));
     } else {
-        TF_CUDA(launch_exp_scan(pl, pr, partials, st));
+        TF_CUDA(launch_exp_scan(pl, pr, packed, partials, st));
     }
     if (pl.ev_main_end) TF_CUDA(cudaEventRecord(pl.ev_main_end, st));
     if (out)
@@ -336,7 +344,7 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.tile_c = pl.tile.C;
         p.tile_nt = pl.tile.NT;
         p.n_ctas = pl.tiles_per_template * n_templates;
-        p.n_launches = 3;  // bounds, sums + closure + marginals, finalize
+        p.n_launches = 4;  // bounds, pack, sums + closure + marginals, finalize
     } else if (window == TFSTAT_WINDOW_EXP) {
         p.kernel = TFSTAT_KERNEL_EXP_SLIDE;
         p.tile_c = pl.slide_tpc;
@@ -344,7 +352,7 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.seg_len = pl.seg_len;
         p.n_segs = pl.n_segs;
         p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
-        p.n_launches = 3;
+        p.n_launches = 4;
     } else if (pl.rect_small) {
         p.kernel = TFSTAT_KERNEL_RECT_SMALL;
         p.tile_c = 1;

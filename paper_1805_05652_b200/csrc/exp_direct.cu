@@ -29,76 +29,131 @@
 //    SHORTEST windows, and CTAs are launched heaviest (largest tau) first.
 #include "plan.h"
 
-// Tuning constants of the core loop, swept on B200 (config 4, 592 templates): staging chunk KC in
-// {256, 512, 1024} atoms x unroll in {2 .. 64}.  Unrolling is what matters (unroll 4: 3.79e12
-// terms/s, 8: 3.94, 16: 4.10, 24..32: 4.12-4.17, 64: 4.11; the loop counter, the shared-memory address
-// arithmetic and the branch are per iteration, and the scheduler gets more independent LDS /
-// MUFU to hoist above the FFMA2 stream); KC = 1024 adds ~1 % over 512 (half the barriers).
-constexpr int kStageAtoms = 1024;
-constexpr int kCoreUnroll = 24;
+// Tuning constants of the core loop, swept on B200 (config 4).  Unrolling is what matters (unroll
+// 4: 3.79e12 terms/s, 8: 3.94, 16: 4.10, 24..32: 4.12-4.17, 64: 4.11; the loop counter, the
+// shared-memory address arithmetic and the branch are per iteration, and the scheduler gets more
+// independent LDS / MUFU to hoist above the FFMA2 stream).
+constexpr int kChunkAtoms = 192;  // atoms per bulk copy (6 KB); divides kPackBlock
+constexpr int kStages = 2;        // ring slots per warp
+constexpr int kCoreUnroll = 24;   // divides kChunkAtoms
 namespace tfstat {
 
 namespace {
 
+static_assert(kPackBlock % kChunkAtoms == 0, "a staged chunk must lie inside one packed time block");
+static_assert(kChunkAtoms % kCoreUnroll == 0, "whole unrolled trips per full chunk");
+
+// Accumulators: channel k of the cells (2p, 2p + 1) as one packed fp32x2 pair.
+//   k: 0 A, 1 B, 2 C, 3 Re Fa, 4 Im Fa, 5 Re Fb, 6 Im Fb
+// The C cells of a thread share the weight AND the atom, so a pair of CELLS is updated by one
+// fma.rn.f32x2 whose two multiplicands are both broadcast scalars (SASS: FFMA2 Racc, Rw.F32,
+// Rx.F32, Racc).  Measured on B200 (profiles/r02_ffma2_forms.md): this is the one packed form
+// that issues every 2 clocks; a register-pair multiplicand (channel pairs of ONE cell: the
+// round-1 layout) takes 2.4.  Isolated loop, C = 8: 15.85 against 15.20 terms/clk/SM; C = 16:
+// 16.60 against 15.98.
 template <int C>
 struct Acc {
-    u64 ab[C];            // (A, B)
-    u64 fa[C];            // (Re Fa, Im Fa)
-    u64 fb[C];            // (Re Fb, Im Fb)
-    u64 cc[(C + 1) / 2];  // (C of cell 2p, C of cell 2p+1)
+    u64 ch[7][(C + 1) / 2];
 };
 
-// one staged atom: rec_a = {(dt, ab), (a2, b2)}, rec_b = {(Re Fa, Im Fa), (Re Fb, Im Fb)}
 template <int C>
-__device__ __forceinline__ void accumulate_core(Acc<C> &acc, const ulonglong2 ra,
-                                                const ulonglong2 rb, const float kexp)
+__device__ __forceinline__ void acc_zero(Acc<C> &acc)
 {
-    float dt, ab;
-    unpack2(ra.x, dt, ab);
-    const float w = ex2_approx(dt * kexp);
-    const float w2 = w * w;
-    // Multiplier as a broadcast scalar, atom operand as a register pair.  Measured on B200
-    // (DESIGN.md "FFMA2 operand forms"): this form and the pre-multiplied FADD2 form both end
-    // at ~13 terms/clk/SM once the LDS write-backs share the register file with the
-    // accumulator updates; two-pair forms (w2 as a pair from FMUL2) are ~2 % slower.
-    const u64 ww = pack2(w, w);
-    const u64 w2w2 = pack2(w2, w2);
-    const u64 abab = pack2(ab, ab);
 #pragma unroll
-    for (int c = 0; c < C; ++c) {
-        ffma2(acc.ab[c], w2w2, ra.y);
-        ffma2(acc.fa[c], ww, rb.x);
-        ffma2(acc.fb[c], ww, rb.y);
-    }
+    for (int k = 0; k < 7; ++k)
 #pragma unroll
-    for (int p = 0; p < (C + 1) / 2; ++p) ffma2(acc.cc[p], w2w2, abab);
+        for (int p = 0; p < (C + 1) / 2; ++p) acc.ch[k][p] = 0ull;
 }
 
-template <int C, int NT, int KC>
-__global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C > 8 ? 384 : 512) / NT))
-    exp_direct_kernel(const Problem pr, Partial *__restrict__ partials, const int n_mtiles,
-                      const int n_nblocks)
+// one staged atom: rec_a = {(dtc, ab), (a2, b2)}, rec_b = {(Re Fa, Im Fa), (Re Fb, Im Fb)};
+// weight argument (t - t_ref) kexp = dtc kexp + cexp (pack.cu)
+template <int C>
+__device__ __forceinline__ void accumulate_core(Acc<C> &acc, const ulonglong2 ra,
+                                                const ulonglong2 rb, const float kexp,
+                                                const float cexp)
 {
-    __shared__ ulonglong2 s_a[KC];
-    __shared__ ulonglong2 s_b[KC];
+    float x[7], dt;
+    unpack2(ra.x, dt, x[2]);
+    unpack2(ra.y, x[0], x[1]);
+    unpack2(rb.x, x[3], x[4]);
+    unpack2(rb.y, x[5], x[6]);
+    const float w = ex2_approx(fmaf(dt, kexp, cexp));
+    const float w2 = w * w;
+    const u64 ww = pack2(w, w);
+    const u64 w2w2 = pack2(w2, w2);
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        const u64 xx = pack2(x[k], x[k]);
+#pragma unroll
+        for (int p = 0; p < (C + 1) / 2; ++p) ffma2(acc.ch[k][p], k < 3 ? w2w2 : ww, xx);
+    }
+}
+
+// cell c alone (head / tail atoms that belong to some of the thread's cells only): a scalar FMA on
+// one half of the pair
+template <int C>
+__device__ __forceinline__ void accumulate_cell(Acc<C> &acc, const int c, const float w,
+                                                const float w2, const float (&x)[7])
+{
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        float lo, hi;
+        unpack2(acc.ch[k][c / 2], lo, hi);
+        if (c & 1) hi = fmaf(k < 3 ? w2 : w, x[k], hi);
+        else lo = fmaf(k < 3 ? w2 : w, x[k], lo);
+        acc.ch[k][c / 2] = pack2(lo, hi);
+    }
+}
+
+// Staging: every WARP streams the atoms of its own windows through its own ring
+// of kStages slots of kChunkAtoms packed atoms, filled by bulk asynchronous copies
+// (cp.async.bulk global -> shared, one elected lane issues them, completion on the slot's
+// mbarrier).  No thread moves atom data, and there is no CTA barrier in the loop: a warp waits
+// for its own data only, never for the other warps of the CTA (whose windows -- larger tau --
+// are longer).
+template <int C, int NT, int KW, int NS>
+__global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
+    exp_direct_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+                      Partial *__restrict__ partials, const int n_mtiles, const int n_nblocks)
+{
+    constexpr int NW = NT / 32;
+    extern __shared__ __align__(128) unsigned char smem_raw[];  // rings: [NW][NS][2 KW] x 16 B
+    __shared__ __align__(8) unsigned long long s_bar[NW][NS];
     __shared__ Marg s_red[32];
     pdl_trigger();
-    pdl_wait();  // bounds_kernel's lo / edge tables
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t tiles = (int64_t)n_mtiles * n_nblocks;
     const int tpl = (int)(blockIdx.x / tiles);
     const int tile = (int)(blockIdx.x % tiles);
     const int nb = n_nblocks - 1 - tile / n_mtiles;  // heaviest (largest tau) first
     const int m0 = (tile % n_mtiles) * C;
+    // Warp w of a CTA runs on scheduler w of its SM, and the windows of a CTA grow with the warp
+    // index (32 more tau values each): left alone, scheduler 0 of every SM would get the lightest
+    // quarter of every resident CTA and scheduler NW-1 the heaviest.  Rotating the quarter a warp
+    // takes with the CTA index evens the schedulers out.
+    const int tq = ((warp + (int)(blockIdx.x % NW)) % NW) * 32 + lane;  // tau slot in the CTA
     // tau blocks: block 0 holds the N_tau % NT shortest windows (if any), the others are full
     const int ragged = g.N_tau % NT;
     const int n_first = (ragged && nb > 0) ? ragged + (nb - 1) * NT : nb * NT;
     const int n_count = (ragged && nb == 0) ? ragged : NT;
-    const bool n_ok = (int)threadIdx.x < n_count;
-    const int n = n_first + (n_ok ? (int)threadIdx.x : 0);
+    const bool n_ok = tq < n_count;
+    const int n = n_first + (n_ok ? tq : 0);
     const int m_last = min(m0 + C - 1, g.N_t0 - 1);  // cells beyond N_t0 duplicate the last one
+
+    const uint32_t bar0 = smem_u32(&s_bar[warp][0]);
+    constexpr uint32_t kChunkBytes = 2 * KW * sizeof(ulonglong2);
+    const ulonglong2 *s_ring = reinterpret_cast<const ulonglong2 *>(smem_raw) + warp * (NS * 2 * KW);
+    const uint32_t ring0 = smem_u32(s_ring);
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(bar0 + 8 * s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
 
     // per-thread ranges: head [h0, cb) and tail [ce, h1) take 0/1 weights per cell, the core
     // [cb, ce) belongs to all C cells
@@ -110,11 +165,22 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
         h1 = max(hi_index(bd, g, m_last, n), lo_last);
         cb = lo_last;
         ce = max(hi_index(bd, g, m0, n), lo_first);
-        if (ce <= cb) cb = ce = h1;  // no common core: everything goes through the head loop
     }
-    // atom range the CTA streams through shared memory: the union of its threads' cores
-    const int cta_b = lo_last;
-    const int cta_e = hi_index(bd, g, m0, n_first + n_count - 1);
+    const bool has_core = ce > cb;  // else: windows shorter than the tile's t0 span (or no cell)
+    // atom range the WARP streams through its ring: the union of its threads' cores, in whole
+    // chunks of KW atoms aligned to multiples of KW (one packed time base per chunk)
+    const int warp_b = lo_last;
+    const int warp_e = __reduce_max_sync(0xffffffffu, has_core ? ce : 0);
+    const int q0 = warp_b / KW;
+    const int nq = warp_e > warp_b ? (warp_e + KW - 1) / KW - q0 : 0;
+    const ulonglong2 *__restrict__ rec = packed + (int64_t)tpl * n_pad * 2;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s)
+            if (s < nq)
+                bulk_load(ring0 + s * kChunkBytes, rec + (int64_t)(q0 + s) * KW * 2, kChunkBytes,
+                          bar0 + 8 * s);
+    }
 
     const long long t_ref = t0_of(g, m0);
     const float kexp = (float)(-1.4426950408889634 / (double)tau_of(g, n));
@@ -123,15 +189,16 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
     const int64_t ld = pr.ld;
 
     Acc<C> acc;
-#pragma unroll
-    for (int c = 0; c < C; ++c) acc.ab[c] = acc.fa[c] = acc.fb[c] = 0ull;
-#pragma unroll
-    for (int p = 0; p < (C + 1) / 2; ++p) acc.cc[p] = 0ull;
+    acc_zero<C>(acc);
 
     // ---- head and tail: atoms that belong to some of the thread's cells only ----------------
+    // (measured on B200, config 4: an unrolled "staircase" -- the atoms in [lo_c, lo_c+1) belong
+    // to cells 0..c, so every step adds to a fixed set of cells without predicates -- is 2.4 %
+    // SLOWER than this plain predicated loop: twice the code, one short loop per step)
 #pragma unroll 1
     for (int ph = 0; ph < 2; ++ph) {
-        const int xb = ph ? ce : h0, xe = ph ? h1 : cb;
+        const int xb = has_core ? (ph ? ce : h0) : (ph ? h1 : h0);
+        const int xe = has_core ? (ph ? h1 : cb) : h1;
         if (xb >= xe) continue;
         int lo[C], hi[C];
 #pragma unroll
@@ -144,54 +211,37 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
         for (int al = xb; al < xe; ++al) {
             const float dt = (float)((long long)__ldg(bd.t + al) - t_ref);
             const float w = ex2_approx(dt * kexp);
-            const u64 a2b2 = pack2(__ldg(base + al), __ldg(base + ld + al));
-            const float ab = __ldg(base + 2 * ld + al);
-            const u64 fa = pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al));
-            const u64 fb = pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al));
+            const float w2 = w * w;
+            float x[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) x[k] = __ldg(base + k * ld + al);
             // cells that do not hold this atom are SKIPPED, not weighted by zero: 0 x NaN of a
             // non-finite atom (a bad SFT) would spoil windows it is not part of
-            const u64 ww = pack2(w, w);
-            const u64 w2 = fmul2(ww, ww);
-            const float w2ab = w * w * ab;
 #pragma unroll
-            for (int c = 0; c < C; ++c) {
-                if (al >= lo[c] && al < hi[c]) {
-                    ffma2(acc.ab[c], w2, a2b2);
-                    ffma2(acc.fa[c], ww, fa);
-                    ffma2(acc.fb[c], ww, fb);
-                    float c0, c1;
-                    unpack2(acc.cc[c / 2], c0, c1);
-                    if (c & 1) c1 += w2ab;
-                    else c0 += w2ab;
-                    acc.cc[c / 2] = pack2(c0, c1);
-                }
-            }
+            for (int c = 0; c < C; ++c)
+                if (al >= lo[c] && al < hi[c]) accumulate_cell<C>(acc, c, w, w2, x);
         }
     }
 
-    // ---- core: atoms common to all C cells, streamed through shared memory ------------------
+    // ---- core: atoms common to all C cells, streamed through the warp's ring ----------------
 #pragma unroll 1
-    for (int cs = cta_b; cs < cta_e; cs += KC) {
-        const int n_stage = min(KC, cta_e - cs);
-        // a0: stage atoms [cs, cs + n_stage)
-        for (int i = threadIdx.x; i < n_stage; i += NT) {
-            const int al = cs + i;
-            const float dt = (float)((long long)__ldg(bd.t + al) - t_ref);
-            ulonglong2 ra, rb;
-            ra.x = pack2(dt, __ldg(base + 2 * ld + al));
-            ra.y = pack2(__ldg(base + al), __ldg(base + ld + al));
-            rb.x = pack2(__ldg(base + 3 * ld + al), __ldg(base + 4 * ld + al));
-            rb.y = pack2(__ldg(base + 5 * ld + al), __ldg(base + 6 * ld + al));
-            s_a[i] = ra;
-            s_b[i] = rb;
-        }
-        __syncthreads();
-        // a3: weighted sums over this chunk, per-thread bounds
+    for (int k = 0; k < nq; ++k) {
+        const int s = k % NS;
+        const int cs = (q0 + k) * KW;  // first atom of the chunk
+        // weight argument of atom i: dtc_i kexp + cexp, dtc_i relative to the chunk's time base
+        const int tb = __ldg(bd.t + cs - cs % kPackBlock);
+        const float cexp = (float)((long long)tb - t_ref) * kexp;
         const int x0 = max(cs, cb) - cs;
-        const int x1 = min(cs + n_stage, ce) - cs;
+        const int x1 = has_core ? min(cs + KW, ce) - cs : x0;
+        mbar_wait(bar0 + 8 * s, (uint32_t)(k / NS) & 1u);
+        const ulonglong2 *__restrict__ slot = s_ring + s * (2 * KW);
 #pragma unroll kCoreUnroll
-        for (int i = x0; i < x1; ++i) accumulate_core<C>(acc, s_a[i], s_b[i], kexp);
-        __syncthreads();
+        for (int i = x0; i < x1; ++i)
+            accumulate_core<C>(acc, slot[2 * i], slot[2 * i + 1], kexp, cexp);
+        __syncwarp();  // every lane is done with the slot: refill it
+        if (lane == 0 && k + NS < nq)
+            bulk_load(ring0 + s * kChunkBytes, rec + (int64_t)(q0 + k + NS) * KW * 2, kChunkBytes,
+                      bar0 + 8 * s);
     }
 
     // ---- a4 closure + a5 marginals ----------------------------------------------------------
@@ -202,12 +252,15 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
     for (int c = 0; c < C; ++c) {
         const int m = m0 + c;
         if (n_ok && m < g.N_t0) {
-            float A, B, Cc, cc0, cc1, far, fai, fbr, fbi;
-            unpack2(acc.ab[c], A, B);
-            unpack2(acc.fa[c], far, fai);
-            unpack2(acc.fb[c], fbr, fbi);
-            unpack2(acc.cc[c / 2], cc0, cc1);
-            Cc = (c & 1) ? cc1 : cc0;
+            float S[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                float e, o;
+                unpack2(acc.ch[k][c / 2], e, o);
+                S[k] = (c & 1) ? o : e;
+            }
+            const float A = S[0], B = S[1], Cc = S[2], far = S[3], fai = S[4], fbr = S[5],
+                        fbi = S[6];
             const int lo_c = __ldg(bd.lo + m);
             const int cnt = max(hi_index(bd, g, m, n) - lo_c, 0);
             uint32_t fl;
@@ -229,34 +282,41 @@ __global__ void __launch_bounds__(NT, ((C > 8 ? 384 : 512) / NT) > 12 ? 12 : ((C
 }
 
 template <int C, int NT>
-cudaError_t launch_one(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
+cudaError_t launch_one(const Plan &pl, const Problem &pr, const void *packed, Partial *partials,
+                       cudaStream_t st)
 {
     const int64_t n_ctas = pl.tiles_per_template * pl.n_templates;
-    return launch_pdl(exp_direct_kernel<C, NT, kStageAtoms>, (unsigned)n_ctas, NT, 0, st, pr, partials,
-                      pl.n_mtiles, pl.n_nblocks);
+    auto kern = exp_direct_kernel<C, NT, kChunkAtoms, kStages>;
+    const size_t smem = (size_t)(NT / 32) * kStages * 2 * kChunkAtoms * sizeof(ulonglong2);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(kern, (unsigned)n_ctas, NT, smem, st,
+                      pr, static_cast<const ulonglong2 *>(packed), pl.n_pad, partials, pl.n_mtiles,
+                      pl.n_nblocks);
 }
 
 template <int C>
-cudaError_t launch_c(const Plan &pl, const Problem &pr, Partial *partials, cudaStream_t st)
+cudaError_t launch_c(const Plan &pl, const Problem &pr, const void *packed, Partial *partials,
+                     cudaStream_t st)
 {
-    if (pl.tile.NT == 256) return launch_one<C, 256>(pl, pr, partials, st);
-    if (pl.tile.NT == 128) return launch_one<C, 128>(pl, pr, partials, st);
-    if (pl.tile.NT == 64) return launch_one<C, 64>(pl, pr, partials, st);
-    if (pl.tile.NT == 32) return launch_one<C, 32>(pl, pr, partials, st);
+    if (pl.tile.NT == 256) return launch_one<C, 256>(pl, pr, packed, partials, st);
+    if (pl.tile.NT == 128) return launch_one<C, 128>(pl, pr, packed, partials, st);
+    if (pl.tile.NT == 64) return launch_one<C, 64>(pl, pr, packed, partials, st);
+    if (pl.tile.NT == 32) return launch_one<C, 32>(pl, pr, packed, partials, st);
     return cudaErrorInvalidValue;
 }
 
 }  // namespace
 
-cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,
-                              cudaStream_t st)
+cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, const void *packed,
+                              Partial *partials, cudaStream_t st)
 {
     switch (pl.tile.C) {
-    case 16: return launch_c<16>(pl, pr, partials, st);
-    case 8: return launch_c<8>(pl, pr, partials, st);
-    case 4: return launch_c<4>(pl, pr, partials, st);
-    case 2: return launch_c<2>(pl, pr, partials, st);
-    case 1: return launch_c<1>(pl, pr, partials, st);
+    case 16: return launch_c<16>(pl, pr, packed, partials, st);
+    case 8: return launch_c<8>(pl, pr, packed, partials, st);
+    case 4: return launch_c<4>(pl, pr, packed, partials, st);
+    case 2: return launch_c<2>(pl, pr, packed, partials, st);
+    case 1: return launch_c<1>(pl, pr, packed, partials, st);
     }
     return cudaErrorInvalidValue;
 }

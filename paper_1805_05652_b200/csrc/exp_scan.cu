@@ -301,9 +301,10 @@ cudaError_t launch_nt(const Plan &pl, const Problem &pr, Partial *partials, cuda
 
 }  // namespace
 
-cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,
-                            cudaStream_t st)
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packed,
+                            Partial *partials, cudaStream_t st)
 {
+    (void)packed;
     switch (pl.tile.NT) {
     case 128: return launch_nt<128>(pl, pr, partials, st);
     case 64: return launch_nt<64>(pl, pr, partials, st);

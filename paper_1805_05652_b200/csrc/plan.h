@@ -61,7 +61,9 @@ struct Plan {
     int32_t cell_blocks_per_template;
     RectRun rect;
     // workspace layout (byte offsets)
-    size_t off_lo, off_edge, off_partials, off_prefix, off_tot, off_flags, off_steps, bytes;
+    size_t off_lo, off_edge, off_partials, off_prefix, off_tot, off_flags, off_steps, off_pack,
+        bytes;
+    int32_t n_pad;  // exp: atoms per template in the packed records (pack.cu), padded
     size_t flags_bytes;  // rect: scan flags the bounds kernel (or a memset) zeroes
     int64_t partials_per_template;
     cudaEvent_t ev_main_begin, ev_main_end;  // optional profiling hooks (tfstat_opts)
@@ -79,8 +81,9 @@ cudaError_t launch_validate_timestamps(const int32_t *t_atoms, int32_t n_atoms,
 int rect_run_threads(const Plan &pl);
 cudaError_t launch_count_terms(const Plan &pl, const Bounds &b, int64_t *out_terms,
                                cudaStream_t st);
-cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, Partial *partials,
-                              cudaStream_t st);
+cudaError_t launch_pack(const Plan &pl, const Problem &pr, void *packed, cudaStream_t st);
+cudaError_t launch_exp_direct(const Plan &pl, const Problem &pr, const void *packed,
+                              Partial *partials, cudaStream_t st);
 RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_t n_templates,
                       int32_t q_override, int32_t seg_override);
 int rect_scan_blocks(int32_t n_atoms);
@@ -88,8 +91,8 @@ bool rect_small_applies(int32_t n_atoms, int32_t n_templates, int64_t cells);
 cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st);
 cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,
                         int32_t *flags, void *steps, Partial *partials, cudaStream_t st);
-cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, Partial *partials,
-                            cudaStream_t st);
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packed,
+                            Partial *partials, cudaStream_t st);
 cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_template,
                             int32_t n_templates, int32_t N_tau, tfstat_result *out,
                             cudaStream_t st);

@@ -340,6 +340,52 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned 
 }
 
 // ---------------------------------------------------------------------------------------
+// Packed atoms (pack.cu) and the bulk asynchronous copy that stages them: cp.async.bulk
+// global -> shared, completion signalled on an mbarrier (the 1-D TMA path of sm_90+/sm_100).
+// ---------------------------------------------------------------------------------------
+constexpr int kPackBlock = 768;  // atoms per block of the packed time base; divisible by every
+                                 // staging chunk (128, 192, 256, 384), so a chunk has ONE base
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(const uint32_t bar, const uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+// makes the barrier initialisation visible to the async proxy (the copy engine)
+__device__ __forceinline__ void mbar_fence_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+// arm the barrier for `bytes` and issue the copy; src, dst 16-byte aligned, bytes % 16 == 0
+__device__ __forceinline__ void bulk_load(const uint32_t dst, const void *src, const uint32_t bytes,
+                                          const uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_wait(const uint32_t bar, const uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MBAR_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MBAR_DONE_%=;\n"
+        "bra MBAR_WAIT_%=;\n"
+        "MBAR_DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
+// ---------------------------------------------------------------------------------------
 // host-side launchers (one per .cu file)
 // ---------------------------------------------------------------------------------------
 struct Problem {
