@@ -95,11 +95,12 @@ typedef struct tfstat_opts {
                            whenever the atoms fit its shared memory (n_atoms <= 2048)          */
     int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
                            per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
-                           (1,2,4); tfstat_map_general: tau cells per thread (1,2,4); lattice
+                           (1,2,4; 11,12: 1,2 with two tau values per thread); tfstat_map_general: tau cells per thread (1,2,4); lattice
                            rect kernel: rows per thread (1, 2, 4)                             */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
     int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice
-                           rect kernel: columns per CTA (rounded up to 16)                   */
+                           rect kernel: columns per CTA (rounded up to 16); direct exp kernel:
+                           1 = the warps of a CTA split the windows' atoms, 2 = they never do */
     int32_t reserved0;  /* must be 0 */
     /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
      * immediately before and after the dominant kernel of the call (the window-sum +

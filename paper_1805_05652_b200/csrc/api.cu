@@ -109,8 +109,18 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
     // one weight per t0 tile (exp_direct.cu): the per-cell factor exp(-(c dt0)/tau) that the
     // closure is invariant to must stay well inside fp32 range
     while (C > 1 && (int64_t)(C - 1) * pl.grid.dt0 > (int64_t)8 * tau_min) C >>= 1;
-    pl.tile = ExpTile{C, n_ctas(C, 128) >= wave ? 128 : 64};
-    if (opts && opts->tile_c) {
+    pl.tile = ExpTile{C, n_ctas(C, 128) >= wave ? 128 : 64, 0};
+    // Too few CTAs to fill the GPU several times over (a single map): the warps of a CTA split
+    // the windows' atoms instead of the tau values (exp_direct.cu, SPLIT): 32 tau per CTA, four
+    // times the CTAs, a quarter of the critical path each.  C from the same rule on that grid.
+    if (n_ctas(8, 128) < 8 * wave) {
+        // (measured on B200, single maps: config 2 C = 8 / 4 / 2: 166 / 169 / 190 us; config 3:
+        // 528 / 563 / 647 us; unsplit C = 4: 170 / 593 us)
+        int Cs = n_ctas(8, 32) >= 2 * wave ? 8 : n_ctas(4, 32) >= wave ? 4 : 2;
+        while (Cs > 1 && (int64_t)(Cs - 1) * pl.grid.dt0 > (int64_t)8 * tau_min) Cs >>= 1;
+        pl.tile = ExpTile{Cs, 128, 1};
+    }
+    if (opts && opts->tile_c && !(window == TFSTAT_WINDOW_EXP && method == TFSTAT_EXP_SCAN)) {
         const int c = opts->tile_c;
         if (c != 1 && c != 2 && c != 4 && c != 8 && c != 16) return pl;
         pl.tile.C = c;
@@ -124,8 +134,14 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         if (nt != 32 && nt != 64 && nt != 128 && nt != 256) return pl;
         pl.tile.NT = nt;
     }
+    if (opts && opts->seg_len && window == TFSTAT_WINDOW_EXP && method == TFSTAT_EXP_DIRECT) {
+        if (opts->seg_len != 1 && opts->seg_len != 2) return pl;
+        pl.tile.split = opts->seg_len == 1;
+    }
+    if (pl.tile.C > 8 || pl.tile.NT != 128) pl.tile.split = 0;  // the split form's one shape
+    const int tpb = pl.tile.split ? 32 : pl.tile.NT;  // tau values per CTA
     pl.n_mtiles = (N_t0 + pl.tile.C - 1) / pl.tile.C;
-    pl.n_nblocks = (N_tau + pl.tile.NT - 1) / pl.tile.NT;
+    pl.n_nblocks = (N_tau + tpb - 1) / tpb;
     pl.tiles_per_template = (int64_t)pl.n_mtiles * pl.n_nblocks;
     pl.cell_blocks_per_template = (int32_t)((cells + 255) / 256);
 
@@ -153,15 +169,18 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         if (opts && opts->seg_len > 0) len = opts->seg_len < N_t0 ? opts->seg_len : N_t0;
         pl.seg_len = len;
         pl.n_segs = (N_t0 + len - 1) / len;
-        // templates per CTA (they share the weights): 2 while that still leaves ~16 CTAs per SM
-        // (measured on B200, config 4 x 2048: 1 -> 5.26 ms, 2 -> 4.57 ms, 4 -> 4.78 ms: at 4 the
-        // 162 registers cost more occupancy than the shared weights save; 4 only on request)
+        // templates per CTA (they share the weights) and tau values per thread (they share the
+        // atom loads): 2 each while that still leaves the GPU several CTAs per SM (exp_scan.cu)
         const int64_t ctas1 = (int64_t)n_templates * pl.n_nblocks * pl.n_segs;
         pl.slide_tpc = (n_templates >= 2 && ctas1 / 2 >= 148 * 16) ? 2 : 1;
-        if (opts && opts->tile_c) {
-            if (opts->tile_c != 1 && opts->tile_c != 2 && opts->tile_c != 4) return pl;
-            pl.slide_tpc = opts->tile_c;
+        pl.slide_rt = 1;  // 2 only on request: measured slower (168 registers, 3 CTAs per SM)
+        if (opts && opts->tile_c) {  // 1, 2, 4: templates per CTA; + 10: two tau values per thread
+            const int c = opts->tile_c;
+            if (c != 1 && c != 2 && c != 4 && c != 11 && c != 12) return pl;
+            pl.slide_rt = c > 10 ? 2 : 1;
+            pl.slide_tpc = c > 10 ? c - 10 : c;
         }
+        pl.n_nblocks = (N_tau + NT * pl.slide_rt - 1) / (NT * pl.slide_rt);
     }
     if (window == TFSTAT_WINDOW_RECT) {
         const int rm = opts ? opts->rect_method : 0;
@@ -347,12 +366,12 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.n_launches = 4;  // bounds, pack, sums + closure + marginals, finalize
     } else if (window == TFSTAT_WINDOW_EXP) {
         p.kernel = TFSTAT_KERNEL_EXP_SLIDE;
-        p.tile_c = pl.slide_tpc;
+        p.tile_c = pl.slide_tpc + (pl.slide_rt > 1 ? 10 : 0);
         p.tile_nt = pl.tile.NT;
         p.seg_len = pl.seg_len;
         p.n_segs = pl.n_segs;
         p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
-        p.n_launches = 4;
+        p.n_launches = 4;  // bounds, pack, window sums + slide + closure + marginals, finalize
     } else if (pl.rect_small) {
         p.kernel = TFSTAT_KERNEL_RECT_SMALL;
         p.tile_c = 1;

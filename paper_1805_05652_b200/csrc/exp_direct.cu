@@ -111,7 +111,14 @@ __device__ __forceinline__ void accumulate_cell(Acc<C> &acc, const int c, const 
 // mbarrier).  No thread moves atom data, and there is no CTA barrier in the loop: a warp waits
 // for its own data only, never for the other warps of the CTA (whose windows -- larger tau --
 // are longer).
-template <int C, int NT, int KW, int NS>
+//
+// SPLIT (single maps: too few CTAs to fill 148 SMs several times over): the NW warps of a CTA
+// share the SAME 32 tau values and split the atoms of their windows between them, chunk k to warp
+// k mod NW; their partial sums meet in shared memory at the end and the cells are closed by
+// the warps in turn.  Same arithmetic per term; a CTA's critical path is NW times shorter and
+// every warp of it carries the same load, so the tail of a small grid shrinks accordingly
+// (config 2: 0.176 -> see DESIGN.md 6.1).
+template <int C, int NT, int KW, int NS, bool SPLIT>
 __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
     exp_direct_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
                       Partial *__restrict__ partials, const int n_mtiles, const int n_nblocks)
@@ -134,11 +141,12 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
     // index (32 more tau values each): left alone, scheduler 0 of every SM would get the lightest
     // quarter of every resident CTA and scheduler NW-1 the heaviest.  Rotating the quarter a warp
     // takes with the CTA index evens the schedulers out.
-    const int tq = ((warp + (int)(blockIdx.x % NW)) % NW) * 32 + lane;  // tau slot in the CTA
-    // tau blocks: block 0 holds the N_tau % NT shortest windows (if any), the others are full
-    const int ragged = g.N_tau % NT;
-    const int n_first = (ragged && nb > 0) ? ragged + (nb - 1) * NT : nb * NT;
-    const int n_count = (ragged && nb == 0) ? ragged : NT;
+    const int tq = SPLIT ? lane : ((warp + (int)(blockIdx.x % NW)) % NW) * 32 + lane;  // tau slot
+    // tau blocks: block 0 holds the N_tau % TPB shortest windows (if any), the others are full
+    constexpr int TPB = SPLIT ? 32 : NT;  // tau values per CTA
+    const int ragged = g.N_tau % TPB;
+    const int n_first = (ragged && nb > 0) ? ragged + (nb - 1) * TPB : nb * TPB;
+    const int n_count = (ragged && nb == 0) ? ragged : TPB;
     const bool n_ok = tq < n_count;
     const int n = n_first + (n_ok ? tq : 0);
     const int m_last = min(m0 + C - 1, g.N_t0 - 1);  // cells beyond N_t0 duplicate the last one
@@ -173,13 +181,15 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
     const int warp_e = __reduce_max_sync(0xffffffffu, has_core ? ce : 0);
     const int q0 = warp_b / KW;
     const int nq = warp_e > warp_b ? (warp_e + KW - 1) / KW - q0 : 0;
+    constexpr int KSTEP = SPLIT ? NW : 1;  // this warp's chunks: k0, k0 + KSTEP, ...
+    const int k0 = SPLIT ? warp : 0;
     const ulonglong2 *__restrict__ rec = packed + (int64_t)tpl * n_pad * 2;
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s)
-            if (s < nq)
-                bulk_load(ring0 + s * kChunkBytes, rec + (int64_t)(q0 + s) * KW * 2, kChunkBytes,
-                          bar0 + 8 * s);
+            if (k0 + s * KSTEP < nq)
+                bulk_load(ring0 + s * kChunkBytes, rec + (int64_t)(q0 + k0 + s * KSTEP) * KW * 2,
+                          kChunkBytes, bar0 + 8 * s);
     }
 
     const long long t_ref = t0_of(g, m0);
@@ -197,6 +207,7 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
     // SLOWER than this plain predicated loop: twice the code, one short loop per step)
 #pragma unroll 1
     for (int ph = 0; ph < 2; ++ph) {
+        if (SPLIT && warp != (ph ? NW - 1 : 0)) continue;  // head: first warp, tail: last warp
         const int xb = has_core ? (ph ? ce : h0) : (ph ? h1 : h0);
         const int xe = has_core ? (ph ? h1 : cb) : h1;
         if (xb >= xe) continue;
@@ -225,33 +236,80 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
 
     // ---- core: atoms common to all C cells, streamed through the warp's ring ----------------
 #pragma unroll 1
-    for (int k = 0; k < nq; ++k) {
-        const int s = k % NS;
+    for (int k = k0, j = 0; k < nq; k += KSTEP, ++j) {
+        const int s = j % NS;
         const int cs = (q0 + k) * KW;  // first atom of the chunk
         // weight argument of atom i: dtc_i kexp + cexp, dtc_i relative to the chunk's time base
         const int tb = __ldg(bd.t + cs - cs % kPackBlock);
         const float cexp = (float)((long long)tb - t_ref) * kexp;
         const int x0 = max(cs, cb) - cs;
         const int x1 = has_core ? min(cs + KW, ce) - cs : x0;
-        mbar_wait(bar0 + 8 * s, (uint32_t)(k / NS) & 1u);
+        mbar_wait(bar0 + 8 * s, (uint32_t)(j / NS) & 1u);
         const ulonglong2 *__restrict__ slot = s_ring + s * (2 * KW);
 #pragma unroll kCoreUnroll
         for (int i = x0; i < x1; ++i)
             accumulate_core<C>(acc, slot[2 * i], slot[2 * i + 1], kexp, cexp);
         __syncwarp();  // every lane is done with the slot: refill it
-        if (lane == 0 && k + NS < nq)
-            bulk_load(ring0 + s * kChunkBytes, rec + (int64_t)(q0 + k + NS) * KW * 2, kChunkBytes,
-                      bar0 + 8 * s);
+        if (lane == 0 && k + NS * KSTEP < nq)
+            bulk_load(ring0 + s * kChunkBytes, rec + (int64_t)(q0 + k + NS * KSTEP) * KW * 2,
+                      kChunkBytes, bar0 + 8 * s);
     }
 
     // ---- a4 closure + a5 marginals ----------------------------------------------------------
     Marg mg;
     marg_init(mg);
     const int64_t map_base = (int64_t)tpl * g.N_t0 * g.N_tau;
-#pragma unroll
-    for (int c = 0; c < C; ++c) {
+    auto close_cell = [&](const int c, const float(&S)[7]) {
         const int m = m0 + c;
         if (n_ok && m < g.N_t0) {
+            const int lo_c = __ldg(bd.lo + m);
+            const int cnt = max(hi_index(bd, g, m, n) - lo_c, 0);
+            uint32_t fl;
+            // the sums carry the weight of the tile's first cell; eq. (7) does not care, and the
+            // fp64 redo of short ill-conditioned windows uses the cell's own t0
+            const float twoF = closure_2F_exp<false>(S[0], S[1], S[2], S[3], S[4], S[5], S[6], lo_c,
+                                                     cnt, pr.min_atoms, fl, base, ld, bd.t,
+                                                     t0_of(g, m), (double)tau_of(g, n));
+            const int32_t flat = m * g.N_tau + n;
+            if (pr.out_maps) pr.out_maps[map_base + flat] = twoF;
+            if (pr.out_flags) pr.out_flags[map_base + flat] = (uint8_t)fl;
+            if (!fl) marg_add(mg, twoF, flat);
+        }
+    };
+    constexpr int CP = (C + 1) / 2;
+    if (SPLIT) {
+        // the warps' partial sums meet in shared memory (the rings are done with), pair p of
+        // every channel is summed and closed by warp p mod NW
+        __syncthreads();
+        u64 *red = reinterpret_cast<u64 *>(smem_raw);  // [NW][7][CP][32]
+#pragma unroll
+        for (int k = 0; k < 7; ++k)
+#pragma unroll
+            for (int p = 0; p < CP; ++p) red[((warp * 7 + k) * CP + p) * 32 + lane] = acc.ch[k][p];
+        __syncthreads();
+#pragma unroll
+        for (int p = 0; p < CP; ++p) {
+            if (p % NW != warp) continue;
+            float S0[7], S1[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                float e = 0.0f, o = 0.0f;
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    float pe, po;
+                    unpack2(red[((w * 7 + k) * CP + p) * 32 + lane], pe, po);
+                    e += pe;
+                    o += po;
+                }
+                S0[k] = e;
+                S1[k] = o;
+            }
+            close_cell(2 * p, S0);
+            if (2 * p + 1 < C) close_cell(2 * p + 1, S1);
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
             float S[7];
 #pragma unroll
             for (int k = 0; k < 7; ++k) {
@@ -259,20 +317,7 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
                 unpack2(acc.ch[k][c / 2], e, o);
                 S[k] = (c & 1) ? o : e;
             }
-            const float A = S[0], B = S[1], Cc = S[2], far = S[3], fai = S[4], fbr = S[5],
-                        fbi = S[6];
-            const int lo_c = __ldg(bd.lo + m);
-            const int cnt = max(hi_index(bd, g, m, n) - lo_c, 0);
-            uint32_t fl;
-            // the sums carry the weight of the tile's first cell; eq. (7) does not care, and the
-            // fp64 redo of short ill-conditioned windows uses the cell's own t0
-            const float twoF = closure_2F_exp<false>(A, B, Cc, far, fai, fbr, fbi, lo_c, cnt,
-                                              pr.min_atoms, fl, base, ld, bd.t, t0_of(g, m),
-                                              (double)tau_of(g, n));
-            const int32_t flat = m * g.N_tau + n;
-            if (pr.out_maps) pr.out_maps[map_base + flat] = twoF;
-            if (pr.out_flags) pr.out_flags[map_base + flat] = (uint8_t)fl;
-            if (!fl) marg_add(mg, twoF, flat);
+            close_cell(c, S);
         }
     }
     if (partials) {
@@ -286,13 +331,21 @@ cudaError_t launch_one(const Plan &pl, const Problem &pr, const void *packed, Pa
                        cudaStream_t st)
 {
     const int64_t n_ctas = pl.tiles_per_template * pl.n_templates;
-    auto kern = exp_direct_kernel<C, NT, kChunkAtoms, kStages>;
     const size_t smem = (size_t)(NT / 32) * kStages * 2 * kChunkAtoms * sizeof(ulonglong2);
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    return launch_pdl(kern, (unsigned)n_ctas, NT, smem, st,
-                      pr, static_cast<const ulonglong2 *>(packed), pl.n_pad, partials, pl.n_mtiles,
-                      pl.n_nblocks);
+    auto go = [&](auto kern) -> cudaError_t {
+        cudaError_t e =
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        return launch_pdl(kern, (unsigned)n_ctas, NT, smem, st, pr,
+                          static_cast<const ulonglong2 *>(packed), pl.n_pad, partials, pl.n_mtiles,
+                          pl.n_nblocks);
+    };
+    if constexpr (C <= 8 && NT == 128) {  // the partial sums of the split form fit in the rings
+        static_assert((size_t)(NT / 32) * 7 * ((C + 1) / 2) * 32 * 8 <=
+                      (size_t)(NT / 32) * kStages * 2 * kChunkAtoms * sizeof(ulonglong2));
+        if (pl.tile.split) return go(exp_direct_kernel<C, NT, kChunkAtoms, kStages, true>);
+    }
+    return go(exp_direct_kernel<C, NT, kChunkAtoms, kStages, false>);
 }
 
 template <int C>

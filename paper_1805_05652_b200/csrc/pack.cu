@@ -10,7 +10,8 @@
 // first atom of its block of kPackBlock atoms, exact in fp32 while a block spans < 2^24 s (194
 // days).  A kernel turns it into its own weight argument with one FMA:
 //     (t_i - t_ref) k = dtc_i k + c,   c = (t_{block(i)} - t_ref) k   (per thread and block),
-// the same instruction count as the multiply it replaces.
+// the same instruction count as the multiply it replaces.  Atoms that are not finite become
+// dtc = NaN with zero channels (see below).
 #include "plan.h"
 
 namespace tfstat {
@@ -31,11 +32,27 @@ __global__ void __launch_bounds__(kPackNT)
         ulonglong2 ra = make_ulonglong2(0ull, 0ull), rb = ra;  // padding: zeros, never summed
         if (i < n_atoms) {
             const float *__restrict__ base = atoms + (int64_t)tpl * template_stride + i;
-            const float dtc = (float)((long long)__ldg(t + i) - (long long)__ldg(t + i - i % kPackBlock));
-            ra.x = pack2(dtc, __ldg(base + 2 * ld));
-            ra.y = pack2(__ldg(base), __ldg(base + ld));
-            rb.x = pack2(__ldg(base + 3 * ld), __ldg(base + 4 * ld));
-            rb.y = pack2(__ldg(base + 5 * ld), __ldg(base + 6 * ld));
+            float dtc = (float)((long long)__ldg(t + i) - (long long)__ldg(t + i - i % kPackBlock));
+            float x[7];
+            bool bad = false;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                x[k] = __ldg(base + k * ld);
+                bad = bad || !(fabsf(x[k]) < INFINITY);
+            }
+            // An atom that is not finite (a bad SFT) is stored as dtc = NaN with zero channels:
+            // its WEIGHT is then NaN in every window that holds it (those cells are flagged
+            // D <= 0, as in the oracle), while a kernel that masks atoms outside a window with a
+            // zero weight gets 0 x 0 = 0 there, not 0 x NaN.
+            if (bad) {
+                dtc = nanf("");
+#pragma unroll
+                for (int k = 0; k < 7; ++k) x[k] = 0.0f;
+            }
+            ra.x = pack2(dtc, x[2]);
+            ra.y = pack2(x[0], x[1]);
+            rb.x = pack2(x[3], x[4]);
+            rb.y = pack2(x[5], x[6]);
         }
         ulonglong2 *__restrict__ dst = rec + ((int64_t)tpl * n_pad + i) * 2;
         dst[0] = ra;

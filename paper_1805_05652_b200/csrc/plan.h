@@ -28,6 +28,7 @@ inline int64_t gcd64(int64_t a, int64_t b)
 struct ExpTile {
     int C;
     int NT;
+    int split;  // 1: the warps of a CTA share 32 tau values and split the windows' atoms
 };
 
 // rect running-sum kernel (rect.cu): a thread owns Q rows m, m+r, ..; a CTA owns NTu residues
@@ -57,6 +58,7 @@ struct Plan {
     // exp sliding form (exp_scan.cu): t0 segments per (template, tau block)
     int32_t n_segs, seg_len;
     int32_t slide_tpc;  // templates per CTA (1, 2, 4): they share the weights
+    int32_t slide_rt;   // tau values per thread (1, 2): they share the atom loads
     // rect / marginalise tiling
     int32_t cell_blocks_per_template;
     RectRun rect;
