@@ -33,7 +33,16 @@ WORKLOAD = "cfg4_search_4096x2880atoms_96x1417"
 # + 7 FFMA (A,B,C,Re/Im Fa,Re/Im Fb) on the FP32 pipe, + 1 MUFU.EX2 on the XU pipe
 FP32_OPS_PER_TERM = 9
 FP32_LANES_PER_CLK_SM = 128  # cc 10.0: 4 SMSPs x 32 FP32 lanes
-NCU_DRAM_BYTES_PER_TEMPLATE = 23.976704e6 / 296  # profiles/r01_pass4_kernels_full.md
+# dram__bytes_read.sum + dram__bytes_write.sum of exp_direct_kernel, 296 templates of config 4
+NCU_CAPTURE = "profiles/r02_exp_direct_full.md"
+NCU_DRAM_BYTES_PER_TEMPLATE = (51.314944e6 + 2.098432e6) / 296
+PACK_BLOCK = 768  # kPackBlock of csrc/tfstat_dev.cuh: packed records are padded to whole blocks
+
+
+def plan_packed_bytes(n_atoms: int, n_templates: int) -> int:
+    """Bytes of packed atom records (32 B per atom) the exponential-window kernels stream."""
+    n_pad = (n_atoms + PACK_BLOCK - 1) // PACK_BLOCK * PACK_BLOCK
+    return 32 * n_pad * n_templates
 
 
 def read_peaks():
@@ -130,7 +139,8 @@ def run_reference(args):
 
     cores = oracle.num_threads()
     n_tpl = max(1, min(cores, 16))  # one template (2.6e8 terms, a few seconds) per core
-    for _ in range(args.warmup if args.warmup < 1 else 1):
+    n_warm = min(args.warmup, 1)  # one 1-template pass (pages in the library and the inputs);
+    for _ in range(n_warm):        # more would only burn host-core minutes: nothing here is cached
         oracle_leg(1)
     times, terms = [], 0
     for s in range(args.steps):
@@ -142,7 +152,8 @@ def run_reference(args):
               f"{terms:.3e} terms), OpenMP over templates")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "steps": args.steps, "warmup": n_warm, "warmup_requested": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": min(cores, n_tpl),
@@ -460,9 +471,10 @@ def run_ours(args):
     # "the roofline fraction is always computed from the executed mix, while
     # terms/s always uses the A.6 count" -- so `achieved` / `frac` are the executed ones (<= 1 by
     # construction) and the 9-op algorithmic figures are given beside them (they can exceed 1).
-    # C as chosen by make_plan (csrc/api.cu): 8 if that fills 148 SMs x 4 CTAs 8 times over.
-    n_ctas8 = ((grid.N_t0 + 7) // 8) * ((grid.N_tau + 127) // 128) * n_tpl
-    tile_c = 8 if n_ctas8 >= 8 * 148 * 4 else 4
+    # C is what the library ran (tfstat_plan_info), not a copy of its rule.
+    plan = pkg.plan_info(pkg.EXP, int(t.shape[0]), n_tpl, grid, exp_method=pkg.EXP_DIRECT)
+    assert plan["kernel_name"] == "exp_direct"
+    tile_c = plan["tile_c"]
     exec_ops_per_term = 7.0 + 2.0 / tile_c
     ach_ops = terms * exec_ops_per_term / (k_ms * 1e-3)
     alg_ops = terms * FP32_OPS_PER_TERM / (k_ms * 1e-3)
@@ -485,12 +497,14 @@ def run_ours(args):
         ((clocks or {}).get("sm_mhz") or peaks["sm_max_mhz"]) / 1e6,
         "measured_ffma_lane_ops_per_s": probes["ffma"]["lane_ops_per_s"],
         "frac_of_measured_ffma": ach_ops / probes["ffma"]["lane_ops_per_s"],
-        # dram__bytes_read.sum + dram__bytes_write.sum of exp_direct_kernel from the ncu --set full
-        # capture in profiles/r01_pass4_kernels_full.md (23.98 MB for 296 templates, written
-        # bytes 0), scaled per template to this launch
+        # NOT measured in this run: dram__bytes_read.sum + dram__bytes_write.sum of the kernel in
+        # the ncu --set full capture NCU_CAPTURE (296 templates), scaled per template to this launch
         "traffic": NCU_DRAM_BYTES_PER_TEMPLATE * n_tpl,
-        "traffic_unit": "bytes per launch (ncu capture of 296 templates, scaled per template)",
-        "algorithmic_bytes": int(atoms.numel() * 4 + t.numel() * 4),
+        "traffic_unit": f"bytes per launch, scaled per template from the capture {NCU_CAPTURE}",
+        "algorithmic_bytes": int(plan_packed_bytes(int(t.shape[0]), n_tpl)),
+        "algorithmic_bytes_note": "the kernel reads the PACKED records (32 B per atom, padded to "
+                                  "768 atoms); pack_atoms_kernel reads the caller's 28 B + writes them",
+        "plan": plan,
         "probes_ops_per_clk_sm": {k: round(v["ops_per_clk_sm"], 2) for k, v in probes.items()},
         "probe_sm_mhz": round(probes["ffma"]["sm_mhz"], 1),
     }
@@ -538,6 +552,35 @@ def run_ours(args):
         side["cfg4_exp_scan_e2e_host_buffers"] = {
             "ms_per_step": ms_s_e2e, "effective_terms_per_s": terms / (ms_s_e2e * 1e-3),
             "h2d_GBps": h2d / (ms_s_e2e * 1e-3) / 1e9}
+        # roofline of the path a caller gets by default (EXP_AUTO = the sliding form): the weighted
+        # terms the kernel EXECUTED, counted by the kernel itself (tfstat_opts.stats, in a separate
+        # untimed call), as FP32 lane-ops: 7 multiply-adds per term, 2 per weight (its argument
+        # and E^2; the MUFU.EX2 runs on the XU pipe) shared by the templates of a CTA, and the
+        # fp32 closure + marginal update per cell (23 lane-ops: csrc/tfstat_dev.cuh)
+        plan_s = pkg.plan_info(pkg.EXP, int(t.shape[0]), n_tpl, grid, exp_method=pkg.EXP_SCAN)
+        st = torch.zeros(pkg.binding.N_STATS, dtype=torch.int64, device="cuda")
+        pkg.tfstat_search(atoms, t, pkg.EXP, grid, exp_method=pkg.EXP_SCAN, stats=st)
+        stv = dict(zip(pkg.binding.STAT_NAMES, (int(x) for x in st.cpu().numpy())))
+        ev_s = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+        ev_s[0].record(), ev_s[1].record()
+        pkg.tfstat_search(atoms, t, pkg.EXP, grid, workspace=ws_s, out=out_s,
+                          exp_method=pkg.EXP_SCAN, main_kernel_events=ev_s)
+        torch.cuda.synchronize()
+        k_ms_s = ev_s[0].elapsed_time(ev_s[1])
+        tpc = plan_s["tile_c"] % 10
+        w_terms = (stv["terms_window"] + stv["terms_enter"] + stv["terms_leave"] +
+                   stv["terms_resum"])
+        lane_ops = 7.0 * w_terms + 2.0 * w_terms / tpc + 23.0 * stv["cells"]
+        packed_b = plan_packed_bytes(int(t.shape[0]), n_tpl)
+        side["cfg4_exp_scan_roofline"] = {
+            "bound": "alu", "kernel": "exp_slide_kernel", "kernel_ms": k_ms_s,
+            "executed": stv, "weighted_terms": w_terms, "templates_per_cta": tpc,
+            "executed_fp32_lane_ops": lane_ops,
+            "achieved": lane_ops / (k_ms_s * 1e-3) / 1e12, "peak": peak_ops / 1e12,
+            "unit": "T FP32 lane-op/s", "frac": lane_ops / (k_ms_s * 1e-3) / peak_ops,
+            "hbm_floor_us": packed_b / (peaks["hbm_gbs"] * 1e9) * 1e6,
+            "hbm_frac": packed_b / (k_ms_s * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "terms_vs_direct": terms / max(w_terms, 1), "plan": plan_s}
         side["cfg4_exp_scan"] = {"ms_per_step": ms_s, "effective_terms_per_s": terms / (ms_s * 1e-3),
                                  "speedup_vs_direct": ms_per_step / ms_s,
                                  "max_rel_diff_max2F_vs_direct": dmax,
@@ -557,7 +600,7 @@ def run_ours(args):
         "cells_per_s": cells * world / (ms_per_step * 1e-3),
         "e2e": {"value": terms * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
-        "gpu_launches": 3 * args.steps,
+        "gpu_launches": plan["n_launches"] * args.steps,
         "roofline": roofline,
         "cpu_baseline": cpu,
         "clocks": clocks,

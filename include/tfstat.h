@@ -278,7 +278,8 @@ int tfstat_merge_detectors(const float *const *atoms_dets, const int64_t *templa
  * copy-out without the per-template round trip.
  *   atoms_host, t_atoms_host, out_host, out_maps_host (nullable): HOST pointers, layouts as
  *   in tfstat_search.
- *   device_scratch: DEVICE buffer of device_scratch_bytes bytes (256-B aligned) that holds the
+ *   device_scratch: DEVICE buffer of device_scratch_bytes bytes (256-B aligned; not in use by
+ *   work still running on any stream of the caller: the library uses streams of its own) that holds the
  *   double-buffered chunks, the workspace and the results.  Any size from one template's worth
  *   up works (smaller => more, smaller chunks); tfstat_search_host_scratch_bytes() gives the
  *   size for the preferred chunks.  NULL: the library cudaMallocs up to

@@ -458,6 +458,11 @@ def tfstat_search_host(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, 
     maps = (torch.empty((T, grid.N_t0, grid.N_tau), dtype=torch.float32).pin_memory()
             if want_maps else None)
     o = _opts(min_atoms, exp_method)
+    # The library works on streams of its own and returns when everything has completed.  A torch
+    # scratch tensor may be a block the caching allocator has just taken back from work that is
+    # still running on the current stream (e.g. the workspace of an earlier tfstat_search):
+    # stream-ordered reuse is only safe on that stream, so let it drain first.
+    torch.cuda.current_stream().synchronize()
     if library_malloc:
         rc = lib.tfstat_search_host(atoms.data_ptr(), int(atoms.stride(0)), int(atoms.stride(1)),
                                     t_atoms.data_ptr(), n_atoms, T, window, *_grid_args(grid),

@@ -26,3 +26,15 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(autouse=True)
+def _device_errors_belong_to_their_test(request):
+    """A kernel fault is reported asynchronously, at the next synchronising call: without this, a
+    fault in one GPU test would surface in (and be blamed on) a later one."""
+    yield
+    if "gpu" in request.keywords:
+        import torch
+
+        if torch.cuda.is_available():
+            torch.cuda.synchronize()
