@@ -35,6 +35,7 @@ struct ExpTile {
 // x 128 / NTu row groups x seg_cols columns
 struct RectRun {
     int32_t enabled;  // 0: per-cell kernel (no edge lattice / very few rows)
+    int32_t tile;     // 1: direct form by tiles (rect_tile_kernel); r = row offset, NTu = column offset
     int32_t Q, r, NTu, seg_cols, n_rowtiles, n_coltiles;
     int32_t ks_lg;   // >= 0: the staged run is stored in two halves of runs of 2^ks_lg entries
     int32_t ks_cap;  // lattice points of K one CTA stages in shared memory (0: K read through L1)

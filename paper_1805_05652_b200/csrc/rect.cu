@@ -976,6 +976,397 @@ __global__ void __launch_bounds__(kRunNT, 8)
     }
 }
 
+
+// ---------------------------------------------------------------------------------------
+// rect_tile_kernel: the rectangular map in its DIRECT form, tile by tile, for grids whose lattice
+// steps are small (dt0 and dtau within a factor 4 of each other: the paper's full-resolution
+// setups).
+//
+// Every cell is S(m, n) = P[hi(m, n)] - P[lo_m].  A CTA owns TR rows x TC columns and picks an
+// anchor atom a at the low end of its window ENDS; in fp64 it stages, once,
+//     Phi[j] = P[edge[j]] - P[a]   for the few hundred lattice points j the tile touches, and
+//     U[m]   = P[a] - P[lo_m]      for its rows,
+// rounded to fp32 (32 bytes each).  A cell is then Phi[j(m, n)] + U[m]: 8 additions, no running
+// sum, no dependency between cells, no restart.  As long as the anchor lies inside the window
+// (lo_m <= a <= hi) both terms are partial sums of the window and the fp32 rounding is that of
+// the window's own sums; where it does not (short windows in the first column tile) the cell is
+// sent to the fp64 path whenever the sum is smaller than an eighth of the larger term.
+//
+// The cells (m, n) and (m + r, n - c) with r e_m = c e_n sit on the SAME lattice point: a thread
+// takes them as one packed pair -- Phi is a broadcast operand, U a row pair -- and closes them
+// with the packed eq. (7) of pair_closure.  Lanes run along n, so both cells of a pair are stored
+// by plain coalesced 128-byte warp stores: no shared-memory transpose, no barrier in the loop.
+// Per cell: 16 bytes of shared-memory reads (the running-sum kernel: 32 + the transpose).
+// ---------------------------------------------------------------------------------------
+constexpr int kTileNT = 128;
+constexpr int kTileNH = 1;                       // packed cell pairs per thread and lattice point
+constexpr int kTileCells = 2 * kTileNH;          // cells per thread and lattice point
+constexpr int kTileQuads = kTileNT / kTileCells;  // such groups of rows per CTA (128 rows)
+constexpr int kTileCols = 256;  // columns per CTA
+constexpr int kTileMaxRun = 1280;  // lattice points a tile may touch (40 KB of shared memory)
+constexpr float kTileSafeMag = 1073741824.0f;  // 2^30: below it eq. (7) cannot overflow in fp32
+constexpr float kAnchorGuard = 8.0f;
+constexpr int kTileGroup = 4 / kTileNH;  // column strips of a group summed as one straight-line block
+
+// eq. (7) for two cells on the tile kernel's channels: 0 A, 1 B, 2 C/2, 3 -2C, 4..7 sqrt2 (Re Fa,
+// Im Fa, Re Fb, Im Fb), so that D = A B + (-2C)(C/2) and the cross term is one multiply-add.
+// SAFE: every staged value of the CTA is below 2^30 in magnitude, so nothing can overflow and
+// the fast path holds where t = D - A B / 64 > kTiny (13 packed operations); otherwise t also
+// carries the -kTiny offset and the overflow poison of pair_closure.
+template <bool SAFE>
+__device__ __forceinline__ PairOut pair_closure_tile(const u64 (&S)[8])
+{
+    const u64 p = fmul2(S[0], S[1]);
+    u64 D = p;
+    ffma2(D, S[3], S[2]);
+    PairOut o;
+    o.t = SAFE ? D : fadd2(D, pack2(-kTiny, -kTiny));
+    ffma2(o.t, p, pack2(-kCondFast, -kCondFast));
+    u64 na = fmul2(S[4], S[4]);
+    ffma2(na, S[5], S[5]);
+    u64 nb = fmul2(S[6], S[6]);
+    ffma2(nb, S[7], S[7]);
+    u64 re = fmul2(S[4], S[6]);
+    ffma2(re, S[5], S[7]);
+    u64 num = fmul2(S[1], na);
+    ffma2(num, S[0], nb);
+    ffma2(num, S[3], re);
+    if (!SAFE) ffma2(o.t, fmul2(num, p), 0ull);
+    float d0, d1;
+    unpack2(D, d0, d1);
+    o.res = fmul2(num, pack2(rcp_approx(d0), rcp_approx(d1)));
+    return o;
+}
+
+// marginal update of one thread for two cells (values -inf where a cell does not count)
+__device__ __forceinline__ void tile_marg2(RunMarg &rm, const float x0, const float x1,
+                                           const int32_t flat0, const int32_t flat1)
+{
+    const float gmax = fmaxf(x0, x1);
+    if (gmax >= rm.best && gmax > -INFINITY) {
+        // rare: a new maximum, or an exact tie (the lowest flat index wins)
+        int32_t cand = 0x7fffffff;
+        if (x0 == gmax) cand = flat0;
+        if (x1 == gmax) cand = min(cand, flat1);
+        if (gmax > rm.best || cand < rm.idx) rm.idx = cand;
+        rm.best = gmax;
+    }
+    if (fmaf(gmax, kHalfLog2e, -rm.ref2) > 60.0f) {  // rare: move the reference
+        rm.sum *= ex2_approx(rm.ref2 - gmax * kHalfLog2e);
+        rm.ref2 = gmax * kHalfLog2e;
+    }
+    rm.sum += ex2_approx(fmaf(x0, kHalfLog2e, -rm.ref2)) + ex2_approx(fmaf(x1, kHalfLog2e, -rm.ref2));
+    rm.nv += (x0 > -INFINITY ? 1 : 0) + (x1 > -INFINITY ? 1 : 0);
+}
+
+// A thread's unit of work is a GROUP of kTileCells cells (m, n), (m + r, n - c), (m + 2r, n - 2c),
+// .. which all sit on the lattice point j = m e_m + n e_n, as kTileNH packed pairs that share one
+// Phi[j].  Measured on B200 (one-year map): one pair per thread 390 us (112 registers), two pairs
+// 400 us (128 registers: half the shared-memory wavefronts, but fewer independent eq. (7) chains
+// in flight and more address arithmetic per store).
+template <bool MARG, bool FLAGS, bool MAP>
+__global__ void __launch_bounds__(kTileNT, 4)
+    rect_tile_kernel(const Problem pr, const double *__restrict__ prefix,
+                     Partial *__restrict__ partials, const int r, const int c, const int n_rowtiles,
+                     const int n_coltiles)
+{
+    __shared__ __align__(16) float4 s_phiA[kTileMaxRun];  // A, B, C/2, -2C
+    __shared__ __align__(16) float4 s_phiB[kTileMaxRun];  // sqrt2 (Re Fa, Im Fa, Re Fb, Im Fb)
+    __shared__ __align__(16) u64 s_u[kTileQuads][kTileNH][8];  // channel pairs (U[m0], U[m1]), ..
+    __shared__ int s_nfirst[kTileQuads][kTileCells];              // first column with >= min_atoms atoms
+    __shared__ int s_row0[kTileQuads];                    // first row of quad q
+    __shared__ unsigned s_mag;                            // largest staged magnitude (float bits)
+    __shared__ Marg s_red[32];
+    pdl_trigger();
+    pdl_wait();  // rect_scan_kernel's prefix sums (and the bounds tables before it)
+
+    const Grid g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    const int rowtile = blockIdx.x % n_rowtiles;
+    const int coltile = (blockIdx.x / n_rowtiles) % n_coltiles;
+    const int tpl = blockIdx.x / (n_rowtiles * n_coltiles);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int m0 = rowtile * (kTileCells * kTileQuads);
+    const int n0 = coltile * kTileCols;
+    const double2 *__restrict__ P =
+        reinterpret_cast<const double2 *>(prefix + (int64_t)tpl * (bd.n_atoms + 1) * 8);
+
+    // ---- staging ---------------------------------------------------------------------------
+    // lattice points of the tile: those of the quads' first cells (m, n0 .. n0 + TC - 1)
+    const int j_lo = (int)min((int64_t)m0 * bd.e_m + (int64_t)n0 * bd.e_n, (int64_t)bd.J - 1);
+    const int j_hi = (int)min((int64_t)(m0 + kTileCells * kTileQuads - (kTileCells - 1) * r - 1) * bd.e_m +
+                                  (int64_t)(n0 + kTileCols - 1) * bd.e_n,
+                              (int64_t)bd.J - 1);
+    const int a = __ldg(bd.edge + j_lo);  // the anchor: the smallest window end of the tile
+    const double2 a0 = __ldg(P + (int64_t)a * 4), a1 = __ldg(P + (int64_t)a * 4 + 1),
+                  a2 = __ldg(P + (int64_t)a * 4 + 2), a3 = __ldg(P + (int64_t)a * 4 + 3);
+    // P[i] - P[a] as the 8 fp32 channels; NaN if a non-finite atom lies between the two
+    auto rel = [&](const int i, float(&v)[8]) {
+        const double2 h0 = __ldg(P + (int64_t)i * 4), h1 = __ldg(P + (int64_t)i * 4 + 1),
+                      h2 = __ldg(P + (int64_t)i * 4 + 2), h3 = __ldg(P + (int64_t)i * 4 + 3);
+        const double cc = h1.x - a1.x;
+        v[0] = (float)(h0.x - a0.x);
+        v[1] = (float)(h0.y - a0.y);
+        v[2] = (float)(0.5 * cc);
+        v[3] = (float)(-2.0 * cc);
+        v[4] = (float)(kSqrt2 * (h1.y - a1.y));
+        v[5] = (float)(kSqrt2 * (h2.x - a2.x));
+        v[6] = (float)(kSqrt2 * (h2.y - a2.y));
+        v[7] = (float)(kSqrt2 * (h3.x - a3.x));
+        if (fabs(h3.y - a3.y) > 0.5) v[0] = nanf("");  // a bad SFT in between: fp64 path decides
+    };
+    if (threadIdx.x == 0) s_mag = 0u;
+    unsigned mag_bits = 0u;  // (a NaN's bit pattern is above that of any finite value)
+    auto track = [&](const float(&v)[8]) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mag_bits = max(mag_bits, __float_as_uint(fabsf(v[k])));
+    };
+    static_assert(kTileCells * kTileQuads == kTileNT, "one thread per row of the tile");
+    {
+        // row of this thread: group q, member k4; U[m] = P[a] - P[lo_m]
+        const int q = threadIdx.x / kTileCells, k4 = threadIdx.x % kTileCells;
+        const int mq = m0 + (q / r) * kTileCells * r + q % r;
+        const int m = mq + k4 * r;
+        float v[8];
+        int nfirst = 0x7fffffff;  // rows outside the map: no cell
+        if (m < g.N_t0) {
+            const int lo = __ldg(bd.lo + m);
+            rel(lo, v);
+            track(v);
+            // first column of the row with at least min_atoms atoms (counts grow with n); mostly
+            // the very first one: a search only where it is not
+            int x = 0, e = g.N_tau;
+            if (__ldg(bd.edge + (int64_t)m * bd.e_m) - lo >= pr.min_atoms) e = 0;
+            while (x < e) {
+                const int mid = (x + e) >> 1;
+                const int cnt = __ldg(bd.edge + (int64_t)m * bd.e_m + (int64_t)mid * bd.e_n) - lo;
+                if (cnt < pr.min_atoms) x = mid + 1;
+                else e = mid;
+            }
+            nfirst = x;
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = 0.0f;
+            v[0] = v[1] = -1.0e15f;  // a dummy, perfectly conditioned row
+        }
+        float *u = reinterpret_cast<float *>(&s_u[q][k4 >> 1][0]);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) u[2 * k + (k4 & 1)] = -v[k];
+        s_nfirst[q][k4] = nfirst;
+        if (k4 == 0) s_row0[q] = mq;
+    }
+    for (int jj = threadIdx.x; jj <= j_hi - j_lo; jj += kTileNT) {
+        float v[8];
+        rel(__ldg(bd.edge + j_lo + jj), v);
+        track(v);
+        s_phiA[jj] = make_float4(v[0], v[1], v[2], v[3]);
+        s_phiB[jj] = make_float4(v[4], v[5], v[6], v[7]);
+    }
+    mag_bits = __reduce_max_sync(0xffffffffu, mag_bits);
+    __syncthreads();  // s_mag = 0 is in place
+    if (lane == 0) atomicMax(&s_mag, mag_bits);
+    __syncthreads();
+    const bool mag_ok = s_mag <= __float_as_uint(kTileSafeMag);
+
+    // ---- cells -------------------------------------------------------------------------------
+    RunMarg rm;
+    rm.best = -INFINITY;
+    rm.idx = 0x7fffffff;
+    rm.ref2 = -1.0e30f;
+    rm.sum = 0.0f;
+    rm.nv = 0;
+    const int64_t map_base = (int64_t)tpl * g.N_t0 * g.N_tau;
+    float *__restrict__ const maps = MAP ? pr.out_maps + map_base : nullptr;
+    uint8_t *__restrict__ const flg = FLAGS ? pr.out_flags + map_base : nullptr;
+    constexpr int n_strips = kTileCols / 32;
+    // every cell of the tile lies inside the map
+    const bool interior =
+        m0 + kTileCells * kTileQuads <= g.N_t0 && n0 - (kTileCells - 1) * c >= 0 &&
+        n0 + kTileCols <= g.N_tau;
+    // a warp takes quads warp, warp + 4, ..: U and the row addresses stay in registers while it
+    // walks the quad's column strips
+#pragma unroll 1
+    for (int q = warp; q < kTileQuads; q += kTileNT / 32) {
+        const int mq = s_row0[q];
+        if (mq >= g.N_t0) continue;
+        u64 U[kTileNH][8];
+#pragma unroll
+        for (int h = 0; h < kTileNH; ++h)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) U[h][k] = s_u[q][h][k];
+        float ua[kTileCells];
+#pragma unroll
+        for (int h = 0; h < kTileNH; ++h) unpack2(U[h][0], ua[2 * h], ua[2 * h + 1]);
+        int nf[kTileCells];
+#pragma unroll
+        for (int k = 0; k < kTileCells; ++k) nf[k] = s_nfirst[q][k];
+        const int jl = (int)((int64_t)mq * bd.e_m + (int64_t)n0 * bd.e_n - j_lo) + lane * bd.e_n;
+        int32_t flat0[kTileCells];  // flat index of the group's cells at strip 0
+#pragma unroll
+        for (int k = 0; k < kTileCells; ++k) flat0[k] = (mq + k * r) * g.N_tau + n0 - k * c + lane;
+        // lean: interior tile, values in range, the anchor inside every window of the quad
+        // (U >= 0: lo_m <= a), and enough atoms from the tile's first column on
+        bool lean = interior && mag_ok;
+#pragma unroll
+        for (int k = 0; k < kTileCells; ++k) lean = lean && ua[k] >= 0.0f && nf[k] <= n0 - k * c;
+        if (lean) {
+            // kTileGroup strips of the quad as ONE straight-line block: their eq. (7) chains are
+            // independent and interleave (a branch per strip would fence them off from one
+            // another); the rare cells that fail the conditioning test are redone afterwards
+#pragma unroll 1
+            for (int s0 = 0; s0 < n_strips; s0 += kTileGroup) {
+                float res[kTileGroup][kTileCells];
+                uint32_t slow = 0u;
+                const int jg = jl + 32 * s0 * bd.e_n;
+#pragma unroll
+                for (int strip = 0; strip < kTileGroup; ++strip) {
+                    const int jj = jg + 32 * strip * bd.e_n;
+                    const float4 fa = s_phiA[jj], fb = s_phiB[jj];
+                    const u64 ph[8] = {pack2(fa.x, fa.x), pack2(fa.y, fa.y), pack2(fa.z, fa.z),
+                                       pack2(fa.w, fa.w), pack2(fb.x, fb.x), pack2(fb.y, fb.y),
+                                       pack2(fb.z, fb.z), pack2(fb.w, fb.w)};
+#pragma unroll
+                    for (int h = 0; h < kTileNH; ++h) {
+                        u64 S[8];
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) S[k] = fadd2(ph[k], U[h][k]);
+                        const PairOut o = pair_closure_tile<true>(S);
+                        float t0, t1;
+                        unpack2(o.res, res[strip][2 * h], res[strip][2 * h + 1]);
+                        unpack2(o.t, t0, t1);
+                        slow |= ((t0 > kTiny ? 0u : 1u) | (t1 > kTiny ? 0u : 2u)) << (kTileCells * strip + 2 * h);
+                    }
+                }
+                uint32_t fl = 0u;  // D <= 0 / count flags of the redone cells, 2 bits per cell
+                if (slow) {  // rare: the plain way, in fp64 from P
+#pragma unroll
+                    for (int strip = 0; strip < kTileGroup; ++strip) {
+                        const int64_t j = (int64_t)j_lo + jg + 32 * strip * bd.e_n;
+#pragma unroll
+                        for (int k = 0; k < kTileCells; ++k) {
+                            if (slow & (1u << (kTileCells * strip + k))) {
+                                float flf;
+                                unpack2(rect_cell_slow(P, bd.lo, bd.edge, mq + k * r, j,
+                                                       pr.min_atoms),
+                                        res[strip][k], flf);
+                                fl |= (__float_as_uint(flf) & 3u) << (2 * (kTileCells * strip + k));
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int strip = 0; strip < kTileGroup; ++strip) {
+                    float x[kTileCells];
+#pragma unroll
+                    for (int k = 0; k < kTileCells; ++k) {
+                        const int32_t flat = flat0[k] + 32 * (s0 + strip);
+                        const uint32_t f = (fl >> (2 * (kTileCells * strip + k))) & 3u;
+                        if (MAP) __stcs(maps + flat, res[strip][k]);
+                        if (FLAGS) flg[flat] = (uint8_t)f;
+                        x[k] = f ? -INFINITY : res[strip][k];
+                    }
+                    if (MARG) {
+#pragma unroll
+                        for (int h = 0; h < kTileNH; ++h)
+                            tile_marg2(rm, x[2 * h], x[2 * h + 1], flat0[2 * h] + 32 * (s0 + strip),
+                                       flat0[2 * h + 1] + 32 * (s0 + strip));
+                    }
+                }
+            }
+        } else {
+            // edge tiles, short windows, values far from unity: every cell is tested for being
+            // inside the map, for its atom count and for an anchor outside its window
+#pragma unroll 1
+            for (int strip = 0; strip < n_strips; ++strip) {
+                const int n = n0 + 32 * strip + lane;
+                if (n0 + 32 * strip - (kTileCells - 1) * c >= g.N_tau) break;  // beyond the map
+                const int jj = min(jl + 32 * strip * bd.e_n, j_hi - j_lo);
+                const int64_t j = (int64_t)mq * bd.e_m + (int64_t)n * bd.e_n;
+                const float4 fa = s_phiA[jj], fb = s_phiB[jj];
+                const u64 ph[8] = {pack2(fa.x, fa.x), pack2(fa.y, fa.y), pack2(fa.z, fa.z),
+                                   pack2(fa.w, fa.w), pack2(fb.x, fb.x), pack2(fb.y, fb.y),
+                                   pack2(fb.z, fb.z), pack2(fb.w, fb.w)};
+                float x[kTileCells];
+#pragma unroll
+                for (int h = 0; h < kTileNH; ++h) {
+                    u64 S[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) S[k] = fadd2(ph[k], U[h][k]);
+                    const PairOut o = pair_closure_tile<false>(S);
+                    float rr[2], tt[2], sa[2];
+                    unpack2(o.res, rr[0], rr[1]);
+                    unpack2(o.t, tt[0], tt[1]);
+                    unpack2(S[0], sa[0], sa[1]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int k = 2 * h + e;
+                        const int m = mq + k * r, nk = n - k * c;
+                        const bool ok = m < g.N_t0 && nk >= 0 && nk < g.N_tau;
+                        // an anchor outside the window: the sum must not be a small difference
+                        // of the two terms
+                        const bool fast = tt[e] > 0.0f && nk >= nf[k] &&
+                                          sa[e] * kAnchorGuard >= fmaxf(fabsf(fa.x), fabsf(ua[k]));
+                        uint32_t f = 0u;
+                        if (ok && !fast) {  // the plain way, in fp64 from P
+                            float flf;
+                            unpack2(rect_cell_slow(P, bd.lo, bd.edge, m, j, pr.min_atoms), rr[e],
+                                    flf);
+                            f = __float_as_uint(flf);
+                        }
+                        const int32_t flat = flat0[k] + 32 * strip;
+                        if (ok) {
+                            if (MAP) __stcs(maps + flat, rr[e]);
+                            if (FLAGS) flg[flat] = (uint8_t)f;
+                        }
+                        x[k] = (ok && f == 0u) ? rr[e] : -INFINITY;
+                    }
+                }
+                if (MARG) {
+#pragma unroll
+                    for (int h = 0; h < kTileNH; ++h)
+                        tile_marg2(rm, x[2 * h], x[2 * h + 1], flat0[2 * h] + 32 * strip,
+                                   flat0[2 * h + 1] + 32 * strip);
+                }
+            }
+        }
+    }
+    if (MARG) {
+        Marg mg;
+        marg_init(mg);
+        if (rm.nv > 0) {
+            mg.best = rm.best;
+            mg.idx = rm.idx;
+            mg.M = 0.5f * rm.best;
+            mg.S = rm.sum * ex2_approx(rm.ref2 - rm.best * kHalfLog2e);
+            mg.nvalid = rm.nv;
+        }
+        marg_block_reduce<kTileNT>(mg, s_red);
+        if (threadIdx.x == 0) partial_store(partials + blockIdx.x, mg);
+    }
+}
+
+cudaError_t launch_tile(const Plan &pl, const Problem &pr, const double *prefix, Partial *partials,
+                        cudaStream_t st)
+{
+    const RectRun &rr = pl.rect;
+    const int64_t n_ctas = (int64_t)rr.n_rowtiles * rr.n_coltiles * pl.n_templates;
+    auto go = [&](auto kern) {
+        return launch_pdl(kern, (unsigned)n_ctas, kTileNT, 0, st, pr, prefix, partials, rr.r, rr.NTu,
+                          rr.n_rowtiles, rr.n_coltiles);
+    };
+    if (pr.out_flags) {
+        if (pr.out_maps)
+            return partials ? go(rect_tile_kernel<true, true, true>)
+                            : go(rect_tile_kernel<false, true, true>);
+        return partials ? go(rect_tile_kernel<true, true, false>)
+                        : go(rect_tile_kernel<false, true, false>);
+    }
+    if (pr.out_maps)
+        return partials ? go(rect_tile_kernel<true, false, true>)
+                        : go(rect_tile_kernel<false, false, true>);
+    return go(rect_tile_kernel<true, false, false>);
+}
+
 template <int Q>
 cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
                        const ulonglong2 *K, Partial *partials, cudaStream_t st)
@@ -1012,6 +1403,31 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
 {
     RectRun rr;
     rr.enabled = (J > 0 && g.N_t0 >= 8) ? 1 : 0;
+    rr.tile = 0;
+    // direct form, tile by tile (rect_tile_kernel): lattice steps small enough for a tile's run of
+    // lattice points to sit in shared memory; seg_override < 0 keeps the running-sum kernel
+    if (rr.enabled && e_m >= 1 && e_n >= 1 && e_m <= 4 && e_n <= 4 && seg_override >= 0 &&
+        q_override == 0 && (kTileQuads % e_n) == 0 &&
+        (int64_t)(kTileCells * kTileQuads - (kTileCells - 1) * e_n - 1) * e_m +
+                (int64_t)(kTileCols - 1) * e_n + 1 <=
+            kTileMaxRun) {
+        const int64_t n_rt = (g.N_t0 + kTileCells * kTileQuads - 1) / (kTileCells * kTileQuads);
+        const int64_t n_ct = (g.N_tau + (kTileCells - 1) * e_m + kTileCols - 1) / kTileCols;
+        // (a small map gives too few 128 x 256 tiles to fill 148 SMs: config 3's 96 x 5736 cells
+        // are 23 tiles, 58 us against 44 us for the running-sum kernel)
+        if (n_rt * n_ct * n_templates >= 2 * 148) rr.tile = 1;
+    }
+    if (rr.tile) {
+        rr.Q = kTileCells;
+        rr.r = e_n;    // rows m, m + r, ...
+        rr.NTu = e_m;  // ... meet on one lattice point, c = e_m columns apart each
+        rr.seg_cols = kTileCols;
+        rr.n_rowtiles = (g.N_t0 + kTileCells * kTileQuads - 1) / (kTileCells * kTileQuads);
+        rr.n_coltiles = (g.N_tau + (kTileCells - 1) * e_m + kTileCols - 1) / kTileCols;
+        rr.ks_cap = 0;
+        rr.ks_lg = -1;
+        return rr;
+    }
     rr.Q = 1;
     rr.r = 1;
     bool perm_ok = false;
@@ -1112,7 +1528,7 @@ cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st
     return cudaGetLastError();
 }
 
-int rect_run_threads(const Plan &) { return kRunNT; }
+int rect_run_threads(const Plan &pl) { return pl.rect.tile ? kTileNT : kRunNT; }
 
 int rect_scan_blocks(int32_t n_atoms) { return (n_atoms + kScanBlock - 1) / kScanBlock; }
 
@@ -1124,7 +1540,8 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
     const int nblk = rect_scan_blocks(pl.n_atoms);
     const int n_scan = nblk * pl.n_templates;
     ulonglong2 *K = static_cast<ulonglong2 *>(steps);
-    const int spt = pl.rect.enabled ? (int)((pl.J + 1 + kStepPts - 1) / kStepPts) : 0;
+    // (the tile kernel works from P alone: no step table)
+    const int spt = pl.rect.enabled && !pl.rect.tile ? (int)((pl.J + 1 + kStepPts - 1) / kStepPts) : 0;
     const int64_t n_blocks = (int64_t)n_scan + (int64_t)spt * pl.n_templates;
     cudaError_t e = launch_pdl(rect_scan_kernel, (unsigned)n_blocks, kScanNT, 0, st, pr, agg, flags,
                                prefix, K, nblk, n_scan, spt);
@@ -1134,6 +1551,7 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
         return launch_pdl(rect_cells_kernel, (unsigned)n_ctas, kCellNT, 0, st, pr, prefix, partials,
                           pl.cell_blocks_per_template);
     }
+    if (pl.rect.tile) return launch_tile(pl, pr, prefix, partials, st);
     if (pl.rect.Q == 2) return launch_run<2>(pl, pr, prefix, K, partials, st);
     return launch_run<1>(pl, pr, prefix, K, partials, st);
 }
