@@ -1003,7 +1003,7 @@ constexpr int kTileNH = 1;                       // packed cell pairs per thread
 constexpr int kTileCells = 2 * kTileNH;          // cells per thread and lattice point
 constexpr int kTileQuads = kTileNT / kTileCells;  // such groups of rows per CTA (128 rows)
 constexpr int kTileCols = 256;  // columns per CTA
-constexpr int kTileMaxRun = 1280;  // lattice points a tile may touch (40 KB of shared memory)
+constexpr int kTileMaxRun = 768;  // lattice points a tile may touch (24 KB of shared memory)
 constexpr float kTileSafeMag = 1073741824.0f;  // 2^30: below it eq. (7) cannot overflow in fp32
 constexpr float kAnchorGuard = 8.0f;
 constexpr int kTileGroup = 4 / kTileNH;  // column strips of a group summed as one straight-line block
@@ -1065,7 +1065,7 @@ __device__ __forceinline__ void tile_marg2(RunMarg &rm, const float x0, const fl
 // 400 us (128 registers: half the shared-memory wavefronts, but fewer independent eq. (7) chains
 // in flight and more address arithmetic per store).
 template <bool MARG, bool FLAGS, bool MAP>
-__global__ void __launch_bounds__(kTileNT, 4)
+__global__ void __launch_bounds__(kTileNT, 6)
     rect_tile_kernel(const Problem pr, const double *__restrict__ prefix,
                      Partial *__restrict__ partials, const int r, const int c, const int n_rowtiles,
                      const int n_coltiles)
@@ -1215,8 +1215,7 @@ __global__ void __launch_bounds__(kTileNT, 4)
             // another); the rare cells that fail the conditioning test are redone afterwards
 #pragma unroll 1
             for (int s0 = 0; s0 < n_strips; s0 += kTileGroup) {
-                float res[kTileGroup][kTileCells];
-                uint32_t slow = 0u;
+                float res[kTileGroup][kTileCells], tt[kTileGroup][kTileCells];
                 const int jg = jl + 32 * s0 * bd.e_n;
 #pragma unroll
                 for (int strip = 0; strip < kTileGroup; ++strip) {
@@ -1231,14 +1230,28 @@ __global__ void __launch_bounds__(kTileNT, 4)
 #pragma unroll
                         for (int k = 0; k < 8; ++k) S[k] = fadd2(ph[k], U[h][k]);
                         const PairOut o = pair_closure_tile<true>(S);
-                        float t0, t1;
                         unpack2(o.res, res[strip][2 * h], res[strip][2 * h + 1]);
-                        unpack2(o.t, t0, t1);
-                        slow |= ((t0 > kTiny ? 0u : 1u) | (t1 > kTiny ? 0u : 2u)) << (kTileCells * strip + 2 * h);
+                        unpack2(o.t, tt[strip][2 * h], tt[strip][2 * h + 1]);
                     }
                 }
+                // one test for the whole block (fminf drops a NaN, so NaNs are looked for with
+                // the sum); which cells failed is only worked out in the rare case that one did
+                float tmin = tt[0][0], tsum = 0.0f;
+#pragma unroll
+                for (int strip = 0; strip < kTileGroup; ++strip)
+#pragma unroll
+                    for (int k = 0; k < kTileCells; ++k) {
+                        tmin = fminf(tmin, tt[strip][k]);
+                        tsum += tt[strip][k];
+                    }
                 uint32_t fl = 0u;  // D <= 0 / count flags of the redone cells, 2 bits per cell
-                if (slow) {  // rare: the plain way, in fp64 from P
+                if (!(tmin > kTiny) || !(tsum == tsum)) {  // rare: the plain way, in fp64 from P
+                    uint32_t slow = 0u;
+#pragma unroll
+                    for (int strip = 0; strip < kTileGroup; ++strip)
+#pragma unroll
+                        for (int k = 0; k < kTileCells; ++k)
+                            slow |= (tt[strip][k] > kTiny ? 0u : 1u) << (kTileCells * strip + k);
 #pragma unroll
                     for (int strip = 0; strip < kTileGroup; ++strip) {
                         const int64_t j = (int64_t)j_lo + jg + 32 * strip * bd.e_n;
