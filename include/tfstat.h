@@ -95,7 +95,7 @@ typedef struct tfstat_opts {
                            whenever the atoms fit its shared memory (n_atoms <= 2048)          */
     int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
                            per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
-                           (1,2,4; 11,12: 1,2 with two tau values per thread); tfstat_map_general: tau cells per thread (1,2,4); lattice
+                           (1,2,4) + 10 x (10 RT + TPC of the window-sum kernel, e.g. 422); tfstat_map_general: tau cells per thread (1,2,4); lattice
                            rect kernel: rows per thread (1, 2, 4)                             */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
     int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice

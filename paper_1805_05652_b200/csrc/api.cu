@@ -169,18 +169,29 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         if (opts && opts->seg_len > 0) len = opts->seg_len < N_t0 ? opts->seg_len : N_t0;
         pl.seg_len = len;
         pl.n_segs = (N_t0 + len - 1) / len;
-        // templates per CTA (they share the weights) and tau values per thread (they share the
-        // atom loads): 2 each while that still leaves the GPU several CTAs per SM (exp_scan.cu)
+        // slide kernel: templates per CTA (they share the weights): 2 while that still leaves the
+        // GPU ~16 CTAs per SM
         const int64_t ctas1 = (int64_t)n_templates * pl.n_nblocks * pl.n_segs;
         pl.slide_tpc = (n_templates >= 2 && ctas1 / 2 >= 148 * 16) ? 2 : 1;
-        pl.slide_rt = 1;  // 2 only on request: measured slower (168 registers, 3 CTAs per SM)
-        if (opts && opts->tile_c) {  // 1, 2, 4: templates per CTA; + 10: two tau values per thread
-            const int c = opts->tile_c;
-            if (c != 1 && c != 2 && c != 4 && c != 11 && c != 12) return pl;
-            pl.slide_rt = c > 10 ? 2 : 1;
-            pl.slide_tpc = c > 10 ? c - 10 : c;
+        pl.slide_rt = 1;
+        // window kernel (exp_window_kernel): RT tau values per thread x TPC templates per CTA share
+        // every broadcast load of an atom; the largest tile that still gives ~4 CTAs per SM
+        auto win_ctas = [&](int nt, int rt, int tpc) {
+            return (int64_t)((N_tau + nt * rt - 1) / (nt * rt)) * pl.n_segs *
+                   ((n_templates + tpc - 1) / tpc);
+        };
+        const int64_t fill = 148 * 4;
+        pl.win_rt = 1, pl.win_tpc = 1;
+        if (n_templates >= 2 && win_ctas(128, 4, 2) >= fill) pl.win_rt = 4, pl.win_tpc = 2;
+        else if (win_ctas(128, 4, 1) >= fill) pl.win_rt = 4;
+        else if (win_ctas(128, 2, 1) >= fill) pl.win_rt = 2;
+        if (opts && opts->tile_c) {  // TPC of the slide kernel + 10 x (RT TPC code of the window kernel)
+            const int c = opts->tile_c, w = c / 10, sl = c % 10;
+            if (sl != 1 && sl != 2 && sl != 4) return pl;
+            if (w != 0 && w != 11 && w != 12 && w != 21 && w != 22 && w != 41 && w != 42) return pl;
+            pl.slide_tpc = sl;
+            if (w) pl.win_rt = w / 10, pl.win_tpc = w % 10;
         }
-        pl.n_nblocks = (N_tau + NT * pl.slide_rt - 1) / (NT * pl.slide_rt);
     }
     if (window == TFSTAT_WINDOW_RECT) {
         const int rm = opts ? opts->rect_method : 0;
@@ -227,6 +238,8 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         pl.n_pad = (int32_t)(((int64_t)n_atoms + kPackBlock - 1) / kPackBlock * kPackBlock);
         off += align_up((size_t)32 * (size_t)pl.n_pad * n_templates);
     }
+    pl.off_w0 = off;  // sliding form: window sums of each segment's last t0, 32 B per (template, segment, tau)
+    if (slide) off += align_up((size_t)32 * (size_t)n_templates * pl.n_segs * N_tau);
     pl.bytes = off;
     pl.status = TFSTAT_OK;
     return pl;
@@ -274,7 +287,7 @@ static int run_device(const Plan &pl, const float *atoms, int64_t template_strid
     } else if (pl.exp_method == TFSTAT_EXP_DIRECT) {
         TF_CUDA(launch_exp_direct(pl, pr, packed, partials, st));
     } else {
-        TF_CUDA(launch_exp_scan(pl, pr, packed, partials, st));
+        TF_CUDA(launch_exp_scan(pl, pr, packed, static_cast<char *>(ws) + pl.off_w0, partials, st));
     }
     if (pl.ev_main_end) TF_CUDA(cudaEventRecord(pl.ev_main_end, st));
     if (out)
@@ -366,12 +379,12 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.n_launches = 4;  // bounds, pack, sums + closure + marginals, finalize
     } else if (window == TFSTAT_WINDOW_EXP) {
         p.kernel = TFSTAT_KERNEL_EXP_SLIDE;
-        p.tile_c = pl.slide_tpc + (pl.slide_rt > 1 ? 10 : 0);
+        p.tile_c = pl.slide_tpc + 10 * (10 * pl.win_rt + pl.win_tpc);
         p.tile_nt = pl.tile.NT;
         p.seg_len = pl.seg_len;
         p.n_segs = pl.n_segs;
         p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
-        p.n_launches = 4;  // bounds, pack, window sums + slide + closure + marginals, finalize
+        p.n_launches = 5;  // bounds, pack, window sums, slide + closure + marginals, finalize
     } else if (pl.rect_small) {
         p.kernel = TFSTAT_KERNEL_RECT_SMALL;
         p.tile_c = 1;

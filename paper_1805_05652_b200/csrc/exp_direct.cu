@@ -77,7 +77,7 @@ __device__ __forceinline__ void accumulate_core(Acc<C> &acc, const ulonglong2 ra
     unpack2(ra.y, x[0], x[1]);
     unpack2(rb.x, x[3], x[4]);
     unpack2(rb.y, x[5], x[6]);
-    const float w = ex2_approx(fmaf(dt, kexp, cexp));
+    const float w = ex2_approx(fmaf(fabsf(dt), kexp, cexp));  // (sign bit of dtc: a flag, pack.cu)
     const float w2 = w * w;
     const u64 ww = pack2(w, w);
     const u64 w2w2 = pack2(w2, w2);

@@ -96,33 +96,242 @@ __device__ __forceinline__ void bulk_copy(const uint32_t dst, const void *src, c
 }
 
 // ---------------------------------------------------------------------------------------
-// exp_slide_kernel: a thread owns RT tau values (n, n + NT, ..) x TPC templates.  The weights E_a
-// depend on (atom, tau) only, so one MUFU.EX2 (+ its argument and E^2) serves the TPC templates,
-// and one broadcast LDS.128 pair of an atom serves the RT tau values.
+// exp_window_kernel: the window sum of the LAST t0 of every (template, segment, tau) -- more than
+// 90 % of the weighted terms of the sliding form -- by a multiplicative recurrence (north_star:
+// "exp/MUFU pressure is reduced by multiplicative recurrences where timestamps allow").
 //
-// The atoms of the initial window (more than 90 % of the weighted terms of this form) come through
-// a ring of kSlideStages slots shared by the CTA, filled by bulk asynchronous copies from the
-// packed records (cp.async.bulk + mbarrier; thread 0 issues them, a slot is refilled once every
-// warp has released it): no thread moves atom data, no CTA barrier in the loop.  While sliding,
-// the atoms that enter (the same for every thread of the CTA) and leave (one gather per thread)
-// are read from the same records with two 16-byte loads each.
+// With f_i = exp(-(t_{i+1} - t_i)/tau) the weighted sum of atoms [lo, hi) relative to its first
+// atom is the backward recurrence (Horner)  S_i = x_i + f_i S_{i+1},  S_hi = 0,  S = S_lo  (f^2 for
+// a2, b2, ab).  On gapless stretches f_i is ONE constant per tau, so a term costs its 7
+// multiply-adds and nothing else: no exponential, no weight multiply.  f is recomputed
+// (MUFU.EX2 from the integer time step) only at the atoms pack.cu has flagged: where the time
+// step changes (the two edges of a gap) -- a warp-uniform branch, every lane is on the same atom.
+// Every factor is <= 1 and is taken from its own time step, so nothing drifts; the rounding of a
+// sum of n terms grows like sqrt(n) 2^-24 (1.5e-5 for a year of SFTs).
 //
-// Also measured (B200, config 4): the initial window sums in a kernel of their own with the LANES
-// ON ATOMS (a lane loads its own atom, the warp walks 8 tau values in uniform registers, a
-// transposing butterfly combines the 56 partial sums per lane): 4.2-4.8 terms/clk/SM against
-// ~9.8 for the broadcast form below, whichever way the loads were staged -- one MUFU per term
-// and lane instead of one per TPC terms, and half the lanes idle at the window's ragged end.
+// A thread owns RT neighbouring tau values x TPC templates: one broadcast LDS.128 pair of an atom
+// serves RT TPC terms.  That ratio is what the form needs: the broadcast loads return 512 bytes
+// per warp instruction to the register file, and at one tau per thread the shared-memory return
+// path, not the FP32 pipe, is the limit (ncu: lsu_writeback 72 %, FMA pipe 45 %: r02 profile).
+// The atoms come through a ring of kSlideStages slots shared by the CTA, filled back to front by
+// bulk asynchronous copies of the packed records (cp.async.bulk + mbarrier).  The sums, scaled
+// to the weight exp(-(t_lo - t0)/tau) of their first atom, go to the workspace (32 bytes per
+// (template, segment, tau)); exp_slide_kernel starts from them.
 // ---------------------------------------------------------------------------------------
 template <int NT, int RT, int TPC, bool STATS>
-__global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT == 128 ? 3 : 1))
-    exp_slide_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
-                     Partial *__restrict__ partials, const int n_nblocks, const int n_segs,
-                     const int seg_len, unsigned long long *__restrict__ stats)
+__global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
+    exp_window_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+                      float4 *__restrict__ W0, const int n_nblocks, const int n_segs,
+                      const int seg_len, unsigned long long *__restrict__ stats)
 {
     constexpr int KW = kSlideChunk, NS = TPC > 2 ? 2 : kSlideStages, NW = NT / 32;
     constexpr uint32_t kTplBytes = KW * 2 * sizeof(ulonglong2);  // one template's share of a slot
     __shared__ __align__(128) ulonglong2 s_ring[NS][TPC][2 * KW];
     __shared__ __align__(8) unsigned long long s_full[NS], s_empty[NS];
+    pdl_trigger();
+
+    const Grid g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    const int lane = threadIdx.x & 31;
+    // blockIdx.x = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
+    const int j = (int)(blockIdx.x % n_nblocks);
+    const int seg = (int)((blockIdx.x / n_nblocks) % n_segs);
+    const int tpl0 = (int)(blockIdx.x / ((int64_t)n_nblocks * n_segs)) * TPC;
+    const int n_first = (n_nblocks - 1 - j) * (NT * RT);
+    const int n_count = min(NT * RT, g.N_tau - n_first);
+    const int m = min(seg * seg_len + seg_len, g.N_t0) - 1;  // the segment's last t0
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            mbar_init(smem_u32(&s_full[s]), 1);
+            mbar_init(smem_u32(&s_empty[s]), NW);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
+
+    // templates beyond the batch (ragged last group) alias the last real one; nothing of theirs
+    // is stored
+    const ulonglong2 *__restrict__ rec[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q)
+        rec[q] = packed + (int64_t)min(tpl0 + q, pr.n_templates - 1) * n_pad * 2;
+
+    // this thread's tau values: neighbours, so that their windows end within 3 (RT - 1) atoms
+    const int lo_m = __ldg(bd.lo + m);
+    bool n_ok[RT];
+    int n[RT], hi[RT];
+    float kexp[RT];
+    int hi_min = 0x7fffffff, hi_max = lo_m;
+#pragma unroll
+    for (int r = 0; r < RT; ++r) {
+        // slots beyond the grid alias the last tau of the block (nothing of theirs is stored):
+        // a thread's windows then still end within a few atoms of one another
+        const int slot = (int)threadIdx.x * RT + r;
+        n_ok[r] = slot < n_count;
+        n[r] = n_first + min(slot, n_count - 1);
+        kexp[r] = (float)(-1.4426950408889634 / (double)tau_of(g, n[r]));
+        hi[r] = max(hi_index(bd, g, m, n[r]), lo_m);
+        hi_min = min(hi_min, hi[r]);
+        hi_max = max(hi_max, hi[r]);
+    }
+    const int cta_e = max(hi_index(bd, g, m, n_first + n_count - 1), lo_m);  // hi is monotone in n
+    const int q0 = lo_m / KW;
+    const int nq = cta_e > lo_m ? (cta_e + KW - 1) / KW - q0 : 0;
+    // chunks are consumed from the last (k = nq - 1) to the first: the ring is filled in that order
+    auto fill = [&](const int k) {  // thread 0: chunk k -> slot (nq - 1 - k) % NS
+        const int s = (nq - 1 - k) % NS;
+        const uint32_t bar = smem_u32(&s_full[s]);
+        mbar_expect_tx(bar, TPC * kTplBytes);
+#pragma unroll
+        for (int q = 0; q < TPC; ++q)
+            bulk_copy(smem_u32(&s_ring[s][q][0]), rec[q] + (int64_t)(q0 + k) * KW * 2, kTplBytes, bar);
+    };
+    if (threadIdx.x == 0)
+        for (int u = 0; u < NS && u < nq; ++u) fill(nq - 1 - u);
+
+    // accumulators: (A, B), (Re Fa, Im Fa), (Re Fb, Im Fb), C of (tau r, template q)
+    u64 s_ab[RT][TPC], s_fa[RT][TPC], s_fb[RT][TPC];
+    float s_c[RT][TPC];
+#pragma unroll
+    for (int r = 0; r < RT; ++r)
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            s_ab[r][q] = s_fa[r][q] = s_fb[r][q] = 0ull;
+            s_c[r][q] = 0.0f;
+        }
+    // step factor of the atom in hand, f = exp(-(t_{i+1} - t_i)/tau), and its square
+    float f[RT] = {}, f2[RT] = {};
+    auto step_factor = [&](const int al) {
+        const int dt = __ldg(bd.t + min(al + 1, bd.n_atoms - 1)) - __ldg(bd.t + al);
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            f[r] = ex2_approx((float)dt * kexp[r]);
+            f2[r] = f[r] * f[r];
+        }
+    };
+    // one atom into the sums of tau r: S = x + f S
+    auto horner = [&](const int r, const int q, const ulonglong2 ra, const ulonglong2 rb) {
+        float dtc, ab;
+        unpack2(ra.x, dtc, ab);
+        asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(s_ab[r][q]) : "l"(pack2(f2[r], f2[r])), "l"(ra.y));
+        asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(s_fa[r][q]) : "l"(pack2(f[r], f[r])), "l"(rb.x));
+        asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(s_fb[r][q]) : "l"(pack2(f[r], f[r])), "l"(rb.y));
+        s_c[r][q] = fmaf(s_c[r][q], f2[r], ab);
+    };
+    // a bad SFT (packed as dtc = NaN on zero channels) spoils the sums of its template
+    auto poison = [&](const int q, const ulonglong2 ra) {
+        float dtc, ab;
+        unpack2(ra.x, dtc, ab);
+        if (dtc != dtc) {
+#pragma unroll
+            for (int r = 0; r < RT; ++r) s_c[r][q] = dtc;
+        }
+    };
+
+    // ---- the few atoms at the ragged end: [hi_min, hi_r) belong to tau r only (3 per tau step) ----
+    if (hi_max > hi_min) {
+#pragma unroll 1
+        for (int al = hi_max - 1; al >= hi_min; --al) {
+            step_factor(al);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                const ulonglong2 ra = __ldg(rec[q] + 2 * (int64_t)al), rb = __ldg(rec[q] + 2 * (int64_t)al + 1);
+#pragma unroll
+                for (int r = 0; r < RT; ++r)
+                    if (al < hi[r]) horner(r, q, ra, rb);
+                poison(q, ra);
+            }
+        }
+    }
+    if (hi_min > lo_m) step_factor(hi_min - 1);  // the factor the main loop starts with
+
+    // ---- atoms [lo_m, hi_min), back to front, through the ring --------------------------------
+#pragma unroll 1
+    for (int u = 0; u < nq; ++u) {
+        const int k = nq - 1 - u;  // chunk
+        const int s = u % NS;
+        const int cs = (q0 + k) * KW;
+        // refill the slot of the chunk before this one once every warp has released it
+        if (threadIdx.x == 0 && u >= 1 && u - 1 + NS < nq) {
+            mbar_wait(smem_u32(&s_empty[(u - 1) % NS]), (uint32_t)((u - 1) / NS) & 1u);
+            fill(nq - 1 - (u - 1 + NS));
+        }
+        const int x0 = max(cs, lo_m) - cs;
+        const int x1 = min(cs + KW, hi_min) - cs;
+        mbar_wait(smem_u32(&s_full[s]), (uint32_t)(u / NS) & 1u);
+#pragma unroll 4
+        for (int i = x1 - 1; i >= x0; --i) {
+            ulonglong2 ra[TPC], rb[TPC];
+            unsigned flag = 0u;
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                ra[q] = s_ring[s][q][2 * i];
+                rb[q] = s_ring[s][q][2 * i + 1];
+                flag |= (unsigned)(ra[q].x & 0x80000000ull);
+            }
+            if (flag) {  // warp-uniform, rare: the time step changes here, or a bad SFT
+                step_factor(cs + i);
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) poison(q, ra[q]);
+            }
+#pragma unroll
+            for (int r = 0; r < RT; ++r)
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) horner(r, q, ra[q], rb[q]);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&s_empty[s]));
+    }
+
+    // ---- scale to the weight of the first atom and store ---------------------------------------
+    const int t_ref = (int)t0_of(g, m);
+    const int t_lo = __ldg(bd.t + min(lo_m, bd.n_atoms - 1));
+#pragma unroll
+    for (int r = 0; r < RT; ++r) {
+        if (!n_ok[r]) continue;
+        const float e0 = hi[r] > lo_m ? ex2_approx((float)(t_lo - t_ref) * kexp[r]) : 0.0f;
+        const float e02 = e0 * e0;
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            if (tpl0 + q >= pr.n_templates) continue;
+            float A, B, far, fai, fbr, fbi;
+            unpack2(s_ab[r][q], A, B);
+            unpack2(s_fa[r][q], far, fai);
+            unpack2(s_fb[r][q], fbr, fbi);
+            float4 *__restrict__ dst =
+                W0 + (((int64_t)(tpl0 + q) * n_segs + seg) * g.N_tau + n[r]) * 2;
+            dst[0] = make_float4(A * e02, B * e02, s_c[r][q] * e02, far * e0);
+            dst[1] = make_float4(fai * e0, fbr * e0, fbi * e0, 0.0f);
+        }
+    }
+    if (STATS) {
+        unsigned long long nt = 0;
+#pragma unroll
+        for (int r = 0; r < RT; ++r) nt += (unsigned long long)(hi[r] - lo_m);
+        nt *= (unsigned long long)min(TPC, pr.n_templates - tpl0);
+#pragma unroll
+        for (int sft = 16; sft >= 1; sft >>= 1) nt += __shfl_xor_sync(0xffffffffu, nt, sft);
+        if (lane == 0 && nt) atomicAdd(stats + 0, nt);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// exp_slide_kernel: a thread owns RT tau values x TPC templates, starts from the window sums of
+// the segment's last t0 (exp_window_kernel) and slides backwards in t0.  The weights E_a depend
+// on (atom, tau) only, so one MUFU.EX2 (+ its argument and E^2) serves the TPC templates.  The
+// atoms that enter (the same for every thread of the CTA) and leave (one gather per thread) come
+// from the packed records with two 16-byte loads each.
+// ---------------------------------------------------------------------------------------
+template <int NT, int RT, int TPC, bool STATS>
+__global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT == 128 ? (RT * TPC <= 4 ? 4 : 3) : 1))
+    exp_slide_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+                     const float4 *__restrict__ W0, Partial *__restrict__ partials,
+                     const int n_nblocks, const int n_segs, const int seg_len,
+                     unsigned long long *__restrict__ stats)
+{
     __shared__ Marg s_red[32];
     pdl_trigger();
 
@@ -139,16 +348,7 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
     const int m_beg = seg * seg_len;
     const int m_end = min(m_beg + seg_len, g.N_t0);
 
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int s = 0; s < NS; ++s) {
-            mbar_init(smem_u32(&s_full[s]), 1);
-            mbar_init(smem_u32(&s_empty[s]), NW);
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
-    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
+    pdl_wait();  // exp_window_kernel's sums (and, before it, the bounds tables and the records)
 
     // templates beyond the batch (ragged last group) alias the last real one; nothing of theirs
     // is stored
@@ -168,7 +368,7 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
     float kexp[RT], inv_tau[RT];
 #pragma unroll
     for (int r = 0; r < RT; ++r) {
-        const int slot = r * NT + (int)threadIdx.x;
+        const int slot = (int)threadIdx.x * RT + r;  // neighbouring tau values: windows 3 atoms apart
         n_ok[r] = slot < n_count;
         n[r] = n_first + (n_ok[r] ? slot : 0);
         const double tau = (double)tau_of(g, n[r]);
@@ -176,93 +376,30 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
         inv_tau[r] = (float)(1.0 / tau);
     }
 
-    // ---- initial window: cell (m_end - 1, n), streamed through the ring ----------------------
+    // ---- the segment's last cell (m_end - 1, n): its window sums come from exp_window_kernel ----
     int m = m_end - 1;
     int lo_m = __ldg(bd.lo + m);
     int hi[RT];
     int t_ref[RT];  // seconds (int32: every grid time fits, TFSTAT_EOVERFLOW otherwise)
+    SlideAcc acc[RT][TPC];
+    float A_max[RT][TPC];
 #pragma unroll
     for (int r = 0; r < RT; ++r) {
         hi[r] = n_ok[r] ? max(hi_index(bd, g, m, n[r]), lo_m) : lo_m;
         t_ref[r] = (int)t0_of(g, m);
-    }
-    const int cta_e = max(hi_index(bd, g, m, n_first + n_count - 1), lo_m);  // hi is monotone in n
-    const int q0 = lo_m / KW;
-    const int nq = cta_e > lo_m ? (cta_e + KW - 1) / KW - q0 : 0;
-    auto fill = [&](const int k) {  // thread 0: chunk k -> slot k % NS
-        const int s = k % NS;
-        const uint32_t bar = smem_u32(&s_full[s]);
-        mbar_expect_tx(bar, TPC * kTplBytes);
-#pragma unroll
-        for (int q = 0; q < TPC; ++q)
-            bulk_copy(smem_u32(&s_ring[s][q][0]), rec[q] + (int64_t)(q0 + k) * KW * 2, kTplBytes, bar);
-    };
-    if (threadIdx.x == 0)
-        for (int k = 0; k < NS && k < nq; ++k) fill(k);
-
-    SlideAcc acc[RT][TPC];
-#pragma unroll
-    for (int r = 0; r < RT; ++r)
-#pragma unroll
-        for (int q = 0; q < TPC; ++q) acc_zero(acc[r][q]);
-    unsigned n_term[4] = {0u, 0u, 0u, 0u};  // STATS: window, enter, leave, re-sum (x TPC templates)
-
-    int hi_max = hi[0];
-#pragma unroll
-    for (int r = 1; r < RT; ++r) hi_max = max(hi_max, hi[r]);
-#pragma unroll 1
-    for (int k = 0; k < nq; ++k) {
-        const int s = k % NS;
-        const int cs = (q0 + k) * KW;
-        // refill the slot of chunk k - 1 with chunk k - 1 + NS once every warp has released it
-        if (threadIdx.x == 0 && k >= 1 && k - 1 + NS < nq) {
-            mbar_wait(smem_u32(&s_empty[(k - 1) % NS]), (uint32_t)((k - 1) / NS) & 1u);
-            fill(k - 1 + NS);
-        }
-        const int tb = __ldg(bd.t + cs - cs % kPackBlock);
-        float cexp[RT];
-#pragma unroll
-        for (int r = 0; r < RT; ++r) cexp[r] = (float)(tb - t_ref[r]) * kexp[r];
-        const int x0 = max(cs, lo_m) - cs;
-        const int x1 = min(cs + KW, hi_max) - cs;
-        mbar_wait(smem_u32(&s_full[s]), (uint32_t)(k / NS) & 1u);
-#pragma unroll kWindowUnroll
-        for (int i = x0; i < x1; ++i) {
-            ulonglong2 ra[TPC], rb[TPC];
-#pragma unroll
-            for (int q = 0; q < TPC; ++q) {
-                ra[q] = s_ring[s][q][2 * i];
-                rb[q] = s_ring[s][q][2 * i + 1];
-            }
-            float dtc, ab0;
-            unpack2(ra[0].x, dtc, ab0);
-#pragma unroll
-            for (int r = 0; r < RT; ++r) {
-                // atoms beyond this tau's own window are skipped, never weighted by zero (0 x NaN)
-                if (RT == 1 || cs + i < hi[r]) {
-                    const float e = ex2_approx(fmaf(dtc, kexp[r], cexp[r]));
-                    const float e2 = e * e;
-#pragma unroll
-                    for (int q = 0; q < TPC; ++q) acc_add(acc[r][q], e, e2, ra[q], rb[q]);
-                }
-            }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&s_empty[s]));
-    }
-    if (STATS) {
-#pragma unroll
-        for (int r = 0; r < RT; ++r) n_term[0] += (unsigned)(hi[r] - lo_m);
-    }
-    float A_max[RT][TPC];
-#pragma unroll
-    for (int r = 0; r < RT; ++r)
 #pragma unroll
         for (int q = 0; q < TPC; ++q) {
-            float A, B;
-            unpack2(acc[r][q].ab, A, B);
-            A_max[r][q] = A;
+            const int tq = min(tpl0 + q, pr.n_templates - 1);
+            const float4 *__restrict__ w = W0 + (((int64_t)tq * n_segs + seg) * g.N_tau + n[r]) * 2;
+            const float4 w0 = __ldg(w), w1 = __ldg(w + 1);
+            acc[r][q].ab = pack2(w0.x, w0.y);
+            acc[r][q].c = w0.z;
+            acc[r][q].fa = pack2(w0.w, w1.x);
+            acc[r][q].fb = pack2(w1.y, w1.z);
+            A_max[r][q] = w0.x;
         }
+    }
+    unsigned n_term[4] = {0u, 0u, 0u, 0u};  // STATS: (window), enter, leave, re-sum (x TPC templates)
 
     // one atom straight from the packed records (entering / leaving / re-summed atoms), one weight
     // for the TPC templates
@@ -399,42 +536,65 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
 
 template <int NT, int RT, int TPC>
 cudaError_t launch_tpc(const Plan &pl, const Problem &pr, const ulonglong2 *packed,
-                       Partial *partials, cudaStream_t st)
+                       const float4 *W0, Partial *partials, cudaStream_t st)
 {
     const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
     const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * groups;
     if (pl.stats)
         return launch_pdl(exp_slide_kernel<NT, RT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr,
-                          packed, pl.n_pad, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
+                          packed, pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len,
+                          pl.stats);
     return launch_pdl(exp_slide_kernel<NT, RT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr, packed,
-                      pl.n_pad, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
+                      pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 
 template <int NT>
 cudaError_t launch_nt(const Plan &pl, const Problem &pr, const ulonglong2 *packed,
-                      Partial *partials, cudaStream_t st)
+                      const float4 *W0, Partial *partials, cudaStream_t st)
 {
-    if (pl.slide_rt == 2) {
-        if (pl.slide_tpc == 2) return launch_tpc<NT, 2, 2>(pl, pr, packed, partials, st);
-        return launch_tpc<NT, 2, 1>(pl, pr, packed, partials, st);
-    }
     switch (pl.slide_tpc) {
-    case 4: return launch_tpc<NT, 1, 4>(pl, pr, packed, partials, st);
-    case 2: return launch_tpc<NT, 1, 2>(pl, pr, packed, partials, st);
-    default: return launch_tpc<NT, 1, 1>(pl, pr, packed, partials, st);
+    case 4: return launch_tpc<NT, 1, 4>(pl, pr, packed, W0, partials, st);
+    case 2: return launch_tpc<NT, 1, 2>(pl, pr, packed, W0, partials, st);
+    default: return launch_tpc<NT, 1, 1>(pl, pr, packed, W0, partials, st);
     }
+}
+
+// window sums: RT tau values per thread x TPC templates per CTA
+template <int NT, int RT, int TPC>
+cudaError_t launch_win(const Plan &pl, const Problem &pr, const ulonglong2 *packed, float4 *W0,
+                       cudaStream_t st)
+{
+    const int nblk = (pl.grid.N_tau + NT * RT - 1) / (NT * RT);
+    const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
+    const int64_t n_ctas = (int64_t)nblk * pl.n_segs * groups;
+    if (pl.stats)
+        return launch_pdl(exp_window_kernel<NT, RT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr,
+                          packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, pl.stats);
+    return launch_pdl(exp_window_kernel<NT, RT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr,
+                      packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, pl.stats);
 }
 
 }  // namespace
 
-cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packed,
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packed, void *w0,
                             Partial *partials, cudaStream_t st)
 {
     const ulonglong2 *rec = static_cast<const ulonglong2 *>(packed);
+    float4 *W0 = static_cast<float4 *>(w0);
+    cudaError_t e;
+    switch (pl.win_rt * 10 + pl.win_tpc) {
+    case 42: e = launch_win<128, 4, 2>(pl, pr, rec, W0, st); break;
+    case 41: e = launch_win<128, 4, 1>(pl, pr, rec, W0, st); break;
+    case 22: e = launch_win<128, 2, 2>(pl, pr, rec, W0, st); break;
+    case 21: e = launch_win<128, 2, 1>(pl, pr, rec, W0, st); break;
+    case 12: e = launch_win<64, 1, 2>(pl, pr, rec, W0, st); break;
+    default: e = launch_win<64, 1, 1>(pl, pr, rec, W0, st); break;
+    }
+    if (e != cudaSuccess) return e;
     switch (pl.tile.NT) {
-    case 128: return launch_nt<128>(pl, pr, rec, partials, st);
-    case 64: return launch_nt<64>(pl, pr, rec, partials, st);
-    case 32: return launch_nt<32>(pl, pr, rec, partials, st);
+    case 128: return launch_nt<128>(pl, pr, rec, W0, partials, st);
+    case 64: return launch_nt<64>(pl, pr, rec, W0, partials, st);
+    case 32: return launch_nt<32>(pl, pr, rec, W0, partials, st);
     }
     return cudaErrorInvalidValue;
 }

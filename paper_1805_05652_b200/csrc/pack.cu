@@ -11,7 +11,8 @@
 // days).  A kernel turns it into its own weight argument with one FMA:
 //     (t_i - t_ref) k = dtc_i k + c,   c = (t_{block(i)} - t_ref) k   (per thread and block),
 // the same instruction count as the multiply it replaces.  Atoms that are not finite become
-// dtc = NaN with zero channels (see below).
+// dtc = NaN with zero channels, and the SIGN bit of dtc marks the atoms at which the time step
+// changes (see below): readers take |dtc|.
 #include "plan.h"
 
 namespace tfstat {
@@ -32,7 +33,8 @@ __global__ void __launch_bounds__(kPackNT)
         ulonglong2 ra = make_ulonglong2(0ull, 0ull), rb = ra;  // padding: zeros, never summed
         if (i < n_atoms) {
             const float *__restrict__ base = atoms + (int64_t)tpl * template_stride + i;
-            float dtc = (float)((long long)__ldg(t + i) - (long long)__ldg(t + i - i % kPackBlock));
+            const long long ti = __ldg(t + i);
+            float dtc = (float)(ti - (long long)__ldg(t + i - i % kPackBlock));
             float x[7];
             bool bad = false;
 #pragma unroll
@@ -49,7 +51,19 @@ __global__ void __launch_bounds__(kPackNT)
 #pragma unroll
                 for (int k = 0; k < 7; ++k) x[k] = 0.0f;
             }
-            ra.x = pack2(dtc, x[2]);
+            // Sign bit of dtc: "the step t_{i+1} - t_i differs from the step behind it" (or there
+            // is none, or this atom is a bad one).  exp_window_kernel walks the atoms backwards
+            // with the multiplicative recurrence S_i = x_i + f S_{i+1}, f = exp(-(t_{i+1} - t_i)/tau):
+            // f only has to be recomputed where this bit is set, i.e. at the edges of gaps.
+            bool change = i + 2 >= n_atoms || bad;
+            if (!change) {
+                const long long t1 = __ldg(t + i + 1), t2 = __ldg(t + i + 2);
+                change = (t1 - ti) != (t2 - t1);
+            }
+            // (assembled as integers: a NaN moved through float arithmetic may lose its sign bit)
+            unsigned dtc_bits = bad ? 0x7fc00000u : __float_as_uint(dtc);
+            if (change) dtc_bits |= 0x80000000u;
+            ra.x = ((u64)__float_as_uint(x[2]) << 32) | (u64)dtc_bits;
             ra.y = pack2(x[0], x[1]);
             rb.x = pack2(x[3], x[4]);
             rb.y = pack2(x[5], x[6]);

@@ -59,13 +59,14 @@ struct Plan {
     // exp sliding form (exp_scan.cu): t0 segments per (template, tau block)
     int32_t n_segs, seg_len;
     int32_t slide_tpc;  // templates per CTA (1, 2, 4): they share the weights
-    int32_t slide_rt;   // tau values per thread (1, 2): they share the atom loads
+    int32_t slide_rt;   // (always 1: kept for the launchers)
+    int32_t win_rt, win_tpc;  // exp_window_kernel: tau values per thread, templates per CTA
     // rect / marginalise tiling
     int32_t cell_blocks_per_template;
     RectRun rect;
     // workspace layout (byte offsets)
     size_t off_lo, off_edge, off_partials, off_prefix, off_tot, off_flags, off_steps, off_pack,
-        bytes;
+        off_w0, bytes;
     int32_t n_pad;  // exp: atoms per template in the packed records (pack.cu), padded
     size_t flags_bytes;  // rect: scan flags the bounds kernel (or a memset) zeroes
     int64_t partials_per_template;
@@ -94,7 +95,7 @@ bool rect_small_applies(int32_t n_atoms, int32_t n_templates, int64_t cells);
 cudaError_t launch_rect_small(const Plan &pl, const Problem &pr, cudaStream_t st);
 cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, double *agg,
                         int32_t *flags, void *steps, Partial *partials, cudaStream_t st);
-cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packed,
+cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packed, void *w0,
                             Partial *partials, cudaStream_t st);
 cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_template,
                             int32_t n_templates, int32_t N_tau, tfstat_result *out,
