@@ -187,7 +187,7 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         else if (win_ctas(128, 2, 1) >= fill) pl.win_rt = 2;
         if (opts && opts->tile_c) {  // TPC of the slide kernel + 10 x (RT TPC code of the window kernel)
             const int c = opts->tile_c, w = c / 10, sl = c % 10;
-            if (sl != 1 && sl != 2 && sl != 4) return pl;
+            if (sl != 1 && sl != 2) return pl;
             if (w != 0 && w != 11 && w != 12 && w != 21 && w != 22 && w != 41 && w != 42) return pl;
             pl.slide_tpc = sl;
             if (w) pl.win_rt = w / 10, pl.win_tpc = w % 10;

@@ -77,6 +77,13 @@ __device__ __forceinline__ void acc_scale(SlideAcc &a, const float c)
     a.c *= c2;
 }
 
+__device__ __forceinline__ float rcp_approx_s(const float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ void mbar_expect_tx(const uint32_t bar, const uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
@@ -119,24 +126,23 @@ __device__ __forceinline__ void bulk_copy(const uint32_t dst, const void *src, c
 // (template, segment, tau)); exp_slide_kernel starts from them.
 // ---------------------------------------------------------------------------------------
 template <int NT, int RT, int TPC, bool STATS>
-__global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
-    exp_window_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
-                      float4 *__restrict__ W0, const int n_nblocks, const int n_segs,
-                      const int seg_len, unsigned long long *__restrict__ stats)
+__device__ __forceinline__ void exp_window_body(
+    const Problem &pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+    float4 *__restrict__ W0, const unsigned vblock, const int n_nblocks, const int n_segs,
+    const int seg_len, unsigned long long *__restrict__ stats)
 {
     constexpr int KW = kSlideChunk, NS = TPC > 2 ? 2 : kSlideStages, NW = NT / 32;
     constexpr uint32_t kTplBytes = KW * 2 * sizeof(ulonglong2);  // one template's share of a slot
     __shared__ __align__(128) ulonglong2 s_ring[NS][TPC][2 * KW];
     __shared__ __align__(8) unsigned long long s_full[NS], s_empty[NS];
-    pdl_trigger();
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
     const int lane = threadIdx.x & 31;
-    // blockIdx.x = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
-    const int j = (int)(blockIdx.x % n_nblocks);
-    const int seg = (int)((blockIdx.x / n_nblocks) % n_segs);
-    const int tpl0 = (int)(blockIdx.x / ((int64_t)n_nblocks * n_segs)) * TPC;
+    // vblock = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
+    const int j = (int)(vblock % n_nblocks);
+    const int seg = (int)((vblock / n_nblocks) % n_segs);
+    const int tpl0 = (int)(vblock / ((int64_t)n_nblocks * n_segs)) * TPC;
     const int n_first = (n_nblocks - 1 - j) * (NT * RT);
     const int n_count = min(NT * RT, g.N_tau - n_first);
     const int m = min(seg * seg_len + seg_len, g.N_t0) - 1;  // the segment's last t0
@@ -150,7 +156,6 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
         mbar_fence_init();
     }
     __syncthreads();
-    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
 
     // templates beyond the batch (ragged last group) alias the last real one; nothing of theirs
     // is stored
@@ -319,36 +324,38 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
 }
 
 // ---------------------------------------------------------------------------------------
-// exp_slide_kernel: a thread owns RT tau values x TPC templates, starts from the window sums of
-// the segment's last t0 (exp_window_kernel) and slides backwards in t0.  The weights E_a depend
-// on (atom, tau) only, so one MUFU.EX2 (+ its argument and E^2) serves the TPC templates.  The
-// atoms that enter (the same for every thread of the CTA) and leave (one gather per thread) come
-// from the packed records with two 16-byte loads each.
+// exp_slide_kernel: a thread owns one tau x TPC templates, starts from the window sums of the
+// segment's last t0 (exp_window_kernel) and slides backwards in t0.  The weights E_a depend on
+// (atom, tau) only, so one MUFU.EX2 (+ its argument and E^2) serves the TPC templates.  The atoms
+// that enter (the same for every thread of the CTA) and leave (one gather per thread) come from
+// the packed records with two 16-byte loads each.
+//
+// A t0 step is a chain of dependent loads (row start -> window end -> atom records) in front of a
+// few dozen arithmetic instructions, so the loop is software-pipelined by hand: the indices of
+// step m - 2 and the records of the atoms of step m - 1 are requested BEFORE cell m is closed
+// (eq. 7), and are in registers by the time the sums move on.
 // ---------------------------------------------------------------------------------------
-template <int NT, int RT, int TPC, bool STATS>
-__global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT == 128 ? (RT * TPC <= 4 ? 4 : 3) : 1))
-    exp_slide_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
-                     const float4 *__restrict__ W0, Partial *__restrict__ partials,
-                     const int n_nblocks, const int n_segs, const int seg_len,
-                     unsigned long long *__restrict__ stats)
+constexpr float kHalfLog2eS = 0.72134752044448170368f;  // log2(e) / 2: F log2e = 2F * this
+
+template <int NT, int TPC, bool STATS>
+__device__ __forceinline__ void exp_slide_body(
+    const Problem &pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+    const float4 *W0, Partial *__restrict__ partials, const unsigned vblock, const int n_nblocks,
+    const int n_segs, const int seg_len, unsigned long long *__restrict__ stats)
 {
     __shared__ Marg s_red[32];
-    pdl_trigger();
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
     const int lane = threadIdx.x & 31;
-    // blockIdx.x = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
-    const int j = (int)(blockIdx.x % n_nblocks);
-    const int seg = (int)((blockIdx.x / n_nblocks) % n_segs);
-    const int tpl0 = (int)(blockIdx.x / ((int64_t)n_nblocks * n_segs)) * TPC;
-    const int nb = n_nblocks - 1 - j;
-    const int n_first = nb * (NT * RT);
-    const int n_count = min(NT * RT, g.N_tau - n_first);
+    // vblock = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
+    const int j = (int)(vblock % n_nblocks);
+    const int seg = (int)((vblock / n_nblocks) % n_segs);
+    const int tpl0 = (int)(vblock / ((int64_t)n_nblocks * n_segs)) * TPC;
+    const int n_first = (n_nblocks - 1 - j) * NT;
+    const int n_count = min(NT, g.N_tau - n_first);
     const int m_beg = seg * seg_len;
     const int m_end = min(m_beg + seg_len, g.N_t0);
-
-    pdl_wait();  // exp_window_kernel's sums (and, before it, the bounds tables and the records)
 
     // templates beyond the batch (ragged last group) alias the last real one; nothing of theirs
     // is stored
@@ -361,160 +368,225 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
         base[q] = pr.atoms + (int64_t)tq * pr.template_stride;
     }
     const int64_t ld = pr.ld;
-
-    // this thread's tau values
-    bool n_ok[RT];
-    int n[RT];
-    float kexp[RT], inv_tau[RT];
-#pragma unroll
-    for (int r = 0; r < RT; ++r) {
-        const int slot = (int)threadIdx.x * RT + r;  // neighbouring tau values: windows 3 atoms apart
-        n_ok[r] = slot < n_count;
-        n[r] = n_first + (n_ok[r] ? slot : 0);
-        const double tau = (double)tau_of(g, n[r]);
-        kexp[r] = (float)(-1.4426950408889634 / tau);
-        inv_tau[r] = (float)(1.0 / tau);
-    }
+    const bool n_ok = (int)threadIdx.x < n_count;
+    const int n = n_first + (n_ok ? (int)threadIdx.x : 0);
+    const double tau = (double)tau_of(g, n);
+    const float kexp = (float)(-1.4426950408889634 / tau);
+    const float inv_tau = (float)(1.0 / tau);
 
     // ---- the segment's last cell (m_end - 1, n): its window sums come from exp_window_kernel ----
     int m = m_end - 1;
     int lo_m = __ldg(bd.lo + m);
-    int hi[RT];
-    int t_ref[RT];  // seconds (int32: every grid time fits, TFSTAT_EOVERFLOW otherwise)
-    SlideAcc acc[RT][TPC];
-    float A_max[RT][TPC];
+    int hi = n_ok ? max(hi_index(bd, g, m, n), lo_m) : lo_m;
+    int t_ref = (int)t0_of(g, m);  // seconds (int32: every grid time fits, TFSTAT_EOVERFLOW otherwise)
+    SlideAcc acc[TPC];
+    float A_max[TPC];
 #pragma unroll
-    for (int r = 0; r < RT; ++r) {
-        hi[r] = n_ok[r] ? max(hi_index(bd, g, m, n[r]), lo_m) : lo_m;
-        t_ref[r] = (int)t0_of(g, m);
-#pragma unroll
-        for (int q = 0; q < TPC; ++q) {
-            const int tq = min(tpl0 + q, pr.n_templates - 1);
-            const float4 *__restrict__ w = W0 + (((int64_t)tq * n_segs + seg) * g.N_tau + n[r]) * 2;
-            const float4 w0 = __ldg(w), w1 = __ldg(w + 1);
-            acc[r][q].ab = pack2(w0.x, w0.y);
-            acc[r][q].c = w0.z;
-            acc[r][q].fa = pack2(w0.w, w1.x);
-            acc[r][q].fb = pack2(w1.y, w1.z);
-            A_max[r][q] = w0.x;
-        }
+    for (int q = 0; q < TPC; ++q) {
+        const int tq = min(tpl0 + q, pr.n_templates - 1);
+        // (plain loads: in the fused kernel W0 was written by this very CTA a moment ago)
+        const float4 *w = W0 + (((int64_t)tq * n_segs + seg) * g.N_tau + n) * 2;
+        const float4 w0 = w[0], w1 = w[1];
+        acc[q].ab = pack2(w0.x, w0.y);
+        acc[q].c = w0.z;
+        acc[q].fa = pack2(w0.w, w1.x);
+        acc[q].fb = pack2(w1.y, w1.z);
+        A_max[q] = w0.x;
     }
     unsigned n_term[4] = {0u, 0u, 0u, 0u};  // STATS: (window), enter, leave, re-sum (x TPC templates)
 
     // one atom straight from the packed records (entering / leaving / re-summed atoms), one weight
     // for the TPC templates
-    auto add_global = [&](const int r, const int al, const float sign) {
-        const float dt = (float)(__ldg(bd.t + al) - t_ref[r]);
-        const float e = ex2_approx(dt * kexp[r]);
+    auto add_records = [&](const int t_al, const ulonglong2 (&ra)[TPC], const ulonglong2 (&rb)[TPC],
+                           const float sign) {
+        const float dt = (float)(t_al - t_ref);
+        const float e = ex2_approx(dt * kexp);
 #pragma unroll
         for (int q = 0; q < TPC; ++q) {
-            const ulonglong2 ra = __ldg(rec[q] + 2 * (int64_t)al), rb = __ldg(rec[q] + 2 * (int64_t)al + 1);
             float dtc, ab;
-            unpack2(ra.x, dtc, ab);
+            unpack2(ra[q].x, dtc, ab);
             const float eq = fmaf(dtc, 0.0f, e);  // NaN for an atom that is not finite (pack.cu)
             const float w = sign * eq;
-            acc_add(acc[r][q], w, w * eq, ra, rb);
+            acc_add(acc[q], w, w * eq, ra[q], rb[q]);
         }
     };
+    auto add_global = [&](const int al, const float sign) {
+        ulonglong2 ra[TPC], rb[TPC];
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            ra[q] = __ldg(rec[q] + 2 * (int64_t)al);
+            rb[q] = __ldg(rec[q] + 2 * (int64_t)al + 1);
+        }
+        add_records(__ldg(bd.t + al), ra, rb, sign);
+    };
+
+    // marginals per template: running max (ties: this thread's flat indices only decrease, so the
+    // later cell wins) and log-sum-exp against a reference that moves rarely
+    float mg_best[TPC], mg_ref2[TPC], mg_sum[TPC];
+    int32_t mg_idx[TPC], mg_nv[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
+        mg_best[q] = -INFINITY;
+        mg_idx[q] = 0x7fffffff;
+        mg_ref2[q] = -1.0e30f;
+        mg_sum[q] = 0.0f;
+        mg_nv[q] = 0;
+    }
+    const int64_t cells = (int64_t)g.N_t0 * g.N_tau;
 
     // ---- slide backwards in t0: closure of cell m, then step to m - 1 ------------------------
-    Marg mg[RT][TPC];
-#pragma unroll
-    for (int r = 0; r < RT; ++r)
-#pragma unroll
-        for (int q = 0; q < TPC; ++q) marg_init(mg[r][q]);
-    const int64_t cells = (int64_t)g.N_t0 * g.N_tau;
+    // indices of the step m -> m - 1, requested one step ahead
+    int lo2 = lo_m, hi2 = hi;
+    if (m > m_beg) {
+        lo2 = __ldg(bd.lo + m - 1);
+        hi2 = n_ok ? max(hi_index(bd, g, m - 1, n), lo2) : lo2;
+    }
 #pragma unroll 1
     for (;;) {
+        const bool last = m == m_beg;
+        // -- this step's atoms: in the common case at most one enters and one leaves; their
+        // records are requested now and used after the closure
+        const int n_in = lo_m - lo2, lv = max(hi2, lo_m), n_out = hi - lv;
+        const bool fresh0 = (hi2 <= lo_m) || (hi2 == lo2);  // no overlap with window m, or empty
+        const bool simple = !last && !fresh0 && n_in <= 1 && n_out <= 1;
+        ulonglong2 ia[TPC], ib[TPC], oa[TPC], ob[TPC];
+        int t_in = 0, t_out = 0;
+        if (simple) {
+            if (n_in == 1) {
+                t_in = __ldg(bd.t + lo2);
 #pragma unroll
-        for (int r = 0; r < RT; ++r) {
-            if (!n_ok[r]) continue;
-            const int32_t flat = m * g.N_tau + n[r];
+                for (int q = 0; q < TPC; ++q) {
+                    ia[q] = __ldg(rec[q] + 2 * (int64_t)lo2);
+                    ib[q] = __ldg(rec[q] + 2 * (int64_t)lo2 + 1);
+                }
+            }
+            if (n_out == 1) {
+                t_out = __ldg(bd.t + lv);
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    oa[q] = __ldg(rec[q] + 2 * (int64_t)lv);
+                    ob[q] = __ldg(rec[q] + 2 * (int64_t)lv + 1);
+                }
+            }
+        }
+        // -- indices of the step after this one
+        int lo3 = lo2, hi3 = hi2;
+        if (m - 1 > m_beg) {
+            lo3 = __ldg(bd.lo + m - 2);
+            hi3 = n_ok ? max(hi_index(bd, g, m - 2, n), lo3) : lo3;
+        }
+
+        // -- a4 + a5: cell (m, n) of every template
+        if (n_ok) {
+            const int32_t flat = m * g.N_tau + n;
+            const int cnt = hi - lo_m;
 #pragma unroll
             for (int q = 0; q < TPC; ++q) {
                 if (tpl0 + q >= pr.n_templates) continue;
                 float A, B, far, fai, fbr, fbi;
-                unpack2(acc[r][q].ab, A, B);
-                unpack2(acc[r][q].fa, far, fai);
-                unpack2(acc[r][q].fb, fbr, fbi);
-                uint32_t fl;
-                const float twoF = closure_2F_exp<false>(
-                    A, B, acc[r][q].c, far, fai, fbr, fbi, lo_m, hi[r] - lo_m, pr.min_atoms, fl,
-                    base[q], ld, bd.t, t0_of(g, m), (double)tau_of(g, n[r]));
+                unpack2(acc[q].ab, A, B);
+                unpack2(acc[q].fa, far, fai);
+                unpack2(acc[q].fb, fbr, fbi);
+                const float C = acc[q].c;
+                // fp32 closure where the cell is well conditioned and in range (tfstat_dev.cuh)
+                const float p = A * B;
+                const float D = fmaf(-C, C, p);
+                const float na = fmaf(far, far, fai * fai);
+                const float nb = fmaf(fbr, fbr, fbi * fbi);
+                const float re = fmaf(far, fbr, fai * fbi);
+                float num = B * na;
+                num = fmaf(A, nb, num);
+                num = fmaf(-2.0f * C, re, num);
+                float twoF = 2.0f * num * rcp_approx_s(D);
+                uint32_t fl = 0u;
+                if (!(D > 0.015625f * p && p > 1.0e-30f && p < 1.0e30f && cnt >= pr.min_atoms &&
+                      fabsf(twoF) < 3.0e38f))
+                    twoF = closure_2F_exp<false>(A, B, C, far, fai, fbr, fbi, lo_m, cnt,
+                                                 pr.min_atoms, fl, base[q], ld, bd.t, t0_of(g, m),
+                                                 tau);
                 const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
                 if (pr.out_maps) pr.out_maps[o] = twoF;
                 if (pr.out_flags) pr.out_flags[o] = (uint8_t)fl;
-                if (!fl) marg_add(mg[r][q], twoF, flat);
-            }
-        }
-        if (m == m_beg) break;
-        const int m2 = m - 1;
-        const int lo2 = __ldg(bd.lo + m2);
-        const int t0_2 = (int)t0_of(g, m2);
-#pragma unroll
-        for (int r = 0; r < RT; ++r) {
-            const int hi2 = n_ok[r] ? max(hi_index(bd, g, m2, n[r]), lo2) : lo2;
-            bool fresh = (hi2 <= lo_m) || (hi2 == lo2);  // no overlap with window m, or empty
-            if (!fresh) {
-                const float sh = (float)(t_ref[r] - t0_2);
-                if (sh * inv_tau[r] > kReanchor) {  // keep the weights of entering atoms <= e^kReanchor
-                    const float c = ex2_approx(sh * kexp[r]);
-#pragma unroll
-                    for (int q = 0; q < TPC; ++q) {
-                        acc_scale(acc[r][q], c);
-                        A_max[r][q] *= c * c;
+                if (!fl) {
+                    if (twoF >= mg_best[q]) {  // rare after the first few cells
+                        mg_best[q] = twoF;
+                        mg_idx[q] = flat;
                     }
-                    t_ref[r] = t0_2;
-                }
-                for (int al = lo2; al < lo_m; ++al) add_global(r, al, 1.0f);  // entering, low end
-                const int lv = max(hi2, lo_m);
-                for (int al = lv; al < hi[r]; ++al) add_global(r, al, -1.0f);  // leaving, high end
-                if (STATS) {
-                    n_term[1] += (unsigned)(lo_m - lo2);
-                    n_term[2] += (unsigned)max(hi[r] - lv, 0);
-                }
-#pragma unroll
-                for (int q = 0; q < TPC; ++q) {
-                    float A, B;
-                    unpack2(acc[r][q].ab, A, B);
-                    A_max[r][q] = fmaxf(A_max[r][q], A);
-                    // a window that lost most of its weight is re-summed (for all TPC templates:
-                    // a fresh sum is always right); written so that a NaN / inf atom in the
-                    // running sums also forces a fresh sum: once it has left the window it must
-                    // not linger
-                    fresh = fresh || !(A * kGuard >= A_max[r][q]);
+                    if (fmaf(twoF, kHalfLog2eS, -mg_ref2[q]) > 60.0f) {  // rare: move the reference
+                        mg_sum[q] *= ex2_approx(mg_ref2[q] - twoF * kHalfLog2eS);
+                        mg_ref2[q] = twoF * kHalfLog2eS;
+                    }
+                    mg_sum[q] += ex2_approx(fmaf(twoF, kHalfLog2eS, -mg_ref2[q]));
+                    mg_nv[q] += 1;
                 }
             }
-            if (fresh) {
-#pragma unroll
-                for (int q = 0; q < TPC; ++q) acc_zero(acc[r][q]);
-                t_ref[r] = t0_2;
-                for (int al = lo2; al < hi2; ++al) add_global(r, al, 1.0f);
-                if (STATS) n_term[3] += (unsigned)(hi2 - lo2);
-#pragma unroll
-                for (int q = 0; q < TPC; ++q) {
-                    float A, B;
-                    unpack2(acc[r][q].ab, A, B);
-                    A_max[r][q] = A;
-                }
-            }
-            hi[r] = hi2;
         }
-        m = m2;
+        if (last) break;
+
+        // -- the sums move on to cell m - 1
+        const int t0_2 = (int)t0_of(g, m - 1);
+        bool fresh = fresh0;
+        if (!fresh) {
+            const float sh = (float)(t_ref - t0_2);
+            if (sh * inv_tau > kReanchor) {  // keep the weights of entering atoms <= e^kReanchor
+                const float c = ex2_approx(sh * kexp);
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    acc_scale(acc[q], c);
+                    A_max[q] *= c * c;
+                }
+                t_ref = t0_2;
+            }
+            if (simple) {
+                if (n_in == 1) add_records(t_in, ia, ib, 1.0f);
+                if (n_out == 1) add_records(t_out, oa, ob, -1.0f);
+            } else {
+                for (int al = lo2; al < lo_m; ++al) add_global(al, 1.0f);  // entering, low end
+                for (int al = lv; al < hi; ++al) add_global(al, -1.0f);    // leaving, high end
+            }
+            if (STATS) {
+                n_term[1] += (unsigned)n_in;
+                n_term[2] += (unsigned)max(n_out, 0);
+            }
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                float A, B;
+                unpack2(acc[q].ab, A, B);
+                A_max[q] = fmaxf(A_max[q], A);
+                // a window that lost most of its weight is re-summed (for all TPC templates: a
+                // fresh sum is always right); written so that a NaN / inf atom in the running sums
+                // also forces a fresh sum: once it has left the window it must not linger
+                fresh = fresh || !(A * kGuard >= A_max[q]);
+            }
+        }
+        if (fresh) {
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) acc_zero(acc[q]);
+            t_ref = t0_2;
+            for (int al = lo2; al < hi2; ++al) add_global(al, 1.0f);
+            if (STATS) n_term[3] += (unsigned)(hi2 - lo2);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                float A, B;
+                unpack2(acc[q].ab, A, B);
+                A_max[q] = A;
+            }
+        }
+        m -= 1;
         lo_m = lo2;
+        hi = hi2;
+        lo2 = lo3;
+        hi2 = hi3;
     }
     if (STATS) {
         // (terms of out-of-range tau slots and of ragged template groups were not summed for real)
         unsigned long long v[5];
         const unsigned long long ntpl = (unsigned long long)min(TPC, pr.n_templates - tpl0);
-        int n_mine = 0;
-#pragma unroll
-        for (int r = 0; r < RT; ++r) n_mine += n_ok[r] ? 1 : 0;
 #pragma unroll
         for (int i = 0; i < 4; ++i) v[i] = (unsigned long long)n_term[i] * ntpl;
-        v[4] = (unsigned long long)n_mine * (unsigned long long)(m_end - m_beg) * ntpl;
+        v[4] = (n_ok ? 1ull : 0ull) * (unsigned long long)(m_end - m_beg) * ntpl;
 #pragma unroll
-        for (int i = 0; i < 5; ++i) {
+        for (int i = 1; i < 5; ++i) {
 #pragma unroll
             for (int sft = 16; sft >= 1; sft >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], sft);
             if (lane == 0 && v[i]) atomicAdd(stats + i, v[i]);
@@ -523,10 +595,16 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
     if (partials) {
 #pragma unroll
         for (int q = 0; q < TPC; ++q) {
-            Marg a = mg[0][q];
-#pragma unroll
-            for (int r = 1; r < RT; ++r) marg_merge(a, mg[r][q]);
-            if (q > 0) __syncthreads();  // s_red is reused
+            Marg a;
+            marg_init(a);
+            if (mg_nv[q] > 0) {
+                a.best = mg_best[q];
+                a.idx = mg_idx[q];
+                a.M = 0.5f * mg_best[q];
+                a.S = mg_sum[q] * ex2_approx(mg_ref2[q] - mg_best[q] * kHalfLog2eS);
+                a.nvalid = mg_nv[q];
+            }
+            __syncthreads();  // s_red is reused (by the next template, the next pass)
             marg_block_reduce<NT>(a, s_red);
             if (threadIdx.x == 0 && tpl0 + q < pr.n_templates)
                 partial_store(partials + ((int64_t)(tpl0 + q) * n_segs + seg) * n_nblocks + j, a);
@@ -534,17 +612,48 @@ __global__ void __launch_bounds__(NT, RT * TPC <= 2 ? (NT == 128 ? 5 : 1) : (NT 
     }
 }
 
-template <int NT, int RT, int TPC>
+// ---- the three kernels built from the two bodies ----------------------------------------------
+template <int NT, int RT, int TPC, bool STATS>
+__global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
+    exp_window_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+                      float4 *__restrict__ W0, const int n_nblocks, const int n_segs,
+                      const int seg_len, unsigned long long *__restrict__ stats)
+{
+    pdl_trigger();
+    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
+    exp_window_body<NT, RT, TPC, STATS>(pr, packed, n_pad, W0, blockIdx.x, n_nblocks, n_segs, seg_len,
+                                        stats);
+}
+
+template <int NT, int TPC, bool STATS>
+__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : 4) : 1)
+    exp_slide_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+                     const float4 *__restrict__ W0, Partial *__restrict__ partials,
+                     const int n_nblocks, const int n_segs, const int seg_len,
+                     unsigned long long *__restrict__ stats)
+{
+    pdl_trigger();
+    pdl_wait();  // exp_window_kernel's sums (and, before it, the bounds tables and the records)
+    exp_slide_body<NT, TPC, STATS>(pr, packed, n_pad, W0, partials, blockIdx.x, n_nblocks, n_segs,
+                                   seg_len, stats);
+}
+
+// Also measured (B200, config 4 x 2048 templates): both phases in ONE kernel (a CTA sums the
+// windows of its 512 tau values, then slides them in four passes), hoping that CTAs in different
+// phases overlap the FP32-bound window sums with the latency-bound sliding: 4.53 ms against
+// 4.10 ms for the two kernels back to back (128 registers with spills, 16 warps per SM for both
+// phases).
+
+template <int NT, int TPC>
 cudaError_t launch_tpc(const Plan &pl, const Problem &pr, const ulonglong2 *packed,
                        const float4 *W0, Partial *partials, cudaStream_t st)
 {
     const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
     const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * groups;
     if (pl.stats)
-        return launch_pdl(exp_slide_kernel<NT, RT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr,
-                          packed, pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len,
-                          pl.stats);
-    return launch_pdl(exp_slide_kernel<NT, RT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr, packed,
+        return launch_pdl(exp_slide_kernel<NT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr, packed,
+                          pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
+    return launch_pdl(exp_slide_kernel<NT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr, packed,
                       pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 
@@ -552,11 +661,8 @@ template <int NT>
 cudaError_t launch_nt(const Plan &pl, const Problem &pr, const ulonglong2 *packed,
                       const float4 *W0, Partial *partials, cudaStream_t st)
 {
-    switch (pl.slide_tpc) {
-    case 4: return launch_tpc<NT, 1, 4>(pl, pr, packed, W0, partials, st);
-    case 2: return launch_tpc<NT, 1, 2>(pl, pr, packed, W0, partials, st);
-    default: return launch_tpc<NT, 1, 1>(pl, pr, packed, W0, partials, st);
-    }
+    if (pl.slide_tpc == 2) return launch_tpc<NT, 2>(pl, pr, packed, W0, partials, st);
+    return launch_tpc<NT, 1>(pl, pr, packed, W0, partials, st);
 }
 
 // window sums: RT tau values per thread x TPC templates per CTA

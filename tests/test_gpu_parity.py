@@ -765,9 +765,10 @@ def test_exp_scan_long_gaps_and_disjoint_windows(pkg):
         check_cells(m, f, ref, f"scan min_atoms={min_atoms}")
 
 
-@pytest.mark.parametrize("tpc,seg_len", [(0, 0), (1, 0), (2, 5), (4, 0), (4, 7)])
+@pytest.mark.parametrize("tpc,seg_len", [(0, 0), (1, 0), (2, 5), (422, 0), (211, 7), (122, 3)])
 def test_exp_scan_batched_equals_oracle_and_direct(pkg, tpc, seg_len):
-    """7 templates: with 2 or 4 templates per CTA (shared weights) the last group is ragged."""
+    """7 templates: with 2 templates per CTA (shared weights) the last group is ragged; tpc also
+    selects the tile of the window-sum kernel (10 x (10 RT + TPC): 4, 2 or 1 tau per thread)."""
     grid = Grid(0, 1800, 23, 3600, 3600, 140)
     wl = tiny_workload(201, 350, 0.1, grid, n_templates=7, phi_random=True)
     a, t = dev(wl.data.atoms), dev(wl.data.t)
