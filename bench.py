@@ -506,6 +506,11 @@ def run_ours(args):
                                   "768 atoms); pack_atoms_kernel reads the caller's 28 B + writes them",
         "plan": plan,
         "probes_ops_per_clk_sm": {k: round(v["ops_per_clk_sm"], 2) for k, v in probes.items()},
+        # the kernel's core loop with nothing around it, in the shipped accumulator layout (pairs
+        # of cells: two broadcast-scalar multiplicands) and in round 1's (pairs of channels)
+        "isolated_core_loop_terms_per_clk_sm": {
+            f"{d['form']}_c{d['cells']}": round(d["terms_per_clk_sm"], 2)
+            for d in (pkg.probe_direct_loop(f, c) for f in (0, 1) for c in (8, 16))},
         "probe_sm_mhz": round(probes["ffma"]["sm_mhz"], 1),
     }
 
@@ -553,10 +558,9 @@ def run_ours(args):
             "ms_per_step": ms_s_e2e, "effective_terms_per_s": terms / (ms_s_e2e * 1e-3),
             "h2d_GBps": h2d / (ms_s_e2e * 1e-3) / 1e9}
         # roofline of the path a caller gets by default (EXP_AUTO = the sliding form): the weighted
-        # terms the kernel EXECUTED, counted by the kernel itself (tfstat_opts.stats, in a separate
-        # untimed call), as FP32 lane-ops: 7 multiply-adds per term, 2 per weight (its argument
-        # and E^2; the MUFU.EX2 runs on the XU pipe) shared by the templates of a CTA, and the
-        # fp32 closure + marginal update per cell (23 lane-ops: csrc/tfstat_dev.cuh)
+        # terms the two kernels EXECUTED, counted by the kernels themselves (tfstat_opts.stats, in a
+        # separate untimed call), as FP32 lane-ops, plus the fp32 closure + marginal update per
+        # cell (23 lane-ops: csrc/exp_scan.cu)
         plan_s = pkg.plan_info(pkg.EXP, int(t.shape[0]), n_tpl, grid, exp_method=pkg.EXP_SCAN)
         st = torch.zeros(pkg.binding.N_STATS, dtype=torch.int64, device="cuda")
         pkg.tfstat_search(atoms, t, pkg.EXP, grid, exp_method=pkg.EXP_SCAN, stats=st)
@@ -570,10 +574,13 @@ def run_ours(args):
         tpc = plan_s["tile_c"] % 10
         w_terms = (stv["terms_window"] + stv["terms_enter"] + stv["terms_leave"] +
                    stv["terms_resum"])
-        lane_ops = 7.0 * w_terms + 2.0 * w_terms / tpc + 23.0 * stv["cells"]
+        # window sums (exp_window_kernel): the multiplicative recurrence, 7 multiply-adds per term
+        # and nothing else; entering / leaving / re-summed atoms: 7 + 2 / TPC (weight argument, E^2)
+        slide_terms = stv["terms_enter"] + stv["terms_leave"] + stv["terms_resum"]
+        lane_ops = 7.0 * w_terms + 2.0 * slide_terms / tpc + 23.0 * stv["cells"]
         packed_b = plan_packed_bytes(int(t.shape[0]), n_tpl)
         side["cfg4_exp_scan_roofline"] = {
-            "bound": "alu", "kernel": "exp_slide_kernel", "kernel_ms": k_ms_s,
+            "bound": "alu", "kernel": "exp_window_kernel + exp_slide_kernel", "kernel_ms": k_ms_s,
             "executed": stv, "weighted_terms": w_terms, "templates_per_cta": tpc,
             "executed_fp32_lane_ops": lane_ops,
             "achieved": lane_ops / (k_ms_s * 1e-3) / 1e12, "peak": peak_ops / 1e12,
@@ -612,6 +619,42 @@ def run_ours(args):
     return 0
 
 
+def run_leg(args):
+    """One small workload, a few calls, for profiling (ncu -k ... python bench.py --leg ...): not a
+    bench line."""
+    import torch
+
+    import paper_1805_05652_b200 as pkg
+    from synth import make_workload
+    from synth.atoms import Grid as SGrid, make_atoms
+
+    torch.cuda.set_device(0)
+    if args.leg == "exp_scan":  # config 4 through the default (sliding) form
+        wl = make_workload(4, templates=list(range(args.templates)))
+        a, t = torch.from_numpy(wl.data.atoms).cuda(), torch.from_numpy(wl.data.t).cuda()
+        fn = lambda: pkg.tfstat_search(a, t, pkg.EXP, wl.grid)
+    elif args.leg == "rect_1yr":  # one year at dt0 = dtau = T_SFT, rows 16-byte aligned
+        n_y = 17520
+        t_y = np.arange(n_y, dtype=np.int64) * 1800
+        a = torch.from_numpy(make_atoms(t_y, np.random.default_rng(11)).astype(np.float32)).cuda()
+        t = torch.from_numpy(t_y.astype(np.int32)).cuda()
+        g_y = SGrid(0, 1800, n_y - 2, 3600, 1800, n_y - 4)
+        m_y = torch.empty((g_y.N_t0, g_y.N_tau), dtype=torch.float32, device="cuda")
+        fn = lambda: pkg.tfstat_map(a, t, pkg.RECT, g_y, out_map=m_y, rect_method=1)
+    elif args.leg == "cfg5_rect":
+        wl = make_workload(5)
+        a, t = torch.from_numpy(wl.data.atoms[0]).cuda(), torch.from_numpy(wl.data.t).cuda()
+        m5 = torch.empty((wl.grid.N_t0, wl.grid.N_tau), dtype=torch.float32, device="cuda")
+        fn = lambda: pkg.tfstat_map(a, t, pkg.RECT, wl.grid, out_map=m5)
+    else:
+        raise SystemExit(f"unknown --leg {args.leg}")
+    for _ in range(args.warmup):
+        fn()
+    ms = time_calls(torch, fn, args.steps)
+    print(json.dumps({"leg": args.leg, "ms_per_call": ms, "calls": args.steps}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -623,9 +666,13 @@ def main():
                          "for debugging only and are not a valid bench line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side", action="store_true", help="skip the other-config numbers")
+    ap.add_argument("--leg", default=None, choices=["exp_scan", "rect_1yr", "cfg5_rect"],
+                    help="profiling aid: run ONE small workload a few times and exit")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg:
+        return run_leg(args)
     return run_ours(args)
 
 

@@ -34,6 +34,16 @@ extern "C" {
 int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s, double *ops_per_clk_sm,
                      double *sm_mhz);
 
+/* The core loop of the direct exponential sum (exp_direct.cu) with NOTHING around it: 192 atoms
+ * resident in shared memory, summed `reps` times by 128-thread CTAs (4 per SM for 8 cells per
+ * thread, 3 for 16), in one of two accumulator layouts:
+ *   form 0  pairs of CHANNELS of one cell: FFMA2 acc, w (broadcast scalar), atom register pair
+ *   form 1  pairs of CELLS of one channel: FFMA2 acc, w, x (two broadcast scalars)
+ * cells = 8 or 16 per thread.  Outputs (HOST pointers): window-atom terms per SM clock per SM
+ * (clock64 span on SM 0) and terms per second over the whole GPU. */
+int tfstat_probe_direct_loop(int form, int cells, int reps, double *terms_per_clk_sm,
+                             double *terms_per_s);
+
 #ifdef __cplusplus
 }
 #endif

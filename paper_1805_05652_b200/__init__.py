@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     load_probe_library,
     plan_info,
     probe_alu,
+    probe_direct_loop,
     search_host_scratch_bytes,
     tfstat_map,
     tfstat_map_general,

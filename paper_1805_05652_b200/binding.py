@@ -115,6 +115,8 @@ def load_probe_library():
     lib = C.CDLL(_PROBE_LIB_PATH)
     lib.tfstat_probe_alu.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double),
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.tfstat_probe_direct_loop.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double),
+                                             C.POINTER(C.c_double)]
     _probe_lib = lib
     return lib
 
@@ -508,3 +510,15 @@ def probe_alu(kind: str, reps: int = 3) -> dict:
     if rc != 0:
         raise TfstatError(f"tfstat_probe_alu({kind}): status {rc}")
     return dict(kind=kind, lane_ops_per_s=a.value, ops_per_clk_sm=b.value, sm_mhz=c.value)
+
+
+def probe_direct_loop(form: int, cells: int, reps: int = 200) -> dict:
+    """The isolated core loop of the direct exponential sum in one of its two accumulator layouts
+    (tfstat_probe.h): 0 = channel pairs (scalar x register pair), 1 = cell pairs (two scalars)."""
+    lib = load_probe_library()
+    a, b = C.c_double(0), C.c_double(0)
+    rc = lib.tfstat_probe_direct_loop(int(form), int(cells), int(reps), C.byref(a), C.byref(b))
+    if rc != 0:
+        raise TfstatError(f"tfstat_probe_direct_loop({form}, {cells}): status {rc}")
+    return dict(form="cell_pairs" if form else "channel_pairs", cells=cells,
+                terms_per_clk_sm=a.value, terms_per_s=b.value)

@@ -315,7 +315,7 @@ __device__ __forceinline__ void exp_window_body(
     if (STATS) {
         unsigned long long nt = 0;
 #pragma unroll
-        for (int r = 0; r < RT; ++r) nt += (unsigned long long)(hi[r] - lo_m);
+        for (int r = 0; r < RT; ++r) nt += n_ok[r] ? (unsigned long long)(hi[r] - lo_m) : 0ull;
         nt *= (unsigned long long)min(TPC, pr.n_templates - tpl0);
 #pragma unroll
         for (int sft = 16; sft >= 1; sft >>= 1) nt += __shfl_xor_sync(0xffffffffu, nt, sft);

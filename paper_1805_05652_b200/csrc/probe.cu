@@ -8,6 +8,13 @@
 
 namespace {
 
+__device__ __forceinline__ float exp2f_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 constexpr int kNT = 256;
 constexpr int kIters = 4096;  // multiple of the unroll factor below
 constexpr int kChains = 16;
@@ -117,6 +124,153 @@ void launch(int grid, const float *in, float *out, long long *cyc)
 }
 
 }  // namespace
+
+// ---- the isolated core loop of the direct exponential sum, in two operand forms ---------------
+// (what bounds exp_direct_kernel once everything around the loop is taken away)
+namespace {
+
+typedef unsigned long long u64p;
+__device__ __forceinline__ u64p pk2(float lo, float hi)
+{
+    u64p r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(u64p v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ void fma2(u64p &d, u64p a, u64p b)
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+}
+constexpr int kLoopAtoms = 192;
+
+// FORM 0: accumulators paired by CHANNEL of one cell, (A,B) (Re Fa,Im Fa) (Re Fb,Im Fb) (C_c,C_c+1):
+//         FFMA2 acc, w.F32 (broadcast), x pair
+// FORM 1: accumulators paired by CELL, (X_c, X_c+1) for each of the 7 channels:
+//         FFMA2 acc, w.F32, x.F32 (two broadcast scalars)
+template <int FORM, int C, int MINB>
+__global__ void __launch_bounds__(128, MINB)
+    probe_loop_kernel(const ulonglong2 *__restrict__ g, float *__restrict__ out, const int reps,
+                      const float kexp0, long long *__restrict__ cycles)
+{
+    __shared__ ulonglong2 s[2 * kLoopAtoms];
+    for (int i = threadIdx.x; i < 2 * kLoopAtoms; i += 128) s[i] = g[i];
+    __syncthreads();
+    const float kexp = kexp0 * (1.0f + 1e-3f * threadIdx.x), cexp = 0.1f;
+    u64p acc[7 * C / 2];
+#pragma unroll
+    for (int i = 0; i < 7 * C / 2; ++i) acc[i] = 0ull;
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    const long long c0 = clock64();
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll 24
+        for (int i = 0; i < kLoopAtoms; ++i) {
+            const ulonglong2 ra = s[2 * i], rb = s[2 * i + 1];
+            float x[7], dt;
+            upk2(ra.x, dt, x[2]);
+            upk2(ra.y, x[0], x[1]);
+            upk2(rb.x, x[3], x[4]);
+            upk2(rb.y, x[5], x[6]);
+            const float w = exp2f_approx(fmaf(dt, kexp, cexp));
+            const float w2 = w * w;
+            const u64p ww = pk2(w, w), w2w2 = pk2(w2, w2);
+            if (FORM == 0) {
+                const u64p abab = pk2(x[2], x[2]);
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    fma2(acc[3 * c], w2w2, ra.y);
+                    fma2(acc[3 * c + 1], ww, rb.x);
+                    fma2(acc[3 * c + 2], ww, rb.y);
+                }
+#pragma unroll
+                for (int p = 0; p < C / 2; ++p) fma2(acc[3 * C + p], w2w2, abab);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 7; ++k) {
+                    const u64p xx = pk2(x[k], x[k]);
+#pragma unroll
+                    for (int p = 0; p < C / 2; ++p) fma2(acc[k * (C / 2) + p], k < 3 ? w2w2 : ww, xx);
+                }
+            }
+        }
+    }
+    const long long c1 = clock64();
+    float sum = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 7 * C / 2; ++i) {
+        float a, b;
+        upk2(acc[i], a, b);
+        sum += a + b;
+    }
+    out[(size_t)blockIdx.x * 128 + threadIdx.x] = sum;
+    if (smid == 0 && (threadIdx.x & 31) == 0) {
+        atomicMin(reinterpret_cast<unsigned long long *>(cycles), (unsigned long long)c0);
+        atomicMax(reinterpret_cast<unsigned long long *>(cycles) + 1, (unsigned long long)c1);
+    }
+}
+
+}  // namespace
+
+extern "C" int tfstat_probe_direct_loop(int form, int cells, int reps, double *terms_per_clk_sm,
+                                        double *terms_per_s)
+{
+    if ((form != 0 && form != 1) || (cells != 8 && cells != 16) || !terms_per_clk_sm)
+        return TFSTAT_EINVAL;
+    if (reps < 1) reps = 200;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return TFSTAT_ECUDA;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return TFSTAT_ECUDA;
+    const int per_sm = cells == 8 ? 4 : 3;
+    const int grid = n_sm * per_sm;
+    ulonglong2 *g = nullptr;
+    float *out = nullptr;
+    long long *cyc = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = TFSTAT_ECUDA;
+    do {
+        if (cudaMalloc(&g, sizeof(ulonglong2) * 2 * kLoopAtoms) != cudaSuccess) break;
+        if (cudaMalloc(&out, sizeof(float) * (size_t)grid * 128) != cudaSuccess) break;
+        if (cudaMalloc(&cyc, 2 * sizeof(long long)) != cudaSuccess) break;
+        float h[8 * kLoopAtoms];
+        for (int i = 0; i < kLoopAtoms; ++i) {
+            h[8 * i] = (float)i;
+            for (int k = 1; k < 8; ++k) h[8 * i + k] = 0.01f * k;
+        }
+        if (cudaMemcpy(g, h, sizeof(h), cudaMemcpyHostToDevice) != cudaSuccess) break;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+        float ms = 0.0f;
+        for (int pass = 0; pass < 2; ++pass) {  // warm-up, then the timed launch
+            const unsigned long long init[2] = {~0ull, 0ull};
+            cudaMemcpy(cyc, init, sizeof(init), cudaMemcpyHostToDevice);
+            cudaEventRecord(e0);
+            const int n = pass ? reps : 4;
+            if (form == 0 && cells == 8) probe_loop_kernel<0, 8, 4><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 1 && cells == 8) probe_loop_kernel<1, 8, 4><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 0 && cells == 16) probe_loop_kernel<0, 16, 3><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 1 && cells == 16) probe_loop_kernel<1, 16, 3><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            cudaEventRecord(e1);
+            if (cudaEventSynchronize(e1) != cudaSuccess) break;
+            cudaEventElapsedTime(&ms, e0, e1);
+        }
+        if (cudaGetLastError() != cudaSuccess || ms <= 0.0f) break;
+        unsigned long long span[2] = {0, 0};
+        if (cudaMemcpy(span, cyc, sizeof(span), cudaMemcpyDeviceToHost) != cudaSuccess) break;
+        const double terms_sm = (double)per_sm * 128 * cells * kLoopAtoms * reps;
+        *terms_per_clk_sm = terms_sm / (double)(span[1] - span[0]);
+        if (terms_per_s) *terms_per_s = terms_sm * n_sm / (ms * 1e-3);
+        rc = TFSTAT_OK;
+    } while (0);
+    cudaFree(g);
+    cudaFree(out);
+    cudaFree(cyc);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    return rc;
+}
 
 extern "C" int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s,
                                 double *ops_per_clk_sm, double *sm_mhz)

@@ -41,21 +41,14 @@ TSFT = 1800
 
 
 def _atoms(n_atoms: int, seed: int = 1):
-    """Gapless two-detector atoms with the sidereal-day antenna modulation of DESIGN.md 4 (values
-    only matter through the conditioning of the cells)."""
-    g = torch.Generator(device="cuda").manual_seed(seed)
-    t = torch.arange(n_atoms, device="cuda", dtype=torch.float64) * TSFT
-    ph = 2.0 * np.pi * t / 86164.0
-    a = [0.4 * torch.cos(ph + 0.3 + d) + 0.2 for d in (0, 1)]
-    b = [0.35 * torch.sin(ph + 1.1 + d) - 0.1 for d in (0, 1)]
-    n = [torch.complex(*(torch.randn(2, n_atoms, generator=g, device="cuda", dtype=torch.float64)
-                         * np.sqrt(0.5))) for _ in (0, 1)]
-    fa = a[0] * n[0] + a[1] * n[1]
-    fb = b[0] * n[0] + b[1] * n[1]
-    rows = [a[0] ** 2 + a[1] ** 2, b[0] ** 2 + b[1] ** 2, a[0] * b[0] + a[1] * b[1],
-            fa.real, fa.imag, fb.real, fb.imag]
-    atoms = torch.stack(rows).to(torch.float32).contiguous()
-    return atoms, (torch.arange(n_atoms, device="cuda", dtype=torch.int32) * TSFT).contiguous()
+    """Gapless two-detector atoms of the seeded input generators (`synth/`: the one
+    place the atom model lives; values only matter through the conditioning of the cells)."""
+    from synth.atoms import make_atoms  # the repo's input generators, not part of the product
+
+    t = np.arange(n_atoms, dtype=np.int64) * TSFT
+    atoms = make_atoms(t, np.random.default_rng(seed)).astype(np.float32)
+    return (torch.from_numpy(atoms).cuda().contiguous(),
+            torch.from_numpy(t.astype(np.int32)).cuda().contiguous())
 
 
 class _Grid:

@@ -38,7 +38,7 @@ def test_exports_every_declared_symbol(lib):
 
     probe = load_probe_library()
     pnames = declared_symbols("tfstat_probe.h")
-    assert pnames == {"tfstat_probe_alu"}
+    assert pnames == {"tfstat_probe_alu", "tfstat_probe_direct_loop"}
     for n in pnames:
         assert hasattr(probe, n)
         assert not hasattr(lib, n), f"{n} must not ship inside libtfstat.so"
@@ -78,7 +78,9 @@ def test_opts_struct_size_and_plan_info(lib):
     assert p.workspace_bytes == lib.tfstat_workspace_bytes(1, 2880, 4096, *b._grid_args(g), C.byref(o))
     # defaults: the sliding form; config 1: the one-launch rect kernel; invalid shapes: errors
     info = pkg.plan_info(pkg.EXP, 2880, 4096, g)
-    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 2
+    # (tile_c of the sliding form: templates per CTA of the slide kernel + 10 x (10 RT + TPC) of the
+    # window-sum kernel: 4 tau values per thread x 2 templates, 2 templates)
+    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 422 and info["n_launches"] == 5
     assert pkg.plan_info(pkg.RECT, 48, 1, G(0, 1800, 24, 1800, 1800, 24))["kernel_name"] == "rect_small"
     big = pkg.plan_info(pkg.RECT, 13140, 1, G(0, 1800, 17520, 43200, 43200, 720))
     assert big["kernel_name"] == "rect_run" and big["lattice_J"] == 17519 + 719 * 24 + 1
