@@ -35,7 +35,11 @@ namespace tfstat {
 namespace {
 
 constexpr float kReanchor = 4.0f;  // move t_ref when (t_ref - t0_m)/tau exceeds this
+constexpr float kReanchorArg = -kReanchor * 1.4426950408889634f;  // the same on (t_ref - t0_m) kexp
 constexpr float kGuard = 64.0f;    // re-sum a window whose A fell below 1/kGuard of its maximum
+#ifndef SLIDE_CTAS
+#define SLIDE_CTAS 4
+#endif
 constexpr int kSlideChunk = 128;   // atoms per bulk copy and template (4 KB); divides kPackBlock
 constexpr int kSlideStages = 3;    // ring slots per CTA
 constexpr int kWindowUnroll = 8;   // unroll of the initial-window loop
@@ -100,6 +104,15 @@ __device__ __forceinline__ void bulk_copy(const uint32_t dst, const void *src, c
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
             "r"(dst), "l"(src), "r"(bytes), "r"(bar)
         : "memory");
+}
+
+// one packed atom (32 bytes, 32-byte aligned) with ONE 256-bit load: a gather of 32 records costs
+// half the L1 wavefronts of two 128-bit loads per lane
+__device__ __forceinline__ void ldg_record(const ulonglong2 *p, ulonglong2 &ra, ulonglong2 &rb)
+{
+    asm("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];"
+        : "=l"(ra.x), "=l"(ra.y), "=l"(rb.x), "=l"(rb.y)
+        : "l"(p));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -343,7 +356,13 @@ __device__ __forceinline__ void exp_slide_body(
     const float4 *W0, Partial *__restrict__ partials, const unsigned vblock, const int n_nblocks,
     const int n_segs, const int seg_len, unsigned long long *__restrict__ stats)
 {
+    constexpr unsigned kFull = 0xffffffffu;
+    constexpr int NW = NT / 32;
     __shared__ Marg s_red[32];
+    // the atoms that ENTER the windows are the same for every lane (they depend on t0 only): each
+    // warp keeps the next 32 of them, for its TPC templates, in shared memory (see the fast path)
+    __shared__ __align__(16) ulonglong2 s_in[NW][TPC][64];
+    __shared__ int s_tin[NW][32];
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -357,34 +376,37 @@ __device__ __forceinline__ void exp_slide_body(
     const int m_beg = seg * seg_len;
     const int m_end = min(m_beg + seg_len, g.N_t0);
 
-    // templates beyond the batch (ragged last group) alias the last real one; nothing of theirs
-    // is stored
+    // Templates beyond the batch (ragged last group) alias the last real one, tau slots beyond
+    // the grid alias the block's last tau: they run the same instructions as their neighbours
+    // (the fast path below is taken warp by warp) and nothing of theirs is stored.
     const ulonglong2 *__restrict__ rec[TPC];
-    const float *__restrict__ base[TPC];
 #pragma unroll
-    for (int q = 0; q < TPC; ++q) {
-        const int tq = min(tpl0 + q, pr.n_templates - 1);
-        rec[q] = packed + (int64_t)tq * n_pad * 2;
-        base[q] = pr.atoms + (int64_t)tq * pr.template_stride;
-    }
-    const int64_t ld = pr.ld;
+    for (int q = 0; q < TPC; ++q)
+        rec[q] = packed + (int64_t)min(tpl0 + q, pr.n_templates - 1) * n_pad * 2;
     const bool n_ok = (int)threadIdx.x < n_count;
-    const int n = n_first + (n_ok ? (int)threadIdx.x : 0);
-    const double tau = (double)tau_of(g, n);
-    const float kexp = (float)(-1.4426950408889634 / tau);
-    const float inv_tau = (float)(1.0 / tau);
+    const int n = n_first + min((int)threadIdx.x, n_count - 1);
+    const float kexp = (float)(-1.4426950408889634 / (double)tau_of(g, n));
+    const int a_last = bd.n_atoms - 1;
+    const int warp = (int)threadIdx.x >> 5;
+    // window end of cell (mm, n): one entry of the lattice table (bounds.cu), else a binary search
+    const bool has_edge = bd.edge != nullptr;
+    const int jn = n * bd.e_n;  // (the lattice has at most 2^22 points: 32-bit indices)
+    auto hi_at = [&](const int mm) {
+        return has_edge ? __ldg(bd.edge + (jn + mm * bd.e_m)) : hi_index(bd, g, mm, n);
+    };
+    int in_base = 0x7fffffff;  // first atom of the warp's staged entering atoms (none yet)
 
     // ---- the segment's last cell (m_end - 1, n): its window sums come from exp_window_kernel ----
     int m = m_end - 1;
     int lo_m = __ldg(bd.lo + m);
-    int hi = n_ok ? max(hi_index(bd, g, m, n), lo_m) : lo_m;
+    int hi = max(hi_at(m), lo_m);
     int t_ref = (int)t0_of(g, m);  // seconds (int32: every grid time fits, TFSTAT_EOVERFLOW otherwise)
     SlideAcc acc[TPC];
     float A_max[TPC];
 #pragma unroll
     for (int q = 0; q < TPC; ++q) {
         const int tq = min(tpl0 + q, pr.n_templates - 1);
-        // (plain loads: in the fused kernel W0 was written by this very CTA a moment ago)
+        // (plain loads: in a fused kernel W0 would have been written by this very CTA)
         const float4 *w = W0 + (((int64_t)tq * n_segs + seg) * g.N_tau + n) * 2;
         const float4 w0 = w[0], w1 = w[1];
         acc[q].ab = pack2(w0.x, w0.y);
@@ -422,73 +444,131 @@ __device__ __forceinline__ void exp_slide_body(
 
     // marginals per template: running max (ties: this thread's flat indices only decrease, so the
     // later cell wins) and log-sum-exp against a reference that moves rarely
+    // (mg_m: the row of the best cell; n_bad: cells that do not count -- flagged ones)
     float mg_best[TPC], mg_ref2[TPC], mg_sum[TPC];
-    int32_t mg_idx[TPC], mg_nv[TPC];
+    int32_t mg_m[TPC], n_bad[TPC];
 #pragma unroll
     for (int q = 0; q < TPC; ++q) {
         mg_best[q] = -INFINITY;
-        mg_idx[q] = 0x7fffffff;
+        mg_m[q] = 0;
         mg_ref2[q] = -1.0e30f;
         mg_sum[q] = 0.0f;
-        mg_nv[q] = 0;
+        n_bad[q] = 0;
     }
     const int64_t cells = (int64_t)g.N_t0 * g.N_tau;
 
+    // a4 + a5 of cell (m, n) of template q, the careful way: fp32 closure where the cell is well
+    // conditioned and in range, closure_2F_exp (fp64, re-sum of short windows) otherwise
+    auto close_full = [&](const int q, const int cnt) {
+        const int32_t flat = m * g.N_tau + n;
+        float A, B, far, fai, fbr, fbi;
+        unpack2(acc[q].ab, A, B);
+        unpack2(acc[q].fa, far, fai);
+        unpack2(acc[q].fb, fbr, fbi);
+        const float C = acc[q].c;
+        const float p = A * B;
+        const float D = fmaf(-C, C, p);
+        const float na = fmaf(far, far, fai * fai);
+        const float nb = fmaf(fbr, fbr, fbi * fbi);
+        const float re = fmaf(far, fbr, fai * fbi);
+        float num = B * na;
+        num = fmaf(A, nb, num);
+        num = fmaf(-2.0f * C, re, num);
+        float twoF = 2.0f * num * rcp_approx_s(D);
+        uint32_t fl = 0u;
+        if (!(D > 0.015625f * p && p > 1.0e-30f && p < 1.0e30f && cnt >= pr.min_atoms &&
+              fabsf(twoF) < 3.0e38f)) {
+            const int tq = min(tpl0 + q, pr.n_templates - 1);
+            twoF = closure_2F_exp<false>(A, B, C, far, fai, fbr, fbi, lo_m, cnt, pr.min_atoms, fl,
+                                         pr.atoms + (int64_t)tq * pr.template_stride, pr.ld, bd.t,
+                                         t0_of(g, m), (double)tau_of(g, n));
+        }
+        if (n_ok && tpl0 + q < pr.n_templates) {
+            const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
+            if (pr.out_maps) pr.out_maps[o] = twoF;
+            if (pr.out_flags) pr.out_flags[o] = (uint8_t)fl;
+        }
+        if (!fl) {
+            if (twoF >= mg_best[q]) {
+                mg_best[q] = twoF;
+                mg_m[q] = m;
+            }
+            if (fmaf(twoF, kHalfLog2eS, -mg_ref2[q]) > 60.0f) {  // rare: move the reference
+                mg_sum[q] *= ex2_approx(mg_ref2[q] - twoF * kHalfLog2eS);
+                mg_ref2[q] = twoF * kHalfLog2eS;
+            }
+            mg_sum[q] += ex2_approx(fmaf(twoF, kHalfLog2eS, -mg_ref2[q]));
+        } else {
+            n_bad[q] += 1;
+        }
+    };
+
     // ---- slide backwards in t0: closure of cell m, then step to m - 1 ------------------------
-    // indices of the step m -> m - 1, requested one step ahead
+    // A t0 step is a chain of dependent loads (row start -> window end -> atom records) in front
+    // of the arithmetic, so the indices of the step m -> m - 1 are requested one step ahead and
+    // the records of its atoms BEFORE cell m is closed.
+    //
+    // FAST PATH, taken when every lane of the warp is in the common case -- at most one atom
+    // enters and one leaves, the windows of m and m - 1 overlap, t_ref stays: straight-line code.
+    // An atom that does not exist (n_in = 0, n_out = 0) is loaded from a clamped address and
+    // gets the weight 0 by a select.  Cells are closed in fp32 and the lanes VOTE on whether any
+    // of them needs the careful closure; the marginals are updated without branches.  Everything
+    // else (several atoms per step, disjoint windows, re-anchoring, the segment's first row)
+    // takes the generic path below.  ncu on config 4 before this split: 304 warp instructions
+    // per step, of which 50 BRA/BSSY/BSYNC, 47 integer compares and 21 spill loads/stores.
     int lo2 = lo_m, hi2 = hi;
     if (m > m_beg) {
         lo2 = __ldg(bd.lo + m - 1);
-        hi2 = n_ok ? max(hi_index(bd, g, m - 1, n), lo2) : lo2;
+        hi2 = max(hi_at(m - 1), lo2);
     }
+    // (a warp whose tau slots all lie beyond the grid has nothing to do but the final reduction)
 #pragma unroll 1
-    for (;;) {
+    for (; warp * 32 < n_count;) {
         const bool last = m == m_beg;
-        // -- this step's atoms: in the common case at most one enters and one leaves; their
-        // records are requested now and used after the closure
         const int n_in = lo_m - lo2, lv = max(hi2, lo_m), n_out = hi - lv;
         const bool fresh0 = (hi2 <= lo_m) || (hi2 == lo2);  // no overlap with window m, or empty
-        const bool simple = !last && !fresh0 && n_in <= 1 && n_out <= 1;
-        ulonglong2 ia[TPC], ib[TPC], oa[TPC], ob[TPC];
-        int t_in = 0, t_out = 0;
-        if (simple) {
-            if (n_in == 1) {
-                t_in = __ldg(bd.t + lo2);
-#pragma unroll
-                for (int q = 0; q < TPC; ++q) {
-                    ia[q] = __ldg(rec[q] + 2 * (int64_t)lo2);
-                    ib[q] = __ldg(rec[q] + 2 * (int64_t)lo2 + 1);
-                }
-            }
-            if (n_out == 1) {
-                t_out = __ldg(bd.t + lv);
-#pragma unroll
-                for (int q = 0; q < TPC; ++q) {
-                    oa[q] = __ldg(rec[q] + 2 * (int64_t)lv);
-                    ob[q] = __ldg(rec[q] + 2 * (int64_t)lv + 1);
-                }
-            }
-        }
-        // -- indices of the step after this one
+        const int t0_2 = (int)t0_of(g, m - 1);
+        const float sh = (float)(t_ref - t0_2);
+        const bool calm =
+            has_edge && !fresh0 && n_in <= 1 && n_out <= 1 && !(sh * kexp < kReanchorArg);
+        const int cnt = hi - lo_m;
         int lo3 = lo2, hi3 = hi2;
-        if (m - 1 > m_beg) {
-            lo3 = __ldg(bd.lo + m - 2);
-            hi3 = n_ok ? max(hi_index(bd, g, m - 2, n), lo3) : lo3;
-        }
-
-        // -- a4 + a5: cell (m, n) of every template
-        if (n_ok) {
-            const int32_t flat = m * g.N_tau + n;
-            const int cnt = hi - lo_m;
+        bool fresh;
+        if (!last && __all_sync(kFull, calm)) {
+            // -- the entering atom is the same for all lanes: the warp stages 32 of them at a time
+            // in shared memory (coalesced, once per 32 steps) and reads them back by broadcast
+            const int a_in = min(lo2, a_last), a_out = min(lv, a_last);
+            if ((unsigned)(a_in - in_base) >= 32u) {  // warp-uniform
+                in_base = max(a_in - 31, 0);
+                const int al = min(in_base + lane, a_last);
+                __syncwarp();
+                s_tin[warp][lane] = __ldg(bd.t + al);
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    s_in[warp][q][2 * lane] = __ldg(rec[q] + 2 * al);
+                    s_in[warp][q][2 * lane + 1] = __ldg(rec[q] + 2 * al + 1);
+                }
+                __syncwarp();
+            }
+            // -- records of the leaving atom (one gather per lane), indices of the next step
+            const int t_out = __ldg(bd.t + a_out);
+            ulonglong2 oa[TPC], ob[TPC];
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) ldg_record(rec[q] + 2 * a_out, oa[q], ob[q]);
+            if (m - 1 > m_beg) {
+                lo3 = __ldg(bd.lo + m - 2);
+                hi3 = max(__ldg(bd.edge + (jn + (m - 2) * bd.e_m)), lo3);
+            }
+            // -- a4: eq. (7) in fp32 for the TPC templates, one vote on "all well conditioned"
+            float twoF[TPC];
+            bool bad = cnt < pr.min_atoms;
 #pragma unroll
             for (int q = 0; q < TPC; ++q) {
-                if (tpl0 + q >= pr.n_templates) continue;
                 float A, B, far, fai, fbr, fbi;
                 unpack2(acc[q].ab, A, B);
                 unpack2(acc[q].fa, far, fai);
                 unpack2(acc[q].fb, fbr, fbi);
                 const float C = acc[q].c;
-                // fp32 closure where the cell is well conditioned and in range (tfstat_dev.cuh)
                 const float p = A * B;
                 const float D = fmaf(-C, C, p);
                 const float na = fmaf(far, far, fai * fai);
@@ -497,66 +577,114 @@ __device__ __forceinline__ void exp_slide_body(
                 float num = B * na;
                 num = fmaf(A, nb, num);
                 num = fmaf(-2.0f * C, re, num);
-                float twoF = 2.0f * num * rcp_approx_s(D);
-                uint32_t fl = 0u;
-                if (!(D > 0.015625f * p && p > 1.0e-30f && p < 1.0e30f && cnt >= pr.min_atoms &&
-                      fabsf(twoF) < 3.0e38f))
-                    twoF = closure_2F_exp<false>(A, B, C, far, fai, fbr, fbi, lo_m, cnt,
-                                                 pr.min_atoms, fl, base[q], ld, bd.t, t0_of(g, m),
-                                                 tau);
-                const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
-                if (pr.out_maps) pr.out_maps[o] = twoF;
-                if (pr.out_flags) pr.out_flags[o] = (uint8_t)fl;
-                if (!fl) {
-                    if (twoF >= mg_best[q]) {  // rare after the first few cells
-                        mg_best[q] = twoF;
-                        mg_idx[q] = flat;
-                    }
-                    if (fmaf(twoF, kHalfLog2eS, -mg_ref2[q]) > 60.0f) {  // rare: move the reference
-                        mg_sum[q] *= ex2_approx(mg_ref2[q] - twoF * kHalfLog2eS);
-                        mg_ref2[q] = twoF * kHalfLog2eS;
-                    }
-                    mg_sum[q] += ex2_approx(fmaf(twoF, kHalfLog2eS, -mg_ref2[q]));
-                    mg_nv[q] += 1;
-                }
+                twoF[q] = 2.0f * num * rcp_approx_s(D);
+                // (no short-circuit: four compares into one predicate)
+                const bool ok = (D > 0.015625f * p) & (p > 1.0e-30f) & (p < 1.0e30f) &
+                                (fabsf(twoF[q]) < 3.0e38f);
+                bad = bad | !ok;
             }
-        }
-        if (last) break;
-
-        // -- the sums move on to cell m - 1
-        const int t0_2 = (int)t0_of(g, m - 1);
-        bool fresh = fresh0;
-        if (!fresh) {
-            const float sh = (float)(t_ref - t0_2);
-            if (sh * inv_tau > kReanchor) {  // keep the weights of entering atoms <= e^kReanchor
-                const float c = ex2_approx(sh * kexp);
+            if (__any_sync(kFull, bad)) {
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) close_full(q, cnt);
+            } else {
+                // -- a5, branch-free
+                if (pr.out_maps) {  // (uniform; a search stores no maps)
+                    const int32_t flat = m * g.N_tau + n;
+#pragma unroll
+                    for (int q = 0; q < TPC; ++q)
+                        if (n_ok && tpl0 + q < pr.n_templates) {
+                            const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
+                            pr.out_maps[o] = twoF[q];
+                            if (pr.out_flags) pr.out_flags[o] = (uint8_t)0;
+                        }
+                }
+                float x[TPC];
+                bool move = false;
 #pragma unroll
                 for (int q = 0; q < TPC; ++q) {
-                    acc_scale(acc[q], c);
-                    A_max[q] *= c * c;
+                    const bool better = twoF[q] >= mg_best[q];
+                    mg_best[q] = better ? twoF[q] : mg_best[q];
+                    mg_m[q] = better ? m : mg_m[q];
+                    x[q] = fmaf(twoF[q], kHalfLog2eS, -mg_ref2[q]);
+                    move = move | (x[q] > 60.0f);
                 }
-                t_ref = t0_2;
+                if (__any_sync(kFull, move)) {  // rare: move the reference of the log-sum-exp
+#pragma unroll
+                    for (int q = 0; q < TPC; ++q)
+                        if (x[q] > 60.0f) {
+                            mg_sum[q] *= ex2_approx(-x[q]);
+                            mg_ref2[q] = twoF[q] * kHalfLog2eS;
+                            x[q] = 0.0f;
+                        }
+                }
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    mg_sum[q] += ex2_approx(x[q]);
+                }
             }
-            if (simple) {
-                if (n_in == 1) add_records(t_in, ia, ib, 1.0f);
-                if (n_out == 1) add_records(t_out, oa, ob, -1.0f);
-            } else {
-                for (int al = lo2; al < lo_m; ++al) add_global(al, 1.0f);  // entering, low end
-                for (int al = lv; al < hi; ++al) add_global(al, -1.0f);    // leaving, high end
-            }
-            if (STATS) {
-                n_term[1] += (unsigned)n_in;
-                n_term[2] += (unsigned)max(n_out, 0);
-            }
+            // -- the sums move on to cell m - 1
+            const int t_in = s_tin[warp][a_in - in_base];
+            const float e_in = ex2_approx((float)(t_in - t_ref) * kexp);
+            const float e_out = ex2_approx((float)(t_out - t_ref) * kexp);
+            fresh = false;
 #pragma unroll
             for (int q = 0; q < TPC; ++q) {
+                const ulonglong2 ia = s_in[warp][q][2 * (a_in - in_base)];
+                const ulonglong2 ib = s_in[warp][q][2 * (a_in - in_base) + 1];
+                float dtc, ab;
+                unpack2(ia.x, dtc, ab);
+                // (fmaf(dtc, 0, e): NaN for an atom that is not finite, pack.cu; the select keeps
+                // an atom that is not part of this step out even then)
+                const float wi = n_in ? fmaf(dtc, 0.0f, e_in) : 0.0f;
+                acc_add(acc[q], wi, wi * wi, ia, ib);
+                unpack2(oa[q].x, dtc, ab);
+                const float wo = n_out ? -fmaf(dtc, 0.0f, e_out) : 0.0f;
+                acc_add(acc[q], wo, wo * fabsf(wo), oa[q], ob[q]);
                 float A, B;
                 unpack2(acc[q].ab, A, B);
                 A_max[q] = fmaxf(A_max[q], A);
-                // a window that lost most of its weight is re-summed (for all TPC templates: a
-                // fresh sum is always right); written so that a NaN / inf atom in the running sums
-                // also forces a fresh sum: once it has left the window it must not linger
-                fresh = fresh || !(A * kGuard >= A_max[q]);
+                fresh = fresh | !(A * kGuard >= A_max[q]);  // (see the generic path)
+            }
+            if (STATS) {
+                n_term[1] += (unsigned)n_in;
+                n_term[2] += (unsigned)n_out;
+            }
+        } else {
+            // -- generic path: the same steps with loops and branches
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) close_full(q, cnt);
+            if (last) break;
+            if (m - 1 > m_beg) {
+                lo3 = __ldg(bd.lo + m - 2);
+                hi3 = max(hi_at(m - 2), lo3);
+            }
+            fresh = fresh0;
+            if (!fresh) {
+                if (sh * kexp < kReanchorArg) {  // keep the weights of entering atoms <= e^kReanchor
+                    const float c = ex2_approx(sh * kexp);
+#pragma unroll
+                    for (int q = 0; q < TPC; ++q) {
+                        acc_scale(acc[q], c);
+                        A_max[q] *= c * c;
+                    }
+                    t_ref = t0_2;
+                }
+                for (int al = lo2; al < lo_m; ++al) add_global(al, 1.0f);  // entering, low end
+                for (int al = lv; al < hi; ++al) add_global(al, -1.0f);    // leaving, high end
+                if (STATS) {
+                    n_term[1] += (unsigned)n_in;
+                    n_term[2] += (unsigned)max(n_out, 0);
+                }
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    float A, B;
+                    unpack2(acc[q].ab, A, B);
+                    A_max[q] = fmaxf(A_max[q], A);
+                    // a window that lost most of its weight is re-summed (for all TPC templates: a
+                    // fresh sum is always right); written so that a NaN / inf atom in the running sums
+                    // also forces a fresh sum: once it has left the window it must not linger
+                    fresh = fresh || !(A * kGuard >= A_max[q]);
+                }
             }
         }
         if (fresh) {
@@ -578,13 +706,14 @@ __device__ __forceinline__ void exp_slide_body(
         lo2 = lo3;
         hi2 = hi3;
     }
+    const int n_visited = warp * 32 < n_count ? m_end - m_beg : 0;
     if (STATS) {
         // (terms of out-of-range tau slots and of ragged template groups were not summed for real)
         unsigned long long v[5];
-        const unsigned long long ntpl = (unsigned long long)min(TPC, pr.n_templates - tpl0);
+        const unsigned long long ntpl = n_ok ? (unsigned long long)min(TPC, pr.n_templates - tpl0) : 0ull;
 #pragma unroll
         for (int i = 0; i < 4; ++i) v[i] = (unsigned long long)n_term[i] * ntpl;
-        v[4] = (n_ok ? 1ull : 0ull) * (unsigned long long)(m_end - m_beg) * ntpl;
+        v[4] = (unsigned long long)(m_end - m_beg) * ntpl;
 #pragma unroll
         for (int i = 1; i < 5; ++i) {
 #pragma unroll
@@ -597,12 +726,13 @@ __device__ __forceinline__ void exp_slide_body(
         for (int q = 0; q < TPC; ++q) {
             Marg a;
             marg_init(a);
-            if (mg_nv[q] > 0) {
+            const int nv = n_visited - n_bad[q];
+            if (n_ok && nv > 0) {
                 a.best = mg_best[q];
-                a.idx = mg_idx[q];
+                a.idx = mg_m[q] * g.N_tau + n;
                 a.M = 0.5f * mg_best[q];
                 a.S = mg_sum[q] * ex2_approx(mg_ref2[q] - mg_best[q] * kHalfLog2eS);
-                a.nvalid = mg_nv[q];
+                a.nvalid = nv;
             }
             __syncthreads();  // s_red is reused (by the next template, the next pass)
             marg_block_reduce<NT>(a, s_red);
@@ -626,7 +756,7 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
 }
 
 template <int NT, int TPC, bool STATS>
-__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : 4) : 1)
+__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : SLIDE_CTAS) : 1)
     exp_slide_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
                      const float4 *__restrict__ W0, Partial *__restrict__ partials,
                      const int n_nblocks, const int n_segs, const int seg_len,
