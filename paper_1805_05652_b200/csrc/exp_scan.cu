@@ -339,133 +339,142 @@ __device__ __forceinline__ void exp_window_body(
 // ---------------------------------------------------------------------------------------
 // exp_slide_kernel: a thread owns one tau x TPC templates, starts from the window sums of the
 // segment's last t0 (exp_window_kernel) and slides backwards in t0.  The weights E_a depend on
-// (atom, tau) only, so one MUFU.EX2 (+ its argument and E^2) serves the TPC templates.  The atoms
-// that enter (the same for every thread of the CTA) and leave (one gather per thread) come from
-// the packed records with two 16-byte loads each.
+// (atom, tau) only, so one MUFU.EX2 (+ its argument and E^2) serves the TPC templates.
 //
-// A t0 step is a chain of dependent loads (row start -> window end -> atom records) in front of a
-// few dozen arithmetic instructions, so the loop is software-pipelined by hand: the indices of
-// step m - 2 and the records of the atoms of step m - 1 are requested BEFORE cell m is closed
-// (eq. 7), and are in registers by the time the sums move on.
+// A t0 step is a chain of dependent loads (row start -> window end -> atom records) in front of
+// the arithmetic, so the indices of the step m -> m - 1 are requested one step ahead and the
+// record of the leaving atom BEFORE cell m is closed.
+//
+// FAST PATH, taken when every lane of the warp is in the common case -- at most one atom enters
+// and one leaves, the windows of m and m - 1 overlap, t_ref stays, every cell of the warp is
+// well conditioned: straight-line code.  The entering atom is the same for all lanes (it depends
+// on t0 only): each warp stages 32 of them at a time in shared memory (coalesced, once per 32
+// steps) and reads them back by broadcast; the leaving atom is one gather per lane, one 256-bit
+// load per template.  An atom that does not exist (n_in = 0, n_out = 0) is read from a clamped
+// address and gets the weight 0 by a select.  Cells are closed in fp32 and the lanes VOTE on
+// whether any of them needs the careful closure; the marginals are updated without branches.
+// Everything else (several atoms per step, disjoint windows, re-anchoring, ill-conditioned or
+// short cells, the segment's first row, re-summing a window that lost its weight) is in two
+// functions that are NOT inlined and work on a copy of the thread's state in local memory, so
+// that the register allocation of the loop is that of the fast path alone.  ncu on config 4
+// with everything in one loop body: 304 warp instructions per step, of which 50
+// BRA/BSSY/BSYNC, 47 integer compares and 21 spill loads/stores; L1 wavefronts 62 % of peak.
 // ---------------------------------------------------------------------------------------
 constexpr float kHalfLog2eS = 0.72134752044448170368f;  // log2(e) / 2: F log2e = 2F * this
 
-template <int NT, int TPC, bool STATS>
-__device__ __forceinline__ void exp_slide_body(
-    const Problem &pr, const ulonglong2 *__restrict__ packed, const int n_pad,
-    const float4 *W0, Partial *__restrict__ partials, const unsigned vblock, const int n_nblocks,
-    const int n_segs, const int seg_len, unsigned long long *__restrict__ stats)
-{
-    constexpr unsigned kFull = 0xffffffffu;
-    constexpr int NW = NT / 32;
-    __shared__ Marg s_red[32];
-    // the atoms that ENTER the windows are the same for every lane (they depend on t0 only): each
-    // warp keeps the next 32 of them, for its TPC templates, in shared memory (see the fast path)
-    __shared__ __align__(16) ulonglong2 s_in[NW][TPC][64];
-    __shared__ int s_tin[NW][32];
-
-    const Grid g = pr.grid;
-    const Bounds &bd = pr.bounds;
-    const int lane = threadIdx.x & 31;
-    // vblock = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
-    const int j = (int)(vblock % n_nblocks);
-    const int seg = (int)((vblock / n_nblocks) % n_segs);
-    const int tpl0 = (int)(vblock / ((int64_t)n_nblocks * n_segs)) * TPC;
-    const int n_first = (n_nblocks - 1 - j) * NT;
-    const int n_count = min(NT, g.N_tau - n_first);
-    const int m_beg = seg * seg_len;
-    const int m_end = min(m_beg + seg_len, g.N_t0);
-
-    // Templates beyond the batch (ragged last group) alias the last real one, tau slots beyond
-    // the grid alias the block's last tau: they run the same instructions as their neighbours
-    // (the fast path below is taken warp by warp) and nothing of theirs is stored.
-    const ulonglong2 *__restrict__ rec[TPC];
-#pragma unroll
-    for (int q = 0; q < TPC; ++q)
-        rec[q] = packed + (int64_t)min(tpl0 + q, pr.n_templates - 1) * n_pad * 2;
-    const bool n_ok = (int)threadIdx.x < n_count;
-    const int n = n_first + min((int)threadIdx.x, n_count - 1);
-    const float kexp = (float)(-1.4426950408889634 / (double)tau_of(g, n));
-    const int a_last = bd.n_atoms - 1;
-    const int warp = (int)threadIdx.x >> 5;
-    // window end of cell (mm, n): one entry of the lattice table (bounds.cu), else a binary search
-    const bool has_edge = bd.edge != nullptr;
-    const int jn = n * bd.e_n;  // (the lattice has at most 2^22 points: 32-bit indices)
-    auto hi_at = [&](const int mm) {
-        return has_edge ? __ldg(bd.edge + (jn + mm * bd.e_m)) : hi_index(bd, g, mm, n);
-    };
-    int in_base = 0x7fffffff;  // first atom of the warp's staged entering atoms (none yet)
-
-    // ---- the segment's last cell (m_end - 1, n): its window sums come from exp_window_kernel ----
-    int m = m_end - 1;
-    int lo_m = __ldg(bd.lo + m);
-    int hi = max(hi_at(m), lo_m);
-    int t_ref = (int)t0_of(g, m);  // seconds (int32: every grid time fits, TFSTAT_EOVERFLOW otherwise)
+template <int TPC>
+struct SlideState {
     SlideAcc acc[TPC];
     float A_max[TPC];
-#pragma unroll
-    for (int q = 0; q < TPC; ++q) {
-        const int tq = min(tpl0 + q, pr.n_templates - 1);
-        // (plain loads: in a fused kernel W0 would have been written by this very CTA)
-        const float4 *w = W0 + (((int64_t)tq * n_segs + seg) * g.N_tau + n) * 2;
-        const float4 w0 = w[0], w1 = w[1];
-        acc[q].ab = pack2(w0.x, w0.y);
-        acc[q].c = w0.z;
-        acc[q].fa = pack2(w0.w, w1.x);
-        acc[q].fb = pack2(w1.y, w1.z);
-        A_max[q] = w0.x;
-    }
-    unsigned n_term[4] = {0u, 0u, 0u, 0u};  // STATS: (window), enter, leave, re-sum (x TPC templates)
-
-    // one atom straight from the packed records (entering / leaving / re-summed atoms), one weight
-    // for the TPC templates
-    auto add_records = [&](const int t_al, const ulonglong2 (&ra)[TPC], const ulonglong2 (&rb)[TPC],
-                           const float sign) {
-        const float dt = (float)(t_al - t_ref);
-        const float e = ex2_approx(dt * kexp);
-#pragma unroll
-        for (int q = 0; q < TPC; ++q) {
-            float dtc, ab;
-            unpack2(ra[q].x, dtc, ab);
-            const float eq = fmaf(dtc, 0.0f, e);  // NaN for an atom that is not finite (pack.cu)
-            const float w = sign * eq;
-            acc_add(acc[q], w, w * eq, ra[q], rb[q]);
-        }
-    };
-    auto add_global = [&](const int al, const float sign) {
-        ulonglong2 ra[TPC], rb[TPC];
-#pragma unroll
-        for (int q = 0; q < TPC; ++q) {
-            ra[q] = __ldg(rec[q] + 2 * (int64_t)al);
-            rb[q] = __ldg(rec[q] + 2 * (int64_t)al + 1);
-        }
-        add_records(__ldg(bd.t + al), ra, rb, sign);
-    };
-
-    // marginals per template: running max (ties: this thread's flat indices only decrease, so the
-    // later cell wins) and log-sum-exp against a reference that moves rarely
-    // (mg_m: the row of the best cell; n_bad: cells that do not count -- flagged ones)
+    // marginals per template: running max (ties: a thread's rows only decrease, so the later cell
+    // wins), the row of the best cell, log-sum-exp against a reference that moves rarely, and the
+    // number of cells that do not count (flagged ones)
     float mg_best[TPC], mg_ref2[TPC], mg_sum[TPC];
     int32_t mg_m[TPC], n_bad[TPC];
+    int m, lo_m, hi, lo2, hi2, t_ref;
+    unsigned n_term[4];  // STATS: (window), enter, leave, re-sum (x TPC templates)
+};
+
+struct SlideCtx {  // what a thread's cold paths need besides its state
+    const ulonglong2 *packed;
+    int n_pad, tpl0, n, n_ok, m_beg;
+    float kexp;
+};
+
+template <int TPC>
+__device__ __forceinline__ void slide_copy(SlideState<TPC> &d, const SlideState<TPC> &s)
+{
 #pragma unroll
     for (int q = 0; q < TPC; ++q) {
-        mg_best[q] = -INFINITY;
-        mg_m[q] = 0;
-        mg_ref2[q] = -1.0e30f;
-        mg_sum[q] = 0.0f;
-        n_bad[q] = 0;
+        d.acc[q].ab = s.acc[q].ab;
+        d.acc[q].fa = s.acc[q].fa;
+        d.acc[q].fb = s.acc[q].fb;
+        d.acc[q].c = s.acc[q].c;
+        d.A_max[q] = s.A_max[q];
+        d.mg_best[q] = s.mg_best[q];
+        d.mg_ref2[q] = s.mg_ref2[q];
+        d.mg_sum[q] = s.mg_sum[q];
+        d.mg_m[q] = s.mg_m[q];
+        d.n_bad[q] = s.n_bad[q];
     }
-    const int64_t cells = (int64_t)g.N_t0 * g.N_tau;
+    d.m = s.m;
+    d.lo_m = s.lo_m;
+    d.hi = s.hi;
+    d.lo2 = s.lo2;
+    d.hi2 = s.hi2;
+    d.t_ref = s.t_ref;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) d.n_term[i] = s.n_term[i];
+}
 
-    // a4 + a5 of cell (m, n) of template q, the careful way: fp32 closure where the cell is well
-    // conditioned and in range, closure_2F_exp (fp64, re-sum of short windows) otherwise
-    auto close_full = [&](const int q, const int cnt) {
-        const int32_t flat = m * g.N_tau + n;
+// acc += sign * E x for one atom read straight from the packed records, one weight for the TPC
+// templates
+template <int TPC>
+__device__ __forceinline__ void slide_add_global(SlideState<TPC> &s, const Bounds &bd,
+                                                 const ulonglong2 *const (&rec)[TPC],
+                                                 const float kexp, const int al, const float sign)
+{
+    const float e = ex2_approx((float)(__ldg(bd.t + al) - s.t_ref) * kexp);
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
+        const ulonglong2 ra = __ldg(rec[q] + 2 * (int64_t)al), rb = __ldg(rec[q] + 2 * (int64_t)al + 1);
+        float dtc, ab;
+        unpack2(ra.x, dtc, ab);
+        const float eq = fmaf(dtc, 0.0f, e);  // NaN for an atom that is not finite (pack.cu)
+        const float w = sign * eq;
+        acc_add(s.acc[q], w, w * eq, ra, rb);
+    }
+}
+
+// a window summed afresh (t_ref = the t0 of row m - 1): lanes whose window lost most of its
+// weight, or does not overlap its neighbour
+template <int TPC, bool STATS>
+__device__ __noinline__ void slide_resum(SlideState<TPC> &s, const Problem &pr, const SlideCtx &c)
+{
+    const ulonglong2 *rec[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
+        rec[q] = c.packed + (int64_t)min(c.tpl0 + q, pr.n_templates - 1) * c.n_pad * 2;
+        acc_zero(s.acc[q]);
+    }
+    s.t_ref = (int)t0_of(pr.grid, s.m - 1);
+    for (int al = s.lo2; al < s.hi2; ++al) slide_add_global<TPC>(s, pr.bounds, rec, c.kexp, al, 1.0f);
+    if (STATS) s.n_term[3] += (unsigned)(s.hi2 - s.lo2);
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
+        float A, B;
+        unpack2(s.acc[q].ab, A, B);
+        s.A_max[q] = A;
+    }
+}
+
+// one t0 step the careful way: closure of cell (m, n) with closure_2F_exp where fp32 does not
+// do, then the sums move on to row m - 1 with loops over the entering and leaving atoms.
+// Returns true after the segment's first row.
+template <int TPC, bool STATS>
+__device__ __noinline__ bool slide_step_generic(SlideState<TPC> &s, const Problem &pr,
+                                                const SlideCtx &c)
+{
+    const Grid &g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    const int m = s.m, n = c.n;
+    const ulonglong2 *rec[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q)
+        rec[q] = c.packed + (int64_t)min(c.tpl0 + q, pr.n_templates - 1) * c.n_pad * 2;
+    const int64_t cells = (int64_t)g.N_t0 * g.N_tau;
+    const int32_t flat = m * g.N_tau + n;
+    const int cnt = s.hi - s.lo_m;
+
+    // ---- a4 + a5 of cell (m, n) of every template
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
         float A, B, far, fai, fbr, fbi;
-        unpack2(acc[q].ab, A, B);
-        unpack2(acc[q].fa, far, fai);
-        unpack2(acc[q].fb, fbr, fbi);
-        const float C = acc[q].c;
+        unpack2(s.acc[q].ab, A, B);
+        unpack2(s.acc[q].fa, far, fai);
+        unpack2(s.acc[q].fb, fbr, fbi);
+        const float C = s.acc[q].c;
+        // the fast path's arithmetic, so that a cell's value does not depend on its neighbours
         const float p = A * B;
         const float D = fmaf(-C, C, p);
         const float na = fmaf(far, far, fai * fai);
@@ -478,97 +487,195 @@ __device__ __forceinline__ void exp_slide_body(
         uint32_t fl = 0u;
         if (!(D > 0.015625f * p && p > 1.0e-30f && p < 1.0e30f && cnt >= pr.min_atoms &&
               fabsf(twoF) < 3.0e38f)) {
-            const int tq = min(tpl0 + q, pr.n_templates - 1);
-            twoF = closure_2F_exp<false>(A, B, C, far, fai, fbr, fbi, lo_m, cnt, pr.min_atoms, fl,
+            const int tq = min(c.tpl0 + q, pr.n_templates - 1);
+            twoF = closure_2F_exp<false>(A, B, C, far, fai, fbr, fbi, s.lo_m, cnt, pr.min_atoms, fl,
                                          pr.atoms + (int64_t)tq * pr.template_stride, pr.ld, bd.t,
                                          t0_of(g, m), (double)tau_of(g, n));
         }
-        if (n_ok && tpl0 + q < pr.n_templates) {
-            const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
+        if (c.n_ok && c.tpl0 + q < pr.n_templates) {
+            const int64_t o = (int64_t)(c.tpl0 + q) * cells + flat;
             if (pr.out_maps) pr.out_maps[o] = twoF;
             if (pr.out_flags) pr.out_flags[o] = (uint8_t)fl;
         }
         if (!fl) {
-            if (twoF >= mg_best[q]) {
-                mg_best[q] = twoF;
-                mg_m[q] = m;
+            if (twoF >= s.mg_best[q]) {
+                s.mg_best[q] = twoF;
+                s.mg_m[q] = m;
             }
-            if (fmaf(twoF, kHalfLog2eS, -mg_ref2[q]) > 60.0f) {  // rare: move the reference
-                mg_sum[q] *= ex2_approx(mg_ref2[q] - twoF * kHalfLog2eS);
-                mg_ref2[q] = twoF * kHalfLog2eS;
+            if (fmaf(twoF, kHalfLog2eS, -s.mg_ref2[q]) > 60.0f) {  // move the reference
+                s.mg_sum[q] *= ex2_approx(s.mg_ref2[q] - twoF * kHalfLog2eS);
+                s.mg_ref2[q] = twoF * kHalfLog2eS;
             }
-            mg_sum[q] += ex2_approx(fmaf(twoF, kHalfLog2eS, -mg_ref2[q]));
+            s.mg_sum[q] += ex2_approx(fmaf(twoF, kHalfLog2eS, -s.mg_ref2[q]));
         } else {
-            n_bad[q] += 1;
+            s.n_bad[q] += 1;
         }
-    };
+    }
+    if (m == c.m_beg) return true;
+
+    // ---- the sums move on to cell m - 1
+    int lo3 = s.lo2, hi3 = s.hi2;
+    if (m - 1 > c.m_beg) {
+        lo3 = __ldg(bd.lo + m - 2);
+        hi3 = max(hi_index(bd, g, m - 2, n), lo3);
+    }
+    const int lo2 = s.lo2, hi2 = s.hi2, lv = max(hi2, s.lo_m);
+    bool fresh = (hi2 <= s.lo_m) || (hi2 == lo2);  // no overlap with window m, or empty
+    if (!fresh) {
+        const int t0_2 = (int)t0_of(g, m - 1);
+        const float sh = (float)(s.t_ref - t0_2);
+        if (sh * c.kexp < kReanchorArg) {  // keep the weights of entering atoms <= e^kReanchor
+            const float sc = ex2_approx(sh * c.kexp);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                acc_scale(s.acc[q], sc);
+                s.A_max[q] *= sc * sc;
+            }
+            s.t_ref = t0_2;
+        }
+        for (int al = lo2; al < s.lo_m; ++al)  // entering, low end
+            slide_add_global<TPC>(s, bd, rec, c.kexp, al, 1.0f);
+        for (int al = lv; al < s.hi; ++al)  // leaving, high end
+            slide_add_global<TPC>(s, bd, rec, c.kexp, al, -1.0f);
+        if (STATS) {
+            s.n_term[1] += (unsigned)(s.lo_m - lo2);
+            s.n_term[2] += (unsigned)max(s.hi - lv, 0);
+        }
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            float A, B;
+            unpack2(s.acc[q].ab, A, B);
+            s.A_max[q] = fmaxf(s.A_max[q], A);
+            // a window that lost most of its weight is re-summed (for all TPC templates: a fresh
+            // sum is always right); written so that a NaN / inf atom in the running sums also
+            // forces a fresh sum: once it has left the window it must not linger
+            fresh = fresh || !(A * kGuard >= s.A_max[q]);
+        }
+    }
+    if (fresh) slide_resum<TPC, STATS>(s, pr, c);
+    s.m = m - 1;
+    s.lo_m = lo2;
+    s.hi = hi2;
+    s.lo2 = lo3;
+    s.hi2 = hi3;
+    return false;
+}
+
+template <int NT, int TPC, bool STATS>
+__device__ __forceinline__ void exp_slide_body(
+    const Problem &pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+    const float4 *W0, Partial *__restrict__ partials, const unsigned vblock, const int n_nblocks,
+    const int n_segs, const int seg_len, unsigned long long *__restrict__ stats)
+{
+    constexpr unsigned kFull = 0xffffffffu;
+    constexpr int NW = NT / 32;
+    __shared__ Marg s_red[32];
+    __shared__ __align__(16) ulonglong2 s_in[NW][TPC][64];  // a warp's next 32 entering atoms
+    __shared__ int s_tin[NW][32];                           // and their time stamps
+
+    const Grid &g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    const int lane = threadIdx.x & 31;
+    const int warp = (int)threadIdx.x >> 5;
+    // vblock = (tplgrp * n_segs + seg) * n_nblocks + j, heaviest tau block (largest tau) first
+    const int j = (int)(vblock % n_nblocks);
+    const int seg = (int)((vblock / n_nblocks) % n_segs);
+    const int tpl0 = (int)(vblock / ((int64_t)n_nblocks * n_segs)) * TPC;
+    const int n_first = (n_nblocks - 1 - j) * NT;
+    const int n_count = min(NT, g.N_tau - n_first);
+    const int m_beg = seg * seg_len;
+    const int m_end = min(m_beg + seg_len, g.N_t0);
+
+    // Templates beyond the batch (ragged last group) alias the last real one, tau slots beyond
+    // the grid alias the block's last tau: they run the same instructions as their neighbours
+    // (the fast path is taken warp by warp) and nothing of theirs is stored.
+    const ulonglong2 *__restrict__ rec[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q)
+        rec[q] = packed + (int64_t)min(tpl0 + q, pr.n_templates - 1) * n_pad * 2;
+    const bool n_ok = (int)threadIdx.x < n_count;
+    const int n = n_first + min((int)threadIdx.x, n_count - 1);
+    const float kexp = (float)(-1.4426950408889634 / (double)tau_of(g, n));
+    const int a_last = bd.n_atoms - 1;
+    // window end of cell (mm, n): one entry of the lattice table (bounds.cu), else a binary search
+    const bool has_edge = bd.edge != nullptr;
+    const int jn = n * bd.e_n;  // (the lattice has at most 2^22 points: 32-bit indices)
+    int in_base = 0x40000000;   // first atom of the warp's staged entering atoms (none yet)
+
+    // ---- the segment's last cell (m_end - 1, n): its window sums come from exp_window_kernel ----
+    SlideState<TPC> s;
+    s.m = m_end - 1;
+    s.lo_m = __ldg(bd.lo + s.m);
+    s.hi = max(hi_index(bd, g, s.m, n), s.lo_m);
+    s.t_ref = (int)t0_of(g, s.m);  // seconds (int32: every grid time fits, TFSTAT_EOVERFLOW otherwise)
+#pragma unroll
+    for (int q = 0; q < TPC; ++q) {
+        const int tq = min(tpl0 + q, pr.n_templates - 1);
+        const float4 *w = W0 + (((int64_t)tq * n_segs + seg) * g.N_tau + n) * 2;
+        const float4 w0 = w[0], w1 = w[1];
+        s.acc[q].ab = pack2(w0.x, w0.y);
+        s.acc[q].c = w0.z;
+        s.acc[q].fa = pack2(w0.w, w1.x);
+        s.acc[q].fb = pack2(w1.y, w1.z);
+        s.A_max[q] = w0.x;
+        s.mg_best[q] = -INFINITY;
+        s.mg_m[q] = 0;
+        s.mg_ref2[q] = -1.0e30f;
+        s.mg_sum[q] = 0.0f;
+        s.n_bad[q] = 0;
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) s.n_term[i] = 0u;
+    s.lo2 = s.lo_m;
+    s.hi2 = s.hi;
+    if (s.m > m_beg) {
+        s.lo2 = __ldg(bd.lo + s.m - 1);
+        s.hi2 = max(hi_index(bd, g, s.m - 1, n), s.lo2);
+    }
 
     // ---- slide backwards in t0: closure of cell m, then step to m - 1 ------------------------
-    // A t0 step is a chain of dependent loads (row start -> window end -> atom records) in front
-    // of the arithmetic, so the indices of the step m -> m - 1 are requested one step ahead and
-    // the records of its atoms BEFORE cell m is closed.
-    //
-    // FAST PATH, taken when every lane of the warp is in the common case -- at most one atom
-    // enters and one leaves, the windows of m and m - 1 overlap, t_ref stays: straight-line code.
-    // An atom that does not exist (n_in = 0, n_out = 0) is loaded from a clamped address and
-    // gets the weight 0 by a select.  Cells are closed in fp32 and the lanes VOTE on whether any
-    // of them needs the careful closure; the marginals are updated without branches.  Everything
-    // else (several atoms per step, disjoint windows, re-anchoring, the segment's first row)
-    // takes the generic path below.  ncu on config 4 before this split: 304 warp instructions
-    // per step, of which 50 BRA/BSSY/BSYNC, 47 integer compares and 21 spill loads/stores.
-    int lo2 = lo_m, hi2 = hi;
-    if (m > m_beg) {
-        lo2 = __ldg(bd.lo + m - 1);
-        hi2 = max(hi_at(m - 1), lo2);
-    }
     // (a warp whose tau slots all lie beyond the grid has nothing to do but the final reduction)
 #pragma unroll 1
     for (; warp * 32 < n_count;) {
-        const bool last = m == m_beg;
-        const int n_in = lo_m - lo2, lv = max(hi2, lo_m), n_out = hi - lv;
-        const bool fresh0 = (hi2 <= lo_m) || (hi2 == lo2);  // no overlap with window m, or empty
-        const int t0_2 = (int)t0_of(g, m - 1);
-        const float sh = (float)(t_ref - t0_2);
-        const bool calm =
-            has_edge && !fresh0 && n_in <= 1 && n_out <= 1 && !(sh * kexp < kReanchorArg);
-        const int cnt = hi - lo_m;
-        int lo3 = lo2, hi3 = hi2;
-        bool fresh;
-        if (!last && __all_sync(kFull, calm)) {
-            // -- the entering atom is the same for all lanes: the warp stages 32 of them at a time
-            // in shared memory (coalesced, once per 32 steps) and reads them back by broadcast
-            const int a_in = min(lo2, a_last), a_out = min(lv, a_last);
-            if ((unsigned)(a_in - in_base) >= 32u) {  // warp-uniform
+        const int m = s.m;
+        const int n_in = s.lo_m - s.lo2, lv = max(s.hi2, s.lo_m), n_out = s.hi - lv;
+        const bool fresh0 = (s.hi2 <= s.lo_m) || (s.hi2 == s.lo2);
+        const float sh = (float)(s.t_ref - (int)t0_of(g, m - 1));
+        const bool calm = has_edge && m != m_beg && !fresh0 && n_in <= 1 && n_out <= 1 &&
+                          !(sh * kexp < kReanchorArg) && s.hi - s.lo_m >= pr.min_atoms;
+        bool done = false;  // this step was taken by the fast path
+        if (__all_sync(kFull, calm)) {
+            const int a_in = min(s.lo2, a_last), a_out = min(lv, a_last);
+            if ((unsigned)(a_in - in_base) >= 32u) {  // warp-uniform: stage the next 32 entering atoms
                 in_base = max(a_in - 31, 0);
                 const int al = min(in_base + lane, a_last);
                 __syncwarp();
                 s_tin[warp][lane] = __ldg(bd.t + al);
 #pragma unroll
-                for (int q = 0; q < TPC; ++q) {
-                    s_in[warp][q][2 * lane] = __ldg(rec[q] + 2 * al);
-                    s_in[warp][q][2 * lane + 1] = __ldg(rec[q] + 2 * al + 1);
-                }
+                for (int q = 0; q < TPC; ++q)
+                    ldg_record(rec[q] + 2 * al, s_in[warp][q][2 * lane], s_in[warp][q][2 * lane + 1]);
                 __syncwarp();
             }
-            // -- records of the leaving atom (one gather per lane), indices of the next step
+            // -- record of the leaving atom, indices of the next step
             const int t_out = __ldg(bd.t + a_out);
             ulonglong2 oa[TPC], ob[TPC];
 #pragma unroll
             for (int q = 0; q < TPC; ++q) ldg_record(rec[q] + 2 * a_out, oa[q], ob[q]);
+            int lo3 = s.lo2, hi3 = s.hi2;
             if (m - 1 > m_beg) {
                 lo3 = __ldg(bd.lo + m - 2);
                 hi3 = max(__ldg(bd.edge + (jn + (m - 2) * bd.e_m)), lo3);
             }
             // -- a4: eq. (7) in fp32 for the TPC templates, one vote on "all well conditioned"
             float twoF[TPC];
-            bool bad = cnt < pr.min_atoms;
+            bool bad = false;
 #pragma unroll
             for (int q = 0; q < TPC; ++q) {
                 float A, B, far, fai, fbr, fbi;
-                unpack2(acc[q].ab, A, B);
-                unpack2(acc[q].fa, far, fai);
-                unpack2(acc[q].fb, fbr, fbi);
-                const float C = acc[q].c;
+                unpack2(s.acc[q].ab, A, B);
+                unpack2(s.acc[q].fa, far, fai);
+                unpack2(s.acc[q].fb, fbr, fbi);
+                const float C = s.acc[q].c;
                 const float p = A * B;
                 const float D = fmaf(-C, C, p);
                 const float na = fmaf(far, far, fai * fai);
@@ -583,17 +690,14 @@ __device__ __forceinline__ void exp_slide_body(
                                 (fabsf(twoF[q]) < 3.0e38f);
                 bad = bad | !ok;
             }
-            if (__any_sync(kFull, bad)) {
-#pragma unroll
-                for (int q = 0; q < TPC; ++q) close_full(q, cnt);
-            } else {
+            if (!__any_sync(kFull, bad)) {
+                done = true;
                 // -- a5, branch-free
                 if (pr.out_maps) {  // (uniform; a search stores no maps)
-                    const int32_t flat = m * g.N_tau + n;
 #pragma unroll
                     for (int q = 0; q < TPC; ++q)
                         if (n_ok && tpl0 + q < pr.n_templates) {
-                            const int64_t o = (int64_t)(tpl0 + q) * cells + flat;
+                            const int64_t o = ((int64_t)(tpl0 + q) * g.N_t0 + m) * g.N_tau + n;
                             pr.out_maps[o] = twoF[q];
                             if (pr.out_flags) pr.out_flags[o] = (uint8_t)0;
                         }
@@ -602,109 +706,75 @@ __device__ __forceinline__ void exp_slide_body(
                 bool move = false;
 #pragma unroll
                 for (int q = 0; q < TPC; ++q) {
-                    const bool better = twoF[q] >= mg_best[q];
-                    mg_best[q] = better ? twoF[q] : mg_best[q];
-                    mg_m[q] = better ? m : mg_m[q];
-                    x[q] = fmaf(twoF[q], kHalfLog2eS, -mg_ref2[q]);
+                    const bool better = twoF[q] >= s.mg_best[q];
+                    s.mg_best[q] = better ? twoF[q] : s.mg_best[q];
+                    s.mg_m[q] = better ? m : s.mg_m[q];
+                    x[q] = fmaf(twoF[q], kHalfLog2eS, -s.mg_ref2[q]);
                     move = move | (x[q] > 60.0f);
                 }
                 if (__any_sync(kFull, move)) {  // rare: move the reference of the log-sum-exp
 #pragma unroll
                     for (int q = 0; q < TPC; ++q)
                         if (x[q] > 60.0f) {
-                            mg_sum[q] *= ex2_approx(-x[q]);
-                            mg_ref2[q] = twoF[q] * kHalfLog2eS;
+                            s.mg_sum[q] *= ex2_approx(-x[q]);
+                            s.mg_ref2[q] = twoF[q] * kHalfLog2eS;
                             x[q] = 0.0f;
                         }
                 }
 #pragma unroll
-                for (int q = 0; q < TPC; ++q) {
-                    mg_sum[q] += ex2_approx(x[q]);
-                }
-            }
-            // -- the sums move on to cell m - 1
-            const int t_in = s_tin[warp][a_in - in_base];
-            const float e_in = ex2_approx((float)(t_in - t_ref) * kexp);
-            const float e_out = ex2_approx((float)(t_out - t_ref) * kexp);
-            fresh = false;
-#pragma unroll
-            for (int q = 0; q < TPC; ++q) {
-                const ulonglong2 ia = s_in[warp][q][2 * (a_in - in_base)];
-                const ulonglong2 ib = s_in[warp][q][2 * (a_in - in_base) + 1];
-                float dtc, ab;
-                unpack2(ia.x, dtc, ab);
-                // (fmaf(dtc, 0, e): NaN for an atom that is not finite, pack.cu; the select keeps
-                // an atom that is not part of this step out even then)
-                const float wi = n_in ? fmaf(dtc, 0.0f, e_in) : 0.0f;
-                acc_add(acc[q], wi, wi * wi, ia, ib);
-                unpack2(oa[q].x, dtc, ab);
-                const float wo = n_out ? -fmaf(dtc, 0.0f, e_out) : 0.0f;
-                acc_add(acc[q], wo, wo * fabsf(wo), oa[q], ob[q]);
-                float A, B;
-                unpack2(acc[q].ab, A, B);
-                A_max[q] = fmaxf(A_max[q], A);
-                fresh = fresh | !(A * kGuard >= A_max[q]);  // (see the generic path)
-            }
-            if (STATS) {
-                n_term[1] += (unsigned)n_in;
-                n_term[2] += (unsigned)n_out;
-            }
-        } else {
-            // -- generic path: the same steps with loops and branches
-#pragma unroll
-            for (int q = 0; q < TPC; ++q) close_full(q, cnt);
-            if (last) break;
-            if (m - 1 > m_beg) {
-                lo3 = __ldg(bd.lo + m - 2);
-                hi3 = max(hi_at(m - 2), lo3);
-            }
-            fresh = fresh0;
-            if (!fresh) {
-                if (sh * kexp < kReanchorArg) {  // keep the weights of entering atoms <= e^kReanchor
-                    const float c = ex2_approx(sh * kexp);
-#pragma unroll
-                    for (int q = 0; q < TPC; ++q) {
-                        acc_scale(acc[q], c);
-                        A_max[q] *= c * c;
-                    }
-                    t_ref = t0_2;
-                }
-                for (int al = lo2; al < lo_m; ++al) add_global(al, 1.0f);  // entering, low end
-                for (int al = lv; al < hi; ++al) add_global(al, -1.0f);    // leaving, high end
-                if (STATS) {
-                    n_term[1] += (unsigned)n_in;
-                    n_term[2] += (unsigned)max(n_out, 0);
-                }
+                for (int q = 0; q < TPC; ++q) s.mg_sum[q] += ex2_approx(x[q]);
+
+                // -- the sums move on to cell m - 1
+                const int t_in = s_tin[warp][a_in - in_base];
+                const float e_in = ex2_approx((float)(t_in - s.t_ref) * kexp);
+                const float e_out = ex2_approx((float)(t_out - s.t_ref) * kexp);
+                bool fresh = false;
 #pragma unroll
                 for (int q = 0; q < TPC; ++q) {
+                    const ulonglong2 ia = s_in[warp][q][2 * (a_in - in_base)];
+                    const ulonglong2 ib = s_in[warp][q][2 * (a_in - in_base) + 1];
+                    float dtc, ab;
+                    unpack2(ia.x, dtc, ab);
+                    // (fmaf(dtc, 0, e): NaN for an atom that is not finite, pack.cu; the select
+                    // keeps an atom that is not part of this step out even then)
+                    const float wi = n_in ? fmaf(dtc, 0.0f, e_in) : 0.0f;
+                    acc_add(s.acc[q], wi, wi * wi, ia, ib);
+                    unpack2(oa[q].x, dtc, ab);
+                    const float wo = n_out ? -fmaf(dtc, 0.0f, e_out) : 0.0f;
+                    acc_add(s.acc[q], wo, wo * fabsf(wo), oa[q], ob[q]);
                     float A, B;
-                    unpack2(acc[q].ab, A, B);
-                    A_max[q] = fmaxf(A_max[q], A);
-                    // a window that lost most of its weight is re-summed (for all TPC templates: a
-                    // fresh sum is always right); written so that a NaN / inf atom in the running sums
-                    // also forces a fresh sum: once it has left the window it must not linger
-                    fresh = fresh || !(A * kGuard >= A_max[q]);
+                    unpack2(s.acc[q].ab, A, B);
+                    s.A_max[q] = fmaxf(s.A_max[q], A);
+                    fresh = fresh | !(A * kGuard >= s.A_max[q]);  // (see slide_step_generic)
                 }
+                if (STATS) {
+                    s.n_term[1] += (unsigned)n_in;
+                    s.n_term[2] += (unsigned)n_out;
+                }
+                if (__any_sync(kFull, fresh)) {  // rare: some lane's window lost its weight
+                    if (fresh) {
+                        const SlideCtx c = {packed, n_pad, tpl0, n, n_ok ? 1 : 0, m_beg, kexp};
+                        SlideState<TPC> tmp;
+                        slide_copy<TPC>(tmp, s);
+                        slide_resum<TPC, STATS>(tmp, pr, c);
+                        slide_copy<TPC>(s, tmp);
+                    }
+                }
+                s.m = m - 1;
+                s.lo_m = s.lo2;
+                s.hi = s.hi2;
+                s.lo2 = lo3;
+                s.hi2 = hi3;
             }
         }
-        if (fresh) {
-#pragma unroll
-            for (int q = 0; q < TPC; ++q) acc_zero(acc[q]);
-            t_ref = t0_2;
-            for (int al = lo2; al < hi2; ++al) add_global(al, 1.0f);
-            if (STATS) n_term[3] += (unsigned)(hi2 - lo2);
-#pragma unroll
-            for (int q = 0; q < TPC; ++q) {
-                float A, B;
-                unpack2(acc[q].ab, A, B);
-                A_max[q] = A;
-            }
+        if (!done) {
+            const SlideCtx c = {packed, n_pad, tpl0, n, n_ok ? 1 : 0, m_beg, kexp};
+            SlideState<TPC> tmp;
+            slide_copy<TPC>(tmp, s);
+            const bool last = slide_step_generic<TPC, STATS>(tmp, pr, c);
+            slide_copy<TPC>(s, tmp);
+            if (last) break;
         }
-        m -= 1;
-        lo_m = lo2;
-        hi = hi2;
-        lo2 = lo3;
-        hi2 = hi3;
     }
     const int n_visited = warp * 32 < n_count ? m_end - m_beg : 0;
     if (STATS) {
@@ -712,8 +782,8 @@ __device__ __forceinline__ void exp_slide_body(
         unsigned long long v[5];
         const unsigned long long ntpl = n_ok ? (unsigned long long)min(TPC, pr.n_templates - tpl0) : 0ull;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) v[i] = (unsigned long long)n_term[i] * ntpl;
-        v[4] = (unsigned long long)(m_end - m_beg) * ntpl;
+        for (int i = 0; i < 4; ++i) v[i] = (unsigned long long)s.n_term[i] * ntpl;
+        v[4] = (unsigned long long)n_visited * ntpl;
 #pragma unroll
         for (int i = 1; i < 5; ++i) {
 #pragma unroll
@@ -726,12 +796,12 @@ __device__ __forceinline__ void exp_slide_body(
         for (int q = 0; q < TPC; ++q) {
             Marg a;
             marg_init(a);
-            const int nv = n_visited - n_bad[q];
+            const int nv = n_visited - s.n_bad[q];
             if (n_ok && nv > 0) {
-                a.best = mg_best[q];
-                a.idx = mg_m[q] * g.N_tau + n;
-                a.M = 0.5f * mg_best[q];
-                a.S = mg_sum[q] * ex2_approx(mg_ref2[q] - mg_best[q] * kHalfLog2eS);
+                a.best = s.mg_best[q];
+                a.idx = s.mg_m[q] * g.N_tau + n;
+                a.M = 0.5f * s.mg_best[q];
+                a.S = s.mg_sum[q] * ex2_approx(s.mg_ref2[q] - s.mg_best[q] * kHalfLog2eS);
                 a.nvalid = nv;
             }
             __syncthreads();  // s_red is reused (by the next template, the next pass)
@@ -757,7 +827,8 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
 
 template <int NT, int TPC, bool STATS>
 __global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : SLIDE_CTAS) : 1)
-    exp_slide_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
+    exp_slide_kernel(const __grid_constant__ Problem pr, const ulonglong2 *__restrict__ packed,
+                     const int n_pad,
                      const float4 *__restrict__ W0, Partial *__restrict__ partials,
                      const int n_nblocks, const int n_segs, const int seg_len,
                      unsigned long long *__restrict__ stats)
