@@ -37,12 +37,8 @@ namespace {
 constexpr float kReanchor = 4.0f;  // move t_ref when (t_ref - t0_m)/tau exceeds this
 constexpr float kReanchorArg = -kReanchor * 1.4426950408889634f;  // the same on (t_ref - t0_m) kexp
 constexpr float kGuard = 64.0f;    // re-sum a window whose A fell below 1/kGuard of its maximum
-#ifndef SLIDE_CTAS
-#define SLIDE_CTAS 4
-#endif
 constexpr int kSlideChunk = 128;   // atoms per bulk copy and template (4 KB); divides kPackBlock
 constexpr int kSlideStages = 3;    // ring slots per CTA
-constexpr int kWindowUnroll = 8;   // unroll of the initial-window loop
 static_assert(kPackBlock % kSlideChunk == 0, "a staged chunk must lie inside one packed time block");
 
 struct SlideAcc {
@@ -113,6 +109,21 @@ __device__ __forceinline__ void ldg_record(const ulonglong2 *p, ulonglong2 &ra, 
     asm("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];"
         : "=l"(ra.x), "=l"(ra.y), "=l"(rb.x), "=l"(rb.y)
         : "l"(p));
+}
+// the same, and a 32-bit load, pinned where they are written (volatile): the slide kernel requests
+// the data of the NEXT step before it closes a cell, and the compiler must not sink the loads
+// into the branch that uses them
+__device__ __forceinline__ void ldg_record_now(const ulonglong2 *p, ulonglong2 &ra, ulonglong2 &rb)
+{
+    asm volatile("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];"
+                 : "=l"(ra.x), "=l"(ra.y), "=l"(rb.x), "=l"(rb.y)
+                 : "l"(p));
+}
+__device__ __forceinline__ int ldg_int_now(const int32_t *p)
+{
+    int v;
+    asm volatile("ld.global.nc.b32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -238,6 +249,8 @@ __device__ __forceinline__ void exp_window_body(
         asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(s_fa[r][q]) : "l"(pack2(f[r], f[r])), "l"(rb.x));
         asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(s_fb[r][q]) : "l"(pack2(f[r], f[r])), "l"(rb.y));
         s_c[r][q] = fmaf(s_c[r][q], f2[r], ab);
+        // (measured: Fb, or Fa and Fb, as scalar FFMA pairs instead of FFMA2 -- fewer FMA-pipe
+        // cycles, more issue slots -- is 9 % and 13 % slower)
     };
     // a bad SFT (packed as dtc = NaN on zero channels) spoils the sums of its template
     auto poison = [&](const int q, const ulonglong2 ra) {
@@ -657,10 +670,10 @@ __device__ __forceinline__ void exp_slide_body(
                 __syncwarp();
             }
             // -- record of the leaving atom, indices of the next step
-            const int t_out = __ldg(bd.t + a_out);
+            const int t_out = ldg_int_now(bd.t + a_out);
             ulonglong2 oa[TPC], ob[TPC];
 #pragma unroll
-            for (int q = 0; q < TPC; ++q) ldg_record(rec[q] + 2 * a_out, oa[q], ob[q]);
+            for (int q = 0; q < TPC; ++q) ldg_record_now(rec[q] + 2 * a_out, oa[q], ob[q]);
             int lo3 = s.lo2, hi3 = s.hi2;
             if (m - 1 > m_beg) {
                 lo3 = __ldg(bd.lo + m - 2);
@@ -826,7 +839,7 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
 }
 
 template <int NT, int TPC, bool STATS>
-__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : SLIDE_CTAS) : 1)
+__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : 4) : 1)
     exp_slide_kernel(const __grid_constant__ Problem pr, const ulonglong2 *__restrict__ packed,
                      const int n_pad,
                      const float4 *__restrict__ W0, Partial *__restrict__ partials,
