@@ -96,10 +96,14 @@ typedef struct tfstat_opts {
     int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
                            per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
                            (1,2,4) + 10 x (10 RT + TPC of the window-sum kernel, e.g. 422); tfstat_map_general: tau cells per thread (1,2,4); lattice
-                           rect kernel: rows per thread (1, 2, 4)                             */
+                           rect kernels: rows per thread of the running-sum kernel (1, 2), or 8 =
+                           the tile kernel on any grid whose lattice qualifies (auto only takes
+                           it when the map has enough tiles to fill the GPU)                  */
     int32_t tile_nt;    /* tuning: threads (= tau values) per CTA (32,64,128,256); 0 = auto */
     int32_t seg_len;    /* tuning, 0 = auto.  Sliding exp kernel: t0 steps per segment; lattice
-                           rect kernel: columns per CTA (rounded up to 16); direct exp kernel:
+                           rect kernels: columns per CTA of the running-sum kernel (rounded up
+                           to 16), < 0 = the running-sum kernel even where the tile kernel
+                           (direct form) would be chosen; direct exp kernel:
                            1 = the warps of a CTA split the windows' atoms, 2 = they never do */
     int32_t reserved0;  /* must be 0 */
     /* Optional profiling hooks: cudaEvent_t handles (as void*), recorded on `stream`
@@ -131,6 +135,7 @@ typedef struct tfstat_opts {
 #define TFSTAT_KERNEL_RECT_SMALL 3
 #define TFSTAT_KERNEL_RECT_RUN 4   /* lattice running-sum kernel                              */
 #define TFSTAT_KERNEL_RECT_CELLS 5 /* per-cell prefix differences (no lattice / few rows)     */
+#define TFSTAT_KERNEL_RECT_TILE 6  /* lattice direct form, tile by tile (small lattice steps)     */
 typedef struct tfstat_plan {
     uint32_t struct_size; /* in: sizeof(tfstat_plan) of the caller                           */
     int32_t kernel;       /* TFSTAT_KERNEL_* of the dominant kernel                          */

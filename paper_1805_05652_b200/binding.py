@@ -23,7 +23,8 @@ _lib = None
 _probe_lib = None
 N_STATS = 8  # TFSTAT_N_STATS
 STAT_NAMES = ("terms_window", "terms_enter", "terms_leave", "terms_resum", "cells", "redo64")
-KERNEL_NAMES = {1: "exp_direct", 2: "exp_slide", 3: "rect_small", 4: "rect_run", 5: "rect_cells"}
+KERNEL_NAMES = {1: "exp_direct", 2: "exp_slide", 3: "rect_small", 4: "rect_run", 5: "rect_cells",
+                6: "rect_tile"}
 
 # tfstat_result, 20 bytes (include/tfstat.h)
 RESULT_DTYPE = np.dtype([("max2F", "<f4"), ("m", "<i4"), ("n", "<i4"), ("logB", "<f4"),

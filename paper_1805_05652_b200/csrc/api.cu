@@ -392,7 +392,7 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.n_ctas = n_templates;
         p.n_launches = 1;
     } else if (pl.rect.enabled) {
-        p.kernel = TFSTAT_KERNEL_RECT_RUN;
+        p.kernel = pl.rect.tile ? TFSTAT_KERNEL_RECT_TILE : TFSTAT_KERNEL_RECT_RUN;
         p.tile_c = pl.rect.Q;
         p.tile_nt = rect_run_threads(pl);
         p.seg_len = pl.rect.seg_cols;

@@ -852,11 +852,11 @@ __global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : 4) : 1)
                                    seg_len, stats);
 }
 
-// Also measured (B200, config 4 x 2048 templates): both phases in ONE kernel (a CTA sums the
-// windows of its 512 tau values, then slides them in four passes), hoping that CTAs in different
-// phases overlap the FP32-bound window sums with the latency-bound sliding: 4.53 ms against
-// 4.10 ms for the two kernels back to back (128 registers with spills, 16 warps per SM for both
-// phases).
+// Also measured (B200, config 4 x 2048 templates, with the slide loop of that time): both phases
+// in ONE kernel (a CTA sums the windows of its 512 tau values, then slides them in four passes),
+// hoping that CTAs in different phases overlap the FP32-bound window sums with the latency-bound
+// sliding: 4.53 ms against 4.10 ms for the two kernels back to back (128 registers with spills,
+// 16 warps per SM for both phases).  The two kernels take 2.06 + 1.15 ms now.
 
 template <int NT, int TPC>
 cudaError_t launch_tpc(const Plan &pl, const Problem &pr, const ulonglong2 *packed,

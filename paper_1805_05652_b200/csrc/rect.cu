@@ -1419,8 +1419,9 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
     rr.tile = 0;
     // direct form, tile by tile (rect_tile_kernel): lattice steps small enough for a tile's run of
     // lattice points to sit in shared memory; seg_override < 0 keeps the running-sum kernel
+    // (q_override == 8 forces it on any grid whose lattice qualifies: the tests' small maps)
     if (rr.enabled && e_m >= 1 && e_n >= 1 && e_m <= 4 && e_n <= 4 && seg_override >= 0 &&
-        q_override == 0 && (kTileQuads % e_n) == 0 &&
+        (q_override == 0 || q_override == 8) && (kTileQuads % e_n) == 0 &&
         (int64_t)(kTileCells * kTileQuads - (kTileCells - 1) * e_n - 1) * e_m +
                 (int64_t)(kTileCols - 1) * e_n + 1 <=
             kTileMaxRun) {
@@ -1428,7 +1429,7 @@ RectRun plan_rect_run(const Grid &g, int32_t e_m, int32_t e_n, int64_t J, int32_
         const int64_t n_ct = (g.N_tau + (kTileCells - 1) * e_m + kTileCols - 1) / kTileCols;
         // (a small map gives too few 128 x 256 tiles to fill 148 SMs: config 3's 96 x 5736 cells
         // are 23 tiles, 58 us against 44 us for the running-sum kernel)
-        if (n_rt * n_ct * n_templates >= 2 * 148) rr.tile = 1;
+        if (n_rt * n_ct * n_templates >= 2 * 148 || q_override == 8) rr.tile = 1;
     }
     if (rr.tile) {
         rr.Q = kTileCells;

@@ -220,7 +220,12 @@ def test_random_grids_all_kernel_families(pkg, case):
     for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN},
                                  {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 3)}]),
                         (RECT, [{"rect_method": 1}, {"rect_method": 2},
-                                  {"rect_method": 1, "tile": (2, 0, 0)}])):  # two rows per thread
+                                  {"rect_method": 1, "tile": (2, 0, 0)},  # two rows per thread
+                                  # seg_len < 0: the running-sum kernel where the tile kernel
+                                  # would take over
+                                  {"rect_method": 1, "tile": (0, 0, -1)},
+                                  # the tile kernel (direct form) wherever the lattice qualifies
+                                  {"rect_method": 1, "tile": (8, 0, 0)}])):
         ref = oracle.map2F(atoms, t, window, grid, min_atoms=min_atoms)
         for kw in kws:
             what = f"case {case} window {window} {kw}"
@@ -652,8 +657,9 @@ def test_config5_year_sampled(pkg, window):
 def test_one_year_full_resolution_rect_map_sampled(pkg, n_tau):
     """The largest of the paper's setups (one year at dt0 = dtau = T_SFT,
     3.07e8 cells, 1.23 GB), in the launch configuration bench.py's rect_map_1yr_full_resolution
-    leg times: one row per thread, K run in shared memory, 192-column tiles.  N_tau = 17519 leaves
-    the rows unaligned (coalesced scalar write-out), 17516 takes the vector write-out."""
+    leg times: rect_tile_kernel, 128 x 256-cell tiles.  N_tau = 17519 leaves the rows unaligned to
+    16 bytes, 17516 aligns them (the running-sum kernel of round 1 cared; the tile kernel stores
+    128-byte warp rows either way)."""
     from synth.atoms import Grid, make_atoms
     rng = np.random.default_rng(2026)
     t = np.arange(17520, dtype=np.int64) * 1800
@@ -687,6 +693,51 @@ def test_one_year_full_resolution_rect_map_sampled(pkg, n_tau):
     at = oracle.cells(atoms, t, RECT, grid, np.array([r0["m"]], np.int32),
                       np.array([r0["n"]], np.int32))
     assert at["flags"][0] == 0 and abs(at["twoF"][0] - best) <= TOL_2F * max(1.0, at["twoF"][0])
+
+
+TILE_GRIDS = [
+    # slots, gaps, grid                                   lattice (e_m, e_n), what it exercises
+    (700, 0.0, Grid(0, 1800, 300, 1800, 1800, 600)),       # (1, 1): 3 x 3 tiles, ragged both ways
+    (700, 0.3, Grid(-3600, 1800, 200, 1, 1800, 300)),      # (1, 1): gaps, tau from one second, t0 before the data
+    (900, 0.1, Grid(0, 900, 260, 3600, 1800, 280)),        # (1, 2): pairs two rows down, one column back
+    (900, 0.1, Grid(0, 3600, 140, 1800, 900, 520)),        # (4, 1)
+    (600, 0.2, Grid(300 * 1800, 1800, 150, 5400, 900, 300)),  # (2, 1): windows overrun the data
+    (400, 0.0, Grid(0, 1800, 9, 3600, 3600, 40)),          # (1, 2): fewer rows than one pair group
+]
+
+
+@pytest.mark.parametrize("slots,gaps,grid", TILE_GRIDS)
+def test_rect_tile_kernel_small_grids(pkg, slots, gaps, grid):
+    """rect_tile_kernel (the direct, anchored form the one-year map runs through) forced on small
+    grids (tile_c = 8; the plan itself only takes it when the map fills the GPU): every cell and
+    flag of every template against the oracle, map + flags, map only and results only, with
+    min_atoms 1..3 and a bad SFT."""
+    T = 3
+    wl = tiny_workload(7000 + slots + grid.N_t0, slots, gaps, grid, n_templates=T, phi_random=True)
+    atoms, t = wl.data.atoms.copy(), wl.data.t
+    atoms[1, :, len(t) // 3] = np.nan  # template 1: one bad SFT (every channel, DESIGN.md R19)
+    kw = {"rect_method": 1, "tile": (8, 0, 0)}
+    assert pkg.plan_info(RECT, len(t), T, grid, **kw)["kernel_name"] == "rect_tile"
+    assert pkg.plan_info(RECT, len(t), T, grid, rect_method=1)["kernel_name"] != "rect_tile"
+    for min_atoms in (2, 1, 3):
+        full = pkg.tfstat_search(dev(atoms), dev(t), RECT, grid, want_maps=True, want_flags=True,
+                                 min_atoms=min_atoms, **kw)
+        maps_only = pkg.tfstat_search(dev(atoms), dev(t), RECT, grid, want_maps=True,
+                                      min_atoms=min_atoms, **kw)
+        res_only = pkg.tfstat_search(dev(atoms), dev(t), RECT, grid, min_atoms=min_atoms, **kw)
+        torch.cuda.synchronize()
+        assert torch.equal(full.maps, maps_only.maps)
+        assert np.array_equal(full.numpy(), maps_only.numpy())
+        assert np.array_equal(full.numpy(), res_only.numpy())
+        for k in range(T):
+            with np.errstate(invalid="ignore"):
+                ref = oracle.map2F(atoms[k], t, RECT, grid, min_atoms=min_atoms)
+            what = f"rect tile {grid} min_atoms {min_atoms} tpl{k}"
+            check_cells(full.maps[k].cpu().numpy(), full.flags[k].cpu().numpy(), ref, what)
+            check_result(full.numpy()[k], ref["twoF"], ref["flags"], grid.N_tau, what)
+    # the same bits through tfstat_map (one template, no batch)
+    m, f = run_map(pkg, atoms[0], t, RECT, grid, min_atoms=3, **kw)
+    assert np.array_equal(m, full.maps[0].cpu().numpy()) and np.array_equal(f, full.flags[0].cpu().numpy())
 
 
 # ---------------------------------------------------------------------------------------
