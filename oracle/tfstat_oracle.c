@@ -27,7 +27,11 @@
  *   degenerate cells   fewer than `min_atoms` atoms (default 2: "at least 2 SFTs per
  *                      F_mn") -> flag bit 0;  !(D > 0) -> flag bit 1.
  *                      Degenerate cells store 2F = 0 and are excluded from the
- *                      marginals.
+ *                      marginals.  Atoms that are not finite are NOT special here:
+ *                      the arithmetic is followed (a NaN in a2 / b2 / ab makes D NaN
+ *                      -> bit 1; a NaN confined to Fa / Fb gives a NaN 2F with flag
+ *                      0).  The paper is silent on bad SFTs: PARITY UNPINNED BY THE
+ *                      PAPER; the GPU's convention is DESIGN.md reading R19.
  *   map layout         map[m*N_tau + n], m <-> t0, n <-> tau (eq. 8).
  *   marginals          max 2F over valid cells, lowest flat index on exact ties;
  *                      logB = log sum_valid exp(F), F = 2F/2 (eq. 5, PAPER.md:56;
