@@ -95,7 +95,8 @@ typedef struct tfstat_opts {
                            whenever the atoms fit its shared memory (n_atoms <= 2048)          */
     int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
                            per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
-                           (1,2,4) + 10 x (10 RT + TPC of the window-sum kernel, e.g. 422); tfstat_map_general: tau cells per thread (1,2,4); lattice
+                           (1,2) + 10 x (10 RT + TPC of the per-tau window-sum kernel, e.g. 422) + 1000 to
+                           keep EVERY window sum with that kernel (no grouped moments); tfstat_map_general: tau cells per thread (1,2,4); lattice
                            rect kernels: rows per thread of the running-sum kernel (1, 2), or 8 =
                            the tile kernel on any grid whose lattice qualifies (auto only takes
                            it when the map has enough tiles to fill the GPU)                  */
@@ -126,6 +127,8 @@ typedef struct tfstat_opts {
 #define TFSTAT_STAT_TERMS_RESUM 3  /* sliding form: windows summed afresh (guard, no overlap) */
 #define TFSTAT_STAT_CELLS 4        /* cells closed (eq. 7 evaluated)                          */
 #define TFSTAT_STAT_REDO64 5       /* cells re-summed in fp64 (short ill-conditioned windows) */
+#define TFSTAT_STAT_MOMENT 6       /* sliding form: (atom, moment, template) terms of the grouped
+                                      window sums, 7 multiply-adds each                        */
 #define TFSTAT_N_STATS 8
 
 /* What the library will run for a problem shape (host-only; tfstat_plan_info()).  bench.py reads

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/tfstat.h: argument validation, the problem plan (workspace
 // layout, tile shapes) and the launch sequences.  No arithmetic of the method lives here.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <vector>
@@ -185,8 +186,27 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         if (n_templates >= 2 && win_ctas(128, 4, 2) >= fill) pl.win_rt = 4, pl.win_tpc = 2;
         else if (win_ctas(128, 4, 1) >= fill) pl.win_rt = 4;
         else if (win_ctas(128, 2, 1) >= fill) pl.win_rt = 2;
-        if (opts && opts->tile_c) {  // TPC of the slide kernel + 10 x (RT TPC code of the window kernel)
-            const int c = opts->tile_c, w = c / 10, sl = c % 10;
+        // grouped window sums (exp_moment_kernel): a group of R neighbouring tau shares 8 moments
+        // while z = (window length) x (half width of the group in 1/tau) <= 1.5 (R - 1) dtau / tau
+        // stays below kMomZCap = 0.17 (exp_scan.cu); R = 64 above that tau, R = 32 above half of
+        // it, the per-tau recurrence below.  Regions shorter than one group are not worth a launch.
+        bool moments = n_templates >= 2;
+        int tile_code = opts ? opts->tile_c : 0;
+        if (tile_code >= 1000) moments = false, tile_code -= 1000;  // 1000 + ...: never
+        pl.mom_n32 = pl.mom_n64 = N_tau;
+        if (moments) {
+            auto first_n = [&](int R) {  // first tau index with tau >= 1.5 (R - 1) dtau / 0.17
+                const double tau_R = 1.5 * (R - 1) * (double)pl.grid.dtau / 0.17;
+                const double x = std::ceil((tau_R - (double)pl.grid.tau_min) / (double)pl.grid.dtau);
+                return (int32_t)std::min<double>(std::max(x, 0.0), (double)N_tau);
+            };
+            pl.mom_n64 = first_n(64);
+            pl.mom_n32 = first_n(32);
+            if (N_tau - pl.mom_n64 < 64) pl.mom_n64 = N_tau;
+            if (pl.mom_n64 - pl.mom_n32 < 32) pl.mom_n32 = pl.mom_n64;
+        }
+        if (tile_code) {  // TPC of the slide kernel + 10 x (RT TPC code of the window kernel)
+            const int c = tile_code, w = c / 10, sl = c % 10;
             if (sl != 1 && sl != 2) return pl;
             if (w != 0 && w != 11 && w != 12 && w != 21 && w != 22 && w != 41 && w != 42) return pl;
             pl.slide_tpc = sl;
@@ -384,7 +404,9 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.seg_len = pl.seg_len;
         p.n_segs = pl.n_segs;
         p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
-        p.n_launches = 5;  // bounds, pack, window sums, slide + closure + marginals, finalize
+        // bounds, pack, window sums (per-tau recurrence / groups of 32 / groups of 64: whichever
+        // regions exist), slide + closure + marginals, finalize
+        p.n_launches = 4 + (pl.mom_n32 > 0) + (pl.mom_n64 > pl.mom_n32) + (pl.grid.N_tau > pl.mom_n64);
     } else if (pl.rect_small) {
         p.kernel = TFSTAT_KERNEL_RECT_SMALL;
         p.tile_c = 1;

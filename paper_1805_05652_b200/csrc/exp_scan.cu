@@ -153,8 +153,9 @@ template <int NT, int RT, int TPC, bool STATS>
 __device__ __forceinline__ void exp_window_body(
     const Problem &pr, const ulonglong2 *__restrict__ packed, const int n_pad,
     float4 *__restrict__ W0, const unsigned vblock, const int n_nblocks, const int n_segs,
-    const int seg_len, unsigned long long *__restrict__ stats)
+    const int seg_len, const int n_limit, unsigned long long *__restrict__ stats)
 {
+    // (tau indices [0, n_limit) only: the larger ones are exp_moment_kernel's)
     constexpr int KW = kSlideChunk, NS = TPC > 2 ? 2 : kSlideStages, NW = NT / 32;
     constexpr uint32_t kTplBytes = KW * 2 * sizeof(ulonglong2);  // one template's share of a slot
     __shared__ __align__(128) ulonglong2 s_ring[NS][TPC][2 * KW];
@@ -168,7 +169,7 @@ __device__ __forceinline__ void exp_window_body(
     const int seg = (int)((vblock / n_nblocks) % n_segs);
     const int tpl0 = (int)(vblock / ((int64_t)n_nblocks * n_segs)) * TPC;
     const int n_first = (n_nblocks - 1 - j) * (NT * RT);
-    const int n_count = min(NT * RT, g.N_tau - n_first);
+    const int n_count = min(NT * RT, n_limit - n_first);
     const int m = min(seg * seg_len + seg_len, g.N_t0) - 1;  // the segment's last t0
 
     if (threadIdx.x == 0) {
@@ -346,6 +347,317 @@ __device__ __forceinline__ void exp_window_body(
 #pragma unroll
         for (int sft = 16; sft >= 1; sft >>= 1) nt += __shfl_xor_sync(0xffffffffu, nt, sft);
         if (lane == 0 && nt) atomicAdd(stats + 0, nt);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// exp_moment_kernel: the same window sums for GROUPS of R neighbouring tau values at once, by a
+// Taylor expansion of the weights in 1/tau about the group's centre.
+//
+// With u = 1/tau, u_c the centre of the group's u range, d_max its half width and s = t - t_lo,
+//     exp(-s u_n) = exp(-s u_c) exp(-s (u_n - u_c)) = e(s) sum_k (-rho_n)^k z(s)^k / k!,
+//     z = s d_max  (>= 0),   rho_n = (u_n - u_c) / d_max  in [-1, 1],
+// so the window sums of ALL tau_n of the group are combinations of 8 moments that do not depend
+// on n:  Q_k = sum_a e_a z_a^k / k! x_a  (e^2 and (2z)^k for a2, b2, ab),
+//     S_n = sum_{k<8} (-rho_n)^k Q_k  + the few atoms of [hi_{n0}, hi_n) (added to the moments as n
+// grows).  A window is at most 3 tau long, so z <= 1.5 (R - 1) dtau / tau; the plan (api.cu)
+// takes a group size R in {32, 64} only where that is <= kMomZCap = 0.17: the truncation error of
+// a WEIGHT is then below (2 x 0.17)^8 / 8! = 4.4e-9 relative (the squared weights are the worse
+// case), a tenth of the fp32 rounding of the sums it enters (DESIGN.md 6.2 has the numbers).
+// Every weight is positive and evaluated from its own time stamp with one MUFU.EX2: nothing
+// drifts, gaps are just time stamps.  Work per atom and template: 8 x 7 multiply-adds for R tau
+// values instead of 7 R.
+//
+// A thread owns HALF the moments of one group -- the even powers (lane & 1 = 0) or the odd ones
+// -- for TPC = 2 templates: 4 x 7 x 2 accumulators, so that one broadcast LDS.128 pair of an
+// atom serves 56 multiply-adds as in exp_window_kernel.  A warp is 16 groups x 2 halves of one
+// template pair.  That is few threads (config 4: 46 per template pair), each with a long loop, so
+// the 4 warps of a CTA share the SAME groups and templates and split the atoms between them,
+// chunk k to warp k mod 4, each through its own ring of bulk asynchronous copies (as the split
+// form of exp_direct.cu): moments are plain sums, so the partial ones meet in shared memory.
+// Then every warp finishes a quarter of the group's tau values.
+// ---------------------------------------------------------------------------------------
+constexpr float kMomZCap = 0.17f;
+constexpr int kMomKW = 64;   // atoms per bulk copy and template (2 KB); divides kPackBlock
+constexpr int kMomNS = 2;    // ring slots per warp
+constexpr int kMomNW = 4;    // warps per CTA: they split the atoms of the same windows
+static_assert(kPackBlock % kMomKW == 0, "a staged chunk must lie inside one packed time block");
+
+struct MomAcc {  // one moment of one template
+    u64 ab, fa, fb;
+    float c;
+};
+
+template <int R, bool STATS>
+__global__ void __launch_bounds__(32 * kMomNW, 4)
+    exp_moment_kernel(const __grid_constant__ Problem pr, const ulonglong2 *__restrict__ packed,
+                      const int n_pad, float4 *__restrict__ W0, const int n_lo, const int n_hi,
+                      const int n_gblocks, const int n_segs, const int seg_len,
+                      unsigned long long *__restrict__ stats)
+{
+    constexpr int TPC = 2, KW = kMomKW, NS = kMomNS;
+    constexpr uint32_t kTplBytes = KW * 2 * sizeof(ulonglong2);
+    __shared__ __align__(128) ulonglong2 s_ring[kMomNW][NS][TPC][2 * KW];
+    __shared__ __align__(8) unsigned long long s_bar[kMomNW][NS];
+    pdl_trigger();
+
+    const Grid &g = pr.grid;
+    const Bounds &bd = pr.bounds;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int h = lane & 1;  // 0: powers 0, 2, 4, 6;  1: powers 1, 3, 5, 7
+    // blockIdx = (tplpair * n_segs + seg) * n_gblocks + gb, heaviest groups (largest tau) first
+    const int gb = (int)(blockIdx.x % n_gblocks);
+    const int seg = (int)((blockIdx.x / n_gblocks) % n_segs);
+    const int tpl0 = (int)(blockIdx.x / ((int64_t)n_gblocks * n_segs)) * TPC;
+    const int n_groups = (n_hi - n_lo + R - 1) / R;
+    const int gi = n_groups - 1 - (gb * 16 + (lane >> 1));  // < 0: no group, alias the lightest
+    const bool g_ok = gi >= 0;
+    const int n0 = n_lo + max(gi, 0) * R;
+    const int Rg = min(R, n_hi - n0);
+    const int m = min(seg * seg_len + seg_len, g.N_t0) - 1;  // the segment's last t0
+
+    const uint32_t bar0 = smem_u32(&s_bar[warp][0]);
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(bar0 + 8 * s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
+
+    const ulonglong2 *__restrict__ rec[TPC];
+#pragma unroll
+    for (int q = 0; q < TPC; ++q)
+        rec[q] = packed + (int64_t)min(tpl0 + q, pr.n_templates - 1) * n_pad * 2;
+
+    // the group's expansion: u_c, d_max from its first and last tau (double, then fp32)
+    const double u_first = 1.0 / (double)tau_of(g, n0), u_last = 1.0 / (double)tau_of(g, n0 + Rg - 1);
+    const double u_c = 0.5 * (u_first + u_last), d_max = 0.5 * (u_first - u_last);
+    const float kc = (float)(-1.4426950408889634 * u_c);  // e = 2^(s kc)
+    const float dm = (float)d_max;                        // z = s dm
+    // steps between this thread's powers k, k + 2, k + 4, k + 6:  z^2 / ((k + 1)(k + 2))
+    const float c1 = h ? 1.0f / 6.0f : 0.5f, c2 = h ? 0.05f : 1.0f / 12.0f,
+                c3 = h ? 1.0f / 42.0f : 1.0f / 30.0f;
+
+    const int lo_m = __ldg(bd.lo + m);
+    const int t_lo = __ldg(bd.t + min(lo_m, bd.n_atoms - 1));
+    const int hi1 = max(hi_index(bd, g, m, n0), lo_m);  // end of the group's SHORTEST window
+
+    MomAcc acc[4][TPC];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            acc[j][q].ab = acc[j][q].fa = acc[j][q].fb = 0ull;
+            acc[j][q].c = 0.0f;
+        }
+    // one atom into the thread's four moments of both templates; dt = t - t_lo (finite), e its
+    // weight (0 for an atom outside this thread's window)
+    auto add_atom = [&](const float e, const float z, const ulonglong2 (&ra)[TPC],
+                        const ulonglong2 (&rb)[TPC]) {
+        const float zz = z * z;
+        float p[4], s2[4];
+        p[0] = e * (h ? z : 1.0f);
+        s2[0] = p[0] * (e * (h ? 2.0f : 1.0f));  // e^2 (2z)^k / k!
+        const float zc1 = zz * c1, zc2 = zz * c2, zc3 = zz * c3;
+        p[1] = p[0] * zc1;
+        p[2] = p[1] * zc2;
+        p[3] = p[2] * zc3;
+        s2[1] = s2[0] * (4.0f * zc1);
+        s2[2] = s2[1] * (4.0f * zc2);
+        s2[3] = s2[2] * (4.0f * zc3);
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+            float dtc, ab;
+            unpack2(ra[q].x, dtc, ab);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                ffma2(acc[j][q].ab, pack2(s2[j], s2[j]), ra[q].y);
+                ffma2(acc[j][q].fa, pack2(p[j], p[j]), rb[q].x);
+                ffma2(acc[j][q].fb, pack2(p[j], p[j]), rb[q].y);
+                acc[j][q].c = fmaf(s2[j], ab, acc[j][q].c);
+            }
+        }
+    };
+    // a bad SFT (packed as dtc = NaN on zero channels) spoils the sums of its template
+    auto poison = [&](const int q) { acc[0][q].c = nanf(""); };
+
+    // ---- phase 1: atoms [lo_m, hi1), chunk k by warp k mod kMomNW through its ring -------------
+    const int warp_e = __reduce_max_sync(0xffffffffu, hi1);
+    const int q0 = lo_m / KW;
+    const int nq = warp_e > lo_m ? (warp_e + KW - 1) / KW - q0 : 0;
+    auto fill = [&](const int k) {  // lane 0: chunk k -> slot (k / kMomNW) % NS
+        const int s = (k / kMomNW) % NS;
+        mbar_expect_tx(bar0 + 8 * s, TPC * kTplBytes);
+#pragma unroll
+        for (int q = 0; q < TPC; ++q)
+            bulk_copy(smem_u32(&s_ring[warp][s][q][0]), rec[q] + (int64_t)(q0 + k) * KW * 2, kTplBytes,
+                      bar0 + 8 * s);
+    };
+    if (lane == 0)
+        for (int u = 0; u < NS && warp + u * kMomNW < nq; ++u) fill(warp + u * kMomNW);
+#pragma unroll 1
+    for (int k = warp, u = 0; k < nq; k += kMomNW, ++u) {
+        const int s = u % NS;
+        const int cs = (q0 + k) * KW;  // first atom of the chunk
+        // s = t - t_lo = dtc + (t_block - t_lo): one FMA each for the exponent and for z
+        const int tb = __ldg(bd.t + cs - cs % kPackBlock);
+        const float sb = (float)(tb - t_lo);
+        const float cc = sb * kc, cz = sb * dm;
+        const int x0 = max(cs, lo_m) - cs;
+        const int x1 = min(cs + KW, warp_e) - cs;
+        mbar_wait(bar0 + 8 * s, (uint32_t)(u / NS) & 1u);
+#pragma unroll 2
+        for (int i = x0; i < x1; ++i) {
+            ulonglong2 ra[TPC], rb[TPC];
+            unsigned flag = 0u;
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                ra[q] = s_ring[warp][s][q][2 * i];
+                rb[q] = s_ring[warp][s][q][2 * i + 1];
+                flag |= (unsigned)(ra[q].x & 0x80000000ull);
+            }
+            const bool inside = cs + i < hi1;
+            float dtc = fabsf(__uint_as_float((unsigned)ra[0].x));
+            if (flag) {  // warp-uniform, rare: a gap edge (nothing to do) or a bad SFT
+                bool any_bad = false;
+#pragma unroll
+                for (int q = 0; q < TPC; ++q) {
+                    const float d = __uint_as_float((unsigned)ra[q].x);
+                    if (d != d) {
+                        any_bad = true;
+                        if (inside) poison(q);
+                    }
+                }
+                if (any_bad) dtc = (float)(__ldg(bd.t + cs + i) - tb);  // the record's is NaN
+            }
+            const float e = inside ? ex2_approx(fmaf(dtc, kc, cc)) : 0.0f;
+            add_atom(e, fmaf(dtc, dm, cz), ra, rb);
+        }
+        __syncwarp();  // every lane is done with the slot: refill it
+        if (lane == 0 && k + NS * kMomNW < nq) fill(k + NS * kMomNW);
+    }
+
+    // ---- the warps' partial moments meet in shared memory (the rings are done with); every warp
+    // leaves with the full sums
+    {
+        float *red = reinterpret_cast<float *>(&s_ring[0][0][0][0]);  // [NW][56][32]
+        static_assert(sizeof(s_ring) >= sizeof(float) * kMomNW * 56 * 32, "reduction buffer");
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                float v[7];
+                unpack2(acc[j][q].ab, v[0], v[1]);
+                unpack2(acc[j][q].fa, v[2], v[3]);
+                unpack2(acc[j][q].fb, v[4], v[5]);
+                v[6] = acc[j][q].c;
+#pragma unroll
+                for (int c = 0; c < 7; ++c) red[(warp * 56 + (j * TPC + q) * 7 + c) * 32 + lane] = v[c];
+            }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                float v[7];
+#pragma unroll
+                for (int c = 0; c < 7; ++c) {
+                    float t = 0.0f;
+#pragma unroll
+                    for (int w = 0; w < kMomNW; ++w) t += red[(w * 56 + (j * TPC + q) * 7 + c) * 32 + lane];
+                    v[c] = t;
+                }
+                acc[j][q].ab = pack2(v[0], v[1]);
+                acc[j][q].fa = pack2(v[2], v[3]);
+                acc[j][q].fb = pack2(v[4], v[5]);
+                acc[j][q].c = v[6];
+            }
+    }
+
+    // ---- phase 2: tau by tau -- the atoms [hi_{n-1}, hi_n) join the moments (a gather per lane:
+    // every group is at its own place by now), then S_n = sum_k (-rho_n)^k Q_k ------------------
+    // (warp w takes the tau values [w R/4, (w + 1) R/4) of every group: it first catches up with
+    // the atoms of the tau values before its own)
+    const int t_ref = (int)t0_of(g, m);
+    int hi_prev = hi1;
+    constexpr int RQ = R / kMomNW;
+#pragma unroll 1
+    for (int qn = warp * RQ - (warp ? 1 : 0); qn < (warp + 1) * RQ; ++qn) {
+        const bool catch_up = qn < warp * RQ;  // only extends the moments, stores nothing
+        // (lanes beyond their group's last tau repeat it: the shuffles below need every lane)
+        const int n = n0 + min(qn, Rg - 1);
+        const int hi_n = max(hi_index(bd, g, m, n), lo_m);
+        for (int al = hi_prev; al < hi_n; ++al) {
+            ulonglong2 ra[TPC], rb[TPC];
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) ldg_record(rec[q] + 2 * (int64_t)al, ra[q], rb[q]);
+            const float sdt = (float)(__ldg(bd.t + al) - t_lo);
+#pragma unroll
+            for (int q = 0; q < TPC; ++q) {
+                const float d = __uint_as_float((unsigned)ra[q].x);
+                if (d != d) poison(q);
+            }
+            add_atom(ex2_approx(sdt * kc), sdt * dm, ra, rb);
+        }
+        hi_prev = max(hi_prev, hi_n);
+        if (catch_up) continue;  // (warp-uniform)
+        // this thread's powers of -rho: (-rho)^h, then steps of rho^2
+        const double un = 1.0 / (double)tau_of(g, n);
+        const float rho = d_max > 0.0 ? (float)((un - u_c) / d_max) : 0.0f;
+        const float r2 = rho * rho;
+        float cj[4];
+        cj[0] = h ? -rho : 1.0f;
+        cj[1] = cj[0] * r2;
+        cj[2] = cj[1] * r2;
+        cj[3] = cj[2] * r2;
+        float S[TPC][7];
+#pragma unroll
+        for (int q = 0; q < TPC; ++q) {
+#pragma unroll
+            for (int c = 0; c < 7; ++c) S[q][c] = 0.0f;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float A, B, far, fai, fbr, fbi;
+                unpack2(acc[j][q].ab, A, B);
+                unpack2(acc[j][q].fa, far, fai);
+                unpack2(acc[j][q].fb, fbr, fbi);
+                S[q][0] = fmaf(cj[j], A, S[q][0]);
+                S[q][1] = fmaf(cj[j], B, S[q][1]);
+                S[q][2] = fmaf(cj[j], acc[j][q].c, S[q][2]);
+                S[q][3] = fmaf(cj[j], far, S[q][3]);
+                S[q][4] = fmaf(cj[j], fai, S[q][4]);
+                S[q][5] = fmaf(cj[j], fbr, S[q][5]);
+                S[q][6] = fmaf(cj[j], fbi, S[q][6]);
+            }
+#pragma unroll
+            for (int c = 0; c < 7; ++c) S[q][c] += __shfl_xor_sync(0xffffffffu, S[q][c], 1);
+        }
+        // scaled to the weight exp(-(t_lo - t0)/tau_n) of the window's first atom, as
+        // exp_window_kernel stores them; the even lane stores template 0, the odd one template 1
+        if (g_ok && qn < Rg && tpl0 + h < pr.n_templates) {
+            const float kexp = (float)(-1.4426950408889634 * un);
+            const float e0 = hi_n > lo_m ? ex2_approx((float)(t_lo - t_ref) * kexp) : 0.0f;
+            const float e02 = e0 * e0;
+            float Sq[7];
+#pragma unroll
+            for (int c = 0; c < 7; ++c) Sq[c] = h ? S[1][c] : S[0][c];
+            float4 *__restrict__ dst = W0 + (((int64_t)(tpl0 + h) * n_segs + seg) * g.N_tau + n) * 2;
+            dst[0] = make_float4(Sq[0] * e02, Sq[1] * e02, Sq[2] * e02, Sq[3] * e0);
+            dst[1] = make_float4(Sq[4] * e0, Sq[5] * e0, Sq[6] * e0, 0.0f);
+        }
+    }
+    if (STATS) {
+        // moment terms: (atom, power, template) triples of 7 multiply-adds each
+        const int hi_last = max(hi_index(bd, g, m, n0 + Rg - 1), lo_m);
+        unsigned long long nt = (g_ok && warp == 0)
+                                    ? (unsigned long long)(hi_last - lo_m) * 4ull *
+                                          (unsigned long long)min(TPC, pr.n_templates - tpl0)
+                                    : 0ull;
+#pragma unroll
+        for (int sft = 16; sft >= 1; sft >>= 1) nt += __shfl_xor_sync(0xffffffffu, nt, sft);
+        if (lane == 0 && nt) atomicAdd(stats + TFSTAT_STAT_MOMENT, nt);
     }
 }
 
@@ -830,12 +1142,12 @@ template <int NT, int RT, int TPC, bool STATS>
 __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
     exp_window_kernel(const Problem pr, const ulonglong2 *__restrict__ packed, const int n_pad,
                       float4 *__restrict__ W0, const int n_nblocks, const int n_segs,
-                      const int seg_len, unsigned long long *__restrict__ stats)
+                      const int seg_len, const int n_limit, unsigned long long *__restrict__ stats)
 {
     pdl_trigger();
     pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
     exp_window_body<NT, RT, TPC, STATS>(pr, packed, n_pad, W0, blockIdx.x, n_nblocks, n_segs, seg_len,
-                                        stats);
+                                        n_limit, stats);
 }
 
 template <int NT, int TPC, bool STATS>
@@ -884,14 +1196,33 @@ template <int NT, int RT, int TPC>
 cudaError_t launch_win(const Plan &pl, const Problem &pr, const ulonglong2 *packed, float4 *W0,
                        cudaStream_t st)
 {
-    const int nblk = (pl.grid.N_tau + NT * RT - 1) / (NT * RT);
+    const int n_limit = pl.mom_n32;  // tau indices below the moment kernel's regions
+    if (n_limit <= 0) return cudaSuccess;
+    const int nblk = (n_limit + NT * RT - 1) / (NT * RT);
     const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
     const int64_t n_ctas = (int64_t)nblk * pl.n_segs * groups;
     if (pl.stats)
         return launch_pdl(exp_window_kernel<NT, RT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr,
-                          packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, pl.stats);
+                          packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, n_limit, pl.stats);
     return launch_pdl(exp_window_kernel<NT, RT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr,
-                      packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, pl.stats);
+                      packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, n_limit, pl.stats);
+}
+
+// window sums of the tau indices [n_lo, n_hi) in groups of R (exp_moment_kernel)
+template <int R>
+cudaError_t launch_mom(const Plan &pl, const Problem &pr, const ulonglong2 *packed, float4 *W0,
+                       const int n_lo, const int n_hi, cudaStream_t st)
+{
+    if (n_hi <= n_lo) return cudaSuccess;
+    const int n_groups = (n_hi - n_lo + R - 1) / R;
+    const int n_gblocks = (n_groups + 15) / 16;
+    const int64_t pairs = (pl.n_templates + 1) / 2;
+    const int64_t n_ctas = (int64_t)n_gblocks * pl.n_segs * pairs;
+    if (pl.stats)
+        return launch_pdl(exp_moment_kernel<R, true>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
+                          pl.n_pad, W0, n_lo, n_hi, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
+    return launch_pdl(exp_moment_kernel<R, false>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
+                      pl.n_pad, W0, n_lo, n_hi, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 
 }  // namespace
@@ -910,6 +1241,10 @@ cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packe
     case 12: e = launch_win<64, 1, 2>(pl, pr, rec, W0, st); break;
     default: e = launch_win<64, 1, 1>(pl, pr, rec, W0, st); break;
     }
+    if (e != cudaSuccess) return e;
+    e = launch_mom<32>(pl, pr, rec, W0, pl.mom_n32, pl.mom_n64, st);
+    if (e != cudaSuccess) return e;
+    e = launch_mom<64>(pl, pr, rec, W0, pl.mom_n64, pl.grid.N_tau, st);
     if (e != cudaSuccess) return e;
     switch (pl.tile.NT) {
     case 128: return launch_nt<128>(pl, pr, rec, W0, partials, st);
