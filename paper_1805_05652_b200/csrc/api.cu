@@ -175,17 +175,6 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         const int64_t ctas1 = (int64_t)n_templates * pl.n_nblocks * pl.n_segs;
         pl.slide_tpc = (n_templates >= 2 && ctas1 / 2 >= 148 * 16) ? 2 : 1;
         pl.slide_rt = 1;
-        // window kernel (exp_window_kernel): RT tau values per thread x TPC templates per CTA share
-        // every broadcast load of an atom; the largest tile that still gives ~4 CTAs per SM
-        auto win_ctas = [&](int nt, int rt, int tpc) {
-            return (int64_t)((N_tau + nt * rt - 1) / (nt * rt)) * pl.n_segs *
-                   ((n_templates + tpc - 1) / tpc);
-        };
-        const int64_t fill = 148 * 4;
-        pl.win_rt = 1, pl.win_tpc = 1;
-        if (n_templates >= 2 && win_ctas(128, 4, 2) >= fill) pl.win_rt = 4, pl.win_tpc = 2;
-        else if (win_ctas(128, 4, 1) >= fill) pl.win_rt = 4;
-        else if (win_ctas(128, 2, 1) >= fill) pl.win_rt = 2;
         // grouped window sums (exp_moment_kernel): a group of R neighbouring tau shares 8 moments
         // while z = (window length) x (half width of the group in 1/tau) <= 1.5 (R - 1) dtau / tau
         // stays below kMomZCap = 0.17 (exp_scan.cu); R = 64 above that tau, R = 32 above half of
@@ -204,6 +193,30 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
             pl.mom_n32 = first_n(32);
             if (N_tau - pl.mom_n64 < 64) pl.mom_n64 = N_tau;
             if (pl.mom_n64 - pl.mom_n32 < 32) pl.mom_n32 = pl.mom_n64;
+        }
+        // per-tau window kernel (exp_window_kernel) for the tau indices [0, mom_n32): RT tau values
+        // per thread x TPC templates per CTA share every broadcast load of an atom.  The largest
+        // tile that still gives ~4 CTAs per SM -- unless a smaller one wastes fewer slots on a short
+        // range (relative cost per slot: RT = 4 1.0, RT = 2 1.15, one tau per thread 1.6)
+        {
+            const int n_lim = pl.mom_n32 > 0 ? pl.mom_n32 : 1;
+            auto win_ctas = [&](int nt, int rt, int tpc) {
+                return (int64_t)((n_lim + nt * rt - 1) / (nt * rt)) * pl.n_segs *
+                       ((n_templates + tpc - 1) / tpc);
+            };
+            const int64_t fill = 148 * 4;
+            const int tpc = n_templates >= 2 ? 2 : 1;
+            auto cost = [&](int nt, int rt, double per_slot) {
+                const int64_t b = (int64_t)nt * rt;
+                return (double)((n_lim + b - 1) / b * b) * per_slot;
+            };
+            pl.win_rt = 1, pl.win_tpc = 1;
+            double best = cost(64, 1, 1.6);
+            if (win_ctas(128, 2, tpc) >= fill && cost(128, 2, 1.15) <= best)
+                pl.win_rt = 2, pl.win_tpc = tpc, best = cost(128, 2, 1.15);
+            if (win_ctas(128, 4, tpc) >= fill && cost(128, 4, 1.0) <= best)
+                pl.win_rt = 4, pl.win_tpc = tpc;
+            if (pl.win_rt == 1 && tpc == 2 && win_ctas(64, 1, 2) >= fill) pl.win_tpc = 2;
         }
         if (tile_code) {  // TPC of the slide kernel + 10 x (RT TPC code of the window kernel)
             const int c = tile_code, w = c / 10, sl = c % 10;
@@ -404,9 +417,9 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.seg_len = pl.seg_len;
         p.n_segs = pl.n_segs;
         p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
-        // bounds, pack, window sums (per-tau recurrence / groups of 32 / groups of 64: whichever
-        // regions exist), slide + closure + marginals, finalize
-        p.n_launches = 4 + (pl.mom_n32 > 0) + (pl.mom_n64 > pl.mom_n32) + (pl.grid.N_tau > pl.mom_n64);
+        // bounds, pack, window sums (per-tau recurrence / groups of tau: whichever regions exist),
+        // slide + closure + marginals, finalize
+        p.n_launches = 4 + (pl.mom_n32 > 0) + (pl.grid.N_tau > pl.mom_n32);
     } else if (pl.rect_small) {
         p.kernel = TFSTAT_KERNEL_RECT_SMALL;
         p.tile_c = 1;

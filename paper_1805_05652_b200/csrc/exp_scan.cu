@@ -370,15 +370,17 @@ __device__ __forceinline__ void exp_window_body(
 //
 // A thread owns HALF the moments of one group -- the even powers (lane & 1 = 0) or the odd ones
 // -- for TPC = 2 templates: 4 x 7 x 2 accumulators, so that one broadcast LDS.128 pair of an
-// atom serves 56 multiply-adds as in exp_window_kernel.  A warp is 16 groups x 2 halves of one
-// template pair.  That is few threads (config 4: 46 per template pair), each with a long loop, so
+// atom serves 56 multiply-adds as in exp_window_kernel.  A warp is 8 groups x 2 halves x 2
+// template pairs (a half-warp per pair, so every quarter-warp phase of an LDS.128 still reads one
+// address).  That is few threads (config 4: 46 per template pair), each with a long loop, so
 // the 4 warps of a CTA share the SAME groups and templates and split the atoms between them,
 // chunk k to warp k mod 4, each through its own ring of bulk asynchronous copies (as the split
 // form of exp_direct.cu): moments are plain sums, so the partial ones meet in shared memory.
 // Then every warp finishes a quarter of the group's tau values.
 // ---------------------------------------------------------------------------------------
 constexpr float kMomZCap = 0.17f;
-constexpr int kMomKW = 64;   // atoms per bulk copy and template (2 KB); divides kPackBlock
+constexpr int kMomKW = 32;   // atoms per bulk copy and template (1 KB); divides kPackBlock
+constexpr int kMomGW = 8;    // groups per warp
 constexpr int kMomNS = 2;    // ring slots per warp
 constexpr int kMomNW = 4;    // warps per CTA: they split the atoms of the same windows
 static_assert(kPackBlock % kMomKW == 0, "a staged chunk must lie inside one packed time block");
@@ -388,32 +390,41 @@ struct MomAcc {  // one moment of one template
     float c;
 };
 
-template <int R, bool STATS>
+// tau indices [n32, n64) in groups of 32, [n64, N_tau) in groups of 64
+template <bool STATS>
 __global__ void __launch_bounds__(32 * kMomNW, 4)
     exp_moment_kernel(const __grid_constant__ Problem pr, const ulonglong2 *__restrict__ packed,
-                      const int n_pad, float4 *__restrict__ W0, const int n_lo, const int n_hi,
+                      const int n_pad, float4 *__restrict__ W0, const int n32, const int n64,
                       const int n_gblocks, const int n_segs, const int seg_len,
                       unsigned long long *__restrict__ stats)
 {
     constexpr int TPC = 2, KW = kMomKW, NS = kMomNS;
     constexpr uint32_t kTplBytes = KW * 2 * sizeof(ulonglong2);
-    __shared__ __align__(128) ulonglong2 s_ring[kMomNW][NS][TPC][2 * KW];
+    // a warp's ring slot: [pair][template of the pair][records]
+    __shared__ __align__(128) ulonglong2 s_ring[kMomNW][NS][2][TPC][2 * KW];
     __shared__ __align__(8) unsigned long long s_bar[kMomNW][NS];
     pdl_trigger();
 
     const Grid &g = pr.grid;
     const Bounds &bd = pr.bounds;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int h = lane & 1;  // 0: powers 0, 2, 4, 6;  1: powers 1, 3, 5, 7
-    // blockIdx = (tplpair * n_segs + seg) * n_gblocks + gb, heaviest groups (largest tau) first
+    const int h = lane & 1;    // 0: powers 0, 2, 4, 6;  1: powers 1, 3, 5, 7
+    const int tp = lane >> 4;  // which of the warp's two template pairs
+    // blockIdx = (tplquad * n_segs + seg) * n_gblocks + gb, heaviest groups (largest tau) first
     const int gb = (int)(blockIdx.x % n_gblocks);
     const int seg = (int)((blockIdx.x / n_gblocks) % n_segs);
-    const int tpl0 = (int)(blockIdx.x / ((int64_t)n_gblocks * n_segs)) * TPC;
-    const int n_groups = (n_hi - n_lo + R - 1) / R;
-    const int gi = n_groups - 1 - (gb * 16 + (lane >> 1));  // < 0: no group, alias the lightest
-    const bool g_ok = gi >= 0;
-    const int n0 = n_lo + max(gi, 0) * R;
-    const int Rg = min(R, n_hi - n0);
+    const int quad0 = (int)(blockIdx.x / ((int64_t)n_gblocks * n_segs)) * 2 * TPC;
+    // a pair beyond the batch aliases the last one (nothing of its is stored)
+    const int tpl0 = quad0 + tp * TPC;
+    const bool tp_ok = tpl0 < pr.n_templates;
+    // groups, from the largest tau down: G64 of 64 tau values, then G32 of 32
+    const int G64 = (g.N_tau - n64 + 63) / 64, G32 = (n64 - n32 + 31) / 32;
+    const int gx = gb * kMomGW + ((lane >> 1) & (kMomGW - 1));
+    const bool g_ok = gx < G64 + G32;
+    const int gi = g_ok ? gx : G64 + G32 - 1;  // no group: alias the lightest one
+    const int R = gi < G64 ? 64 : 32;
+    const int n0 = gi < G64 ? n64 + (G64 - 1 - gi) * 64 : n32 + (G64 + G32 - 1 - gi) * 32;
+    const int Rg = min(R, (gi < G64 ? g.N_tau : n64) - n0);
     const int m = min(seg * seg_len + seg_len, g.N_t0) - 1;  // the segment's last t0
 
     const uint32_t bar0 = smem_u32(&s_bar[warp][0]);
@@ -429,6 +440,14 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
 #pragma unroll
     for (int q = 0; q < TPC; ++q)
         rec[q] = packed + (int64_t)min(tpl0 + q, pr.n_templates - 1) * n_pad * 2;
+    // (lane 0 fills the ring for BOTH pairs of the warp)
+    const ulonglong2 *__restrict__ rec_fill[2][TPC];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int q = 0; q < TPC; ++q)
+            rec_fill[a][q] =
+                packed + (int64_t)min(quad0 + a * TPC + q, pr.n_templates - 1) * n_pad * 2;
 
     // the group's expansion: u_c, d_max from its first and last tau (double, then fp32)
     const double u_first = 1.0 / (double)tau_of(g, n0), u_last = 1.0 / (double)tau_of(g, n0 + Rg - 1);
@@ -488,11 +507,13 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     const int nq = warp_e > lo_m ? (warp_e + KW - 1) / KW - q0 : 0;
     auto fill = [&](const int k) {  // lane 0: chunk k -> slot (k / kMomNW) % NS
         const int s = (k / kMomNW) % NS;
-        mbar_expect_tx(bar0 + 8 * s, TPC * kTplBytes);
+        mbar_expect_tx(bar0 + 8 * s, 2 * TPC * kTplBytes);
 #pragma unroll
-        for (int q = 0; q < TPC; ++q)
-            bulk_copy(smem_u32(&s_ring[warp][s][q][0]), rec[q] + (int64_t)(q0 + k) * KW * 2, kTplBytes,
-                      bar0 + 8 * s);
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int q = 0; q < TPC; ++q)
+                bulk_copy(smem_u32(&s_ring[warp][s][a][q][0]),
+                          rec_fill[a][q] + (int64_t)(q0 + k) * KW * 2, kTplBytes, bar0 + 8 * s);
     };
     if (lane == 0)
         for (int u = 0; u < NS && warp + u * kMomNW < nq; ++u) fill(warp + u * kMomNW);
@@ -513,10 +534,11 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
             unsigned flag = 0u;
 #pragma unroll
             for (int q = 0; q < TPC; ++q) {
-                ra[q] = s_ring[warp][s][q][2 * i];
-                rb[q] = s_ring[warp][s][q][2 * i + 1];
+                ra[q] = s_ring[warp][s][tp][q][2 * i];
+                rb[q] = s_ring[warp][s][tp][q][2 * i + 1];
                 flag |= (unsigned)(ra[q].x & 0x80000000ull);
             }
+            flag = __any_sync(0xffffffffu, flag != 0u);  // (the two pairs may differ: bad SFTs)
             const bool inside = cs + i < hi1;
             float dtc = fabsf(__uint_as_float((unsigned)ra[0].x));
             if (flag) {  // warp-uniform, rare: a gap edge (nothing to do) or a bad SFT
@@ -541,7 +563,7 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     // ---- the warps' partial moments meet in shared memory (the rings are done with); every warp
     // leaves with the full sums
     {
-        float *red = reinterpret_cast<float *>(&s_ring[0][0][0][0]);  // [NW][56][32]
+        float *red = reinterpret_cast<float *>(&s_ring[0][0][0][0][0]);  // [NW][56][32]
         static_assert(sizeof(s_ring) >= sizeof(float) * kMomNW * 56 * 32, "reduction buffer");
         __syncthreads();
 #pragma unroll
@@ -582,11 +604,16 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     // the atoms of the tau values before its own)
     const int t_ref = (int)t0_of(g, m);
     int hi_prev = hi1;
-    constexpr int RQ = R / kMomNW;
+    // (a group of 64 takes 16 steps per warp, a group of 32 eight: the lanes of the shorter ones
+    // idle through the rest, the shuffles below need every lane)
+    const int RQ = R / kMomNW;
+    const int steps = __reduce_max_sync(0xffffffffu, RQ);
 #pragma unroll 1
-    for (int qn = warp * RQ - (warp ? 1 : 0); qn < (warp + 1) * RQ; ++qn) {
-        const bool catch_up = qn < warp * RQ;  // only extends the moments, stores nothing
-        // (lanes beyond their group's last tau repeat it: the shuffles below need every lane)
+    for (int it = warp ? -1 : 0; it < steps; ++it) {
+        const bool catch_up = it < 0;  // only extends the moments, stores nothing
+        const bool mine = it < RQ;
+        const int qn = warp * RQ + min(it, RQ - 1);
+        // (lanes beyond their group's last tau repeat it)
         const int n = n0 + min(qn, Rg - 1);
         const int hi_n = max(hi_index(bd, g, m, n), lo_m);
         for (int al = hi_prev; al < hi_n; ++al) {
@@ -636,7 +663,7 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
         }
         // scaled to the weight exp(-(t_lo - t0)/tau_n) of the window's first atom, as
         // exp_window_kernel stores them; the even lane stores template 0, the odd one template 1
-        if (g_ok && qn < Rg && tpl0 + h < pr.n_templates) {
+        if (g_ok && mine && qn < Rg && tp_ok && tpl0 + h < pr.n_templates) {
             const float kexp = (float)(-1.4426950408889634 * un);
             const float e0 = hi_n > lo_m ? ex2_approx((float)(t_lo - t_ref) * kexp) : 0.0f;
             const float e02 = e0 * e0;
@@ -651,7 +678,7 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     if (STATS) {
         // moment terms: (atom, power, template) triples of 7 multiply-adds each
         const int hi_last = max(hi_index(bd, g, m, n0 + Rg - 1), lo_m);
-        unsigned long long nt = (g_ok && warp == 0)
+        unsigned long long nt = (g_ok && tp_ok && warp == 0)
                                     ? (unsigned long long)(hi_last - lo_m) * 4ull *
                                           (unsigned long long)min(TPC, pr.n_templates - tpl0)
                                     : 0ull;
@@ -1208,21 +1235,21 @@ cudaError_t launch_win(const Plan &pl, const Problem &pr, const ulonglong2 *pack
                       packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, n_limit, pl.stats);
 }
 
-// window sums of the tau indices [n_lo, n_hi) in groups of R (exp_moment_kernel)
-template <int R>
+// window sums of the tau indices [mom_n32, N_tau) in groups of 32 and 64 (exp_moment_kernel)
 cudaError_t launch_mom(const Plan &pl, const Problem &pr, const ulonglong2 *packed, float4 *W0,
-                       const int n_lo, const int n_hi, cudaStream_t st)
+                       cudaStream_t st)
 {
-    if (n_hi <= n_lo) return cudaSuccess;
-    const int n_groups = (n_hi - n_lo + R - 1) / R;
-    const int n_gblocks = (n_groups + 15) / 16;
-    const int64_t pairs = (pl.n_templates + 1) / 2;
-    const int64_t n_ctas = (int64_t)n_gblocks * pl.n_segs * pairs;
+    const int G64 = (pl.grid.N_tau - pl.mom_n64 + 63) / 64, G32 = (pl.mom_n64 - pl.mom_n32 + 31) / 32;
+    if (G64 + G32 <= 0) return cudaSuccess;
+    const int n_gblocks = (G64 + G32 + kMomGW - 1) / kMomGW;
+    const int64_t quads = (pl.n_templates + 3) / 4;
+    const int64_t n_ctas = (int64_t)n_gblocks * pl.n_segs * quads;
     if (pl.stats)
-        return launch_pdl(exp_moment_kernel<R, true>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
-                          pl.n_pad, W0, n_lo, n_hi, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
-    return launch_pdl(exp_moment_kernel<R, false>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
-                      pl.n_pad, W0, n_lo, n_hi, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
+        return launch_pdl(exp_moment_kernel<true>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
+                          pl.n_pad, W0, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len,
+                          pl.stats);
+    return launch_pdl(exp_moment_kernel<false>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
+                      pl.n_pad, W0, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 
 }  // namespace
@@ -1242,9 +1269,7 @@ cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packe
     default: e = launch_win<64, 1, 1>(pl, pr, rec, W0, st); break;
     }
     if (e != cudaSuccess) return e;
-    e = launch_mom<32>(pl, pr, rec, W0, pl.mom_n32, pl.mom_n64, st);
-    if (e != cudaSuccess) return e;
-    e = launch_mom<64>(pl, pr, rec, W0, pl.mom_n64, pl.grid.N_tau, st);
+    e = launch_mom(pl, pr, rec, W0, st);
     if (e != cudaSuccess) return e;
     switch (pl.tile.NT) {
     case 128: return launch_nt<128>(pl, pr, rec, W0, partials, st);

@@ -218,7 +218,8 @@ def test_random_grids_all_kernel_families(pkg, case):
     wl = tiny_workload(6000 + case, slots, gaps, grid, n_templates=T, phi_random=True)
     atoms, t = wl.data.atoms[T - 1], wl.data.t
     for window, kws in ((EXP, [{"exp_method": pkg.EXP_DIRECT}, {"exp_method": pkg.EXP_SCAN},
-                                 {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 3)}]),
+                                 {"exp_method": pkg.EXP_SCAN, "tile": (0, 0, 3)},
+                                 {"exp_method": pkg.EXP_SCAN, "tile": (1000, 0, 0)}]),
                         (RECT, [{"rect_method": 1}, {"rect_method": 2},
                                   {"rect_method": 1, "tile": (2, 0, 0)},  # two rows per thread
                                   # seg_len < 0: the running-sum kernel where the tile kernel
@@ -816,7 +817,8 @@ def test_exp_scan_long_gaps_and_disjoint_windows(pkg):
         check_cells(m, f, ref, f"scan min_atoms={min_atoms}")
 
 
-@pytest.mark.parametrize("tpc,seg_len", [(0, 0), (1, 0), (2, 5), (422, 0), (211, 7), (122, 3)])
+@pytest.mark.parametrize("tpc,seg_len", [(0, 0), (1, 0), (2, 5), (422, 0), (211, 7), (122, 3),
+                                         (1000, 0), (1412, 4)])
 def test_exp_scan_batched_equals_oracle_and_direct(pkg, tpc, seg_len):
     """7 templates: with 2 templates per CTA (shared weights) the last group is ragged; tpc also
     selects the tile of the window-sum kernel (10 x (10 RT + TPC): 4, 2 or 1 tau per thread)."""
@@ -833,6 +835,49 @@ def test_exp_scan_batched_equals_oracle_and_direct(pkg, tpc, seg_len):
         ref = oracle.map2F(wl.data.atoms[k], wl.data.t, EXP, grid)
         check_cells(res.maps[k].cpu().numpy(), res.flags[k].cpu().numpy(), ref, f"scan tpl{k}")
         check_result(got[k], ref["twoF"], ref["flags"], grid.N_tau, f"scan tpl{k}")
+
+
+MOMENT_GRIDS = [
+    # slots, gaps, grid, seg_len                            which tau regions the plan groups
+    (2400, 0.0, Grid(0, 1800, 20, 1800, 1800, 700), 0),     # 32s above tau = 273 steps, 64s above 556
+    (2400, 0.15, Grid(-7200, 1800, 33, 3600, 1800, 650), 7),  # gaps, t0 before the data, 5 segments
+    (1500, 0.1, Grid(0, 3600, 12, 7200, 3600, 420), 0),     # dtau = 2 SFTs: windows overrun the data
+    (1300, 0.3, Grid(0, 900, 40, 900, 900, 620), 16),       # half-SFT steps, heavy gaps
+]
+
+
+@pytest.mark.parametrize("slots,gaps,grid,seg_len", MOMENT_GRIDS)
+def test_exp_scan_grouped_window_sums(pkg, slots, gaps, grid, seg_len):
+    """exp_moment_kernel: the window sums of large tau in groups of 32 / 64 neighbouring tau by the
+    Taylor expansion in 1/tau.  Grids on which the plan takes it, 3 templates (a
+    ragged template pair), a bad SFT in one of them, min_atoms 1 and 3: every cell of every
+    template against the oracle, and against the same search with every window sum by the
+    per-tau recurrence (tile code 1000)."""
+    T = 3
+    wl = tiny_workload(8000 + slots + grid.N_tau, slots, gaps, grid, n_templates=T, phi_random=True)
+    atoms, t = wl.data.atoms.copy(), wl.data.t
+    atoms[2, :, len(t) // 2] = np.nan  # template 2: one bad SFT (every channel, DESIGN.md R19)
+    grouped = pkg.plan_info(EXP, len(t), T, grid, exp_method=SCAN, tile=(0, 0, seg_len))
+    plain = pkg.plan_info(EXP, len(t), T, grid, exp_method=SCAN, tile=(1000, 0, seg_len))
+    assert grouped["n_launches"] == plain["n_launches"] + 1  # the grouped kernel does run
+    a, td = dev(atoms), dev(t)
+    for min_atoms in (2, 1, 3):
+        res = pkg.tfstat_search(a, td, EXP, grid, exp_method=SCAN, want_maps=True, want_flags=True,
+                                min_atoms=min_atoms, tile=(0, 0, seg_len))
+        ref_k = pkg.tfstat_search(a, td, EXP, grid, exp_method=SCAN, want_maps=True, want_flags=True,
+                                  min_atoms=min_atoms, tile=(1000, 0, seg_len))
+        torch.cuda.synchronize()
+        assert torch.equal(res.flags, ref_k.flags)
+        assert not torch.equal(res.maps, ref_k.maps)  # another kernel summed the windows
+        worst = 0.0
+        for k in range(T):
+            with np.errstate(invalid="ignore"):
+                ref = oracle.map2F(atoms[k], t, EXP, grid, min_atoms=min_atoms)
+            what = f"grouped window sums {grid} min_atoms {min_atoms} tpl{k}"
+            worst = max(worst, check_cells(res.maps[k].cpu().numpy(), res.flags[k].cpu().numpy(),
+                                           ref, what))
+            check_result(res.numpy()[k], ref["twoF"], ref["flags"], grid.N_tau, what)
+        assert worst < 0.25, worst  # (fraction of the tolerance used by the worst cell)
 
 
 def test_exp_scan_config2_full(pkg):
