@@ -577,17 +577,24 @@ def run_ours(args):
         # window sums (exp_window_kernel): the multiplicative recurrence, 7 multiply-adds per term
         # and nothing else; entering / leaving / re-summed atoms: 7 + 2 / TPC (weight argument, E^2)
         slide_terms = stv["terms_enter"] + stv["terms_leave"] + stv["terms_resum"]
-        lane_ops = 7.0 * w_terms + 2.0 * slide_terms / tpc + 23.0 * stv["cells"]
+        # grouped window sums (exp_moment_kernel): 7 multiply-adds per (atom, moment, template)
+        # term + the 22 FP32 operations of a thread's four weights and their squares per atom,
+        # shared by its 8 terms
+        mom_terms = stv.get("terms_moment", 0)
+        lane_ops = (7.0 * w_terms + 2.0 * slide_terms / tpc + 23.0 * stv["cells"] +
+                    (7.0 + 22.0 / 8.0) * mom_terms)
         packed_b = plan_packed_bytes(int(t.shape[0]), n_tpl)
         side["cfg4_exp_scan_roofline"] = {
-            "bound": "alu", "kernel": "exp_window_kernel + exp_slide_kernel", "kernel_ms": k_ms_s,
-            "executed": stv, "weighted_terms": w_terms, "templates_per_cta": tpc,
+            "bound": "alu", "kernel": "exp_window_kernel + exp_moment_kernel + exp_slide_kernel",
+            "kernel_ms": k_ms_s,
+            "executed": stv, "weighted_terms": w_terms, "moment_terms": mom_terms,
+            "templates_per_cta": tpc,
             "executed_fp32_lane_ops": lane_ops,
             "achieved": lane_ops / (k_ms_s * 1e-3) / 1e12, "peak": peak_ops / 1e12,
             "unit": "T FP32 lane-op/s", "frac": lane_ops / (k_ms_s * 1e-3) / peak_ops,
             "hbm_floor_us": packed_b / (peaks["hbm_gbs"] * 1e9) * 1e6,
             "hbm_frac": packed_b / (k_ms_s * 1e-3) / 1e9 / peaks["hbm_gbs"],
-            "terms_vs_direct": terms / max(w_terms, 1), "plan": plan_s}
+            "terms_vs_direct": terms / max(w_terms + mom_terms, 1), "plan": plan_s}
         side["cfg4_exp_scan"] = {"ms_per_step": ms_s, "effective_terms_per_s": terms / (ms_s * 1e-3),
                                  "speedup_vs_direct": ms_per_step / ms_s,
                                  "max_rel_diff_max2F_vs_direct": dmax,

@@ -22,7 +22,8 @@ _PROBE_LIB_PATH = os.path.join(_HERE, "libtfstat_probe.so")
 _lib = None
 _probe_lib = None
 N_STATS = 8  # TFSTAT_N_STATS
-STAT_NAMES = ("terms_window", "terms_enter", "terms_leave", "terms_resum", "cells", "redo64")
+STAT_NAMES = ("terms_window", "terms_enter", "terms_leave", "terms_resum", "cells", "redo64",
+              "terms_moment")
 KERNEL_NAMES = {1: "exp_direct", 2: "exp_slide", 3: "rect_small", 4: "rect_run", 5: "rect_cells",
                 6: "rect_tile"}
 

@@ -880,6 +880,40 @@ def test_exp_scan_grouped_window_sums(pkg, slots, gaps, grid, seg_len):
         assert worst < 0.25, worst  # (fraction of the tolerance used by the worst cell)
 
 
+def test_exp_scan_work_counters(pkg):
+    """tfstat_opts.stats (what bench.py's roofline of the sliding path is computed from): the
+    kernels count what they executed.  Per-tau window sums: exactly the atoms of the last row's
+    windows; cells: every cell once; grouped window sums: 8 moments x the atoms of each group's
+    LONGEST window."""
+    grid = Grid(0, 1800, 20, 1800, 1800, 700)
+    T = 4
+    wl = tiny_workload(8100, 2400, 0.1, grid, n_templates=T, phi_random=True)
+    a, t = dev(wl.data.atoms), dev(wl.data.t)
+    ref = oracle.map2F(wl.data.atoms[0], wl.data.t, EXP, grid)
+    last = ref["cnt"][grid.N_t0 - 1].astype(np.int64)  # atoms per window of the last t0
+    st = torch.zeros(pkg.binding.N_STATS, dtype=torch.int64, device="cuda")
+    pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, tile=(1000, 0, 0), stats=st)
+    v = dict(zip(pkg.binding.STAT_NAMES, (int(x) for x in st.cpu().numpy())))
+    assert v["terms_window"] == T * int(last.sum()) and v["terms_moment"] == 0
+    assert v["cells"] == T * grid.n_cells
+    # every step of every (template, tau) lets at most dt0 / T_SFT = 1 atom in and one out
+    assert 0 < v["terms_enter"] <= T * grid.N_tau * (grid.N_t0 - 1)
+    assert 0 < v["terms_leave"] <= T * grid.N_tau * (grid.N_t0 - 1)
+    st.zero_()
+    pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, stats=st)
+    w = dict(zip(pkg.binding.STAT_NAMES, (int(x) for x in st.cpu().numpy())))
+    # tau >= 1.5 (R - 1) dtau / 0.17 in groups of R = 32 and 64 (DESIGN.md 6.2)
+    n32, n64 = (int(np.ceil((1.5 * (R - 1) * grid.dtau / 0.17 - grid.tau_min) / grid.dtau))
+                for R in (32, 64))
+    assert (n32, n64) == (273, 555)
+    assert w["terms_window"] == T * int(last[:n32].sum())
+    groups = [(n, min(n + 32, n64)) for n in range(n32, n64, 32)] + \
+             [(n, min(n + 64, grid.N_tau)) for n in range(n64, grid.N_tau, 64)]
+    assert w["terms_moment"] == T * 8 * sum(int(last[b - 1]) for _, b in groups)
+    assert (w["cells"], w["terms_enter"], w["terms_leave"]) == (v["cells"], v["terms_enter"],
+                                                                 v["terms_leave"])
+
+
 def test_exp_scan_config2_full(pkg):
     wl = make_workload(2)
     atoms, t = wl.data.atoms[0], wl.data.t
