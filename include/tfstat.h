@@ -95,7 +95,7 @@ typedef struct tfstat_opts {
                            whenever the atoms fit its shared memory (n_atoms <= 2048)          */
     int32_t tile_c;     /* tuning, 0 = chosen from the problem shape.  Direct exp kernel: t0 cells
                            per thread (1,2,4,8,16); sliding exp kernel: templates per CTA
-                           (1,2) + 10 x (10 RT + TPC of the per-tau window-sum kernel, e.g. 422) + 1000 to
+                           (1,2,4) + 10 x (10 RT + TPC of the per-tau window-sum kernel, e.g. 422) + 1000 to
                            keep EVERY window sum with that kernel (no grouped moments); tfstat_map_general: tau cells per thread (1,2,4); lattice
                            rect kernels: rows per thread of the running-sum kernel (1, 2), or 8 =
                            the tile kernel on any grid whose lattice qualifies (auto only takes

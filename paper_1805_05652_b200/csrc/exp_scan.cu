@@ -1178,7 +1178,7 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
 }
 
 template <int NT, int TPC, bool STATS>
-__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : 4) : 1)
+__global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : TPC == 2 ? 4 : 3) : 1)
     exp_slide_kernel(const __grid_constant__ Problem pr, const ulonglong2 *__restrict__ packed,
                      const int n_pad,
                      const float4 *__restrict__ W0, Partial *__restrict__ partials,
@@ -1214,6 +1214,7 @@ template <int NT>
 cudaError_t launch_nt(const Plan &pl, const Problem &pr, const ulonglong2 *packed,
                       const float4 *W0, Partial *partials, cudaStream_t st)
 {
+    if (pl.slide_tpc == 4 && NT == 128) return launch_tpc<128, 4>(pl, pr, packed, W0, partials, st);
     if (pl.slide_tpc == 2) return launch_tpc<NT, 2>(pl, pr, packed, W0, partials, st);
     return launch_tpc<NT, 1>(pl, pr, packed, W0, partials, st);
 }

@@ -80,12 +80,12 @@ def test_opts_struct_size_and_plan_info(lib):
     info = pkg.plan_info(pkg.EXP, 2880, 4096, g)
     # (tile_c of the sliding form: templates per CTA of the slide kernel + 10 x (10 RT + TPC) of the
     # per-tau window-sum kernel, which here only has the 250 smallest tau values left: 2 per thread
-    # x 2 templates; 6 launches: bounds, pack, per-tau window sums, grouped window sums, slide,
-    # finalize)
-    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 222 and info["n_launches"] == 6
+    # x 2 templates; 4 templates per CTA in the slide kernel; 6 launches: bounds, pack, per-tau
+    # window sums, grouped window sums, slide, finalize)
+    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 224 and info["n_launches"] == 6
     # 1000 + ...: every window sum by the per-tau kernel
     info = pkg.plan_info(pkg.EXP, 2880, 4096, g, tile=(1000, 0, 0))
-    assert info["tile_c"] == 422 and info["n_launches"] == 5
+    assert info["tile_c"] == 424 and info["n_launches"] == 5
     assert pkg.plan_info(pkg.RECT, 48, 1, G(0, 1800, 24, 1800, 1800, 24))["kernel_name"] == "rect_small"
     big = pkg.plan_info(pkg.RECT, 13140, 1, G(0, 1800, 17520, 43200, 43200, 720))
     assert big["kernel_name"] == "rect_run" and big["lattice_J"] == 17519 + 719 * 24 + 1

@@ -818,15 +818,19 @@ def test_exp_scan_long_gaps_and_disjoint_windows(pkg):
 
 
 @pytest.mark.parametrize("tpc,seg_len", [(0, 0), (1, 0), (2, 5), (422, 0), (211, 7), (122, 3),
-                                         (1000, 0), (1412, 4)])
+                                         (1000, 0), (1412, 4), (4, 0), (424, 3)])
 def test_exp_scan_batched_equals_oracle_and_direct(pkg, tpc, seg_len):
     """7 templates: with 2 templates per CTA (shared weights) the last group is ragged; tpc also
     selects the tile of the window-sum kernel (10 x (10 RT + TPC): 4, 2 or 1 tau per thread)."""
     grid = Grid(0, 1800, 23, 3600, 3600, 140)
     wl = tiny_workload(201, 350, 0.1, grid, n_templates=7, phi_random=True)
     a, t = dev(wl.data.atoms), dev(wl.data.t)
+    # (4 templates per CTA exist for 128-thread CTAs only: ask for them)
+    tile = (tpc, 128 if tpc % 10 == 4 else 0, seg_len)
+    if tpc % 10 == 4:
+        assert pkg.plan_info(EXP, int(t.shape[0]), 7, grid, exp_method=SCAN, tile=tile)["tile_c"] % 10 == 4
     res = pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, want_maps=True, want_flags=True,
-                            tile=(tpc, 0, seg_len))
+                            tile=tile)
     direct = pkg.tfstat_search(a, t, EXP, grid, exp_method=1, want_flags=True)
     torch.cuda.synchronize()
     assert torch.equal(res.flags, direct.flags)
