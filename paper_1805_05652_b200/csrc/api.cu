@@ -180,11 +180,11 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         // grouped window sums (exp_moment_kernel): a group of R neighbouring tau shares 8 moments
         // while z = (window length) x (half width of the group in 1/tau) <= 1.5 (R - 1) dtau / tau
         // stays below kMomZCap = 0.17 (exp_scan.cu); R = 64 above that tau, R = 32 above half of
-        // it, the per-tau recurrence below.  Regions shorter than one group are not worth a launch.
+        // it, R = 16 above a quarter, the per-tau recurrence below.  Regions shorter than one group are not worth a launch.
         bool moments = n_templates >= 2;
         int tile_code = opts ? opts->tile_c : 0;
         if (tile_code >= 1000) moments = false, tile_code -= 1000;  // 1000 + ...: never
-        pl.mom_n32 = pl.mom_n64 = N_tau;
+        pl.mom_n16 = pl.mom_n32 = pl.mom_n64 = N_tau;
         if (moments) {
             auto first_n = [&](int R) {  // first tau index with tau >= 1.5 (R - 1) dtau / 0.17
                 const double tau_R = 1.5 * (R - 1) * (double)pl.grid.dtau / 0.17;
@@ -193,15 +193,17 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
             };
             pl.mom_n64 = first_n(64);
             pl.mom_n32 = first_n(32);
+            pl.mom_n16 = first_n(16);
             if (N_tau - pl.mom_n64 < 64) pl.mom_n64 = N_tau;
             if (pl.mom_n64 - pl.mom_n32 < 32) pl.mom_n32 = pl.mom_n64;
+            if (pl.mom_n32 - pl.mom_n16 < 16) pl.mom_n16 = pl.mom_n32;
         }
-        // per-tau window kernel (exp_window_kernel) for the tau indices [0, mom_n32): RT tau values
+        // per-tau window kernel (exp_window_kernel) for the tau indices [0, mom_n16): RT tau values
         // per thread x TPC templates per CTA share every broadcast load of an atom.  The largest
         // tile that still gives ~4 CTAs per SM -- unless a smaller one wastes fewer slots on a short
         // range (relative cost per slot: RT = 4 1.0, RT = 2 1.15, one tau per thread 1.6)
         {
-            const int n_lim = pl.mom_n32 > 0 ? pl.mom_n32 : 1;
+            const int n_lim = pl.mom_n16 > 0 ? pl.mom_n16 : 1;
             auto win_ctas = [&](int nt, int rt, int tpc) {
                 return (int64_t)((n_lim + nt * rt - 1) / (nt * rt)) * pl.n_segs *
                        ((n_templates + tpc - 1) / tpc);
@@ -421,7 +423,7 @@ int tfstat_plan_info(int window, int32_t n_atoms, int32_t n_templates, int32_t t
         p.n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * ((n_templates + pl.slide_tpc - 1) / pl.slide_tpc);
         // bounds, pack, window sums (per-tau recurrence / groups of tau: whichever regions exist),
         // slide + closure + marginals, finalize
-        p.n_launches = 4 + (pl.mom_n32 > 0) + (pl.grid.N_tau > pl.mom_n32);
+        p.n_launches = 4 + (pl.mom_n16 > 0) + (pl.grid.N_tau > pl.mom_n16);
     } else if (pl.rect_small) {
         p.kernel = TFSTAT_KERNEL_RECT_SMALL;
         p.tile_c = 1;

@@ -390,11 +390,12 @@ struct MomAcc {  // one moment of one template
     float c;
 };
 
-// tau indices [n32, n64) in groups of 32, [n64, N_tau) in groups of 64
+// tau indices [n16, n32) in groups of 16, [n32, n64) in groups of 32, [n64, N_tau) in groups of 64
 template <bool STATS>
 __global__ void __launch_bounds__(32 * kMomNW, 4)
     exp_moment_kernel(const __grid_constant__ Problem pr, const ulonglong2 *__restrict__ packed,
-                      const int n_pad, float4 *__restrict__ W0, const int n32, const int n64,
+                      const int n_pad, float4 *__restrict__ W0, const int n16, const int n32,
+                      const int n64,
                       const int n_gblocks, const int n_segs, const int seg_len,
                       unsigned long long *__restrict__ stats)
 {
@@ -417,14 +418,16 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     // a pair beyond the batch aliases the last one (nothing of its is stored)
     const int tpl0 = quad0 + tp * TPC;
     const bool tp_ok = tpl0 < pr.n_templates;
-    // groups, from the largest tau down: G64 of 64 tau values, then G32 of 32
-    const int G64 = (g.N_tau - n64 + 63) / 64, G32 = (n64 - n32 + 31) / 32;
+    // groups, from the largest tau down: G64 of 64 tau values, then G32 of 32, then G16 of 16
+    const int G64 = (g.N_tau - n64 + 63) / 64, G32 = (n64 - n32 + 31) / 32, G16 = (n32 - n16 + 15) / 16;
     const int gx = gb * kMomGW + ((lane >> 1) & (kMomGW - 1));
-    const bool g_ok = gx < G64 + G32;
-    const int gi = g_ok ? gx : G64 + G32 - 1;  // no group: alias the lightest one
-    const int R = gi < G64 ? 64 : 32;
-    const int n0 = gi < G64 ? n64 + (G64 - 1 - gi) * 64 : n32 + (G64 + G32 - 1 - gi) * 32;
-    const int Rg = min(R, (gi < G64 ? g.N_tau : n64) - n0);
+    const bool g_ok = gx < G64 + G32 + G16;
+    const int gi = g_ok ? gx : G64 + G32 + G16 - 1;  // no group: alias the lightest one
+    const int R = gi < G64 ? 64 : gi < G64 + G32 ? 32 : 16;
+    const int n0 = gi < G64         ? n64 + (G64 - 1 - gi) * 64
+                   : gi < G64 + G32 ? n32 + (G64 + G32 - 1 - gi) * 32
+                                    : n16 + (G64 + G32 + G16 - 1 - gi) * 16;
+    const int Rg = min(R, (gi < G64 ? g.N_tau : gi < G64 + G32 ? n64 : n32) - n0);
     const int m = min(seg * seg_len + seg_len, g.N_t0) - 1;  // the segment's last t0
 
     const uint32_t bar0 = smem_u32(&s_bar[warp][0]);
@@ -604,8 +607,8 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     // the atoms of the tau values before its own)
     const int t_ref = (int)t0_of(g, m);
     int hi_prev = hi1;
-    // (a group of 64 takes 16 steps per warp, a group of 32 eight: the lanes of the shorter ones
-    // idle through the rest, the shuffles below need every lane)
+    // (a group of 64 takes 16 steps per warp, one of 32 eight, one of 16 four: the lanes of the
+    // shorter ones idle through the rest, the shuffles below need every lane)
     const int RQ = R / kMomNW;
     const int steps = __reduce_max_sync(0xffffffffu, RQ);
 #pragma unroll 1
@@ -1224,7 +1227,7 @@ template <int NT, int RT, int TPC>
 cudaError_t launch_win(const Plan &pl, const Problem &pr, const ulonglong2 *packed, float4 *W0,
                        cudaStream_t st)
 {
-    const int n_limit = pl.mom_n32;  // tau indices below the moment kernel's regions
+    const int n_limit = pl.mom_n16;  // tau indices below the moment kernel's regions
     if (n_limit <= 0) return cudaSuccess;
     const int nblk = (n_limit + NT * RT - 1) / (NT * RT);
     const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
@@ -1236,21 +1239,22 @@ cudaError_t launch_win(const Plan &pl, const Problem &pr, const ulonglong2 *pack
                       packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, n_limit, pl.stats);
 }
 
-// window sums of the tau indices [mom_n32, N_tau) in groups of 32 and 64 (exp_moment_kernel)
+// window sums of the tau indices [mom_n16, N_tau) in groups of 16, 32 and 64 (exp_moment_kernel)
 cudaError_t launch_mom(const Plan &pl, const Problem &pr, const ulonglong2 *packed, float4 *W0,
                        cudaStream_t st)
 {
-    const int G64 = (pl.grid.N_tau - pl.mom_n64 + 63) / 64, G32 = (pl.mom_n64 - pl.mom_n32 + 31) / 32;
-    if (G64 + G32 <= 0) return cudaSuccess;
-    const int n_gblocks = (G64 + G32 + kMomGW - 1) / kMomGW;
+    const int G64 = (pl.grid.N_tau - pl.mom_n64 + 63) / 64, G32 = (pl.mom_n64 - pl.mom_n32 + 31) / 32,
+              G16 = (pl.mom_n32 - pl.mom_n16 + 15) / 16;
+    if (G64 + G32 + G16 <= 0) return cudaSuccess;
+    const int n_gblocks = (G64 + G32 + G16 + kMomGW - 1) / kMomGW;
     const int64_t quads = (pl.n_templates + 3) / 4;
     const int64_t n_ctas = (int64_t)n_gblocks * pl.n_segs * quads;
     if (pl.stats)
         return launch_pdl(exp_moment_kernel<true>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
-                          pl.n_pad, W0, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len,
+                          pl.n_pad, W0, pl.mom_n16, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len,
                           pl.stats);
     return launch_pdl(exp_moment_kernel<false>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
-                      pl.n_pad, W0, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
+                      pl.n_pad, W0, pl.mom_n16, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 
 }  // namespace

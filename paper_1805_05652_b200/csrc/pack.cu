@@ -90,7 +90,8 @@ cudaError_t launch_pack(const Plan &pl, const Problem &pr, void *packed, cudaStr
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    // (early launch only for small grids: see launch_pdl)
+    cfg.numAttrs = (uint64_t)grid.x * grid.y * kPackNT <= kPdlMaxThreads ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, pack_atoms_kernel, pr.atoms, pr.template_stride, pr.ld,
                               pr.bounds.t, pl.n_atoms, pl.n_pad,
                               static_cast<ulonglong2 *>(packed));

@@ -906,12 +906,13 @@ def test_exp_scan_work_counters(pkg):
     st.zero_()
     pkg.tfstat_search(a, t, EXP, grid, exp_method=SCAN, stats=st)
     w = dict(zip(pkg.binding.STAT_NAMES, (int(x) for x in st.cpu().numpy())))
-    # tau >= 1.5 (R - 1) dtau / 0.17 in groups of R = 32 and 64
-    n32, n64 = (int(np.ceil((1.5 * (R - 1) * grid.dtau / 0.17 - grid.tau_min) / grid.dtau))
-                for R in (32, 64))
-    assert (n32, n64) == (273, 555)
-    assert w["terms_window"] == T * int(last[:n32].sum())
-    groups = [(n, min(n + 32, n64)) for n in range(n32, n64, 32)] + \
+    # tau >= 1.5 (R - 1) dtau / 0.17 in groups of R = 16, 32 and 64
+    n16, n32, n64 = (int(np.ceil((1.5 * (R - 1) * grid.dtau / 0.17 - grid.tau_min) / grid.dtau))
+                     for R in (16, 32, 64))
+    assert (n16, n32, n64) == (132, 273, 555)
+    assert w["terms_window"] == T * int(last[:n16].sum())
+    groups = [(n, min(n + 16, n32)) for n in range(n16, n32, 16)] + \
+             [(n, min(n + 32, n64)) for n in range(n32, n64, 32)] + \
              [(n, min(n + 64, grid.N_tau)) for n in range(n64, grid.N_tau, 64)]
     assert w["terms_moment"] == T * 8 * sum(int(last[b - 1]) for _, b in groups)
     assert (w["cells"], w["terms_enter"], w["terms_leave"]) == (v["cells"], v["terms_enter"],
