@@ -581,6 +581,14 @@ def run_ours(args):
         # term + the 22 FP32 operations of a thread's four weights and their squares per atom,
         # shared by its 8 terms
         mom_terms = stv.get("terms_moment", 0)
+        # the same search with EVERY window sum by the per-tau recurrence (tile code 1000): the
+        # work the grouped sums stand for, for `frac_per_tau_form` below
+        st.zero_()
+        pkg.tfstat_search(atoms, t, pkg.EXP, grid, exp_method=pkg.EXP_SCAN, stats=st,
+                          tile=(1000, 0, 0))
+        stv_pt = dict(zip(pkg.binding.STAT_NAMES, (int(x) for x in st.cpu().numpy())))
+        lane_ops_pt = (7.0 * (stv_pt["terms_window"] + slide_terms) + 2.0 * slide_terms / tpc +
+                       23.0 * stv_pt["cells"])
         lane_ops = (7.0 * w_terms + 2.0 * slide_terms / tpc + 23.0 * stv["cells"] +
                     (7.0 + 22.0 / 8.0) * mom_terms)
         packed_b = plan_packed_bytes(int(t.shape[0]), n_tpl)
@@ -592,6 +600,11 @@ def run_ours(args):
             "executed_fp32_lane_ops": lane_ops,
             "achieved": lane_ops / (k_ms_s * 1e-3) / 1e12, "peak": peak_ops / 1e12,
             "unit": "T FP32 lane-op/s", "frac": lane_ops / (k_ms_s * 1e-3) / peak_ops,
+            "per_tau_form_fp32_lane_ops": lane_ops_pt,
+            "frac_per_tau_form": lane_ops_pt / (k_ms_s * 1e-3) / peak_ops,
+            "note": ("frac counts the EXECUTED lane-ops; the grouped window sums (8 moments per "
+                     "group of 16-64 tau) execute fewer than the per-tau recurrence they replace, "
+                     "whose lane-ops / this time / peak is frac_per_tau_form"),
             "hbm_floor_us": packed_b / (peaks["hbm_gbs"] * 1e9) * 1e6,
             "hbm_frac": packed_b / (k_ms_s * 1e-3) / 1e9 / peaks["hbm_gbs"],
             "terms_vs_direct": terms / max(w_terms + mom_terms, 1), "plan": plan_s}
