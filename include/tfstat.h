@@ -54,7 +54,10 @@ extern "C" {
                                E_a = exp(-(t_a - t_ref)/tau) shared by all t0 (the per-cell
                                factor cancels in eq. 7); one initial window sum, then each
                                t0 step adds the entering and subtracts the leaving atoms,
-                               backwards in t0 (csrc/exp_scan.cu)            */
+                               backwards in t0; the initial sums of large tau are shared
+                               between 16-64 neighbouring tau through an 8-term Taylor
+                               expansion of the weight in 1/tau, truncation < 5e-9 relative
+                               (csrc/exp_scan.cu)                            */
 
 typedef enum tfstat_status {
     TFSTAT_OK = 0,

@@ -24,6 +24,11 @@
 // |window| atoms per cell: 60x fewer weighted terms on BASELINE.json config 4, 300x on
 // config 5.  Terms/s reported for this path are EFFECTIVE terms (eq. A.6 count / time).
 //
+// Three kernels: exp_window_kernel (the window sum of a segment's last t0, one tau at a time, by a
+// multiplicative recurrence: the small tau), exp_moment_kernel (the same sums for groups of 16 to
+// 64 neighbouring tau at once, by a Taylor expansion of the weights in 1/tau: the large tau,
+// where almost all the terms are) and exp_slide_kernel (from there backwards in t0).
+//
 // Layout: lanes of a warp hold consecutive tau_n (same template), so the initial window is
 // streamed through shared memory and broadcast exactly like exp_direct.cu; a CTA is
 // (template, block of NT tau, segment of t0).  Long t0 grids with few tau (config 5) are cut
