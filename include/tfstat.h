@@ -192,6 +192,22 @@ int tfstat_marginalise(const float *map, const uint8_t *flags, int32_t N_t0, int
                        tfstat_result *out, void *workspace, size_t workspace_bytes,
                        void *stream, const tfstat_opts *opts_host);
 
+/* tfstat_marginalise WITHOUT a workspace and without any allocation, for callers that cannot
+ * call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * the scratch is a static __device__ array inside the library (37 888 bytes on every GPU that
+ * loads it).  Same kernels, same results as tfstat_marginalise, bit for bit.
+ *   Maximum: N_t0 * N_tau <= tfstat_marginalise_static_max_cells() = 2^31 - 1 (the scratch serves
+ *   every such map); beyond it TFSTAT_EINVAL, and TFSTAT_EWORKSPACE should a map ever need more
+ *   scratch records than the array holds.
+ *   The device that is current at the call must be the one `map`, `flags`, `out` and `stream`
+ *   belong to.  Every call on a device shares the one array: calls ordered on a stream are safe,
+ *   calls that OVERLAP on the GPU (other streams, concurrent graph replays) race on it.  Nothing
+ *   in it needs clearing between calls.  The first call on a device looks the array's address
+ *   up (cudaGetSymbolAddress: no allocation); make it outside graph capture. */
+size_t tfstat_marginalise_static_max_cells(void);
+int tfstat_marginalise_static(const float *map, const uint8_t *flags, int32_t N_t0,
+                              int32_t N_tau, tfstat_result *out, void *stream);
+
 /* Batched search over n_templates independent atom sets that share timestamps and grid;
  * map evaluation, cell closure and marginalisation fused, so only n_templates results reach
  * memory unless out_maps is given (eq. 5).

@@ -26,6 +26,7 @@ from .binding import (  # noqa: F401
     tfstat_map,
     tfstat_map_general,
     tfstat_marginalise,
+    tfstat_marginalise_static,
     tfstat_merge_detectors,
     tfstat_search,
     tfstat_search_host,

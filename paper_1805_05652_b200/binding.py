@@ -88,6 +88,9 @@ def load_library():
     lib.tfstat_marginalise_workspace_bytes.restype = sz
     lib.tfstat_marginalise_workspace_bytes.argtypes = [i32, i32]
     lib.tfstat_marginalise.argtypes = [vp, vp, i32, i32, vp, vp, sz, vp, op]
+    lib.tfstat_marginalise_static_max_cells.restype = sz
+    lib.tfstat_marginalise_static_max_cells.argtypes = []
+    lib.tfstat_marginalise_static.argtypes = [vp, vp, i32, i32, vp, vp]
     lib.tfstat_plan_info.argtypes = [C.c_int, i32, i32] + grid + [op, C.POINTER(_Plan)]
     lib.tfstat_validate_timestamps.argtypes = [vp, i32, vp, vp, op]
     lib.tfstat_search.argtypes = [vp, i64, i64, vp, i32, i32, C.c_int] + grid + [
@@ -289,6 +292,32 @@ def tfstat_marginalise(map2F: torch.Tensor, flags: Optional[torch.Tensor] = None
                                 _stream_ptr(stream), None)
     _check(rc, "tfstat_marginalise")
     return Results(out)
+
+
+def tfstat_marginalise_static(map2F: torch.Tensor, flags: Optional[torch.Tensor] = None, *,
+                              out: Optional[torch.Tensor] = None, stream=None) -> Results:
+    """tfstat_marginalise without a workspace: the library's static device scratch is used and
+    nothing is allocated by the call (pass `out`, a [1, 5] int32 CUDA tensor, to keep torch from
+    allocating either).  Calls that overlap on the GPU race on the scratch (include/tfstat.h)."""
+    lib = load_library()
+    _dev_f32(map2F, "map")
+    if map2F.dim() != 2 or not map2F.is_contiguous():
+        raise TfstatError("map must be a contiguous [N_t0, N_tau] tensor")
+    if flags is not None and not (flags.is_cuda and flags.dtype == torch.uint8
+                                  and flags.is_contiguous() and flags.shape == map2F.shape):
+        raise TfstatError("flags must be a contiguous CUDA uint8 tensor shaped like map")
+    N_t0, N_tau = map2F.shape
+    if out is None:
+        out = torch.empty((1, 5), dtype=torch.int32, device=map2F.device)
+    elif not (out.is_cuda and out.dtype == torch.int32 and out.is_contiguous()
+              and out.numel() == 5):
+        raise TfstatError("out must be a contiguous CUDA int32 tensor of 5 elements")
+    with torch.cuda.device(map2F.device):  # the static scratch is looked up on the CURRENT device
+        rc = lib.tfstat_marginalise_static(map2F.data_ptr(),
+                                           flags.data_ptr() if flags is not None else None,
+                                           N_t0, N_tau, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "tfstat_marginalise_static")
+    return Results(out.view(1, 5))
 
 
 def tfstat_search(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, grid, *,

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "plan.h"
@@ -746,6 +747,73 @@ size_t tfstat_search_host_scratch_bytes(int64_t template_stride, int32_t n_atoms
     return 2 * (align_up(Tc * tpl_bytes) + align_up(Tc * map_bytes)) + ws_bytes +
            align_up(sizeof(int32_t) * (size_t)n_atoms) +
            align_up(sizeof(tfstat_result) * (size_t)n_templates);
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------
+// tfstat_marginalise_static: tfstat_marginalise for callers that cannot allocate (code under
+// CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc) and have no
+// workspace to hand over.  The scratch of the marginalisation -- one Partial per CTA of
+// marginalise_kernel, read back by finalize_kernel -- lives in a file-scope __device__ array of
+// kStaticPartials records (37 888 bytes; every GPU that loads the library holds it until exit).
+// marginalise_blocks() never asks for more than 148 x 8 CTAs, so that serves every map the
+// entry point accepts (N_t0 N_tau < 2^31); a request beyond the array is refused.
+//
+// In host code the array's NAME is a host-side stand-in, not a device address: its address on
+// the current device comes from cudaGetSymbolAddress, asked for once per device with that
+// device current, and that pointer is what the kernels get.
+//
+// Every call shares the array.  Nothing in it has to start at zero (every CTA of
+// marginalise_kernel writes its own record before finalize_kernel reads any), so a call does
+// not care what the last one left; but two calls that OVERLAP on the GPU (different streams,
+// or graphs replayed concurrently) race on it.  Calls on one stream are ordered and safe.
+// ---------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticPartials = 148 * 8;
+constexpr int kStaticMaxDevices = 64;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticPartials * sizeof(Partial)];
+
+// device address of g_static_scratch on the CURRENT device; no allocation
+int static_scratch(Partial **out)
+{
+    static std::mutex mu;
+    static Partial *ptr[kStaticMaxDevices] = {};
+    int dev = -1;
+    TF_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return TFSTAT_EINVAL;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void *p = nullptr;
+        TF_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return TFSTAT_EWORKSPACE;
+        ptr[dev] = static_cast<Partial *>(p);
+    }
+    *out = ptr[dev];
+    return TFSTAT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t tfstat_marginalise_static_max_cells(void) { return ((size_t)1 << 31) - 1; }
+
+int tfstat_marginalise_static(const float *map, const uint8_t *flags, int32_t N_t0,
+                              int32_t N_tau, tfstat_result *out, void *stream)
+{
+    if (!map || !out || N_t0 < 1 || N_tau < 1) return TFSTAT_EINVAL;
+    const int64_t n_cells = (int64_t)N_t0 * N_tau;
+    if ((uint64_t)n_cells > tfstat_marginalise_static_max_cells()) return TFSTAT_EINVAL;
+    const int32_t nb = marginalise_blocks(n_cells);
+    if (nb > kStaticPartials) return TFSTAT_EWORKSPACE;  // beyond the static scratch
+    Partial *scratch = nullptr;
+    const int rc = static_scratch(&scratch);
+    if (rc != TFSTAT_OK) return rc;
+    TF_CUDA(launch_marginalise(map, flags, n_cells, N_tau, scratch, nb, out,
+                               static_cast<cudaStream_t>(stream)));
+    return TFSTAT_OK;
 }
 
 }  // extern "C"

@@ -168,6 +168,12 @@ def test_error_codes_before_any_cuda_call(lib):
     # a workspace that is not 16-byte aligned is an error, not a device fault
     assert lib.tfstat_marginalise(fake, None, 4, 4, fake, C.c_void_p(0x1004), 1 << 20, None,
                                   None) == -2
+    # the no-allocation variant: null pointers, empty maps, maps beyond its stated maximum
+    assert lib.tfstat_marginalise_static(None, None, 4, 4, fake, None) == -1
+    assert lib.tfstat_marginalise_static(fake, None, 4, 4, None, None) == -1
+    assert lib.tfstat_marginalise_static(fake, None, 0, 4, fake, None) == -1
+    assert lib.tfstat_marginalise_static(fake, None, 65536, 32768, fake, None) == -1
+    assert lib.tfstat_marginalise_static_max_cells() == 2**31 - 1
     # tfstat_validate_timestamps / tfstat_count_terms: null pointers, empty input
     assert lib.tfstat_validate_timestamps(None, 10, fake, None, None) == -1
     assert lib.tfstat_validate_timestamps(fake, 10, None, None, None) == -1
