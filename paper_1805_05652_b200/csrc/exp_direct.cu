@@ -77,8 +77,14 @@ __device__ __forceinline__ void accumulate_core(Acc<C> &acc, const ulonglong2 ra
     unpack2(ra.y, x[0], x[1]);
     unpack2(rb.x, x[3], x[4]);
     unpack2(rb.y, x[5], x[6]);
-    const float w = ex2_approx(fmaf(fabsf(dt), kexp, cexp));  // (sign bit of dtc: a flag, pack.cu)
-    const float w2 = w * w;
+    const float arg = fmaf(fabsf(dt), kexp, cexp);  // (sign bit of dtc: a flag, pack.cu)
+    const float w = ex2_approx(arg);
+    // w^2 = 2^(2 arg) by a second MUFU.EX2 on the argument with its exponent field bumped by one
+    // (an integer add on the ALU pipe): takes the multiply w * w off the FMA pipe, which is what
+    // this loop is bound by (measured on B200, config 4: 4.43e12 -> 4.49e12 terms/s).  arg = 0
+    // becomes 2^-126 and 2^that = 1, as it must.  A NaN argument (a bad SFT: pack.cu) does NOT
+    // survive the integer add -- w is NaN, w2 is not: close_cell carries the NaN over.
+    const float w2 = ex2_approx(__int_as_float(__float_as_int(arg) + 0x00800000));
     const u64 ww = pack2(w, w);
     const u64 w2w2 = pack2(w2, w2);
 #pragma unroll
@@ -265,9 +271,12 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
             const int lo_c = __ldg(bd.lo + m);
             const int cnt = max(hi_index(bd, g, m, n) - lo_c, 0);
             uint32_t fl;
+            // a bad SFT among the core atoms made w NaN but not w2 (accumulate_core): Fa, Fb are
+            // NaN, A is not -- make it, so that the cell is flagged as before
+            const float A = fmaf(0.0f, (S[3] + S[4]) + (S[5] + S[6]), S[0]);
             // the sums carry the weight of the tile's first cell; eq. (7) does not care, and the
             // fp64 redo of short ill-conditioned windows uses the cell's own t0
-            const float twoF = closure_2F_exp<false>(S[0], S[1], S[2], S[3], S[4], S[5], S[6], lo_c,
+            const float twoF = closure_2F_exp<false>(A, S[1], S[2], S[3], S[4], S[5], S[6], lo_c,
                                                      cnt, pr.min_atoms, fl, base, ld, bd.t,
                                                      t0_of(g, m), (double)tau_of(g, n));
             const int32_t flat = m * g.N_tau + n;
