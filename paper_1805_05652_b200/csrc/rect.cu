@@ -1064,7 +1064,9 @@ __device__ __forceinline__ void tile_marg2(RunMarg &rm, const float x0, const fl
 // Phi[j].  Measured on B200 (one-year map): one pair per thread 390 us (112 registers), two pairs
 // 400 us (128 registers: half the shared-memory wavefronts, but fewer independent eq. (7) chains
 // in flight and more address arithmetic per store).
-template <bool MARG, bool FLAGS, bool MAP>
+// EN: the lattice step e_n of a column if it is 1 (the full-resolution grids: strides become
+// immediates), 0 = taken from the bounds tables.
+template <bool MARG, bool FLAGS, bool MAP, int EN>
 __global__ void __launch_bounds__(kTileNT, 6)
     rect_tile_kernel(const Problem pr, const double *__restrict__ prefix,
                      Partial *__restrict__ partials, const int r, const int c, const int n_rowtiles,
@@ -1082,6 +1084,7 @@ __global__ void __launch_bounds__(kTileNT, 6)
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
+    const int e_n = EN ? EN : bd.e_n;
     const int rowtile = blockIdx.x % n_rowtiles;
     const int coltile = (blockIdx.x / n_rowtiles) % n_coltiles;
     const int tpl = blockIdx.x / (n_rowtiles * n_coltiles);
@@ -1212,15 +1215,26 @@ __global__ void __launch_bounds__(kTileNT, 6)
         if (lean) {
             // kTileGroup strips of the quad as ONE straight-line block: their eq. (7) chains are
             // independent and interleave (a branch per strip would fence them off from one
-            // another); the rare cells that fail the conditioning test are redone afterwards
+            // another); the rare cells that fail the conditioning test are redone afterwards.
+            // Addresses are carried as pointers that advance by one block per trip, so that a
+            // strip's loads and stores take immediate offsets (ncu before: 59 of the 170
+            // instructions of a block were address arithmetic and the conditioning test).
+            const int jstep = 32 * e_n;  // lattice points per strip
+            const float4 *pA = s_phiA + jl, *pB = s_phiB + jl;
+            float *pm[kTileCells];
+            uint8_t *pf[kTileCells];
+#pragma unroll
+            for (int k = 0; k < kTileCells; ++k) {
+                pm[k] = MAP ? maps + flat0[k] : nullptr;
+                pf[k] = FLAGS ? flg + flat0[k] : nullptr;
+            }
 #pragma unroll 1
             for (int s0 = 0; s0 < n_strips; s0 += kTileGroup) {
-                float res[kTileGroup][kTileCells], tt[kTileGroup][kTileCells];
-                const int jg = jl + 32 * s0 * bd.e_n;
+                float res[kTileGroup][kTileCells];
+                u64 tt2[kTileGroup][kTileNH];
 #pragma unroll
                 for (int strip = 0; strip < kTileGroup; ++strip) {
-                    const int jj = jg + 32 * strip * bd.e_n;
-                    const float4 fa = s_phiA[jj], fb = s_phiB[jj];
+                    const float4 fa = pA[strip * jstep], fb = pB[strip * jstep];
                     const u64 ph[8] = {pack2(fa.x, fa.x), pack2(fa.y, fa.y), pack2(fa.z, fa.z),
                                        pack2(fa.w, fa.w), pack2(fb.x, fb.x), pack2(fb.y, fb.y),
                                        pack2(fb.z, fb.z), pack2(fb.w, fb.w)};
@@ -1231,21 +1245,31 @@ __global__ void __launch_bounds__(kTileNT, 6)
                         for (int k = 0; k < 8; ++k) S[k] = fadd2(ph[k], U[h][k]);
                         const PairOut o = pair_closure_tile<true>(S);
                         unpack2(o.res, res[strip][2 * h], res[strip][2 * h + 1]);
-                        unpack2(o.t, tt[strip][2 * h], tt[strip][2 * h + 1]);
+                        tt2[strip][h] = o.t;
                     }
                 }
                 // one test for the whole block (fminf drops a NaN, so NaNs are looked for with
-                // the sum); which cells failed is only worked out in the rare case that one did
-                float tmin = tt[0][0], tsum = 0.0f;
+                // the sum, taken pairwise); which cells failed is only worked out in the rare case
+                // that one did
+                float tt[kTileGroup][kTileCells];
+                u64 ts2 = tt2[0][0];
 #pragma unroll
                 for (int strip = 0; strip < kTileGroup; ++strip)
 #pragma unroll
-                    for (int k = 0; k < kTileCells; ++k) {
-                        tmin = fminf(tmin, tt[strip][k]);
-                        tsum += tt[strip][k];
+                    for (int h = 0; h < kTileNH; ++h) {
+                        unpack2(tt2[strip][h], tt[strip][2 * h], tt[strip][2 * h + 1]);
+                        if (strip + h) ts2 = fadd2(ts2, tt2[strip][h]);
                     }
+                float tmin = tt[0][0], ts_lo, ts_hi;
+#pragma unroll
+                for (int strip = 0; strip < kTileGroup; ++strip)
+#pragma unroll
+                    for (int k = 0; k < kTileCells; ++k) tmin = fminf(tmin, tt[strip][k]);
+                unpack2(ts2, ts_lo, ts_hi);
+                const float tsum = ts_lo + ts_hi;
                 uint32_t fl = 0u;  // D <= 0 / count flags of the redone cells, 2 bits per cell
                 if (!(tmin > kTiny) || !(tsum == tsum)) {  // rare: the plain way, in fp64 from P
+                    const int jg = (int)(pA - s_phiA);
                     uint32_t slow = 0u;
 #pragma unroll
                     for (int strip = 0; strip < kTileGroup; ++strip)
@@ -1254,7 +1278,7 @@ __global__ void __launch_bounds__(kTileNT, 6)
                             slow |= (tt[strip][k] > kTiny ? 0u : 1u) << (kTileCells * strip + k);
 #pragma unroll
                     for (int strip = 0; strip < kTileGroup; ++strip) {
-                        const int64_t j = (int64_t)j_lo + jg + 32 * strip * bd.e_n;
+                        const int64_t j = (int64_t)j_lo + jg + strip * jstep;
 #pragma unroll
                         for (int k = 0; k < kTileCells; ++k) {
                             if (slow & (1u << (kTileCells * strip + k))) {
@@ -1272,10 +1296,9 @@ __global__ void __launch_bounds__(kTileNT, 6)
                     float x[kTileCells];
 #pragma unroll
                     for (int k = 0; k < kTileCells; ++k) {
-                        const int32_t flat = flat0[k] + 32 * (s0 + strip);
                         const uint32_t f = (fl >> (2 * (kTileCells * strip + k))) & 3u;
-                        if (MAP) __stcs(maps + flat, res[strip][k]);
-                        if (FLAGS) flg[flat] = (uint8_t)f;
+                        if (MAP) __stcs(pm[k] + 32 * strip, res[strip][k]);
+                        if (FLAGS) pf[k][32 * strip] = (uint8_t)f;
                         x[k] = f ? -INFINITY : res[strip][k];
                     }
                     if (MARG) {
@@ -1284,6 +1307,13 @@ __global__ void __launch_bounds__(kTileNT, 6)
                             tile_marg2(rm, x[2 * h], x[2 * h + 1], flat0[2 * h] + 32 * (s0 + strip),
                                        flat0[2 * h + 1] + 32 * (s0 + strip));
                     }
+                }
+                pA += kTileGroup * jstep;
+                pB += kTileGroup * jstep;
+#pragma unroll
+                for (int k = 0; k < kTileCells; ++k) {
+                    if (MAP) pm[k] += 32 * kTileGroup;
+                    if (FLAGS) pf[k] += 32 * kTileGroup;
                 }
             }
         } else {
@@ -1367,17 +1397,18 @@ cudaError_t launch_tile(const Plan &pl, const Problem &pr, const double *prefix,
         return launch_pdl(kern, (unsigned)n_ctas, kTileNT, 0, st, pr, prefix, partials, rr.r, rr.NTu,
                           rr.n_rowtiles, rr.n_coltiles);
     };
+    const bool e1 = pl.e_n == 1;
+#define TFSTAT_TILE_GO(M, F, P) \
+    (e1 ? go(rect_tile_kernel<M, F, P, 1>) : go(rect_tile_kernel<M, F, P, 0>))
     if (pr.out_flags) {
         if (pr.out_maps)
-            return partials ? go(rect_tile_kernel<true, true, true>)
-                            : go(rect_tile_kernel<false, true, true>);
-        return partials ? go(rect_tile_kernel<true, true, false>)
-                        : go(rect_tile_kernel<false, true, false>);
+            return partials ? TFSTAT_TILE_GO(true, true, true) : TFSTAT_TILE_GO(false, true, true);
+        return partials ? TFSTAT_TILE_GO(true, true, false) : TFSTAT_TILE_GO(false, true, false);
     }
     if (pr.out_maps)
-        return partials ? go(rect_tile_kernel<true, false, true>)
-                        : go(rect_tile_kernel<false, false, true>);
-    return go(rect_tile_kernel<true, false, false>);
+        return partials ? TFSTAT_TILE_GO(true, false, true) : TFSTAT_TILE_GO(false, false, true);
+    return TFSTAT_TILE_GO(true, false, false);
+#undef TFSTAT_TILE_GO
 }
 
 template <int Q>
