@@ -83,7 +83,7 @@ __device__ __forceinline__ void accumulate_core(Acc<C> &acc, const ulonglong2 ra
     // (an integer add on the ALU pipe): takes the multiply w * w off the FMA pipe, which is what
     // this loop is bound by (measured on B200, config 4: 4.43e12 -> 4.49e12 terms/s).  arg = 0
     // becomes 2^-126 and 2^that = 1, as it must.  A NaN argument (a bad SFT: pack.cu) does NOT
-    // survive the integer add -- w is NaN, w2 is not: close_cell carries the NaN over.
+    // survive the integer add -- w is NaN, w2 is not: close_cell flags the cell.
     const float w2 = ex2_approx(__int_as_float(__float_as_int(arg) + 0x00800000));
     const u64 ww = pack2(w, w);
     const u64 w2w2 = pack2(w2, w2);
@@ -271,14 +271,19 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
             const int lo_c = __ldg(bd.lo + m);
             const int cnt = max(hi_index(bd, g, m, n) - lo_c, 0);
             uint32_t fl;
-            // a bad SFT among the core atoms made w NaN but not w2 (accumulate_core): Fa, Fb are
-            // NaN, A is not -- make it, so that the cell is flagged as before
-            const float A = fmaf(0.0f, (S[3] + S[4]) + (S[5] + S[6]), S[0]);
             // the sums carry the weight of the tile's first cell; eq. (7) does not care, and the
             // fp64 redo of short ill-conditioned windows uses the cell's own t0
-            const float twoF = closure_2F_exp<false>(A, S[1], S[2], S[3], S[4], S[5], S[6], lo_c,
+            float twoF = closure_2F_exp<false>(S[0], S[1], S[2], S[3], S[4], S[5], S[6], lo_c,
                                                      cnt, pr.min_atoms, fl, base, ld, bd.t,
                                                      t0_of(g, m), (double)tau_of(g, n));
+            // a bad SFT among the core atoms made w NaN but not w2 (accumulate_core): Fa, Fb are
+            // NaN while D is fine, and eq. (7) comes out NaN: the cell is degenerate (flag bit 1),
+            // as it is when D itself is NaN.  (Carrying the NaN over to A in front of the closure
+            // instead cost 1.8 %: the register allocation of the loop is that touchy.)
+            if (twoF != twoF) {
+                twoF = 0.0f;
+                fl = 2u;
+            }
             const int32_t flat = m * g.N_tau + n;
             if (pr.out_maps) pr.out_maps[map_base + flat] = twoF;
             if (pr.out_flags) pr.out_flags[map_base + flat] = (uint8_t)fl;
