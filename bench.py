@@ -35,7 +35,7 @@ FP32_OPS_PER_TERM = 9
 FP32_LANES_PER_CLK_SM = 128  # cc 10.0: 4 SMSPs x 32 FP32 lanes
 # dram__bytes_read.sum + dram__bytes_write.sum of exp_direct_kernel, 296 templates of config 4
 NCU_CAPTURE = "profiles/r02_exp_direct_full.md"
-NCU_DRAM_BYTES_PER_TEMPLATE = (51.314944e6 + 2.098432e6) / 296
+NCU_DRAM_BYTES_PER_TEMPLATE = (51.410176e6 + 1.434368e6) / 296
 PACK_BLOCK = 768  # kPackBlock of csrc/tfstat_dev.cuh: packed records are padded to whole blocks
 
 
