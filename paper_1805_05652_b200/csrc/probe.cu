@@ -174,8 +174,10 @@ __global__ void __launch_bounds__(128, MINB)
             upk2(ra.y, x[0], x[1]);
             upk2(rb.x, x[3], x[4]);
             upk2(rb.y, x[5], x[6]);
-            const float w = exp2f_approx(fmaf(dt, kexp, cexp));
-            const float w2 = w * w;
+            // (as exp_direct.cu: w^2 from a second MUFU.EX2 on the exponent-bumped argument)
+            const float arg = fmaf(dt, kexp, cexp);
+            const float w = exp2f_approx(arg);
+            const float w2 = exp2f_approx(__int_as_float(__float_as_int(arg) + 0x00800000));
             const u64p ww = pk2(w, w), w2w2 = pk2(w2, w2);
             if (FORM == 0) {
                 const u64p abab = pk2(x[2], x[2]);
