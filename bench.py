@@ -224,6 +224,23 @@ def side_workloads(torch, pkg, peaks):
             rec["cells_per_s_map"] = cells / (med_map * 1e-3)
             rec["algorithmic_GBps_map"] = by / (med_map * 1e-3) / 1e9
             rec["hbm_frac_map"] = rec["algorithmic_GBps_map"] / peaks["hbm_gbs"]
+            # the same call captured ONCE in a CUDA graph and replayed (what a caller in a loop
+            # does with a launch-bound call: a cold single call above pays the host's launch
+            # latency of every kernel of the chain, the replay only the chain itself)
+            a1 = atoms[0]
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                fn_map()
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                pkg.tfstat_map(a1, t, window, wl.grid, out_map=maps, workspace=ws)
+            _, med_graph = timed(graph.replay)
+            rec["map_graph_replay_ms"] = med_graph
+            rec["hbm_frac_map_graph_replay"] = by / (med_graph * 1e-3) / 1e9 / peaks["hbm_gbs"]
+            del graph
         if cfg == 2:
             # the same map through tfstat_map_general (explicit grid arrays, one weight per term:
             # the paper's own brute-force design), exp and a 1025-point table
