@@ -995,16 +995,25 @@ __device__ __forceinline__ void exp_slide_body(
 
     // ---- slide backwards in t0: closure of cell m, then step to m - 1 ------------------------
     // (a warp whose tau slots all lie beyond the grid has nothing to do but the final reduction)
+    // The fast path is a tight loop of its own, left through one of two cold exits.  (ptxas still
+    // ends every step with ~45 register moves -- it builds the new sums next to the old ones and
+    // copies them back -- which neither this loop shape nor forcing eq. (7) in front of the
+    // update changes.)
+    bool finished = !(warp * 32 < n_count);
 #pragma unroll 1
-    for (; warp * 32 < n_count;) {
-        const int m = s.m;
-        const int n_in = s.lo_m - s.lo2, lv = max(s.hi2, s.lo_m), n_out = s.hi - lv;
-        const bool fresh0 = (s.hi2 <= s.lo_m) || (s.hi2 == s.lo2);
-        const float sh = (float)(s.t_ref - (int)t0_of(g, m - 1));
-        const bool calm = has_edge && m != m_beg && !fresh0 && n_in <= 1 && n_out <= 1 &&
-                          !(sh * kexp < kReanchorArg) && s.hi - s.lo_m >= pr.min_atoms;
-        bool done = false;  // this step was taken by the fast path
-        if (__all_sync(kFull, calm)) {
+    while (!finished) {
+        int lo3 = 0, hi3 = 0;
+        bool fresh = false;
+        bool resum_exit = false;  // left after the sums had moved on: re-sum, then advance
+#pragma unroll 1
+        for (;;) {
+            const int m = s.m;
+            const int n_in = s.lo_m - s.lo2, lv = max(s.hi2, s.lo_m), n_out = s.hi - lv;
+            const bool fresh0 = (s.hi2 <= s.lo_m) || (s.hi2 == s.lo2);
+            const float sh = (float)(s.t_ref - (int)t0_of(g, m - 1));
+            const bool calm = has_edge && m != m_beg && !fresh0 && n_in <= 1 && n_out <= 1 &&
+                              !(sh * kexp < kReanchorArg) && s.hi - s.lo_m >= pr.min_atoms;
+            if (!__all_sync(kFull, calm)) break;
             const int a_in = min(s.lo2, a_last), a_out = min(lv, a_last);
             if ((unsigned)(a_in - in_base) >= 32u) {  // warp-uniform: stage the next 32 entering atoms
                 in_base = max(a_in - 31, 0);
@@ -1021,7 +1030,7 @@ __device__ __forceinline__ void exp_slide_body(
             ulonglong2 oa[TPC], ob[TPC];
 #pragma unroll
             for (int q = 0; q < TPC; ++q) ldg_record_now(rec[q] + 2 * a_out, oa[q], ob[q]);
-            int lo3 = s.lo2, hi3 = s.hi2;
+            lo3 = s.lo2, hi3 = s.hi2;
             if (m - 1 > m_beg) {
                 lo3 = __ldg(bd.lo + m - 2);
                 hi3 = max(__ldg(bd.edge + (jn + (m - 2) * bd.e_m)), lo3);
@@ -1050,8 +1059,8 @@ __device__ __forceinline__ void exp_slide_body(
                                 (fabsf(twoF[q]) < 3.0e38f);
                 bad = bad | !ok;
             }
-            if (!__any_sync(kFull, bad)) {
-                done = true;
+            if (__any_sync(kFull, bad)) break;
+            {
                 // -- a5, branch-free
                 if (pr.out_maps) {  // (uniform; a search stores no maps)
 #pragma unroll
@@ -1088,7 +1097,7 @@ __device__ __forceinline__ void exp_slide_body(
                 const int t_in = s_tin[warp][a_in - in_base];
                 const float e_in = ex2_approx((float)(t_in - s.t_ref) * kexp);
                 const float e_out = ex2_approx((float)(t_out - s.t_ref) * kexp);
-                bool fresh = false;
+                fresh = false;
 #pragma unroll
                 for (int q = 0; q < TPC; ++q) {
                     const ulonglong2 ia = s_in[warp][q][2 * (a_in - in_base)];
@@ -1112,13 +1121,8 @@ __device__ __forceinline__ void exp_slide_body(
                     s.n_term[2] += (unsigned)n_out;
                 }
                 if (__any_sync(kFull, fresh)) {  // rare: some lane's window lost its weight
-                    if (fresh) {
-                        const SlideCtx c = {packed, n_pad, tpl0, n, n_ok ? 1 : 0, m_beg, kexp};
-                        SlideState<TPC> tmp;
-                        slide_copy<TPC>(tmp, s);
-                        slide_resum<TPC, STATS>(tmp, pr, c);
-                        slide_copy<TPC>(s, tmp);
-                    }
+                    resum_exit = true;
+                    break;
                 }
                 s.m = m - 1;
                 s.lo_m = s.lo2;
@@ -1127,13 +1131,24 @@ __device__ __forceinline__ void exp_slide_body(
                 s.hi2 = hi3;
             }
         }
-        if (!done) {
-            const SlideCtx c = {packed, n_pad, tpl0, n, n_ok ? 1 : 0, m_beg, kexp};
-            SlideState<TPC> tmp;
+        // ---- cold: what the fast path left undone
+        const SlideCtx c = {packed, n_pad, tpl0, n, n_ok ? 1 : 0, m_beg, kexp};
+        SlideState<TPC> tmp;
+        if (resum_exit) {
+            if (fresh) {
+                slide_copy<TPC>(tmp, s);
+                slide_resum<TPC, STATS>(tmp, pr, c);
+                slide_copy<TPC>(s, tmp);
+            }
+            s.m -= 1;
+            s.lo_m = s.lo2;
+            s.hi = s.hi2;
+            s.lo2 = lo3;
+            s.hi2 = hi3;
+        } else {
             slide_copy<TPC>(tmp, s);
-            const bool last = slide_step_generic<TPC, STATS>(tmp, pr, c);
+            finished = slide_step_generic<TPC, STATS>(tmp, pr, c);
             slide_copy<TPC>(s, tmp);
-            if (last) break;
         }
     }
     const int n_visited = warp * 32 < n_count ? m_end - m_beg : 0;
