@@ -200,35 +200,39 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
             if (pl.mom_n32 - pl.mom_n16 < 16) pl.mom_n16 = pl.mom_n32;
         }
         // per-tau window kernel (exp_window_kernel) for the tau indices [0, mom_n16): RT tau values
-        // per thread x TPC templates per CTA share every broadcast load of an atom.  The largest
-        // tile that still gives ~4 CTAs per SM -- unless a smaller one wastes fewer slots on a short
-        // range (relative cost per slot: RT = 4 1.0, RT = 2 1.15, one tau per thread 1.6)
+        // per thread x TPC templates per CTA share every broadcast load of an atom.  Of the tiles
+        // that give the GPU ~8 warps per SM, the one with the least cost: slots (the range rounded
+        // up to whole CTAs) x the relative cost of a slot (RT = 4 1.0, RT = 2 1.15, one tau per
+        // thread 1.6); short ranges -- what the grouped sums leave over -- take 64-thread CTAs.
         {
             const int n_lim = pl.mom_n16 > 0 ? pl.mom_n16 : 1;
-            auto win_ctas = [&](int nt, int rt, int tpc) {
-                return (int64_t)((n_lim + nt * rt - 1) / (nt * rt)) * pl.n_segs *
-                       ((n_templates + tpc - 1) / tpc);
-            };
-            const int64_t fill = 148 * 4;
             const int tpc = n_templates >= 2 ? 2 : 1;
+            auto warps = [&](int nt, int rt, int t) {
+                return (int64_t)((n_lim + nt * rt - 1) / (nt * rt)) * pl.n_segs *
+                       ((n_templates + t - 1) / t) * (nt / 32);
+            };
             auto cost = [&](int nt, int rt, double per_slot) {
                 const int64_t b = (int64_t)nt * rt;
                 return (double)((n_lim + b - 1) / b * b) * per_slot;
             };
-            pl.win_rt = 1, pl.win_tpc = 1;
+            pl.win_nt = 64, pl.win_rt = 1, pl.win_tpc = warps(64, 1, tpc) >= 148 * 8 ? tpc : 1;
             double best = cost(64, 1, 1.6);
-            if (win_ctas(128, 2, tpc) >= fill && cost(128, 2, 1.15) <= best)
-                pl.win_rt = 2, pl.win_tpc = tpc, best = cost(128, 2, 1.15);
-            if (win_ctas(128, 4, tpc) >= fill && cost(128, 4, 1.0) <= best)
-                pl.win_rt = 4, pl.win_tpc = tpc;
-            if (pl.win_rt == 1 && tpc == 2 && win_ctas(64, 1, 2) >= fill) pl.win_tpc = 2;
+            const int cand[4][2] = {{64, 2}, {128, 2}, {64, 4}, {128, 4}};
+            for (const auto &cd : cand) {
+                const double cst = cost(cd[0], cd[1], cd[1] == 2 ? 1.15 : 1.0);
+                if (warps(cd[0], cd[1], tpc) >= 148 * 8 && cst <= best)
+                    pl.win_nt = cd[0], pl.win_rt = cd[1], pl.win_tpc = tpc, best = cst;
+            }
         }
         if (tile_code) {  // TPC of the slide kernel + 10 x (RT TPC code of the window kernel)
             const int c = tile_code, w = c / 10, sl = c % 10;
             if (sl != 1 && sl != 2 && sl != 4) return pl;
             if (w != 0 && w != 11 && w != 12 && w != 21 && w != 22 && w != 41 && w != 42) return pl;
             pl.slide_tpc = (sl == 4 && pl.tile.NT != 128) ? 2 : sl;  // 4: 128-thread CTAs only
-            if (w) pl.win_rt = w / 10, pl.win_tpc = w % 10;
+            if (w) {  // (a requested tile keeps 128-thread CTAs, but one tau per thread has 64)
+                pl.win_rt = w / 10, pl.win_tpc = w % 10;
+                pl.win_nt = pl.win_rt == 1 ? 64 : 128;
+            }
         }
     }
     if (window == TFSTAT_WINDOW_RECT) {

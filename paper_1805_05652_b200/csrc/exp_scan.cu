@@ -1285,11 +1285,16 @@ cudaError_t launch_exp_scan(const Plan &pl, const Problem &pr, const void *packe
     const ulonglong2 *rec = static_cast<const ulonglong2 *>(packed);
     float4 *W0 = static_cast<float4 *>(w0);
     cudaError_t e;
-    switch (pl.win_rt * 10 + pl.win_tpc) {
+    switch ((pl.win_nt == 64 ? 100 : 0) + pl.win_rt * 10 + pl.win_tpc) {
     case 42: e = launch_win<128, 4, 2>(pl, pr, rec, W0, st); break;
     case 41: e = launch_win<128, 4, 1>(pl, pr, rec, W0, st); break;
     case 22: e = launch_win<128, 2, 2>(pl, pr, rec, W0, st); break;
     case 21: e = launch_win<128, 2, 1>(pl, pr, rec, W0, st); break;
+    case 142: e = launch_win<64, 4, 2>(pl, pr, rec, W0, st); break;
+    case 141: e = launch_win<64, 4, 1>(pl, pr, rec, W0, st); break;
+    case 122: e = launch_win<64, 2, 2>(pl, pr, rec, W0, st); break;
+    case 121: e = launch_win<64, 2, 1>(pl, pr, rec, W0, st); break;
+    case 112:
     case 12: e = launch_win<64, 1, 2>(pl, pr, rec, W0, st); break;
     default: e = launch_win<64, 1, 1>(pl, pr, rec, W0, st); break;
     }

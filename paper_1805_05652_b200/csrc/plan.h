@@ -61,6 +61,7 @@ struct Plan {
     int32_t slide_tpc;  // templates per CTA (1, 2, 4): they share the weights
     int32_t slide_rt;   // (always 1: kept for the launchers)
     int32_t win_rt, win_tpc;  // exp_window_kernel: tau values per thread, templates per CTA
+    int32_t win_nt;           // ... and threads per CTA (64 or 128; one tau per thread: 64)
     // exp_moment_kernel: tau indices [mom_n16, mom_n32) in groups of 16, [mom_n32, mom_n64) in
     // groups of 32, [mom_n64, N_tau) in groups of 64; [0, mom_n16) stay with exp_window_kernel
     // (all = N_tau: no grouped sums at all)

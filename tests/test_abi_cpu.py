@@ -79,10 +79,10 @@ def test_opts_struct_size_and_plan_info(lib):
     # defaults: the sliding form; config 1: the one-launch rect kernel; invalid shapes: errors
     info = pkg.plan_info(pkg.EXP, 2880, 4096, g)
     # (tile_c of the sliding form: templates per CTA of the slide kernel + 10 x (10 RT + TPC) of the
-    # per-tau window-sum kernel, which here only has the 109 smallest tau values left: one per
+    # per-tau window-sum kernel, which here only has the 109 smallest tau values left: two per
     # thread x 2 templates; 4 templates per CTA in the slide kernel; 6 launches: bounds, pack,
     # per-tau window sums, grouped window sums, slide, finalize)
-    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 124 and info["n_launches"] == 6
+    assert info["kernel_name"] == "exp_slide" and info["tile_c"] == 224 and info["n_launches"] == 6
     # 1000 + ...: every window sum by the per-tau kernel
     info = pkg.plan_info(pkg.EXP, 2880, 4096, g, tile=(1000, 0, 0))
     assert info["tile_c"] == 424 and info["n_launches"] == 5
