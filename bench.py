@@ -219,6 +219,18 @@ def side_workloads(torch, pkg, peaks):
         if window == 1:
             rec["terms_per_s_map"] = terms / (med_map * 1e-3)
             rec["terms_per_s_fused"] = terms / (med_fused * 1e-3)
+            # the same map through the DEFAULT form (EXP_AUTO = the exact sliding form, DESIGN.md
+            # 6.2): what a caller gets without options; EFFECTIVE terms/s (A.6 count / time)
+            ws_a = torch.empty(pkg.workspace_bytes(window, t.shape[0], 1, wl.grid),
+                               dtype=torch.uint8, device="cuda")
+            fn_auto = lambda: pkg.tfstat_map(atoms[0], t, window, wl.grid, out_map=maps,
+                                             workspace=ws_a)
+            for _ in range(3):
+                fn_auto()
+            _, med_auto = timed(fn_auto)
+            rec["default_form_map_ms"] = med_auto
+            rec["default_form_effective_terms_per_s"] = terms / (med_auto * 1e-3)
+            rec["default_form_plan"] = pkg.plan_info(window, int(t.shape[0]), 1, wl.grid)
         else:
             by = 32 * int(t.shape[0]) + 4 * cells  # atoms once + 4 B per cell
             rec["cells_per_s_map"] = cells / (med_map * 1e-3)
