@@ -540,10 +540,12 @@ def run_ours(args):
         "plan": plan,
         "probes_ops_per_clk_sm": {k: round(v["ops_per_clk_sm"], 2) for k, v in probes.items()},
         # the kernel's core loop with nothing around it, in the shipped accumulator layout (pairs
-        # of cells: two broadcast-scalar multiplicands) and in round 1's (pairs of channels)
+        # of cells: two broadcast-scalar multiplicands) and in round 1's (pairs of channels); and
+        # with 2 / 4 more LDS.128 per atom whose results nobody uses (what do register
+        # write-backs that are not accumulator updates cost the FMA stream? DESIGN.md 6.1)
         "isolated_core_loop_terms_per_clk_sm": {
             f"{d['form']}_c{d['cells']}": round(d["terms_per_clk_sm"], 2)
-            for d in (pkg.probe_direct_loop(f, c) for f in (0, 1) for c in (8, 16))},
+            for d in (pkg.probe_direct_loop(f, c) for f in (0, 1, 2, 3) for c in (8, 16))},
         "probe_sm_mhz": round(probes["ffma"]["sm_mhz"], 1),
     }
 

@@ -39,6 +39,8 @@ int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s, double *ops_per
  * thread, 3 for 16), in one of two accumulator layouts:
  *   form 0  pairs of CHANNELS of one cell: FFMA2 acc, w (broadcast scalar), atom register pair
  *   form 1  pairs of CELLS of one channel: FFMA2 acc, w, x (two broadcast scalars)
+ *   form 2, 3  form 1 with two / four more broadcast LDS.128 per atom whose results are not used:
+ *           8 / 16 more register write-backs per atom and nothing else
  * cells = 8 or 16 per thread.  Outputs (HOST pointers): window-atom terms per SM clock per SM
  * (clock64 span on SM 0) and terms per second over the whole GPU. */
 int tfstat_probe_direct_loop(int form, int cells, int reps, double *terms_per_clk_sm,

@@ -545,11 +545,13 @@ def probe_alu(kind: str, reps: int = 3) -> dict:
 
 def probe_direct_loop(form: int, cells: int, reps: int = 200) -> dict:
     """The isolated core loop of the direct exponential sum in one of its two accumulator layouts
-    (tfstat_probe.h): 0 = channel pairs (scalar x register pair), 1 = cell pairs (two scalars)."""
+    (tfstat_probe.h): 0 = channel pairs (scalar x register pair), 1 = cell pairs (two scalars);
+    2, 3 = cell pairs with two / four more LDS.128 per atom whose results are not used."""
     lib = load_probe_library()
     a, b = C.c_double(0), C.c_double(0)
     rc = lib.tfstat_probe_direct_loop(int(form), int(cells), int(reps), C.byref(a), C.byref(b))
     if rc != 0:
         raise TfstatError(f"tfstat_probe_direct_loop({form}, {cells}): status {rc}")
-    return dict(form="cell_pairs" if form else "channel_pairs", cells=cells,
+    names = ("channel_pairs", "cell_pairs", "cell_pairs_plus_2_lds128", "cell_pairs_plus_4_lds128")
+    return dict(form=names[form], cells=cells,
                 terms_per_clk_sm=a.value, terms_per_s=b.value)

@@ -169,6 +169,18 @@ __global__ void __launch_bounds__(128, MINB)
 #pragma unroll 24
         for (int i = 0; i < kLoopAtoms; ++i) {
             const ulonglong2 ra = s[2 * i], rb = s[2 * i + 1];
+            if (FORM >= 2) {
+                // FORM 2 / 3: two / four more broadcast LDS.128 per atom whose results nobody
+                // uses -- 8 / 16 more register write-backs and nothing else (do they cost what
+                // the FMA pipe's own write-backs cost?)
+#pragma unroll
+                for (int e = 0; e < 2 * (FORM - 1); ++e) {
+                    float d0, d1, d2, d3;
+                    asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                 : "=f"(d0), "=f"(d1), "=f"(d2), "=f"(d3)
+                                 : "r"((unsigned)__cvta_generic_to_shared(&s[(2 * i + e) % (2 * kLoopAtoms)])));
+                }
+            }
             float x[7], dt;
             upk2(ra.x, dt, x[2]);
             upk2(ra.y, x[0], x[1]);
@@ -219,7 +231,7 @@ __global__ void __launch_bounds__(128, MINB)
 extern "C" int tfstat_probe_direct_loop(int form, int cells, int reps, double *terms_per_clk_sm,
                                         double *terms_per_s)
 {
-    if ((form != 0 && form != 1) || (cells != 8 && cells != 16) || !terms_per_clk_sm)
+    if (form < 0 || form > 3 || (cells != 8 && cells != 16) || !terms_per_clk_sm)
         return TFSTAT_EINVAL;
     if (reps < 1) reps = 200;
     int dev = 0, n_sm = 0;
@@ -254,6 +266,10 @@ extern "C" int tfstat_probe_direct_loop(int form, int cells, int reps, double *t
             if (form == 1 && cells == 8) probe_loop_kernel<1, 8, 4><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
             if (form == 0 && cells == 16) probe_loop_kernel<0, 16, 3><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
             if (form == 1 && cells == 16) probe_loop_kernel<1, 16, 3><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 2 && cells == 8) probe_loop_kernel<2, 8, 4><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 3 && cells == 8) probe_loop_kernel<3, 8, 4><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 2 && cells == 16) probe_loop_kernel<2, 16, 3><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
+            if (form == 3 && cells == 16) probe_loop_kernel<3, 16, 3><<<grid, 128>>>(g, out, n, -1e-3f, cyc);
             cudaEventRecord(e1);
             if (cudaEventSynchronize(e1) != cudaSuccess) break;
             cudaEventElapsedTime(&ms, e0, e1);
