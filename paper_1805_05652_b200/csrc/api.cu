@@ -180,7 +180,7 @@ Plan make_plan(int window, int32_t n_atoms, int32_t n_templates, int32_t t0_min,
         pl.slide_rt = 1;
         // grouped window sums (exp_moment_kernel): a group of R neighbouring tau shares 8 moments
         // while z = (window length) x (half width of the group in 1/tau) <= 1.5 (R - 1) dtau / tau
-        // stays below kMomZCap = 0.17 (exp_scan.cu); R = 64 above that tau, R = 32 above half of
+        // stays below 0.17 (exp_scan.cu: the truncation bound); R = 64 above that tau, R = 32 above half of
         // it, R = 16 above a quarter, the per-tau recurrence below.  Regions shorter than one group are not worth a launch.
         bool moments = n_templates >= 2;
         int tile_code = opts ? opts->tile_c : 0;

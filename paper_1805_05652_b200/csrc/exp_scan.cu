@@ -366,7 +366,7 @@ __device__ __forceinline__ void exp_window_body(
 // on n:  Q_k = sum_a e_a z_a^k / k! x_a  (e^2 and (2z)^k for a2, b2, ab),
 //     S_n = sum_{k<8} (-rho_n)^k Q_k  + the few atoms of [hi_{n0}, hi_n) (added to the moments as n
 // grows).  A window is at most 3 tau long, so z <= 1.5 (R - 1) dtau / tau; the plan (api.cu)
-// takes a group size R in {32, 64} only where that is <= kMomZCap = 0.17: the truncation error of
+// takes a group size R in {16, 32, 64} only where that is <= 0.17: the truncation error of
 // a WEIGHT is then below (2 x 0.17)^8 / 8! = 4.4e-9 relative (the squared weights are the worse
 // case), a tenth of the fp32 rounding of the sums it enters (DESIGN.md 6.2 has the numbers).
 // Every weight is positive and evaluated from its own time stamp with one MUFU.EX2: nothing
@@ -383,7 +383,6 @@ __device__ __forceinline__ void exp_window_body(
 // form of exp_direct.cu): moments are plain sums, so the partial ones meet in shared memory.
 // Then every warp finishes a quarter of the group's tau values.
 // ---------------------------------------------------------------------------------------
-constexpr float kMomZCap = 0.17f;
 constexpr int kMomKW = 32;   // atoms per bulk copy and template (1 KB); divides kPackBlock
 constexpr int kMomGW = 8;    // groups per warp
 constexpr int kMomNS = 2;    // ring slots per warp
