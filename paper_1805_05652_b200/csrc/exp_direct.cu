@@ -2,37 +2,38 @@
 // ("brute-force grid", eq. (4) PAPER.md:44, 3 tau cut PAPER.md:52/238), fused with
 // the cell closure (eq. 7) and the marginalisation, batched over templates.
 //
-// B200 design (DESIGN.md "exp direct kernel"):
+// B200 design (DESIGN.md 6.1):
 //  * one thread owns C cells (m0..m0+C-1, n): same tau, C consecutive t0.  For fixed tau the
 //    weight exp(-(t - t0_c)/tau) = exp(-(t - t_ref)/tau) * const_c, and F is invariant under a
 //    per-cell rescaling of the window (A,B,C ~ k^2, Fa,Fb ~ k), so ONE weight
-//    w = exp(-(t - t_ref)/tau), t_ref = t0_{m0}, serves all C cells: 1 FMUL + 1 MUFU.EX2 per
-//    atom instead of per term.  The plan only picks C > 1 when (C-1) dt0 <= 8 tau_min, so the
-//    dropped factor const_c stays within e^-8..1 and nothing underflows.
-//  * every term is still accumulated on its own: 7 fp32 FMAs per (cell, atom) pair.  They are
-//    issued as packed fma.rn.f32x2 (SASS FFMA2, sm_100): the accumulator pairs are (A,B),
-//    (Re Fa, Im Fa), (Re Fb, Im Fb) of one cell and (C_c, C_c+1) of two cells, so the atom
-//    operands (a2,b2), (Re Fa, Im Fa), (Re Fb, Im Fb) are the natural 64-bit halves of the
-//    staged atom record.  FFMA2 has the lane throughput of FFMA at half the issue slots
-//    (measured by tfstat_probe_alu), which leaves room to issue the LDS/MUFU/loop instructions
-//    beside a saturated FMA pipe.
-//  * lanes of a warp hold consecutive tau_n, so every lane reads the SAME atom: atoms are
-//    staged per CTA in shared memory as two 16-byte records (dt, ab | a2, b2) and
-//    (Re Fa, Im Fa | Re Fb, Im Fb) and read with broadcast LDS.128; the int->float conversion
-//    of the timestamps happens once in the staging, not in the loop.
-//  * the window of a CTA is streamed through shared memory in chunks of KC atoms, so a 1-year
-//    atom set (13 140 atoms) needs no more shared memory than a 1-day one.
+//    w = exp(-(t - t_ref)/tau), t_ref = t0_{m0}, serves all C cells: its argument (1 FFMA) and
+//    two MUFU.EX2 (w and w^2) per atom instead of per term.  The plan only picks C > 1 when
+//    (C-1) dt0 <= 8 tau_min, so the dropped factor const_c stays within e^-8..1 and nothing
+//    underflows.
+//  * every term is still accumulated on its own: 7 fp32 FMAs per (cell, atom) pair, issued as
+//    packed fma.rn.f32x2 (SASS FFMA2, sm_100) on accumulator pairs of two CELLS of one channel:
+//    both multiplicands (weight, atom channel) are then broadcast scalars, the one FFMA2
+//    operand form that issues every 2 cycles (a pair x a scalar takes 2.4: tfstat_probe).
+//  * lanes of a warp hold consecutive tau_n, so every lane reads the SAME atom: the atoms come
+//    as the packed 32-byte records of pack.cu, (dtc, ab | a2, b2) and (Re Fa, Im Fa | Re Fb,
+//    Im Fb), and are read with two broadcast LDS.128.
+//  * every WARP streams the atoms of its own windows through its own ring of kStages slots of
+//    kChunkAtoms records, filled by bulk asynchronous copies (cp.async.bulk + mbarrier): no
+//    thread moves atom data, there is no CTA barrier in the loop, and a 1-year atom set needs no
+//    more shared memory than a 1-day one.
 //  * ragged window edges: the atoms [lo_{C-1}, hi_0) belong to all C cells of a thread and are
 //    summed with per-thread loop bounds and no predicates; the few head atoms [lo_0, lo_{C-1})
-//    and tail atoms [hi_0, hi_{C-1}) are read straight from global memory with 0/1 weights.
+//    and tail atoms [hi_0, hi_{C-1}) are read straight from global memory and added per cell
+//    under a predicate.
 //  * a CTA is (one t0 tile) x (NT consecutive tau); the ragged tau block is the one with the
-//    SHORTEST windows, and CTAs are launched heaviest (largest tau) first.
+//    SHORTEST windows, and CTAs are launched heaviest (largest tau) first.  SPLIT (single maps):
+//    the warps of a CTA share 32 tau values and split the atoms of their windows instead.
 #include "plan.h"
 
-// Tuning constants of the core loop, swept on B200 (config 4).  Unrolling is what matters (unroll
-// 4: 3.79e12 terms/s, 8: 3.94, 16: 4.10, 24..32: 4.12-4.17, 64: 4.11; the loop counter, the
-// shared-memory address arithmetic and the branch are per iteration, and the scheduler gets more
-// independent LDS / MUFU to hoist above the FFMA2 stream).
+// Tuning constants of the core loop, swept on B200 (config 4).  Unrolling is what matters (round
+// 1's loop: unroll 4: 3.79e12 terms/s, 8: 3.94, 16: 4.10, 24..32: 4.12-4.17, 64: 4.11; the loop
+// counter, the shared-memory address arithmetic and the branch are per iteration, and the
+// scheduler gets more independent LDS / MUFU to hoist above the FFMA2 stream).
 constexpr int kChunkAtoms = 192;  // atoms per bulk copy (6 KB); divides kPackBlock
 constexpr int kStages = 2;        // ring slots per warp
 constexpr int kCoreUnroll = 24;   // divides kChunkAtoms

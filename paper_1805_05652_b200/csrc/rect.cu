@@ -25,8 +25,15 @@
 //     (swizzled) shared memory (thread = row, but the map is tau-fastest) and leave as 64-byte
 //     row segments.
 //
+//  3'. rect_tile_kernel (further down), instead of 2. and 3. where the lattice steps are small
+//     (dt0 and dtau within a factor 4 of each other: the full-resolution grids): the direct form
+//     S(m, n) = P[hi] - P[lo_m] tile by tile, as Phi[j] + U[m] with both terms staged once per
+//     tile relative to an anchor atom -- no running sum, no dependency between cells, two cells
+//     that share a lattice point per packed instruction, plain coalesced stores.
+//
 // Grids without an edge lattice (J = 0) or with very few t0 rows use the per-cell kernel
-// rect_cells_kernel: S(m,n) = P[hi(m,n)] - P[lo(m)], closure in fp64.
+// rect_cells_kernel: S(m,n) = P[hi(m,n)] - P[lo(m)], closure in fp64.  Small problems take
+// rect_small_kernel: everything in one launch, one CTA per template.
 #include <algorithm>
 
 #include "plan.h"
