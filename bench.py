@@ -527,7 +527,8 @@ def run_ours(args):
     ach_ops = terms * exec_ops_per_term / (k_ms * 1e-3)
     alg_ops = terms * FP32_OPS_PER_TERM / (k_ms * 1e-3)
     probes = {k: pkg.probe_alu(k) for k in ("ffma", "fadd", "mufu_ex2", "ffma2", "ffma_mufu",
-                                             "lds128", "dfma")}
+                                             "lds128", "dfma", "ffma2_two_pairs",
+                                             "ffma2_scalar_pair", "ffma2_two_scalars")}
     roofline = {
         "bound": "alu", "kernel": "exp_direct_kernel",
         "achieved": ach_ops / 1e12, "peak": peak_ops / 1e12, "unit": "T FP32 lane-op/s",

@@ -22,7 +22,10 @@ extern "C" {
 #define TFSTAT_PROBE_FFMA_MUFU 5 /* 8 FFMA : 1 MUFU.EX2 mix (do the pipes overlap?)           */
 #define TFSTAT_PROBE_LDS128 6   /* broadcast LDS.128 (one address per warp)                    */
 #define TFSTAT_PROBE_DFMA 7     /* fp64 fma                                                    */
-#define TFSTAT_PROBE_KINDS 8
+#define TFSTAT_PROBE_FFMA2_PAIRS 8       /* fma.rn.f32x2 acc, X, Y: two distinct register pairs */
+#define TFSTAT_PROBE_FFMA2_SCALAR_PAIR 9 /* ... acc, (w, w), X: a broadcast scalar and a pair   */
+#define TFSTAT_PROBE_FFMA2_SCALARS 10    /* ... acc, (w, w), (x, x): two broadcast scalars      */
+#define TFSTAT_PROBE_KINDS 11
 
 /* Runs probe `kind` on the current device (synchronous; default stream; CUDA-event timed,
  * 1 warm-up + `reps` timed launches, best taken).  All outputs are HOST pointers:

@@ -529,7 +529,8 @@ def tfstat_search_host(atoms: torch.Tensor, t_atoms: torch.Tensor, window: int, 
 
 
 PROBE_KINDS = {"ffma": 0, "fadd": 1, "mufu_ex2": 2, "ffma2": 3, "fadd2": 4, "ffma_mufu": 5,
-               "lds128": 6, "dfma": 7}
+               "lds128": 6, "dfma": 7,
+               "ffma2_two_pairs": 8, "ffma2_scalar_pair": 9, "ffma2_two_scalars": 10}
 
 
 def probe_alu(kind: str, reps: int = 3) -> dict:

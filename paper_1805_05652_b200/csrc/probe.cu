@@ -38,6 +38,16 @@ __global__ void __launch_bounds__(kNT) probe_kernel(const float *__restrict__ in
                   __float_as_uint(acc[2 * j]);
     const unsigned long long ab2 =
         ((unsigned long long)__float_as_uint(b) << 32) | __float_as_uint(a);
+    // operand forms of fma.rn.f32x2 (kinds 8-10): two distinct register pairs, a broadcast scalar
+    // and a pair, two broadcast scalars (what the multiplicands of exp_direct.cu's loop are)
+    // (per-thread values, so that the operands live in the register file as in the kernel: a
+    // block-uniform operand would go to a uniform register, which every form takes at full rate)
+    const float sw = in[2] + 1e-9f * (float)threadIdx.x, sx = in[3] * (float)(threadIdx.x + 1);
+    unsigned long long ba2, ww2, xx2, ab2v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ba2) : "f"(b + sw), "f"(a + sx));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ab2v) : "f"(a + sx), "f"(b + sx));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(ww2) : "f"(sw));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(xx2) : "f"(sx));
     double dacc[kChains / 2];
 #pragma unroll
     for (int j = 0; j < kChains / 2; ++j) dacc[j] = (double)acc[j];
@@ -64,6 +74,18 @@ __global__ void __launch_bounds__(kNT) probe_kernel(const float *__restrict__ in
 #pragma unroll
             for (int j = 0; j < kChains / 2; ++j)
                 asm volatile("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(acc2[j]) : "l"(ab2));
+        } else if (KIND == TFSTAT_PROBE_FFMA2_PAIRS) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j)
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc2[j]) : "l"(ab2v), "l"(ba2));
+        } else if (KIND == TFSTAT_PROBE_FFMA2_SCALAR_PAIR) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j)
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc2[j]) : "l"(ww2), "l"(ab2v));
+        } else if (KIND == TFSTAT_PROBE_FFMA2_SCALARS) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j)
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc2[j]) : "l"(ww2), "l"(xx2));
         } else if (KIND == TFSTAT_PROBE_FADD2) {
 #pragma unroll
             for (int j = 0; j < kChains / 2; ++j)
@@ -109,6 +131,9 @@ int ops_per_iter(int kind)
     case TFSTAT_PROBE_FADD:
     case TFSTAT_PROBE_MUFU_EX2:
     case TFSTAT_PROBE_FFMA2:
+    case TFSTAT_PROBE_FFMA2_PAIRS:
+    case TFSTAT_PROBE_FFMA2_SCALAR_PAIR:
+    case TFSTAT_PROBE_FFMA2_SCALARS:
     case TFSTAT_PROBE_FADD2: return kChains;
     case TFSTAT_PROBE_FFMA_MUFU: return kChains + 2;
     case TFSTAT_PROBE_LDS128: return kChains / 4;
@@ -306,11 +331,11 @@ extern "C" int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s,
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     int rc = TFSTAT_ECUDA;
     do {
-        if (cudaMalloc(&in, 2 * sizeof(float)) != cudaSuccess) break;
+        if (cudaMalloc(&in, 4 * sizeof(float)) != cudaSuccess) break;
         if (cudaMalloc(&out, sizeof(float) * (size_t)grid * kNT) != cudaSuccess) break;
         if (cudaMalloc(&cyc, 2 * sizeof(long long)) != cudaSuccess) break;
-        const float h_in[2] = {kind == TFSTAT_PROBE_MUFU_EX2 ? -0.5f : 1.0000001f,
-                               kind == TFSTAT_PROBE_LDS128 ? 0.0f : 1e-9f};
+        const float h_in[4] = {kind == TFSTAT_PROBE_MUFU_EX2 ? -0.5f : 1.0000001f,
+                               kind == TFSTAT_PROBE_LDS128 ? 0.0f : 1e-9f, 0.9999999f, 1e-9f};
         if (cudaMemcpy(in, h_in, sizeof(h_in), cudaMemcpyHostToDevice) != cudaSuccess) break;
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
         float best_ms = 1e30f;
@@ -327,6 +352,9 @@ extern "C" int tfstat_probe_alu(int kind, int reps, double *lane_ops_per_s,
             case 5: launch<5>(grid, in, out, cyc); break;
             case 6: launch<6>(grid, in, out, cyc); break;
             case 7: launch<7>(grid, in, out, cyc); break;
+            case 8: launch<8>(grid, in, out, cyc); break;
+            case 9: launch<9>(grid, in, out, cyc); break;
+            case 10: launch<10>(grid, in, out, cyc); break;
             }
             cudaEventRecord(e1);
             if (cudaEventSynchronize(e1) != cudaSuccess) break;
