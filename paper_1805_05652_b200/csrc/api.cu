@@ -716,9 +716,10 @@ int tfstat_search_host(const float *atoms_host, int64_t template_stride, int64_t
         chk(cudaMemcpyAsync(out_host, d_out, sizeof(tfstat_result) * (size_t)n_templates,
                             cudaMemcpyDeviceToHost, s_comp));
     } while (0);
-    if (s_copy) cudaStreamSynchronize(s_copy);
-    if (s_comp) cudaStreamSynchronize(s_comp);
-    if (s_back) cudaStreamSynchronize(s_back);
+    // (a fault of a kernel or a copy surfaces here: it is this call's error, not a later one's)
+    if (s_copy) chk(cudaStreamSynchronize(s_copy));
+    if (s_comp) chk(cudaStreamSynchronize(s_comp));
+    if (s_back) chk(cudaStreamSynchronize(s_back));
     for (int b = 0; b < 2; ++b) {
         if (ev_in[b]) cudaEventDestroy(ev_in[b]);
         if (ev_done[b]) cudaEventDestroy(ev_done[b]);

@@ -47,7 +47,6 @@ __global__ void __launch_bounds__(kBoundsNT)
                   int stride, int n_samples, int32_t *__restrict__ lo,
                   int32_t *__restrict__ edge, int32_t *__restrict__ zero, int64_t n_zero)
 {
-    pdl_trigger();
     // scan flags of the rectangular path (rect.cu), zeroed here to save a memset node
     for (int64_t z = (int64_t)blockIdx.x * kBoundsNT + threadIdx.x; z < n_zero;
          z += (int64_t)gridDim.x * kBoundsNT)
@@ -110,7 +109,6 @@ cudaError_t launch_validate_timestamps(const int32_t *t_atoms, int32_t n_atoms,
 
 __global__ void count_terms_kernel(Grid g, Bounds b, unsigned long long *out)
 {
-    pdl_wait();
     const int64_t n_cells = (int64_t)g.N_t0 * g.N_tau;
     unsigned long long acc = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_cells;

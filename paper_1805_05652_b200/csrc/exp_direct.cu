@@ -134,7 +134,6 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
     extern __shared__ __align__(128) unsigned char smem_raw[];  // rings: [NW][NS][2 KW] x 16 B
     __shared__ __align__(8) unsigned long long s_bar[NW][NS];
     __shared__ Marg s_red[32];
-    pdl_trigger();
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -168,7 +167,6 @@ __global__ void __launch_bounds__(NT, (C > 8 ? 384 : 512) / NT)
         mbar_fence_init();
     }
     __syncwarp();
-    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
 
     // per-thread ranges: head [h0, cb) and tail [ce, h1) take 0/1 weights per cell, the core
     // [cb, ce) belongs to all C cells
@@ -351,7 +349,7 @@ cudaError_t launch_one(const Plan &pl, const Problem &pr, const void *packed, Pa
         cudaError_t e =
             cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        return launch_pdl(kern, (unsigned)n_ctas, NT, smem, st, pr,
+        return launch_k(kern, (unsigned)n_ctas, NT, smem, st, pr,
                           static_cast<const ulonglong2 *>(packed), pl.n_pad, partials, pl.n_mtiles,
                           pl.n_nblocks);
     };

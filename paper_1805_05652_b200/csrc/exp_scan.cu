@@ -408,7 +408,6 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
     // a warp's ring slot: [pair][template of the pair][records]
     __shared__ __align__(128) ulonglong2 s_ring[kMomNW][NS][2][TPC][2 * KW];
     __shared__ __align__(8) unsigned long long s_bar[kMomNW][NS];
-    pdl_trigger();
 
     const Grid &g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -441,7 +440,6 @@ __global__ void __launch_bounds__(32 * kMomNW, 4)
         mbar_fence_init();
     }
     __syncwarp();
-    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
 
     const ulonglong2 *__restrict__ rec[TPC];
 #pragma unroll
@@ -1193,8 +1191,6 @@ __global__ void __launch_bounds__(NT, RT * TPC >= 8 ? 4 : 5)
                       float4 *__restrict__ W0, const int n_nblocks, const int n_segs,
                       const int seg_len, const int n_limit, unsigned long long *__restrict__ stats)
 {
-    pdl_trigger();
-    pdl_wait();  // bounds_kernel's lo / edge tables, pack_atoms_kernel's records
     exp_window_body<NT, RT, TPC, STATS>(pr, packed, n_pad, W0, blockIdx.x, n_nblocks, n_segs, seg_len,
                                         n_limit, stats);
 }
@@ -1207,8 +1203,6 @@ __global__ void __launch_bounds__(NT, NT == 128 ? (TPC == 1 ? 5 : TPC == 2 ? 4 :
                      const int n_nblocks, const int n_segs, const int seg_len,
                      unsigned long long *__restrict__ stats)
 {
-    pdl_trigger();
-    pdl_wait();  // exp_window_kernel's sums (and, before it, the bounds tables and the records)
     exp_slide_body<NT, TPC, STATS>(pr, packed, n_pad, W0, partials, blockIdx.x, n_nblocks, n_segs,
                                    seg_len, stats);
 }
@@ -1226,9 +1220,9 @@ cudaError_t launch_tpc(const Plan &pl, const Problem &pr, const ulonglong2 *pack
     const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
     const int64_t n_ctas = (int64_t)pl.n_nblocks * pl.n_segs * groups;
     if (pl.stats)
-        return launch_pdl(exp_slide_kernel<NT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr, packed,
+        return launch_k(exp_slide_kernel<NT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr, packed,
                           pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
-    return launch_pdl(exp_slide_kernel<NT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr, packed,
+    return launch_k(exp_slide_kernel<NT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr, packed,
                       pl.n_pad, W0, partials, pl.n_nblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 
@@ -1252,9 +1246,9 @@ cudaError_t launch_win(const Plan &pl, const Problem &pr, const ulonglong2 *pack
     const int64_t groups = (pl.n_templates + TPC - 1) / TPC;
     const int64_t n_ctas = (int64_t)nblk * pl.n_segs * groups;
     if (pl.stats)
-        return launch_pdl(exp_window_kernel<NT, RT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr,
+        return launch_k(exp_window_kernel<NT, RT, TPC, true>, (unsigned)n_ctas, NT, 0, st, pr,
                           packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, n_limit, pl.stats);
-    return launch_pdl(exp_window_kernel<NT, RT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr,
+    return launch_k(exp_window_kernel<NT, RT, TPC, false>, (unsigned)n_ctas, NT, 0, st, pr,
                       packed, pl.n_pad, W0, nblk, pl.n_segs, pl.seg_len, n_limit, pl.stats);
 }
 
@@ -1269,10 +1263,10 @@ cudaError_t launch_mom(const Plan &pl, const Problem &pr, const ulonglong2 *pack
     const int64_t quads = (pl.n_templates + 3) / 4;
     const int64_t n_ctas = (int64_t)n_gblocks * pl.n_segs * quads;
     if (pl.stats)
-        return launch_pdl(exp_moment_kernel<true>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
+        return launch_k(exp_moment_kernel<true>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
                           pl.n_pad, W0, pl.mom_n16, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len,
                           pl.stats);
-    return launch_pdl(exp_moment_kernel<false>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
+    return launch_k(exp_moment_kernel<false>, (unsigned)n_ctas, 32 * kMomNW, 0, st, pr, packed,
                       pl.n_pad, W0, pl.mom_n16, pl.mom_n32, pl.mom_n64, n_gblocks, pl.n_segs, pl.seg_len, pl.stats);
 }
 

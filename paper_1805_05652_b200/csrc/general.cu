@@ -93,7 +93,6 @@ __global__ void __launch_bounds__(kGenNT)
     __shared__ Marg s_red[32];
     __shared__ int s_hi[kGenNT / 32];
     __shared__ float s_tab[KIND == TFSTAT_WINDOW_TABLE ? kGenTableSmem : 1];
-    pdl_trigger();
 
     const int m = blockIdx.x / n_nblocks;
     // a thread's CT cells are CONSECUTIVE entries of the tau array: on a sorted array their

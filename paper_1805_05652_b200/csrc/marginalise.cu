@@ -196,8 +196,6 @@ __global__ void __launch_bounds__(256)
     finalize_kernel(const Partial *__restrict__ partials, const int64_t per_template,
                     const int32_t N_tau, tfstat_result *__restrict__ out)
 {
-    pdl_trigger();
-    pdl_wait();  // the partial marginals of the map kernel
     finalize_body(partials + (int64_t)blockIdx.x * per_template, per_template, N_tau,
                   out + blockIdx.x);
 }
@@ -205,13 +203,12 @@ __global__ void __launch_bounds__(256)
 // tfstat_marginalise: stream the map into one partial per CTA; finalize_kernel follows.  (One
 // launch instead of two was measured and is no faster on B200: a cooperative launch with a grid
 // barrier costs 8.6 us per call on a 2 MB map, a memset node for a last-CTA ticket 10.4 us, the
-// two kernels chained by programmatic dependent launch 8.8 us.)
+// two kernels chained by programmatic dependent launch 8.8 us: withdrawn since, tfstat_dev.cuh.)
 __global__ void __launch_bounds__(kMargNT)
     marginalise_kernel(const float *__restrict__ map, const uint8_t *__restrict__ flags,
                        const int64_t n_cells, Partial *__restrict__ partials)
 {
     __shared__ Marg s_red[32];
-    pdl_trigger();
     Marg mg;
     if (flags) marginalise_body<true>(map, flags, n_cells, mg);
     else marginalise_body<false>(map, flags, n_cells, mg);
@@ -234,7 +231,7 @@ cudaError_t launch_finalize(const Partial *partials, int64_t partials_per_templa
                             int32_t n_templates, int32_t N_tau, tfstat_result *out,
                             cudaStream_t st)
 {
-    return launch_pdl(finalize_kernel, (unsigned)n_templates, 256, 0, st, partials,
+    return launch_k(finalize_kernel, (unsigned)n_templates, 256, 0, st, partials,
                       partials_per_template, N_tau, out);
 }
 

@@ -26,7 +26,6 @@ __global__ void __launch_bounds__(kPackNT)
                       const int64_t ld, const int32_t *__restrict__ t, const int n_atoms,
                       const int n_pad, ulonglong2 *__restrict__ rec)
 {
-    pdl_trigger();
     const int i = blockIdx.x * kPackNT + threadIdx.x;
     const int tpl = blockIdx.y;
     if (i < n_pad) {
@@ -72,9 +71,6 @@ __global__ void __launch_bounds__(kPackNT)
         dst[0] = ra;
         dst[1] = rb;
     }
-    // nothing here depends on the kernel in front (bounds), but the kernel BEHIND this one
-    // relies on "my predecessor is complete => everything before it is too"
-    pdl_wait();
 }
 
 }  // namespace
@@ -82,19 +78,10 @@ __global__ void __launch_bounds__(kPackNT)
 cudaError_t launch_pack(const Plan &pl, const Problem &pr, void *packed, cudaStream_t st)
 {
     const dim3 grid((unsigned)((pl.n_pad + kPackNT - 1) / kPackNT), (unsigned)pl.n_templates, 1);
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid;
-    cfg.blockDim = dim3(kPackNT, 1, 1);
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    // (early launch only for small grids: see launch_pdl)
-    cfg.numAttrs = (uint64_t)grid.x * grid.y * kPackNT <= kPdlMaxThreads ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, pack_atoms_kernel, pr.atoms, pr.template_stride, pr.ld,
-                              pr.bounds.t, pl.n_atoms, pl.n_pad,
-                              static_cast<ulonglong2 *>(packed));
+    pack_atoms_kernel<<<grid, kPackNT, 0, st>>>(pr.atoms, pr.template_stride, pr.ld, pr.bounds.t,
+                                                pl.n_atoms, pl.n_pad,
+                                                static_cast<ulonglong2 *>(packed));
+    return cudaGetLastError();
 }
 
 }  // namespace tfstat

@@ -113,8 +113,6 @@ __global__ void __launch_bounds__(kScanNT)
 {
     __shared__ double s_off[8];
     __shared__ double s_w[8][kScanNT / 32];
-    pdl_trigger();
-    pdl_wait();  // bounds_kernel: edge table and the zeroed scan flags
     const Bounds &bd = pr.bounds;
     const int N = bd.n_atoms;
     int32_t *ready = flags, *done = flags + n_scan;
@@ -318,8 +316,6 @@ __global__ void __launch_bounds__(kCellNT)
                       Partial *__restrict__ partials, const int blocks_per_template)
 {
     __shared__ Marg s_red[32];
-    pdl_trigger();
-    pdl_wait();  // rect_scan_kernel's prefix sums
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
     const int tpl = blockIdx.x / blocks_per_template;
@@ -572,8 +568,6 @@ __global__ void __launch_bounds__(kRunNT, 8)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Marg s_red[32];
-    pdl_trigger();
-    pdl_wait();  // rect_scan_kernel's prefix sums and K table
     constexpr int nrows = Q * kRunNT;
     float *tile = reinterpret_cast<float *>(smem_raw);                     // [nrows][kPitch]
     int *s_rowm = reinterpret_cast<int *>(tile + (size_t)nrows * kPitch);  // [nrows]
@@ -1086,8 +1080,6 @@ __global__ void __launch_bounds__(kTileNT, 6)
     __shared__ int s_row0[kTileQuads];                    // first row of quad q
     __shared__ unsigned s_mag;                            // largest staged magnitude (float bits)
     __shared__ Marg s_red[32];
-    pdl_trigger();
-    pdl_wait();  // rect_scan_kernel's prefix sums (and the bounds tables before it)
 
     const Grid g = pr.grid;
     const Bounds &bd = pr.bounds;
@@ -1401,7 +1393,7 @@ cudaError_t launch_tile(const Plan &pl, const Problem &pr, const double *prefix,
     const RectRun &rr = pl.rect;
     const int64_t n_ctas = (int64_t)rr.n_rowtiles * rr.n_coltiles * pl.n_templates;
     auto go = [&](auto kern) {
-        return launch_pdl(kern, (unsigned)n_ctas, kTileNT, 0, st, pr, prefix, partials, rr.r, rr.NTu,
+        return launch_k(kern, (unsigned)n_ctas, kTileNT, 0, st, pr, prefix, partials, rr.r, rr.NTu,
                           rr.n_rowtiles, rr.n_coltiles);
     };
     const bool e1 = pl.e_n == 1;
@@ -1438,7 +1430,7 @@ cudaError_t launch_run(const Plan &pl, const Problem &pr, const double *prefix,
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)smem_all);
         if (e != cudaSuccess) return e;
-        return launch_pdl(kern, (unsigned)n_ctas, kRunNT, smem_all, st, pr, prefix, K, partials,
+        return launch_k(kern, (unsigned)n_ctas, kRunNT, smem_all, st, pr, prefix, K, partials,
                           rr.r, rr.NTu, rr.seg_cols, rr.n_rowtiles, rr.n_coltiles, vec ? 1 : 0,
                           ks_cap, rr.ks_lg);
     };
@@ -1595,12 +1587,12 @@ cudaError_t launch_rect(const Plan &pl, const Problem &pr, double *prefix, doubl
     // (the tile kernel works from P alone: no step table)
     const int spt = pl.rect.enabled && !pl.rect.tile ? (int)((pl.J + 1 + kStepPts - 1) / kStepPts) : 0;
     const int64_t n_blocks = (int64_t)n_scan + (int64_t)spt * pl.n_templates;
-    cudaError_t e = launch_pdl(rect_scan_kernel, (unsigned)n_blocks, kScanNT, 0, st, pr, agg, flags,
+    cudaError_t e = launch_k(rect_scan_kernel, (unsigned)n_blocks, kScanNT, 0, st, pr, agg, flags,
                                prefix, K, nblk, n_scan, spt);
     if (e != cudaSuccess) return e;
     if (!pl.rect.enabled) {
         const int64_t n_ctas = (int64_t)pl.cell_blocks_per_template * pl.n_templates;
-        return launch_pdl(rect_cells_kernel, (unsigned)n_ctas, kCellNT, 0, st, pr, prefix, partials,
+        return launch_k(rect_cells_kernel, (unsigned)n_ctas, kCellNT, 0, st, pr, prefix, partials,
                           pl.cell_blocks_per_template);
     }
     if (pl.rect.tile) return launch_tile(pl, pr, prefix, partials, st);

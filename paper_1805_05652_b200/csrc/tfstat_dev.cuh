@@ -312,36 +312,28 @@ __device__ __forceinline__ void partial_store(Partial *p, const Marg &a)
 }
 
 // ---------------------------------------------------------------------------------------
-// Programmatic dependent launch (sm_90+): the kernels of one call form a chain on the stream
-// (bounds -> sums -> finalize).  A kernel launched with launch_pdl() may be scheduled while its
-// predecessor is still running; it must call pdl_wait() before touching anything the
-// predecessor writes (the wait returns once the predecessor grid has completed and its writes
-// are visible), and every kernel calls pdl_trigger() at its start so that its own successor
-// can be set up early.  Only the launch latency is overlapped: ~2-3 us per kernel boundary,
-// which is what a small call is made of.
+// Kernel launches.  The kernels of one call form a chain on the caller's stream (bounds -> pack
+// -> sums -> finalize) in plain stream order.
+//
+// Programmatic dependent launch (griddepcontrol: a kernel is set up while its predecessor
+// drains and waits before it reads what the predecessor wrote) was in here for two rounds and
+// has been WITHDRAWN.  It bought 1-5 us per call on launch-bound calls, cost 15 % where the
+// early-launched grid was big (its CTAs hold their registers while they wait), and it was
+// behind a rare illegal-address fault, seen mostly where the library runs on non-blocking
+// streams (3 of 20 runs of the GPU suite; 0 of 24 + 24 without it): every kernel here reads
+// its predecessor's output through the read-only path (ld.global.nc, which `const __restrict__`
+// lets the compiler pick), and that path's contract -- the memory is not written while the
+// kernel lives -- does not hold for a kernel that is resident before its predecessor is done.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
-
-constexpr uint64_t kPdlMaxThreads = 148 * 2048;  // the threads one B200 holds at a time
 template <typename... KArgs, typename... Args>
-inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem,
-                              cudaStream_t st, Args... args)
+inline cudaError_t launch_k(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem,
+                            cudaStream_t st, Args... args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid, 1, 1);
     cfg.blockDim = dim3(block, 1, 1);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    // ... and only for grids that do not fill the GPU by themselves: the CTAs of an early
-    // launched kernel sit on their registers and shared memory while they wait, and a big grid
-    // takes them away from its predecessor (measured on B200, config 4 through the sliding form:
-    // 4.42 ms with the attribute on the grouped-sums and slide kernels, 3.71 ms without)
-    cfg.numAttrs = (uint64_t)grid * block <= kPdlMaxThreads ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
